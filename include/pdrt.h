@@ -1,0 +1,204 @@
+/*
+ * pdrt.h — C ABI of the B200-native PyDoseRT dose hot path (libpdrt.so).
+ *
+ * The library computes, entirely in hand-written CUDA kernels for sm_100a, the forward and
+ * backward dose computation of arxiv 2512.18863 ("A physics-informed, plug-and-play dose engine
+ * for gradient-based radiotherapy treatment planning", /root/reference/PAPER.md) from delivery
+ * parameters:
+ *
+ *   S1  aperture -> fluence map          PAPER.md:103-119, Eq. 4 (+ transmission, penumbra,
+ *                                        head scatter, off-axis)
+ *   S2  radiological depth               PAPER.md:135-143, Eq. 7 (central-axis ray per gantry angle)
+ *   S4  depth-dependent lateral kernels
+ *   S3  divergent projection             PAPER.md:123-133, Eq. 5-6
+ *   S5  per-slice 2-D convolution        PAPER.md:151-158, Eq. 8
+ *   S6  beam -> patient resampling and MU-weighted accumulation   PAPER.md:160-168, Eq. 9
+ *   S7-S10  the exact transposes of S6, S5, S3, S1 that map dL/dDose to dL/d(leaf, jaw, MU)
+ *           (PAPER.md:33-35, :67; depth and kernels carry no gradient, :143, :149)
+ *
+ * Where the paper is silent the readings G1-G22 of DESIGN.md §3 apply (geometry conventions,
+ * kernel form, sampling rules).  Units: millimetres and degrees.  All arithmetic on the dose path
+ * is float32 (float64 only in the ray marcher's positions and prefix sum).
+ *
+ * Conventions
+ *   Patient grid: nx*ny*nz voxels, memory [z][y][x] (x fastest), centre of voxel (i,j,k) at
+ *     (ox + i*sx, oy + j*sy, oz + k*sz).
+ *   Gantry angle phi: u^ = (cos phi, sin phi, 0), w^ = (-sin phi, cos phi, 0), v^ = (0,0,1);
+ *     the source sits at iso - SID*w^ (phi = 0: beam travels +y; phi = 90: source on the +x side).
+ *   Beam grid: Nu x Nv x Nw with Nv = nz, dv = sz (beam v-slices are patient z-slices),
+ *     u_i = (i - (Nu-1)/2) du,  w_k = beam_wmin + k dw,  v_j = oz + j sz - iso_z.
+ *   Fluence map: flu_nu x flu_nv pixels, memory [v][u], pixel centres
+ *     uf_a = (a - (flu_nu-1)/2) flu_du,  vf_b = (b - (flu_nv-1)/2) flu_dv  at the isocentre plane.
+ *   Leaves: [n_cp][2][n_pairs], bank 0 = left edge l_i, bank 1 = right edge r_i (along u, mm at
+ *     the isocentre plane); leaf pair i shadows v in [leaf_bounds_mm[i], leaf_bounds_mm[i+1]].
+ *   Jaws: [n_cp][4] = x1, x2 (along u), y1, y2 (along v).
+ *
+ * Ownership and execution
+ *   The caller owns every buffer it passes.  pdrt_create copies the density volume and all tables
+ *   (they may be freed on return).  Pointers named *_dev are device pointers on the engine's
+ *   device; pointers named *_host are host pointers (pinned memory makes the copies asynchronous).
+ *   Outputs are caller-allocated and fully overwritten.  Scratch memory is engine-owned, grown
+ *   lazily to the largest n_cp seen.  pdrt_dose / pdrt_dose_backward enqueue work on `cuda_stream`
+ *   (a cudaStream_t, may be NULL for the default stream) and return without synchronising;
+ *   the *_host variants copy in, run, copy out and synchronise the stream before returning.
+ *   An engine must not be used from two threads at once.
+ *
+ * Errors
+ *   Every function returning int returns PDRT_OK (0) or a negative code; pdrt_last_error gives
+ *   the message of the last failure on that engine (or of the last failed pdrt_create when the
+ *   engine argument is NULL).  Nothing aborts or throws across this boundary.  Device-resident
+ *   parameters are not validated: l_i > r_i is a closed pair by Eq. 4's max(0, .), NaN in gives
+ *   NaN out.  There is no CPU fallback: without a CUDA device pdrt_create fails with PDRT_ECUDA.
+ */
+#ifndef PDRT_H
+#define PDRT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define PDRT_API __attribute__((visibility("default")))
+#else
+#define PDRT_API
+#endif
+
+#define PDRT_OK       0
+#define PDRT_EINVAL  (-1)   /* null pointer, non-positive size, even/out-of-range kernel size, bad table */
+#define PDRT_ENOMEM  (-2)   /* host or device allocation failed                                        */
+#define PDRT_ECUDA   (-3)   /* CUDA runtime error (message from cudaGetErrorString)                    */
+
+typedef struct pdrt_engine pdrt_engine;   /* opaque */
+
+/* Patient dose / density grid (CT volume as relative electron density). */
+typedef struct {
+    int32_t nx, ny, nz;      /* voxels                                   */
+    float   sx, sy, sz;      /* spacing [mm]                             */
+    float   ox, oy, oz;      /* centre of voxel (0,0,0) [mm]             */
+    float   iso[3];          /* isocentre [mm], patient frame            */
+} pdrt_grid;
+
+/* "Beam-model tables": the machine-specific coefficients of PAPER.md:119, :176.  All pointers are
+ * HOST pointers, read during pdrt_create only. */
+typedef struct {
+    float   sid_mm;                      /* source-isocentre distance (1000)                              */
+    int32_t n_pairs;                     /* MLC leaf pairs                                                */
+    const float *leaf_bounds_mm;         /* n_pairs+1 leaf boundaries along v, strictly ascending         */
+    int32_t flu_nu, flu_nv;              /* fluence map pixels                                            */
+    float   flu_du, flu_dv;              /* fluence pixel size [mm]                                       */
+    float   tau;                         /* MLC transmission (~0.002)                       */
+    float   fwhm_mlc_mm, fwhm_jaw_mm;    /* source penumbra FWHM along u / along v; 0 = off */
+    int32_t n_hs;                        /* head-scatter Gaussians; 0 = off                */
+    const float *hs_amp, *hs_sigma_mm;   /* n_hs amplitudes and sigmas                                    */
+    int32_t n_oar; float oar_dr_mm;      /* radial off-axis table; n_oar = 0 = off         */
+    const float *oar;                    /* n_oar factors at r = n * oar_dr_mm, clamped at the last entry */
+    int32_t n_z; float dz_mm;            /* kernel parameters tabulated at radiological depth z = n * dz  */
+    const float *kA, *ka, *kB, *kb;      /* n_z each: K(r;z) = (A e^{-a r} + B e^{-b r}) / r */
+    int32_t kernel_size;                 /* lateral kernel size in beam-grid pixels: odd, 3..63           */
+    float   cal;                         /* global dose scale (PAPER.md:178 energy scaling factor)        */
+    int32_t beam_nu, beam_nw;            /* beam grid; beam_nu == 0 selects the default grid as a whole:  */
+    float   beam_du, beam_dw, beam_wmin; /*   Nu = nx, Nw = ny, du = dw = sx, wmin = -(Nw-1)/2 * dw       */
+    float   ray_step_mm;                 /* ray-march step; 0 => 0.5 * min(sx, sy, sz)                    */
+} pdrt_beam_model;
+
+/* Resolved sizes of an engine (after defaults). */
+typedef struct {
+    int32_t nx, ny, nz;
+    int32_t beam_nu, beam_nv, beam_nw;
+    float   beam_du, beam_dv, beam_dw, beam_wmin;
+    int32_t flu_nu, flu_nv, n_pairs;
+    int32_t kernel_size;                 /* as requested                                      */
+    int32_t kernel_size_compiled;        /* smallest compiled conv variant >= kernel_size     */
+    float   ray_step_mm;
+    int32_t ray_samples;                 /* samples per central-axis ray                      */
+    int32_t sm_count;
+    uint64_t scratch_bytes;              /* device scratch currently held                     */
+} pdrt_info;
+
+/* Work counters of the most recent pdrt_dose / pdrt_dose_backward (device-counted from the actual
+ * fluence support of that call).  Reading them synchronises the call's stream. */
+typedef struct {
+    int32_t  n_cp;
+    int64_t  conv_items;        /* (control point, slice, chunk) work items of the conv kernel    */
+    int64_t  support_voxels;    /* sum over CPs and slices of |S_k| (possibly non-zero Phi_vol)   */
+    int64_t  footprint_voxels;  /* sum over CPs and slices of |F_k| = |S_k (+) k x k|             */
+    int64_t  region_voxels;     /* voxels of the compact per-CP beam-frame regions (materialised) */
+    int64_t  conv_macs;         /* multiply-adds the conv kernel issues (k_compiled^2 per output) */
+    int32_t  kernel_size, kernel_size_compiled;
+} pdrt_work;
+
+/* pdrt_create: grid geometry, density volume [nz][ny][nx] (host OR device pointer; copied) and
+ * beam-model tables.  Builds the pencil-kernel table W_tab[n_z][k][k] on the host in float64 by
+ * 8x8 midpoint sub-sampling of K over each pixel (G4) and uploads it as float32.
+ * Uses the current CUDA device. */
+PDRT_API int pdrt_create(const pdrt_grid *grid, const float *density, const pdrt_beam_model *model,
+                pdrt_engine **out);
+PDRT_API void pdrt_destroy(pdrt_engine *engine);
+
+/* Message of the last failure; valid until the next call on that engine. */
+PDRT_API const char *pdrt_last_error(const pdrt_engine *engine);
+
+/* Rebuilds W_tab for another lateral kernel size (odd, 3..63); used by the kernel-size sweep
+ * (Table 4).  Synchronises the device. */
+PDRT_API int pdrt_set_kernel_size(pdrt_engine *engine, int32_t kernel_size);
+
+PDRT_API int pdrt_get_info(const pdrt_engine *engine, pdrt_info *info);
+PDRT_API int pdrt_get_work(pdrt_engine *engine, pdrt_work *work);
+
+/* Forward (S1-S6, Eq. 4-9):  dose = cal * sum_b MU_b * R_b[ (P Phi_b) (*) K(z_rad) ].
+ *   leaves_dev [n_cp][2][n_pairs], jaws_dev [n_cp][4], gantry_deg_dev [n_cp], mu_dev [n_cp],
+ *   dose_dev [nz][ny][nx] overwritten.  n_cp >= 1. */
+PDRT_API int pdrt_dose(pdrt_engine *engine, int32_t n_cp,
+              const float *leaves_dev, const float *jaws_dev,
+              const float *gantry_deg_dev, const float *mu_dev,
+              float *dose_dev, void *cuda_stream);
+
+/* Backward (S7-S10): from dL_ddose_dev [nz][ny][nx] to d_leaves_dev [n_cp][2][n_pairs],
+ * d_jaws_dev [n_cp][4], d_mu_dev [n_cp], all overwritten.  Stateless: takes the parameters again
+ * and recomputes the fluence maps and depths.  Subgradient convention at the kinks of Eq. 4:
+ * DESIGN.md G9.  No gradient w.r.t. gantry angle, density or tables. */
+PDRT_API int pdrt_dose_backward(pdrt_engine *engine, int32_t n_cp,
+                       const float *leaves_dev, const float *jaws_dev,
+                       const float *gantry_deg_dev, const float *mu_dev,
+                       const float *dL_ddose_dev,
+                       float *d_leaves_dev, float *d_jaws_dev, float *d_mu_dev,
+                       void *cuda_stream);
+
+/* The same two calls with HOST buffers: host->device copies of the parameters (and dL/dDose),
+ * the kernels, the device->host copy of the result, and a stream synchronise. */
+PDRT_API int pdrt_dose_host(pdrt_engine *engine, int32_t n_cp,
+                   const float *leaves_host, const float *jaws_host,
+                   const float *gantry_deg_host, const float *mu_host,
+                   float *dose_host, void *cuda_stream);
+PDRT_API int pdrt_dose_backward_host(pdrt_engine *engine, int32_t n_cp,
+                            const float *leaves_host, const float *jaws_host,
+                            const float *gantry_deg_host, const float *mu_host,
+                            const float *dL_ddose_host,
+                            float *d_leaves_host, float *d_jaws_host, float *d_mu_host,
+                            void *cuda_stream);
+
+/* Stage taps for parity tests (device pointers, outputs overwritten; they run the same kernels
+ * as pdrt_dose / pdrt_dose_backward and copy an intermediate out):
+ *   pdrt_stage_fluence   S1: fluence maps            phimap_dev [n_cp][flu_nv][flu_nu]
+ *   pdrt_stage_depth     S2: radiological depths     zrad_dev   [n_cp][beam_nw]
+ *   pdrt_stage_beam_dose S3-S5: beam-frame dose D_b of ONE control point, dense
+ *                                                    db_dev     [beam_nw][beam_nv][beam_nu]
+ *   pdrt_stage_grad_fluence S7-S9: dL/dPhimap per control point (zero outside the fluence
+ *                        support of that control point) gphimap_dev [n_cp][flu_nv][flu_nu]      */
+PDRT_API int pdrt_stage_fluence(pdrt_engine *engine, int32_t n_cp, const float *leaves_dev, const float *jaws_dev,
+                       float *phimap_dev, void *cuda_stream);
+PDRT_API int pdrt_stage_depth(pdrt_engine *engine, int32_t n_cp, const float *gantry_deg_dev,
+                     float *zrad_dev, void *cuda_stream);
+PDRT_API int pdrt_stage_beam_dose(pdrt_engine *engine, const float *leaves_dev, const float *jaws_dev,
+                         const float *gantry_deg_dev, float *db_dev, void *cuda_stream);
+PDRT_API int pdrt_stage_grad_fluence(pdrt_engine *engine, int32_t n_cp, const float *leaves_dev, const float *jaws_dev,
+                            const float *gantry_deg_dev, const float *dL_ddose_dev,
+                            float *gphimap_dev, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PDRT_H */

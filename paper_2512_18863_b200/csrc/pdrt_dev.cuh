@@ -1,0 +1,144 @@
+// pdrt_dev.cuh — device-side parameter blocks and geometry helpers shared by all kernels.
+//
+// Data layout in HBM:
+//   density, dose, dL/dDose : patient grid [nz][ny][nx] float32
+//   phimap, gphimap, P0, ... : [n_cp][Nvf][Nuf] float32, valid only inside the fluence support
+//                              bbox of each control point (CpDesc a0..a1, b0..b1)
+//   zrad                    : [n_cp][Nw] float32
+//   D_b / G_b / H_b         : per control point a COMPACT beam-frame block, layout [v][w][u]:
+//        index(cp; i,j,k) = cp_slot*stride_cp + ((j - rj0)*Nw + k)*pu + (i - ri0)
+//     covering the region [ri0, ri0+pu) x [rj0, rj0+pv) x [0, Nw) that bounds the conv footprint
+//     of that control point (jaw opening magnified per slice, dilated by blur and kernel halo).
+//     v outermost makes the (u,w) plane of one patient z-slice contiguous for the resampler.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pdrt {
+
+constexpr int RU = 8;              // conv outputs per thread along u
+constexpr int RV = 4;              // conv outputs per thread along v
+constexpr int CONV_THREADS = 128;  // threads per conv block
+constexpr int NTXC_MAX = 8;        // conv chunk width in thread-tiles (64 outputs)
+constexpr int MAX_TAPS = 64;       // largest Gaussian half-width [pixels]
+constexpr int MAX_HS = 4;          // largest number of head-scatter Gaussians
+
+struct Params {
+    // patient grid
+    int nx, ny, nz;
+    float sx, sy, sz, ox, oy, oz, isox, isoy, isoz;
+    // beam grid (Nv = nz, dv = sz)
+    int Nu, Nv, Nw;
+    float du, dv, dw, wmin, cu, v0;      // cu = (Nu-1)/2, v0 = oz - iso_z  (v_j = v0 + j dv)
+    // fluence map
+    int Nuf, Nvf;
+    float Du, Dv, cuf, cvf;              // cuf = (Nuf-1)/2
+    float sid, tau, cal;
+    int Np;                              // leaf pairs
+    // lateral kernel
+    int K, KT;                           // requested size, compiled variant (KT >= K)
+    int n_z;
+    float dz;
+    int tile_floats;                     // conv input-tile budget in shared memory [floats]
+    // fluence corrections
+    int Tu_max, Tv_max;                  // largest Gaussian half-widths along u / v
+    // ray marcher
+    int M_ray;
+    double ray_step;
+    // compact beam-frame blocks
+    long long stride_cp;                 // floats per control point
+};
+
+// Gaussian taps and tables of the fluence corrections (device pointers into one float pool).
+struct FluTables {
+    const float *leaf_bounds;            // [Np+1]
+    const float *oar;                    // [n_oar]
+    int n_oar;
+    float oar_dr;
+    int Tu, Tv;                          // penumbra half-widths: MLC (along u), jaw (along v)
+    const float *gu, *gv;                // [2Tu+1], [2Tv+1]
+    int n_hs;
+    float hs_amp[MAX_HS];
+    int hs_Tu[MAX_HS], hs_Tv[MAX_HS];
+    const float *hs_gu[MAX_HS], *hs_gv[MAX_HS];
+};
+
+// Per-control-point descriptor, built on the device by k_fluence (no host sync on the path).
+struct CpDesc {
+    float cg, sg;                // cos / sin of the gantry angle
+    float scale;                 // cal * MU
+    int a0, a1, b0, b1;          // fluence support bbox (inclusive); empty when a0 > a1
+    int ja0, ja1, jb0, jb1;      // jaw bbox (pixels where Phi0 or its jaw derivative can be non-zero)
+    int ri0, rj0, pu, pv;        // compact region origin and pitch (pu % 8 == 0, ri0 % 4 == 0)
+    int ntx, nty;                // region size in RU x RV thread-tiles
+    int ncx, ncy, ntxc, ntyc;    // conv chunk grid and chunk size [thread-tiles]
+    int n_items;                 // Nw * ncx * ncy conv work items (0 when empty)
+    int pad_;
+    unsigned long long support_vox, footprint_vox, region_vox, macs_fwd, macs_adj;
+};
+
+struct WorkCounters {
+    long long items, support_vox, footprint_vox, region_vox, macs_fwd, macs_adj;
+};
+
+struct SliceBox { int u0, u1, v0, v1; };   // inclusive voxel-index box; empty when u0 > u1 or v0 > v1
+
+__device__ __forceinline__ bool box_empty(const SliceBox &b) { return b.u0 > b.u1 || b.v0 > b.v1; }
+
+// S_k: beam voxels of slice k whose bilinear stencil (Eq. 5) can touch a pixel of the fluence
+// support bbox, i.e. fa in (a0-1, a1+1), fb in (b0-1, b1+1); rounded outward, clipped to the grid.
+// Every kernel derives its per-slice extents from this one function.
+__device__ __forceinline__ SliceBox slice_support(const Params &P, const CpDesc &d, int k)
+{
+    const float inv_mag = (P.sid + P.wmin + k * P.dw) / P.sid;
+    const float ulo = (d.a0 - 1 - P.cuf) * P.Du * inv_mag, uhi = (d.a1 + 1 - P.cuf) * P.Du * inv_mag;
+    const float vlo = (d.b0 - 1 - P.cvf) * P.Dv * inv_mag, vhi = (d.b1 + 1 - P.cvf) * P.Dv * inv_mag;
+    SliceBox s;
+    s.u0 = max(0, (int)floorf(ulo / P.du + P.cu));
+    s.u1 = min(P.Nu - 1, (int)ceilf(uhi / P.du + P.cu));
+    s.v0 = max(0, (int)floorf((vlo - P.v0) / P.dv));
+    s.v1 = min(P.Nv - 1, (int)ceilf((vhi - P.v0) / P.dv));
+    return s;
+}
+
+// F_k = S_k dilated by the kernel half-width, clipped to the beam grid.
+__device__ __forceinline__ SliceBox dilate(const Params &P, const SliceBox &s, int c)
+{
+    SliceBox f;
+    f.u0 = max(0, s.u0 - c); f.u1 = min(P.Nu - 1, s.u1 + c);
+    f.v0 = max(0, s.v0 - c); f.v1 = min(P.Nv - 1, s.v1 + c);
+    if (box_empty(s)) { f.u0 = 1; f.u1 = 0; }
+    return f;
+}
+
+__device__ __forceinline__ size_t compact_index(const Params &P, const CpDesc &d, int slot, int i, int j, int k)
+{
+    return (size_t)slot * (size_t)P.stride_cp + ((size_t)(j - d.rj0) * P.Nw + k) * d.pu + (i - d.ri0);
+}
+
+// Eq. 4: fractional overlap of [lo,hi] with the pixel centred at c, width D.
+__device__ __forceinline__ float ov(float c, float D, float lo, float hi)
+{
+    const float a = fminf(hi, c + 0.5f * D) - fmaxf(lo, c - 0.5f * D);
+    return a > 0.f ? a / D : 0.f;
+}
+// Subgradients of Eq. 4 with the half-open convention of DESIGN.md G9.
+__device__ __forceinline__ float dov_dhi(float c, float D, float lo, float hi)
+{
+    const float pl = c - 0.5f * D, pr = c + 0.5f * D;
+    return (pl <= hi && hi < pr && hi >= fmaxf(lo, pl)) ? 1.f / D : 0.f;
+}
+__device__ __forceinline__ float dov_dlo(float c, float D, float lo, float hi)
+{
+    const float pl = c - 0.5f * D, pr = c + 0.5f * D;
+    return (pl < lo && lo <= pr && lo <= fminf(hi, pr)) ? -1.f / D : 0.f;
+}
+
+__device__ __forceinline__ float warp_sum(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+}  // namespace pdrt

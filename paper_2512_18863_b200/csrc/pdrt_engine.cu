@@ -1,0 +1,577 @@
+// pdrt_engine.cu — engine object and the C ABI of include/pdrt.h.  Host code only marshals arguments,
+// builds the depth-indexed kernel table once (float64 -> float32) and enqueues kernels; every step of
+// the dose path runs in the kernels of pdrt_{fluence,depth,conv,resample}.cuh.  No CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <initializer_list>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/pdrt.h"
+#include "pdrt_conv.cuh"
+#include "pdrt_depth.cuh"
+#include "pdrt_dev.cuh"
+#include "pdrt_fluence.cuh"
+#include "pdrt_resample.cuh"
+
+using namespace pdrt;
+
+namespace {
+
+std::string g_create_error;
+
+// compiled conv variants; a requested size k runs on the smallest KT >= k with the table embedded in zeros
+const int kCompiled[] = { 5, 11, 15, 21, 25, 31, 41, 51, 63 };
+int compiled_size(int k)
+{
+    for (int kt : kCompiled)
+        if (kt >= k) return kt;
+    return -1;
+}
+int tile_floats_for(int kt) { return kt <= 21 ? 8192 : 12288; }
+size_t conv_smem_bytes(int kt) { return sizeof(float) * ((size_t)kt * ((kt + 3) & ~3) + tile_floats_for(kt)); }
+
+template <typename T> struct DevBuf {
+    T *p = nullptr;
+    size_t n = 0;
+    cudaError_t ensure(size_t count)
+    {
+        if (count <= n) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; n = 0;
+        cudaError_t e = cudaMalloc((void **)&p, count * sizeof(T));
+        if (e == cudaSuccess) n = count;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+    size_t bytes() const { return n * sizeof(T); }
+};
+
+}  // namespace
+
+struct pdrt_engine {
+    int device = 0, sm_count = 148;
+    Params P{};
+    FluTables T{};
+    int K = 0;
+    std::vector<double> kA, ka, kB, kb;
+    std::string err;
+    // persistent device data
+    DevBuf<float> density, wtab, pool;
+    // per-call scratch (sized by control-point capacity)
+    DevBuf<CpDesc> desc;
+    DevBuf<int> tile_base;
+    DevBuf<WorkCounters> counters;
+    DevBuf<float> phimap, P0, T1, T2, T3, Abuf, gphimap, zrad;
+    DevBuf<double> rho_s, Z_s;
+    DevBuf<float> bufA, bufB;         // compact beam-frame blocks: D_b / G_b and H_b
+    // staging for the *_host entry points
+    DevBuf<float> s_leaves, s_jaws, s_gantry, s_mu, s_vol, s_dleaves, s_djaws, s_dmu;
+    size_t scratch_cap_bytes = (size_t)48 << 30;
+    int last_n_cp = 0;
+    bool last_backward = false;
+    cudaStream_t last_stream = nullptr;
+    int conv_grid = 0;
+
+    size_t scratch_bytes() const
+    {
+        return desc.bytes() + tile_base.bytes() + phimap.bytes() + P0.bytes() + T1.bytes() + T2.bytes() + T3.bytes() +
+               Abuf.bytes() + gphimap.bytes() + zrad.bytes() + rho_s.bytes() + Z_s.bytes() + bufA.bytes() + bufB.bytes();
+    }
+};
+
+namespace {
+
+int fail(pdrt_engine *e, int code, const std::string &msg)
+{
+    if (e) e->err = msg; else g_create_error = msg;
+    return code;
+}
+#define CU(e, call)                                                                                  \
+    do {                                                                                             \
+        cudaError_t _s = (call);                                                                     \
+        if (_s != cudaSuccess)                                                                       \
+            return fail((e), _s == cudaErrorMemoryAllocation ? PDRT_ENOMEM : PDRT_ECUDA,             \
+                        std::string(#call) + ": " + cudaGetErrorString(_s));                         \
+    } while (0)
+
+// Gaussian taps (G13): g[t] ∝ exp(-(t D)^2 / 2 sigma^2), |t| <= ceil(3 sigma / D), normalised.
+int gaussian_taps(double sigma, double D, std::vector<float> &g)
+{
+    if (!(sigma > 0.0)) { g.assign(1, 1.f); return 0; }
+    const int T = (int)std::ceil(3.0 * sigma / D);
+    std::vector<double> w(2 * T + 1);
+    double sum = 0.0;
+    for (int t = -T; t <= T; ++t) { w[t + T] = std::exp(-0.5 * (t * D / sigma) * (t * D / sigma)); sum += w[t + T]; }
+    g.resize(2 * T + 1);
+    for (int t = 0; t <= 2 * T; ++t) g[t] = (float)(w[t] / sum);
+    return T;
+}
+
+// Pencil-kernel table (G3, G4): pixel-integrated weights of
+// K(r;z) = (A e^{-a r} + B e^{-b r}) / r  by 8x8 midpoint sub-sampling, one quadrant computed and mirrored,
+// embedded centred in the compiled KT x KT window.
+int build_kernel_table(pdrt_engine *e, int k)
+{
+    const int kt = compiled_size(k);
+    const int c = (k - 1) / 2, ct = (kt - 1) / 2, nz = e->P.n_z;
+    const double du = e->P.du, dv = e->P.dv;
+    std::vector<float> tab((size_t)nz * kt * kt, 0.f);
+    std::vector<double> rad((size_t)(c + 1) * (c + 1) * 64);
+    for (int qj = 0; qj <= c; ++qj)
+        for (int qi = 0; qi <= c; ++qi)
+            for (int sj = 0; sj < 8; ++sj)
+                for (int si = 0; si < 8; ++si) {
+                    const double x = (qi + (si + 0.5) / 8.0 - 0.5) * du, y = (qj + (sj + 0.5) / 8.0 - 0.5) * dv;
+                    rad[(((size_t)qj * (c + 1) + qi) * 8 + sj) * 8 + si] = std::sqrt(x * x + y * y);
+                }
+    for (int n = 0; n < nz; ++n) {
+        const double A = e->kA[n], a = e->ka[n], B = e->kB[n], b = e->kb[n];
+        for (int qj = 0; qj <= c; ++qj)
+            for (int qi = 0; qi <= c; ++qi) {
+                double s = 0.0;
+                const double *r = &rad[((size_t)qj * (c + 1) + qi) * 64];
+                for (int q = 0; q < 64; ++q) s += (A * std::exp(-a * r[q]) + B * std::exp(-b * r[q])) / r[q];
+                const float w = (float)(s * du * dv / 64.0);
+                float *slice = &tab[(size_t)n * kt * kt];
+                slice[(ct + qj) * kt + (ct + qi)] = w; slice[(ct + qj) * kt + (ct - qi)] = w;
+                slice[(ct - qj) * kt + (ct + qi)] = w; slice[(ct - qj) * kt + (ct - qi)] = w;
+            }
+    }
+    CU(e, e->wtab.ensure(tab.size()));
+    CU(e, cudaMemcpy(e->wtab.p, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice));
+    e->K = k;
+    e->P.K = k;
+    e->P.KT = kt;
+    e->P.tile_floats = tile_floats_for(kt);
+    return PDRT_OK;
+}
+
+template <int KT, bool ADJ>
+int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *Gin, float *out, cudaStream_t st)
+{
+    static int per_sm = 0;                            // resident blocks per SM, queried once per variant
+    const size_t smem = conv_smem_bytes(KT);
+    if (per_sm == 0) {
+        CU(e, cudaFuncSetAttribute(k_conv<KT, ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int n_res = 0;
+        CU(e, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n_res, k_conv<KT, ADJ>, CONV_THREADS, smem));
+        per_sm = n_res < 1 ? 1 : n_res;
+    }
+    e->conv_grid = e->sm_count * per_sm;              // persistent grid: a multiple of the SM count
+    k_conv<KT, ADJ><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->phimap.p,
+                                                             e->zrad.p, e->wtab.p, Gin, out);
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+template <bool ADJ> int launch_conv(pdrt_engine *e, int cp0, int n, const float *Gin, float *out, cudaStream_t st)
+{
+    switch (e->P.KT) {
+    case 5: return launch_conv_t<5, ADJ>(e, cp0, n, Gin, out, st);
+    case 11: return launch_conv_t<11, ADJ>(e, cp0, n, Gin, out, st);
+    case 15: return launch_conv_t<15, ADJ>(e, cp0, n, Gin, out, st);
+    case 21: return launch_conv_t<21, ADJ>(e, cp0, n, Gin, out, st);
+    case 25: return launch_conv_t<25, ADJ>(e, cp0, n, Gin, out, st);
+    case 31: return launch_conv_t<31, ADJ>(e, cp0, n, Gin, out, st);
+    case 41: return launch_conv_t<41, ADJ>(e, cp0, n, Gin, out, st);
+    case 51: return launch_conv_t<51, ADJ>(e, cp0, n, Gin, out, st);
+    case 63: return launch_conv_t<63, ADJ>(e, cp0, n, Gin, out, st);
+    }
+    return fail(e, PDRT_EINVAL, "no compiled convolution variant for this kernel size");
+}
+
+int ensure_cp_scratch(pdrt_engine *e, int n_cp)
+{
+    const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
+    CU(e, e->desc.ensure(n_cp));
+    CU(e, e->tile_base.ensure((size_t)n_cp + 1));
+    CU(e, e->counters.ensure(1));
+    CU(e, e->phimap.ensure(nmap)); CU(e, e->P0.ensure(nmap)); CU(e, e->T1.ensure(nmap));
+    CU(e, e->T2.ensure(nmap)); CU(e, e->Abuf.ensure(nmap));
+    CU(e, e->zrad.ensure((size_t)n_cp * e->P.Nw));
+    CU(e, e->rho_s.ensure((size_t)n_cp * e->P.M_ray));
+    CU(e, e->Z_s.ensure((size_t)n_cp * (e->P.M_ray + 1)));
+    return PDRT_OK;
+}
+// control points per batch so that `nbuf` compact buffers stay within the scratch cap
+int batch_size(const pdrt_engine *e, int n_cp, int nbuf)
+{
+    const size_t per_cp = (size_t)e->P.stride_cp * sizeof(float) * nbuf;
+    size_t b = e->scratch_cap_bytes / per_cp;
+    if (b < 1) b = 1;
+    return (int)(b < (size_t)n_cp ? b : (size_t)n_cp);
+}
+
+int check_call(pdrt_engine *e, int n_cp, std::initializer_list<const void *> ptrs)
+{
+    if (!e) return fail(nullptr, PDRT_EINVAL, "null engine");
+    if (n_cp < 1) return fail(e, PDRT_EINVAL, "n_cp must be >= 1");
+    for (const void *p : ptrs)
+        if (!p) return fail(e, PDRT_EINVAL, "null pointer argument");
+    CU(e, cudaSetDevice(e->device));
+    return PDRT_OK;
+}
+
+// S1 + descriptors for all control points, S2 depths
+int run_setup(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry, const float *mu,
+              bool need_depth, cudaStream_t st)
+{
+    int rc = ensure_cp_scratch(e, n_cp);
+    if (rc) return rc;
+    k_fluence<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, gantry, mu, e->desc.p, e->P0.p, e->T1.p,
+                                           e->T2.p, e->Abuf.p, e->phimap.p);
+    CU(e, cudaGetLastError());
+    if (need_depth) {
+        k_depth<<<n_cp, DEPTH_THREADS, 0, st>>>(e->P, n_cp, e->density.p, gantry, e->rho_s.p, e->Z_s.p, e->zrad.p);
+        CU(e, cudaGetLastError());
+    }
+    return PDRT_OK;
+}
+
+int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry, const float *mu,
+                 float *dose, cudaStream_t st)
+{
+    int rc = run_setup(e, n_cp, leaves, jaws, gantry, mu, true, st);
+    if (rc) return rc;
+    const int nb = batch_size(e, n_cp, 1);
+    CU(e, e->bufA.ensure((size_t)nb * e->P.stride_cp));
+    const dim3 gg((e->P.nx + GATHER_TX - 1) / GATHER_TX, (e->P.ny + GATHER_TY - 1) / GATHER_TY, e->P.nz);
+    for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
+        const int n = std::min(nb, n_cp - cp0);
+        k_scan_items<<<1, 32, 0, st>>>(e->desc.p, cp0, n, e->tile_base.p, e->counters.p);
+        CU(e, cudaGetLastError());
+        rc = launch_conv<false>(e, cp0, n, nullptr, e->bufA.p, st);
+        if (rc) return rc;
+        k_gather_dose<<<gg, dim3(GATHER_TX, GATHER_TY), 0, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, dose, cp0 > 0);
+        CU(e, cudaGetLastError());
+    }
+    e->last_n_cp = n_cp; e->last_backward = false; e->last_stream = st;
+    return PDRT_OK;
+}
+
+// S7-S9 for all control points: leaves dL/dPhimap (per control point, inside its support bbox) in e->gphimap
+int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry,
+                        const float *mu, const float *gdose, cudaStream_t st)
+{
+    int rc = run_setup(e, n_cp, leaves, jaws, gantry, mu, true, st);
+    if (rc) return rc;
+    const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
+    CU(e, e->gphimap.ensure(nmap));
+    CU(e, e->T3.ensure(nmap));
+    const int nb = batch_size(e, n_cp, 2);
+    CU(e, e->bufA.ensure((size_t)nb * e->P.stride_cp));
+    CU(e, e->bufB.ensure((size_t)nb * e->P.stride_cp));
+    for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
+        const int n = std::min(nb, n_cp - cp0);
+        k_scan_items<<<1, 32, 0, st>>>(e->desc.p, cp0, n, e->tile_base.p, e->counters.p);
+        CU(e, cudaGetLastError());
+        k_resample_adjoint<<<dim3(64, n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, gdose, e->bufA.p);
+        CU(e, cudaGetLastError());
+        rc = launch_conv<true>(e, cp0, n, e->bufA.p, e->bufB.p, st);
+        if (rc) return rc;
+        k_project_adjoint<<<dim3(e->P.Nvf, n), 128, 0, st>>>(e->P, e->desc.p, cp0, n, e->bufB.p, e->gphimap.p);
+        CU(e, cudaGetLastError());
+    }
+    return PDRT_OK;
+}
+
+int backward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry, const float *mu,
+                  const float *gdose, float *d_leaves, float *d_jaws, float *d_mu, cudaStream_t st)
+{
+    int rc = backward_to_fluence(e, n_cp, leaves, jaws, gantry, mu, gdose, st);
+    if (rc) return rc;
+    k_fluence_adjoint<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, e->desc.p, e->phimap.p, e->Abuf.p,
+                                                   e->gphimap.p, e->T1.p, e->T2.p, e->T3.p, d_leaves, d_jaws, d_mu);
+    CU(e, cudaGetLastError());
+    e->last_n_cp = n_cp; e->last_backward = true; e->last_stream = st;
+    return PDRT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *pdrt_last_error(const pdrt_engine *engine) { return engine ? engine->err.c_str() : g_create_error.c_str(); }
+
+int pdrt_create(const pdrt_grid *grid, const float *density, const pdrt_beam_model *m, pdrt_engine **out)
+{
+    if (!grid || !density || !m || !out) return fail(nullptr, PDRT_EINVAL, "null argument");
+    *out = nullptr;
+    if (grid->nx < 1 || grid->ny < 1 || grid->nz < 1 || !(grid->sx > 0) || !(grid->sy > 0) || !(grid->sz > 0))
+        return fail(nullptr, PDRT_EINVAL, "grid sizes and spacings must be positive");
+    if ((long long)grid->nx * grid->ny * grid->nz > (1ll << 31) - 1) return fail(nullptr, PDRT_EINVAL, "grid too large");
+    if (!(m->sid_mm > 0)) return fail(nullptr, PDRT_EINVAL, "sid_mm must be positive");
+    if (m->n_pairs < 1 || !m->leaf_bounds_mm) return fail(nullptr, PDRT_EINVAL, "n_pairs >= 1 and leaf_bounds_mm required");
+    for (int i = 0; i < m->n_pairs; ++i)
+        if (!(m->leaf_bounds_mm[i] < m->leaf_bounds_mm[i + 1])) return fail(nullptr, PDRT_EINVAL, "leaf_bounds_mm must be strictly ascending");
+    if (m->flu_nu < 1 || m->flu_nv < 1 || !(m->flu_du > 0) || !(m->flu_dv > 0)) return fail(nullptr, PDRT_EINVAL, "bad fluence map geometry");
+    if (!(m->tau >= 0.f && m->tau <= 1.f)) return fail(nullptr, PDRT_EINVAL, "tau must lie in [0,1]");
+    if (!(m->fwhm_mlc_mm >= 0) || !(m->fwhm_jaw_mm >= 0)) return fail(nullptr, PDRT_EINVAL, "penumbra FWHM must be >= 0");
+    if (m->n_hs < 0 || m->n_hs > MAX_HS || (m->n_hs > 0 && (!m->hs_amp || !m->hs_sigma_mm)))
+        return fail(nullptr, PDRT_EINVAL, "n_hs must lie in 0..4 with both tables given");
+    if (m->n_oar < 0 || (m->n_oar > 0 && (!m->oar || !(m->oar_dr_mm > 0)))) return fail(nullptr, PDRT_EINVAL, "bad off-axis table");
+    if (m->n_z < 2 || !(m->dz_mm > 0) || !m->kA || !m->ka || !m->kB || !m->kb) return fail(nullptr, PDRT_EINVAL, "kernel tables need n_z >= 2 and dz_mm > 0");
+    for (int n = 0; n < m->n_z; ++n)
+        if (!std::isfinite(m->kA[n]) || !std::isfinite(m->ka[n]) || !std::isfinite(m->kB[n]) || !std::isfinite(m->kb[n]))
+            return fail(nullptr, PDRT_EINVAL, "non-finite kernel table entry");
+    if (m->kernel_size < 3 || m->kernel_size > 63 || m->kernel_size % 2 == 0) return fail(nullptr, PDRT_EINVAL, "kernel_size must be odd, 3..63");
+    if (m->beam_nu < 0 || (m->beam_nu > 0 && (m->beam_nw < 1 || !(m->beam_du > 0) || !(m->beam_dw > 0))))
+        return fail(nullptr, PDRT_EINVAL, "bad beam grid");
+    if (!(m->ray_step_mm >= 0)) return fail(nullptr, PDRT_EINVAL, "ray_step_mm must be >= 0");
+
+    pdrt_engine *e = new (std::nothrow) pdrt_engine();
+    if (!e) return fail(nullptr, PDRT_ENOMEM, "out of host memory");
+    auto bail = [&](int code) { g_create_error = e->err; pdrt_destroy(e); return code; };
+    cudaError_t s = cudaGetDevice(&e->device);
+    if (s != cudaSuccess) { fail(e, PDRT_ECUDA, std::string("no CUDA device: ") + cudaGetErrorString(s)); return bail(PDRT_ECUDA); }
+    cudaDeviceProp prop;
+    s = cudaGetDeviceProperties(&prop, e->device);
+    if (s != cudaSuccess) { fail(e, PDRT_ECUDA, std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(s)); return bail(PDRT_ECUDA); }
+    e->sm_count = prop.multiProcessorCount;
+    if (const char *cap = std::getenv("PDRT_SCRATCH_GB")) {
+        const double gb = std::atof(cap);
+        if (gb > 0) e->scratch_cap_bytes = (size_t)(gb * (double)(1ull << 30));
+    }
+    {   // leave headroom on smaller devices
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && e->scratch_cap_bytes > free_b / 2) e->scratch_cap_bytes = free_b / 2;
+    }
+
+    Params &P = e->P;
+    P.nx = grid->nx; P.ny = grid->ny; P.nz = grid->nz;
+    P.sx = grid->sx; P.sy = grid->sy; P.sz = grid->sz;
+    P.ox = grid->ox; P.oy = grid->oy; P.oz = grid->oz;
+    P.isox = grid->iso[0]; P.isoy = grid->iso[1]; P.isoz = grid->iso[2];
+    if (m->beam_nu > 0) { P.Nu = m->beam_nu; P.Nw = m->beam_nw; P.du = m->beam_du; P.dw = m->beam_dw; P.wmin = m->beam_wmin; }
+    else { P.Nu = grid->nx; P.Nw = grid->ny; P.du = P.dw = grid->sx; P.wmin = -0.5f * (P.Nw - 1) * P.dw; }
+    P.Nv = grid->nz; P.dv = grid->sz;
+    P.cu = 0.5f * (P.Nu - 1); P.v0 = grid->oz - grid->iso[2];
+    P.Nuf = m->flu_nu; P.Nvf = m->flu_nv; P.Du = m->flu_du; P.Dv = m->flu_dv;
+    P.cuf = 0.5f * (P.Nuf - 1); P.cvf = 0.5f * (P.Nvf - 1);
+    P.sid = m->sid_mm; P.tau = m->tau; P.cal = m->cal; P.Np = m->n_pairs;
+    P.n_z = m->n_z; P.dz = m->dz_mm;
+    if (!(P.sid + P.wmin > 0)) { fail(e, PDRT_EINVAL, "beam grid must lie in front of the source (sid + beam_wmin > 0)"); return bail(PDRT_EINVAL); }
+    P.ray_step = m->ray_step_mm > 0 ? (double)m->ray_step_mm : 0.5 * (double)std::fmin(grid->sx, std::fmin(grid->sy, grid->sz));
+    const double dmax = (double)P.sid + (double)P.wmin + (P.Nw - 1) * (double)P.dw;
+    P.M_ray = (int)std::floor(dmax / P.ray_step) + 2;
+    P.stride_cp = (long long)((P.Nu + 7) / 8 * 8) * P.Nw * P.Nv;
+    e->kA.assign(m->kA, m->kA + m->n_z); e->ka.assign(m->ka, m->ka + m->n_z);
+    e->kB.assign(m->kB, m->kB + m->n_z); e->kb.assign(m->kb, m->kb + m->n_z);
+
+    // fluence tables: one float pool on the device
+    std::vector<float> pool;
+    auto push = [&](const float *src, size_t n) { size_t off = pool.size(); pool.insert(pool.end(), src, src + n); while (pool.size() % 4) pool.push_back(0.f); return off; };
+    const size_t o_lb = push(m->leaf_bounds_mm, m->n_pairs + 1);
+    const float one = 1.f;
+    const size_t o_oar = m->n_oar > 0 ? push(m->oar, m->n_oar) : push(&one, 1);
+    std::vector<float> gu, gv, hgu[MAX_HS], hgv[MAX_HS];
+    FluTables &T = e->T;
+    T.Tu = gaussian_taps(m->fwhm_mlc_mm / 2.354820045, m->flu_du, gu);
+    T.Tv = gaussian_taps(m->fwhm_jaw_mm / 2.354820045, m->flu_dv, gv);
+    int tu_max = T.Tu, tv_max = T.Tv;
+    size_t o_hgu[MAX_HS] = {}, o_hgv[MAX_HS] = {};
+    T.n_hs = m->n_hs;
+    for (int q = 0; q < m->n_hs; ++q) {
+        T.hs_amp[q] = m->hs_amp[q];
+        T.hs_Tu[q] = gaussian_taps(m->hs_sigma_mm[q], m->flu_du, hgu[q]);
+        T.hs_Tv[q] = gaussian_taps(m->hs_sigma_mm[q], m->flu_dv, hgv[q]);
+        tu_max = std::max(tu_max, T.hs_Tu[q]); tv_max = std::max(tv_max, T.hs_Tv[q]);
+    }
+    if (tu_max > MAX_TAPS || tv_max > MAX_TAPS) { fail(e, PDRT_EINVAL, "Gaussian wider than 64 pixels"); return bail(PDRT_EINVAL); }
+    const size_t o_gu = push(gu.data(), gu.size()), o_gv = push(gv.data(), gv.size());
+    for (int q = 0; q < m->n_hs; ++q) { o_hgu[q] = push(hgu[q].data(), hgu[q].size()); o_hgv[q] = push(hgv[q].data(), hgv[q].size()); }
+    P.Tu_max = tu_max; P.Tv_max = tv_max;
+
+    auto cuda_bail = [&](cudaError_t st, const char *what) {
+        fail(e, st == cudaErrorMemoryAllocation ? PDRT_ENOMEM : PDRT_ECUDA, std::string(what) + ": " + cudaGetErrorString(st));
+        return bail(st == cudaErrorMemoryAllocation ? PDRT_ENOMEM : PDRT_ECUDA);
+    };
+    if ((s = e->pool.ensure(pool.size())) != cudaSuccess) return cuda_bail(s, "cudaMalloc(tables)");
+    if ((s = cudaMemcpy(e->pool.p, pool.data(), pool.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_bail(s, "cudaMemcpy(tables)");
+    T.leaf_bounds = e->pool.p + o_lb; T.oar = e->pool.p + o_oar; T.n_oar = m->n_oar; T.oar_dr = m->n_oar > 0 ? m->oar_dr_mm : 1.f;
+    T.gu = e->pool.p + o_gu; T.gv = e->pool.p + o_gv;
+    for (int q = 0; q < m->n_hs; ++q) { T.hs_gu[q] = e->pool.p + o_hgu[q]; T.hs_gv[q] = e->pool.p + o_hgv[q]; }
+
+    const size_t nvox = (size_t)P.nx * P.ny * P.nz;
+    if ((s = e->density.ensure(nvox)) != cudaSuccess) return cuda_bail(s, "cudaMalloc(density)");
+    if ((s = cudaMemcpy(e->density.p, density, nvox * sizeof(float), cudaMemcpyDefault)) != cudaSuccess) return cuda_bail(s, "cudaMemcpy(density)");
+    int rc = build_kernel_table(e, m->kernel_size);
+    if (rc) return bail(rc);
+    *out = e;
+    return PDRT_OK;
+}
+
+void pdrt_destroy(pdrt_engine *e)
+{
+    if (!e) return;
+    cudaSetDevice(e->device);
+    cudaDeviceSynchronize();
+    e->density.release(); e->wtab.release(); e->pool.release(); e->desc.release(); e->tile_base.release();
+    e->counters.release(); e->phimap.release(); e->P0.release(); e->T1.release(); e->T2.release(); e->T3.release();
+    e->Abuf.release(); e->gphimap.release(); e->zrad.release(); e->rho_s.release(); e->Z_s.release();
+    e->bufA.release(); e->bufB.release();
+    e->s_leaves.release(); e->s_jaws.release(); e->s_gantry.release(); e->s_mu.release(); e->s_vol.release();
+    e->s_dleaves.release(); e->s_djaws.release(); e->s_dmu.release();
+    delete e;
+}
+
+int pdrt_set_kernel_size(pdrt_engine *e, int32_t k)
+{
+    if (!e) return fail(nullptr, PDRT_EINVAL, "null engine");
+    if (k < 3 || k > 63 || k % 2 == 0) return fail(e, PDRT_EINVAL, "kernel_size must be odd, 3..63");
+    CU(e, cudaSetDevice(e->device));
+    CU(e, cudaDeviceSynchronize());
+    return build_kernel_table(e, k);
+}
+
+int pdrt_get_info(const pdrt_engine *e, pdrt_info *info)
+{
+    if (!e || !info) return PDRT_EINVAL;
+    const Params &P = e->P;
+    info->nx = P.nx; info->ny = P.ny; info->nz = P.nz;
+    info->beam_nu = P.Nu; info->beam_nv = P.Nv; info->beam_nw = P.Nw;
+    info->beam_du = P.du; info->beam_dv = P.dv; info->beam_dw = P.dw; info->beam_wmin = P.wmin;
+    info->flu_nu = P.Nuf; info->flu_nv = P.Nvf; info->n_pairs = P.Np;
+    info->kernel_size = P.K; info->kernel_size_compiled = P.KT;
+    info->ray_step_mm = (float)P.ray_step; info->ray_samples = P.M_ray;
+    info->sm_count = e->sm_count;
+    info->scratch_bytes = e->scratch_bytes();
+    return PDRT_OK;
+}
+
+int pdrt_get_work(pdrt_engine *e, pdrt_work *w)
+{
+    if (!e || !w) return fail(e, PDRT_EINVAL, "null argument");
+    if (e->last_n_cp < 1 || !e->counters.p) return fail(e, PDRT_EINVAL, "no dose call has run on this engine yet");
+    CU(e, cudaSetDevice(e->device));
+    CU(e, cudaStreamSynchronize(e->last_stream));
+    WorkCounters wc;
+    CU(e, cudaMemcpy(&wc, e->counters.p, sizeof(wc), cudaMemcpyDeviceToHost));
+    w->n_cp = e->last_n_cp;
+    w->conv_items = wc.items; w->support_voxels = wc.support_vox; w->footprint_voxels = wc.footprint_vox;
+    w->region_voxels = wc.region_vox; w->conv_macs = e->last_backward ? wc.macs_adj : wc.macs_fwd;
+    w->kernel_size = e->P.K; w->kernel_size_compiled = e->P.KT;
+    return PDRT_OK;
+}
+
+int pdrt_dose(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry, const float *mu,
+              float *dose, void *stream)
+{
+    int rc = check_call(e, n_cp, { leaves, jaws, gantry, mu, dose });
+    if (rc) return rc;
+    return forward_impl(e, n_cp, leaves, jaws, gantry, mu, dose, (cudaStream_t)stream);
+}
+
+int pdrt_dose_backward(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry,
+                       const float *mu, const float *gdose, float *d_leaves, float *d_jaws, float *d_mu, void *stream)
+{
+    int rc = check_call(e, n_cp, { leaves, jaws, gantry, mu, gdose, d_leaves, d_jaws, d_mu });
+    if (rc) return rc;
+    return backward_impl(e, n_cp, leaves, jaws, gantry, mu, gdose, d_leaves, d_jaws, d_mu, (cudaStream_t)stream);
+}
+
+static int stage_params_in(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry,
+                           const float *mu, cudaStream_t st)
+{
+    CU(e, e->s_leaves.ensure((size_t)n_cp * 2 * e->P.Np)); CU(e, e->s_jaws.ensure((size_t)n_cp * 4));
+    CU(e, e->s_gantry.ensure(n_cp)); CU(e, e->s_mu.ensure(n_cp));
+    CU(e, cudaMemcpyAsync(e->s_leaves.p, leaves, sizeof(float) * n_cp * 2 * e->P.Np, cudaMemcpyHostToDevice, st));
+    CU(e, cudaMemcpyAsync(e->s_jaws.p, jaws, sizeof(float) * n_cp * 4, cudaMemcpyHostToDevice, st));
+    CU(e, cudaMemcpyAsync(e->s_gantry.p, gantry, sizeof(float) * n_cp, cudaMemcpyHostToDevice, st));
+    CU(e, cudaMemcpyAsync(e->s_mu.p, mu, sizeof(float) * n_cp, cudaMemcpyHostToDevice, st));
+    return PDRT_OK;
+}
+
+int pdrt_dose_host(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry,
+                   const float *mu, float *dose, void *stream)
+{
+    int rc = check_call(e, n_cp, { leaves, jaws, gantry, mu, dose });
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nvox = (size_t)e->P.nx * e->P.ny * e->P.nz;
+    if ((rc = stage_params_in(e, n_cp, leaves, jaws, gantry, mu, st))) return rc;
+    CU(e, e->s_vol.ensure(nvox));
+    if ((rc = forward_impl(e, n_cp, e->s_leaves.p, e->s_jaws.p, e->s_gantry.p, e->s_mu.p, e->s_vol.p, st))) return rc;
+    CU(e, cudaMemcpyAsync(dose, e->s_vol.p, nvox * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CU(e, cudaStreamSynchronize(st));
+    return PDRT_OK;
+}
+
+int pdrt_dose_backward_host(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry,
+                            const float *mu, const float *gdose, float *d_leaves, float *d_jaws, float *d_mu, void *stream)
+{
+    int rc = check_call(e, n_cp, { leaves, jaws, gantry, mu, gdose, d_leaves, d_jaws, d_mu });
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nvox = (size_t)e->P.nx * e->P.ny * e->P.nz, nl = (size_t)n_cp * 2 * e->P.Np;
+    if ((rc = stage_params_in(e, n_cp, leaves, jaws, gantry, mu, st))) return rc;
+    CU(e, e->s_vol.ensure(nvox)); CU(e, e->s_dleaves.ensure(nl)); CU(e, e->s_djaws.ensure((size_t)n_cp * 4)); CU(e, e->s_dmu.ensure(n_cp));
+    CU(e, cudaMemcpyAsync(e->s_vol.p, gdose, nvox * sizeof(float), cudaMemcpyHostToDevice, st));
+    if ((rc = backward_impl(e, n_cp, e->s_leaves.p, e->s_jaws.p, e->s_gantry.p, e->s_mu.p, e->s_vol.p, e->s_dleaves.p,
+                            e->s_djaws.p, e->s_dmu.p, st))) return rc;
+    CU(e, cudaMemcpyAsync(d_leaves, e->s_dleaves.p, nl * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CU(e, cudaMemcpyAsync(d_jaws, e->s_djaws.p, sizeof(float) * n_cp * 4, cudaMemcpyDeviceToHost, st));
+    CU(e, cudaMemcpyAsync(d_mu, e->s_dmu.p, sizeof(float) * n_cp, cudaMemcpyDeviceToHost, st));
+    CU(e, cudaStreamSynchronize(st));
+    return PDRT_OK;
+}
+
+int pdrt_stage_fluence(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, float *phimap, void *stream)
+{
+    int rc = check_call(e, n_cp, { leaves, jaws, phimap });
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = ensure_cp_scratch(e, n_cp))) return rc;
+    const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
+    CU(e, cudaMemsetAsync(e->phimap.p, 0, nmap * sizeof(float), st));     // outside the support bbox the map is zero
+    if ((rc = run_setup(e, n_cp, leaves, jaws, nullptr, nullptr, false, st))) return rc;
+    CU(e, cudaMemcpyAsync(phimap, e->phimap.p, nmap * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    return PDRT_OK;
+}
+
+int pdrt_stage_depth(pdrt_engine *e, int32_t n_cp, const float *gantry, float *zrad, void *stream)
+{
+    int rc = check_call(e, n_cp, { gantry, zrad });
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = ensure_cp_scratch(e, n_cp))) return rc;
+    k_depth<<<n_cp, DEPTH_THREADS, 0, st>>>(e->P, n_cp, e->density.p, gantry, e->rho_s.p, e->Z_s.p, e->zrad.p);
+    CU(e, cudaGetLastError());
+    CU(e, cudaMemcpyAsync(zrad, e->zrad.p, sizeof(float) * n_cp * e->P.Nw, cudaMemcpyDeviceToDevice, st));
+    return PDRT_OK;
+}
+
+int pdrt_stage_beam_dose(pdrt_engine *e, const float *leaves, const float *jaws, const float *gantry, float *db, void *stream)
+{
+    int rc = check_call(e, 1, { leaves, jaws, gantry, db });
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = run_setup(e, 1, leaves, jaws, gantry, nullptr, true, st))) return rc;
+    CU(e, e->bufA.ensure((size_t)e->P.stride_cp));
+    k_scan_items<<<1, 32, 0, st>>>(e->desc.p, 0, 1, e->tile_base.p, e->counters.p);
+    CU(e, cudaGetLastError());
+    if ((rc = launch_conv<false>(e, 0, 1, nullptr, e->bufA.p, st))) return rc;
+    k_expand_dense<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, 0, 0, e->bufA.p, db);
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+
+int pdrt_stage_grad_fluence(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry,
+                            const float *gdose, float *gphimap, void *stream)
+{
+    int rc = check_call(e, n_cp, { leaves, jaws, gantry, gdose, gphimap });
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
+    CU(e, e->gphimap.ensure(nmap));
+    CU(e, cudaMemsetAsync(e->gphimap.p, 0, nmap * sizeof(float), st));
+    if ((rc = backward_to_fluence(e, n_cp, leaves, jaws, gantry, nullptr, gdose, st))) return rc;
+    CU(e, cudaMemcpyAsync(gphimap, e->gphimap.p, nmap * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    return PDRT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,314 @@
+// pdrt_fluence.cuh — S1 aperture -> fluence rasteriser, the per-control-point descriptor, and S10
+// (rasteriser adjoint + MU gradient).  One block per control point; everything is confined to the
+// fluence support bbox (jaw opening dilated by the blur half-widths), so cost follows the field size.
+//
+// PAPER.md:103-119:  A = sum_i ov_v ov_u (Eq. 4), J = jaw mask, Phi0 = J (tau + (1-tau) A),
+// Phi1 = G_v(jaw) G_u(mlc) Phi0, Phi2 = Phi1 + sum_q amp_q G_u G_v Phi0, Phimap = Phi2 * OAR(r).
+#pragma once
+#include "pdrt_dev.cuh"
+
+namespace pdrt {
+
+constexpr int FLU_THREADS = 256;
+
+__device__ __forceinline__ float flu_u(const Params &P, int a) { return (a - P.cuf) * P.Du; }
+__device__ __forceinline__ float flu_v(const Params &P, int b) { return (b - P.cvf) * P.Dv; }
+
+__device__ __forceinline__ float oar_factor(const FluTables &T, float r)
+{
+    if (T.n_oar <= 0) return 1.f;
+    const float t = r / T.oar_dr;
+    const int n0 = (int)floorf(t);
+    if (n0 >= T.n_oar - 1) return T.oar[T.n_oar - 1];
+    const float f = t - n0;
+    return (1.f - f) * T.oar[n0] + f * T.oar[n0 + 1];
+}
+
+// value of a bbox-confined map at (a,b); zero outside the bbox (zero padding of the blurs)
+__device__ __forceinline__ float at_bbox(const float *m, const Params &P, const CpDesc &d, int a, int b)
+{
+    return (a >= d.a0 && a <= d.a1 && b >= d.b0 && b <= d.b1) ? m[b * P.Nuf + a] : 0.f;
+}
+
+// 1-D zero-padded convolution of a bbox-confined map along u (axis 0) or v (axis 1) at pixel (a,b)
+__device__ __forceinline__ float blur_at(const float *m, const Params &P, const CpDesc &d, int a, int b,
+                                         int axis, int T, const float *g)
+{
+    float s = 0.f;
+    for (int t = -T; t <= T; ++t) {
+        const int aa = axis == 0 ? a + t : a, bb = axis == 1 ? b + t : b;
+        s += g[t + T] * at_bbox(m, P, d, aa, bb);
+    }
+    return s;
+}
+
+// Builds CpDesc: gantry axes, jaw and support bboxes, compact region, conv chunking, work counters.
+__device__ void build_desc(const Params &P, const float *jaws, float gantry_deg, float mu, CpDesc &d)
+{
+    const double phi = (double)gantry_deg * 3.14159265358979323846 / 180.0;
+    d.cg = (float)cos(phi);
+    d.sg = (float)sin(phi);
+    d.scale = P.cal * mu;
+    const float x1 = jaws[0], x2 = jaws[1], y1 = jaws[2], y2 = jaws[3];
+    const float eu = -0.5f * P.Nuf * P.Du, ev = -0.5f * P.Nvf * P.Dv;     // left edge of pixel 0
+    // pixel of d ov/d lo: e_a < lo <= e_{a+1}; pixel of d ov/d hi: e_a <= hi < e_{a+1}
+    d.ja0 = max(0, (int)ceilf((x1 - eu) / P.Du) - 1);
+    d.ja1 = min(P.Nuf - 1, (int)floorf((x2 - eu) / P.Du));
+    d.jb0 = max(0, (int)ceilf((y1 - ev) / P.Dv) - 1);
+    d.jb1 = min(P.Nvf - 1, (int)floorf((y2 - ev) / P.Dv));
+    const bool empty = d.ja0 > d.ja1 || d.jb0 > d.jb1 || !(x1 <= x2) || !(y1 <= y2);
+    d.a0 = max(0, d.ja0 - P.Tu_max); d.a1 = min(P.Nuf - 1, d.ja1 + P.Tu_max);
+    d.b0 = max(0, d.jb0 - P.Tv_max); d.b1 = min(P.Nvf - 1, d.jb1 + P.Tv_max);
+    d.ri0 = d.rj0 = d.pu = d.pv = d.ntx = d.nty = 0;
+    d.ncx = d.ncy = d.ntxc = d.ntyc = d.n_items = 0;
+    d.pad_ = 0;
+    d.support_vox = d.footprint_vox = d.region_vox = d.macs_fwd = d.macs_adj = 0ull;
+    if (empty) { d.a0 = d.ja0 = 1; d.a1 = d.ja1 = 0; d.b0 = d.jb0 = 1; d.b1 = d.jb1 = 0; return; }
+    const int C = (P.KT - 1) / 2;
+    const SliceBox s0 = slice_support(P, d, 0), s1 = slice_support(P, d, P.Nw - 1);
+    const int u0 = max(0, min(s0.u0, s1.u0) - C), u1 = min(P.Nu - 1, max(s0.u1, s1.u1) + C);
+    const int v0 = max(0, min(s0.v0, s1.v0) - C), v1 = min(P.Nv - 1, max(s0.v1, s1.v1) + C);
+    if (u0 > u1 || v0 > v1) { d.a0 = d.ja0 = 1; d.a1 = d.ja1 = 0; d.b0 = d.jb0 = 1; d.b1 = d.jb1 = 0; return; }
+    d.ri0 = u0 & ~3;
+    d.pu = ((u1 - d.ri0 + 1) + RU - 1) / RU * RU;
+    d.rj0 = v0;
+    d.pv = v1 - v0 + 1;
+    d.ntx = d.pu / RU;
+    d.nty = (d.pv + RV - 1) / RV;
+    d.ncx = (d.ntx + NTXC_MAX - 1) / NTXC_MAX;
+    d.ntxc = (d.ntx + d.ncx - 1) / d.ncx;
+    const int XW = (P.KT + RU - 1 + 3) & ~3;
+    const int pitch = d.ntxc * RU + XW - RU;
+    int ntyc_max = (P.tile_floats / pitch - (P.KT - 1)) / RV;
+    if (ntyc_max < 1) ntyc_max = 1;
+    d.ncy = (d.nty + ntyc_max - 1) / ntyc_max;
+    d.ntyc = (d.nty + d.ncy - 1) / d.ncy;
+    d.n_items = P.Nw * d.ncx * d.ncy;
+    d.region_vox = (unsigned long long)d.pu * d.pv * P.Nw;
+}
+
+// S1.  Grid: n_cp blocks.  Scratch maps P0, T1, T2, A are [n_cp][Nvf][Nuf].
+__global__ void __launch_bounds__(FLU_THREADS)
+k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, const float *__restrict__ jaws,
+          const float *__restrict__ gantry_deg, const float *__restrict__ mu, CpDesc *desc,
+          float *P0, float *T1, float *T2, float *Abuf, float *phimap)
+{
+    const int cp = blockIdx.x, tid = threadIdx.x;
+    if (cp >= n_cp) return;
+    __shared__ CpDesc d;
+    __shared__ unsigned long long cnt[4];
+    if (tid == 0) {
+        build_desc(P, jaws + 4 * cp, gantry_deg ? gantry_deg[cp] : 0.f, mu ? mu[cp] : 0.f, d);
+        cnt[0] = cnt[1] = cnt[2] = cnt[3] = 0ull;
+    }
+    __syncthreads();
+    const bool empty = d.a0 > d.a1;
+    if (!empty) {     // per-slice work counters: |S_k|, |F_k|, thread-tiles
+        const int C = (P.KT - 1) / 2;
+        unsigned long long sup = 0, fp = 0, tf = 0, ta = 0;
+        for (int k = tid; k < P.Nw; k += FLU_THREADS) {
+            const SliceBox s = slice_support(P, d, k), f = dilate(P, s, C);
+            if (box_empty(s)) continue;
+            sup += (unsigned long long)(s.u1 - s.u0 + 1) * (s.v1 - s.v0 + 1);
+            fp += (unsigned long long)(f.u1 - f.u0 + 1) * (f.v1 - f.v0 + 1);
+            tf += (unsigned long long)((f.u1 - d.ri0) / RU - (f.u0 - d.ri0) / RU + 1) * ((f.v1 - d.rj0) / RV - (f.v0 - d.rj0) / RV + 1);
+            ta += (unsigned long long)((s.u1 - d.ri0) / RU - (s.u0 - d.ri0) / RU + 1) * ((s.v1 - d.rj0) / RV - (s.v0 - d.rj0) / RV + 1);
+        }
+        atomicAdd(&cnt[0], sup); atomicAdd(&cnt[1], fp); atomicAdd(&cnt[2], tf); atomicAdd(&cnt[3], ta);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        d.support_vox = cnt[0]; d.footprint_vox = cnt[1];
+        d.macs_fwd = cnt[2] * (unsigned long long)(RU * RV * P.KT * P.KT);
+        d.macs_adj = cnt[3] * (unsigned long long)(RU * RV * P.KT * P.KT);
+        desc[cp] = d;
+    }
+    if (empty) return;
+
+    const size_t mo = (size_t)cp * P.Nuf * P.Nvf;
+    float *p0 = P0 + mo, *t1 = T1 + mo, *t2 = T2 + mo, *Am = Abuf + mo, *pm = phimap + mo;
+    const float *lv = leaves + (size_t)cp * 2 * P.Np, *jw = jaws + 4 * cp;
+    const int bw = d.a1 - d.a0 + 1, bh = d.b1 - d.b0 + 1, npx = bw * bh;
+    const float x1 = jw[0], x2 = jw[1], y1 = jw[2], y2 = jw[3];
+
+    // O1, O2: A, J, Phi0
+    for (int p = tid; p < npx; p += FLU_THREADS) {
+        const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+        float A = 0.f, J = 0.f;
+        if (a >= d.ja0 && a <= d.ja1 && b >= d.jb0 && b <= d.jb1) {
+            const float uf = flu_u(P, a), vf = flu_v(P, b);
+            for (int i = 0; i < P.Np; ++i) {
+                const float ovv = ov(vf, P.Dv, T.leaf_bounds[i], T.leaf_bounds[i + 1]);
+                if (ovv != 0.f) A += ovv * ov(uf, P.Du, lv[i], lv[P.Np + i]);
+            }
+            J = ov(uf, P.Du, x1, x2) * ov(vf, P.Dv, y1, y2);
+        }
+        Am[b * P.Nuf + a] = A;
+        p0[b * P.Nuf + a] = J * (P.tau + (1.f - P.tau) * A);
+    }
+    __syncthreads();
+    // O3: penumbra, u with the MLC width then v with the jaw width
+    for (int p = tid; p < npx; p += FLU_THREADS) {
+        const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+        t1[b * P.Nuf + a] = blur_at(p0, P, d, a, b, 0, T.Tu, T.gu);
+    }
+    __syncthreads();
+    for (int p = tid; p < npx; p += FLU_THREADS) {
+        const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+        pm[b * P.Nuf + a] = blur_at(t1, P, d, a, b, 1, T.Tv, T.gv);
+    }
+    // O4: head scatter
+    for (int q = 0; q < T.n_hs; ++q) {
+        __syncthreads();
+        for (int p = tid; p < npx; p += FLU_THREADS) {
+            const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+            t2[b * P.Nuf + a] = blur_at(p0, P, d, a, b, 1, T.hs_Tv[q], T.hs_gv[q]);
+        }
+        __syncthreads();
+        for (int p = tid; p < npx; p += FLU_THREADS) {
+            const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+            pm[b * P.Nuf + a] += T.hs_amp[q] * blur_at(t2, P, d, a, b, 0, T.hs_Tu[q], T.hs_gu[q]);
+        }
+    }
+    __syncthreads();
+    // O5: off-axis
+    for (int p = tid; p < npx; p += FLU_THREADS) {
+        const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+        const float uf = flu_u(P, a), vf = flu_v(P, b);
+        pm[b * P.Nuf + a] *= oar_factor(T, sqrtf(uf * uf + vf * vf));
+    }
+}
+
+// Exclusive prefix of the conv work items over the control points [cp0, cp0+n) and the totals.
+__global__ void k_scan_items(const CpDesc *desc, int cp0, int n, int *tile_base, WorkCounters *wc)
+{
+    __shared__ long long tot[6];
+    if (threadIdx.x == 0) {
+        long long items = 0, sup = 0, fp = 0, reg = 0, mf = 0, ma = 0;
+        for (int c = 0; c < n; ++c) {
+            const CpDesc &d = desc[cp0 + c];
+            tile_base[c] = (int)items;
+            items += d.n_items; sup += d.support_vox; fp += d.footprint_vox; reg += d.region_vox;
+            mf += d.macs_fwd; ma += d.macs_adj;
+        }
+        tile_base[n] = (int)items;
+        tot[0] = items; tot[1] = sup; tot[2] = fp; tot[3] = reg; tot[4] = mf; tot[5] = ma;
+        if (cp0 == 0) { wc->items = 0; wc->support_vox = 0; wc->footprint_vox = 0; wc->region_vox = 0; wc->macs_fwd = 0; wc->macs_adj = 0; }
+        wc->items += tot[0]; wc->support_vox += tot[1]; wc->footprint_vox += tot[2];
+        wc->region_vox += tot[3]; wc->macs_fwd += tot[4]; wc->macs_adj += tot[5];
+    }
+}
+
+// S10.  d_mu = cal <Phimap, gPhimap>; then cal*MU*gPhimap back through OAR, the (self-adjoint,
+// zero-padded) Gaussians, the product Phi0 = J (tau + (1-tau) A) and Eq. 4's subgradients.
+// One block per control point; leaf gradients need no reduction (one thread per leaf edge),
+// jaw and MU gradients use warp-shuffle + shared-memory block reductions (no global atomics).
+__global__ void __launch_bounds__(FLU_THREADS)
+k_fluence_adjoint(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, const float *__restrict__ jaws,
+                  const CpDesc *__restrict__ desc, const float *__restrict__ phimap, const float *__restrict__ Abuf,
+                  const float *__restrict__ gphimap, float *T1, float *T2, float *T3,
+                  float *d_leaves, float *d_jaws, float *d_mu)
+{
+    const int cp = blockIdx.x, tid = threadIdx.x;
+    if (cp >= n_cp) return;
+    __shared__ CpDesc d;
+    __shared__ float red[5][FLU_THREADS / 32];
+    if (tid == 0) d = desc[cp];
+    __syncthreads();
+    float *dl = d_leaves + (size_t)cp * 2 * P.Np;
+    if (d.a0 > d.a1) {      // closed jaws: nothing reaches the patient
+        for (int e = tid; e < 2 * P.Np; e += FLU_THREADS) dl[e] = 0.f;
+        if (tid < 4) d_jaws[4 * cp + tid] = 0.f;
+        if (tid == 0) d_mu[cp] = 0.f;
+        return;
+    }
+    const size_t mo = (size_t)cp * P.Nuf * P.Nvf;
+    const float *pm = phimap + mo, *Am = Abuf + mo, *gp = gphimap + mo;
+    float *g2 = T1 + mo, *t = T2 + mo, *gP0 = T3 + mo;
+    const float *lv = leaves + (size_t)cp * 2 * P.Np, *jw = jaws + 4 * cp;
+    const int bw = d.a1 - d.a0 + 1, bh = d.b1 - d.b0 + 1, npx = bw * bh;
+    const float x1 = jw[0], x2 = jw[1], y1 = jw[2], y2 = jw[3];
+    float acc[5] = { 0.f, 0.f, 0.f, 0.f, 0.f };     // d_x1, d_x2, d_y1, d_y2, <Phimap, gPhimap>
+
+    for (int p = tid; p < npx; p += FLU_THREADS) {          // O5 transposed, scaled by cal*MU
+        const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+        const float uf = flu_u(P, a), vf = flu_v(P, b);
+        const float gv = gp[b * P.Nuf + a];
+        acc[4] += pm[b * P.Nuf + a] * gv;
+        g2[b * P.Nuf + a] = d.scale * gv * oar_factor(T, sqrtf(uf * uf + vf * vf));
+    }
+    __syncthreads();
+    for (int p = tid; p < npx; p += FLU_THREADS) {          // O3 transposed: v (jaw) ...
+        const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+        t[b * P.Nuf + a] = blur_at(g2, P, d, a, b, 1, T.Tv, T.gv);
+    }
+    __syncthreads();
+    for (int p = tid; p < npx; p += FLU_THREADS) {          // ... then u (MLC)
+        const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+        gP0[b * P.Nuf + a] = blur_at(t, P, d, a, b, 0, T.Tu, T.gu);
+    }
+    for (int q = 0; q < T.n_hs; ++q) {                      // O4 transposed
+        __syncthreads();
+        for (int p = tid; p < npx; p += FLU_THREADS) {
+            const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+            t[b * P.Nuf + a] = blur_at(g2, P, d, a, b, 0, T.hs_Tu[q], T.hs_gu[q]);
+        }
+        __syncthreads();
+        for (int p = tid; p < npx; p += FLU_THREADS) {
+            const int a = d.a0 + p % bw, b = d.b0 + p / bw;
+            gP0[b * P.Nuf + a] += T.hs_amp[q] * blur_at(t, P, d, a, b, 1, T.hs_Tv[q], T.hs_gv[q]);
+        }
+    }
+    __syncthreads();
+    // O2: jaws (product rule; d ov is non-zero on one pixel column / row only)
+    const int jw_w = d.ja1 - d.ja0 + 1, jw_n = jw_w * (d.jb1 - d.jb0 + 1);
+    for (int p = tid; p < jw_n; p += FLU_THREADS) {
+        const int a = d.ja0 + p % jw_w, b = d.jb0 + p / jw_w;
+        const float uf = flu_u(P, a), vf = flu_v(P, b);
+        const float ju = ov(uf, P.Du, x1, x2), jv = ov(vf, P.Dv, y1, y2);
+        const float gJ = gP0[b * P.Nuf + a] * (P.tau + (1.f - P.tau) * Am[b * P.Nuf + a]);
+        acc[0] += gJ * dov_dlo(uf, P.Du, x1, x2) * jv;
+        acc[1] += gJ * dov_dhi(uf, P.Du, x1, x2) * jv;
+        acc[2] += gJ * ju * dov_dlo(vf, P.Dv, y1, y2);
+        acc[3] += gJ * ju * dov_dhi(vf, P.Dv, y1, y2);
+    }
+    // O1: leaves — one thread per leaf edge, a handful of pixel rows each
+    const float eu = -0.5f * P.Nuf * P.Du, ev = -0.5f * P.Nvf * P.Dv;
+    for (int e = tid; e < 2 * P.Np; e += FLU_THREADS) {
+        const int bank = e / P.Np, i = e % P.Np;
+        const float lo = lv[i], hi = lv[P.Np + i];
+        const int ac = bank == 0 ? (int)ceilf((lo - eu) / P.Du) - 1 : (int)floorf((hi - eu) / P.Du);
+        float s = 0.f;
+        for (int a = ac - 1; a <= ac + 1; ++a) {      // the index arithmetic may be off by one at a pixel edge
+            if (a < d.ja0 || a > d.ja1) continue;
+            const float uf = flu_u(P, a);
+            const float dv_ = bank == 0 ? dov_dlo(uf, P.Du, lo, hi) : dov_dhi(uf, P.Du, lo, hi);
+            if (dv_ == 0.f) continue;
+            const float ju = ov(uf, P.Du, x1, x2);
+            const int blo = max(d.jb0, (int)floorf((T.leaf_bounds[i] - ev) / P.Dv) - 1);
+            const int bhi = min(d.jb1, (int)floorf((T.leaf_bounds[i + 1] - ev) / P.Dv) + 1);
+            for (int b = blo; b <= bhi; ++b) {
+                const float vf = flu_v(P, b);
+                const float ovv = ov(vf, P.Dv, T.leaf_bounds[i], T.leaf_bounds[i + 1]);
+                const float gA = gP0[b * P.Nuf + a] * ju * ov(vf, P.Dv, y1, y2) * (1.f - P.tau);
+                s += gA * ovv * dv_;
+            }
+        }
+        dl[e] = s;
+    }
+    // block reduction of the five scalars
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+        const float v = warp_sum(acc[q]);
+        if ((tid & 31) == 0) red[q][tid >> 5] = v;
+    }
+    __syncthreads();
+    if (tid < 5) {
+        float s = 0.f;
+        for (int w = 0; w < FLU_THREADS / 32; ++w) s += red[tid][w];
+        if (tid < 4) d_jaws[4 * cp + tid] = s;
+        else d_mu[cp] = P.cal * s;
+    }
+}
+
+}  // namespace pdrt

@@ -1,0 +1,195 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by element, on the same
+seeded inputs.  Acceptance (BASELINE.json north_star): dose  max|D_gpu - D_orc| <= 1e-4 * max(D_orc);
+gradients  ||g_gpu - g_orc||_2 / ||g_orc||_2 <= 1e-3 per group (leaves, jaws, MU) and max-abs <= 1e-3 * max|g_orc|.
+"""
+import numpy as np
+import pytest
+
+from paper_2512_18863_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+DOSE_TOL = 1e-4
+GRAD_TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def pair(wl):
+    from oracle.oracle import Oracle
+    from paper_2512_18863_b200 import Engine
+    return Engine(wl.grid, wl.model, wl.density), Oracle(wl.grid, wl.model, wl.density)
+
+
+def assert_dose(gpu, orc, what=""):
+    gpu = gpu.double().cpu().numpy() if hasattr(gpu, "cpu") else np.asarray(gpu, np.float64)
+    scale = np.abs(orc).max()
+    err = np.abs(gpu - orc).max()
+    assert np.isfinite(gpu).all(), what
+    assert scale > 0, f"{what}: oracle dose is identically zero"
+    assert err <= DOSE_TOL * scale, f"{what}: max err {err:.3e} vs {DOSE_TOL}*max {scale:.3e} (ratio {err / scale:.2e})"
+    return err / scale
+
+
+def assert_grad(gpu, orc, what=""):
+    gpu = gpu.double().cpu().numpy()
+    assert np.isfinite(gpu).all(), what
+    n = np.linalg.norm(orc)
+    assert n > 0, f"{what}: oracle gradient is identically zero"
+    rel = np.linalg.norm(gpu - orc) / n
+    mx = np.abs(gpu - orc).max() / np.abs(orc).max()
+    assert rel <= GRAD_TOL and mx <= GRAD_TOL, f"{what}: rel L2 {rel:.2e}, max-abs ratio {mx:.2e}"
+    return rel
+
+
+TINY_CASES = [
+    dict(seed=7),
+    dict(seed=8, kernel_size=3, head_scatter=False),
+    dict(seed=9, kernel_size=7, nx=37, ny=29, nz=17, n_cp=4, flu=(26, 22)),
+    dict(seed=10, kernel_size=11, nx=45, ny=40, nz=21, spacing=3.0, flu=(40, 30), flu_d=2.0, n_pairs=11),
+    dict(seed=11, kernel_size=13, nx=70, ny=33, nz=40, spacing=2.5, flu=(48, 44), flu_d=2.5, n_pairs=9, n_cp=2),
+]
+
+
+@pytest.mark.parametrize("case", TINY_CASES, ids=lambda c: f"seed{c['seed']}")
+def test_stages_tiny(torch, case):
+    wl = W.tiny(**case)
+    eng, orc = pair(wl)
+    phim = eng.stage_fluence(wl.leaves, wl.jaws).double().cpu().numpy()
+    zr = eng.stage_depth(wl.gantry_deg).double().cpu().numpy()
+    for b in range(wl.n_cp):
+        ref = orc.fluence(wl.leaves[b], wl.jaws[b])
+        assert np.abs(phim[b] - ref).max() <= 2e-6 * max(ref.max(), 1e-30), f"fluence map cp {b}"
+        zref = orc.radiological_depth(wl.gantry_deg[b])
+        assert np.abs(zr[b] - zref).max() <= 1e-5 * max(zref.max(), 1.0), f"radiological depth cp {b}"
+        db = eng.stage_beam_dose(wl.leaves[b:b + 1], wl.jaws[b:b + 1], wl.gantry_deg[b:b + 1])
+        assert_dose(db, orc.beam_dose(wl.leaves[b], wl.jaws[b], wl.gantry_deg[b]), f"beam dose cp {b}")
+
+
+@pytest.mark.parametrize("case", TINY_CASES, ids=lambda c: f"seed{c['seed']}")
+def test_forward_backward_tiny(torch, case):
+    wl = W.tiny(**case)
+    eng, orc = pair(wl)
+    d_ref = orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
+    assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), d_ref, "dose")
+    g = W.seeded_dose_gradient(wl, seed=case["seed"])
+    gphi = eng.stage_grad_fluence(wl.leaves, wl.jaws, wl.gantry_deg, g).double().cpu().numpy()
+    dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    Wt = orc.kernel_table()
+    for b in range(wl.n_cp):        # dL/dPhimap inside the fluence support of each control point
+        z = orc.radiological_depth(wl.gantry_deg[b])
+        ref = orc.project_adjoint(orc.convolve(Wt, z, orc.resample_adjoint(wl.gantry_deg[b], g), transpose=True))
+        sup = gphi[b] != 0
+        assert sup.any()
+        assert np.abs(gphi[b][sup] - ref[sup]).max() <= 1e-4 * np.abs(ref).max(), f"dL/dPhimap cp {b}"
+    assert_grad(dm, rm, "d_mu")
+    assert_grad(dj, rj, "d_jaws")
+    assert_grad(dl, rl, "d_leaves")
+
+
+def test_config1_water_phantom(torch):
+    """c1: 64^3 water, one open 10x10 field, beam grid == patient grid (S6 is the identity)."""
+    wl = W.config1()
+    eng, orc = pair(wl)
+    d_ref = orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
+    d = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
+    assert_dose(d, d_ref, "c1 dose")
+    # properties on the GPU result itself: mirror symmetry of the symmetric field (P3), MU linearity (P1)
+    dn = d.cpu().numpy()
+    assert np.allclose(dn, dn[:, :, ::-1], rtol=1e-4, atol=1e-6 * dn.max())
+    assert np.allclose(dn, dn[::-1], rtol=1e-4, atol=1e-6 * dn.max())
+    d2 = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, 2.0 * wl.mu).cpu().numpy()
+    assert np.allclose(d2, 2.0 * dn, rtol=1e-6)
+    closed = wl.jaws.copy()
+    closed[:, 1] = closed[:, 0] - 1.0
+    assert float(eng.dose(wl.leaves, closed, wl.gantry_deg, wl.mu).abs().max()) == 0.0     # P2
+
+
+def test_config2_slab_phantom_forward_and_backward(torch):
+    """c2: heterogeneous slabs, 5 beams with irregular apertures, k = 21; forward and (beyond BASELINE) backward."""
+    wl = W.config2()
+    eng, orc = pair(wl)
+    d_ref = orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
+    assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), d_ref, "c2 dose")
+    g = W.seeded_dose_gradient(wl, seed=2)
+    dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    assert_grad(dm, rm, "c2 d_mu")
+    assert_grad(dj, rj, "c2 d_jaws")
+    assert_grad(dl, rl, "c2 d_leaves")
+
+
+def test_edge_cases(torch):
+    """Closed and inverted jaws, closed leaves, fields cut by the map / grid edge, a single control point,
+    kernel sizes that run on a larger compiled variant."""
+    wl = W.tiny(seed=12, n_cp=5, kernel_size=9, nx=40, ny=36, nz=14, flu=(24, 20))
+    half_u = 0.5 * wl.model["flu_nu"] * wl.model["flu_du"]
+    wl.jaws[0, :2] = (3.0, 3.0)                    # closed
+    wl.jaws[1, :2] = (9.0, -9.0)                   # inverted
+    wl.leaves[2] = 0.0                             # all pairs closed: transmission only
+    wl.jaws[3] = (-10 * half_u, 10 * half_u, -1e3, 1e3)   # wider than the map and the grid
+    wl.leaves[3, 0], wl.leaves[3, 1] = -1e3, 1e3
+    eng, orc = pair(wl)
+    d_ref = orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
+    assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), d_ref, "edge dose")
+    g = W.seeded_dose_gradient(wl, seed=12)
+    dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    assert float(dm[0]) == 0.0 and float(dm[1]) == 0.0 and float(dl[0].abs().max()) == 0.0
+    assert_grad(dm, rm, "edge d_mu")
+    assert_grad(dl[2:], rl[2:], "edge d_leaves")
+    assert_grad(dj[2:], rj[2:], "edge d_jaws")
+    for b in range(wl.n_cp):                        # single control points, one at a time
+        one = eng.dose(wl.leaves[b:b + 1], wl.jaws[b:b + 1], wl.gantry_deg[b:b + 1], wl.mu[b:b + 1])
+        ref = orc.dose(wl.leaves[b:b + 1], wl.jaws[b:b + 1], wl.gantry_deg[b:b + 1], wl.mu[b:b + 1])
+        if ref.max() > 0:
+            assert_dose(one, ref, f"edge single cp {b}")
+        else:
+            assert float(one.abs().max()) == 0.0
+
+
+@pytest.mark.parametrize("k", [3, 5, 9, 17, 23, 33])
+def test_kernel_size_sweep_small(torch, k):
+    """pdrt_set_kernel_size, including sizes that have no compiled variant of their own."""
+    wl = W.tiny(seed=13, n_cp=2, kernel_size=5, nx=48, ny=44, nz=36, spacing=3.0, flu=(30, 30))
+    eng, orc = pair(wl)
+    eng.set_kernel_size(k)
+    orc.set_kernel_size(k)
+    assert eng.info.kernel_size == k and eng.info.kernel_size_compiled >= k
+    assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), f"k={k}")
+    g = W.seeded_dose_gradient(wl, seed=k)
+    dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    assert_grad(dm, rm, f"k={k} d_mu")
+    assert_grad(dl, rl, f"k={k} d_leaves")
+
+
+def test_host_entry_points_and_errors(torch):
+    from paper_2512_18863_b200 import Engine, PdrtError
+    wl = W.tiny(seed=14)
+    eng, orc = pair(wl)
+    out = torch.empty(eng.dose_shape, dtype=torch.float32).pin_memory()
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    eng.dose_host(t(wl.leaves), t(wl.jaws), t(wl.gantry_deg), t(wl.mu), out)
+    assert_dose(out, orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), "dose_host")
+    g = W.seeded_dose_gradient(wl, seed=14)
+    dl, dj, dm = (torch.empty(wl.leaves.shape).pin_memory(), torch.empty(wl.jaws.shape).pin_memory(), torch.empty(wl.mu.shape).pin_memory())
+    eng.dose_backward_host(t(wl.leaves), t(wl.jaws), t(wl.gantry_deg), t(wl.mu), t(g), dl, dj, dm)
+    rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    assert_grad(dl, rl, "host d_leaves"); assert_grad(dj, rj, "host d_jaws"); assert_grad(dm, rm, "host d_mu")
+    w = eng.get_work()
+    assert w.n_cp == wl.n_cp and w.support_voxels > 0 and w.footprint_voxels >= w.support_voxels and w.conv_macs > 0
+    bad = dict(wl.model, kernel_size=8)
+    with pytest.raises(PdrtError):
+        Engine(wl.grid, bad, wl.density)
+    with pytest.raises(PdrtError):
+        eng.set_kernel_size(65)
+    with pytest.raises(PdrtError):
+        Engine(wl.grid, dict(wl.model, leaf_bounds_mm=np.zeros(wl.model["n_pairs"] + 1, np.float32)), wl.density)

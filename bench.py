@@ -1,0 +1,367 @@
+#!/usr/bin/env python
+"""bench.py — full-arc VMAT dose forward + backward on B200 through the pdrt C ABI.
+
+One "step" is one pass of the whole hot path over the workload: pdrt_dose (S1-S6) followed by
+pdrt_dose_backward (S7-S10) for every control point of the arc.  Default workload: BASELINE.json
+configs[3] ("c4": synthetic prostate CT 200x200x120 @ 2.5 mm, 178 control points, 80 leaf pairs,
+k = 21) — the configuration the headline metric "ms per full-arc dose forward+backward" is quoted on.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c4|c5] [--kernel-size k] [--sweep]
+  python bench.py --impl reference ...      # the float64 CPU oracle on a bounded sample (context, not a target)
+
+Prints ONE JSON line (rank 0).  Timing: CUDA events on the launch stream, every timed step preceded by an
+L2 flush (a 256 MiB memset, outside the timed events); inputs resident in HBM for `value`, host buffers
+and copies inside the timed region for `e2e`.  N > 1 shards control points over ranks (one all-reduce of
+the dose grid per forward; gradients are disjoint), strong scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "ms per full-arc dose forward+backward"
+FP32_LANES_PER_SM = 128
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            self.proc.terminate()
+            self.thread.join(timeout=2)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            if len(r) >= 7:
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def make_workload(name, kernel_size):
+    from paper_2512_18863_b200 import workloads as W
+    if name == "c4":
+        return W.config4(kernel_size or 21)
+    wl = W.CONFIGS[name]()
+    if kernel_size:
+        wl.model["kernel_size"] = kernel_size
+    return wl
+
+
+def config_dict(wl, n_gpus, extra=None):
+    g, m = wl.grid, wl.model
+    c = dict(workload=f"{wl.name}: synthetic prostate CT {g['nx']}x{g['ny']}x{g['nz']} @ {g['sx']} mm, "
+                      f"{wl.n_cp} control points, {m['n_pairs']} leaf pairs, fluence {m['flu_nu']}x{m['flu_nv']}, "
+                      f"kernel {m['kernel_size']}, forward+backward",
+             n_cp=wl.n_cp, kernel_size=m["kernel_size"], seed=wl.seed,
+             parallelism=f"control points sharded over {n_gpus} GPU(s)" if n_gpus > 1 else "1 GPU",
+             l2="256 MiB memset between timed steps (L2 flush); compact D_b/G_b blocks exceed L2")
+    if extra:
+        c.update(extra)
+    return c
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def run_reference(args):
+    """The float64 oracle, as it stands, on the host cores.  Each step = forward+backward of a bounded sample of
+    control points; the line's value is that time scaled to the full arc."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle.oracle import Oracle
+    from paper_2512_18863_b200 import workloads as W
+    wl = make_workload(args.workload, args.kernel_size)
+    orc = Oracle(wl.grid, wl.model, wl.density)
+    n_s = max(1, min(args.ref_cps, wl.n_cp))
+    idx = np.linspace(0, wl.n_cp - 1, n_s).round().astype(int)
+    lv, jw, ga, mu = wl.leaves[idx], wl.jaws[idx], wl.gantry_deg[idx], wl.mu[idx]
+    g = W.seeded_dose_gradient(wl, seed=0)
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        orc.dose(lv, jw, ga, mu)
+        orc.dose_backward(lv, jw, ga, mu, g)
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            times.append(dt)
+    ms_full = float(np.mean(times)) * 1e3 * wl.n_cp / n_s
+    sample = f"{n_s} of {wl.n_cp} control points (evenly spaced), forward+backward, time scaled by {wl.n_cp}/{n_s}"
+    line = dict(impl="reference", metric=METRIC, value=ms_full, unit="ms", n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=ms_full, higher_is_better=False, scaling="strong", vs_baseline=None,
+                dtype="f64", data="synthetic", config=config_dict(wl, 1),
+                cpu_baseline=dict(value=ms_full, unit="ms", cores=orc.num_threads(), kind="oracle", sample=sample),
+                e2e=dict(value=ms_full, unit="ms", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def cpu_baseline(wl, seconds_budget=20.0):
+    """The oracle on a bounded sample of the same workload (rank 0, N = 1): forward+backward of a few control points."""
+    from oracle.oracle import Oracle
+    from paper_2512_18863_b200 import workloads as W
+    orc = Oracle(wl.grid, wl.model, wl.density)
+    g = W.seeded_dose_gradient(wl, seed=0)
+    n_s, total = 0, 0.0
+    idx_all = np.linspace(0, wl.n_cp - 1, min(wl.n_cp, 8)).round().astype(int)
+    for b in idx_all:
+        t0 = time.perf_counter()
+        orc.dose(wl.leaves[b:b + 1], wl.jaws[b:b + 1], wl.gantry_deg[b:b + 1], wl.mu[b:b + 1])
+        orc.dose_backward(wl.leaves[b:b + 1], wl.jaws[b:b + 1], wl.gantry_deg[b:b + 1], wl.mu[b:b + 1], g)
+        total += time.perf_counter() - t0
+        n_s += 1
+        if total > seconds_budget:
+            break
+    return dict(value=total / n_s * wl.n_cp * 1e3, unit="ms", cores=orc.num_threads(), kind="oracle",
+                sample=f"{n_s} of {wl.n_cp} control points, forward+backward, {total:.1f} s of CPU time scaled by {wl.n_cp}/{n_s}")
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2512_18863_b200 import Engine, STAGES, workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(dev)
+    peaks = load_peaks()
+    wl = make_workload(args.workload, args.kernel_size)
+    eng = Engine(wl.grid, wl.model, wl.density, device=str(dev))
+
+    # shard control points (contiguous blocks); every rank holds the density, tables and dL/dDose
+    lo, hi = (wl.n_cp * rank) // world, (wl.n_cp * (rank + 1)) // world
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    lv, jw, ga, mu = t(wl.leaves[lo:hi]), t(wl.jaws[lo:hi]), t(wl.gantry_deg[lo:hi]), t(wl.mu[lo:hi])
+    dose = torch.empty(eng.dose_shape, dtype=torch.float32, device=dev)
+    grads = (torch.empty_like(lv), torch.empty_like(jw), torch.empty_like(mu))
+    # objective gradient (harness): weights and prescriptions of the quadratic target/OAR objective
+    wmask = torch.zeros(eng.dose_shape, dtype=torch.float32, device=dev)
+    pmask = torch.zeros_like(wmask)
+    for mask, weight, presc in wl.masks.values():
+        mt = torch.from_numpy(mask).to(dev)
+        wmask[mt] += 2.0 * weight / max(int(mask.sum()), 1)
+        if presc:
+            pmask[mt] = presc
+    if not wl.masks:
+        wmask.fill_(1.0 / wmask.numel())
+
+    def forward():
+        eng.dose(lv, jw, ga, mu, out=dose)
+        if world > 1:
+            dist.all_reduce(dose)
+
+    def objective_grad():
+        return wmask * (dose - pmask)
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    forward()
+    g = objective_grad().contiguous()          # fixed dL/dDose for the timed steps
+    torch.cuda.synchronize()
+
+    def step():
+        forward()
+        eng.dose_backward(lv, jw, ga, mu, g, out=grads)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+
+    eng.set_profiling(True)
+    ev = [tuple(torch.cuda.Event(enable_timing=True) for _ in range(4)) for _ in range(args.steps)]
+    stage_ms = {s: 0.0 for s in STAGES}
+    launches = 0
+    t_wall0 = time.perf_counter()
+    with ClockSampler(local) as clk:
+        for a, b, b2, c in ev:
+            flush.zero_()                      # L2 flush, outside the timed events
+            a.record()
+            forward()
+            b.record()
+            fw_ms, fw_n = None, None
+            if world == 1:                     # per-stage events of the forward call, read before the backward resets them
+                fw_ms, fw_n = eng.get_stage_ms()
+            b2.record()
+            eng.dose_backward(lv, jw, ga, mu, g, out=grads)
+            c.record()
+            bw_ms, bw_n = eng.get_stage_ms()
+            for s in STAGES:
+                stage_ms[s] += bw_ms[s] + (fw_ms[s] if fw_ms else 0.0)
+            launches += sum(bw_n.values()) + (sum(fw_n.values()) if fw_n else 0)
+        torch.cuda.synchronize()
+    t_wall = time.perf_counter() - t_wall0
+    eng.set_profiling(False)
+    fwd_ms = float(np.mean([a.elapsed_time(b) for a, b, _, _ in ev]))
+    bwd_ms = float(np.mean([b2.elapsed_time(c) for _, _, b2, c in ev]))
+    step_ms = fwd_ms + bwd_ms
+    if world > 1:
+        tt = torch.tensor([step_ms, fwd_ms, bwd_ms], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        step_ms, fwd_ms, bwd_ms = [float(v) for v in tt]
+    for s in STAGES:
+        stage_ms[s] /= args.steps
+
+    # work counters of the forward and the backward call (device-counted from the actual fluence support)
+    forward(); wf = eng.get_work()
+    eng.dose_backward(lv, jw, ga, mu, g, out=grads); wb = eng.get_work()
+    K = wf.kernel_size
+    fp32_peak = eng.info.sm_count * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12      # TFLOP/s
+    conv_flops = 2.0 * K * K * wf.footprint_voxels                 # algorithmic: k^2 MAC per footprint voxel
+    conv_adj_flops = 2.0 * K * K * wb.support_voxels
+    stages = {}
+    if world == 1:
+        nvox = eng.info.nx * eng.info.ny * eng.info.nz
+        byts = dict(gather=4.0 * wf.region_voxels + 4.0 * nvox,                   # read D_b blocks once, write dose once
+                    resample_adj=4.0 * wb.region_voxels + 4.0 * nvox,             # read g once (L2-resident after), write G_b
+                    project_adj=4.0 * wb.support_voxels, conv=4.0 * wf.region_voxels, conv_adj=4.0 * (wb.region_voxels + wb.support_voxels))
+        for s in STAGES:
+            stages[s] = dict(ms=round(stage_ms[s], 4))
+            if s in byts and stage_ms[s] > 0:
+                gbs = byts[s] / (stage_ms[s] * 1e-3) / 1e9
+                stages[s].update(algorithmic_gb=round(byts[s] / 1e9, 4), gbs=round(gbs, 1), hbm_frac=round(gbs / peaks["hbm_gbs"], 4))
+        stages["conv"].update(tflops=round(conv_flops / (stage_ms["conv"] * 1e-3) / 1e12, 2) if stage_ms["conv"] > 0 else None,
+                              issued_tflops=round(2.0 * wf.conv_macs / (stage_ms["conv"] * 1e-3) / 1e12, 2) if stage_ms["conv"] > 0 else None)
+        stages["conv_adj"].update(tflops=round(conv_adj_flops / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None,
+                                  issued_tflops=round(2.0 * wb.conv_macs / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None)
+    achieved = conv_flops / (stage_ms["conv"] * 1e-3) / 1e12 if stage_ms["conv"] > 0 else None
+    roofline = dict(bound="alu", kernel="k_conv<K,false> (S3+S4+S5 fused projection + lateral convolution)",
+                    achieved=achieved, peak=fp32_peak, unit="TFLOP/s", frac=(achieved / fp32_peak) if achieved else None,
+                    traffic=None,
+                    note=f"algorithmic flops = 2*k^2*|footprint| per launch; peak = {eng.info.sm_count} SMs x 128 FP32 lanes x 2 x "
+                         f"{peaks['sm_max_mhz']:.0f} MHz (plain FP32 FMA pipe; FFMA microbenchmark on this pool: 72.5 TFLOP/s); "
+                         f"HBM fractions of the bandwidth-bound stages are under 'stages' against {peaks['hbm_gbs']} GB/s {peaks['source']}")
+
+    # end to end through the host-buffer C-ABI calls: H2D of parameters and dL/dDose, D2H of dose and gradients
+    e2e = None
+    if world == 1:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        h_lv, h_jw, h_ga, h_mu = pin(wl.leaves), pin(wl.jaws), pin(wl.gantry_deg), pin(wl.mu)
+        h_dose = torch.empty(eng.dose_shape, dtype=torch.float32).pin_memory()
+        h_g = g.cpu().pin_memory()
+        h_out = (torch.empty(wl.leaves.shape).pin_memory(), torch.empty(wl.jaws.shape).pin_memory(), torch.empty(wl.mu.shape).pin_memory())
+        times = []
+        for it in range(args.warmup + args.steps):
+            flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            eng.dose_host(h_lv, h_jw, h_ga, h_mu, h_dose)
+            eng.dose_backward_host(h_lv, h_jw, h_ga, h_mu, h_g, *h_out)
+            dt = time.perf_counter() - t0
+            if it >= args.warmup:
+                times.append(dt)
+        par_b = 4 * (h_lv.numel() + h_jw.numel() + h_ga.numel() + h_mu.numel())
+        e2e = dict(value=float(np.mean(times)) * 1e3, unit="ms", h2d_bytes_per_step=int(2 * par_b + 4 * h_g.numel()),
+                   d2h_bytes_per_step=int(4 * h_dose.numel() + 4 * sum(o.numel() for o in h_out)),
+                   note="pdrt_dose_host + pdrt_dose_backward_host with pinned host buffers; host wall clock around both calls")
+
+    sweep = None
+    if args.sweep and world == 1:
+        sweep = {}
+        for k in wl.kernel_sizes:
+            eng.set_kernel_size(k)
+            for _ in range(2):
+                step()
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(max(3, args.steps)):
+                flush.zero_()
+                a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+                a.record(); forward(); b.record(); eng.dose_backward(lv, jw, ga, mu, g, out=grads); c.record()
+                torch.cuda.synchronize()
+                ts.append((a.elapsed_time(b), b.elapsed_time(c)))
+            sweep[str(k)] = dict(forward_ms=round(float(np.median([x[0] for x in ts])), 4), backward_ms=round(float(np.median([x[1] for x in ts])), 4))
+        eng.set_kernel_size(wl.model["kernel_size"])
+
+    if rank == 0:
+        clocks = clk.summary()
+        line = dict(metric=METRIC, value=step_ms, unit="ms", n_gpus=world, steps=args.steps, warmup=args.warmup,
+                    ms_per_step=step_ms, higher_is_better=False, scaling="strong", vs_baseline=None, dtype="f32",
+                    data="synthetic", config=config_dict(wl, world),
+                    forward_ms=fwd_ms, backward_ms=bwd_ms, control_points_per_s=wl.n_cp / (step_ms * 1e-3),
+                    wall_ms_per_step_incl_flush=t_wall / args.steps * 1e3,
+                    clocks=clocks, gpu_launches=launches, e2e=e2e, roofline=roofline, stages=stages,
+                    work=dict(support_voxels=wf.support_voxels, footprint_voxels=wf.footprint_voxels, region_voxels=wf.region_voxels,
+                              conv_items=wf.conv_items, conv_macs_issued_fwd=wf.conv_macs, conv_macs_issued_bwd=wb.conv_macs,
+                              kernel_size_compiled=wf.kernel_size_compiled),
+                    paper_context="PAPER.md Table 6: 2.051 s forward / 5.102 s forward+backward, 180 CPs, grid 105x224x224, k=55, NVIDIA A40 (other machine, other workload)")
+        if sweep:
+            line["kernel_size_sweep"] = sweep
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(wl)
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--workload", default="c4", choices=("c3", "c4", "c5"))
+    ap.add_argument("--kernel-size", type=int, default=0)
+    ap.add_argument("--sweep", action="store_true", help="also time the kernel-size sweep of the workload")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-cps", type=int, default=2, help="control points per step of the reference arm")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -148,6 +148,25 @@ PDRT_API int pdrt_set_kernel_size(pdrt_engine *engine, int32_t kernel_size);
 PDRT_API int pdrt_get_info(const pdrt_engine *engine, pdrt_info *info);
 PDRT_API int pdrt_get_work(pdrt_engine *engine, pdrt_work *work);
 
+/* Per-stage device timing.  With profiling enabled every stage's kernel launches are bracketed by CUDA
+ * events on the call's stream; pdrt_get_stage_ms synchronises that stream and returns, for the most recent
+ * call, the milliseconds and the number of kernel launches of each stage (launches are counted even with
+ * profiling off; ms are then zero). */
+enum {
+    PDRT_STAGE_FLUENCE = 0,      /* S1  k_fluence (+ control-point descriptors)        */
+    PDRT_STAGE_DEPTH = 1,        /* S2  k_depth                                       */
+    PDRT_STAGE_SCAN = 2,         /*     k_scan_items (work-item prefix, counters)     */
+    PDRT_STAGE_CONV = 3,         /* S3+S4+S5  k_conv<K,false>                         */
+    PDRT_STAGE_GATHER = 4,       /* S6  k_gather_dose                                 */
+    PDRT_STAGE_RESAMPLE_ADJ = 5, /* S7  k_resample_adjoint                            */
+    PDRT_STAGE_CONV_ADJ = 6,     /* S8  k_conv<K,true>                                */
+    PDRT_STAGE_PROJECT_ADJ = 7,  /* S9  k_project_adjoint                             */
+    PDRT_STAGE_FLUENCE_ADJ = 8,  /* S10 k_fluence_adjoint                             */
+    PDRT_N_STAGES = 9
+};
+PDRT_API int pdrt_set_profiling(pdrt_engine *engine, int32_t enable);
+PDRT_API int pdrt_get_stage_ms(pdrt_engine *engine, float *ms /*[PDRT_N_STAGES]*/, int32_t *launches /*[PDRT_N_STAGES]*/);
+
 /* Forward (S1-S6, Eq. 4-9):  dose = cal * sum_b MU_b * R_b[ (P Phi_b) (*) K(z_rad) ].
  *   leaves_dev [n_cp][2][n_pairs], jaws_dev [n_cp][4], gantry_deg_dev [n_cp], mu_dev [n_cp],
  *   dose_dev [nz][ny][nx] overwritten.  n_cp >= 1. */

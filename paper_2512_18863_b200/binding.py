@@ -15,8 +15,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpdrt.so")
 
 SYMBOLS = ("pdrt_create", "pdrt_destroy", "pdrt_last_error", "pdrt_set_kernel_size", "pdrt_get_info", "pdrt_get_work",
+           "pdrt_set_profiling", "pdrt_get_stage_ms",
            "pdrt_dose", "pdrt_dose_backward", "pdrt_dose_host", "pdrt_dose_backward_host",
            "pdrt_stage_fluence", "pdrt_stage_depth", "pdrt_stage_beam_dose", "pdrt_stage_grad_fluence")
+
+STAGES = ("fluence", "depth", "scan", "conv", "gather", "resample_adj", "conv_adj", "project_adj", "fluence_adj")
 
 _FP = C.POINTER(C.c_float)
 
@@ -86,6 +89,8 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.pdrt_set_kernel_size.argtypes = [vp, i32]
     lib.pdrt_get_info.argtypes = [vp, C.POINTER(PdrtInfo)]
     lib.pdrt_get_work.argtypes = [vp, C.POINTER(PdrtWork)]
+    lib.pdrt_set_profiling.argtypes = [vp, i32]
+    lib.pdrt_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i32)]
     lib.pdrt_dose.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
     lib.pdrt_dose_backward.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.pdrt_dose_host.argtypes = lib.pdrt_dose.argtypes
@@ -190,6 +195,16 @@ class Engine:
         w = PdrtWork()
         self._check(self.lib.pdrt_get_work(self.handle, C.byref(w)))
         return w
+
+    def set_profiling(self, enable: bool):
+        self._check(self.lib.pdrt_set_profiling(self.handle, int(bool(enable))))
+
+    def get_stage_ms(self):
+        """(ms, launches) per stage of the most recent call, as dicts keyed by STAGES; synchronises."""
+        ms = (C.c_float * len(STAGES))()
+        n = (C.c_int32 * len(STAGES))()
+        self._check(self.lib.pdrt_get_stage_ms(self.handle, ms, n))
+        return dict(zip(STAGES, [float(v) for v in ms])), dict(zip(STAGES, [int(v) for v in n]))
 
     def set_kernel_size(self, k: int):
         self._check(self.lib.pdrt_set_kernel_size(self.handle, int(k)))

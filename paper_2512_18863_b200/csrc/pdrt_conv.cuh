@@ -18,6 +18,11 @@
 
 namespace pdrt {
 
+// Shared-memory tile columns are stored with an XOR swizzle on 16-byte quads: quad Q of a row lives at
+// Q ^ ((Q >> 3) & 1).  Lanes tx and tx+4 of one row (32 floats apart, same banks) then hit different banks,
+// so the LDS.128 window loads of 8 neighbouring thread-tiles are conflict-free.
+__device__ __forceinline__ int swz_col(int c) { return c ^ (((c >> 5) & 1) << 2); }
+
 __device__ __forceinline__ int find_cp(const int *__restrict__ tile_base, int n, int item)
 {
     int lo = 0, hi = n;            // largest c with tile_base[c] <= item
@@ -83,7 +88,7 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
         }
         if (!active) continue;                        // uniform across the block
         const int nax = atx1 - atx0 + 1, nay = aty1 - aty0 + 1;
-        const int pitch = nax * RU + XW - RU;
+        const int pitch = conv_pitch(KT, nax);
         const int rows = nay * RV + KT - 1;
         const int tu0 = d.ri0 + atx0 * RU - C, tv0 = d.rj0 + aty0 * RV - C;   // input coords of tile[0][0]
 
@@ -104,40 +109,54 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                 Ws[e] = v;
             }
         }
-        // input tile
+        // input tile: one warp per row, lanes along u (no integer division; coalesced for the adjoint)
+        const int warp = tid >> 5, lane = tid & 31;
         if (!ADJ) {
             // S3: divergent projection of the fluence map, sampled on the fly (Eq. 5-6)
             const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
+            const float su = mag * P.du / P.Du, sv = mag / P.Dv;
             const float *pm = phimap + (size_t)cp * P.Nuf * P.Nvf;
-            for (int e = tid; e < rows * pitch; e += CONV_THREADS) {
-                const int r = e / pitch, c = e - r * pitch;
-                const int i = tu0 + c, j = tv0 + r;
-                float v = 0.f;
-                if (i >= S.u0 && i <= S.u1 && j >= S.v0 && j <= S.v1) {
-                    const float fa = mag * ((i - P.cu) * P.du) / P.Du + P.cuf;
-                    const float fb = mag * (P.v0 + j * P.dv) / P.Dv + P.cvf;
-                    const float fla = floorf(fa), flb = floorf(fb);
-                    const int a = (int)fla, b = (int)flb;
-                    const float ta = fa - fla, tb = fb - flb;
-                    const bool a0 = a >= d.a0 && a <= d.a1, a1 = a + 1 >= d.a0 && a + 1 <= d.a1;
-                    const bool b0 = b >= d.b0 && b <= d.b1, b1 = b + 1 >= d.b0 && b + 1 <= d.b1;
-                    float s = 0.f;
-                    if (a0 && b0) s += (1.f - ta) * (1.f - tb) * __ldg(pm + b * P.Nuf + a);
-                    if (a1 && b0) s += ta * (1.f - tb) * __ldg(pm + b * P.Nuf + a + 1);
-                    if (a0 && b1) s += (1.f - ta) * tb * __ldg(pm + (b + 1) * P.Nuf + a);
-                    if (a1 && b1) s += ta * tb * __ldg(pm + (b + 1) * P.Nuf + a + 1);
-                    v = m2 * s;
+            for (int r = warp; r < rows; r += CONV_THREADS / 32) {
+                const int j = tv0 + r;
+                float *trow = tile + r * pitch;
+                if (j < S.v0 || j > S.v1) {
+                    for (int c = lane; c < pitch; c += 32) trow[c] = 0.f;
+                    continue;
                 }
-                tile[e] = v;
+                const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
+                const float flb = floorf(fb);
+                const int b = (int)flb;
+                const float tb = fb - flb;
+                const bool b0 = b >= d.b0 && b <= d.b1, b1 = b + 1 >= d.b0 && b + 1 <= d.b1;
+                const float *pr0 = pm + b * P.Nuf, *pr1 = pr0 + P.Nuf;
+                for (int c = lane; c < pitch; c += 32) {
+                    const int i = tu0 + c;
+                    float v = 0.f;
+                    if (i >= S.u0 && i <= S.u1) {
+                        const float fa = (i - P.cu) * su + P.cuf;
+                        const float fla = floorf(fa);
+                        const int a = (int)fla;
+                        const float ta = fa - fla;
+                        const bool a0 = a >= d.a0 && a <= d.a1, a1 = a + 1 >= d.a0 && a + 1 <= d.a1;
+                        float s0 = 0.f, s1 = 0.f;
+                        if (b0) s0 = (a0 ? (1.f - ta) * __ldg(pr0 + a) : 0.f) + (a1 ? ta * __ldg(pr0 + a + 1) : 0.f);
+                        if (b1) s1 = (a0 ? (1.f - ta) * __ldg(pr1 + a) : 0.f) + (a1 ? ta * __ldg(pr1 + a + 1) : 0.f);
+                        v = m2 * ((1.f - tb) * s0 + tb * s1);
+                    }
+                    trow[swz_col(c)] = v;
+                }
             }
         } else {
-            for (int e = tid; e < rows * pitch; e += CONV_THREADS) {
-                const int r = e / pitch, c = e - r * pitch;
-                const int i = tu0 + c, j = tv0 + r;
-                float v = 0.f;
-                if (i >= d.ri0 && i < d.ri0 + d.pu && i < P.Nu && j >= d.rj0 && j < d.rj0 + d.pv)
-                    v = __ldg(Gin + compact_index(P, d, slot, i, j, k));
-                tile[e] = v;
+            const int iend = min(d.ri0 + d.pu, P.Nu);
+            for (int r = warp; r < rows; r += CONV_THREADS / 32) {
+                const int j = tv0 + r;
+                float *trow = tile + r * pitch;
+                const bool rowin = j >= d.rj0 && j < d.rj0 + d.pv;
+                const float *grow = Gin + (size_t)slot * (size_t)P.stride_cp + ((long long)(j - d.rj0) * P.Nw + k) * d.pu - d.ri0;
+                for (int c = lane; c < pitch; c += 32) {
+                    const int i = tu0 + c;
+                    trow[swz_col(c)] = (rowin && i >= d.ri0 && i < iend) ? __ldg(grow + i) : 0.f;
+                }
             }
         }
         __syncthreads();
@@ -149,13 +168,16 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
             for (int jj = 0; jj < RV; ++jj)
 #pragma unroll
                 for (int r = 0; r < RU; ++r) acc[jj][r] = 0.f;
-            const float *xrow = tile + (ty * RV) * pitch + tx * RU;
+            const float *xrow = tile + (ty * RV) * pitch;
+            int xoff[NXQ];
+#pragma unroll
+            for (int q = 0; q < NXQ; ++q) xoff[q] = swz_col(tx * RU + 4 * q);
 #pragma unroll 1
             for (int y = 0; y < KT + RV - 1; ++y) {
                 float x[XW];
 #pragma unroll
                 for (int q = 0; q < NXQ; ++q) {
-                    const float4 v = *reinterpret_cast<const float4 *>(xrow + 4 * q);
+                    const float4 v = *reinterpret_cast<const float4 *>(xrow + xoff[q]);
                     x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
                 }
 #pragma unroll

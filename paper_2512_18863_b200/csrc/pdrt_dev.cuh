@@ -81,6 +81,14 @@ struct WorkCounters {
     long long items, support_vox, footprint_vox, region_vox, macs_fwd, macs_adj;
 };
 
+// Row pitch [floats] of the conv input tile for `nax` thread-tiles along u: the (K+7)-wide register window of
+// the last thread-tile must fit, rounded to 8 floats so that the quad swizzle stays inside the row.
+__host__ __device__ __forceinline__ int conv_pitch(int kt, int nax)
+{
+    const int xw = (kt + RU - 1 + 3) & ~3;
+    return (nax * RU + xw - RU + 7) & ~7;
+}
+
 struct SliceBox { int u0, u1, v0, v1; };   // inclusive voxel-index box; empty when u0 > u1 or v0 > v1
 
 __device__ __forceinline__ bool box_empty(const SliceBox &b) { return b.u0 > b.u1 || b.v0 > b.v1; }

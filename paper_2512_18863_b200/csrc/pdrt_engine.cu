@@ -76,6 +76,13 @@ struct pdrt_engine {
     bool last_backward = false;
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
+    // per-stage device timing of the most recent call (CUDA events on the call's stream)
+    bool profiling = false;
+    struct StageRec { int stage; cudaEvent_t a, b; };
+    std::vector<StageRec> recs;
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;
+    int launches[PDRT_N_STAGES] = {};
 
     size_t scratch_bytes() const
     {
@@ -98,6 +105,35 @@ int fail(pdrt_engine *e, int code, const std::string &msg)
             return fail((e), _s == cudaErrorMemoryAllocation ? PDRT_ENOMEM : PDRT_ECUDA,             \
                         std::string(#call) + ": " + cudaGetErrorString(_s));                         \
     } while (0)
+
+// Brackets the kernel launches of one stage with CUDA events when profiling is on; always counts launches.
+struct StageTimer {
+    pdrt_engine *e; cudaStream_t st; size_t rec = (size_t)-1;
+    StageTimer(pdrt_engine *e_, int stage, cudaStream_t st_, int n_launches = 1) : e(e_), st(st_)
+    {
+        e->launches[stage] += n_launches;
+        if (!e->profiling) return;
+        cudaEvent_t ev[2];
+        for (int q = 0; q < 2; ++q) {
+            if (e->ev_used == e->ev_pool.size()) {
+                cudaEvent_t n;
+                if (cudaEventCreate(&n) != cudaSuccess) return;
+                e->ev_pool.push_back(n);
+            }
+            ev[q] = e->ev_pool[e->ev_used++];
+        }
+        e->recs.push_back({ stage, ev[0], ev[1] });
+        rec = e->recs.size() - 1;
+        cudaEventRecord(ev[0], st);
+    }
+    ~StageTimer() { if (rec != (size_t)-1) cudaEventRecord(e->recs[rec].b, st); }
+};
+void reset_stage_records(pdrt_engine *e)
+{
+    e->recs.clear();
+    e->ev_used = 0;
+    for (int q = 0; q < PDRT_N_STAGES; ++q) e->launches[q] = 0;
+}
 
 // Gaussian taps (G13): g[t] ∝ exp(-(t D)^2 / 2 sigma^2), |t| <= ceil(3 sigma / D), normalised.
 int gaussian_taps(double sigma, double D, std::vector<float> &g)
@@ -213,6 +249,7 @@ int check_call(pdrt_engine *e, int n_cp, std::initializer_list<const void *> ptr
     for (const void *p : ptrs)
         if (!p) return fail(e, PDRT_EINVAL, "null pointer argument");
     CU(e, cudaSetDevice(e->device));
+    reset_stage_records(e);
     return PDRT_OK;
 }
 
@@ -222,13 +259,17 @@ int run_setup(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, 
 {
     int rc = ensure_cp_scratch(e, n_cp);
     if (rc) return rc;
-    k_fluence<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, gantry, mu, e->desc.p, e->P0.p, e->T1.p,
-                                           e->T2.p, e->Abuf.p, e->phimap.p);
+    {
+        StageTimer t(e, PDRT_STAGE_FLUENCE, st);
+        k_fluence<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, gantry, mu, e->desc.p, e->P0.p, e->T1.p,
+                                               e->T2.p, e->Abuf.p, e->phimap.p);
+    }
     CU(e, cudaGetLastError());
     if (need_depth) {
+        StageTimer t(e, PDRT_STAGE_DEPTH, st);
         k_depth<<<n_cp, DEPTH_THREADS, 0, st>>>(e->P, n_cp, e->density.p, gantry, e->rho_s.p, e->Z_s.p, e->zrad.p);
-        CU(e, cudaGetLastError());
     }
+    CU(e, cudaGetLastError());
     return PDRT_OK;
 }
 
@@ -242,11 +283,20 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
     const dim3 gg((e->P.nx + GATHER_TX - 1) / GATHER_TX, (e->P.ny + GATHER_TY - 1) / GATHER_TY, e->P.nz);
     for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
         const int n = std::min(nb, n_cp - cp0);
-        k_scan_items<<<1, 32, 0, st>>>(e->desc.p, cp0, n, e->tile_base.p, e->counters.p);
+        {
+            StageTimer t(e, PDRT_STAGE_SCAN, st);
+            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, e->tile_base.p, e->counters.p);
+        }
         CU(e, cudaGetLastError());
-        rc = launch_conv<false>(e, cp0, n, nullptr, e->bufA.p, st);
+        {
+            StageTimer t(e, PDRT_STAGE_CONV, st);
+            rc = launch_conv<false>(e, cp0, n, nullptr, e->bufA.p, st);
+        }
         if (rc) return rc;
-        k_gather_dose<<<gg, dim3(GATHER_TX, GATHER_TY), 0, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, dose, cp0 > 0);
+        {
+            StageTimer t(e, PDRT_STAGE_GATHER, st);
+            k_gather_dose<<<gg, dim3(GATHER_TX, GATHER_TY), 0, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, dose, cp0 > 0);
+        }
         CU(e, cudaGetLastError());
     }
     e->last_n_cp = n_cp; e->last_backward = false; e->last_stream = st;
@@ -267,13 +317,25 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
     CU(e, e->bufB.ensure((size_t)nb * e->P.stride_cp));
     for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
         const int n = std::min(nb, n_cp - cp0);
-        k_scan_items<<<1, 32, 0, st>>>(e->desc.p, cp0, n, e->tile_base.p, e->counters.p);
+        {
+            StageTimer t(e, PDRT_STAGE_SCAN, st);
+            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, e->tile_base.p, e->counters.p);
+        }
         CU(e, cudaGetLastError());
-        k_resample_adjoint<<<dim3(64, n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, gdose, e->bufA.p);
+        {
+            StageTimer t(e, PDRT_STAGE_RESAMPLE_ADJ, st);
+            k_resample_adjoint<<<dim3(48, n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, gdose, e->bufA.p);
+        }
         CU(e, cudaGetLastError());
-        rc = launch_conv<true>(e, cp0, n, e->bufA.p, e->bufB.p, st);
+        {
+            StageTimer t(e, PDRT_STAGE_CONV_ADJ, st);
+            rc = launch_conv<true>(e, cp0, n, e->bufA.p, e->bufB.p, st);
+        }
         if (rc) return rc;
-        k_project_adjoint<<<dim3(e->P.Nvf, n), 128, 0, st>>>(e->P, e->desc.p, cp0, n, e->bufB.p, e->gphimap.p);
+        {
+            StageTimer t(e, PDRT_STAGE_PROJECT_ADJ, st);
+            k_project_adjoint<<<dim3((e->P.Nuf * e->P.Nvf + 31) / 32, n), PROJ_THREADS, sizeof(SliceGeo) * e->P.Nw, st>>>(e->P, e->desc.p, cp0, n, e->bufB.p, e->gphimap.p);
+        }
         CU(e, cudaGetLastError());
     }
     return PDRT_OK;
@@ -284,8 +346,11 @@ int backward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *ja
 {
     int rc = backward_to_fluence(e, n_cp, leaves, jaws, gantry, mu, gdose, st);
     if (rc) return rc;
-    k_fluence_adjoint<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, e->desc.p, e->phimap.p, e->Abuf.p,
-                                                   e->gphimap.p, e->T1.p, e->T2.p, e->T3.p, d_leaves, d_jaws, d_mu);
+    {
+        StageTimer t(e, PDRT_STAGE_FLUENCE_ADJ, st);
+        k_fluence_adjoint<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, e->desc.p, e->phimap.p, e->Abuf.p,
+                                                       e->gphimap.p, e->T1.p, e->T2.p, e->T3.p, d_leaves, d_jaws, d_mu);
+    }
     CU(e, cudaGetLastError());
     e->last_n_cp = n_cp; e->last_backward = true; e->last_stream = st;
     return PDRT_OK;
@@ -416,6 +481,7 @@ void pdrt_destroy(pdrt_engine *e)
     e->bufA.release(); e->bufB.release();
     e->s_leaves.release(); e->s_jaws.release(); e->s_gantry.release(); e->s_mu.release(); e->s_vol.release();
     e->s_dleaves.release(); e->s_djaws.release(); e->s_dmu.release();
+    for (cudaEvent_t ev : e->ev_pool) cudaEventDestroy(ev);
     delete e;
 }
 
@@ -455,6 +521,27 @@ int pdrt_get_work(pdrt_engine *e, pdrt_work *w)
     w->conv_items = wc.items; w->support_voxels = wc.support_vox; w->footprint_voxels = wc.footprint_vox;
     w->region_voxels = wc.region_vox; w->conv_macs = e->last_backward ? wc.macs_adj : wc.macs_fwd;
     w->kernel_size = e->P.K; w->kernel_size_compiled = e->P.KT;
+    return PDRT_OK;
+}
+
+int pdrt_set_profiling(pdrt_engine *e, int32_t enable)
+{
+    if (!e) return fail(nullptr, PDRT_EINVAL, "null engine");
+    e->profiling = enable != 0;
+    return PDRT_OK;
+}
+
+int pdrt_get_stage_ms(pdrt_engine *e, float *ms, int32_t *launches)
+{
+    if (!e || !ms || !launches) return fail(e, PDRT_EINVAL, "null argument");
+    CU(e, cudaSetDevice(e->device));
+    CU(e, cudaStreamSynchronize(e->last_stream));
+    for (int q = 0; q < PDRT_N_STAGES; ++q) { ms[q] = 0.f; launches[q] = e->launches[q]; }
+    for (const pdrt_engine::StageRec &r : e->recs) {
+        float t = 0.f;
+        CU(e, cudaEventElapsedTime(&t, r.a, r.b));
+        ms[r.stage] += t;
+    }
     return PDRT_OK;
 }
 
@@ -552,7 +639,7 @@ int pdrt_stage_beam_dose(pdrt_engine *e, const float *leaves, const float *jaws,
     cudaStream_t st = (cudaStream_t)stream;
     if ((rc = run_setup(e, 1, leaves, jaws, gantry, nullptr, true, st))) return rc;
     CU(e, e->bufA.ensure((size_t)e->P.stride_cp));
-    k_scan_items<<<1, 32, 0, st>>>(e->desc.p, 0, 1, e->tile_base.p, e->counters.p);
+    k_scan_items<<<1, 256, 0, st>>>(e->desc.p, 0, 1, e->tile_base.p, e->counters.p);
     CU(e, cudaGetLastError());
     if ((rc = launch_conv<false>(e, 0, 1, nullptr, e->bufA.p, st))) return rc;
     k_expand_dense<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, 0, 0, e->bufA.p, db);

@@ -77,8 +77,7 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     d.nty = (d.pv + RV - 1) / RV;
     d.ncx = (d.ntx + NTXC_MAX - 1) / NTXC_MAX;
     d.ntxc = (d.ntx + d.ncx - 1) / d.ncx;
-    const int XW = (P.KT + RU - 1 + 3) & ~3;
-    const int pitch = d.ntxc * RU + XW - RU;
+    const int pitch = conv_pitch(P.KT, d.ntxc);
     int ntyc_max = (P.tile_floats / pitch - (P.KT - 1)) / RV;
     if (ntyc_max < 1) ntyc_max = 1;
     d.ncy = (d.nty + ntyc_max - 1) / ntyc_max;
@@ -180,22 +179,54 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
 }
 
 // Exclusive prefix of the conv work items over the control points [cp0, cp0+n) and the totals.
-__global__ void k_scan_items(const CpDesc *desc, int cp0, int n, int *tile_base, WorkCounters *wc)
+// One block of 256 threads: warp-shuffle scan per 256-entry chunk with a running carry.
+__global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0, int n, int *tile_base, WorkCounters *wc)
 {
-    __shared__ long long tot[6];
-    if (threadIdx.x == 0) {
-        long long items = 0, sup = 0, fp = 0, reg = 0, mf = 0, ma = 0;
-        for (int c = 0; c < n; ++c) {
+    __shared__ int wsum[8];
+    __shared__ unsigned long long tot[5];
+    __shared__ int carry_s;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid < 5) tot[tid] = 0ull;
+    if (tid == 0) carry_s = 0;
+    __syncthreads();
+    unsigned long long acc[5] = { 0ull, 0ull, 0ull, 0ull, 0ull };
+    for (int c0 = 0; c0 < n; c0 += 256) {
+        const int c = c0 + tid;
+        int v = 0;
+        if (c < n) {
             const CpDesc &d = desc[cp0 + c];
-            tile_base[c] = (int)items;
-            items += d.n_items; sup += d.support_vox; fp += d.footprint_vox; reg += d.region_vox;
-            mf += d.macs_fwd; ma += d.macs_adj;
+            v = d.n_items;
+            acc[0] += d.support_vox; acc[1] += d.footprint_vox; acc[2] += d.region_vox; acc[3] += d.macs_fwd; acc[4] += d.macs_adj;
         }
-        tile_base[n] = (int)items;
-        tot[0] = items; tot[1] = sup; tot[2] = fp; tot[3] = reg; tot[4] = mf; tot[5] = ma;
+        int incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) wsum[warp] = incl;
+        __syncthreads();
+        int woff = 0;
+        for (int w = 0; w < warp; ++w) woff += wsum[w];
+        const int carry = carry_s;
+        if (c < n) tile_base[c] = carry + woff + incl - v;
+        __syncthreads();
+        if (tid == 255) carry_s = carry + woff + incl;
+        __syncthreads();
+    }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+        unsigned long long v = acc[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) atomicAdd(&tot[q], v);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        tile_base[n] = carry_s;
         if (cp0 == 0) { wc->items = 0; wc->support_vox = 0; wc->footprint_vox = 0; wc->region_vox = 0; wc->macs_fwd = 0; wc->macs_adj = 0; }
-        wc->items += tot[0]; wc->support_vox += tot[1]; wc->footprint_vox += tot[2];
-        wc->region_vox += tot[3]; wc->macs_fwd += tot[4]; wc->macs_adj += tot[5];
+        wc->items += carry_s; wc->support_vox += tot[0]; wc->footprint_vox += tot[1];
+        wc->region_vox += tot[2]; wc->macs_fwd += tot[3]; wc->macs_adj += tot[4];
     }
 }
 

@@ -26,7 +26,11 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, cons
 {
     __shared__ GatherCp list[GATHER_CHUNK];
     __shared__ int n_list;
-    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * GATHER_TX + tx;
+    // each warp covers an 8(x) x 4(y) patch, so that under any gantry rotation its 32 voxels land in a compact
+    // patch of the beam frame (a handful of 32-byte sectors per load instead of up to 32)
+    const int tid = threadIdx.y * GATHER_TX + threadIdx.x;
+    const int wrp = tid >> 5, lane = tid & 31;
+    const int tx = (wrp & 3) * 8 + (lane & 7), ty = (wrp >> 2) * 4 + (lane >> 3);
     const int ix = blockIdx.x * GATHER_TX + tx, iy = blockIdx.y * GATHER_TY + ty, iz = blockIdx.z;
     const float dx = P.ox + ix * P.sx - P.isox, dy = P.oy + iy * P.sy - P.isoy;
     // tile corners (for culling), relative to the isocentre
@@ -102,8 +106,9 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, cons
 }
 
 // S7.  G_b = R_b^T g in gather form: for every beam voxel of the compact region, the patient voxels of the
-// same z-slice whose bilinear stencil (as evaluated by k_gather_dose) reaches it.  Grid: (X, n_cp), grid-stride
-// over the region; writes the whole region (zeros outside the beam grid) so the conv adjoint can tile freely.
+// same z-slice whose bilinear stencil (as evaluated by k_gather_dose) reaches it.  Grid: (X, n_cp); each warp
+// strides over 8(u) x 4(w) patches of the region (compact in the patient frame under any rotation) and writes
+// the whole region (zeros outside the beam grid) so the conv adjoint can tile freely.
 __global__ void __launch_bounds__(256)
 k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ g,
                    float *__restrict__ G)
@@ -112,15 +117,21 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
     if (slot >= n_cp) return;
     const CpDesc d = desc[cp0 + slot];
     if (d.a0 > d.a1) return;
-    const long long n = (long long)d.pu * d.pv * P.Nw;
+    const int lane = threadIdx.x & 31, li = lane & 7, lk = lane >> 3;
+    const int nti = d.pu >> 3, ntk = (P.Nw + 3) >> 2;
+    const long long n_tiles = (long long)d.pv * ntk * nti;
+    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
     // half-extent, in patient indices, of the rotated unit hat of one beam voxel
     const float hx = (fabsf(d.cg) * P.du + fabsf(d.sg) * P.dw) / P.sx, hy = (fabsf(d.sg) * P.du + fabsf(d.cg) * P.dw) / P.sy;
+    // beam-index increments per patient-index step
+    const float fu_x = d.cg * P.sx / P.du, fu_y = d.sg * P.sy / P.du, fw_x = -d.sg * P.sx / P.dw, fw_y = d.cg * P.sy / P.dw;
     float *Gc = G + (size_t)slot * (size_t)P.stride_cp;
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
-        const int irel = (int)(e % d.pu);
-        const long long r = e / d.pu;
-        const int k = (int)(r % P.Nw), jrel = (int)(r / P.Nw);
-        const int i = d.ri0 + irel, j = d.rj0 + jrel;
+    for (long long wt = warp0; wt < n_tiles; wt += n_warps) {
+        const int ti = (int)(wt % nti);
+        const long long r = wt / nti;
+        const int tk = (int)(r % ntk), jrel = (int)(r / ntk);
+        const int i = d.ri0 + ti * 8 + li, k = tk * 4 + lk, j = d.rj0 + jrel;
+        if (k >= P.Nw) continue;
         float acc = 0.f;
         if (i < P.Nu) {
             const float u = (i - P.cu) * P.du, w = P.wmin + k * P.dw;
@@ -129,67 +140,90 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
             const int xa = max(0, (int)ceilf(fx - hx)), xb = min(P.nx - 1, (int)floorf(fx + hx));
             const int ya = max(0, (int)ceilf(fy - hy)), yb = min(P.ny - 1, (int)floorf(fy + hy));
             const float *gz = g + (size_t)j * P.ny * P.nx;
+            // beam-index offset of candidate (xa, ya) from this voxel, then incremental updates
+            const float dxa = P.ox + xa * P.sx - P.isox, dya = P.oy + ya * P.sy - P.isoy;
+            const float eu0 = (d.cg * dxa + d.sg * dya) / P.du + P.cu - (float)i;
+            const float ew0 = (-d.sg * dxa + d.cg * dya - P.wmin) / P.dw - (float)k;
             for (int yy = ya; yy <= yb; ++yy) {
-                const float dy = P.oy + yy * P.sy - P.isoy;
+                const float euy = eu0 + (yy - ya) * fu_y, ewy = ew0 + (yy - ya) * fw_y;
+                const float *grow = gz + (size_t)yy * P.nx;
                 for (int xx = xa; xx <= xb; ++xx) {
-                    const float dx = P.ox + xx * P.sx - P.isox;
-                    const float fu = (d.cg * dx + d.sg * dy) / P.du + P.cu;
-                    const float fw = (-d.sg * dx + d.cg * dy - P.wmin) / P.dw;
-                    const float wu = 1.f - fabsf(fu - (float)i), ww = 1.f - fabsf(fw - (float)k);
-                    if (wu > 0.f && ww > 0.f) acc = fmaf(wu * ww, __ldg(gz + (size_t)yy * P.nx + xx), acc);
+                    const float wu = 1.f - fabsf(euy + (xx - xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - xa) * fw_x);
+                    if (wu > 0.f && ww > 0.f) acc = fmaf(wu * ww, __ldg(grow + xx), acc);
                 }
             }
         }
-        Gc[e] = acc;
+        Gc[((size_t)jrel * P.Nw + k) * d.pu + (i - d.ri0)] = acc;
     }
 }
 
 // S9.  gPhimap_b[pix] = sum_k mag_k^2 sum_{voxels} weight(voxel -> pix) * H_b[voxel]  in gather form: for each
 // pixel of the fluence support bbox and each slice, the (at most 3x3) voxels of S_k whose bilinear stencil
-// reaches the pixel.  Grid: (Nvf, n_cp); block 128 = 32 pixels x 4 slice groups, reduced through shared memory.
-__global__ void __launch_bounds__(128)
+// reaches the pixel.  Grid: (ceil(Nuf*Nvf/32), n_cp); block 256 = 32 consecutive bbox pixels x 8 slice groups,
+// per-slice geometry staged once in shared memory, slice groups reduced through shared memory.
+struct SliceGeo { float mag, su, sv, iu, iv; int u0, u1, v0, v1; };   // su = mag*du/Du, iu = Du/(mag*du)
+
+constexpr int PROJ_THREADS = 256, PROJ_KG = PROJ_THREADS / 32;
+
+__global__ void __launch_bounds__(PROJ_THREADS)
 k_project_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ H,
                   float *__restrict__ gphimap)
 {
-    const int b = blockIdx.x, slot = blockIdx.y;
+    extern __shared__ float4 proj_smem4[];
+    SliceGeo *geo = reinterpret_cast<SliceGeo *>(proj_smem4);
+    __shared__ float red[PROJ_KG][32];
+    const int slot = blockIdx.y;
     if (slot >= n_cp) return;
     const int cp = cp0 + slot;
     const CpDesc d = desc[cp];
-    if (d.a0 > d.a1 || b < d.b0 || b > d.b1) return;
-    __shared__ float red[4][32];
-    const int lane = threadIdx.x & 31, kg = threadIdx.x >> 5;
+    if (d.a0 > d.a1) return;
+    const int bw = d.a1 - d.a0 + 1, npx = bw * (d.b1 - d.b0 + 1);
+    const int p0 = blockIdx.x * 32;
+    if (p0 >= npx) return;
+    const int tid = threadIdx.x, lane = tid & 31, kg = tid >> 5;
+    for (int k = tid; k < P.Nw; k += PROJ_THREADS) {
+        const SliceBox S = slice_support(P, d, k);
+        const float dist = P.sid + P.wmin + k * P.dw, mag = P.sid / dist;
+        SliceGeo q;
+        q.mag = mag; q.su = mag * P.du / P.Du; q.sv = mag * P.dv / P.Dv;
+        q.iu = P.Du / (mag * P.du); q.iv = P.Dv / (mag * P.dv);
+        q.u0 = S.u0; q.u1 = S.u1; q.v0 = S.v0; q.v1 = S.v1;
+        geo[k] = q;
+    }
+    __syncthreads();
+    const int p = p0 + lane;
+    const bool live = p < npx;
+    const int a = d.a0 + (live ? p % bw : 0), b = d.b0 + (live ? p / bw : 0);
     const float *Hc = H + (size_t)slot * (size_t)P.stride_cp;
-    float *out = gphimap + ((size_t)cp * P.Nvf + b) * P.Nuf;
-    for (int a0 = d.a0; a0 <= d.a1; a0 += 32) {
-        const int a = a0 + lane;
-        float acc = 0.f;
-        if (a <= d.a1) {
-            for (int k = kg; k < P.Nw; k += 4) {
-                const SliceBox S = slice_support(P, d, k);
-                if (box_empty(S)) continue;
-                const float dist = P.sid + P.wmin + k * P.dw, mag = P.sid / dist, inv_mag = dist / P.sid;
-                const int ilo = max(S.u0, (int)floorf((a - 1 - P.cuf) * P.Du * inv_mag / P.du + P.cu));
-                const int ihi = min(S.u1, (int)ceilf((a + 1 - P.cuf) * P.Du * inv_mag / P.du + P.cu));
-                const int jlo = max(S.v0, (int)floorf(((b - 1 - P.cvf) * P.Dv * inv_mag - P.v0) / P.dv));
-                const int jhi = min(S.v1, (int)ceilf(((b + 1 - P.cvf) * P.Dv * inv_mag - P.v0) / P.dv));
-                float s = 0.f;
-                for (int j = jlo; j <= jhi; ++j) {
-                    const float fb = mag * (P.v0 + j * P.dv) / P.Dv + P.cvf;
-                    const float wb = 1.f - fabsf(fb - (float)b);
-                    if (wb <= 0.f) continue;
-                    for (int i = ilo; i <= ihi; ++i) {
-                        const float fa = mag * ((i - P.cu) * P.du) / P.Du + P.cuf;
-                        const float wa = 1.f - fabsf(fa - (float)a);
-                        if (wa > 0.f) s = fmaf(wa * wb, __ldg(Hc + ((size_t)(j - d.rj0) * P.Nw + k) * d.pu + (i - d.ri0)), s);
-                    }
+    const float vb = P.v0 / P.dv;                       // v_j / dv = vb + j
+    float acc = 0.f;
+    if (live) {
+        for (int k = kg; k < P.Nw; k += PROJ_KG) {
+            const SliceGeo q = geo[k];
+            if (q.u0 > q.u1 || q.v0 > q.v1) continue;
+            // voxels with fa(i) in (a-1, a+1):  i - cu in ((a-1-cuf) iu, (a+1-cuf) iu)
+            const int ilo = max(q.u0, (int)floorf((a - 1 - P.cuf) * q.iu + P.cu)), ihi = min(q.u1, (int)ceilf((a + 1 - P.cuf) * q.iu + P.cu));
+            const int jlo = max(q.v0, (int)floorf((b - 1 - P.cvf) * q.iv - vb)), jhi = min(q.v1, (int)ceilf((b + 1 - P.cvf) * q.iv - vb));
+            float s = 0.f;
+            for (int j = jlo; j <= jhi; ++j) {
+                const float wb = 1.f - fabsf((vb + j) * q.sv + P.cvf - (float)b);
+                if (wb <= 0.f) continue;
+                const float *hrow = Hc + ((size_t)(j - d.rj0) * P.Nw + k) * d.pu - d.ri0;
+                for (int i = ilo; i <= ihi; ++i) {
+                    const float wa = 1.f - fabsf((i - P.cu) * q.su + P.cuf - (float)a);
+                    if (wa > 0.f) s = fmaf(wa * wb, __ldg(hrow + i), s);
                 }
-                acc = fmaf(mag * mag, s, acc);
             }
+            acc = fmaf(q.mag * q.mag, s, acc);
         }
-        red[kg][lane] = acc;
-        __syncthreads();
-        if (kg == 0 && a <= d.a1) out[a] = (red[0][lane] + red[1][lane]) + (red[2][lane] + red[3][lane]);
-        __syncthreads();
+    }
+    red[kg][lane] = acc;
+    __syncthreads();
+    if (kg == 0 && live) {
+        float s = 0.f;
+#pragma unroll
+        for (int q = 0; q < PROJ_KG; ++q) s += red[q][lane];
+        gphimap[((size_t)cp * P.Nvf + b) * P.Nuf + a] = s;
     }
 }
 

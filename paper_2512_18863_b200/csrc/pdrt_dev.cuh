@@ -17,9 +17,9 @@
 namespace pdrt {
 
 constexpr int RU = 8;              // conv outputs per thread along u
-constexpr int RV = 4;              // conv outputs per thread along v
+constexpr int RV = 2;              // conv outputs per thread along v
 constexpr int CONV_THREADS = 128;  // threads per conv block
-constexpr int NTXC_MAX = 8;        // conv chunk width in thread-tiles (64 outputs)
+constexpr int NTXC_MAX = 16;       // conv chunk width in thread-tiles (128 outputs)
 constexpr int MAX_TAPS = 64;       // largest Gaussian half-width [pixels]
 constexpr int MAX_HS = 4;          // largest number of head-scatter Gaussians
 

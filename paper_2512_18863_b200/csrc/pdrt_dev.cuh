@@ -5,21 +5,26 @@
 //   phimap, gphimap, P0, ... : [n_cp][Nvf][Nuf] float32, valid only inside the fluence support
 //                              bbox of each control point (CpDesc a0..a1, b0..b1)
 //   zrad                    : [n_cp][Nw] float32
-//   D_b / G_b / H_b         : per control point a COMPACT beam-frame block, layout [v][w][u]:
-//        index(cp; i,j,k) = cp_slot*stride_cp + ((j - rj0)*Nw + k)*pu + (i - ri0)
+//   phimapT                 : [n_cp][Nuf][Nvf] float32, the same maps with v fastest (read by the conv tile fill)
+//   gT                      : dL/dDose transposed to [ny][nx][nz] (z fastest)
+//   D_b / H_b               : per control point a COMPACT beam-frame block, layout [w][u][v], v FASTEST:
+//        index(cp; i,j,k) = cp_slot*stride_cp + (k*pu + (i - ri0))*pv + (j - rj0)
 //     covering the region [ri0, ri0+pu) x [rj0, rj0+pv) x [0, Nw) that bounds the conv footprint
-//     of that control point (jaw opening magnified per slice, dilated by blur and kernel halo).
-//     v outermost makes the (u,w) plane of one patient z-slice contiguous for the resampler.
+//     of that control point (jaw opening magnified per slice, dilated by blur and kernel halo);
+//     rj0 % 4 == 0, pv % 8 == 0, pu % RS == 0, rows / columns past the beam grid hold zeros.
+//     The gantry rotates about patient z = beam v (G1), so the bilinear weights of the
+//     beam <-> patient resampling do not depend on v: with v fastest every resampling thread computes
+//     its weights once and then streams 16-byte vectors along v.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace pdrt {
 
-constexpr int RU = 8;              // conv outputs per thread along u
-constexpr int RV = 2;              // conv outputs per thread along v
+constexpr int RF = 8;              // conv outputs per thread along v (the fast, register-window axis)
+constexpr int RS = 2;              // conv outputs per thread along u (the slow axis)
 constexpr int CONV_THREADS = 128;  // threads per conv block
-constexpr int NTXC_MAX = 16;       // conv chunk width in thread-tiles (128 outputs)
+constexpr int NTFC_MAX = 16;       // conv chunk width in thread-tiles along v (128 outputs)
 constexpr int MAX_TAPS = 64;       // largest Gaussian half-width [pixels]
 constexpr int MAX_HS = 4;          // largest number of head-scatter Gaussians
 
@@ -69,10 +74,10 @@ struct CpDesc {
     float scale;                 // cal * MU
     int a0, a1, b0, b1;          // fluence support bbox (inclusive); empty when a0 > a1
     int ja0, ja1, jb0, jb1;      // jaw bbox (pixels where Phi0 or its jaw derivative can be non-zero)
-    int ri0, rj0, pu, pv;        // compact region origin and pitch (pu % 8 == 0, ri0 % 4 == 0)
-    int ntx, nty;                // region size in RU x RV thread-tiles
-    int ncx, ncy, ntxc, ntyc;    // conv chunk grid and chunk size [thread-tiles]
-    int n_items;                 // Nw * ncx * ncy conv work items (0 when empty)
+    int ri0, rj0, pu, pv;        // compact region origin and extents (rj0 % 4 == 0, pv % 8 == 0, pu % RS == 0)
+    int ntf, nts;                // region size in thread-tiles: RF along v (fast), RS along u (slow)
+    int ncf, ncs, ntfc, ntsc;    // conv chunk grid and chunk size [thread-tiles]
+    int n_items;                 // Nw * ncf * ncs conv work items (0 when empty)
     int pad_;
     unsigned long long support_vox, footprint_vox, region_vox, macs_fwd, macs_adj;
 };
@@ -81,12 +86,12 @@ struct WorkCounters {
     long long items, support_vox, footprint_vox, region_vox, macs_fwd, macs_adj;
 };
 
-// Row pitch [floats] of the conv input tile for `nax` thread-tiles along u: the (K+7)-wide register window of
+// Row pitch [floats] of the conv input tile for `naf` thread-tiles along v: the (K+7)-wide register window of
 // the last thread-tile must fit, rounded to 8 floats so that the quad swizzle stays inside the row.
-__host__ __device__ __forceinline__ int conv_pitch(int kt, int nax)
+__host__ __device__ __forceinline__ int conv_pitch(int kt, int naf)
 {
-    const int xw = (kt + RU - 1 + 3) & ~3;
-    return (nax * RU + xw - RU + 7) & ~7;
+    const int xw = (kt + RF - 1 + 3) & ~3;
+    return (naf * RF + xw - RF + 7) & ~7;
 }
 
 struct SliceBox { int u0, u1, v0, v1; };   // inclusive voxel-index box; empty when u0 > u1 or v0 > v1
@@ -121,7 +126,7 @@ __device__ __forceinline__ SliceBox dilate(const Params &P, const SliceBox &s, i
 
 __device__ __forceinline__ size_t compact_index(const Params &P, const CpDesc &d, int slot, int i, int j, int k)
 {
-    return (size_t)slot * (size_t)P.stride_cp + ((size_t)(j - d.rj0) * P.Nw + k) * d.pu + (i - d.ri0);
+    return (size_t)slot * (size_t)P.stride_cp + ((size_t)k * d.pu + (i - d.ri0)) * d.pv + (j - d.rj0);
 }
 
 // Eq. 4: fractional overlap of [lo,hi] with the pixel centred at c, width D.

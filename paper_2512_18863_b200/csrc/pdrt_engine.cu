@@ -66,9 +66,9 @@ struct pdrt_engine {
     DevBuf<CpDesc> desc;
     DevBuf<int> tile_base;
     DevBuf<WorkCounters> counters;
-    DevBuf<float> phimap, P0, T1, T2, T3, Abuf, gphimap, zrad;
+    DevBuf<float> phimap, phimapT, P0, T1, T2, T3, Abuf, gphimap, zrad, gT;
     DevBuf<double> rho_s, Z_s;
-    DevBuf<float> bufA, bufB;         // compact beam-frame blocks: D_b / G_b and H_b
+    DevBuf<float> bufA;               // compact beam-frame blocks: D_b (forward) or H_b (backward)
     // staging for the *_host entry points
     DevBuf<float> s_leaves, s_jaws, s_gantry, s_mu, s_vol, s_dleaves, s_djaws, s_dmu;
     size_t scratch_cap_bytes = (size_t)48 << 30;
@@ -86,8 +86,8 @@ struct pdrt_engine {
 
     size_t scratch_bytes() const
     {
-        return desc.bytes() + tile_base.bytes() + phimap.bytes() + P0.bytes() + T1.bytes() + T2.bytes() + T3.bytes() +
-               Abuf.bytes() + gphimap.bytes() + zrad.bytes() + rho_s.bytes() + Z_s.bytes() + bufA.bytes() + bufB.bytes();
+        return desc.bytes() + tile_base.bytes() + phimap.bytes() + phimapT.bytes() + P0.bytes() + T1.bytes() + T2.bytes() +
+               T3.bytes() + Abuf.bytes() + gphimap.bytes() + zrad.bytes() + gT.bytes() + rho_s.bytes() + Z_s.bytes() + bufA.bytes();
     }
 };
 
@@ -188,7 +188,7 @@ int build_kernel_table(pdrt_engine *e, int k)
 }
 
 template <int KT, bool ADJ>
-int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *Gin, float *out, cudaStream_t st)
+int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *gT, float *out, cudaStream_t st)
 {
     static int per_sm = 0;                            // resident blocks per SM, queried once per variant
     const size_t smem = conv_smem_bytes(KT);
@@ -199,23 +199,23 @@ int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *Gin, float *out, 
         per_sm = n_res < 1 ? 1 : n_res;
     }
     e->conv_grid = e->sm_count * per_sm;              // persistent grid: a multiple of the SM count
-    k_conv<KT, ADJ><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->phimap.p,
-                                                             e->zrad.p, e->wtab.p, Gin, out);
+    k_conv<KT, ADJ><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->phimapT.p,
+                                                             e->zrad.p, e->wtab.p, gT, out);
     CU(e, cudaGetLastError());
     return PDRT_OK;
 }
-template <bool ADJ> int launch_conv(pdrt_engine *e, int cp0, int n, const float *Gin, float *out, cudaStream_t st)
+template <bool ADJ> int launch_conv(pdrt_engine *e, int cp0, int n, const float *gT, float *out, cudaStream_t st)
 {
     switch (e->P.KT) {
-    case 5: return launch_conv_t<5, ADJ>(e, cp0, n, Gin, out, st);
-    case 11: return launch_conv_t<11, ADJ>(e, cp0, n, Gin, out, st);
-    case 15: return launch_conv_t<15, ADJ>(e, cp0, n, Gin, out, st);
-    case 21: return launch_conv_t<21, ADJ>(e, cp0, n, Gin, out, st);
-    case 25: return launch_conv_t<25, ADJ>(e, cp0, n, Gin, out, st);
-    case 31: return launch_conv_t<31, ADJ>(e, cp0, n, Gin, out, st);
-    case 41: return launch_conv_t<41, ADJ>(e, cp0, n, Gin, out, st);
-    case 51: return launch_conv_t<51, ADJ>(e, cp0, n, Gin, out, st);
-    case 63: return launch_conv_t<63, ADJ>(e, cp0, n, Gin, out, st);
+    case 5: return launch_conv_t<5, ADJ>(e, cp0, n, gT, out, st);
+    case 11: return launch_conv_t<11, ADJ>(e, cp0, n, gT, out, st);
+    case 15: return launch_conv_t<15, ADJ>(e, cp0, n, gT, out, st);
+    case 21: return launch_conv_t<21, ADJ>(e, cp0, n, gT, out, st);
+    case 25: return launch_conv_t<25, ADJ>(e, cp0, n, gT, out, st);
+    case 31: return launch_conv_t<31, ADJ>(e, cp0, n, gT, out, st);
+    case 41: return launch_conv_t<41, ADJ>(e, cp0, n, gT, out, st);
+    case 51: return launch_conv_t<51, ADJ>(e, cp0, n, gT, out, st);
+    case 63: return launch_conv_t<63, ADJ>(e, cp0, n, gT, out, st);
     }
     return fail(e, PDRT_EINVAL, "no compiled convolution variant for this kernel size");
 }
@@ -226,7 +226,7 @@ int ensure_cp_scratch(pdrt_engine *e, int n_cp)
     CU(e, e->desc.ensure(n_cp));
     CU(e, e->tile_base.ensure((size_t)n_cp + 1));
     CU(e, e->counters.ensure(1));
-    CU(e, e->phimap.ensure(nmap)); CU(e, e->P0.ensure(nmap)); CU(e, e->T1.ensure(nmap));
+    CU(e, e->phimap.ensure(nmap)); CU(e, e->phimapT.ensure(nmap)); CU(e, e->P0.ensure(nmap)); CU(e, e->T1.ensure(nmap));
     CU(e, e->T2.ensure(nmap)); CU(e, e->Abuf.ensure(nmap));
     CU(e, e->zrad.ensure((size_t)n_cp * e->P.Nw));
     CU(e, e->rho_s.ensure((size_t)n_cp * e->P.M_ray));
@@ -262,7 +262,7 @@ int run_setup(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, 
     {
         StageTimer t(e, PDRT_STAGE_FLUENCE, st);
         k_fluence<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, gantry, mu, e->desc.p, e->P0.p, e->T1.p,
-                                               e->T2.p, e->Abuf.p, e->phimap.p);
+                                               e->T2.p, e->Abuf.p, e->phimap.p, e->phimapT.p);
     }
     CU(e, cudaGetLastError());
     if (need_depth) {
@@ -280,7 +280,7 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
     if (rc) return rc;
     const int nb = batch_size(e, n_cp, 1);
     CU(e, e->bufA.ensure((size_t)nb * e->P.stride_cp));
-    const dim3 gg((e->P.nx + GATHER_TX - 1) / GATHER_TX, (e->P.ny + GATHER_TY - 1) / GATHER_TY, e->P.nz);
+    const dim3 gg((e->P.nx + GATHER_T - 1) / GATHER_T, (e->P.ny + GATHER_T - 1) / GATHER_T, (e->P.nz + GATHER_Z - 1) / GATHER_Z);
     for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
         const int n = std::min(nb, n_cp - cp0);
         {
@@ -295,7 +295,7 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
         if (rc) return rc;
         {
             StageTimer t(e, PDRT_STAGE_GATHER, st);
-            k_gather_dose<<<gg, dim3(GATHER_TX, GATHER_TY), 0, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, dose, cp0 > 0);
+            k_gather_dose<<<gg, GATHER_THREADS, 0, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, dose, cp0 > 0);
         }
         CU(e, cudaGetLastError());
     }
@@ -312,9 +312,15 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
     const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
     CU(e, e->gphimap.ensure(nmap));
     CU(e, e->T3.ensure(nmap));
-    const int nb = batch_size(e, n_cp, 2);
+    const size_t nxy = (size_t)e->P.nx * e->P.ny;
+    CU(e, e->gT.ensure(nxy * e->P.nz));
+    {   // S7 prologue: dL/dDose with z fastest, so that the conv-adjoint tile fill streams along v
+        StageTimer t(e, PDRT_STAGE_RESAMPLE_ADJ, st);
+        k_transpose_g<<<dim3((unsigned)((nxy + 31) / 32), (e->P.nz + 31) / 32), 256, 0, st>>>((int)nxy, e->P.nz, gdose, e->gT.p);
+    }
+    CU(e, cudaGetLastError());
+    const int nb = batch_size(e, n_cp, 1);
     CU(e, e->bufA.ensure((size_t)nb * e->P.stride_cp));
-    CU(e, e->bufB.ensure((size_t)nb * e->P.stride_cp));
     for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
         const int n = std::min(nb, n_cp - cp0);
         {
@@ -323,18 +329,13 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
         }
         CU(e, cudaGetLastError());
         {
-            StageTimer t(e, PDRT_STAGE_RESAMPLE_ADJ, st);
-            k_resample_adjoint<<<dim3(48, n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, gdose, e->bufA.p);
-        }
-        CU(e, cudaGetLastError());
-        {
             StageTimer t(e, PDRT_STAGE_CONV_ADJ, st);
-            rc = launch_conv<true>(e, cp0, n, e->bufA.p, e->bufB.p, st);
+            rc = launch_conv<true>(e, cp0, n, e->gT.p, e->bufA.p, st);
         }
         if (rc) return rc;
         {
             StageTimer t(e, PDRT_STAGE_PROJECT_ADJ, st);
-            k_project_adjoint<<<dim3((e->P.Nuf * e->P.Nvf + 31) / 32, n), PROJ_THREADS, sizeof(SliceGeo) * e->P.Nw, st>>>(e->P, e->desc.p, cp0, n, e->bufB.p, e->gphimap.p);
+            k_project_adjoint<<<dim3((e->P.Nuf * e->P.Nvf + 31) / 32, n), PROJ_THREADS, sizeof(SliceGeo) * e->P.Nw, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, e->gphimap.p);
         }
         CU(e, cudaGetLastError());
     }
@@ -423,7 +424,7 @@ int pdrt_create(const pdrt_grid *grid, const float *density, const pdrt_beam_mod
     P.ray_step = m->ray_step_mm > 0 ? (double)m->ray_step_mm : 0.5 * (double)std::fmin(grid->sx, std::fmin(grid->sy, grid->sz));
     const double dmax = (double)P.sid + (double)P.wmin + (P.Nw - 1) * (double)P.dw;
     P.M_ray = (int)std::floor(dmax / P.ray_step) + 2;
-    P.stride_cp = (long long)((P.Nu + 7) / 8 * 8) * P.Nw * P.Nv;
+    P.stride_cp = (long long)(P.Nu + 4) * P.Nw * ((P.Nv + 7) / 8 * 8 + 16);   // bound of pu * Nw * pv, multiple of 8
     e->kA.assign(m->kA, m->kA + m->n_z); e->ka.assign(m->ka, m->ka + m->n_z);
     e->kB.assign(m->kB, m->kB + m->n_z); e->kb.assign(m->kb, m->kb + m->n_z);
 
@@ -478,7 +479,7 @@ void pdrt_destroy(pdrt_engine *e)
     e->density.release(); e->wtab.release(); e->pool.release(); e->desc.release(); e->tile_base.release();
     e->counters.release(); e->phimap.release(); e->P0.release(); e->T1.release(); e->T2.release(); e->T3.release();
     e->Abuf.release(); e->gphimap.release(); e->zrad.release(); e->rho_s.release(); e->Z_s.release();
-    e->bufA.release(); e->bufB.release();
+    e->bufA.release(); e->phimapT.release(); e->gT.release();
     e->s_leaves.release(); e->s_jaws.release(); e->s_gantry.release(); e->s_mu.release(); e->s_vol.release();
     e->s_dleaves.release(); e->s_djaws.release(); e->s_dmu.release();
     for (cudaEvent_t ev : e->ev_pool) cudaEventDestroy(ev);

@@ -59,8 +59,8 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     const bool empty = d.ja0 > d.ja1 || d.jb0 > d.jb1 || !(x1 <= x2) || !(y1 <= y2);
     d.a0 = max(0, d.ja0 - P.Tu_max); d.a1 = min(P.Nuf - 1, d.ja1 + P.Tu_max);
     d.b0 = max(0, d.jb0 - P.Tv_max); d.b1 = min(P.Nvf - 1, d.jb1 + P.Tv_max);
-    d.ri0 = d.rj0 = d.pu = d.pv = d.ntx = d.nty = 0;
-    d.ncx = d.ncy = d.ntxc = d.ntyc = d.n_items = 0;
+    d.ri0 = d.rj0 = d.pu = d.pv = d.ntf = d.nts = 0;
+    d.ncf = d.ncs = d.ntfc = d.ntsc = d.n_items = 0;
     d.pad_ = 0;
     d.support_vox = d.footprint_vox = d.region_vox = d.macs_fwd = d.macs_adj = 0ull;
     if (empty) { d.a0 = d.ja0 = 1; d.a1 = d.ja1 = 0; d.b0 = d.jb0 = 1; d.b1 = d.jb1 = 0; return; }
@@ -69,28 +69,28 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     const int u0 = max(0, min(s0.u0, s1.u0) - C), u1 = min(P.Nu - 1, max(s0.u1, s1.u1) + C);
     const int v0 = max(0, min(s0.v0, s1.v0) - C), v1 = min(P.Nv - 1, max(s0.v1, s1.v1) + C);
     if (u0 > u1 || v0 > v1) { d.a0 = d.ja0 = 1; d.a1 = d.ja1 = 0; d.b0 = d.jb0 = 1; d.b1 = d.jb1 = 0; return; }
-    d.ri0 = u0 & ~3;
-    d.pu = ((u1 - d.ri0 + 1) + RU - 1) / RU * RU;
-    d.rj0 = v0;
-    d.pv = v1 - v0 + 1;
-    d.ntx = d.pu / RU;
-    d.nty = (d.pv + RV - 1) / RV;
-    d.ncx = (d.ntx + NTXC_MAX - 1) / NTXC_MAX;
-    d.ntxc = (d.ntx + d.ncx - 1) / d.ncx;
-    const int pitch = conv_pitch(P.KT, d.ntxc);
-    int ntyc_max = (P.tile_floats / pitch - (P.KT - 1)) / RV;
-    if (ntyc_max < 1) ntyc_max = 1;
-    d.ncy = (d.nty + ntyc_max - 1) / ntyc_max;
-    d.ntyc = (d.nty + d.ncy - 1) / d.ncy;
-    d.n_items = P.Nw * d.ncx * d.ncy;
+    d.ri0 = u0;
+    d.pu = ((u1 - u0 + 1) + RS - 1) / RS * RS;
+    d.rj0 = v0 & ~3;
+    d.pv = ((v1 - d.rj0 + 1) + RF - 1) / RF * RF;
+    d.ntf = d.pv / RF;
+    d.nts = d.pu / RS;
+    d.ncf = (d.ntf + NTFC_MAX - 1) / NTFC_MAX;
+    d.ntfc = (d.ntf + d.ncf - 1) / d.ncf;
+    const int pitch = conv_pitch(P.KT, d.ntfc);
+    int ntsc_max = (P.tile_floats / pitch - (P.KT - 1)) / RS;
+    if (ntsc_max < 1) ntsc_max = 1;
+    d.ncs = (d.nts + ntsc_max - 1) / ntsc_max;
+    d.ntsc = (d.nts + d.ncs - 1) / d.ncs;
+    d.n_items = P.Nw * d.ncf * d.ncs;
     d.region_vox = (unsigned long long)d.pu * d.pv * P.Nw;
 }
 
-// S1.  Grid: n_cp blocks.  Scratch maps P0, T1, T2, A are [n_cp][Nvf][Nuf].
+// S1.  Grid: n_cp blocks.  Scratch maps P0, T1, T2, A are [n_cp][Nvf][Nuf]; phimapT is [n_cp][Nuf][Nvf].
 __global__ void __launch_bounds__(FLU_THREADS)
 k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, const float *__restrict__ jaws,
           const float *__restrict__ gantry_deg, const float *__restrict__ mu, CpDesc *desc,
-          float *P0, float *T1, float *T2, float *Abuf, float *phimap)
+          float *P0, float *T1, float *T2, float *Abuf, float *phimap, float *phimapT)
 {
     const int cp = blockIdx.x, tid = threadIdx.x;
     if (cp >= n_cp) return;
@@ -110,22 +110,22 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
             if (box_empty(s)) continue;
             sup += (unsigned long long)(s.u1 - s.u0 + 1) * (s.v1 - s.v0 + 1);
             fp += (unsigned long long)(f.u1 - f.u0 + 1) * (f.v1 - f.v0 + 1);
-            tf += (unsigned long long)((f.u1 - d.ri0) / RU - (f.u0 - d.ri0) / RU + 1) * ((f.v1 - d.rj0) / RV - (f.v0 - d.rj0) / RV + 1);
-            ta += (unsigned long long)((s.u1 - d.ri0) / RU - (s.u0 - d.ri0) / RU + 1) * ((s.v1 - d.rj0) / RV - (s.v0 - d.rj0) / RV + 1);
+            tf += (unsigned long long)((f.u1 - d.ri0) / RS - (f.u0 - d.ri0) / RS + 1) * ((f.v1 - d.rj0) / RF - (f.v0 - d.rj0) / RF + 1);
+            ta += (unsigned long long)((s.u1 - d.ri0) / RS - (s.u0 - d.ri0) / RS + 1) * ((s.v1 - d.rj0) / RF - (s.v0 - d.rj0) / RF + 1);
         }
         atomicAdd(&cnt[0], sup); atomicAdd(&cnt[1], fp); atomicAdd(&cnt[2], tf); atomicAdd(&cnt[3], ta);
     }
     __syncthreads();
     if (tid == 0) {
         d.support_vox = cnt[0]; d.footprint_vox = cnt[1];
-        d.macs_fwd = cnt[2] * (unsigned long long)(RU * RV * P.KT * P.KT);
-        d.macs_adj = cnt[3] * (unsigned long long)(RU * RV * P.KT * P.KT);
+        d.macs_fwd = cnt[2] * (unsigned long long)(RF * RS * P.KT * P.KT);
+        d.macs_adj = cnt[3] * (unsigned long long)(RF * RS * P.KT * P.KT);
         desc[cp] = d;
     }
     if (empty) return;
 
     const size_t mo = (size_t)cp * P.Nuf * P.Nvf;
-    float *p0 = P0 + mo, *t1 = T1 + mo, *t2 = T2 + mo, *Am = Abuf + mo, *pm = phimap + mo;
+    float *p0 = P0 + mo, *t1 = T1 + mo, *t2 = T2 + mo, *Am = Abuf + mo, *pm = phimap + mo, *pmT = phimapT + mo;
     const float *lv = leaves + (size_t)cp * 2 * P.Np, *jw = jaws + 4 * cp;
     const int bw = d.a1 - d.a0 + 1, bh = d.b1 - d.b0 + 1, npx = bw * bh;
     const float x1 = jw[0], x2 = jw[1], y1 = jw[2], y2 = jw[3];
@@ -175,6 +175,12 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
         const int a = d.a0 + p % bw, b = d.b0 + p / bw;
         const float uf = flu_u(P, a), vf = flu_v(P, b);
         pm[b * P.Nuf + a] *= oar_factor(T, sqrtf(uf * uf + vf * vf));
+    }
+    __syncthreads();
+    // the same map with v fastest, for the conv tile fill (lanes run along v there)
+    for (int p = tid; p < npx; p += FLU_THREADS) {
+        const int a = d.a0 + p / bh, b = d.b0 + p % bh;
+        pmT[a * P.Nvf + b] = pm[b * P.Nuf + a];
     }
 }
 

@@ -121,6 +121,20 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
             const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
             const float su = mag * P.du / P.Du, sv = mag / P.Dv;
             const float *pm = phimapT + (size_t)cp * P.Nuf * P.Nvf;
+            // per-column terms (v index, interpolation fraction, validity) do not depend on the row: once per item
+            int cb[MC];
+            float ctb[MC];
+#pragma unroll
+            for (int m = 0; m < MC; ++m) {
+                const int j = tv0 + lane + 32 * m;
+                const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
+                const float flb = floorf(fb);
+                const int b = (int)flb;
+                ctb[m] = fb - flb;
+                const bool jin = lane + 32 * m < pitch && j >= S.v0 && j <= S.v1;
+                const bool b0 = jin && b >= d.b0 && b <= d.b1, b1 = jin && b + 1 >= d.b0 && b + 1 <= d.b1;
+                cb[m] = (b0 || b1) ? (((b + 1) << 2) | (b0 ? 1 : 0) | (b1 ? 2 : 0)) : 0;     // b >= -1 when a flag is set
+            }
             for (int r = warp; r < rows; r += CONV_THREADS / 32) {
                 const int i = tu0 + r;
                 float *trow = tile + r * pitch;
@@ -133,22 +147,23 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                 const int a = (int)fla;
                 const float ta = fa - fla;
                 const bool a0 = a >= d.a0 && a <= d.a1, a1 = a + 1 >= d.a0 && a + 1 <= d.a1;
-                const float *pc0 = pm + a * P.Nvf, *pc1 = pc0 + P.Nvf;
-                for (int c = lane; c < pitch; c += 32) {
-                    const int j = tv0 + c;
+                const float wa0 = a0 ? 1.f - ta : 0.f, wa1 = a1 ? ta : 0.f;
+                // invalid rows of the map get weight 0 and are folded onto a valid one, so every address is readable
+                const float *pc0 = pm + (a0 ? a : a + 1) * P.Nvf, *pc1 = pm + (a1 ? a + 1 : a) * P.Nvf;
+                const bool arow = a0 || a1;
+#pragma unroll
+                for (int m = 0; m < MC; ++m) {
+                    const int c = lane + 32 * m;
                     float v = 0.f;
-                    if (j >= S.v0 && j <= S.v1) {
-                        const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
-                        const float flb = floorf(fb);
-                        const int b = (int)flb;
-                        const float tb = fb - flb;
-                        const bool b0 = b >= d.b0 && b <= d.b1, b1 = b + 1 >= d.b0 && b + 1 <= d.b1;
+                    if (arow && (cb[m] & 3)) {
+                        const int b = (cb[m] >> 2) - 1;
+                        const float tb = ctb[m];
                         float s0 = 0.f, s1 = 0.f;
-                        if (b0) s0 = (a0 ? (1.f - ta) * __ldg(pc0 + b) : 0.f) + (a1 ? ta * __ldg(pc1 + b) : 0.f);
-                        if (b1) s1 = (a0 ? (1.f - ta) * __ldg(pc0 + b + 1) : 0.f) + (a1 ? ta * __ldg(pc1 + b + 1) : 0.f);
+                        if (cb[m] & 1) s0 = wa0 * __ldg(pc0 + b) + wa1 * __ldg(pc1 + b);
+                        if (cb[m] & 2) s1 = wa0 * __ldg(pc0 + b + 1) + wa1 * __ldg(pc1 + b + 1);
                         v = m2 * ((1.f - tb) * s0 + tb * s1);
                     }
-                    trow[swz_col(c)] = v;
+                    if (c < pitch) trow[swz_col(c)] = v;
                 }
             }
         } else {
@@ -172,17 +187,44 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                     const float dxa = P.ox + xa * P.sx - P.isox, dya = P.oy + ya * P.sy - P.isoy;
                     const float eu0 = (d.cg * dxa + d.sg * dya) / P.du + P.cu - (float)i;
                     const float ew0 = (-d.sg * dxa + d.cg * dya - P.wmin) / P.dw - (float)k;
-                    for (int yy = ya; yy <= yb; ++yy) {
-                        const float euy = eu0 + (yy - ya) * fu_y, ewy = ew0 + (yy - ya) * fw_y;
-                        for (int xx = xa; xx <= xb; ++xx) {
-                            const float wu = 1.f - fabsf(euy + (xx - xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - xa) * fw_x);
-                            if (wu > 0.f && ww > 0.f) {           // warp-uniform
-                                const float wgt = wu * ww;
-                                const float *gcol = gT + ((size_t)yy * P.nx + xx) * P.nz;
+                    if (xb - xa <= 2 && yb - ya <= 2) {
+                        // usual case (beam spacing ~ patient spacing): at most 3 x 3 candidates; all weights first,
+                        // then all loads of a column batched so that their latencies overlap
+                        float wg[9];
 #pragma unroll
-                                for (int m = 0; m < MC; ++m) {
-                                    const int j = tv0 + lane + 32 * m;
-                                    if (lane + 32 * m < pitch && j >= 0 && j < P.Nv) acc[m] = fmaf(wgt, __ldg(gcol + j), acc[m]);
+                        for (int cy = 0; cy < 3; ++cy)
+#pragma unroll
+                            for (int cx = 0; cx < 3; ++cx) {
+                                const float wu = 1.f - fabsf(eu0 + cy * fu_y + cx * fu_x), ww = 1.f - fabsf(ew0 + cy * fw_y + cx * fw_x);
+                                wg[cy * 3 + cx] = (wu > 0.f && ww > 0.f && xa + cx <= xb && ya + cy <= yb) ? wu * ww : 0.f;
+                            }
+                        const float *g0 = gT + ((size_t)ya * P.nx + xa) * P.nz;
+#pragma unroll
+                        for (int m = 0; m < MC; ++m) {
+                            const int j = tv0 + lane + 32 * m;
+                            const bool jin = lane + 32 * m < pitch && j >= 0 && j < P.Nv;
+                            float v[9];
+#pragma unroll
+                            for (int cy = 0; cy < 3; ++cy)
+#pragma unroll
+                                for (int cx = 0; cx < 3; ++cx)
+                                    v[cy * 3 + cx] = (jin && wg[cy * 3 + cx] != 0.f) ? __ldg(g0 + ((size_t)cy * P.nx + cx) * P.nz + j) : 0.f;
+#pragma unroll
+                            for (int q = 0; q < 9; ++q) acc[m] = fmaf(wg[q], v[q], acc[m]);
+                        }
+                    } else {
+                        for (int yy = ya; yy <= yb; ++yy) {
+                            const float euy = eu0 + (yy - ya) * fu_y, ewy = ew0 + (yy - ya) * fw_y;
+                            for (int xx = xa; xx <= xb; ++xx) {
+                                const float wu = 1.f - fabsf(euy + (xx - xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - xa) * fw_x);
+                                if (wu > 0.f && ww > 0.f) {           // warp-uniform
+                                    const float wgt = wu * ww;
+                                    const float *gcol = gT + ((size_t)yy * P.nx + xx) * P.nz;
+#pragma unroll
+                                    for (int m = 0; m < MC; ++m) {
+                                        const int j = tv0 + lane + 32 * m;
+                                        if (lane + 32 * m < pitch && j >= 0 && j < P.Nv) acc[m] = fmaf(wgt, __ldg(gcol + j), acc[m]);
+                                    }
                                 }
                             }
                         }
@@ -204,12 +246,14 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
             for (int ii = 0; ii < RS; ++ii)
 #pragma unroll
                 for (int r = 0; r < RF; ++r) acc[ii][r] = 0.f;
-            const float *xrow = tile + (ts * RS) * pitch;
+            // forward: tile rows outside S_k hold zeros (structurally zero fluence) and are skipped
+            const int ylo = ADJ ? 0 : max(0, S.u0 - tu0 - ts * RS), yhi = ADJ ? KT + RS - 2 : min(KT + RS - 2, S.u1 - tu0 - ts * RS);
+            const float *xrow = tile + (ts * RS + ylo) * pitch;
             int xoff[NXQ];
 #pragma unroll
             for (int q = 0; q < NXQ; ++q) xoff[q] = swz_col(tf * RF + 4 * q);
 #pragma unroll 1
-            for (int y = 0; y < KT + RS - 1; ++y) {
+            for (int y = ylo; y <= yhi; ++y) {
                 float x[XW];
 #pragma unroll
                 for (int q = 0; q < NXQ; ++q) {

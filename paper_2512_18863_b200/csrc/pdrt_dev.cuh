@@ -11,7 +11,7 @@
 //        index(cp; i,j,k) = cp_slot*stride_cp + (k*pu + (i - ri0))*pv + (j - rj0)
 //     covering the region [ri0, ri0+pu) x [rj0, rj0+pv) x [0, Nw) that bounds the conv footprint
 //     of that control point (jaw opening magnified per slice, dilated by blur and kernel halo);
-//     rj0 % 4 == 0, pv % 8 == 0, pu % RS == 0, rows / columns past the beam grid hold zeros.
+//     rj0 % 8 == 0, pv % 8 == 0, pu % RS == 0, rows / columns past the beam grid hold zeros.
 //     The gantry rotates about patient z = beam v (G1), so the bilinear weights of the
 //     beam <-> patient resampling do not depend on v: with v fastest every resampling thread computes
 //     its weights once and then streams 16-byte vectors along v.
@@ -74,7 +74,7 @@ struct CpDesc {
     float scale;                 // cal * MU
     int a0, a1, b0, b1;          // fluence support bbox (inclusive); empty when a0 > a1
     int ja0, ja1, jb0, jb1;      // jaw bbox (pixels where Phi0 or its jaw derivative can be non-zero)
-    int ri0, rj0, pu, pv;        // compact region origin and extents (rj0 % 4 == 0, pv % 8 == 0, pu % RS == 0)
+    int ri0, rj0, pu, pv;        // compact region origin and extents (rj0 % 8 == 0, pv % 8 == 0, pu % RS == 0)
     int ntf, nts;                // region size in thread-tiles: RF along v (fast), RS along u (slow)
     int ncf, ncs, ntfc, ntsc;    // conv chunk grid and chunk size [thread-tiles]
     int n_items;                 // Nw * ncf * ncs conv work items (0 when empty)

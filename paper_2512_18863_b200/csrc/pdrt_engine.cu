@@ -335,7 +335,7 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
         if (rc) return rc;
         {
             StageTimer t(e, PDRT_STAGE_PROJECT_ADJ, st);
-            k_project_adjoint<<<dim3((e->P.Nuf * e->P.Nvf + 31) / 32, n), PROJ_THREADS, sizeof(SliceGeo) * e->P.Nw, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, e->gphimap.p);
+            k_project_adjoint<<<dim3(((e->P.Nuf + PROJ_A - 1) / PROJ_A) * ((e->P.Nvf + 31) / 32), n), PROJ_THREADS, sizeof(SliceGeo) * e->P.Nw, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, e->gphimap.p);
         }
         CU(e, cudaGetLastError());
     }

@@ -71,7 +71,7 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     if (u0 > u1 || v0 > v1) { d.a0 = d.ja0 = 1; d.a1 = d.ja1 = 0; d.b0 = d.jb0 = 1; d.b1 = d.jb1 = 0; return; }
     d.ri0 = u0;
     d.pu = ((u1 - u0 + 1) + RS - 1) / RS * RS;
-    d.rj0 = v0 & ~3;
+    d.rj0 = v0 & ~7;
     d.pv = ((v1 - d.rj0 + 1) + RF - 1) / RF * RF;
     d.ntf = d.pv / RF;
     d.nts = d.pu / RS;

@@ -9,7 +9,7 @@
 namespace pdrt {
 
 constexpr int GATHER_T = 16;            // block = 16 x 16 patient columns (x,y) ...
-constexpr int GATHER_Z = 16;            // ... times 16 z-slices per thread
+constexpr int GATHER_Z = 32;            // ... times 32 z-slices
 constexpr int GATHER_THREADS = GATHER_T * GATHER_T;
 constexpr int GATHER_CHUNK = 128;       // control points staged in shared memory per pass
 
@@ -20,14 +20,16 @@ struct GatherCp {                       // the slice of CpDesc the resampler nee
     long long base;                     // slot * stride_cp
 };
 
-// S6.  Grid: (ceil(nx/16), ceil(ny/16), ceil(nz/16)); each thread owns one patient column (x,y) and 16
-// consecutive z-slices.  The gantry rotates about z (G1), so for one control point the beam-frame
-// position (fu, fw) and the four bilinear weights are the same for all 16 voxels: they are computed once and
-// the four neighbouring beam columns are streamed as float4 along v.
+// S6.  Grid: (ceil(nx/16), ceil(ny/16), ceil(nz/32)); a block owns 16 x 16 patient columns (x,y) times 32
+// z-slices, a warp an 8(x) x 4(y) patch of columns (compact in the beam frame under any gantry rotation).
 //   dose[p] (+)= sum_b scale_b * bilinear_0(D_b[.][z][.]; fu, fw)
-// A warp first compacts, in control-point order (deterministic summation), the control points whose compact
-// region can intersect this tile.  Each warp covers an 8(x) x 4(y) patch so that under any gantry rotation
-// its 32 columns land in a compact patch of the beam frame.
+// The gantry rotates about z (G1), so for one control point the beam-frame position (fu, fw) and the
+// four bilinear weights of a column are the same for all its voxels.  Per control point each lane computes
+// them for ONE of the warp's 32 columns; the warp then walks the columns four at a time with 8 lanes along v
+// per column, taking offset and weights by warp shuffle: every load instruction reads four full 128-byte
+// lines of the v-fastest D_b block.  A lane accumulates 8 column groups x 4 z in registers over all control
+// points (in control-point order: deterministic) and every patient voxel is written exactly once.
+// Warp 0 first compacts the control points whose compact region can intersect this block.
 __global__ void __launch_bounds__(GATHER_THREADS)
 k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ D,
               float *__restrict__ dose, int accumulate)
@@ -36,16 +38,19 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, cons
     __shared__ int n_list;
     const int tid = threadIdx.x;
     const int wrp = tid >> 5, lane = tid & 31;
-    const int tx = (wrp & 1) * 8 + (lane & 7), ty = (wrp >> 1) * 4 + (lane >> 3);
-    const int ix = blockIdx.x * GATHER_T + tx, iy = blockIdx.y * GATHER_T + ty, z0 = blockIdx.z * GATHER_Z;
+    const int px0 = blockIdx.x * GATHER_T + (wrp & 1) * 8, py0 = blockIdx.y * GATHER_T + (wrp >> 1) * 4;
+    const int z0 = blockIdx.z * GATHER_Z;
+    // the column this lane sets up
+    const int ix = px0 + (lane & 7), iy = py0 + (lane >> 3);
     const float dx = P.ox + ix * P.sx - P.isox, dy = P.oy + iy * P.sy - P.isoy;
+    const bool inside = ix < P.nx && iy < P.ny;
     // tile corners (for culling), relative to the isocentre
     const float cx0 = P.ox + (blockIdx.x * GATHER_T) * P.sx - P.isox, cx1 = cx0 + (GATHER_T - 1) * P.sx;
     const float cy0 = P.oy + (blockIdx.y * GATHER_T) * P.sy - P.isoy, cy1 = cy0 + (GATHER_T - 1) * P.sy;
-    const bool inside = ix < P.nx && iy < P.ny;
-    float acc[GATHER_Z];
+    const int sub = lane >> 3, zl = 4 * (lane & 7);      // column within a group of four, z offset of this lane's quad
+    float4 acc[8];
 #pragma unroll
-    for (int q = 0; q < GATHER_Z; ++q) acc[q] = 0.f;
+    for (int g = 0; g < 8; ++g) acc[g] = make_float4(0.f, 0.f, 0.f, 0.f);
 
     for (int c0 = 0; c0 < n_cp; c0 += GATHER_CHUNK) {
         __syncthreads();
@@ -80,7 +85,6 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, cons
             if (tid == 0) n_list = count;
         }
         __syncthreads();
-        if (!inside) continue;
         const int n = n_list;
         for (int q = 0; q < n; ++q) {
             const GatherCp g = list[q];
@@ -93,48 +97,66 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, cons
             const int ihi = min(P.Nu, g.ri0 + g.pu);
             const bool iv0 = i0 >= g.ri0 && i0 < ihi, iv1 = i0 + 1 >= g.ri0 && i0 + 1 < ihi;
             const bool kv0 = k0 >= 0 && k0 < P.Nw, kv1 = k0 + 1 >= 0 && k0 + 1 < P.Nw;
-            if (!(iv0 || iv1) || !(kv0 || kv1)) continue;
-            const int zq0 = z0 - g.rj0;                              // multiple of 4 (rj0 % 4 == 0)
-            const float *p = D + g.base + ((long long)k0 * g.pu + (i0 - g.ri0)) * g.pv + zq0;
-            const long long sk = (long long)g.pu * g.pv;
-            const float w00 = g.scale * ((1.f - tu) * (1.f - tw)), w10 = g.scale * (tu * (1.f - tw));
-            const float w01 = g.scale * ((1.f - tu) * tw), w11 = g.scale * (tu * tw);
+            const bool any = inside && (iv0 || iv1) && (kv0 || kv1);
+            if (!__any_sync(0xffffffffu, any)) continue;
+            // invalid neighbours get weight 0 and are folded onto the valid one, so that every address is readable
+            const int ia = iv0 ? i0 : i0 + 1, ka = kv0 ? k0 : k0 + 1;
+            const float wu0 = iv0 ? 1.f - tu : 0.f, wu1 = iv1 ? tu : 0.f, wk0 = kv0 ? 1.f - tw : 0.f, wk1 = kv1 ? tw : 0.f;
+            int offp = 0;
+            if (any) offp = ((ka * g.pu + (ia - g.ri0)) * g.pv) | ((iv0 && iv1) ? 1 : 0) | ((kv0 && kv1) ? 2 : 0) | 4;   // pv % 8 == 0
+            const float w00 = g.scale * (wu0 * wk0), w10 = g.scale * (wu1 * wk0), w01 = g.scale * (wu0 * wk1), w11 = g.scale * (wu1 * wk1);
+            const int zq = z0 - g.rj0 + zl;                              // multiple of 4
+            const bool zok = zq >= 0 && zq + 4 <= g.pv;
+            const float *Dc = D + g.base + zq;
+            const int sk = g.pu * g.pv;
 #pragma unroll
-            for (int qd = 0; qd < GATHER_Z / 4; ++qd) {
-                const int zq = zq0 + 4 * qd;
-                if (zq < 0 || zq + 4 > g.pv) continue;               // uniform across the block
-                float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, e = a;
-                if (kv0 && iv0) a = __ldg(reinterpret_cast<const float4 *>(p + 4 * qd));
-                if (kv0 && iv1) b = __ldg(reinterpret_cast<const float4 *>(p + g.pv + 4 * qd));
-                if (kv1 && iv0) c = __ldg(reinterpret_cast<const float4 *>(p + sk + 4 * qd));
-                if (kv1 && iv1) e = __ldg(reinterpret_cast<const float4 *>(p + sk + g.pv + 4 * qd));
-                acc[4 * qd + 0] += w00 * a.x + w10 * b.x + w01 * c.x + w11 * e.x;
-                acc[4 * qd + 1] += w00 * a.y + w10 * b.y + w01 * c.y + w11 * e.y;
-                acc[4 * qd + 2] += w00 * a.z + w10 * b.z + w01 * c.z + w11 * e.z;
-                acc[4 * qd + 3] += w00 * a.w + w10 * b.w + w01 * c.w + w11 * e.w;
+            for (int gq = 0; gq < 8; ++gq) {
+                const int src = 4 * gq + sub;
+                const int o = __shfl_sync(0xffffffffu, offp, src);
+                const float f00 = __shfl_sync(0xffffffffu, w00, src), f10 = __shfl_sync(0xffffffffu, w10, src);
+                const float f01 = __shfl_sync(0xffffffffu, w01, src), f11 = __shfl_sync(0xffffffffu, w11, src);
+                if ((o & 4) && zok) {
+                    const float *p = Dc + (o & ~7);
+                    const int di = (o & 1) ? g.pv : 0, dk = (o & 2) ? sk : 0;
+                    const float4 a = __ldg(reinterpret_cast<const float4 *>(p));
+                    const float4 b = __ldg(reinterpret_cast<const float4 *>(p + di));
+                    const float4 c = __ldg(reinterpret_cast<const float4 *>(p + dk));
+                    const float4 e = __ldg(reinterpret_cast<const float4 *>(p + dk + di));
+                    acc[gq].x += f00 * a.x + f10 * b.x + f01 * c.x + f11 * e.x;
+                    acc[gq].y += f00 * a.y + f10 * b.y + f01 * c.y + f11 * e.y;
+                    acc[gq].z += f00 * a.z + f10 * b.z + f01 * c.z + f11 * e.z;
+                    acc[gq].w += f00 * a.w + f10 * b.w + f01 * c.w + f11 * e.w;
+                }
             }
         }
     }
-    if (inside) {
 #pragma unroll
-        for (int q = 0; q < GATHER_Z; ++q) {
-            const int iz = z0 + q;
+    for (int gq = 0; gq < 8; ++gq) {
+        const int col = 4 * gq + sub;
+        const int ox = px0 + (col & 7), oy = py0 + (col >> 3);
+        if (ox >= P.nx || oy >= P.ny) continue;
+        const float v[4] = { acc[gq].x, acc[gq].y, acc[gq].z, acc[gq].w };
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int iz = z0 + zl + e;
             if (iz < P.nz) {
-                float *o = dose + ((size_t)iz * P.ny + iy) * P.nx + ix;
-                *o = accumulate ? *o + acc[q] : acc[q];
+                float *o = dose + ((size_t)iz * P.ny + oy) * P.nx + ox;
+                *o = accumulate ? *o + v[e] : v[e];
             }
         }
     }
 }
 
-// S9.  gPhimap_b[pix] = sum_k mag_k^2 sum_{voxels} weight(voxel -> pix) * H_b[voxel]  in gather form: for each
-// pixel of the fluence support bbox and each slice, the (at most 3x3) voxels of S_k whose bilinear stencil
-// reaches the pixel.  Grid: (ceil(Nuf*Nvf/32), n_cp); block 256 = 32 consecutive bbox pixels (running along v,
-// the contiguous axis of H_b) x 8 slice groups, per-slice geometry staged once in shared memory, slice groups
-// reduced through shared memory.
+// S9.  gPhimap_b[pix] = sum_k mag_k^2 sum_{voxels} weight(voxel -> pix) * H_b[voxel]  in gather form.  The bilinear
+// weight is separable, weight = wa(i; a, k) * wb(j; b, k), so a warp owns a tile of 8 (a) x 32 (b, lanes: the
+// contiguous axis of H_b) pixels of the fluence support bbox and, per slice, walks the few voxel rows i that reach
+// its 8 pixel columns: each lane contracts its (at most 4) voxels along v once per row, t = sum_j wb H[k][i][j]
+// (coalesced), and adds wa * t to the pixels a that row reaches.  Grid: (ceil(Nuf/8) * ceil(Nvf/32), n_cp); the
+// 8 warps of a block take the slices k = warp, warp + 8, ... of the same tile and are reduced through shared
+// memory in a fixed order (deterministic, no atomics).
 struct SliceGeo { float mag, su, sv, iu, iv; int u0, u1, v0, v1; };   // su = mag*du/Du, iu = Du/(mag*du)
 
-constexpr int PROJ_THREADS = 256, PROJ_KG = PROJ_THREADS / 32;
+constexpr int PROJ_THREADS = 256, PROJ_KG = PROJ_THREADS / 32, PROJ_A = 8;
 
 __global__ void __launch_bounds__(PROJ_THREADS)
 k_project_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ H,
@@ -142,15 +164,17 @@ k_project_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, 
 {
     extern __shared__ float4 proj_smem4[];
     SliceGeo *geo = reinterpret_cast<SliceGeo *>(proj_smem4);
-    __shared__ float red[PROJ_KG][32];
+    __shared__ float red[PROJ_KG][PROJ_A][32];
     const int slot = blockIdx.y;
     if (slot >= n_cp) return;
     const int cp = cp0 + slot;
     const CpDesc d = desc[cp];
     if (d.a0 > d.a1) return;
-    const int bh = d.b1 - d.b0 + 1, npx = bh * (d.a1 - d.a0 + 1);
-    const int p0 = blockIdx.x * 32;
-    if (p0 >= npx) return;
+    const int nag = (P.Nuf + PROJ_A - 1) / PROJ_A;
+    const int ag = blockIdx.x % nag, bg = blockIdx.x / nag;
+    const int A0 = d.a0 + ag * PROJ_A, B0 = d.b0 + bg * 32;
+    if (A0 > d.a1 || B0 > d.b1) return;
+    const int A1 = min(d.a1, A0 + PROJ_A - 1);
     const int tid = threadIdx.x, lane = tid & 31, kg = tid >> 5;
     for (int k = tid; k < P.Nw; k += PROJ_THREADS) {
         const SliceBox S = slice_support(P, d, k);
@@ -162,39 +186,46 @@ k_project_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, 
         geo[k] = q;
     }
     __syncthreads();
-    const int p = p0 + lane;
-    const bool live = p < npx;
-    const int a = d.a0 + (live ? p / bh : 0), b = d.b0 + (live ? p % bh : 0);
+    const int b = B0 + lane;
+    const bool live = b <= d.b1;
     const float *Hc = H + (size_t)slot * (size_t)P.stride_cp;
     const float vb = P.v0 / P.dv;                       // v_j / dv = vb + j
-    float acc = 0.f;
-    if (live) {
-        for (int k = kg; k < P.Nw; k += PROJ_KG) {
-            const SliceGeo q = geo[k];
-            if (q.u0 > q.u1 || q.v0 > q.v1) continue;
-            // voxels with fa(i) in (a-1, a+1):  i - cu in ((a-1-cuf) iu, (a+1-cuf) iu)
-            const int ilo = max(q.u0, (int)floorf((a - 1 - P.cuf) * q.iu + P.cu)), ihi = min(q.u1, (int)ceilf((a + 1 - P.cuf) * q.iu + P.cu));
-            const int jlo = max(q.v0, (int)floorf((b - 1 - P.cvf) * q.iv - vb)), jhi = min(q.v1, (int)ceilf((b + 1 - P.cvf) * q.iv - vb));
-            float s = 0.f;
-            for (int i = ilo; i <= ihi; ++i) {
-                const float wa = 1.f - fabsf((i - P.cu) * q.su + P.cuf - (float)a);
-                if (wa <= 0.f) continue;
-                const float *hrow = Hc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
-                for (int j = jlo; j <= jhi; ++j) {
-                    const float wb = 1.f - fabsf((vb + j) * q.sv + P.cvf - (float)b);
-                    if (wb > 0.f) s = fmaf(wa * wb, __ldg(hrow + j), s);
-                }
+    float acc[PROJ_A];
+#pragma unroll
+    for (int q = 0; q < PROJ_A; ++q) acc[q] = 0.f;
+    for (int k = kg; k < P.Nw; k += PROJ_KG) {
+        const SliceGeo q = geo[k];
+        if (q.u0 > q.u1 || q.v0 > q.v1) continue;
+        // voxels with fa(i) in (A0-1, A1+1):  i - cu in ((A0-1-cuf) iu, (A1+1-cuf) iu)
+        const int ilo = max(q.u0, (int)floorf((A0 - 1 - P.cuf) * q.iu + P.cu)), ihi = min(q.u1, (int)ceilf((A1 + 1 - P.cuf) * q.iu + P.cu));
+        int jlo = max(q.v0, (int)floorf((b - 1 - P.cvf) * q.iv - vb)), jhi = min(q.v1, (int)ceilf((b + 1 - P.cvf) * q.iv - vb));
+        if (!live) jhi = jlo - 1;
+        const float m2 = q.mag * q.mag;
+        for (int i = ilo; i <= ihi; ++i) {
+            const float *hrow = Hc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
+            float t = 0.f;
+            for (int j = jlo; j <= jhi; ++j) {
+                const float wb = 1.f - fabsf((vb + j) * q.sv + P.cvf - (float)b);
+                if (wb > 0.f) t = fmaf(wb, __ldg(hrow + j), t);
             }
-            acc = fmaf(q.mag * q.mag, s, acc);
+            t *= m2;
+            const float fa = (i - P.cu) * q.su + P.cuf - (float)A0;      // uniform across the warp
+#pragma unroll
+            for (int e = 0; e < PROJ_A; ++e) {
+                const float wa = 1.f - fabsf(fa - (float)e);
+                if (wa > 0.f) acc[e] = fmaf(wa, t, acc[e]);
+            }
         }
     }
-    red[kg][lane] = acc;
+#pragma unroll
+    for (int e = 0; e < PROJ_A; ++e) red[kg][e][lane] = acc[e];
     __syncthreads();
-    if (kg == 0 && live) {
+    {
+        const int e = tid >> 5;                          // PROJ_A == PROJ_KG: thread (e, lane) sums one pixel
         float s = 0.f;
 #pragma unroll
-        for (int q = 0; q < PROJ_KG; ++q) s += red[q][lane];
-        gphimap[((size_t)cp * P.Nvf + b) * P.Nuf + a] = s;
+        for (int q = 0; q < PROJ_KG; ++q) s += red[q][e][lane];
+        if (live && A0 + e <= A1) gphimap[((size_t)cp * P.Nvf + b) * P.Nuf + A0 + e] = s;
     }
 }
 

@@ -156,13 +156,15 @@ enum {
     PDRT_STAGE_FLUENCE = 0,      /* S1  k_fluence (+ control-point descriptors)        */
     PDRT_STAGE_DEPTH = 1,        /* S2  k_depth                                       */
     PDRT_STAGE_SCAN = 2,         /*     k_scan_items (work-item prefix, counters)     */
-    PDRT_STAGE_CONV = 3,         /* S3+S4+S5  k_conv<K,false>                         */
+    PDRT_STAGE_CONV = 3,         /* S4+S5  k_conv<K,false>                            */
     PDRT_STAGE_GATHER = 4,       /* S6  k_gather_dose                                 */
     PDRT_STAGE_RESAMPLE_ADJ = 5, /* S7  k_resample_adjoint                            */
     PDRT_STAGE_CONV_ADJ = 6,     /* S8  k_conv<K,true>                                */
     PDRT_STAGE_PROJECT_ADJ = 7,  /* S9  k_project_adjoint                             */
     PDRT_STAGE_FLUENCE_ADJ = 8,  /* S10 k_fluence_adjoint                             */
-    PDRT_N_STAGES = 9
+    PDRT_STAGE_PROJECT = 9,      /* S3  k_project                                     */
+    PDRT_STAGE_TRANSPOSE = 10,   /*     k_transpose_g (dL/dDose with z fastest)       */
+    PDRT_N_STAGES = 11
 };
 PDRT_API int pdrt_set_profiling(pdrt_engine *engine, int32_t enable);
 PDRT_API int pdrt_get_stage_ms(pdrt_engine *engine, float *ms /*[PDRT_N_STAGES]*/, int32_t *launches /*[PDRT_N_STAGES]*/);

@@ -19,7 +19,7 @@ SYMBOLS = ("pdrt_create", "pdrt_destroy", "pdrt_last_error", "pdrt_set_kernel_si
            "pdrt_dose", "pdrt_dose_backward", "pdrt_dose_host", "pdrt_dose_backward_host",
            "pdrt_stage_fluence", "pdrt_stage_depth", "pdrt_stage_beam_dose", "pdrt_stage_grad_fluence")
 
-STAGES = ("fluence", "depth", "scan", "conv", "gather", "resample_adj", "conv_adj", "project_adj", "fluence_adj")
+STAGES = ("fluence", "depth", "scan", "conv", "gather", "resample_adj", "conv_adj", "project_adj", "fluence_adj", "project", "transpose")
 
 _FP = C.POINTER(C.c_float)
 

@@ -1,16 +1,15 @@
-// pdrt_conv.cuh — S3+S4+S5 fused (forward) and S7+S8 fused (adjoint): the lateral pencil-kernel convolution.
+// pdrt_conv.cuh — S3 (divergent projection), S4+S5 (depth-indexed kernel lookup + lateral convolution),
+// S7 (transpose of the beam -> patient resampling) and S8 (convolution adjoint).
 //
 // Forward (PAPER.md:123-133 Eq. 5-6, :145-149, :151-158 Eq. 8), per control point b and slice k:
-//   Phivol(i,j) = mag^2 * bilinear_0(Phimap_b; mag u_i/Du + cuf, mag v_j/Dv + cvf),  mag = SID/(SID+w_k)
-//   W_k         = lerp of the pre-integrated table W_tab at t = z_rad(b,k)/dz
-//   D_b(i,j,k)  = sum_{dj,di} W_k[dj][di] * Phivol(i+di-c, j+dj-c)
-// The projected fluence is never materialised: it is sampled straight into the shared-memory input tile.
+//   Phivol(i,j) = mag^2 * bilinear_0(Phimap_b; mag u_i/Du + cuf, mag v_j/Dv + cvf),  mag = SID/(SID+w_k)   k_project
+//   W_k         = lerp of the pre-integrated table W_tab at t = z_rad(b,k)/dz                               k_conv
+//   D_b(i,j,k)  = sum_{dj,di} W_k[dj][di] * Phivol(i+di-c, j+dj-c)                                         k_conv
+// Adjoint: G_b = R_b^T g (k_resample_adjoint), H_b = conv of G_b with the flipped kernel, outputs on S_k only.
 //
-// Adjoint (transposes of Eq. 9 and Eq. 8): G_b = R_b^T g is never materialised either.  The gantry rotates
-// about patient z = beam v, so the bilinear weights of a beam voxel (i,k) onto the patient voxels (x,y) of
-// its rotated unit hat do not depend on v: one warp fills one tile row (fixed i, lanes along v), computes
-// the handful of weights once and streams coalesced reads of gT[y][x][v].  Then H_b = conv of G_b with the
-// flipped kernel, outputs restricted to S_k.
+// Phivol and G_b are written once, over S_k resp. F_k only, in the compact v-fastest block layout
+// (pdrt_dev.cuh); that lets the convolution stage its input tiles with cp.async (zero-filled outside the
+// source box).
 //
 // The convolution is bound by the FP32 FMA pipe (k^2 multiply-adds per 4-byte output), so the
 // kernel is organised around FFMA issue slots: each thread owns an RF x RS = 8(v) x 2(u) register tile,
@@ -38,216 +37,320 @@ __device__ __forceinline__ int find_cp(const int *__restrict__ tile_base, int n,
     return lo;
 }
 
+// 4-byte asynchronous global -> shared copy; `ok == false` writes a zero instead (no global read).
+__device__ __forceinline__ void cp_async_f32(float *dst_smem, const float *src, bool ok)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    const int n = ok ? 4 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;\n" ::"r"(d), "l"(src), "r"(n) : "memory");
+}
+// the same with shared-window addresses and an explicit source size (bytes actually read; the rest is zero-filled)
+__device__ __forceinline__ void cp_async_4(unsigned dst, const float *src, int n)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;\n" ::"r"(dst), "l"(src), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_8(unsigned dst, const float *src, int n)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+// S3.  Phivol over S_k (Eq. 5-6) into the compact block of the control point.  Grid: (X, n_cp); a warp per
+// beam row (k, i), lanes along v; the row terms (a, ta) are warp-uniform, the map is read with v fastest.
+__global__ void __launch_bounds__(256)
+k_project(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ phimapT, float *__restrict__ vol)
+{
+    const int slot = blockIdx.y;
+    if (slot >= n_cp) return;
+    const int cp = cp0 + slot;
+    const CpDesc d = desc[cp];
+    if (d.a0 > d.a1) return;
+    const int lane = threadIdx.x & 31;
+    const int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+    const float *pm = phimapT + (size_t)cp * P.Nuf * P.Nvf;
+    float *vc = vol + (size_t)slot * (size_t)P.stride_cp;
+    const int n_rows = P.Nw * d.pu;
+    for (int rr = warp0; rr < n_rows; rr += n_warps) {
+        const int k = rr / d.pu, irel = rr - k * d.pu, i = d.ri0 + irel;
+        const SliceBox S = slice_support(P, d, k);
+        if (i < S.u0 || i > S.u1 || S.v0 > S.v1) continue;
+        const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
+        const float su = mag * P.du / P.Du, sv = mag / P.Dv;
+        const float fa = (i - P.cu) * su + P.cuf;
+        const float fla = floorf(fa);
+        const int a = (int)fla;
+        const float ta = fa - fla;
+        const bool a0 = a >= d.a0 && a <= d.a1, a1 = a + 1 >= d.a0 && a + 1 <= d.a1;
+        const float wa0 = a0 ? 1.f - ta : 0.f, wa1 = a1 ? ta : 0.f;
+        // invalid rows of the map get weight 0 and are folded onto a valid one: every address is readable
+        const float *pc0 = pm + (a0 ? a : a + 1) * P.Nvf, *pc1 = pm + (a1 ? a + 1 : a) * P.Nvf;
+        float *orow = vc + (size_t)rr * d.pv - d.rj0;
+        for (int j = S.v0 + lane; j <= S.v1; j += 32) {
+            float v = 0.f;
+            if (a0 || a1) {
+                const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
+                const float flb = floorf(fb);
+                const int b = (int)flb;
+                const float tb = fb - flb;
+                const bool b0 = b >= d.b0 && b <= d.b1, b1 = b + 1 >= d.b0 && b + 1 <= d.b1;
+                float s0 = 0.f, s1 = 0.f;
+                if (b0) s0 = wa0 * __ldg(pc0 + b) + wa1 * __ldg(pc1 + b);
+                if (b1) s1 = wa0 * __ldg(pc0 + b + 1) + wa1 * __ldg(pc1 + b + 1);
+                v = m2 * ((1.f - tb) * s0 + tb * s1);
+            }
+            orow[j] = v;
+        }
+    }
+}
+
+// S7.  G_b = R_b^T g over F_k in gather form: G_b(i,j,k) = sum over the patient voxels (x,y) of slice z = j whose
+// bilinear stencil (as evaluated by k_gather_dose) reaches beam voxel (i,k), weight (1-|du|)(1-|dw|), times g.
+// The gantry rotates about patient z = beam v (G1), so the weights do not depend on v: a warp owns a beam
+// row (k, i), nine lanes compute the (at most 3 x 3) candidate weights, the warp takes them by shuffle and streams
+// coalesced reads of gT[y][x][v] (dL/dDose with z fastest, L2-resident).  Grid: (X, n_cp).
+__global__ void __launch_bounds__(256)
+k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, int C, const float *__restrict__ gT, float *__restrict__ G)
+{
+    const int slot = blockIdx.y;
+    if (slot >= n_cp) return;
+    const CpDesc d = desc[cp0 + slot];
+    if (d.a0 > d.a1) return;
+    const int lane = threadIdx.x & 31;
+    const int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+    // half-extent, in patient indices, of the rotated unit hat of one beam voxel; beam-index increments per patient step
+    const float hx = (fabsf(d.cg) * P.du + fabsf(d.sg) * P.dw) / P.sx, hy = (fabsf(d.sg) * P.du + fabsf(d.cg) * P.dw) / P.sy;
+    const float fu_x = d.cg * P.sx / P.du, fu_y = d.sg * P.sy / P.du, fw_x = -d.sg * P.sx / P.dw, fw_y = d.cg * P.sy / P.dw;
+    float *Gc = G + (size_t)slot * (size_t)P.stride_cp;
+    const int n_rows = P.Nw * d.pu;
+    const int cx = lane % 3, cy = (lane / 3) % 3;
+    for (int rr = warp0; rr < n_rows; rr += n_warps) {
+        const int k = rr / d.pu, irel = rr - k * d.pu, i = d.ri0 + irel;
+        const SliceBox F = dilate(P, slice_support(P, d, k), C);
+        if (i < F.u0 || i > F.u1 || F.v0 > F.v1) continue;
+        const float w = P.wmin + k * P.dw, u = (i - P.cu) * P.du;
+        const float fx = (P.isox + u * d.cg - w * d.sg - P.ox) / P.sx;
+        const float fy = (P.isoy + u * d.sg + w * d.cg - P.oy) / P.sy;
+        const int xa = max(0, (int)ceilf(fx - hx)), xb = min(P.nx - 1, (int)floorf(fx + hx));
+        const int ya = max(0, (int)ceilf(fy - hy)), yb = min(P.ny - 1, (int)floorf(fy + hy));
+        const float dxa = P.ox + xa * P.sx - P.isox, dya = P.oy + ya * P.sy - P.isoy;
+        const float eu0 = (d.cg * dxa + d.sg * dya) / P.du + P.cu - (float)i;
+        const float ew0 = (-d.sg * dxa + d.cg * dya - P.wmin) / P.dw - (float)k;
+        float *orow = Gc + (size_t)rr * d.pv - d.rj0;
+        if (xb - xa <= 2 && yb - ya <= 2) {
+            // usual case (beam spacing ~ patient spacing): at most 3 x 3 candidates
+            const float wu = 1.f - fabsf(eu0 + cy * fu_y + cx * fu_x), ww = 1.f - fabsf(ew0 + cy * fw_y + cx * fw_x);
+            const float wmine = (wu > 0.f && ww > 0.f && xa + cx <= xb && ya + cy <= yb) ? wu * ww : 0.f;
+            float wq[9];
+#pragma unroll
+            for (int q = 0; q < 9; ++q) wq[q] = __shfl_sync(0xffffffffu, wmine, q);
+            const float *g0 = gT + ((size_t)ya * P.nx + xa) * P.nz;
+            for (int j = F.v0 + lane; j <= F.v1; j += 32) {
+                float v[9];
+#pragma unroll
+                for (int q = 0; q < 9; ++q)        // all loads of the column first, so that their latencies overlap
+                    v[q] = wq[q] != 0.f ? __ldg(g0 + ((size_t)(q / 3) * P.nx + (q % 3)) * P.nz + j) : 0.f;
+                float acc = 0.f;
+#pragma unroll
+                for (int q = 0; q < 9; ++q) acc = fmaf(wq[q], v[q], acc);
+                orow[j] = acc;
+            }
+        } else {
+            for (int j = F.v0 + lane; j <= F.v1; j += 32) {
+                float acc = 0.f;
+                for (int yy = ya; yy <= yb; ++yy) {
+                    const float euy = eu0 + (yy - ya) * fu_y, ewy = ew0 + (yy - ya) * fw_y;
+                    for (int xx = xa; xx <= xb; ++xx) {
+                        const float wu = 1.f - fabsf(euy + (xx - xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - xa) * fw_x);
+                        if (wu > 0.f && ww > 0.f) acc = fmaf(wu * ww, __ldg(gT + ((size_t)yy * P.nx + xx) * P.nz + j), acc);
+                    }
+                }
+                orow[j] = acc;
+            }
+        }
+    }
+}
+
+// Geometry of one conv work unit (control point, slice, chunk along v, group of 32 active thread-tiles);
+// identical in every lane of the warp.
+struct ConvItem {
+    int active;                      // the unit has thread-tiles to compute
+    int zero_duty;                   // forward: this unit also zeroes the inactive thread-tiles of its slice and chunk
+    int slot, cp, k;
+    int pv, nts;
+    long long slice_off;             // slot * stride_cp + k * pu * pv  (start of the [pu][pv] slice in the compact blocks)
+    int ri0, rj0;
+    SliceBox S, B;                   // fluence support of the slice; source box of the input tile (S forward, F adjoint)
+    int ctf0, ctf1;                  // thread-tile range of the chunk along v
+    int atf0, ats0, naf, nas;        // active thread-tiles of the slice and chunk (outputs to compute)
+    int t0, n_tiles, ts_lo;          // first tile of the unit, active tiles, first tile row of the unit
+    int pitch, rows, tv0, tu0;       // input tile: row pitch, rows, input coords of tile[0][0]
+    int n0;                          // slice kernel: table node and fraction
+    float f;
+};
+
+template <int KT, bool ADJ>
+__device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
+                                               const int *__restrict__ tile_base, const float *__restrict__ zrad,
+                                               int unit, int &slot_hint, ConvItem &it)
+{
+    constexpr int C = (KT - 1) / 2;
+    while (slot_hint + 1 < n_cp && unit >= tile_base[slot_hint + 1]) ++slot_hint;   // units arrive in increasing order
+    it.slot = slot_hint;
+    it.cp = cp0 + it.slot;
+    const CpDesc d = desc[it.cp];
+    const int local = unit - tile_base[it.slot];
+    const int nuc = ADJ ? d.nuc_adj : d.nuc_fwd;
+    const int per_slice = d.ncf * nuc;
+    it.k = local / per_slice;
+    const int ch = local - it.k * per_slice;
+    const int cf = ch / nuc, c = ch - cf * nuc;
+    it.ri0 = d.ri0; it.rj0 = d.rj0; it.pv = d.pv; it.nts = d.nts;
+    it.slice_off = (long long)it.slot * P.stride_cp + (long long)it.k * d.pu * d.pv;
+    it.ctf0 = cf * d.ntfc; it.ctf1 = min(d.ntf, it.ctf0 + d.ntfc);
+    it.S = slice_support(P, d, it.k);
+    const SliceBox F = dilate(P, it.S, C);
+    it.B = ADJ ? F : it.S;
+    const SliceBox A = ADJ ? it.S : F;                            // outputs to compute
+    int atf0 = 0, atf1 = -1, ats0 = 0, ats1 = -1;
+    if (!box_empty(A)) {
+        atf0 = max(it.ctf0, (A.v0 - d.rj0) / RF); atf1 = min(it.ctf1 - 1, (A.v1 - d.rj0) / RF);
+        ats0 = (A.u0 - d.ri0) / RS; ats1 = min(d.nts - 1, (A.u1 - d.ri0) / RS);
+    }
+    const bool any = atf0 <= atf1 && ats0 <= ats1;
+    it.atf0 = atf0; it.ats0 = ats0; it.naf = any ? atf1 - atf0 + 1 : 0; it.nas = any ? ats1 - ats0 + 1 : 0;
+    it.n_tiles = it.naf * it.nas;
+    it.t0 = c * CONV_CHUNK_TILES;
+    it.active = it.t0 < it.n_tiles;
+    it.zero_duty = c == 0;
+    it.ts_lo = 0; it.pitch = 8; it.rows = 0; it.tv0 = 0; it.tu0 = 0; it.n0 = 0; it.f = 0.f;
+    if (!it.active) return;
+    it.ts_lo = it.t0 / it.naf;
+    const int ts_hi = (min(it.n_tiles, it.t0 + CONV_CHUNK_TILES) - 1) / it.naf;
+    it.pitch = conv_pitch(KT, it.naf);
+    it.rows = (ts_hi - it.ts_lo + 1) * RS + KT - 1;
+    it.tv0 = d.rj0 + atf0 * RF - C; it.tu0 = d.ri0 + (ats0 + it.ts_lo) * RS - C;
+    // S4: slice kernel = lerp of the table in radiological depth
+    const float t = zrad[(size_t)it.cp * P.Nw + it.k] / P.dz;
+    int n0 = (int)floorf(t);
+    n0 = min(max(n0, 0), P.n_z - 2);
+    it.n0 = n0;
+    it.f = fminf(fmaxf(t - n0, 0.f), 1.f);
+}
+
+// S4 + S5 (forward) / S8 (adjoint).  One WARP per block, many blocks per SM, persistent over the unit list
+// (control point, slice, chunk of <= 32 thread-tiles).  A warp owns its input tile and its copy of the slice
+// kernel in shared memory, so there is no block-level barrier anywhere: the tile streams in by cp.async
+// (zero-filled outside the source box: S_k forward, F_k adjoint) while the warp fetches and interpolates the
+// slice kernel, and the other warps resident on the SM keep the FFMA pipe busy meanwhile.  Slices are small
+// (a few hundred thread-tiles), so a block-wide tile shared through __syncthreads left the warps waiting on each
+// other for almost half of their time (profiles/); independent warps balance by construction.
 template <int KT, bool ADJ>
 __global__ void __launch_bounds__(CONV_THREADS)
 k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
-       const float *__restrict__ phimapT, const float *__restrict__ zrad, const float *__restrict__ wtab,
-       const float *__restrict__ gT, float *__restrict__ out)
+       const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
+       int *unit_counter)
 {
     constexpr int C = (KT - 1) / 2;
     constexpr int KP = (KT + 3) & ~3;                 // weight row pitch [floats]
     constexpr int XW = (KT + RF - 1 + 3) & ~3;        // register window along v [floats]
     constexpr int NXQ = XW / 4;
+    constexpr int CPL = (C % 2 == 0) ? 2 : 1;         // floats per asynchronous copy (source and tile columns share parity when C is even)
     constexpr int PMAX = (NTFC_MAX * RF + XW - RF + 7) & ~7;   // widest tile row
-    constexpr int MC = (PMAX + 31) / 32;              // tile columns per lane in the adjoint fill
+    constexpr int MC = (PMAX / CPL + 31) / 32;        // copies per lane and tile row
     extern __shared__ float4 smem4[];
-    float *Ws = reinterpret_cast<float *>(smem4);     // [KT (du)][KP (dv)]
-    float *tile = Ws + KT * KP;                       // [rows along u][pitch along v]
-    const int tid = threadIdx.x;
+    float *Ws = reinterpret_cast<float *>(smem4);     // slice kernel [KT (du)][KP (dv)]
+    float *tile = Ws + KT * KP;                       // input tile [rows (u)][pitch (v)]
+    const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
+    const int lane = threadIdx.x;
     const int total = tile_base[n_cp];
+    int slot_hint = 0;
 
-    for (int item = blockIdx.x; item < total; item += gridDim.x) {
-        const int slot = find_cp(tile_base, n_cp, item);
-        const int cp = cp0 + slot;
-        const CpDesc d = desc[cp];
-        const int local = item - tile_base[slot];
-        const int nch = d.ncf * d.ncs;
-        const int k = local / nch, ch = local - k * nch;
-        const int cs = ch / d.ncf, cf = ch - cs * d.ncf;
-        // thread-tile range of this chunk inside the region
-        const int ctf0 = cf * d.ntfc, ctf1 = min(d.ntf, ctf0 + d.ntfc);
-        const int cts0 = cs * d.ntsc, cts1 = min(d.nts, cts0 + d.ntsc);
-        const SliceBox S = slice_support(P, d, k);
-        const SliceBox F = dilate(P, S, C);
-        const SliceBox A = ADJ ? S : F;               // outputs to compute
-        int atf0 = 0, atf1 = -1, ats0 = 0, ats1 = -1;
-        if (!box_empty(A)) {
-            atf0 = max(ctf0, (A.v0 - d.rj0) / RF); atf1 = min(ctf1 - 1, (A.v1 - d.rj0) / RF);
-            ats0 = max(cts0, (A.u0 - d.ri0) / RS); ats1 = min(cts1 - 1, (A.u1 - d.ri0) / RS);
-        }
-        const bool active = atf0 <= atf1 && ats0 <= ats1;
-        float *oslice = out + (size_t)slot * (size_t)P.stride_cp + (size_t)k * d.pu * d.pv;   // [pu][pv] of slice k
-        if (!ADJ) {
+    // units are handed out by a global counter: every warp stays busy until the list is empty, whatever the unit sizes
+    for (;;) {
+        int unit = 0;
+        if (lane == 0) unit = atomicAdd(unit_counter, 1);
+        unit = __shfl_sync(0xffffffffu, unit, 0);
+        if (unit >= total) break;
+        ConvItem I;
+        conv_load_item<KT, ADJ>(P, desc, cp0, n_cp, tile_base, zrad, unit, slot_hint, I);
+        float *oslice = out + I.slice_off;             // [pu][pv] of slice k
+        if (!ADJ && I.zero_duty) {
             // the resampler reads the whole compact region: thread-tiles outside F_k hold exact zeros
-            const int cw = ctf1 - ctf0, chn = cw * (cts1 - cts0);
-            for (int t = tid; t < chn; t += CONV_THREADS) {
-                const int ts = cts0 + t / cw, tf = ctf0 + t % cw;
-                if (active && tf >= atf0 && tf <= atf1 && ts >= ats0 && ts <= ats1) continue;
+            const int cw = I.ctf1 - I.ctf0, chn = cw * I.nts;
+            for (int t = lane; t < chn; t += 32) {
+                const int ts = t / cw, tf = I.ctf0 + t % cw;
+                if (tf >= I.atf0 && tf < I.atf0 + I.naf && ts >= I.ats0 && ts < I.ats0 + I.nas) continue;
 #pragma unroll
                 for (int ii = 0; ii < RS; ++ii) {
-                    float4 *o = reinterpret_cast<float4 *>(oslice + (size_t)(ts * RS + ii) * d.pv + tf * RF);
+                    float4 *o = reinterpret_cast<float4 *>(oslice + (size_t)(ts * RS + ii) * I.pv + tf * RF);
                     o[0] = make_float4(0.f, 0.f, 0.f, 0.f);
                     o[1] = make_float4(0.f, 0.f, 0.f, 0.f);
                 }
             }
         }
-        if (!active) continue;                        // uniform across the block
-        const int naf = atf1 - atf0 + 1, nas = ats1 - ats0 + 1;
-        const int pitch = conv_pitch(KT, naf);
-        const int rows = nas * RS + KT - 1;
-        const int tv0 = d.rj0 + atf0 * RF - C, tu0 = d.ri0 + ats0 * RS - C;   // input coords of tile[0][0]
-
-        // S4: slice kernel = lerp of the table in radiological depth, stored [du][dv] (flipped for the adjoint)
-        {
-            const float t = zrad[(size_t)cp * P.Nw + k] / P.dz;
-            int n0 = (int)floorf(t);
-            n0 = min(max(n0, 0), P.n_z - 2);
-            const float f = fminf(fmaxf(t - n0, 0.f), 1.f);
-            const float *w0 = wtab + (size_t)n0 * KT * KT, *w1 = w0 + KT * KT;
-            for (int e = tid; e < KT * KP; e += CONV_THREADS) {
-                const int di = e / KP, dj = e - di * KP;
-                float v = 0.f;
-                if (dj < KT) {
-                    const int src = ADJ ? (KT - 1 - dj) * KT + (KT - 1 - di) : dj * KT + di;
-                    v = (1.f - f) * __ldg(w0 + src) + f * __ldg(w1 + src);
-                }
-                Ws[e] = v;
-            }
-        }
-        // input tile: one warp per row (fixed u index), lanes along v
-        const int warp = tid >> 5, lane = tid & 31;
-        if (!ADJ) {
-            // S3: divergent projection of the fluence map, sampled on the fly (Eq. 5-6)
-            const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
-            const float su = mag * P.du / P.Du, sv = mag / P.Dv;
-            const float *pm = phimapT + (size_t)cp * P.Nuf * P.Nvf;
-            // per-column terms (v index, interpolation fraction, validity) do not depend on the row: once per item
-            int cb[MC];
-            float ctb[MC];
+        if (!I.active) continue;                       // uniform across the warp
+        const int pitch = I.pitch;
+        {   // input tile: asynchronous copies (zero-filled outside the source box), lanes along v.  The column terms
+            // (source offset, swizzled destination, validity) are worked out once per unit, not once per row.
+            const int tv0 = I.tv0, bv0 = I.B.v0, bv1 = I.B.v1;
+            int joff[MC], cfl[MC];
+            unsigned doff[MC];
 #pragma unroll
             for (int m = 0; m < MC; ++m) {
-                const int j = tv0 + lane + 32 * m;
-                const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
-                const float flb = floorf(fb);
-                const int b = (int)flb;
-                ctb[m] = fb - flb;
-                const bool jin = lane + 32 * m < pitch && j >= S.v0 && j <= S.v1;
-                const bool b0 = jin && b >= d.b0 && b <= d.b1, b1 = jin && b + 1 >= d.b0 && b + 1 <= d.b1;
-                cb[m] = (b0 || b1) ? (((b + 1) << 2) | (b0 ? 1 : 0) | (b1 ? 2 : 0)) : 0;     // b >= -1 when a flag is set
+                const int c = CPL * (lane + 32 * m), j = tv0 + c;
+                const bool ex = c < pitch;
+                const bool v0 = ex && j >= bv0 && j <= bv1, v1 = CPL == 2 && ex && j + 1 >= bv0 && j + 1 <= bv1;
+                joff[m] = (v0 || v1) ? j - I.rj0 : 0;
+                doff[m] = 4u * (unsigned)swz_col(c);
+                cfl[m] = (ex ? 4 : 0) | (v0 ? 1 : 0) | (v1 ? 2 : 0);
             }
-            for (int r = warp; r < rows; r += CONV_THREADS / 32) {
-                const int i = tu0 + r;
-                float *trow = tile + r * pitch;
-                if (i < S.u0 || i > S.u1) {
-                    for (int c = lane; c < pitch; c += 32) trow[c] = 0.f;
-                    continue;
-                }
-                const float fa = (i - P.cu) * su + P.cuf;
-                const float fla = floorf(fa);
-                const int a = (int)fla;
-                const float ta = fa - fla;
-                const bool a0 = a >= d.a0 && a <= d.a1, a1 = a + 1 >= d.a0 && a + 1 <= d.a1;
-                const float wa0 = a0 ? 1.f - ta : 0.f, wa1 = a1 ? ta : 0.f;
-                // invalid rows of the map get weight 0 and are folded onto a valid one, so every address is readable
-                const float *pc0 = pm + (a0 ? a : a + 1) * P.Nvf, *pc1 = pm + (a1 ? a + 1 : a) * P.Nvf;
-                const bool arow = a0 || a1;
+            const float *sbase = in + I.slice_off;                         // row i of the slice at sbase + (i - ri0) * pv
+            for (int r = 0; r < I.rows; ++r) {
+                const int i = I.tu0 + r;
+                const bool rin = i >= I.B.u0 && i <= I.B.u1;
+                const float *srow = sbase + (rin ? (long long)(i - I.ri0) * I.pv : 0ll);
+                const unsigned drow = tile_s + 4u * (unsigned)(r * pitch);
 #pragma unroll
                 for (int m = 0; m < MC; ++m) {
-                    const int c = lane + 32 * m;
-                    float v = 0.f;
-                    if (arow && (cb[m] & 3)) {
-                        const int b = (cb[m] >> 2) - 1;
-                        const float tb = ctb[m];
-                        float s0 = 0.f, s1 = 0.f;
-                        if (cb[m] & 1) s0 = wa0 * __ldg(pc0 + b) + wa1 * __ldg(pc1 + b);
-                        if (cb[m] & 2) s1 = wa0 * __ldg(pc0 + b + 1) + wa1 * __ldg(pc1 + b + 1);
-                        v = m2 * ((1.f - tb) * s0 + tb * s1);
-                    }
-                    if (c < pitch) trow[swz_col(c)] = v;
-                }
-            }
-        } else {
-            // S7: G_b(i,j,k) = sum over the patient voxels (x,y) of slice z = j whose bilinear stencil reaches
-            // beam voxel (i,k), weight (1-|du|)(1-|dw|), times g — the exact transpose of k_gather_dose.
-            const float hx = (fabsf(d.cg) * P.du + fabsf(d.sg) * P.dw) / P.sx, hy = (fabsf(d.sg) * P.du + fabsf(d.cg) * P.dw) / P.sy;
-            const float fu_x = d.cg * P.sx / P.du, fu_y = d.sg * P.sy / P.du, fw_x = -d.sg * P.sx / P.dw, fw_y = d.cg * P.sy / P.dw;
-            const float w = P.wmin + k * P.dw;
-            for (int r = warp; r < rows; r += CONV_THREADS / 32) {
-                const int i = tu0 + r;
-                float *trow = tile + r * pitch;
-                float acc[MC];
-#pragma unroll
-                for (int m = 0; m < MC; ++m) acc[m] = 0.f;
-                if (i >= 0 && i < P.Nu) {
-                    const float u = (i - P.cu) * P.du;
-                    const float fx = (P.isox + u * d.cg - w * d.sg - P.ox) / P.sx;
-                    const float fy = (P.isoy + u * d.sg + w * d.cg - P.oy) / P.sy;
-                    const int xa = max(0, (int)ceilf(fx - hx)), xb = min(P.nx - 1, (int)floorf(fx + hx));
-                    const int ya = max(0, (int)ceilf(fy - hy)), yb = min(P.ny - 1, (int)floorf(fy + hy));
-                    const float dxa = P.ox + xa * P.sx - P.isox, dya = P.oy + ya * P.sy - P.isoy;
-                    const float eu0 = (d.cg * dxa + d.sg * dya) / P.du + P.cu - (float)i;
-                    const float ew0 = (-d.sg * dxa + d.cg * dya - P.wmin) / P.dw - (float)k;
-                    if (xb - xa <= 2 && yb - ya <= 2) {
-                        // usual case (beam spacing ~ patient spacing): at most 3 x 3 candidates; all weights first,
-                        // then all loads of a column batched so that their latencies overlap
-                        float wg[9];
-#pragma unroll
-                        for (int cy = 0; cy < 3; ++cy)
-#pragma unroll
-                            for (int cx = 0; cx < 3; ++cx) {
-                                const float wu = 1.f - fabsf(eu0 + cy * fu_y + cx * fu_x), ww = 1.f - fabsf(ew0 + cy * fw_y + cx * fw_x);
-                                wg[cy * 3 + cx] = (wu > 0.f && ww > 0.f && xa + cx <= xb && ya + cy <= yb) ? wu * ww : 0.f;
-                            }
-                        const float *g0 = gT + ((size_t)ya * P.nx + xa) * P.nz;
-#pragma unroll
-                        for (int m = 0; m < MC; ++m) {
-                            const int j = tv0 + lane + 32 * m;
-                            const bool jin = lane + 32 * m < pitch && j >= 0 && j < P.Nv;
-                            float v[9];
-#pragma unroll
-                            for (int cy = 0; cy < 3; ++cy)
-#pragma unroll
-                                for (int cx = 0; cx < 3; ++cx)
-                                    v[cy * 3 + cx] = (jin && wg[cy * 3 + cx] != 0.f) ? __ldg(g0 + ((size_t)cy * P.nx + cx) * P.nz + j) : 0.f;
-#pragma unroll
-                            for (int q = 0; q < 9; ++q) acc[m] = fmaf(wg[q], v[q], acc[m]);
+                    if (!(cfl[m] & 4)) continue;
+                    const int f = rin ? (cfl[m] & 3) : 0;
+                    if (CPL == 2) {
+                        if (f == 2) {                  // only the second float lies inside the box
+                            cp_async_4(drow + doff[m], srow, 0);
+                            cp_async_4(drow + doff[m] + 4u, srow + joff[m] + 1, 4);
+                        } else {
+                            cp_async_8(drow + doff[m], srow + joff[m], f == 3 ? 8 : (f == 1 ? 4 : 0));
                         }
                     } else {
-                        for (int yy = ya; yy <= yb; ++yy) {
-                            const float euy = eu0 + (yy - ya) * fu_y, ewy = ew0 + (yy - ya) * fw_y;
-                            for (int xx = xa; xx <= xb; ++xx) {
-                                const float wu = 1.f - fabsf(euy + (xx - xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - xa) * fw_x);
-                                if (wu > 0.f && ww > 0.f) {           // warp-uniform
-                                    const float wgt = wu * ww;
-                                    const float *gcol = gT + ((size_t)yy * P.nx + xx) * P.nz;
-#pragma unroll
-                                    for (int m = 0; m < MC; ++m) {
-                                        const int j = tv0 + lane + 32 * m;
-                                        if (lane + 32 * m < pitch && j >= 0 && j < P.Nv) acc[m] = fmaf(wgt, __ldg(gcol + j), acc[m]);
-                                    }
-                                }
-                            }
-                        }
+                        cp_async_4(drow + doff[m], srow + joff[m], f ? 4 : 0);
                     }
-                }
-#pragma unroll
-                for (int m = 0; m < MC; ++m) {
-                    const int c = lane + 32 * m;
-                    if (c < pitch) trow[swz_col(c)] = acc[m];
                 }
             }
         }
-        __syncthreads();
+        {   // S4: slice kernel = lerp of the table in radiological depth; the table is stored as the [du][dv] image and is
+            // point-symmetric, so forward and adjoint (flipped kernel) read the same entries
+            const float4 *w0 = reinterpret_cast<const float4 *>(wtab + (size_t)I.n0 * KT * KP), *w1 = w0 + KT * KP / 4;
+            const float f = I.f;
+            float4 *Ws4 = reinterpret_cast<float4 *>(Ws);
+            for (int e = lane; e < KT * KP / 4; e += 32) {
+                const float4 a = __ldg(w0 + e), b = __ldg(w1 + e);
+                Ws4[e] = make_float4((1.f - f) * a.x + f * b.x, (1.f - f) * a.y + f * b.y, (1.f - f) * a.z + f * b.z, (1.f - f) * a.w + f * b.w);
+            }
+        }
+        cp_async_wait_all();
+        __syncwarp();
 
-        for (int t = tid; t < naf * nas; t += CONV_THREADS) {
-            const int ts = t / naf, tf = t - ts * naf;
+        const int naf = I.naf;
+        if (I.t0 + lane < I.n_tiles) {
+            const int t = I.t0 + lane;
+            const int tsa = t / naf, tf = t - tsa * naf, ts = tsa - I.ts_lo;     // ts: tile row relative to the input tile
             float acc[RS][RF];
 #pragma unroll
             for (int ii = 0; ii < RS; ++ii)
 #pragma unroll
                 for (int r = 0; r < RF; ++r) acc[ii][r] = 0.f;
             // forward: tile rows outside S_k hold zeros (structurally zero fluence) and are skipped
-            const int ylo = ADJ ? 0 : max(0, S.u0 - tu0 - ts * RS), yhi = ADJ ? KT + RS - 2 : min(KT + RS - 2, S.u1 - tu0 - ts * RS);
+            const int ylo = ADJ ? 0 : max(0, I.S.u0 - I.tu0 - ts * RS), yhi = ADJ ? KT + RS - 2 : min(KT + RS - 2, I.S.u1 - I.tu0 - ts * RS);
             const float *xrow = tile + (ts * RS + ylo) * pitch;
             int xoff[NXQ];
 #pragma unroll
@@ -267,8 +370,8 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                         const float4 *w4 = reinterpret_cast<const float4 *>(Ws + di * KP);
 #pragma unroll
                         for (int q = 0; q < KP / 4; ++q) {
-                            const float4 wv = w4[q];
-                            const float wq[4] = { wv.x, wv.y, wv.z, wv.w };
+                            const float4 wq4 = w4[q];
+                            const float wq[4] = { wq4.x, wq4.y, wq4.z, wq4.w };
 #pragma unroll
                             for (int e = 0; e < 4; ++e) {
                                 const int dj = 4 * q + e;
@@ -284,12 +387,12 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
             }
 #pragma unroll
             for (int ii = 0; ii < RS; ++ii) {
-                float4 *o = reinterpret_cast<float4 *>(oslice + (size_t)((ats0 + ts) * RS + ii) * d.pv + (atf0 + tf) * RF);
+                float4 *o = reinterpret_cast<float4 *>(oslice + (size_t)((I.ats0 + tsa) * RS + ii) * I.pv + (I.atf0 + tf) * RF);
                 o[0] = make_float4(acc[ii][0], acc[ii][1], acc[ii][2], acc[ii][3]);
                 o[1] = make_float4(acc[ii][4], acc[ii][5], acc[ii][6], acc[ii][7]);
             }
         }
-        __syncthreads();
+        __syncwarp();                                  // the next unit overwrites the tile and the slice kernel
     }
 }
 

@@ -23,8 +23,9 @@ namespace pdrt {
 
 constexpr int RF = 8;              // conv outputs per thread along v (the fast, register-window axis)
 constexpr int RS = 2;              // conv outputs per thread along u (the slow axis)
-constexpr int CONV_THREADS = 128;  // threads per conv block
-constexpr int NTFC_MAX = 16;       // conv chunk width in thread-tiles along v (128 outputs)
+constexpr int CONV_THREADS = 32;   // the conv runs one warp per block (no block-level barriers)
+constexpr int NTFC_MAX = 8;        // conv chunk width in thread-tiles along v (64 outputs)
+constexpr int CONV_CHUNK_TILES = 32;  // thread-tiles per conv chunk: one per lane
 constexpr int MAX_TAPS = 64;       // largest Gaussian half-width [pixels]
 constexpr int MAX_HS = 4;          // largest number of head-scatter Gaussians
 
@@ -76,9 +77,9 @@ struct CpDesc {
     int ja0, ja1, jb0, jb1;      // jaw bbox (pixels where Phi0 or its jaw derivative can be non-zero)
     int ri0, rj0, pu, pv;        // compact region origin and extents (rj0 % 8 == 0, pv % 8 == 0, pu % RS == 0)
     int ntf, nts;                // region size in thread-tiles: RF along v (fast), RS along u (slow)
-    int ncf, ncs, ntfc, ntsc;    // conv chunk grid and chunk size [thread-tiles]
-    int n_items;                 // Nw * ncf * ncs conv work items (0 when empty)
-    int pad_;
+    int ncf, ntfc;               // conv chunks along v and their width [thread-tiles]
+    int nuc_fwd, nuc_adj;        // conv units (<= 32 active thread-tiles each) per slice and chunk: bound over the slices
+    int n_items, n_items_adj;    // Nw * ncf * nuc conv work units, forward / adjoint (0 when empty)
     unsigned long long support_vox, footprint_vox, region_vox, macs_fwd, macs_adj;
 };
 

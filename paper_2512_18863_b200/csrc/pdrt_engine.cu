@@ -32,7 +32,17 @@ int compiled_size(int k)
         if (kt >= k) return kt;
     return -1;
 }
-int tile_floats_for(int kt) { return kt <= 21 ? 8192 : 12288; }
+// input-tile budget of one warp: the rows spanned by 32 consecutive thread-tiles of an active area `naf` tiles wide
+int tile_floats_for(int kt)
+{
+    int best = 0;
+    for (int naf = 1; naf <= NTFC_MAX; ++naf) {
+        const int spans = std::min((CONV_CHUNK_TILES + naf - 1) / naf + 1, CONV_CHUNK_TILES);
+        best = std::max(best, conv_pitch(kt, naf) * (spans * RS + kt - 1));
+    }
+    return best;
+}
+constexpr int ROW_BLOCKS = 16;        // blocks per control point of the row-per-warp kernels (k_project, k_resample_adjoint)
 size_t conv_smem_bytes(int kt) { return sizeof(float) * ((size_t)kt * ((kt + 3) & ~3) + tile_floats_for(kt)); }
 
 template <typename T> struct DevBuf {
@@ -68,7 +78,7 @@ struct pdrt_engine {
     DevBuf<WorkCounters> counters;
     DevBuf<float> phimap, phimapT, P0, T1, T2, T3, Abuf, gphimap, zrad, gT;
     DevBuf<double> rho_s, Z_s;
-    DevBuf<float> bufA;               // compact beam-frame blocks: D_b (forward) or H_b (backward)
+    DevBuf<float> bufA, bufB;         // compact beam-frame blocks: conv output (D_b / H_b) and conv input (Phivol / G_b)
     // staging for the *_host entry points
     DevBuf<float> s_leaves, s_jaws, s_gantry, s_mu, s_vol, s_dleaves, s_djaws, s_dmu;
     size_t scratch_cap_bytes = (size_t)48 << 30;
@@ -87,7 +97,7 @@ struct pdrt_engine {
     size_t scratch_bytes() const
     {
         return desc.bytes() + tile_base.bytes() + phimap.bytes() + phimapT.bytes() + P0.bytes() + T1.bytes() + T2.bytes() +
-               T3.bytes() + Abuf.bytes() + gphimap.bytes() + zrad.bytes() + gT.bytes() + rho_s.bytes() + Z_s.bytes() + bufA.bytes();
+               T3.bytes() + Abuf.bytes() + gphimap.bytes() + zrad.bytes() + gT.bytes() + rho_s.bytes() + Z_s.bytes() + bufA.bytes() + bufB.bytes();
     }
 };
 
@@ -150,13 +160,16 @@ int gaussian_taps(double sigma, double D, std::vector<float> &g)
 
 // Pencil-kernel table (G3, G4): pixel-integrated weights of
 // K(r;z) = (A e^{-a r} + B e^{-b r}) / r  by 8x8 midpoint sub-sampling, one quadrant computed and mirrored,
-// embedded centred in the compiled KT x KT window.
+// embedded centred in the compiled KT x KT window.  Device layout: [n_z][KT (du)][KP (dv)], KP = KT rounded up to 4,
+// i.e. exactly the shared-memory image the conv kernel wants.  The table is point-symmetric (mirrored quadrant), so the
+// flipped kernel of the adjoint is the same table (R3).
 int build_kernel_table(pdrt_engine *e, int k)
 {
     const int kt = compiled_size(k);
     const int c = (k - 1) / 2, ct = (kt - 1) / 2, nz = e->P.n_z;
     const double du = e->P.du, dv = e->P.dv;
-    std::vector<float> tab((size_t)nz * kt * kt, 0.f);
+    const int kp = (kt + 3) & ~3;
+    std::vector<float> tab((size_t)nz * kt * kp, 0.f);
     std::vector<double> rad((size_t)(c + 1) * (c + 1) * 64);
     for (int qj = 0; qj <= c; ++qj)
         for (int qi = 0; qi <= c; ++qi)
@@ -173,9 +186,9 @@ int build_kernel_table(pdrt_engine *e, int k)
                 const double *r = &rad[((size_t)qj * (c + 1) + qi) * 64];
                 for (int q = 0; q < 64; ++q) s += (A * std::exp(-a * r[q]) + B * std::exp(-b * r[q])) / r[q];
                 const float w = (float)(s * du * dv / 64.0);
-                float *slice = &tab[(size_t)n * kt * kt];
-                slice[(ct + qj) * kt + (ct + qi)] = w; slice[(ct + qj) * kt + (ct - qi)] = w;
-                slice[(ct - qj) * kt + (ct + qi)] = w; slice[(ct - qj) * kt + (ct - qi)] = w;
+                float *slice = &tab[(size_t)n * kt * kp];        // [di][dj]: qi runs along u, qj along v
+                slice[(ct + qi) * kp + (ct + qj)] = w; slice[(ct + qi) * kp + (ct - qj)] = w;
+                slice[(ct - qi) * kp + (ct + qj)] = w; slice[(ct - qi) * kp + (ct - qj)] = w;
             }
     }
     CU(e, e->wtab.ensure(tab.size()));
@@ -188,7 +201,7 @@ int build_kernel_table(pdrt_engine *e, int k)
 }
 
 template <int KT, bool ADJ>
-int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *gT, float *out, cudaStream_t st)
+int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
 {
     static int per_sm = 0;                            // resident blocks per SM, queried once per variant
     const size_t smem = conv_smem_bytes(KT);
@@ -199,23 +212,23 @@ int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *gT, float *out, c
         per_sm = n_res < 1 ? 1 : n_res;
     }
     e->conv_grid = e->sm_count * per_sm;              // persistent grid: a multiple of the SM count
-    k_conv<KT, ADJ><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->phimapT.p,
-                                                             e->zrad.p, e->wtab.p, gT, out);
+    k_conv<KT, ADJ><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->zrad.p, e->wtab.p, in, out,
+                                                             e->tile_base.p + n + 1);
     CU(e, cudaGetLastError());
     return PDRT_OK;
 }
-template <bool ADJ> int launch_conv(pdrt_engine *e, int cp0, int n, const float *gT, float *out, cudaStream_t st)
+template <bool ADJ> int launch_conv(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
 {
     switch (e->P.KT) {
-    case 5: return launch_conv_t<5, ADJ>(e, cp0, n, gT, out, st);
-    case 11: return launch_conv_t<11, ADJ>(e, cp0, n, gT, out, st);
-    case 15: return launch_conv_t<15, ADJ>(e, cp0, n, gT, out, st);
-    case 21: return launch_conv_t<21, ADJ>(e, cp0, n, gT, out, st);
-    case 25: return launch_conv_t<25, ADJ>(e, cp0, n, gT, out, st);
-    case 31: return launch_conv_t<31, ADJ>(e, cp0, n, gT, out, st);
-    case 41: return launch_conv_t<41, ADJ>(e, cp0, n, gT, out, st);
-    case 51: return launch_conv_t<51, ADJ>(e, cp0, n, gT, out, st);
-    case 63: return launch_conv_t<63, ADJ>(e, cp0, n, gT, out, st);
+    case 5: return launch_conv_t<5, ADJ>(e, cp0, n, in, out, st);
+    case 11: return launch_conv_t<11, ADJ>(e, cp0, n, in, out, st);
+    case 15: return launch_conv_t<15, ADJ>(e, cp0, n, in, out, st);
+    case 21: return launch_conv_t<21, ADJ>(e, cp0, n, in, out, st);
+    case 25: return launch_conv_t<25, ADJ>(e, cp0, n, in, out, st);
+    case 31: return launch_conv_t<31, ADJ>(e, cp0, n, in, out, st);
+    case 41: return launch_conv_t<41, ADJ>(e, cp0, n, in, out, st);
+    case 51: return launch_conv_t<51, ADJ>(e, cp0, n, in, out, st);
+    case 63: return launch_conv_t<63, ADJ>(e, cp0, n, in, out, st);
     }
     return fail(e, PDRT_EINVAL, "no compiled convolution variant for this kernel size");
 }
@@ -224,7 +237,7 @@ int ensure_cp_scratch(pdrt_engine *e, int n_cp)
 {
     const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
     CU(e, e->desc.ensure(n_cp));
-    CU(e, e->tile_base.ensure((size_t)n_cp + 1));
+    CU(e, e->tile_base.ensure((size_t)n_cp + 2));     // prefix of the conv units + the unit counter of the running conv
     CU(e, e->counters.ensure(1));
     CU(e, e->phimap.ensure(nmap)); CU(e, e->phimapT.ensure(nmap)); CU(e, e->P0.ensure(nmap)); CU(e, e->T1.ensure(nmap));
     CU(e, e->T2.ensure(nmap)); CU(e, e->Abuf.ensure(nmap));
@@ -278,19 +291,25 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
 {
     int rc = run_setup(e, n_cp, leaves, jaws, gantry, mu, true, st);
     if (rc) return rc;
-    const int nb = batch_size(e, n_cp, 1);
+    const int nb = batch_size(e, n_cp, 2);
     CU(e, e->bufA.ensure((size_t)nb * e->P.stride_cp));
+    CU(e, e->bufB.ensure((size_t)nb * e->P.stride_cp));
     const dim3 gg((e->P.nx + GATHER_T - 1) / GATHER_T, (e->P.ny + GATHER_T - 1) / GATHER_T, (e->P.nz + GATHER_Z - 1) / GATHER_Z);
     for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
         const int n = std::min(nb, n_cp - cp0);
         {
             StageTimer t(e, PDRT_STAGE_SCAN, st);
-            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, e->tile_base.p, e->counters.p);
+            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, 0, e->tile_base.p, e->counters.p);
+        }
+        CU(e, cudaGetLastError());
+        {
+            StageTimer t(e, PDRT_STAGE_PROJECT, st);
+            k_project<<<dim3(ROW_BLOCKS, n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, e->phimapT.p, e->bufB.p);
         }
         CU(e, cudaGetLastError());
         {
             StageTimer t(e, PDRT_STAGE_CONV, st);
-            rc = launch_conv<false>(e, cp0, n, nullptr, e->bufA.p, st);
+            rc = launch_conv<false>(e, cp0, n, e->bufB.p, e->bufA.p, st);
         }
         if (rc) return rc;
         {
@@ -314,23 +333,29 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
     CU(e, e->T3.ensure(nmap));
     const size_t nxy = (size_t)e->P.nx * e->P.ny;
     CU(e, e->gT.ensure(nxy * e->P.nz));
-    {   // S7 prologue: dL/dDose with z fastest, so that the conv-adjoint tile fill streams along v
-        StageTimer t(e, PDRT_STAGE_RESAMPLE_ADJ, st);
+    {   // S7 prologue: dL/dDose with z fastest, so that the resampling adjoint streams along v
+        StageTimer t(e, PDRT_STAGE_TRANSPOSE, st);
         k_transpose_g<<<dim3((unsigned)((nxy + 31) / 32), (e->P.nz + 31) / 32), 256, 0, st>>>((int)nxy, e->P.nz, gdose, e->gT.p);
     }
     CU(e, cudaGetLastError());
-    const int nb = batch_size(e, n_cp, 1);
+    const int nb = batch_size(e, n_cp, 2);
     CU(e, e->bufA.ensure((size_t)nb * e->P.stride_cp));
+    CU(e, e->bufB.ensure((size_t)nb * e->P.stride_cp));
     for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
         const int n = std::min(nb, n_cp - cp0);
         {
             StageTimer t(e, PDRT_STAGE_SCAN, st);
-            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, e->tile_base.p, e->counters.p);
+            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, 1, e->tile_base.p, e->counters.p);
+        }
+        CU(e, cudaGetLastError());
+        {
+            StageTimer t(e, PDRT_STAGE_RESAMPLE_ADJ, st);
+            k_resample_adjoint<<<dim3(ROW_BLOCKS, n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, (e->P.KT - 1) / 2, e->gT.p, e->bufB.p);
         }
         CU(e, cudaGetLastError());
         {
             StageTimer t(e, PDRT_STAGE_CONV_ADJ, st);
-            rc = launch_conv<true>(e, cp0, n, e->gT.p, e->bufA.p, st);
+            rc = launch_conv<true>(e, cp0, n, e->bufB.p, e->bufA.p, st);
         }
         if (rc) return rc;
         {
@@ -479,7 +504,7 @@ void pdrt_destroy(pdrt_engine *e)
     e->density.release(); e->wtab.release(); e->pool.release(); e->desc.release(); e->tile_base.release();
     e->counters.release(); e->phimap.release(); e->P0.release(); e->T1.release(); e->T2.release(); e->T3.release();
     e->Abuf.release(); e->gphimap.release(); e->zrad.release(); e->rho_s.release(); e->Z_s.release();
-    e->bufA.release(); e->phimapT.release(); e->gT.release();
+    e->bufA.release(); e->bufB.release(); e->phimapT.release(); e->gT.release();
     e->s_leaves.release(); e->s_jaws.release(); e->s_gantry.release(); e->s_mu.release(); e->s_vol.release();
     e->s_dleaves.release(); e->s_djaws.release(); e->s_dmu.release();
     for (cudaEvent_t ev : e->ev_pool) cudaEventDestroy(ev);
@@ -640,9 +665,12 @@ int pdrt_stage_beam_dose(pdrt_engine *e, const float *leaves, const float *jaws,
     cudaStream_t st = (cudaStream_t)stream;
     if ((rc = run_setup(e, 1, leaves, jaws, gantry, nullptr, true, st))) return rc;
     CU(e, e->bufA.ensure((size_t)e->P.stride_cp));
-    k_scan_items<<<1, 256, 0, st>>>(e->desc.p, 0, 1, e->tile_base.p, e->counters.p);
+    CU(e, e->bufB.ensure((size_t)e->P.stride_cp));
+    k_scan_items<<<1, 256, 0, st>>>(e->desc.p, 0, 1, 0, e->tile_base.p, e->counters.p);
     CU(e, cudaGetLastError());
-    if ((rc = launch_conv<false>(e, 0, 1, nullptr, e->bufA.p, st))) return rc;
+    k_project<<<dim3(ROW_BLOCKS, 1), 256, 0, st>>>(e->P, e->desc.p, 0, 1, e->phimapT.p, e->bufB.p);
+    CU(e, cudaGetLastError());
+    if ((rc = launch_conv<false>(e, 0, 1, e->bufB.p, e->bufA.p, st))) return rc;
     k_expand_dense<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, 0, 0, e->bufA.p, db);
     CU(e, cudaGetLastError());
     return PDRT_OK;

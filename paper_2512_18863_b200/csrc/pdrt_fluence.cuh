@@ -60,8 +60,7 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     d.a0 = max(0, d.ja0 - P.Tu_max); d.a1 = min(P.Nuf - 1, d.ja1 + P.Tu_max);
     d.b0 = max(0, d.jb0 - P.Tv_max); d.b1 = min(P.Nvf - 1, d.jb1 + P.Tv_max);
     d.ri0 = d.rj0 = d.pu = d.pv = d.ntf = d.nts = 0;
-    d.ncf = d.ncs = d.ntfc = d.ntsc = d.n_items = 0;
-    d.pad_ = 0;
+    d.ncf = d.ntfc = d.nuc_fwd = d.nuc_adj = d.n_items = d.n_items_adj = 0;
     d.support_vox = d.footprint_vox = d.region_vox = d.macs_fwd = d.macs_adj = 0ull;
     if (empty) { d.a0 = d.ja0 = 1; d.a1 = d.ja1 = 0; d.b0 = d.jb0 = 1; d.b1 = d.jb1 = 0; return; }
     const int C = (P.KT - 1) / 2;
@@ -77,12 +76,15 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     d.nts = d.pu / RS;
     d.ncf = (d.ntf + NTFC_MAX - 1) / NTFC_MAX;
     d.ntfc = (d.ntf + d.ncf - 1) / d.ncf;
-    const int pitch = conv_pitch(P.KT, d.ntfc);
-    int ntsc_max = (P.tile_floats / pitch - (P.KT - 1)) / RS;
-    if (ntsc_max < 1) ntsc_max = 1;
-    d.ncs = (d.nts + ntsc_max - 1) / ntsc_max;
-    d.ntsc = (d.nts + d.ncs - 1) / d.ncs;
-    d.n_items = P.Nw * d.ncf * d.ncs;
+    // units: the active thread-tiles of a slice (F_k forward, S_k adjoint; both grow monotonically with k) in row-major
+    // order, 32 at a time; the count per slice is bounded by the larger of the two end slices
+    const SliceBox f0 = dilate(P, s0, C), f1 = dilate(P, s1, C);
+    const int nsf = max((f0.u1 - d.ri0) / RS - (f0.u0 - d.ri0) / RS, (f1.u1 - d.ri0) / RS - (f1.u0 - d.ri0) / RS) + 1;
+    const int nsa = max((s0.u1 - d.ri0) / RS - (s0.u0 - d.ri0) / RS, (s1.u1 - d.ri0) / RS - (s1.u0 - d.ri0) / RS) + 1;
+    d.nuc_fwd = (d.ntfc * nsf + CONV_CHUNK_TILES - 1) / CONV_CHUNK_TILES;
+    d.nuc_adj = (d.ntfc * nsa + CONV_CHUNK_TILES - 1) / CONV_CHUNK_TILES;
+    d.n_items = P.Nw * d.ncf * d.nuc_fwd;
+    d.n_items_adj = P.Nw * d.ncf * d.nuc_adj;
     d.region_vox = (unsigned long long)d.pu * d.pv * P.Nw;
 }
 
@@ -186,7 +188,7 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
 
 // Exclusive prefix of the conv work items over the control points [cp0, cp0+n) and the totals.
 // One block of 256 threads: warp-shuffle scan per 256-entry chunk with a running carry.
-__global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0, int n, int *tile_base, WorkCounters *wc)
+__global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0, int n, int adjoint, int *tile_base, WorkCounters *wc)
 {
     __shared__ int wsum[8];
     __shared__ unsigned long long tot[5];
@@ -201,7 +203,7 @@ __global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0,
         int v = 0;
         if (c < n) {
             const CpDesc &d = desc[cp0 + c];
-            v = d.n_items;
+            v = adjoint ? d.n_items_adj : d.n_items;
             acc[0] += d.support_vox; acc[1] += d.footprint_vox; acc[2] += d.region_vox; acc[3] += d.macs_fwd; acc[4] += d.macs_adj;
         }
         int incl = v;
@@ -230,6 +232,7 @@ __global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0,
     __syncthreads();
     if (tid == 0) {
         tile_base[n] = carry_s;
+        tile_base[n + 1] = 0;           // unit counter of the conv launch that follows
         if (cp0 == 0) { wc->items = 0; wc->support_vox = 0; wc->footprint_vox = 0; wc->region_vox = 0; wc->macs_fwd = 0; wc->macs_adj = 0; }
         wc->items += carry_s; wc->support_vox += tot[0]; wc->footprint_vox += tot[1];
         wc->region_vox += tot[2]; wc->macs_fwd += tot[3]; wc->macs_adj += tot[4];

@@ -55,8 +55,11 @@ __device__ __forceinline__ void cp_async_8(unsigned dst, const float *src, int n
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
-// S3.  Phivol over S_k (Eq. 5-6) into the compact block of the control point.  Grid: (X, n_cp); a warp per
-// beam row (k, i), lanes along v; the row terms (a, ta) are warp-uniform, the map is read with v fastest.
+constexpr int ROW_GROUPS = 4;       // k_project / k_resample_adjoint: a warp takes every 4th row of one slice
+
+// S3.  Phivol over S_k (Eq. 5-6) into the compact block of the control point.  Grid: (X, n_cp); a warp per slice
+// and row group, lanes along v; the slice terms (box, magnification) and the row terms (a, ta) are warp-uniform,
+// the map is read with v fastest.
 __global__ void __launch_bounds__(256)
 k_project(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ phimapT, float *__restrict__ vol)
 {
@@ -69,36 +72,35 @@ k_project(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const fl
     const int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
     const float *pm = phimapT + (size_t)cp * P.Nuf * P.Nvf;
     float *vc = vol + (size_t)slot * (size_t)P.stride_cp;
-    const int n_rows = P.Nw * d.pu;
-    for (int rr = warp0; rr < n_rows; rr += n_warps) {
-        const int k = rr / d.pu, irel = rr - k * d.pu, i = d.ri0 + irel;
+    for (int q = warp0; q < P.Nw * ROW_GROUPS; q += n_warps) {
+        const int k = q / ROW_GROUPS, g = q - k * ROW_GROUPS;
         const SliceBox S = slice_support(P, d, k);
-        if (i < S.u0 || i > S.u1 || S.v0 > S.v1) continue;
+        if (box_empty(S)) continue;
         const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
         const float su = mag * P.du / P.Du, sv = mag / P.Dv;
-        const float fa = (i - P.cu) * su + P.cuf;
-        const float fla = floorf(fa);
-        const int a = (int)fla;
-        const float ta = fa - fla;
-        const bool a0 = a >= d.a0 && a <= d.a1, a1 = a + 1 >= d.a0 && a + 1 <= d.a1;
-        const float wa0 = a0 ? 1.f - ta : 0.f, wa1 = a1 ? ta : 0.f;
-        // invalid rows of the map get weight 0 and are folded onto a valid one: every address is readable
-        const float *pc0 = pm + (a0 ? a : a + 1) * P.Nvf, *pc1 = pm + (a1 ? a + 1 : a) * P.Nvf;
-        float *orow = vc + (size_t)rr * d.pv - d.rj0;
-        for (int j = S.v0 + lane; j <= S.v1; j += 32) {
-            float v = 0.f;
-            if (a0 || a1) {
-                const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
-                const float flb = floorf(fb);
-                const int b = (int)flb;
-                const float tb = fb - flb;
-                const bool b0 = b >= d.b0 && b <= d.b1, b1 = b + 1 >= d.b0 && b + 1 <= d.b1;
+        // column terms of this lane (two passes cover 64 columns; wider supports loop)
+        for (int j0 = S.v0; j0 <= S.v1; j0 += 32) {
+            const int j = j0 + lane;
+            const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
+            const float flb = floorf(fb);
+            const int b = (int)flb;
+            const float tb = fb - flb;
+            const bool jin = j <= S.v1;
+            const bool b0 = jin && b >= d.b0 && b <= d.b1, b1 = jin && b + 1 >= d.b0 && b + 1 <= d.b1;
+            for (int i = S.u0 + g; i <= S.u1; i += ROW_GROUPS) {
+                const float fa = (i - P.cu) * su + P.cuf;
+                const float fla = floorf(fa);
+                const int a = (int)fla;
+                const float ta = fa - fla;
+                const bool a0 = a >= d.a0 && a <= d.a1, a1 = a + 1 >= d.a0 && a + 1 <= d.a1;
+                const float wa0 = a0 ? 1.f - ta : 0.f, wa1 = a1 ? ta : 0.f;
+                // invalid rows of the map get weight 0 and are folded onto a valid one: every address is readable
+                const float *pc0 = pm + (a0 ? a : a + 1) * P.Nvf, *pc1 = pm + (a1 ? a + 1 : a) * P.Nvf;
                 float s0 = 0.f, s1 = 0.f;
-                if (b0) s0 = wa0 * __ldg(pc0 + b) + wa1 * __ldg(pc1 + b);
-                if (b1) s1 = wa0 * __ldg(pc0 + b + 1) + wa1 * __ldg(pc1 + b + 1);
-                v = m2 * ((1.f - tb) * s0 + tb * s1);
+                if ((a0 || a1) && b0) s0 = wa0 * __ldg(pc0 + b) + wa1 * __ldg(pc1 + b);
+                if ((a0 || a1) && b1) s1 = wa0 * __ldg(pc0 + b + 1) + wa1 * __ldg(pc1 + b + 1);
+                if (jin) vc[((size_t)k * d.pu + (i - d.ri0)) * d.pv + (j - d.rj0)] = m2 * ((1.f - tb) * s0 + tb * s1);
             }
-            orow[j] = v;
         }
     }
 }
@@ -107,7 +109,8 @@ k_project(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const fl
 // bilinear stencil (as evaluated by k_gather_dose) reaches beam voxel (i,k), weight (1-|du|)(1-|dw|), times g.
 // The gantry rotates about patient z = beam v (G1), so the weights do not depend on v: a warp owns a beam
 // row (k, i), nine lanes compute the (at most 3 x 3) candidate weights, the warp takes them by shuffle and streams
-// coalesced reads of gT[y][x][v] (dL/dDose with z fastest, L2-resident).  Grid: (X, n_cp).
+// coalesced reads of gT[y][x][v] (dL/dDose with z fastest, L2-resident), two v per lane when nz is even.
+// Grid: (X, n_cp); a warp per slice and row group.
 __global__ void __launch_bounds__(256)
 k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, int C, const float *__restrict__ gT, float *__restrict__ G)
 {
@@ -121,50 +124,67 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
     const float hx = (fabsf(d.cg) * P.du + fabsf(d.sg) * P.dw) / P.sx, hy = (fabsf(d.sg) * P.du + fabsf(d.cg) * P.dw) / P.sy;
     const float fu_x = d.cg * P.sx / P.du, fu_y = d.sg * P.sy / P.du, fw_x = -d.sg * P.sx / P.dw, fw_y = d.cg * P.sy / P.dw;
     float *Gc = G + (size_t)slot * (size_t)P.stride_cp;
-    const int n_rows = P.Nw * d.pu;
     const int cx = lane % 3, cy = (lane / 3) % 3;
-    for (int rr = warp0; rr < n_rows; rr += n_warps) {
-        const int k = rr / d.pu, irel = rr - k * d.pu, i = d.ri0 + irel;
+    const bool pairs = (P.nz & 1) == 0;                 // 8-byte alignment of gT[y][x][even j] and of G rows
+    for (int q = warp0; q < P.Nw * ROW_GROUPS; q += n_warps) {
+        const int k = q / ROW_GROUPS, g = q - k * ROW_GROUPS;
         const SliceBox F = dilate(P, slice_support(P, d, k), C);
-        if (i < F.u0 || i > F.u1 || F.v0 > F.v1) continue;
-        const float w = P.wmin + k * P.dw, u = (i - P.cu) * P.du;
-        const float fx = (P.isox + u * d.cg - w * d.sg - P.ox) / P.sx;
-        const float fy = (P.isoy + u * d.sg + w * d.cg - P.oy) / P.sy;
-        const int xa = max(0, (int)ceilf(fx - hx)), xb = min(P.nx - 1, (int)floorf(fx + hx));
-        const int ya = max(0, (int)ceilf(fy - hy)), yb = min(P.ny - 1, (int)floorf(fy + hy));
-        const float dxa = P.ox + xa * P.sx - P.isox, dya = P.oy + ya * P.sy - P.isoy;
-        const float eu0 = (d.cg * dxa + d.sg * dya) / P.du + P.cu - (float)i;
-        const float ew0 = (-d.sg * dxa + d.cg * dya - P.wmin) / P.dw - (float)k;
-        float *orow = Gc + (size_t)rr * d.pv - d.rj0;
-        if (xb - xa <= 2 && yb - ya <= 2) {
-            // usual case (beam spacing ~ patient spacing): at most 3 x 3 candidates
-            const float wu = 1.f - fabsf(eu0 + cy * fu_y + cx * fu_x), ww = 1.f - fabsf(ew0 + cy * fw_y + cx * fw_x);
-            const float wmine = (wu > 0.f && ww > 0.f && xa + cx <= xb && ya + cy <= yb) ? wu * ww : 0.f;
-            float wq[9];
+        if (box_empty(F)) continue;
+        const float w = P.wmin + k * P.dw;
+        const int jv0 = pairs ? (F.v0 & ~1) : F.v0;     // the extra column lies inside the region (rj0 % 8 == 0) and is never read
+        for (int i = F.u0 + g; i <= F.u1; i += ROW_GROUPS) {
+            const float u = (i - P.cu) * P.du;
+            const float fx = (P.isox + u * d.cg - w * d.sg - P.ox) / P.sx;
+            const float fy = (P.isoy + u * d.sg + w * d.cg - P.oy) / P.sy;
+            const int xa = max(0, (int)ceilf(fx - hx)), xb = min(P.nx - 1, (int)floorf(fx + hx));
+            const int ya = max(0, (int)ceilf(fy - hy)), yb = min(P.ny - 1, (int)floorf(fy + hy));
+            const float dxa = P.ox + xa * P.sx - P.isox, dya = P.oy + ya * P.sy - P.isoy;
+            const float eu0 = (d.cg * dxa + d.sg * dya) / P.du + P.cu - (float)i;
+            const float ew0 = (-d.sg * dxa + d.cg * dya - P.wmin) / P.dw - (float)k;
+            float *orow = Gc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
+            if (xb - xa <= 2 && yb - ya <= 2) {
+                // usual case (beam spacing ~ patient spacing): at most 3 x 3 candidates
+                const float wu = 1.f - fabsf(eu0 + cy * fu_y + cx * fu_x), ww = 1.f - fabsf(ew0 + cy * fw_y + cx * fw_x);
+                const float wmine = (wu > 0.f && ww > 0.f && xa + cx <= xb && ya + cy <= yb) ? wu * ww : 0.f;
+                float wq[9];
 #pragma unroll
-            for (int q = 0; q < 9; ++q) wq[q] = __shfl_sync(0xffffffffu, wmine, q);
-            const float *g0 = gT + ((size_t)ya * P.nx + xa) * P.nz;
-            for (int j = F.v0 + lane; j <= F.v1; j += 32) {
-                float v[9];
+                for (int c = 0; c < 9; ++c) wq[c] = __shfl_sync(0xffffffffu, wmine, c);
+                const float *g0 = gT + ((size_t)ya * P.nx + xa) * P.nz;
+                if (pairs) {
+                    for (int j = jv0 + 2 * lane; j <= F.v1; j += 64) {
+                        float2 v[9];
 #pragma unroll
-                for (int q = 0; q < 9; ++q)        // all loads of the column first, so that their latencies overlap
-                    v[q] = wq[q] != 0.f ? __ldg(g0 + ((size_t)(q / 3) * P.nx + (q % 3)) * P.nz + j) : 0.f;
-                float acc = 0.f;
+                        for (int c = 0; c < 9; ++c)    // all loads first, so that their latencies overlap
+                            v[c] = wq[c] != 0.f ? __ldg(reinterpret_cast<const float2 *>(g0 + ((size_t)(c / 3) * P.nx + (c % 3)) * P.nz + j)) : make_float2(0.f, 0.f);
+                        float2 acc = make_float2(0.f, 0.f);
 #pragma unroll
-                for (int q = 0; q < 9; ++q) acc = fmaf(wq[q], v[q], acc);
-                orow[j] = acc;
-            }
-        } else {
-            for (int j = F.v0 + lane; j <= F.v1; j += 32) {
-                float acc = 0.f;
-                for (int yy = ya; yy <= yb; ++yy) {
-                    const float euy = eu0 + (yy - ya) * fu_y, ewy = ew0 + (yy - ya) * fw_y;
-                    for (int xx = xa; xx <= xb; ++xx) {
-                        const float wu = 1.f - fabsf(euy + (xx - xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - xa) * fw_x);
-                        if (wu > 0.f && ww > 0.f) acc = fmaf(wu * ww, __ldg(gT + ((size_t)yy * P.nx + xx) * P.nz + j), acc);
+                        for (int c = 0; c < 9; ++c) { acc.x = fmaf(wq[c], v[c].x, acc.x); acc.y = fmaf(wq[c], v[c].y, acc.y); }
+                        *reinterpret_cast<float2 *>(orow + j) = acc;
+                    }
+                } else {
+                    for (int j = jv0 + lane; j <= F.v1; j += 32) {
+                        float v[9];
+#pragma unroll
+                        for (int c = 0; c < 9; ++c)
+                            v[c] = wq[c] != 0.f ? __ldg(g0 + ((size_t)(c / 3) * P.nx + (c % 3)) * P.nz + j) : 0.f;
+                        float acc = 0.f;
+#pragma unroll
+                        for (int c = 0; c < 9; ++c) acc = fmaf(wq[c], v[c], acc);
+                        orow[j] = acc;
                     }
                 }
-                orow[j] = acc;
+            } else {
+                for (int j = F.v0 + lane; j <= F.v1; j += 32) {
+                    float acc = 0.f;
+                    for (int yy = ya; yy <= yb; ++yy) {
+                        const float euy = eu0 + (yy - ya) * fu_y, ewy = ew0 + (yy - ya) * fw_y;
+                        for (int xx = xa; xx <= xb; ++xx) {
+                            const float wu = 1.f - fabsf(euy + (xx - xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - xa) * fw_x);
+                            if (wu > 0.f && ww > 0.f) acc = fmaf(wu * ww, __ldg(gT + ((size_t)yy * P.nx + xx) * P.nz + j), acc);
+                        }
+                    }
+                    orow[j] = acc;
+                }
             }
         }
     }

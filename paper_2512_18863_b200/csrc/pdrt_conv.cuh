@@ -79,14 +79,15 @@ k_project(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const fl
         const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
         const float su = mag * P.du / P.Du, sv = mag / P.Dv;
         // column terms of this lane (two passes cover 64 columns; wider supports loop)
-        for (int j0 = S.v0; j0 <= S.v1; j0 += 32) {
+        // columns [S.v0 & ~1, S.v1 | 1]: the conv stages its tiles in aligned pairs; the extra columns are structural zeros
+        for (int j0 = S.v0 & ~1; j0 <= (S.v1 | 1); j0 += 32) {
             const int j = j0 + lane;
             const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
             const float flb = floorf(fb);
             const int b = (int)flb;
             const float tb = fb - flb;
-            const bool jin = j <= S.v1;
-            const bool b0 = jin && b >= d.b0 && b <= d.b1, b1 = jin && b + 1 >= d.b0 && b + 1 <= d.b1;
+            const bool jin = j <= (S.v1 | 1), jgrid = j < P.Nv;
+            const bool b0 = jgrid && b >= d.b0 && b <= d.b1, b1 = jgrid && b + 1 >= d.b0 && b + 1 <= d.b1;
             for (int i = S.u0 + g; i <= S.u1; i += ROW_GROUPS) {
                 const float fa = (i - P.cu) * su + P.cuf;
                 const float fla = floorf(fa);
@@ -131,7 +132,8 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
         const SliceBox F = dilate(P, slice_support(P, d, k), C);
         if (box_empty(F)) continue;
         const float w = P.wmin + k * P.dw;
-        const int jv0 = pairs ? (F.v0 & ~1) : F.v0;     // the extra column lies inside the region (rj0 % 8 == 0) and is never read
+        const int jv0 = F.v0 & ~1, jv1 = F.v1 | 1;      // aligned pairs for the conv's tile copies; the extra columns lie inside
+                                                        // the region (rj0 % 8 == 0) and only feed outputs nobody reads
         for (int i = F.u0 + g; i <= F.u1; i += ROW_GROUPS) {
             const float u = (i - P.cu) * P.du;
             const float fx = (P.isox + u * d.cg - w * d.sg - P.ox) / P.sx;
@@ -151,7 +153,7 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
                 for (int c = 0; c < 9; ++c) wq[c] = __shfl_sync(0xffffffffu, wmine, c);
                 const float *g0 = gT + ((size_t)ya * P.nx + xa) * P.nz;
                 if (pairs) {
-                    for (int j = jv0 + 2 * lane; j <= F.v1; j += 64) {
+                    for (int j = jv0 + 2 * lane; j <= jv1; j += 64) {
                         float2 v[9];
 #pragma unroll
                         for (int c = 0; c < 9; ++c)    // all loads first, so that their latencies overlap
@@ -162,11 +164,11 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
                         *reinterpret_cast<float2 *>(orow + j) = acc;
                     }
                 } else {
-                    for (int j = jv0 + lane; j <= F.v1; j += 32) {
+                    for (int j = jv0 + lane; j <= jv1; j += 32) {
                         float v[9];
 #pragma unroll
                         for (int c = 0; c < 9; ++c)
-                            v[c] = wq[c] != 0.f ? __ldg(g0 + ((size_t)(c / 3) * P.nx + (c % 3)) * P.nz + j) : 0.f;
+                            v[c] = (wq[c] != 0.f && j < P.Nv) ? __ldg(g0 + ((size_t)(c / 3) * P.nx + (c % 3)) * P.nz + j) : 0.f;
                         float acc = 0.f;
 #pragma unroll
                         for (int c = 0; c < 9; ++c) acc = fmaf(wq[c], v[c], acc);
@@ -174,9 +176,9 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
                     }
                 }
             } else {
-                for (int j = F.v0 + lane; j <= F.v1; j += 32) {
+                for (int j = jv0 + lane; j <= jv1; j += 32) {
                     float acc = 0.f;
-                    for (int yy = ya; yy <= yb; ++yy) {
+                    for (int yy = ya; yy <= yb && j < P.Nv; ++yy) {
                         const float euy = eu0 + (yy - ya) * fu_y, ewy = ew0 + (yy - ya) * fw_y;
                         for (int xx = xa; xx <= xb; ++xx) {
                             const float wu = 1.f - fabsf(euy + (xx - xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - xa) * fw_x);
@@ -230,6 +232,7 @@ __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__
     it.S = slice_support(P, d, it.k);
     const SliceBox F = dilate(P, it.S, C);
     it.B = ADJ ? F : it.S;
+    if (C % 2 == 0) { it.B.v0 &= ~1; it.B.v1 |= 1; }              // tile copies move aligned pairs (k_project / k_resample_adjoint write them)
     const SliceBox A = ADJ ? it.S : F;                            // outputs to compute
     int atf0 = 0, atf1 = -1, ats0 = 0, ats1 = -1;
     if (!box_empty(A)) {
@@ -313,36 +316,28 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
         {   // input tile: asynchronous copies (zero-filled outside the source box), lanes along v.  The column terms
             // (source offset, swizzled destination, validity) are worked out once per unit, not once per row.
             const int tv0 = I.tv0, bv0 = I.B.v0, bv1 = I.B.v1;
-            int joff[MC], cfl[MC];
+            int joff[MC];
             unsigned doff[MC];
+            bool cex[MC], cin[MC];
 #pragma unroll
             for (int m = 0; m < MC; ++m) {
                 const int c = CPL * (lane + 32 * m), j = tv0 + c;
-                const bool ex = c < pitch;
-                const bool v0 = ex && j >= bv0 && j <= bv1, v1 = CPL == 2 && ex && j + 1 >= bv0 && j + 1 <= bv1;
-                joff[m] = (v0 || v1) ? j - I.rj0 : 0;
+                cex[m] = c < pitch;
+                cin[m] = cex[m] && j >= bv0 && j <= bv1;                   // pairs are inside or outside as a whole (aligned box)
+                joff[m] = cin[m] ? j - I.rj0 : 0;
                 doff[m] = 4u * (unsigned)swz_col(c);
-                cfl[m] = (ex ? 4 : 0) | (v0 ? 1 : 0) | (v1 ? 2 : 0);
             }
             const float *sbase = in + I.slice_off;                         // row i of the slice at sbase + (i - ri0) * pv
             for (int r = 0; r < I.rows; ++r) {
                 const int i = I.tu0 + r;
                 const bool rin = i >= I.B.u0 && i <= I.B.u1;
-                const float *srow = sbase + (rin ? (long long)(i - I.ri0) * I.pv : 0ll);
+                const float *srow = sbase + (rin ? (i - I.ri0) * I.pv : 0);
                 const unsigned drow = tile_s + 4u * (unsigned)(r * pitch);
 #pragma unroll
                 for (int m = 0; m < MC; ++m) {
-                    if (!(cfl[m] & 4)) continue;
-                    const int f = rin ? (cfl[m] & 3) : 0;
-                    if (CPL == 2) {
-                        if (f == 2) {                  // only the second float lies inside the box
-                            cp_async_4(drow + doff[m], srow, 0);
-                            cp_async_4(drow + doff[m] + 4u, srow + joff[m] + 1, 4);
-                        } else {
-                            cp_async_8(drow + doff[m], srow + joff[m], f == 3 ? 8 : (f == 1 ? 4 : 0));
-                        }
-                    } else {
-                        cp_async_4(drow + doff[m], srow + joff[m], f ? 4 : 0);
+                    if (cex[m]) {
+                        if (CPL == 2) cp_async_8(drow + doff[m], srow + joff[m], (rin && cin[m]) ? 8 : 0);
+                        else cp_async_4(drow + doff[m], srow + joff[m], (rin && cin[m]) ? 4 : 0);
                     }
                 }
             }

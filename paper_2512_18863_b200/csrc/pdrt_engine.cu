@@ -294,7 +294,7 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
     const int nb = batch_size(e, n_cp, 2);
     CU(e, e->bufA.ensure((size_t)nb * e->P.stride_cp));
     CU(e, e->bufB.ensure((size_t)nb * e->P.stride_cp));
-    const dim3 gg((e->P.nx + GATHER_T - 1) / GATHER_T, (e->P.ny + GATHER_T - 1) / GATHER_T, (e->P.nz + GATHER_Z - 1) / GATHER_Z);
+    const dim3 gg((e->P.nx + GATHER_TX - 1) / GATHER_TX, (e->P.ny + GATHER_TY - 1) / GATHER_TY, (e->P.nz + GATHER_Z - 1) / GATHER_Z);
     for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
         const int n = std::min(nb, n_cp - cp0);
         {

@@ -8,9 +8,10 @@
 
 namespace pdrt {
 
-constexpr int GATHER_T = 16;            // block = 16 x 16 patient columns (x,y) ...
+constexpr int GATHER_TX = 16, GATHER_TY = 4;   // block = 16 x 4 patient columns (x,y): two warp patches of 8 x 4 ...
 constexpr int GATHER_Z = 32;            // ... times 32 z-slices
-constexpr int GATHER_THREADS = GATHER_T * GATHER_T;
+constexpr int GATHER_SPLIT = 4;         // ... times 4 warps per patch that share the control-point list round-robin
+constexpr int GATHER_THREADS = 2 * GATHER_SPLIT * 32;
 constexpr int GATHER_CHUNK = 128;       // control points staged in shared memory per pass
 
 struct GatherCp {                       // the slice of CpDesc the resampler needs
@@ -29,24 +30,28 @@ struct GatherCp {                       // the slice of CpDesc the resampler nee
 // per column, taking offset and weights by warp shuffle: every load instruction reads four full 128-byte
 // lines of the v-fastest D_b block.  A lane accumulates 8 column groups x 4 z in registers over all control
 // points (in control-point order: deterministic) and every patient voxel is written exactly once.
-// Warp 0 first compacts the control points whose compact region can intersect this block.
+// Warp 0 first compacts the control points whose compact region can intersect this block.  The per-control-point
+// chain (setup -> shuffle -> load -> accumulate) is latency-bound, so four warps share the list of one patch
+// (entries q = s, s+4, ...) and their partial sums are added through shared memory in a fixed order.
 __global__ void __launch_bounds__(GATHER_THREADS)
 k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ D,
               float *__restrict__ dose, int accumulate)
 {
     __shared__ GatherCp list[GATHER_CHUNK];
     __shared__ int n_list;
+    __shared__ float4 part[2 * (GATHER_SPLIT - 1)][8][32];
     const int tid = threadIdx.x;
     const int wrp = tid >> 5, lane = tid & 31;
-    const int px0 = blockIdx.x * GATHER_T + (wrp & 1) * 8, py0 = blockIdx.y * GATHER_T + (wrp >> 1) * 4;
+    const int patch = wrp & 1, split = wrp >> 1;
+    const int px0 = blockIdx.x * GATHER_TX + patch * 8, py0 = blockIdx.y * GATHER_TY;
     const int z0 = blockIdx.z * GATHER_Z;
     // the column this lane sets up
     const int ix = px0 + (lane & 7), iy = py0 + (lane >> 3);
     const float dx = P.ox + ix * P.sx - P.isox, dy = P.oy + iy * P.sy - P.isoy;
     const bool inside = ix < P.nx && iy < P.ny;
     // tile corners (for culling), relative to the isocentre
-    const float cx0 = P.ox + (blockIdx.x * GATHER_T) * P.sx - P.isox, cx1 = cx0 + (GATHER_T - 1) * P.sx;
-    const float cy0 = P.oy + (blockIdx.y * GATHER_T) * P.sy - P.isoy, cy1 = cy0 + (GATHER_T - 1) * P.sy;
+    const float cx0 = P.ox + (blockIdx.x * GATHER_TX) * P.sx - P.isox, cx1 = cx0 + (GATHER_TX - 1) * P.sx;
+    const float cy0 = P.oy + (blockIdx.y * GATHER_TY) * P.sy - P.isoy, cy1 = cy0 + (GATHER_TY - 1) * P.sy;
     const int sub = lane >> 3, zl = 4 * (lane & 7);      // column within a group of four, z offset of this lane's quad
     float4 acc[8];
 #pragma unroll
@@ -86,7 +91,7 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, cons
         }
         __syncthreads();
         const int n = n_list;
-        for (int q = 0; q < n; ++q) {
+        for (int q = split; q < n; q += GATHER_SPLIT) {
             const GatherCp g = list[q];
             const float fu = (g.cg * dx + g.sg * dy) / P.du + P.cu;
             const float fw = (-g.sg * dx + g.cg * dy - P.wmin) / P.dw;
@@ -128,6 +133,22 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, cons
                     acc[gq].w += f00 * a.w + f10 * b.w + f01 * c.w + f11 * e.w;
                 }
             }
+        }
+    }
+    // partial sums of the four warps of a patch, added in a fixed order
+    __syncthreads();
+    if (split > 0) {
+#pragma unroll
+        for (int gq = 0; gq < 8; ++gq) part[(split - 1) * 2 + patch][gq][lane] = acc[gq];
+    }
+    __syncthreads();
+    if (split > 0) return;
+#pragma unroll
+    for (int gq = 0; gq < 8; ++gq) {
+#pragma unroll
+        for (int sp = 0; sp < GATHER_SPLIT - 1; ++sp) {
+            const float4 v = part[sp * 2 + patch][gq][lane];
+            acc[gq].x += v.x; acc[gq].y += v.y; acc[gq].z += v.z; acc[gq].w += v.w;
         }
     }
 #pragma unroll

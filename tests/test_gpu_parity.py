@@ -193,3 +193,80 @@ def test_host_entry_points_and_errors(torch):
         eng.set_kernel_size(65)
     with pytest.raises(PdrtError):
         Engine(wl.grid, dict(wl.model, leaf_bounds_mm=np.zeros(wl.model["n_pairs"] + 1, np.float32)), wl.density)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Full-size configurations, in the launch configuration bench.py times.  The oracle cannot produce a whole dose
+# grid of these sizes in seconds, so the dose is compared on sampled voxels that it computes one by one
+# (orc_dose_at: the same definitions evaluated per output) and the gradients on sampled control points (the
+# gradient rows of different control points are independent given dL/dDose).
+def sample_voxels(dose, n, seed):
+    """Seeded sample of voxel indices (x, y, z): the maximum, voxels above 5 % of it, and voxels anywhere."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    nz, ny, nx = dose.shape
+    flat = dose.reshape(-1)
+    top = int(np.argmax(flat))
+    hot = np.flatnonzero(flat > 0.05 * flat[top])
+    pick = np.concatenate([[top], rng.choice(hot, size=min(len(hot), (2 * n) // 3), replace=False),
+                           rng.integers(0, flat.size, size=n // 3)])
+    z, rem = np.divmod(pick, ny * nx)
+    y, x = np.divmod(rem, nx)
+    return np.stack([x, y, z], axis=1).astype(np.int32), pick
+
+
+def check_sampled_dose(eng, orc, wl, n_pts, seed, what):
+    d = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu).cpu().numpy()
+    assert np.isfinite(d).all()
+    ijk, pick = sample_voxels(d, n_pts, seed)
+    ref = orc.dose_at(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, ijk)
+    scale = ref.max()                                   # includes the voxel where the GPU dose peaks
+    assert scale > 0
+    err = np.abs(d.reshape(-1)[pick].astype(np.float64) - ref).max()
+    assert err <= DOSE_TOL * scale, f"{what}: sampled max err {err:.3e} vs {DOSE_TOL}*{scale:.3e} (ratio {err / scale:.2e})"
+    return d
+
+
+def check_sampled_gradients(eng, orc, wl, g, cps, what):
+    dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    rl, rj, rm = orc.dose_backward(wl.leaves[cps], wl.jaws[cps], wl.gantry_deg[cps], wl.mu[cps], g)
+    assert np.isfinite(dl.cpu().numpy()).all() and np.isfinite(dj.cpu().numpy()).all() and np.isfinite(dm.cpu().numpy()).all()
+    idx = torch_index(dl, cps)
+    assert_grad(dm[idx], rm, f"{what} d_mu")
+    assert_grad(dl[idx], rl, f"{what} d_leaves")
+    assert_grad(dj[idx], rj, f"{what} d_jaws")
+
+
+def torch_index(t, cps):
+    import torch as _t
+    return _t.as_tensor(np.asarray(cps), device=t.device, dtype=_t.long)
+
+
+def test_config3_full_arc_forward_sampled(torch):
+    """c3: 200x200x120 pelvis phantom, 178 control points, 60 leaf pairs, k = 21, forward."""
+    wl = W.config3()
+    eng, orc = pair(wl)
+    check_sampled_dose(eng, orc, wl, 240, 3, "c3")
+
+
+def test_config4_full_arc_forward_backward_sampled(torch):
+    """c4 (the configuration bench.py times): forward on sampled voxels, backward on sampled control points, and a
+    second kernel size of the sweep."""
+    wl = W.config4(21)
+    eng, orc = pair(wl)
+    check_sampled_dose(eng, orc, wl, 240, 4, "c4 k=21")
+    g = W.seeded_dose_gradient(wl, seed=4)
+    check_sampled_gradients(eng, orc, wl, g, [0, 37, 89, 133, 177], "c4 k=21")
+    eng.set_kernel_size(11)
+    orc.set_kernel_size(11)
+    check_sampled_dose(eng, orc, wl, 90, 5, "c4 k=11")
+    check_sampled_gradients(eng, orc, wl, g, [5, 120], "c4 k=11")
+
+
+def test_config5_double_arc_sampled(torch):
+    """c5: 256x256x160 @ 2 mm, two arcs (356 control points), 80 leaf pairs misaligned with the 2 mm map rows,
+    tracking jaws, k = 31: first iteration of the planning loop."""
+    wl = W.config5()
+    eng, orc = pair(wl)
+    check_sampled_dose(eng, orc, wl, 120, 6, "c5")
+    g = W.seeded_dose_gradient(wl, seed=6)
+    check_sampled_gradients(eng, orc, wl, g, [0, 200, 355], "c5")

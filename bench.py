@@ -30,6 +30,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "ms per full-arc dose forward+backward"
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_conv<21,false> launch on c4 (profiles/r1b_ncu_full.md)
+NCU_CONV_DRAM_BYTES = 978.0e6
 FP32_LANES_PER_SM = 128
 
 
@@ -43,45 +45,71 @@ def load_peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
-    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-              "clocks_event_reasons.sw_power_cap")
+    """Samples SM clock, power and throttle reasons through NVML every 20 ms while the load runs."""
 
     def __init__(self, index=0):
-        self.rows, self.proc, self.index = [], None, index
+        self.rows, self.index, self.stop, self.thread, self.mark = [], index, False, None, 0
+        self.max_mhz = None
 
     def __enter__(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.thread = threading.Thread(target=self._read, daemon=True)
+            import pynvml as nv
+            nv.nvmlInit()
+            # CUDA_VISIBLE_DEVICES may renumber: take the NVML handle of the torch device by PCI bus id when possible
+            try:
+                import torch
+                bus = torch.cuda.get_device_properties(self.index).pci_bus_id
+                h = None
+                for i in range(nv.nvmlDeviceGetCount()):
+                    hi = nv.nvmlDeviceGetHandleByIndex(i)
+                    if nv.nvmlDeviceGetPciInfo(hi).bus == bus:
+                        h = hi
+                h = h or nv.nvmlDeviceGetHandleByIndex(self.index)
+            except Exception:
+                h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.nv, self.h = nv, h
+            self.max_mhz = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            self.thread = threading.Thread(target=self._run, daemon=True)
             self.thread.start()
-        except OSError:
-            self.proc = None
+        except Exception:
+            self.thread = None
         return self
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+    def _run(self):
+        nv, h = self.nv, self.h
+        while not self.stop:
+            try:
+                self.rows.append((float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)),
+                                  int(nv.nvmlDeviceGetCurrentClocksEventReasons(h)) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons")
+                                  else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)),
+                                  nv.nvmlDeviceGetPowerUsage(h) / 1e3))
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def wait_first(self, timeout=2.0):
+        t0 = time.perf_counter()
+        while self.thread and not self.rows and time.perf_counter() - t0 < timeout:
+            time.sleep(0.01)
+        self.mark = len(self.rows)
 
     def __exit__(self, *exc):
-        if self.proc:
-            self.proc.terminate()
+        self.stop = True
+        if self.thread:
             self.thread.join(timeout=2)
 
     def summary(self):
-        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
-        reasons = set()
-        for r in self.rows:
-            if len(r) >= 7:
-                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
-                    if v.lower().startswith("active"):
-                        reasons.add(name)
-        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
-        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
-                    reasons=sorted(reasons), samples=len(sm))
+        rows = self.rows[self.mark:] or self.rows       # samples taken while the GPU was under load
+        sm = [r[0] for r in rows]
+        bits = 0
+        for r in rows:
+            bits |= r[1]
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                 0x80: "hw_power_brake_slowdown"}
+        reasons = sorted(n for b, n in names.items() if bits & b)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=self.max_mhz, reasons=reasons, samples=len(sm),
+                    power_w_max=max((r[2] for r in rows), default=None),
+                    window="NVML every 20 ms from the first warm-up step to the end of the timed steps (same load throughout)")
 
 
 def make_workload(name, kernel_size):
@@ -141,14 +169,14 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------ our arm
-def cpu_baseline(wl, seconds_budget=20.0):
+def cpu_baseline(wl, seconds_budget=15.0):
     """The oracle on a bounded sample of the same workload (rank 0, N = 1): forward+backward of a few control points."""
     from oracle.oracle import Oracle
     from paper_2512_18863_b200 import workloads as W
     orc = Oracle(wl.grid, wl.model, wl.density)
     g = W.seeded_dose_gradient(wl, seed=0)
     n_s, total = 0, 0.0
-    idx_all = np.linspace(0, wl.n_cp - 1, min(wl.n_cp, 8)).round().astype(int)
+    idx_all = np.linspace(0, wl.n_cp - 1, min(wl.n_cp, 64)).round().astype(int)
     for b in idx_all:
         t0 = time.perf_counter()
         orc.dose(wl.leaves[b:b + 1], wl.jaws[b:b + 1], wl.gantry_deg[b:b + 1], wl.mu[b:b + 1])
@@ -211,6 +239,9 @@ def run_ours(args):
         forward()
         eng.dose_backward(lv, jw, ga, mu, g, out=grads)
 
+    clk = ClockSampler(local)
+    clk.__enter__()
+    clk.wait_first()
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
@@ -222,7 +253,7 @@ def run_ours(args):
     stage_ms = {s: 0.0 for s in STAGES}
     launches = 0
     t_wall0 = time.perf_counter()
-    with ClockSampler(local) as clk:
+    try:
         for a, b, b2, c in ev:
             flush.zero_()                      # L2 flush, outside the timed events
             a.record()
@@ -239,6 +270,8 @@ def run_ours(args):
                 stage_ms[s] += bw_ms[s] + (fw_ms[s] if fw_ms else 0.0)
             launches += sum(bw_n.values()) + (sum(fw_n.values()) if fw_n else 0)
         torch.cuda.synchronize()
+    finally:
+        clk.__exit__(None, None, None)
     t_wall = time.perf_counter() - t_wall0
     eng.set_profiling(False)
     fwd_ms = float(np.mean([a.elapsed_time(b) for a, b, _, _ in ev]))
@@ -261,9 +294,11 @@ def run_ours(args):
     stages = {}
     if world == 1:
         nvox = eng.info.nx * eng.info.ny * eng.info.nz
-        byts = dict(gather=4.0 * wf.region_voxels + 4.0 * nvox,                   # read D_b blocks once, write dose once
-                    resample_adj=4.0 * wb.region_voxels + 4.0 * nvox,             # read g once (L2-resident after), write G_b
-                    project_adj=4.0 * wb.support_voxels, conv=4.0 * wf.region_voxels, conv_adj=4.0 * (wb.region_voxels + wb.support_voxels))
+        # algorithmic HBM bytes of the dataflow implemented: Phivol over S_k, D_b over the compact regions,
+        # G_b over F_k, H_b over S_k, each written once and read once; dose written once; dL/dDose read once (L2 after)
+        sup, fpr, reg = 4.0 * wf.support_voxels, 4.0 * wf.footprint_voxels, 4.0 * wf.region_voxels
+        byts = dict(project=sup, conv=sup + reg, gather=reg + 4.0 * nvox,
+                    transpose=8.0 * nvox, resample_adj=fpr + 4.0 * nvox, conv_adj=fpr + sup, project_adj=sup)
         for s in STAGES:
             stages[s] = dict(ms=round(stage_ms[s], 4))
             if s in byts and stage_ms[s] > 0:
@@ -274,9 +309,9 @@ def run_ours(args):
         stages["conv_adj"].update(tflops=round(conv_adj_flops / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None,
                                   issued_tflops=round(2.0 * wb.conv_macs / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None)
     achieved = conv_flops / (stage_ms["conv"] * 1e-3) / 1e12 if stage_ms["conv"] > 0 else None
-    roofline = dict(bound="alu", kernel="k_conv<K,false> (S3+S4+S5 fused projection + lateral convolution)",
+    roofline = dict(bound="alu", kernel="k_conv<K,false> (S4+S5: depth-indexed kernel lookup + lateral convolution)",
                     achieved=achieved, peak=fp32_peak, unit="TFLOP/s", frac=(achieved / fp32_peak) if achieved else None,
-                    traffic=None,
+                    traffic=NCU_CONV_DRAM_BYTES if (wl.name == "c4" and K == 21) else None,
                     note=f"algorithmic flops = 2*k^2*|footprint| per launch; peak = {eng.info.sm_count} SMs x 128 FP32 lanes x 2 x "
                          f"{peaks['sm_max_mhz']:.0f} MHz (plain FP32 FMA pipe; FFMA microbenchmark on this pool: 72.5 TFLOP/s); "
                          f"HBM fractions of the bandwidth-bound stages are under 'stages' against {peaks['hbm_gbs']} GB/s {peaks['source']}")
@@ -347,7 +382,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--workload", default="c4", choices=("c3", "c4", "c5"))

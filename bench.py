@@ -206,7 +206,8 @@ def run_ours(args):
     eng = Engine(wl.grid, wl.model, wl.density, device=str(dev))
 
     # shard control points (contiguous blocks); every rank holds the density, tables and dL/dDose
-    lo, hi = (wl.n_cp * rank) // world, (wl.n_cp * (rank + 1)) // world
+    from paper_2512_18863_b200.shard import reduce_dose, shard_range
+    lo, hi = shard_range(wl.n_cp, rank, world)
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     lv, jw, ga, mu = t(wl.leaves[lo:hi]), t(wl.jaws[lo:hi]), t(wl.gantry_deg[lo:hi]), t(wl.mu[lo:hi])
     dose = torch.empty(eng.dose_shape, dtype=torch.float32, device=dev)
@@ -224,8 +225,7 @@ def run_ours(args):
 
     def forward():
         eng.dose(lv, jw, ga, mu, out=dose)
-        if world > 1:
-            dist.all_reduce(dose)
+        reduce_dose(dose)
 
     def objective_grad():
         return wmask * (dose - pmask)

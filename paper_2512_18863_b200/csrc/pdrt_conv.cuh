@@ -192,20 +192,17 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
     }
 }
 
-// Geometry of one conv work unit (control point, slice, chunk along v, group of 32 active thread-tiles);
-// identical in every lane of the warp.
+// Geometry of one conv work item (control point, slice, chunk along v); identical in every lane of the warp.
 struct ConvItem {
-    int active;                      // the unit has thread-tiles to compute
-    int zero_duty;                   // forward: this unit also zeroes the inactive thread-tiles of its slice and chunk
     int slot, cp, k;
     int pv, nts;
     long long slice_off;             // slot * stride_cp + k * pu * pv  (start of the [pu][pv] slice in the compact blocks)
     int ri0, rj0;
-    SliceBox S, B;                   // fluence support of the slice; source box of the input tile (S forward, F adjoint)
+    SliceBox S, B;                   // fluence support of the slice; source box of the input rows (S forward, F adjoint)
     int ctf0, ctf1;                  // thread-tile range of the chunk along v
     int atf0, ats0, naf, nas;        // active thread-tiles of the slice and chunk (outputs to compute)
-    int t0, n_tiles, ts_lo;          // first tile of the unit, active tiles, first tile row of the unit
-    int pitch, rows, tv0, tu0;       // input tile: row pitch, rows, input coords of tile[0][0]
+    int n_tiles;                     // naf * nas
+    int pitch, ring, tv0, tu0;       // input rows: pitch, rows the ring holds, input coords of window row 0 / column 0
     int n0;                          // slice kernel: table node and fraction
     float f;
 };
@@ -213,26 +210,23 @@ struct ConvItem {
 template <int KT, bool ADJ>
 __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
                                                const int *__restrict__ tile_base, const float *__restrict__ zrad,
-                                               int unit, int &slot_hint, ConvItem &it)
+                                               int item, int &slot_hint, ConvItem &it)
 {
     constexpr int C = (KT - 1) / 2;
-    while (slot_hint + 1 < n_cp && unit >= tile_base[slot_hint + 1]) ++slot_hint;   // units arrive in increasing order
+    while (slot_hint + 1 < n_cp && item >= tile_base[slot_hint + 1]) ++slot_hint;   // items arrive in increasing order
     it.slot = slot_hint;
     it.cp = cp0 + it.slot;
     const CpDesc d = desc[it.cp];
-    const int local = unit - tile_base[it.slot];
-    const int nuc = ADJ ? d.nuc_adj : d.nuc_fwd;
-    const int per_slice = d.ncf * nuc;
-    it.k = local / per_slice;
-    const int ch = local - it.k * per_slice;
-    const int cf = ch / nuc, c = ch - cf * nuc;
+    const int local = item - tile_base[it.slot];
+    it.k = local / d.ncf;
+    const int cf = local - it.k * d.ncf;
     it.ri0 = d.ri0; it.rj0 = d.rj0; it.pv = d.pv; it.nts = d.nts;
     it.slice_off = (long long)it.slot * P.stride_cp + (long long)it.k * d.pu * d.pv;
     it.ctf0 = cf * d.ntfc; it.ctf1 = min(d.ntf, it.ctf0 + d.ntfc);
     it.S = slice_support(P, d, it.k);
     const SliceBox F = dilate(P, it.S, C);
     it.B = ADJ ? F : it.S;
-    if (C % 2 == 0) { it.B.v0 &= ~1; it.B.v1 |= 1; }              // tile copies move aligned pairs (k_project / k_resample_adjoint write them)
+    if (C % 2 == 0) { it.B.v0 &= ~1; it.B.v1 |= 1; }              // row copies move aligned pairs (k_project / k_resample_adjoint write them)
     const SliceBox A = ADJ ? it.S : F;                            // outputs to compute
     int atf0 = 0, atf1 = -1, ats0 = 0, ats1 = -1;
     if (!box_empty(A)) {
@@ -242,16 +236,11 @@ __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__
     const bool any = atf0 <= atf1 && ats0 <= ats1;
     it.atf0 = atf0; it.ats0 = ats0; it.naf = any ? atf1 - atf0 + 1 : 0; it.nas = any ? ats1 - ats0 + 1 : 0;
     it.n_tiles = it.naf * it.nas;
-    it.t0 = c * CONV_CHUNK_TILES;
-    it.active = it.t0 < it.n_tiles;
-    it.zero_duty = c == 0;
-    it.ts_lo = 0; it.pitch = 8; it.rows = 0; it.tv0 = 0; it.tu0 = 0; it.n0 = 0; it.f = 0.f;
-    if (!it.active) return;
-    it.ts_lo = it.t0 / it.naf;
-    const int ts_hi = (min(it.n_tiles, it.t0 + CONV_CHUNK_TILES) - 1) / it.naf;
-    it.pitch = conv_pitch(KT, it.naf);
-    it.rows = (ts_hi - it.ts_lo + 1) * RS + KT - 1;
-    it.tv0 = d.rj0 + atf0 * RF - C; it.tu0 = d.ri0 + (ats0 + it.ts_lo) * RS - C;
+    it.pitch = conv_pitch(KT, max(it.naf, 1));
+    it.ring = P.tile_floats / it.pitch;
+    it.tv0 = d.rj0 + atf0 * RF - C; it.tu0 = d.ri0 + ats0 * RS - C;
+    it.n0 = 0; it.f = 0.f;
+    if (!any) return;
     // S4: slice kernel = lerp of the table in radiological depth
     const float t = zrad[(size_t)it.cp * P.Nw + it.k] / P.dz;
     int n0 = (int)floorf(t);
@@ -260,44 +249,46 @@ __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__
     it.f = fminf(fmaxf(t - n0, 0.f), 1.f);
 }
 
-// S4 + S5 (forward) / S8 (adjoint).  One WARP per block, many blocks per SM, persistent over the unit list
-// (control point, slice, chunk of <= 32 thread-tiles).  A warp owns its input tile and its copy of the slice
-// kernel in shared memory, so there is no block-level barrier anywhere: the tile streams in by cp.async
-// (zero-filled outside the source box: S_k forward, F_k adjoint) while the warp fetches and interpolates the
-// slice kernel, and the other warps resident on the SM keep the FFMA pipe busy meanwhile.  Slices are small
-// (a few hundred thread-tiles), so a block-wide tile shared through __syncthreads left the warps waiting on each
-// other for almost half of their time (profiles/); independent warps balance by construction.
+// S4 + S5 (forward) / S8 (adjoint).  One WARP per block, many blocks per SM, persistent over the item list
+// (control point, slice, chunk along v); items are handed out by a global counter.  A warp owns its input rows
+// and its copy of the slice kernel in shared memory, so there is no block-level barrier anywhere.  It walks the
+// active thread-tiles of its slice (F_k forward, S_k adjoint) in row-major order, 32 at a time (one 8(v) x 2(u)
+// thread-tile per lane); the input rows live in a ring of shared-memory rows that slides down the slice, so every
+// input row is fetched once per slice (cp.async in aligned pairs, zero-filled outside the source box: S_k
+// forward, F_k adjoint), and geometry and slice kernel are worked out once per slice.  Slices are small (a few
+// hundred thread-tiles): a block-wide tile shared through __syncthreads left the warps waiting on each other for
+// almost half of their time (profiles/); independent warps balance by construction, and the other warps resident
+// on the SM keep the FFMA pipe busy while one waits for its copies.
 template <int KT, bool ADJ>
 __global__ void __launch_bounds__(CONV_THREADS)
 k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
        const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
-       int *unit_counter)
+       int *item_counter)
 {
     constexpr int C = (KT - 1) / 2;
     constexpr int KP = (KT + 3) & ~3;                 // weight row pitch [floats]
     constexpr int XW = (KT + RF - 1 + 3) & ~3;        // register window along v [floats]
     constexpr int NXQ = XW / 4;
     constexpr int CPL = (C % 2 == 0) ? 2 : 1;         // floats per asynchronous copy (source and tile columns share parity when C is even)
-    constexpr int PMAX = (NTFC_MAX * RF + XW - RF + 7) & ~7;   // widest tile row
-    constexpr int MC = (PMAX / CPL + 31) / 32;        // copies per lane and tile row
+    constexpr int PMAX = (NTFC_MAX * RF + XW - RF + 7) & ~7;   // widest row
+    constexpr int MC = (PMAX / CPL + 31) / 32;        // copies per lane and row
     extern __shared__ float4 smem4[];
     float *Ws = reinterpret_cast<float *>(smem4);     // slice kernel [KT (du)][KP (dv)]
-    float *tile = Ws + KT * KP;                       // input tile [rows (u)][pitch (v)]
+    float *tile = Ws + KT * KP;                       // ring of input rows [ring][pitch (v)]
     const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
     const int lane = threadIdx.x;
     const int total = tile_base[n_cp];
     int slot_hint = 0;
 
-    // units are handed out by a global counter: every warp stays busy until the list is empty, whatever the unit sizes
     for (;;) {
-        int unit = 0;
-        if (lane == 0) unit = atomicAdd(unit_counter, 1);
-        unit = __shfl_sync(0xffffffffu, unit, 0);
-        if (unit >= total) break;
+        int item = 0;
+        if (lane == 0) item = atomicAdd(item_counter, 1);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= total) break;
         ConvItem I;
-        conv_load_item<KT, ADJ>(P, desc, cp0, n_cp, tile_base, zrad, unit, slot_hint, I);
+        conv_load_item<KT, ADJ>(P, desc, cp0, n_cp, tile_base, zrad, item, slot_hint, I);
         float *oslice = out + I.slice_off;             // [pu][pv] of slice k
-        if (!ADJ && I.zero_duty) {
+        if (!ADJ) {
             // the resampler reads the whole compact region: thread-tiles outside F_k hold exact zeros
             const int cw = I.ctf1 - I.ctf0, chn = cw * I.nts;
             for (int t = lane; t < chn; t += 32) {
@@ -311,37 +302,8 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                 }
             }
         }
-        if (!I.active) continue;                       // uniform across the warp
-        const int pitch = I.pitch;
-        {   // input tile: asynchronous copies (zero-filled outside the source box), lanes along v.  The column terms
-            // (source offset, swizzled destination, validity) are worked out once per unit, not once per row.
-            const int tv0 = I.tv0, bv0 = I.B.v0, bv1 = I.B.v1;
-            int joff[MC];
-            unsigned doff[MC];
-            bool cex[MC], cin[MC];
-#pragma unroll
-            for (int m = 0; m < MC; ++m) {
-                const int c = CPL * (lane + 32 * m), j = tv0 + c;
-                cex[m] = c < pitch;
-                cin[m] = cex[m] && j >= bv0 && j <= bv1;                   // pairs are inside or outside as a whole (aligned box)
-                joff[m] = cin[m] ? j - I.rj0 : 0;
-                doff[m] = 4u * (unsigned)swz_col(c);
-            }
-            const float *sbase = in + I.slice_off;                         // row i of the slice at sbase + (i - ri0) * pv
-            for (int r = 0; r < I.rows; ++r) {
-                const int i = I.tu0 + r;
-                const bool rin = i >= I.B.u0 && i <= I.B.u1;
-                const float *srow = sbase + (rin ? (i - I.ri0) * I.pv : 0);
-                const unsigned drow = tile_s + 4u * (unsigned)(r * pitch);
-#pragma unroll
-                for (int m = 0; m < MC; ++m) {
-                    if (cex[m]) {
-                        if (CPL == 2) cp_async_8(drow + doff[m], srow + joff[m], (rin && cin[m]) ? 8 : 0);
-                        else cp_async_4(drow + doff[m], srow + joff[m], (rin && cin[m]) ? 4 : 0);
-                    }
-                }
-            }
-        }
+        if (I.n_tiles == 0) continue;                  // uniform across the warp
+        const int pitch = I.pitch, ring = I.ring, naf = I.naf;
         {   // S4: slice kernel = lerp of the table in radiological depth; the table is stored as the [du][dv] image and is
             // point-symmetric, so forward and adjoint (flipped kernel) read the same entries
             const float4 *w0 = reinterpret_cast<const float4 *>(wtab + (size_t)I.n0 * KT * KP), *w1 = w0 + KT * KP / 4;
@@ -352,62 +314,101 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                 Ws4[e] = make_float4((1.f - f) * a.x + f * b.x, (1.f - f) * a.y + f * b.y, (1.f - f) * a.z + f * b.z, (1.f - f) * a.w + f * b.w);
             }
         }
-        cp_async_wait_all();
-        __syncwarp();
+        // column terms of the row copies (source offset, swizzled destination, validity): once per slice
+        int joff[MC];
+        unsigned doff[MC];
+        bool cex[MC], cin[MC];
+#pragma unroll
+        for (int m = 0; m < MC; ++m) {
+            const int c = CPL * (lane + 32 * m), j = I.tv0 + c;
+            cex[m] = c < pitch;
+            cin[m] = cex[m] && j >= I.B.v0 && j <= I.B.v1;                 // pairs are inside or outside as a whole (aligned box)
+            joff[m] = cin[m] ? j - I.rj0 : 0;
+            doff[m] = 4u * (unsigned)swz_col(c);
+        }
+        const float *sbase = in + I.slice_off;                             // row i of the slice at sbase + (i - ri0) * pv
+        const float *tile_end = tile + ring * pitch;
+        int loaded = 0;                                                    // window rows [0, loaded) have been fetched
 
-        const int naf = I.naf;
-        if (I.t0 + lane < I.n_tiles) {
-            const int t = I.t0 + lane;
-            const int tsa = t / naf, tf = t - tsa * naf, ts = tsa - I.ts_lo;     // ts: tile row relative to the input tile
-            float acc[RS][RF];
+        for (int t0 = 0; t0 < I.n_tiles; t0 += CONV_CHUNK_TILES) {
+            const int ts_lo = t0 / naf, ts_hi = (min(I.n_tiles, t0 + CONV_CHUNK_TILES) - 1) / naf;
+            const int need_lo = ts_lo * RS, need_hi = ts_hi * RS + RS - 1 + KT - 1;     // window rows of this group (inclusive)
+            __syncwarp();                                                  // rows below need_lo are free to be overwritten
+            {
+                int w = max(loaded, need_lo), pos = w % ring;
+                for (; w <= need_hi; ++w) {
+                    const int i = I.tu0 + w;
+                    const bool rin = i >= I.B.u0 && i <= I.B.u1;
+                    const float *srow = sbase + (rin ? (i - I.ri0) * I.pv : 0);
+                    const unsigned drow = tile_s + 4u * (unsigned)(pos * pitch);
 #pragma unroll
-            for (int ii = 0; ii < RS; ++ii)
-#pragma unroll
-                for (int r = 0; r < RF; ++r) acc[ii][r] = 0.f;
-            // forward: tile rows outside S_k hold zeros (structurally zero fluence) and are skipped
-            const int ylo = ADJ ? 0 : max(0, I.S.u0 - I.tu0 - ts * RS), yhi = ADJ ? KT + RS - 2 : min(KT + RS - 2, I.S.u1 - I.tu0 - ts * RS);
-            const float *xrow = tile + (ts * RS + ylo) * pitch;
-            int xoff[NXQ];
-#pragma unroll
-            for (int q = 0; q < NXQ; ++q) xoff[q] = swz_col(tf * RF + 4 * q);
-#pragma unroll 1
-            for (int y = ylo; y <= yhi; ++y) {
-                float x[XW];
-#pragma unroll
-                for (int q = 0; q < NXQ; ++q) {
-                    const float4 v = *reinterpret_cast<const float4 *>(xrow + xoff[q]);
-                    x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
+                    for (int m = 0; m < MC; ++m) {
+                        if (cex[m]) {
+                            if (CPL == 2) cp_async_8(drow + doff[m], srow + joff[m], (rin && cin[m]) ? 8 : 0);
+                            else cp_async_4(drow + doff[m], srow + joff[m], (rin && cin[m]) ? 4 : 0);
+                        }
+                    }
+                    if (++pos == ring) pos = 0;
                 }
+                loaded = need_hi + 1;
+            }
+            cp_async_wait_all();
+            __syncwarp();
+
+            const int t = t0 + lane;
+            if (t < I.n_tiles) {
+                const int tsa = t / naf, tf = t - tsa * naf;
+                float acc[RS][RF];
 #pragma unroll
-                for (int ii = 0; ii < RS; ++ii) {
-                    const int di = y - ii;
-                    if (di >= 0 && di < KT) {
-                        const float4 *w4 = reinterpret_cast<const float4 *>(Ws + di * KP);
+                for (int ii = 0; ii < RS; ++ii)
 #pragma unroll
-                        for (int q = 0; q < KP / 4; ++q) {
-                            const float4 wq4 = w4[q];
-                            const float wq[4] = { wq4.x, wq4.y, wq4.z, wq4.w };
+                    for (int r = 0; r < RF; ++r) acc[ii][r] = 0.f;
+                // forward: input rows outside S_k hold zeros (structurally zero fluence) and are skipped
+                const int ylo = ADJ ? 0 : max(0, I.S.u0 - I.tu0 - tsa * RS), yhi = ADJ ? KT + RS - 2 : min(KT + RS - 2, I.S.u1 - I.tu0 - tsa * RS);
+                const float *xrow = tile + ((tsa * RS + ylo) % ring) * pitch;
+                int xoff[NXQ];
 #pragma unroll
-                            for (int e = 0; e < 4; ++e) {
-                                const int dj = 4 * q + e;
-                                if (dj < KT) {
+                for (int q = 0; q < NXQ; ++q) xoff[q] = swz_col(tf * RF + 4 * q);
+#pragma unroll 1
+                for (int y = ylo; y <= yhi; ++y) {
+                    float x[XW];
 #pragma unroll
-                                    for (int r = 0; r < RF; ++r) acc[ii][r] = fmaf(wq[e], x[r + dj], acc[ii][r]);
+                    for (int q = 0; q < NXQ; ++q) {
+                        const float4 v = *reinterpret_cast<const float4 *>(xrow + xoff[q]);
+                        x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
+                    }
+#pragma unroll
+                    for (int ii = 0; ii < RS; ++ii) {
+                        const int di = y - ii;
+                        if (di >= 0 && di < KT) {
+                            const float4 *w4 = reinterpret_cast<const float4 *>(Ws + di * KP);
+#pragma unroll
+                            for (int q = 0; q < KP / 4; ++q) {
+                                const float4 wq4 = w4[q];
+                                const float wq[4] = { wq4.x, wq4.y, wq4.z, wq4.w };
+#pragma unroll
+                                for (int e = 0; e < 4; ++e) {
+                                    const int dj = 4 * q + e;
+                                    if (dj < KT) {
+#pragma unroll
+                                        for (int r = 0; r < RF; ++r) acc[ii][r] = fmaf(wq[e], x[r + dj], acc[ii][r]);
+                                    }
                                 }
                             }
                         }
                     }
+                    xrow += pitch;
+                    if (xrow == tile_end) xrow = tile;
                 }
-                xrow += pitch;
-            }
 #pragma unroll
-            for (int ii = 0; ii < RS; ++ii) {
-                float4 *o = reinterpret_cast<float4 *>(oslice + (size_t)((I.ats0 + tsa) * RS + ii) * I.pv + (I.atf0 + tf) * RF);
-                o[0] = make_float4(acc[ii][0], acc[ii][1], acc[ii][2], acc[ii][3]);
-                o[1] = make_float4(acc[ii][4], acc[ii][5], acc[ii][6], acc[ii][7]);
+                for (int ii = 0; ii < RS; ++ii) {
+                    float4 *o = reinterpret_cast<float4 *>(oslice + (size_t)((I.ats0 + tsa) * RS + ii) * I.pv + (I.atf0 + tf) * RF);
+                    o[0] = make_float4(acc[ii][0], acc[ii][1], acc[ii][2], acc[ii][3]);
+                    o[1] = make_float4(acc[ii][4], acc[ii][5], acc[ii][6], acc[ii][7]);
+                }
             }
         }
-        __syncwarp();                                  // the next unit overwrites the tile and the slice kernel
+        __syncwarp();                                  // the next item overwrites the rows and the slice kernel
     }
 }
 

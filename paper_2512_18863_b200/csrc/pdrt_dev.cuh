@@ -78,8 +78,8 @@ struct CpDesc {
     int ri0, rj0, pu, pv;        // compact region origin and extents (rj0 % 8 == 0, pv % 8 == 0, pu % RS == 0)
     int ntf, nts;                // region size in thread-tiles: RF along v (fast), RS along u (slow)
     int ncf, ntfc;               // conv chunks along v and their width [thread-tiles]
-    int nuc_fwd, nuc_adj;        // conv units (<= 32 active thread-tiles each) per slice and chunk: bound over the slices
-    int n_items, n_items_adj;    // Nw * ncf * nuc conv work units, forward / adjoint (0 when empty)
+    int nuc_fwd, nuc_adj;        // (reserved)
+    int n_items, n_items_adj;    // Nw * ncf conv work items, forward / adjoint (0 when empty)
     unsigned long long support_vox, footprint_vox, region_vox, macs_fwd, macs_adj;
 };
 

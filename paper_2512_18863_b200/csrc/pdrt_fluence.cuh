@@ -76,15 +76,9 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     d.nts = d.pu / RS;
     d.ncf = (d.ntf + NTFC_MAX - 1) / NTFC_MAX;
     d.ntfc = (d.ntf + d.ncf - 1) / d.ncf;
-    // units: the active thread-tiles of a slice (F_k forward, S_k adjoint; both grow monotonically with k) in row-major
-    // order, 32 at a time; the count per slice is bounded by the larger of the two end slices
-    const SliceBox f0 = dilate(P, s0, C), f1 = dilate(P, s1, C);
-    const int nsf = max((f0.u1 - d.ri0) / RS - (f0.u0 - d.ri0) / RS, (f1.u1 - d.ri0) / RS - (f1.u0 - d.ri0) / RS) + 1;
-    const int nsa = max((s0.u1 - d.ri0) / RS - (s0.u0 - d.ri0) / RS, (s1.u1 - d.ri0) / RS - (s1.u0 - d.ri0) / RS) + 1;
-    d.nuc_fwd = (d.ntfc * nsf + CONV_CHUNK_TILES - 1) / CONV_CHUNK_TILES;
-    d.nuc_adj = (d.ntfc * nsa + CONV_CHUNK_TILES - 1) / CONV_CHUNK_TILES;
-    d.n_items = P.Nw * d.ncf * d.nuc_fwd;
-    d.n_items_adj = P.Nw * d.ncf * d.nuc_adj;
+    // conv work items: one per slice and chunk along v (the warp that takes an item walks its active thread-tiles)
+    d.nuc_fwd = d.nuc_adj = 1;
+    d.n_items = d.n_items_adj = P.Nw * d.ncf;
     d.region_vox = (unsigned long long)d.pu * d.pv * P.Nw;
 }
 

@@ -124,6 +124,12 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
     // half-extent, in patient indices, of the rotated unit hat of one beam voxel; beam-index increments per patient step
     const float hx = (fabsf(d.cg) * P.du + fabsf(d.sg) * P.dw) / P.sx, hy = (fabsf(d.sg) * P.du + fabsf(d.cg) * P.dw) / P.sy;
     const float fu_x = d.cg * P.sx / P.du, fu_y = d.sg * P.sy / P.du, fw_x = -d.sg * P.sx / P.dw, fw_y = d.cg * P.sy / P.dw;
+    // affine maps, hoisted out of the row loop: patient index of beam voxel (i,k), beam index of patient voxel (x,y)
+    const float fx_i = P.du * d.cg / P.sx, fy_i = P.du * d.sg / P.sy;                       // d fx / d i, d fy / d i
+    const float fx_0 = (P.isox - P.cu * P.du * d.cg - P.ox) / P.sx, fy_0 = (P.isoy - P.cu * P.du * d.sg - P.oy) / P.sy;
+    const float fx_w = -d.sg / P.sx, fy_w = d.cg / P.sy;                                    // d fx / d w, d fy / d w  (w in mm)
+    const float fu_0 = (d.cg * (P.ox - P.isox) + d.sg * (P.oy - P.isoy)) / P.du + P.cu;     // fu(x,y) = fu_0 + x fu_x + y fu_y
+    const float fw_0 = (-d.sg * (P.ox - P.isox) + d.cg * (P.oy - P.isoy) - P.wmin) / P.dw;  // fw(x,y) = fw_0 + x fw_x + y fw_y
     float *Gc = G + (size_t)slot * (size_t)P.stride_cp;
     const int cx = lane % 3, cy = (lane / 3) % 3;
     const bool pairs = (P.nz & 1) == 0;                 // 8-byte alignment of gT[y][x][even j] and of G rows
@@ -132,17 +138,15 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
         const SliceBox F = dilate(P, slice_support(P, d, k), C);
         if (box_empty(F)) continue;
         const float w = P.wmin + k * P.dw;
+        const float fx_k = fx_0 + w * fx_w, fy_k = fy_0 + w * fy_w;
         const int jv0 = F.v0 & ~1, jv1 = F.v1 | 1;      // aligned pairs for the conv's tile copies; the extra columns lie inside
                                                         // the region (rj0 % 8 == 0) and only feed outputs nobody reads
         for (int i = F.u0 + g; i <= F.u1; i += ROW_GROUPS) {
-            const float u = (i - P.cu) * P.du;
-            const float fx = (P.isox + u * d.cg - w * d.sg - P.ox) / P.sx;
-            const float fy = (P.isoy + u * d.sg + w * d.cg - P.oy) / P.sy;
+            const float fx = fx_k + i * fx_i, fy = fy_k + i * fy_i;
             const int xa = max(0, (int)ceilf(fx - hx)), xb = min(P.nx - 1, (int)floorf(fx + hx));
             const int ya = max(0, (int)ceilf(fy - hy)), yb = min(P.ny - 1, (int)floorf(fy + hy));
-            const float dxa = P.ox + xa * P.sx - P.isox, dya = P.oy + ya * P.sy - P.isoy;
-            const float eu0 = (d.cg * dxa + d.sg * dya) / P.du + P.cu - (float)i;
-            const float ew0 = (-d.sg * dxa + d.cg * dya - P.wmin) / P.dw - (float)k;
+            const float eu0 = fu_0 + xa * fu_x + ya * fu_y - (float)i;
+            const float ew0 = fw_0 + xa * fw_x + ya * fw_y - (float)k;
             float *orow = Gc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
             if (xb - xa <= 2 && yb - ya <= 2) {
                 // usual case (beam spacing ~ patient spacing): at most 3 x 3 candidates

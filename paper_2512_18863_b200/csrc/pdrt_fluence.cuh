@@ -10,6 +10,7 @@
 namespace pdrt {
 
 constexpr int FLU_THREADS = 256;
+constexpr int FLU_MAX_ROWS = 1024;   // pixel rows of a jaw opening with a precomputed leaf range (wider maps scan all pairs)
 
 __device__ __forceinline__ float flu_u(const Params &P, int a) { return (a - P.cuf) * P.Du; }
 __device__ __forceinline__ float flu_v(const Params &P, int b) { return (b - P.cvf) * P.Dv; }
@@ -126,13 +127,27 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
     const int bw = d.a1 - d.a0 + 1, bh = d.b1 - d.b0 + 1, npx = bw * bh;
     const float x1 = jw[0], x2 = jw[1], y1 = jw[2], y2 = jw[3];
 
+    // leaf pairs that can overlap each pixel row of the jaw opening (the bounds are ascending): once per row
+    __shared__ short leaf_lo[FLU_MAX_ROWS], leaf_hi[FLU_MAX_ROWS];
+    const bool ranged = d.jb1 - d.jb0 < FLU_MAX_ROWS;
+    if (ranged) {
+        for (int r = tid; r <= d.jb1 - d.jb0; r += FLU_THREADS) {
+            const float vf = flu_v(P, d.jb0 + r), vlo = vf - 0.5f * P.Dv, vhi = vf + 0.5f * P.Dv;
+            int lo = 0, hi = P.Np - 1;
+            while (lo < P.Np && T.leaf_bounds[lo + 1] <= vlo) ++lo;
+            while (hi >= 0 && T.leaf_bounds[hi] >= vhi) --hi;
+            leaf_lo[r] = (short)lo; leaf_hi[r] = (short)hi;
+        }
+    }
+    __syncthreads();
     // O1, O2: A, J, Phi0
     for (int p = tid; p < npx; p += FLU_THREADS) {
         const int a = d.a0 + p % bw, b = d.b0 + p / bw;
         float A = 0.f, J = 0.f;
         if (a >= d.ja0 && a <= d.ja1 && b >= d.jb0 && b <= d.jb1) {
             const float uf = flu_u(P, a), vf = flu_v(P, b);
-            for (int i = 0; i < P.Np; ++i) {
+            const int i0 = ranged ? leaf_lo[b - d.jb0] : 0, i1 = ranged ? leaf_hi[b - d.jb0] : P.Np - 1;
+            for (int i = i0; i <= i1; ++i) {
                 const float ovv = ov(vf, P.Dv, T.leaf_bounds[i], T.leaf_bounds[i + 1]);
                 if (ovv != 0.f) A += ovv * ov(uf, P.Du, lv[i], lv[P.Np + i]);
             }

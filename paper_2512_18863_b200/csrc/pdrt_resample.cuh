@@ -177,7 +177,7 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, cons
 // memory in a fixed order (deterministic, no atomics).
 struct SliceGeo { float mag, su, sv, iu, iv; int u0, u1, v0, v1; };   // su = mag*du/Du, iu = Du/(mag*du)
 
-constexpr int PROJ_THREADS = 256, PROJ_KG = PROJ_THREADS / 32, PROJ_A = 8;
+constexpr int PROJ_THREADS = 256, PROJ_KG = PROJ_THREADS / 32, PROJ_A = 8, PROJ_TAPS = 4;
 
 __global__ void __launch_bounds__(PROJ_THREADS)
 k_project_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ H,
@@ -222,12 +222,29 @@ k_project_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, 
         int jlo = max(q.v0, (int)floorf((b - 1 - P.cvf) * q.iv - vb)), jhi = min(q.v1, (int)ceilf((b + 1 - P.cvf) * q.iv - vb));
         if (!live) jhi = jlo - 1;
         const float m2 = q.mag * q.mag;
+        // v weights of this lane's (at most PROJ_TAPS) voxels, once per slice; wider stencils (beam voxels much finer than the
+        // map pixels) take the general loop
+        const bool few = __all_sync(0xffffffffu, jhi - jlo < PROJ_TAPS);
+        float wbq[PROJ_TAPS];
+#pragma unroll
+        for (int e = 0; e < PROJ_TAPS; ++e) {
+            const float wb = 1.f - fabsf((vb + jlo + e) * q.sv + P.cvf - (float)b);
+            wbq[e] = (jlo + e <= jhi && wb > 0.f) ? wb : 0.f;
+        }
         for (int i = ilo; i <= ihi; ++i) {
             const float *hrow = Hc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
             float t = 0.f;
-            for (int j = jlo; j <= jhi; ++j) {
-                const float wb = 1.f - fabsf((vb + j) * q.sv + P.cvf - (float)b);
-                if (wb > 0.f) t = fmaf(wb, __ldg(hrow + j), t);
+            if (few) {
+                float hv[PROJ_TAPS];
+#pragma unroll
+                for (int e = 0; e < PROJ_TAPS; ++e) hv[e] = wbq[e] != 0.f ? __ldg(hrow + jlo + e) : 0.f;
+#pragma unroll
+                for (int e = 0; e < PROJ_TAPS; ++e) t = fmaf(wbq[e], hv[e], t);
+            } else {
+                for (int j = jlo; j <= jhi; ++j) {
+                    const float wb = 1.f - fabsf((vb + j) * q.sv + P.cvf - (float)b);
+                    if (wb > 0.f) t = fmaf(wb, __ldg(hrow + j), t);
+                }
             }
             t *= m2;
             const float fa = (i - P.cu) * q.su + P.cuf - (float)A0;      // uniform across the warp

@@ -205,6 +205,7 @@ struct ConvItem {
     SliceBox S, B;                   // fluence support of the slice; source box of the input rows (S forward, F adjoint)
     int ctf0, ctf1;                  // thread-tile range of the chunk along v
     int atf0, ats0, naf, nas;        // active thread-tiles of the slice and chunk (outputs to compute)
+    int av0;                         // v index of the first active output column (forward: tile-aligned; adjoint: S.v0 & ~1)
     int n_tiles;                     // naf * nas
     int pitch, ring, tv0, tu0;       // input rows: pitch, rows the ring holds, input coords of window row 0 / column 0
     int n0;                          // slice kernel: table node and fraction
@@ -239,10 +240,17 @@ __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__
     }
     const bool any = atf0 <= atf1 && ats0 <= ats1;
     it.atf0 = atf0; it.ats0 = ats0; it.naf = any ? atf1 - atf0 + 1 : 0; it.nas = any ? ats1 - ats0 + 1 : 0;
+    it.av0 = d.rj0 + atf0 * RF;
+    if (ADJ && any && d.ncf == 1) {
+        // adjoint outputs are read back only on S_k: start the thread-tiles at S.v0 (even, for the paired copies) instead of
+        // the region's tile grid, which saves the partly used tile column at either end
+        it.av0 = A.v0 & ~1;
+        it.naf = (A.v1 - it.av0) / RF + 1;
+    }
     it.n_tiles = it.naf * it.nas;
     it.pitch = conv_pitch(KT, max(it.naf, 1));
     it.ring = P.tile_floats / it.pitch;
-    it.tv0 = d.rj0 + atf0 * RF - C; it.tu0 = d.ri0 + ats0 * RS - C;
+    it.tv0 = it.av0 - C; it.tu0 = d.ri0 + ats0 * RS - C;
     it.n0 = 0; it.f = 0.f;
     if (!any) return;
     // S4: slice kernel = lerp of the table in radiological depth
@@ -406,9 +414,17 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                 }
 #pragma unroll
                 for (int ii = 0; ii < RS; ++ii) {
-                    float4 *o = reinterpret_cast<float4 *>(oslice + (size_t)((I.ats0 + tsa) * RS + ii) * I.pv + (I.atf0 + tf) * RF);
-                    o[0] = make_float4(acc[ii][0], acc[ii][1], acc[ii][2], acc[ii][3]);
-                    o[1] = make_float4(acc[ii][4], acc[ii][5], acc[ii][6], acc[ii][7]);
+                    float *op = oslice + (size_t)((I.ats0 + tsa) * RS + ii) * I.pv + (I.av0 - I.rj0) + tf * RF;
+                    if (ADJ) {                     // 8-byte aligned only; columns past the region are never read
+                        const int room = I.pv - ((I.av0 - I.rj0) + tf * RF);
+#pragma unroll
+                        for (int r = 0; r < RF; r += 2)
+                            if (r + 2 <= room) *reinterpret_cast<float2 *>(op + r) = make_float2(acc[ii][r], acc[ii][r + 1]);
+                    } else {
+                        float4 *o = reinterpret_cast<float4 *>(op);
+                        o[0] = make_float4(acc[ii][0], acc[ii][1], acc[ii][2], acc[ii][3]);
+                        o[1] = make_float4(acc[ii][4], acc[ii][5], acc[ii][6], acc[ii][7]);
+                    }
                 }
             }
         }

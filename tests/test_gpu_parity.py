@@ -270,3 +270,49 @@ def test_config5_double_arc_sampled(torch):
     check_sampled_dose(eng, orc, wl, 120, 6, "c5")
     g = W.seeded_dose_gradient(wl, seed=6)
     check_sampled_gradients(eng, orc, wl, g, [0, 200, 355], "c5")
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Code paths the standard cases do not reach
+@pytest.mark.parametrize("beam", [
+    dict(beam_nu=52, beam_nw=70, beam_du=2.1, beam_dw=1.6, beam_wmin=-55.0),     # finer than the patient grid: > 3 x 3 candidates in S7
+    dict(beam_nu=24, beam_nw=20, beam_du=5.5, beam_dw=6.0, beam_wmin=-58.0),     # coarser than the patient grid
+], ids=["fine_beam_grid", "coarse_beam_grid"])
+def test_beam_grid_that_differs_from_the_patient_grid(torch, beam):
+    """Explicit beam grids with du, dw != sx: the general candidate loop of k_resample_adjoint, bilinear stencils that skip
+    or repeat beam voxels in k_gather_dose, and map pixels much coarser / finer than beam voxels in S3 / S9."""
+    wl = W.tiny(seed=31, nx=30, ny=26, nz=14, spacing=4.0, n_cp=3, kernel_size=7, flu=(22, 18), explicit_beam=beam)
+    eng, orc = pair(wl)
+    assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), "dose")
+    g = W.seeded_dose_gradient(wl, seed=31)
+    dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    assert_grad(dm, rm, "d_mu"); assert_grad(dj, rj, "d_jaws"); assert_grad(dl, rl, "d_leaves")
+
+
+def test_control_points_in_several_batches(torch, monkeypatch):
+    """A scratch cap smaller than the arc (PDRT_SCRATCH_GB) makes the engine run the control points in batches: the
+    resampler accumulates into the dose grid across launches and the gradients of later batches use their own blocks."""
+    wl = W.tiny(seed=32, n_cp=7, nx=36, ny=30, nz=16, kernel_size=5, flu=(24, 20))
+    monkeypatch.setenv("PDRT_SCRATCH_GB", "0.0005")          # room for two or three control points per batch
+    eng, orc = pair(wl)
+    assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), "batched dose")
+    g = W.seeded_dose_gradient(wl, seed=32)
+    dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    assert_grad(dm, rm, "batched d_mu"); assert_grad(dj, rj, "batched d_jaws"); assert_grad(dl, rl, "batched d_leaves")
+    n_batches = eng.get_stage_ms()[1]["conv_adj"]
+    assert n_batches >= 2, f"expected several batches, got {n_batches} conv launches"
+
+
+def test_results_are_bit_reproducible(torch):
+    """No atomics on the data path and fixed summation orders: two runs give identical bits."""
+    wl = W.tiny(seed=33, n_cp=6, nx=40, ny=36, nz=20, kernel_size=9, flu=(28, 24))
+    eng, _ = pair(wl)
+    g = W.seeded_dose_gradient(wl, seed=33)
+    d1 = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu).clone()
+    b1 = [t.clone() for t in eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)]
+    d2 = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
+    b2 = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    assert torch.equal(d1, d2)
+    assert all(torch.equal(a, b) for a, b in zip(b1, b2))

@@ -285,8 +285,10 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
     constexpr int PMAX = (NTFC_MAX * RF + XW - RF + 7) & ~7;   // widest row
     constexpr int MC = (PMAX / CPL + 31) / 32;        // copies per lane and row
     extern __shared__ float4 smem4[];
-    float *Ws = reinterpret_cast<float *>(smem4);     // slice kernel [KT (du)][KP (dv)]
-    float *tile = Ws + KT * KP;                       // ring of input rows [ring][pitch (v)]
+    // slice kernel as row pairs: Ws2[y][dj] = (W[y][dj], W[y-1][dj]), y = 0..KT, zero where the row does not exist — the two
+    // weights an input row y contributes to the two output rows of a thread-tile, ready for one packed FFMA2
+    float2 *Ws2 = reinterpret_cast<float2 *>(smem4);  // [(KT + 1) (du)][KP (dv)]
+    float *tile = reinterpret_cast<float *>(smem4) + 2 * (KT + 1) * KP;   // ring of input rows [ring][pitch (v)]
     const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
     const int lane = threadIdx.x;
     const int total = tile_base[n_cp];
@@ -318,12 +320,13 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
         const int pitch = I.pitch, ring = I.ring, naf = I.naf;
         {   // S4: slice kernel = lerp of the table in radiological depth; the table is stored as the [du][dv] image and is
             // point-symmetric, so forward and adjoint (flipped kernel) read the same entries
-            const float4 *w0 = reinterpret_cast<const float4 *>(wtab + (size_t)I.n0 * KT * KP), *w1 = w0 + KT * KP / 4;
+            const float *w0 = wtab + (size_t)I.n0 * KT * KP, *w1 = w0 + KT * KP;
             const float f = I.f;
-            float4 *Ws4 = reinterpret_cast<float4 *>(Ws);
-            for (int e = lane; e < KT * KP / 4; e += 32) {
-                const float4 a = __ldg(w0 + e), b = __ldg(w1 + e);
-                Ws4[e] = make_float4((1.f - f) * a.x + f * b.x, (1.f - f) * a.y + f * b.y, (1.f - f) * a.z + f * b.z, (1.f - f) * a.w + f * b.w);
+            for (int e = lane; e < (KT + 1) * KP; e += 32) {
+                const int y = e / KP;
+                const float hi = y < KT ? (1.f - f) * __ldg(w0 + e) + f * __ldg(w1 + e) : 0.f;
+                const float lo = y > 0 ? (1.f - f) * __ldg(w0 + e - KP) + f * __ldg(w1 + e - KP) : 0.f;
+                Ws2[e] = make_float2(hi, lo);
             }
         }
         // column terms of the row copies (source offset, swizzled destination, validity): once per slice
@@ -370,48 +373,48 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
             const int t = t0 + lane;
             if (t < I.n_tiles) {
                 const int tsa = t / naf, tf = t - tsa * naf;
-                float acc[RS][RF];
+                static_assert(RS == 2, "the packed FFMA2 loop pairs the two output rows of a thread-tile");
+                float2 acc2[RF];                   // (row 0, row 1) of output column r
 #pragma unroll
-                for (int ii = 0; ii < RS; ++ii)
-#pragma unroll
-                    for (int r = 0; r < RF; ++r) acc[ii][r] = 0.f;
+                for (int r = 0; r < RF; ++r) acc2[r] = make_float2(0.f, 0.f);
                 // forward: input rows outside S_k hold zeros (structurally zero fluence) and are skipped
                 const int ylo = ADJ ? 0 : max(0, I.S.u0 - I.tu0 - tsa * RS), yhi = ADJ ? KT + RS - 2 : min(KT + RS - 2, I.S.u1 - I.tu0 - tsa * RS);
                 const float *xrow = tile + ((tsa * RS + ylo) % ring) * pitch;
                 int xoff[NXQ];
 #pragma unroll
                 for (int q = 0; q < NXQ; ++q) xoff[q] = swz_col(tf * RF + 4 * q);
+                const float4 *w4 = reinterpret_cast<const float4 *>(Ws2 + ylo * KP);
 #pragma unroll 1
                 for (int y = ylo; y <= yhi; ++y) {
-                    float x[XW];
+                    float2 xx[XW];                 // window element duplicated: it multiplies the weights of both output rows
 #pragma unroll
                     for (int q = 0; q < NXQ; ++q) {
                         const float4 v = *reinterpret_cast<const float4 *>(xrow + xoff[q]);
-                        x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
+                        xx[4 * q] = make_float2(v.x, v.x); xx[4 * q + 1] = make_float2(v.y, v.y);
+                        xx[4 * q + 2] = make_float2(v.z, v.z); xx[4 * q + 3] = make_float2(v.w, v.w);
                     }
+                    // one FFMA2 (fma.rn.f32x2) does the two multiply-adds of a tap for both output rows: half the issue
+                    // slots of scalar FFMA, which leaves room for the LDS and address instructions beside a busy FMA pipe
 #pragma unroll
-                    for (int ii = 0; ii < RS; ++ii) {
-                        const int di = y - ii;
-                        if (di >= 0 && di < KT) {
-                            const float4 *w4 = reinterpret_cast<const float4 *>(Ws + di * KP);
+                    for (int q = 0; q < KP / 2; ++q) {
+                        const float4 wq4 = w4[q];
+                        const float2 wq[2] = { make_float2(wq4.x, wq4.y), make_float2(wq4.z, wq4.w) };
 #pragma unroll
-                            for (int q = 0; q < KP / 4; ++q) {
-                                const float4 wq4 = w4[q];
-                                const float wq[4] = { wq4.x, wq4.y, wq4.z, wq4.w };
+                        for (int e = 0; e < 2; ++e) {
+                            const int dj = 2 * q + e;
+                            if (dj < KT) {
 #pragma unroll
-                                for (int e = 0; e < 4; ++e) {
-                                    const int dj = 4 * q + e;
-                                    if (dj < KT) {
-#pragma unroll
-                                        for (int r = 0; r < RF; ++r) acc[ii][r] = fmaf(wq[e], x[r + dj], acc[ii][r]);
-                                    }
-                                }
+                                for (int r = 0; r < RF; ++r) acc2[r] = __ffma2_rn(xx[r + dj], wq[e], acc2[r]);
                             }
                         }
                     }
+                    w4 += KP / 2;
                     xrow += pitch;
                     if (xrow == tile_end) xrow = tile;
                 }
+                float acc[RS][RF];
+#pragma unroll
+                for (int r = 0; r < RF; ++r) { acc[0][r] = acc2[r].x; acc[1][r] = acc2[r].y; }
 #pragma unroll
                 for (int ii = 0; ii < RS; ++ii) {
                     float *op = oslice + (size_t)((I.ats0 + tsa) * RS + ii) * I.pv + (I.av0 - I.rj0) + tf * RF;

@@ -43,7 +43,7 @@ int tile_floats_for(int kt)
     return best;
 }
 constexpr int ROW_BLOCKS = 16;        // blocks per control point of the row-per-warp kernels (k_project, k_resample_adjoint)
-size_t conv_smem_bytes(int kt) { return sizeof(float) * ((size_t)kt * ((kt + 3) & ~3) + tile_floats_for(kt)); }
+size_t conv_smem_bytes(int kt) { return sizeof(float) * (2 * (size_t)(kt + 1) * ((kt + 3) & ~3) + tile_floats_for(kt)); }   // row-pair kernel + ring
 
 template <typename T> struct DevBuf {
     T *p = nullptr;

@@ -351,19 +351,27 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
             __syncwarp();                                                  // rows below need_lo are free to be overwritten
             {
                 int w = max(loaded, need_lo), pos = w % ring;
+                // per-lane source pointers and destination offsets advance by one row per iteration (no 64-bit
+                // multiplies in the loop); rows outside the source box read nothing (size 0) from the slice start
+                const float *sp[MC];
+#pragma unroll
+                for (int m = 0; m < MC; ++m) sp[m] = sbase + (long long)(I.tu0 + w - I.ri0) * I.pv + joff[m];
+                unsigned drow = tile_s + 4u * (unsigned)(pos * pitch);
+                const unsigned dstep = 4u * (unsigned)pitch, dend = tile_s + 4u * (unsigned)(ring * pitch);
                 for (; w <= need_hi; ++w) {
                     const int i = I.tu0 + w;
                     const bool rin = i >= I.B.u0 && i <= I.B.u1;
-                    const float *srow = sbase + (rin ? (i - I.ri0) * I.pv : 0);
-                    const unsigned drow = tile_s + 4u * (unsigned)(pos * pitch);
 #pragma unroll
                     for (int m = 0; m < MC; ++m) {
                         if (cex[m]) {
-                            if (CPL == 2) cp_async_8(drow + doff[m], srow + joff[m], (rin && cin[m]) ? 8 : 0);
-                            else cp_async_4(drow + doff[m], srow + joff[m], (rin && cin[m]) ? 4 : 0);
+                            const bool ok = rin && cin[m];
+                            if (CPL == 2) cp_async_8(drow + doff[m], ok ? sp[m] : sbase, ok ? 8 : 0);
+                            else cp_async_4(drow + doff[m], ok ? sp[m] : sbase, ok ? 4 : 0);
                         }
+                        sp[m] += I.pv;
                     }
-                    if (++pos == ring) pos = 0;
+                    drow += dstep;
+                    if (drow == dend) drow = tile_s;
                 }
                 loaded = need_hi + 1;
             }

@@ -12,8 +12,9 @@
 // source box).
 //
 // The convolution is bound by the FP32 FMA pipe (k^2 multiply-adds per 4-byte output), so the
-// kernel is organised around FFMA issue slots: each thread owns an RF x RS = 8(v) x 2(u) register tile,
-// slides a (K+7)-wide register window along v (LDS.128), and takes weights as warp-broadcast LDS.128.
+// kernel is organised around FMA-pipe cycles: each thread owns an RF x RS = 8(v) x 2(u) register tile, slides a
+// (K+7)-wide register window along v (LDS.128), takes weight PAIRS as warp-broadcast LDS.128 and issues packed
+// FFMA2 (fma.rn.f32x2: both output rows of the thread-tile in one instruction).
 // Work items (control point, slice, chunk) come from device-built descriptors, so nothing about the
 // aperture is known to or synchronised with the host; the grid is persistent (a multiple of the SM count)
 // and strides over the item list.

@@ -2,7 +2,7 @@
 // Eq. 9) and S9 (transpose of the divergent projection, Eq. 5-6, in gather form).  These are the
 // bandwidth-bound stages: each patient voxel is written once per call (accumulation over control points
 // stays in registers), the compact D_b blocks are read once as 16-byte vectors along v, and no global
-// atomics are used anywhere.  (S7, the transpose of S6, lives in the tile fill of k_conv<K,true>.)
+// atomics are used anywhere.  (S7, the transpose of S6, is k_resample_adjoint in pdrt_conv.cuh.)
 #pragma once
 #include "pdrt_dev.cuh"
 
@@ -21,7 +21,7 @@ struct GatherCp {                       // the slice of CpDesc the resampler nee
     long long base;                     // slot * stride_cp
 };
 
-// S6.  Grid: (ceil(nx/16), ceil(ny/16), ceil(nz/32)); a block owns 16 x 16 patient columns (x,y) times 32
+// S6.  Grid: (ceil(nx/16), ceil(ny/4), ceil(nz/32)); a block owns 16 x 4 patient columns (x,y) times 32
 // z-slices, a warp an 8(x) x 4(y) patch of columns (compact in the beam frame under any gantry rotation).
 //   dose[p] (+)= sum_b scale_b * bilinear_0(D_b[.][z][.]; fu, fw)
 // The gantry rotates about z (G1), so for one control point the beam-frame position (fu, fw) and the

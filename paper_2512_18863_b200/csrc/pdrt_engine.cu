@@ -42,7 +42,8 @@ int tile_floats_for(int kt)
     }
     return best;
 }
-constexpr int ROW_BLOCKS = 16;        // blocks per control point of the row-per-warp kernels (k_project, k_resample_adjoint)
+// blocks per control point of the row-group kernels (k_project, k_resample_adjoint): four (slice, row group) units per warp
+int row_blocks(const Params &P) { return std::max(1, (P.Nw * ROW_GROUPS + 31) / 32); }
 size_t conv_smem_bytes(int kt) { return sizeof(float) * (2 * (size_t)(kt + 1) * ((kt + 3) & ~3) + tile_floats_for(kt)); }   // row-pair kernel + ring
 
 template <typename T> struct DevBuf {
@@ -304,7 +305,7 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
         CU(e, cudaGetLastError());
         {
             StageTimer t(e, PDRT_STAGE_PROJECT, st);
-            k_project<<<dim3(ROW_BLOCKS, n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, e->phimapT.p, e->bufB.p);
+            k_project<<<dim3(row_blocks(e->P), n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, e->phimapT.p, e->bufB.p);
         }
         CU(e, cudaGetLastError());
         {
@@ -350,7 +351,7 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
         CU(e, cudaGetLastError());
         {
             StageTimer t(e, PDRT_STAGE_RESAMPLE_ADJ, st);
-            k_resample_adjoint<<<dim3(ROW_BLOCKS, n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, (e->P.KT - 1) / 2, e->gT.p, e->bufB.p);
+            k_resample_adjoint<<<dim3(row_blocks(e->P), n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, (e->P.KT - 1) / 2, e->gT.p, e->bufB.p);
         }
         CU(e, cudaGetLastError());
         {
@@ -668,7 +669,7 @@ int pdrt_stage_beam_dose(pdrt_engine *e, const float *leaves, const float *jaws,
     CU(e, e->bufB.ensure((size_t)e->P.stride_cp));
     k_scan_items<<<1, 256, 0, st>>>(e->desc.p, 0, 1, 0, e->tile_base.p, e->counters.p);
     CU(e, cudaGetLastError());
-    k_project<<<dim3(ROW_BLOCKS, 1), 256, 0, st>>>(e->P, e->desc.p, 0, 1, e->phimapT.p, e->bufB.p);
+    k_project<<<dim3(row_blocks(e->P), 1), 256, 0, st>>>(e->P, e->desc.p, 0, 1, e->phimapT.p, e->bufB.p);
     CU(e, cudaGetLastError());
     if ((rc = launch_conv<false>(e, 0, 1, e->bufB.p, e->bufA.p, st))) return rc;
     k_expand_dense<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, 0, 0, e->bufA.p, db);

@@ -75,6 +75,7 @@ class Oracle:
     model: dict
     density: np.ndarray
     _keep: list = field(default_factory=list, repr=False)
+    _tables: dict = field(default_factory=dict, repr=False)
 
     def __post_init__(self):
         self.lib = C.CDLL(build())
@@ -131,6 +132,13 @@ class Oracle:
     def set_kernel_size(self, k: int):
         self.m["kernel_size"] = int(k)
         self.M.kernel_size = int(k)
+
+    def _w_tab(self):
+        """orc_kernel_table for the current kernel size, built once per size (the table depends on nothing else)."""
+        k = int(self.m["kernel_size"])
+        if k not in self._tables:
+            self._tables[k] = _d(self.kernel_table())
+        return self._tables[k]
 
     def num_threads(self) -> int:
         return int(self.lib.orc_num_threads())
@@ -230,7 +238,7 @@ class Oracle:
         return out
 
     def beam_dose(self, leaves, jaws, gantry_deg, W_tab=None):
-        Wt = _d(self.kernel_table() if W_tab is None else W_tab)
+        Wt = self._w_tab() if W_tab is None else _d(W_tab)
         lv, jw = _d(leaves), _d(jaws)
         out = np.zeros(self.beam_shape)
         self.lib.orc_beam_dose(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), _p(Wt),
@@ -247,7 +255,7 @@ class Oracle:
     def dose(self, leaves, jaws, gantry_deg, mu):
         n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)
         out = np.zeros(self.dose_shape)
-        self.lib.orc_dose(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), C.c_int(n_cp),
+        self.lib.orc_dose(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), _p(self._w_tab()), C.c_int(n_cp),
                           _p(lv), _p(jw), _p(ga), _p(mu), _p(out))
         return out
 
@@ -257,7 +265,7 @@ class Oracle:
         assert g.shape == self.dose_shape
         dl, dj, dm = np.zeros_like(lv), np.zeros_like(jw), np.zeros_like(mu)
         self.lib.orc_dose_backward(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p),
-                                   C.c_int(n_cp), _p(lv), _p(jw), _p(ga), _p(mu), g.ctypes.data_as(C.c_void_p),
+                                   _p(self._w_tab()), C.c_int(n_cp), _p(lv), _p(jw), _p(ga), _p(mu), g.ctypes.data_as(C.c_void_p),
                                    _p(dl), _p(dj), _p(dm))
         return dl, dj, dm
 
@@ -266,7 +274,7 @@ class Oracle:
         n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)
         ijk = np.ascontiguousarray(ijk, dtype=np.int32)
         out = np.zeros(ijk.shape[0])
-        self.lib.orc_dose_at(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), C.c_int(n_cp),
+        self.lib.orc_dose_at(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), _p(self._w_tab()), C.c_int(n_cp),
                              _p(lv), _p(jw), _p(ga), _p(mu), C.c_int(ijk.shape[0]),
                              ijk.ctypes.data_as(C.c_void_p), _p(out))
         return out

@@ -539,37 +539,34 @@ void orc_beam_dose(const orc_grid *g, const orc_model *m, const float *rho, cons
     orc_convolve(g, m, W_tab, z, Phivol, Db);
     free(Phimap); free(Phivol); free(z);
 }
-/* PAPER.md:164-168, Eq. 9:  D_total = cal * sum_b MU_b * R_b D_b   (cal: :178 energy scaling factor). */
-void orc_dose(const orc_grid *g, const orc_model *m, const float *rho, int n_cp,
+/* PAPER.md:164-168, Eq. 9:  D_total = cal * sum_b MU_b * R_b D_b   (cal: :178 energy scaling factor).
+ * W_tab is the table of orc_kernel_table for m->kernel_size (the caller builds it once per kernel size). */
+void orc_dose(const orc_grid *g, const orc_model *m, const float *rho, const double *W_tab, int n_cp,
               const double *leaves, const double *jaws, const double *gantry_deg, const double *mu,
               double *dose)
 {
     const size_t nb = (size_t)m->beam_nu * g->nz * m->beam_nw, np = (size_t)g->nx * g->ny * g->nz;
-    const int K = m->kernel_size;
-    double *W_tab = malloc(sizeof(double) * (size_t)m->n_z * K * K), *Db = malloc(sizeof(double) * nb);
-    orc_kernel_table(m, g->sz, W_tab);
+    double *Db = malloc(sizeof(double) * nb);
     memset(dose, 0, sizeof(double) * np);
     for (int b = 0; b < n_cp; ++b) {
         orc_beam_dose(g, m, rho, W_tab, leaves + (size_t)b * 2 * m->n_pairs, jaws + (size_t)b * 4, gantry_deg[b], Db);
         orc_resample_add(g, m, gantry_deg[b], m->cal * mu[b], Db, dose);
     }
-    free(W_tab); free(Db);
+    free(Db);
 }
 /* O10: dL/d(leaves, jaws, MU) from gdose = dL/dDose, by the transposes in reverse order.
  * Everything after the fluence map is linear and MU is a scalar factor, so
  *   d_mu_b = cal <R_b^T g, D_b> = cal <gPhimap_b, Phimap_b>,  gPhimap_b = P^T C^T R_b^T g,
  *   d(leaves,jaws)_b = cal MU_b * (d Phimap_b / d theta)^T gPhimap_b.
  * Radiological depth and kernels carry no gradient.                   */
-void orc_dose_backward(const orc_grid *g, const orc_model *m, const float *rho, int n_cp,
+void orc_dose_backward(const orc_grid *g, const orc_model *m, const float *rho, const double *W_tab, int n_cp,
                        const double *leaves, const double *jaws, const double *gantry_deg, const double *mu,
                        const float *gdose, double *d_leaves, double *d_jaws, double *d_mu)
 {
     const size_t nb = (size_t)m->beam_nu * g->nz * m->beam_nw, nf = (size_t)m->flu_nu * m->flu_nv;
-    const int K = m->kernel_size, np = m->n_pairs;
-    double *W_tab = malloc(sizeof(double) * (size_t)m->n_z * K * K);
+    const int np = m->n_pairs;
     double *G = malloc(sizeof(double) * nb), *H = malloc(sizeof(double) * nb), *z = malloc(sizeof(double) * m->beam_nw);
     double *Phimap = malloc(sizeof(double) * nf), *gPhimap = malloc(sizeof(double) * nf);
-    orc_kernel_table(m, g->sz, W_tab);
     for (int b = 0; b < n_cp; ++b) {
         const double *lv = leaves + (size_t)b * 2 * np, *jw = jaws + (size_t)b * 4;
         orc_fluence(m, lv, jw, NULL, NULL, NULL, Phimap);
@@ -584,20 +581,18 @@ void orc_dose_backward(const orc_grid *g, const orc_model *m, const float *rho, 
         for (int e = 0; e < 2 * np; ++e) d_leaves[(size_t)b * 2 * np + e] *= m->cal * mu[b];
         for (int e = 0; e < 4; ++e) d_jaws[(size_t)b * 4 + e] *= m->cal * mu[b];
     }
-    free(W_tab); free(G); free(H); free(z); free(Phimap); free(gPhimap);
+    free(G); free(H); free(z); free(Phimap); free(gPhimap);
 }
 
 /* Dose at selected patient voxels only (ijk triplets = x,y,z indices): the same definitions as
  * orc_dose, evaluated one output at a time, so that full-size workloads can be spot-checked.
  * For each point and control point: the 4 beam voxels of the bilinear stencil, each the direct
  * sum of Eq. 8 over the k x k window of projected fluence (Eq. 5-6).                           */
-void orc_dose_at(const orc_grid *g, const orc_model *m, const float *rho, int n_cp,
+void orc_dose_at(const orc_grid *g, const orc_model *m, const float *rho, const double *W_tab, int n_cp,
                  const double *leaves, const double *jaws, const double *gantry_deg, const double *mu,
                  int n_pts, const int *ijk, double *out)
 {
     const int Nu = m->beam_nu, Nv = g->nz, Nw = m->beam_nw, K = m->kernel_size, c = (K - 1) / 2;
-    double *W_tab = malloc(sizeof(double) * (size_t)m->n_z * K * K);
-    orc_kernel_table(m, g->sz, W_tab);
     for (int p = 0; p < n_pts; ++p) out[p] = 0.0;
 #pragma omp parallel
     {
@@ -642,7 +637,6 @@ void orc_dose_at(const orc_grid *g, const orc_model *m, const float *rho, int n_
         for (int p = 0; p < n_pts; ++p) out[p] += part[p];
         free(Phimap); free(z); free(W); free(part);
     }
-    free(W_tab);
 }
 
 #ifdef _OPENMP

@@ -47,8 +47,11 @@
  *   Every function returning int returns PDRT_OK (0) or a negative code; pdrt_last_error gives
  *   the message of the last failure on that engine (or of the last failed pdrt_create when the
  *   engine argument is NULL).  Nothing aborts or throws across this boundary.  Device-resident
- *   parameters are not validated: l_i > r_i is a closed pair by Eq. 4's max(0, .), NaN in gives
- *   NaN out.  There is no CPU fallback: without a CUDA device pdrt_create fails with PDRT_ECUDA.
+ *   parameters are not validated: l_i > r_i is a closed pair by Eq. 4's max(0, .); a control point
+ *   whose jaws are inverted or NaN is a closed field (dose contribution and gradients exactly 0);
+ *   NaN or infinite leaf positions and MU are not detected (NaN MU gives NaN dose; results are
+ *   otherwise unspecified but every access stays in bounds).  There is no CPU fallback: without
+ *   a CUDA device pdrt_create fails with PDRT_ECUDA.
  */
 #ifndef PDRT_H
 #define PDRT_H

@@ -87,6 +87,7 @@ struct pdrt_engine {
     bool last_backward = false;
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
+    int conv_per_sm[2][64] = {};      // resident conv blocks per SM on THIS engine's device, by [adjoint][KT]; 0 = not queried yet
     // per-stage device timing of the most recent call (CUDA events on the call's stream)
     bool profiling = false;
     struct StageRec { int stage; cudaEvent_t a, b; };
@@ -204,7 +205,8 @@ int build_kernel_table(pdrt_engine *e, int k)
 template <int KT, bool ADJ>
 int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
 {
-    static int per_sm = 0;                            // resident blocks per SM, queried once per variant
+    static_assert(KT < 64, "conv_per_sm is indexed by KT");
+    int &per_sm = e->conv_per_sm[ADJ ? 1 : 0][KT];    // per engine (= per device): the opt-in attribute is a per-device setting
     const size_t smem = conv_smem_bytes(KT);
     if (per_sm == 0) {
         CU(e, cudaFuncSetAttribute(k_conv<KT, ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

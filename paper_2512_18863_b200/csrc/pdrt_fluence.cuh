@@ -326,10 +326,11 @@ k_fluence_adjoint(Params P, FluTables T, int n_cp, const float *__restrict__ lea
     for (int e = tid; e < 2 * P.Np; e += FLU_THREADS) {
         const int bank = e / P.Np, i = e % P.Np;
         const float lo = lv[i], hi = lv[P.Np + i];
-        const int ac = bank == 0 ? (int)ceilf((lo - eu) / P.Du) - 1 : (int)floorf((hi - eu) / P.Du);
+        // pixel that holds the edge, clamped in float first: positions are unvalidated (inf, huge values)
+        const float fc = fminf(fmaxf(((bank == 0 ? lo : hi) - eu) / P.Du, -2.f), (float)P.Nuf + 2.f);
+        const int ac = bank == 0 ? (int)ceilf(fc) - 1 : (int)floorf(fc);
         float s = 0.f;
-        for (int a = ac - 1; a <= ac + 1; ++a) {      // the index arithmetic may be off by one at a pixel edge
-            if (a < d.ja0 || a > d.ja1) continue;
+        for (int a = max(ac - 1, d.ja0); a <= min(ac + 1, d.ja1); ++a) {      // the index arithmetic may be off by one at a pixel edge
             const float uf = flu_u(P, a);
             const float dv_ = bank == 0 ? dov_dlo(uf, P.Du, lo, hi) : dov_dhi(uf, P.Du, lo, hi);
             if (dv_ == 0.f) continue;

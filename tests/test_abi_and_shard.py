@@ -1,6 +1,8 @@
 """CPU-side checks (no GPU): the C-ABI library loads and exports every symbol include/pdrt.h declares; the
-control-point sharding of DESIGN.md §9 reproduces the single-process result with world_size 2 over gloo (the
-per-rank compute is the float64 oracle here — test infrastructure — because the CUDA path needs a GPU)."""
+control-point sharding of DESIGN.md §9 (the `ShardedDose` driver that bench.py --gpus N runs on every rank) reproduces
+the single-process result with world_size 2 and 3 over gloo.  The per-rank engine is a stand-in with the Engine's call
+signature that evaluates the float64 oracle — test infrastructure — because the CUDA path needs a GPU; the same driver
+around the CUDA Engine is run with world_size 1 in tests/test_gpu_parity.py."""
 import ctypes
 import os
 import re
@@ -52,36 +54,57 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _worker(rank, world, port, out):
+class _OracleEngine:
+    """Stand-in with the call signature of paper_2512_18863_b200.Engine (torch tensors in, `out=` filled)."""
+
+    def __init__(self, wl):
+        from oracle.oracle import Oracle
+        self.orc = Oracle(wl.grid, wl.model, wl.density)
+        self.dose_shape = self.orc.dose_shape
+
+    def dose(self, leaves, jaws, gantry, mu, out):
+        import torch
+        out.copy_(torch.from_numpy(self.orc.dose(leaves.numpy(), jaws.numpy(), gantry.numpy(), mu.numpy())))
+        return out
+
+    def dose_backward(self, leaves, jaws, gantry, mu, g, out):
+        import torch
+        res = self.orc.dose_backward(leaves.numpy(), jaws.numpy(), gantry.numpy(), mu.numpy(), g.numpy())
+        for o, r in zip(out, res):
+            o.copy_(torch.from_numpy(np.ascontiguousarray(r)))
+        return out
+
+
+def _worker(rank, world, port, out, n_cp):
     import torch
     import torch.distributed as dist
-    from oracle.oracle import Oracle
     from paper_2512_18863_b200 import workloads as W
-    from paper_2512_18863_b200.shard import gather_rows, reduce_dose, shard_range
+    from paper_2512_18863_b200.shard import ShardedDose
     os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
-    wl = W.tiny(seed=21, n_cp=5)
-    orc = Oracle(wl.grid, wl.model, wl.density)
-    lo, hi = shard_range(wl.n_cp, rank, world)
-    part = torch.from_numpy(orc.dose(wl.leaves[lo:hi], wl.jaws[lo:hi], wl.gantry_deg[lo:hi], wl.mu[lo:hi]))
-    dose = reduce_dose(part.clone())
-    g = W.seeded_dose_gradient(wl, seed=21)
-    dl, dj, dm = orc.dose_backward(wl.leaves[lo:hi], wl.jaws[lo:hi], wl.gantry_deg[lo:hi], wl.mu[lo:hi], g)
-    dl, dj, dm = (gather_rows(torch.from_numpy(np.ascontiguousarray(a)), wl.n_cp) for a in (dl, dj, dm))
+    wl = W.tiny(seed=21, n_cp=n_cp)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64))
+    eng = _OracleEngine(wl)
+    sh = ShardedDose(eng, t(wl.leaves), t(wl.jaws), t(wl.gantry_deg), t(wl.mu), eng.dose_shape, rank, world)
+    sh.dose = sh.dose.double()                      # the stand-in is float64
+    dose = sh.forward()
+    sh.backward(torch.from_numpy(W.seeded_dose_gradient(wl, seed=21)))
+    dl, dj, dm = sh.gather()
     if rank == 0:
         np.savez(out, dose=dose.numpy(), dl=dl.numpy(), dj=dj.numpy(), dm=dm.numpy())
     dist.barrier()
     dist.destroy_process_group()
 
 
-def test_sharded_arc_equals_single_process_gloo(tmp_path):
+@pytest.mark.parametrize("world,n_cp", [(2, 5), (3, 2)], ids=["world2", "world3_with_an_empty_rank"])
+def test_sharded_arc_equals_single_process_gloo(tmp_path, world, n_cp):
     import torch.multiprocessing as mp
     from oracle.oracle import Oracle
     from paper_2512_18863_b200 import workloads as W
     out = str(tmp_path / "rank0.npz")
-    mp.spawn(_worker, args=(2, _free_port(), out), nprocs=2, join=True)
+    mp.spawn(_worker, args=(world, _free_port(), out, n_cp), nprocs=world, join=True)
     got = np.load(out)
-    wl = W.tiny(seed=21, n_cp=5)
+    wl = W.tiny(seed=21, n_cp=n_cp)
     orc = Oracle(wl.grid, wl.model, wl.density)
     dose = orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
     g = W.seeded_dose_gradient(wl, seed=21)

@@ -278,3 +278,67 @@ class Oracle:
                              _p(lv), _p(jw), _p(ga), _p(mu), C.c_int(ijk.shape[0]),
                              ijk.ctypes.data_as(C.c_void_p), _p(out))
         return out
+
+
+# ---- planning loop: Eq. 1-3 projection, its transpose, Eq. 10 / quadratic objective,
+# jaw tracking and the normalised-gradient step.  These need no grid or beam model, only the library.
+def _lib():
+    lib = C.CDLL(build())
+    lib.orc_objective.restype = C.c_double
+    lib.orc_mu_epsilon.restype = C.c_double
+    lib.orc_mu_epsilon.argtypes = [C.c_double] * 3
+    return lib
+
+
+def plan_limits(leaf_w_min, leaf_F, jaw_w_min, jaw_Fx, jaw_Fy, mu_eps):
+    """lim[6] of orc_validate: leaf w_min, leaf F, jaw w_min, jaw-x F, jaw-y F, mu_eps."""
+    return _d([leaf_w_min, leaf_F, jaw_w_min, jaw_Fx, jaw_Fy, mu_eps])
+
+
+def validate(lim, leaves, jaws, mu):
+    lv, jw, m, lim = _d(leaves), _d(jaws), _d(mu), _d(lim)
+    n_cp, _, n_pairs = lv.shape
+    out = np.zeros_like(lv), np.zeros_like(jw), np.zeros_like(m)
+    _lib().orc_validate(C.c_int(n_cp), C.c_int(n_pairs), _p(lim), _p(lv), _p(jw), _p(m), _p(out[0]), _p(out[1]), _p(out[2]))
+    return out
+
+
+def validate_adjoint(lim, leaves, jaws, mu, g_leaves_hat, g_jaws_hat, g_mu_hat):
+    lv, jw, m, lim = _d(leaves), _d(jaws), _d(mu), _d(lim)
+    gl, gj, gm = _d(g_leaves_hat), _d(g_jaws_hat), _d(g_mu_hat)
+    n_cp, _, n_pairs = lv.shape
+    out = np.zeros_like(lv), np.zeros_like(jw), np.zeros_like(m)
+    _lib().orc_validate_adjoint(C.c_int(n_cp), C.c_int(n_pairs), _p(lim), _p(lv), _p(jw), _p(m), _p(gl), _p(gj), _p(gm),
+                                _p(out[0]), _p(out[1]), _p(out[2]))
+    return out
+
+
+def mu_epsilon(dose_rate_min, delta_phi, gantry_speed_max):
+    return float(_lib().orc_mu_epsilon(float(dose_rate_min), float(delta_phi), float(gantry_speed_max)))
+
+
+def objective(dose, bits, lam, presc, power):
+    """(L, g): weighted-sum objective (power 1 = Eq. 10, power 2 = quadratic) over structure bit masks and dL/dDose (float32)."""
+    d = np.ascontiguousarray(dose, dtype=np.float32)
+    b = np.ascontiguousarray(bits, dtype=np.uint32)
+    lam, presc = _d(lam), _d(presc)
+    g = np.zeros(d.shape, np.float32)
+    L = _lib().orc_objective(C.c_size_t(d.size), d.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p), C.c_int(len(lam)),
+                             _p(lam), _p(presc), C.c_int(int(power)), g.ctypes.data_as(C.c_void_p))
+    return float(L), g
+
+
+def track_jaws(leaf_bounds, leaves, margin, open_gap):
+    lv, lb = _d(leaves), _d(leaf_bounds)
+    n_cp, _, n_pairs = lv.shape
+    jaws = np.zeros((n_cp, 4))
+    _lib().orc_track_jaws(C.c_int(n_cp), C.c_int(n_pairs), _p(lb), _p(lv), C.c_double(float(margin)), C.c_double(float(open_gap)), _p(jaws))
+    return jaws
+
+
+def plan_step(step_leaf, step_mu, g_leaves, g_mu, leaves, mu):
+    """Returns the updated (leaves, mu); inputs are not modified."""
+    lv, m, gl, gm = _d(leaves).copy(), _d(mu).copy(), _d(g_leaves), _d(g_mu)
+    n_cp, _, n_pairs = lv.shape
+    _lib().orc_plan_step(C.c_int(n_cp), C.c_int(n_pairs), C.c_double(float(step_leaf)), C.c_double(float(step_mu)), _p(gl), _p(gm), _p(lv), _p(m))
+    return lv, m

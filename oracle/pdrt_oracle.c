@@ -645,3 +645,121 @@ int orc_num_threads(void) { return omp_get_max_threads(); }
 #else
 int orc_num_threads(void) { return 1; }
 #endif
+
+/* ================================================================== planning loop */
+/* PAPER.md:83-101, Eq. 1-3 (BeamValidationLayer).  For every opposing pair (p_a, p_b) — each leaf pair and the two jaw
+ * pairs (x1,x2), (y1,y2):
+ *   Eq. 1:  c = (p_a + p_b)/2,  w = p_b - p_a;   w >= w_min enforced,  c clamped to [-F, F];
+ *   Eq. 2:  p_a^ = c - w/2,  p_b^ = c + w/2.
+ * Monitor units are clamped to mu_eps > 0 (reading G16).  Limits: lim[0] = leaf w_min, lim[1] = leaf F,
+ * lim[2] = jaw w_min, lim[3] = jaw-x F, lim[4] = jaw-y F, lim[5] = mu_eps.                                          */
+static void validate_pair(double pa, double pb, double w_min, double F, double *qa, double *qb)
+{
+    double c = 0.5 * (pa + pb), w = pb - pa;
+    if (w < w_min) w = w_min;
+    if (c < -F) c = -F;
+    if (c > F) c = F;
+    *qa = c - 0.5 * w;
+    *qb = c + 0.5 * w;
+}
+void orc_validate(int n_cp, int n_pairs, const double *lim, const double *leaves, const double *jaws, const double *mu,
+                  double *leaves_out, double *jaws_out, double *mu_out)
+{
+    for (int b = 0; b < n_cp; ++b) {
+        const double *lv = leaves + (size_t)b * 2 * n_pairs;
+        double *lo = leaves_out + (size_t)b * 2 * n_pairs;
+        for (int i = 0; i < n_pairs; ++i) validate_pair(lv[i], lv[n_pairs + i], lim[0], lim[1], &lo[i], &lo[n_pairs + i]);
+        validate_pair(jaws[4 * b + 0], jaws[4 * b + 1], lim[2], lim[3], &jaws_out[4 * b + 0], &jaws_out[4 * b + 1]);
+        validate_pair(jaws[4 * b + 2], jaws[4 * b + 3], lim[2], lim[4], &jaws_out[4 * b + 2], &jaws_out[4 * b + 3]);
+        mu_out[b] = mu[b] < lim[5] ? lim[5] : mu[b];
+    }
+}
+/* Transpose of the Jacobian of orc_validate at the raw parameters ("preserve gradients").  The map is
+ * piecewise linear; reading G23: a clamp passes the gradient where its input lies inside the closed
+ * interval, i.e. [w >= w_min], [-F <= c <= F], [mu >= mu_eps], and blocks it outside (the convention of a clamp in an
+ * automatic-differentiation framework, which is what the paper's layer is built from).
+ *   g_c^ = g_a^ + g_b^,  g_w^ = (g_b^ - g_a^)/2;   g_c = g_c^ [c in range],  g_w = g_w^ [w >= w_min];
+ *   g_a = g_c/2 - g_w,  g_b = g_c/2 + g_w.                                                                          */
+static void validate_pair_adjoint(double pa, double pb, double w_min, double F, double ga_hat, double gb_hat, double *ga, double *gb)
+{
+    double c = 0.5 * (pa + pb), w = pb - pa;
+    double gc = ga_hat + gb_hat, gw = 0.5 * (gb_hat - ga_hat);
+    if (!(c >= -F && c <= F)) gc = 0.0;
+    if (!(w >= w_min)) gw = 0.0;
+    *ga = 0.5 * gc - gw;
+    *gb = 0.5 * gc + gw;
+}
+void orc_validate_adjoint(int n_cp, int n_pairs, const double *lim, const double *leaves, const double *jaws, const double *mu,
+                          const double *g_leaves_hat, const double *g_jaws_hat, const double *g_mu_hat,
+                          double *g_leaves, double *g_jaws, double *g_mu)
+{
+    for (int b = 0; b < n_cp; ++b) {
+        const size_t o = (size_t)b * 2 * n_pairs;
+        for (int i = 0; i < n_pairs; ++i)
+            validate_pair_adjoint(leaves[o + i], leaves[o + n_pairs + i], lim[0], lim[1], g_leaves_hat[o + i], g_leaves_hat[o + n_pairs + i],
+                                  &g_leaves[o + i], &g_leaves[o + n_pairs + i]);
+        validate_pair_adjoint(jaws[4 * b], jaws[4 * b + 1], lim[2], lim[3], g_jaws_hat[4 * b], g_jaws_hat[4 * b + 1], &g_jaws[4 * b], &g_jaws[4 * b + 1]);
+        validate_pair_adjoint(jaws[4 * b + 2], jaws[4 * b + 3], lim[2], lim[4], g_jaws_hat[4 * b + 2], g_jaws_hat[4 * b + 3], &g_jaws[4 * b + 2], &g_jaws[4 * b + 3]);
+        g_mu[b] = mu[b] >= lim[5] ? g_mu_hat[b] : 0.0;
+    }
+}
+/* PAPER.md:99, Eq. 3: minimum MU per control point from machine dynamics. */
+double orc_mu_epsilon(double dose_rate_min, double delta_phi, double gantry_speed_max) { return dose_rate_min * delta_phi / gantry_speed_max; }
+
+/* Weighted-sum objective over structures and its dose gradient.  PAPER.md:205-210, Eq. 10 is the case power = 1:
+ *   L = sum_s lambda_s || D_s - p_s ||_1     (p_s = prescription of the target, 0 for organs at risk);
+ * power = 2 is the quadratic objective BASELINE.json's configs c4/c5 name: L = sum_s lambda_s sum_{x in s} (D(x)-p_s)^2.
+ * Structures may overlap: bits[x] has bit s set when voxel x belongs to structure s (s < 32).
+ * g = dL/dD:  power 1: sum_s lambda_s sign(D - p_s) (sign(0) = 0, a valid subgradient);  power 2: sum_s 2 lambda_s (D - p_s). */
+double orc_objective(size_t n_vox, const float *dose, const unsigned *bits, int n_struct, const double *lambda, const double *presc,
+                     int power, float *g)
+{
+    double L = 0.0;
+    for (size_t x = 0; x < n_vox; ++x) {
+        double gx = 0.0;
+        for (int s = 0; s < n_struct; ++s) {
+            if (!((bits[x] >> s) & 1u)) continue;
+            double d = (double)dose[x] - presc[s];
+            if (power == 1) { L += lambda[s] * fabs(d); gx += lambda[s] * (d > 0.0 ? 1.0 : (d < 0.0 ? -1.0 : 0.0)); }
+            else { L += lambda[s] * d * d; gx += 2.0 * lambda[s] * d; }
+        }
+        if (g) g[x] = (float)gx;
+    }
+    return L;
+}
+
+/* Jaws tracking the aperture (BASELINE.json configs[4] "jaws tracking the aperture"; recipe of SURVEY.md §8(d) c5): over
+ * the pairs that are open by more than open_gap:  x1 = min l - margin, x2 = max r + margin, y1 / y2 = the v-extent of
+ * those pairs (their leaf boundaries); when no pair is open, all pairs count as open.                               */
+void orc_track_jaws(int n_cp, int n_pairs, const double *leaf_bounds, const double *leaves, double margin, double open_gap, double *jaws)
+{
+    for (int b = 0; b < n_cp; ++b) {
+        const double *lv = leaves + (size_t)b * 2 * n_pairs;
+        int any = 0;
+        for (int i = 0; i < n_pairs; ++i) any |= (lv[n_pairs + i] - lv[i]) > open_gap;
+        double x1 = 0, x2 = 0, y1 = 0, y2 = 0;
+        int first = 1;
+        for (int i = 0; i < n_pairs; ++i) {
+            if (any && !((lv[n_pairs + i] - lv[i]) > open_gap)) continue;
+            if (first) { x1 = lv[i]; x2 = lv[n_pairs + i]; y1 = leaf_bounds[i]; first = 0; }
+            if (lv[i] < x1) x1 = lv[i];
+            if (lv[n_pairs + i] > x2) x2 = lv[n_pairs + i];
+            y2 = leaf_bounds[i + 1];
+        }
+        jaws[4 * b] = x1 - margin; jaws[4 * b + 1] = x2 + margin; jaws[4 * b + 2] = y1; jaws[4 * b + 3] = y2;
+    }
+}
+
+/* Normalised-gradient step of the c5 planning loop: every leaf edge moves by at most step_leaf and
+ * every MU by at most step_mu per iteration:  theta <- theta - step * g / max|g|, the maximum taken over the whole
+ * group (all leaf edges of the arc; all MUs); a group whose gradient is identically zero does not move.             */
+void orc_plan_step(int n_cp, int n_pairs, double step_leaf, double step_mu, const double *g_leaves, const double *g_mu,
+                   double *leaves, double *mu)
+{
+    const size_t nl = (size_t)n_cp * 2 * n_pairs;
+    double ml = 0.0, mm = 0.0;
+    for (size_t e = 0; e < nl; ++e) if (fabs(g_leaves[e]) > ml) ml = fabs(g_leaves[e]);
+    for (int b = 0; b < n_cp; ++b) if (fabs(g_mu[b]) > mm) mm = fabs(g_mu[b]);
+    if (ml > 0.0) for (size_t e = 0; e < nl; ++e) leaves[e] -= step_leaf * g_leaves[e] / ml;
+    if (mm > 0.0) for (int b = 0; b < n_cp; ++b) mu[b] -= step_mu * g_mu[b] / mm;
+}

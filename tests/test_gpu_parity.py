@@ -61,7 +61,7 @@ def fluence_support_mask(wl, b, extra=0):
     sig = [m["fwhm_mlc_mm"] / 2.354820045, m["fwhm_jaw_mm"] / 2.354820045] + [float(x) for x in np.asarray(m["hs_sigma_mm"])[:m["n_hs"]]]
     tu = max(int(np.ceil(3.0 * sg / du)) for sg in [sig[0]] + sig[2:])
     tv = max(int(np.ceil(3.0 * sg / dv)) for sg in [sig[1]] + sig[2:])
-    grow = lambda a, t: np.convolve(a.astype(int), np.ones(2 * t + 1, int), mode="same") > 0
+    grow = lambda a, t: np.convolve(a.astype(int), np.ones(2 * t + 1, int))[t:t + len(a)] > 0      # dilation by t pixels
     return np.outer(grow(vb, tv + extra), grow(ua, tu + extra))
 
 

@@ -56,138 +56,183 @@ __device__ __forceinline__ void cp_async_8(unsigned dst, const float *src, int n
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
-constexpr int ROW_GROUPS = 4;       // k_project / k_resample_adjoint: a warp takes every 4th row of one slice
+constexpr int PROJECT_THREADS = 128;
 
-// S3.  Phivol over S_k (Eq. 5-6) into the compact block of the control point.  Grid: (X, n_cp); a warp per slice
-// and row group, lanes along v; the slice terms (box, magnification) and the row terms (a, ta) are warp-uniform,
-// the map is read with v fastest.
-__global__ void __launch_bounds__(256)
-k_project(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ phimapT, float *__restrict__ vol)
+// S3.  Phivol over S_k (Eq. 5-6) into the compact block of the control point.  Grid: (X, n_cp); a block takes the slices
+// k = blockIdx.x, blockIdx.x + X, ...; a thread owns one 16-byte quad of four consecutive v (the contiguous axis) and walks
+// the rows of S_k that fall to it: the column terms of its four voxels (pixel row b, weights, validity) are worked out
+// once per slice, the row terms once per row, and every store is one aligned float4.  The map is read with v fastest.
+// Columns [S.v0 & ~3, S.v1 | 3] are written (the conv stages its tiles in aligned pairs; the extra columns are
+// structural zeros and lie inside the region because rj0 % 8 == 0 and pv % 8 == 0).
+__global__ void __launch_bounds__(PROJECT_THREADS)
+k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp,
+          const float *__restrict__ phimapT, float *__restrict__ vol)
 {
     const int slot = blockIdx.y;
     if (slot >= n_cp) return;
     const int cp = cp0 + slot;
     const CpDesc d = desc[cp];
     if (d.a0 > d.a1) return;
-    const int lane = threadIdx.x & 31;
-    const int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
     const float *pm = phimapT + (size_t)cp * P.Nuf * P.Nvf;
     float *vc = vol + (size_t)slot * (size_t)P.stride_cp;
-    for (int q = warp0; q < P.Nw * ROW_GROUPS; q += n_warps) {
-        const int k = q / ROW_GROUPS, g = q - k * ROW_GROUPS;
-        const SliceBox S = slice_support(P, d, k);
-        if (box_empty(S)) continue;
+    const int tid = threadIdx.x;
+    for (int k = blockIdx.x; k < P.Nw; k += gridDim.x) {
+        const SliceBox16 S = load_box(sbox, (size_t)cp * P.Nw + k);
+        if (S.u0 > S.u1) continue;
         const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
         const float su = mag * P.du / P.Du, sv = mag / P.Dv;
-        // column terms of this lane (two passes cover 64 columns; wider supports loop)
-        // columns [S.v0 & ~1, S.v1 | 1]: the conv stages its tiles in aligned pairs; the extra columns are structural zeros
-        for (int j0 = S.v0 & ~1; j0 <= (S.v1 | 1); j0 += 32) {
-            const int j = j0 + lane;
-            const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
-            const float flb = floorf(fb);
-            const int b = (int)flb;
-            const float tb = fb - flb;
-            const bool jin = j <= (S.v1 | 1), jgrid = j < P.Nv;
-            const bool b0 = jgrid && b >= d.b0 && b <= d.b1, b1 = jgrid && b + 1 >= d.b0 && b + 1 <= d.b1;
-            for (int i = S.u0 + g; i <= S.u1; i += ROW_GROUPS) {
+        const int j0 = S.v0 & ~3, nq = (((int)S.v1 | 3) - j0 + 1) >> 2;          // quads per row
+        float *slice = vc + (size_t)k * d.pu * d.pv - d.rj0;
+        for (int q0 = 0; q0 < nq; q0 += PROJECT_THREADS) {                       // one pass unless a row holds > 128 quads
+            const int nqc = min(nq - q0, PROJECT_THREADS), rows = PROJECT_THREADS / nqc;
+            const int ri = tid / nqc, jq = q0 + tid - ri * nqc;
+            if (ri >= rows) continue;
+            // column terms of this thread's four voxels: m2-scaled weights of pixel rows b and b+1; invalid rows get weight 0
+            // and are folded onto a valid one, so that every address is readable
+            const int jb = j0 + 4 * jq;
+            float wb0[4], wb1[4];
+            int ib0[4], ib1[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int j = jb + e;
+                const float fb = (P.v0 + j * P.dv) * sv + P.cvf;
+                const float flb = floorf(fb);
+                const int b = (int)flb;
+                const float tb = fb - flb;
+                const bool jgrid = j < P.Nv;
+                const bool v0 = jgrid && b >= d.b0 && b <= d.b1, v1 = jgrid && b + 1 >= d.b0 && b + 1 <= d.b1;
+                wb0[e] = v0 ? m2 * (1.f - tb) : 0.f; wb1[e] = v1 ? m2 * tb : 0.f;
+                ib0[e] = v0 ? b : (v1 ? b + 1 : d.b0); ib1[e] = v1 ? b + 1 : ib0[e];
+            }
+            for (int i = S.u0 + ri; i <= S.u1; i += rows) {
                 const float fa = (i - P.cu) * su + P.cuf;
                 const float fla = floorf(fa);
                 const int a = (int)fla;
                 const float ta = fa - fla;
                 const bool a0 = a >= d.a0 && a <= d.a1, a1 = a + 1 >= d.a0 && a + 1 <= d.a1;
                 const float wa0 = a0 ? 1.f - ta : 0.f, wa1 = a1 ? ta : 0.f;
-                // invalid rows of the map get weight 0 and are folded onto a valid one: every address is readable
-                const float *pc0 = pm + (a0 ? a : a + 1) * P.Nvf, *pc1 = pm + (a1 ? a + 1 : a) * P.Nvf;
-                float s0 = 0.f, s1 = 0.f;
-                if ((a0 || a1) && b0) s0 = wa0 * __ldg(pc0 + b) + wa1 * __ldg(pc1 + b);
-                if ((a0 || a1) && b1) s1 = wa0 * __ldg(pc0 + b + 1) + wa1 * __ldg(pc1 + b + 1);
-                if (jin) vc[((size_t)k * d.pu + (i - d.ri0)) * d.pv + (j - d.rj0)] = m2 * ((1.f - tb) * s0 + tb * s1);
+                const float *pc0 = pm + (a0 ? a : (a1 ? a + 1 : d.a0)) * P.Nvf, *pc1 = pm + (a1 ? a + 1 : (a0 ? a : d.a0)) * P.Nvf;
+                float o[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const float r0 = wb0[e] * __ldg(pc0 + ib0[e]) + wb1[e] * __ldg(pc0 + ib1[e]);
+                    const float r1 = wb0[e] * __ldg(pc1 + ib0[e]) + wb1[e] * __ldg(pc1 + ib1[e]);
+                    o[e] = wa0 * r0 + wa1 * r1;
+                }
+                *reinterpret_cast<float4 *>(slice + (size_t)(i - d.ri0) * d.pv + jb) = make_float4(o[0], o[1], o[2], o[3]);
             }
         }
     }
 }
 
+constexpr int RA_THREADS = 256, RA_MAXC = 9;
+struct RaRow {                      // one beam row (k, i) of G_b: its patient-column candidates, compacted
+    int n;                          // candidates with a non-zero weight; -1: nothing to write; -2: stencil wider than 3 x 3
+    int out;                        // offset of G_b(k, i, v = 0) in the control point's compact block
+    int j0, nq;                     // first column (multiple of 4) and number of quads to write
+    int off[RA_MAXC];               // offsets of gT[y][x][0]
+    float w[RA_MAXC];
+    int xa, xb, ya, yb;             // candidate box of the general path
+    float eu0, ew0;
+};
+
 // S7.  G_b = R_b^T g over F_k in gather form: G_b(i,j,k) = sum over the patient voxels (x,y) of slice z = j whose
 // bilinear stencil (as evaluated by k_gather_dose) reaches beam voxel (i,k), weight (1-|du|)(1-|dw|), times g.
-// The gantry rotates about patient z = beam v (G1), so the weights do not depend on v: a warp owns a beam
-// row (k, i), nine lanes compute the (at most 3 x 3) candidate weights, the warp takes them by shuffle and streams
-// coalesced reads of gT[y][x][v] (dL/dDose with z fastest, L2-resident), two v per lane when nz is even.
-// Grid: (X, n_cp); a warp per slice and row group.
-__global__ void __launch_bounds__(256)
-k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, int C, const float *__restrict__ gT, float *__restrict__ G)
+// The gantry rotates about patient z = beam v (G1), so the weights do not depend on v.  A block takes 256
+// beam rows (k, i) of the control point's region at a time.  Phase A: one THREAD per row works out the (at most 3 x 3)
+// candidate columns and keeps those with a non-zero weight (4 on average) in shared memory.  Phase B: one HALF-WARP per
+// row streams 16-byte vectors along v: coalesced reads of gT[y][x][v] (dL/dDose with z fastest, row pitch padded to a
+// multiple of 4, L2-resident) and one aligned float4 store per lane.  Grid: (X, n_cp), blocks stride over the row chunks.
+__global__ void __launch_bounds__(RA_THREADS)
+k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp, int C,
+                   int nzp, const float *__restrict__ gT, float *__restrict__ G)
 {
+    __shared__ RaRow rows[RA_THREADS];
     const int slot = blockIdx.y;
     if (slot >= n_cp) return;
-    const CpDesc d = desc[cp0 + slot];
+    const int cp = cp0 + slot;
+    const CpDesc d = desc[cp];
     if (d.a0 > d.a1) return;
-    const int lane = threadIdx.x & 31;
-    const int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+    const int tid = threadIdx.x, lane16 = tid & 15, half = tid >> 4;
     // half-extent, in patient indices, of the rotated unit hat of one beam voxel; beam-index increments per patient step
     const float hx = (fabsf(d.cg) * P.du + fabsf(d.sg) * P.dw) / P.sx, hy = (fabsf(d.sg) * P.du + fabsf(d.cg) * P.dw) / P.sy;
     const float fu_x = d.cg * P.sx / P.du, fu_y = d.sg * P.sy / P.du, fw_x = -d.sg * P.sx / P.dw, fw_y = d.cg * P.sy / P.dw;
-    // affine maps, hoisted out of the row loop: patient index of beam voxel (i,k), beam index of patient voxel (x,y)
-    const float fx_i = P.du * d.cg / P.sx, fy_i = P.du * d.sg / P.sy;                       // d fx / d i, d fy / d i
+    // affine maps: patient index of beam voxel (i,k), beam index of patient voxel (x,y)
+    const float fx_i = P.du * d.cg / P.sx, fy_i = P.du * d.sg / P.sy;
     const float fx_0 = (P.isox - P.cu * P.du * d.cg - P.ox) / P.sx, fy_0 = (P.isoy - P.cu * P.du * d.sg - P.oy) / P.sy;
-    const float fx_w = -d.sg / P.sx, fy_w = d.cg / P.sy;                                    // d fx / d w, d fy / d w  (w in mm)
-    const float fu_0 = (d.cg * (P.ox - P.isox) + d.sg * (P.oy - P.isoy)) / P.du + P.cu;     // fu(x,y) = fu_0 + x fu_x + y fu_y
-    const float fw_0 = (-d.sg * (P.ox - P.isox) + d.cg * (P.oy - P.isoy) - P.wmin) / P.dw;  // fw(x,y) = fw_0 + x fw_x + y fw_y
+    const float fx_w = -d.sg / P.sx, fy_w = d.cg / P.sy;
+    const float fu_0 = (d.cg * (P.ox - P.isox) + d.sg * (P.oy - P.isoy)) / P.du + P.cu;
+    const float fw_0 = (-d.sg * (P.ox - P.isox) + d.cg * (P.oy - P.isoy) - P.wmin) / P.dw;
     float *Gc = G + (size_t)slot * (size_t)P.stride_cp;
-    const int cx = lane % 3, cy = (lane / 3) % 3;
-    const bool pairs = (P.nz & 1) == 0;                 // 8-byte alignment of gT[y][x][even j] and of G rows
-    for (int q = warp0; q < P.Nw * ROW_GROUPS; q += n_warps) {
-        const int k = q / ROW_GROUPS, g = q - k * ROW_GROUPS;
-        const SliceBox F = dilate(P, slice_support(P, d, k), C);
-        if (box_empty(F)) continue;
-        const float w = P.wmin + k * P.dw;
-        const float fx_k = fx_0 + w * fx_w, fy_k = fy_0 + w * fy_w;
-        const int jv0 = F.v0 & ~1, jv1 = F.v1 | 1;      // aligned pairs for the conv's tile copies; the extra columns lie inside
-                                                        // the region (rj0 % 8 == 0) and only feed outputs nobody reads
-        for (int i = F.u0 + g; i <= F.u1; i += ROW_GROUPS) {
-            const float fx = fx_k + i * fx_i, fy = fy_k + i * fy_i;
-            const int xa = max(0, (int)ceilf(fx - hx)), xb = min(P.nx - 1, (int)floorf(fx + hx));
-            const int ya = max(0, (int)ceilf(fy - hy)), yb = min(P.ny - 1, (int)floorf(fy + hy));
-            const float eu0 = fu_0 + xa * fu_x + ya * fu_y - (float)i;
-            const float ew0 = fw_0 + xa * fw_x + ya * fw_y - (float)k;
-            float *orow = Gc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
-            if (xb - xa <= 2 && yb - ya <= 2) {
-                // usual case (beam spacing ~ patient spacing): at most 3 x 3 candidates
-                const float wu = 1.f - fabsf(eu0 + cy * fu_y + cx * fu_x), ww = 1.f - fabsf(ew0 + cy * fw_y + cx * fw_x);
-                const float wmine = (wu > 0.f && ww > 0.f && xa + cx <= xb && ya + cy <= yb) ? wu * ww : 0.f;
-                float wq[9];
-#pragma unroll
-                for (int c = 0; c < 9; ++c) wq[c] = __shfl_sync(0xffffffffu, wmine, c);
-                const float *g0 = gT + ((size_t)ya * P.nx + xa) * P.nz;
-                if (pairs) {
-                    for (int j = jv0 + 2 * lane; j <= jv1; j += 64) {
-                        float2 v[9];
-#pragma unroll
-                        for (int c = 0; c < 9; ++c)    // all loads first, so that their latencies overlap
-                            v[c] = wq[c] != 0.f ? __ldg(reinterpret_cast<const float2 *>(g0 + ((size_t)(c / 3) * P.nx + (c % 3)) * P.nz + j)) : make_float2(0.f, 0.f);
-                        float2 acc = make_float2(0.f, 0.f);
-#pragma unroll
-                        for (int c = 0; c < 9; ++c) { acc.x = fmaf(wq[c], v[c].x, acc.x); acc.y = fmaf(wq[c], v[c].y, acc.y); }
-                        *reinterpret_cast<float2 *>(orow + j) = acc;
-                    }
-                } else {
-                    for (int j = jv0 + lane; j <= jv1; j += 32) {
-                        float v[9];
-#pragma unroll
-                        for (int c = 0; c < 9; ++c)
-                            v[c] = (wq[c] != 0.f && j < P.Nv) ? __ldg(g0 + ((size_t)(c / 3) * P.nx + (c % 3)) * P.nz + j) : 0.f;
-                        float acc = 0.f;
-#pragma unroll
-                        for (int c = 0; c < 9; ++c) acc = fmaf(wq[c], v[c], acc);
-                        orow[j] = acc;
+    const int n_rows = P.Nw * d.pu;
+    for (int r0 = blockIdx.x * RA_THREADS; r0 < n_rows; r0 += gridDim.x * RA_THREADS) {
+        __syncthreads();                                     // the previous chunk has been streamed
+        {   // phase A
+            RaRow &R = rows[tid];
+            const int r = r0 + tid;
+            int n = -1;
+            if (r < n_rows) {
+                const int k = r / d.pu, i = d.ri0 + (r - k * d.pu);
+                const SliceBox16 S = load_box(sbox, (size_t)cp * P.Nw + k);
+                const int fu0 = max(0, S.u0 - C), fu1 = min(P.Nu - 1, S.u1 + C), fv0 = max(0, S.v0 - C), fv1 = min(P.Nv - 1, S.v1 + C);
+                if (S.u0 <= S.u1 && i >= fu0 && i <= fu1) {
+                    R.out = (k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
+                    R.j0 = fv0 & ~3; R.nq = ((fv1 | 3) - R.j0 + 1) >> 2;
+                    const float w = P.wmin + k * P.dw;
+                    const float fx = fx_0 + w * fx_w + i * fx_i, fy = fy_0 + w * fy_w + i * fy_i;
+                    const int xa = max(0, (int)ceilf(fx - hx)), xb = min(P.nx - 1, (int)floorf(fx + hx));
+                    const int ya = max(0, (int)ceilf(fy - hy)), yb = min(P.ny - 1, (int)floorf(fy + hy));
+                    const float eu0 = fu_0 + xa * fu_x + ya * fu_y - (float)i;
+                    const float ew0 = fw_0 + xa * fw_x + ya * fw_y - (float)k;
+                    n = 0;
+                    if (xb - xa <= 2 && yb - ya <= 2) {
+                        for (int cy = 0; cy <= yb - ya; ++cy)
+                            for (int cx = 0; cx <= xb - xa; ++cx) {
+                                const float wu = 1.f - fabsf(eu0 + cy * fu_y + cx * fu_x), ww = 1.f - fabsf(ew0 + cy * fw_y + cx * fw_x);
+                                if (wu > 0.f && ww > 0.f) { R.off[n] = ((ya + cy) * P.nx + xa + cx) * nzp; R.w[n] = wu * ww; ++n; }
+                            }
+                    } else {
+                        n = -2;
+                        R.xa = xa; R.xb = xb; R.ya = ya; R.yb = yb; R.eu0 = eu0; R.ew0 = ew0;
                     }
                 }
+            }
+            R.n = n;
+        }
+        __syncthreads();
+        // phase B: half-warp `half` streams rows half, half + 16, ...
+        for (int rr = half; rr < RA_THREADS; rr += RA_THREADS / 16) {
+            const RaRow &R = rows[rr];
+            const int n = R.n;
+            if (n == -1) continue;
+            float *orow = Gc + R.out;
+            if (n >= 0) {
+                for (int q = lane16; q < R.nq; q += 16) {
+                    const int j = R.j0 + 4 * q;
+                    float4 v[RA_MAXC];
+#pragma unroll
+                    for (int c = 0; c < RA_MAXC; ++c)          // all loads first, so that their latencies overlap
+                        if (c < n) v[c] = __ldg(reinterpret_cast<const float4 *>(gT + R.off[c] + j));
+                    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                    for (int c = 0; c < RA_MAXC; ++c)
+                        if (c < n) {
+                            const float wc = R.w[c];
+                            acc.x = fmaf(wc, v[c].x, acc.x); acc.y = fmaf(wc, v[c].y, acc.y);
+                            acc.z = fmaf(wc, v[c].z, acc.z); acc.w = fmaf(wc, v[c].w, acc.w);
+                        }
+                    *reinterpret_cast<float4 *>(orow + j) = acc;
+                }
             } else {
-                for (int j = jv0 + lane; j <= jv1; j += 32) {
+                // stencil wider than 3 x 3 (beam voxels much coarser than patient voxels): plain loop over the candidate box
+                for (int jj = lane16; jj < 4 * R.nq; jj += 16) {
+                    const int j = R.j0 + jj;
                     float acc = 0.f;
-                    for (int yy = ya; yy <= yb && j < P.Nv; ++yy) {
-                        const float euy = eu0 + (yy - ya) * fu_y, ewy = ew0 + (yy - ya) * fw_y;
-                        for (int xx = xa; xx <= xb; ++xx) {
-                            const float wu = 1.f - fabsf(euy + (xx - xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - xa) * fw_x);
-                            if (wu > 0.f && ww > 0.f) acc = fmaf(wu * ww, __ldg(gT + ((size_t)yy * P.nx + xx) * P.nz + j), acc);
+                    for (int yy = R.ya; yy <= R.yb && j < P.Nv; ++yy) {
+                        const float euy = R.eu0 + (yy - R.ya) * fu_y, ewy = R.ew0 + (yy - R.ya) * fw_y;
+                        for (int xx = R.xa; xx <= R.xb; ++xx) {
+                            const float wu = 1.f - fabsf(euy + (xx - R.xa) * fu_x), ww = 1.f - fabsf(ewy + (xx - R.xa) * fw_x);
+                            if (wu > 0.f && ww > 0.f) acc = fmaf(wu * ww, __ldg(gT + ((size_t)yy * P.nx + xx) * nzp + j), acc);
                         }
                     }
                     orow[j] = acc;
@@ -303,20 +348,6 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
         ConvItem I;
         conv_load_item<KT, ADJ>(P, desc, cp0, n_cp, tile_base, zrad, item, slot_hint, I);
         float *oslice = out + I.slice_off;             // [pu][pv] of slice k
-        if (!ADJ) {
-            // the resampler reads the whole compact region: thread-tiles outside F_k hold exact zeros
-            const int cw = I.ctf1 - I.ctf0, chn = cw * I.nts;
-            for (int t = lane; t < chn; t += 32) {
-                const int ts = t / cw, tf = I.ctf0 + t % cw;
-                if (tf >= I.atf0 && tf < I.atf0 + I.naf && ts >= I.ats0 && ts < I.ats0 + I.nas) continue;
-#pragma unroll
-                for (int ii = 0; ii < RS; ++ii) {
-                    float4 *o = reinterpret_cast<float4 *>(oslice + (size_t)(ts * RS + ii) * I.pv + tf * RF);
-                    o[0] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    o[1] = make_float4(0.f, 0.f, 0.f, 0.f);
-                }
-            }
-        }
         if (I.n_tiles == 0) continue;                  // uniform across the warp
         const int pitch = I.pitch, ring = I.ring, naf = I.naf;
         {   // S4: slice kernel = lerp of the table in radiological depth; the table is stored as the [du][dv] image and is
@@ -445,7 +476,7 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
 }
 
 // Expands the compact block of one control point to a dense [Nw][Nv][Nu] volume (stage tap for tests).
-__global__ void k_expand_dense(Params P, const CpDesc *__restrict__ desc, int cp, int slot,
+__global__ void k_expand_dense(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ wbox, int cp, int slot,
                                const float *__restrict__ comp, float *__restrict__ dense)
 {
     const CpDesc d = desc[cp];
@@ -453,14 +484,17 @@ __global__ void k_expand_dense(Params P, const CpDesc *__restrict__ desc, int cp
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         const int i = (int)(e % P.Nu), j = (int)((e / P.Nu) % P.Nv), k = (int)(e / ((size_t)P.Nu * P.Nv));
         float v = 0.f;
-        if (d.a0 <= d.a1 && i >= d.ri0 && i < d.ri0 + d.pu && j >= d.rj0 && j < d.rj0 + d.pv)
-            v = comp[compact_index(P, d, slot, i, j, k)];
+        if (d.a0 <= d.a1) {                      // outside the written box of the slice the block holds stale data: D_b is zero there
+            const SliceBox16 w = load_box(wbox, (size_t)cp * P.Nw + k);
+            if (i >= w.u0 && i <= w.u1 && j >= w.v0 && j <= w.v1) v = comp[compact_index(P, d, slot, i, j, k)];
+        }
         dense[e] = v;
     }
 }
 
-// dL/dDose [nz][ny][nx] -> gT [ny*nx][nz] (z fastest), 32x32 shared-memory tiles.  Grid: (ceil(nxy/32), ceil(nz/32)).
-__global__ void __launch_bounds__(256) k_transpose_g(int nxy, int nz, const float *__restrict__ g, float *__restrict__ gT)
+// dL/dDose [nz][ny][nx] -> gT [ny*nx][nzp] (z fastest, row pitch nzp = nz rounded up to 4, pad zero), 32x32
+// shared-memory tiles.  Grid: (ceil(nxy/32), ceil(nzp/32)).
+__global__ void __launch_bounds__(256) k_transpose_g(int nxy, int nz, int nzp, const float *__restrict__ g, float *__restrict__ gT)
 {
     __shared__ float t[32][33];
     const int p0 = blockIdx.x * 32, z0 = blockIdx.y * 32;
@@ -472,7 +506,7 @@ __global__ void __launch_bounds__(256) k_transpose_g(int nxy, int nz, const floa
     __syncthreads();
     for (int r = ly; r < 32; r += 8) {
         const int p = p0 + r, z = z0 + lx;
-        if (p < nxy && z < nz) gT[(size_t)p * nz + z] = t[lx][r];
+        if (p < nxy && z < nzp) gT[(size_t)p * nzp + z] = t[lx][r];
     }
 }
 

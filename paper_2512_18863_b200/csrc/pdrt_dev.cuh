@@ -97,6 +97,19 @@ __host__ __device__ __forceinline__ int conv_pitch(int kt, int naf)
 
 struct SliceBox { int u0, u1, v0, v1; };   // inclusive voxel-index box; empty when u0 > u1 or v0 > v1
 
+// Per (control point, slice) boxes tabulated once per call by k_fluence ([n_cp][Nw], 8 bytes each, L2-resident), so that
+// the resampling kernels read a box instead of re-deriving it per beam row / patient column:
+//   sbox = S_k;  wbox = the part of slice k of D_b that the forward conv writes (F_k rounded outward to thread-tiles,
+//   clipped to the beam grid) — outside it the compact block holds stale data and must not be read.
+struct __align__(8) SliceBox16 { short u0, u1, v0, v1; };
+__device__ __forceinline__ SliceBox16 load_box(const SliceBox16 *__restrict__ t, size_t idx)
+{
+    const int2 r = __ldg(reinterpret_cast<const int2 *>(t) + idx);
+    SliceBox16 b;
+    b.u0 = (short)(r.x & 0xffff); b.u1 = (short)(r.x >> 16); b.v0 = (short)(r.y & 0xffff); b.v1 = (short)(r.y >> 16);
+    return b;
+}
+
 __device__ __forceinline__ bool box_empty(const SliceBox &b) { return b.u0 > b.u1 || b.v0 > b.v1; }
 
 // S_k: beam voxels of slice k whose bilinear stencil (Eq. 5) can touch a pixel of the fluence

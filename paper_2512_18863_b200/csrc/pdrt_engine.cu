@@ -42,8 +42,9 @@ int tile_floats_for(int kt)
     }
     return best;
 }
-// blocks per control point of the row-group kernels (k_project, k_resample_adjoint): four (slice, row group) units per warp
-int row_blocks(const Params &P) { return std::max(1, (P.Nw * ROW_GROUPS + 31) / 32); }
+// blocks per control point of k_project (a block takes every X-th slice) and of k_resample_adjoint (256 beam rows per chunk)
+int project_blocks(const Params &P) { return std::max(1, std::min(P.Nw, 32)); }
+int resample_adj_blocks(const Params &P) { return std::max(1, std::min(48, (P.Nw * (P.Nu + RS) + RA_THREADS - 1) / RA_THREADS)); }
 size_t conv_smem_bytes(int kt) { return sizeof(float) * (2 * (size_t)(kt + 1) * ((kt + 3) & ~3) + tile_floats_for(kt)); }   // row-pair kernel + ring
 
 template <typename T> struct DevBuf {
@@ -75,6 +76,7 @@ struct pdrt_engine {
     DevBuf<float> density, wtab, pool;
     // per-call scratch (sized by control-point capacity)
     DevBuf<CpDesc> desc;
+    DevBuf<SliceBox16> sbox, wbox;     // [n_cp][Nw] per-slice boxes: fluence support S_k, written part of D_b
     DevBuf<int> tile_base;
     DevBuf<WorkCounters> counters;
     DevBuf<float> phimap, phimapT, P0, T1, T2, T3, Abuf, gphimap, zrad, gT;
@@ -88,6 +90,8 @@ struct pdrt_engine {
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
     int conv_per_sm[2][64] = {};      // resident conv blocks per SM on THIS engine's device, by [adjoint][KT]; 0 = not queried yet
+    int nzp = 0;                      // row pitch of gT: nz rounded up to 4
+    int pa_warps = 0;                 // warps of k_project_adjoint that hold a shared-memory plane (0: attribute not set yet)
     // per-stage device timing of the most recent call (CUDA events on the call's stream)
     bool profiling = false;
     struct StageRec { int stage; cudaEvent_t a, b; };
@@ -98,7 +102,7 @@ struct pdrt_engine {
 
     size_t scratch_bytes() const
     {
-        return desc.bytes() + tile_base.bytes() + phimap.bytes() + phimapT.bytes() + P0.bytes() + T1.bytes() + T2.bytes() +
+        return desc.bytes() + sbox.bytes() + wbox.bytes() + tile_base.bytes() + phimap.bytes() + phimapT.bytes() + P0.bytes() + T1.bytes() + T2.bytes() +
                T3.bytes() + Abuf.bytes() + gphimap.bytes() + zrad.bytes() + gT.bytes() + rho_s.bytes() + Z_s.bytes() + bufA.bytes() + bufB.bytes();
     }
 };
@@ -240,6 +244,7 @@ int ensure_cp_scratch(pdrt_engine *e, int n_cp)
 {
     const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
     CU(e, e->desc.ensure(n_cp));
+    CU(e, e->sbox.ensure((size_t)n_cp * e->P.Nw)); CU(e, e->wbox.ensure((size_t)n_cp * e->P.Nw));
     CU(e, e->tile_base.ensure((size_t)n_cp + 2));     // prefix of the conv units + the unit counter of the running conv
     CU(e, e->counters.ensure(1));
     CU(e, e->phimap.ensure(nmap)); CU(e, e->phimapT.ensure(nmap)); CU(e, e->P0.ensure(nmap)); CU(e, e->T1.ensure(nmap));
@@ -277,8 +282,8 @@ int run_setup(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, 
     if (rc) return rc;
     {
         StageTimer t(e, PDRT_STAGE_FLUENCE, st);
-        k_fluence<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, gantry, mu, e->desc.p, e->P0.p, e->T1.p,
-                                               e->T2.p, e->Abuf.p, e->phimap.p, e->phimapT.p);
+        k_fluence<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, gantry, mu, e->desc.p, e->sbox.p, e->wbox.p,
+                                               e->P0.p, e->T1.p, e->T2.p, e->Abuf.p, e->phimap.p, e->phimapT.p);
     }
     CU(e, cudaGetLastError());
     if (need_depth) {
@@ -297,7 +302,9 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
     const int nb = batch_size(e, n_cp, 2);
     CU(e, e->bufA.ensure((size_t)nb * e->P.stride_cp));
     CU(e, e->bufB.ensure((size_t)nb * e->P.stride_cp));
-    const dim3 gg((e->P.nx + GATHER_TX - 1) / GATHER_TX, (e->P.ny + GATHER_TY - 1) / GATHER_TY, (e->P.nz + GATHER_Z - 1) / GATHER_Z);
+    const dim3 gg((e->P.nx + GD_PX - 1) / GD_PX, (e->P.ny + GD_PY - 1) / GD_PY, 1);
+    // the resampler writes only the z-range that the control points reach; the rest of the grid is zero
+    CU(e, cudaMemsetAsync(dose, 0, sizeof(float) * (size_t)e->P.nx * e->P.ny * e->P.nz, st));
     for (int cp0 = 0; cp0 < n_cp; cp0 += nb) {
         const int n = std::min(nb, n_cp - cp0);
         {
@@ -307,7 +314,7 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
         CU(e, cudaGetLastError());
         {
             StageTimer t(e, PDRT_STAGE_PROJECT, st);
-            k_project<<<dim3(row_blocks(e->P), n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, e->phimapT.p, e->bufB.p);
+            k_project<<<dim3(project_blocks(e->P), n), PROJECT_THREADS, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->phimapT.p, e->bufB.p);
         }
         CU(e, cudaGetLastError());
         {
@@ -317,7 +324,7 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
         if (rc) return rc;
         {
             StageTimer t(e, PDRT_STAGE_GATHER, st);
-            k_gather_dose<<<gg, GATHER_THREADS, 0, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, dose, cp0 > 0);
+            k_gather_dose<<<gg, GD_THREADS, 0, st>>>(e->P, e->desc.p, e->wbox.p, cp0, n, e->bufA.p, dose, cp0 > 0);
         }
         CU(e, cudaGetLastError());
     }
@@ -335,10 +342,17 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
     CU(e, e->gphimap.ensure(nmap));
     CU(e, e->T3.ensure(nmap));
     const size_t nxy = (size_t)e->P.nx * e->P.ny;
-    CU(e, e->gT.ensure(nxy * e->P.nz));
+    CU(e, e->gT.ensure(nxy * e->nzp));
     {   // S7 prologue: dL/dDose with z fastest, so that the resampling adjoint streams along v
         StageTimer t(e, PDRT_STAGE_TRANSPOSE, st);
-        k_transpose_g<<<dim3((unsigned)((nxy + 31) / 32), (e->P.nz + 31) / 32), 256, 0, st>>>((int)nxy, e->P.nz, gdose, e->gT.p);
+        k_transpose_g<<<dim3((unsigned)((nxy + 31) / 32), (e->nzp + 31) / 32), 256, 0, st>>>((int)nxy, e->P.nz, e->nzp, gdose, e->gT.p);
+    }
+    if (e->pa_warps == 0) {   // planes of k_project_adjoint: as many of its 8 warps as fit into shared memory (opt-in above 48 KB, per device)
+        const size_t per_warp = sizeof(float) * 32 * (size_t)e->P.Nuf;
+        const int fit = (int)std::min<size_t>(PA_WARPS, (size_t)(200 << 10) / per_warp);
+        if (fit < 1) return fail(e, PDRT_EINVAL, "fluence map too wide for the projection adjoint (flu_nu > 1600)");
+        CU(e, cudaFuncSetAttribute(k_project_adjoint, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(per_warp * fit)));
+        e->pa_warps = fit;
     }
     CU(e, cudaGetLastError());
     const int nb = batch_size(e, n_cp, 2);
@@ -353,7 +367,8 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
         CU(e, cudaGetLastError());
         {
             StageTimer t(e, PDRT_STAGE_RESAMPLE_ADJ, st);
-            k_resample_adjoint<<<dim3(row_blocks(e->P), n), 256, 0, st>>>(e->P, e->desc.p, cp0, n, (e->P.KT - 1) / 2, e->gT.p, e->bufB.p);
+            k_resample_adjoint<<<dim3(resample_adj_blocks(e->P), n), RA_THREADS, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, (e->P.KT - 1) / 2, e->nzp,
+                                                                                          e->gT.p, e->bufB.p);
         }
         CU(e, cudaGetLastError());
         {
@@ -363,7 +378,8 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
         if (rc) return rc;
         {
             StageTimer t(e, PDRT_STAGE_PROJECT_ADJ, st);
-            k_project_adjoint<<<dim3(((e->P.Nuf + PROJ_A - 1) / PROJ_A) * ((e->P.Nvf + 31) / 32), n), PROJ_THREADS, sizeof(SliceGeo) * e->P.Nw, st>>>(e->P, e->desc.p, cp0, n, e->bufA.p, e->gphimap.p);
+            k_project_adjoint<<<dim3(PA_CLUSTER * ((e->P.Nvf + 31) / 32), n), PA_THREADS, sizeof(float) * 32 * (size_t)e->P.Nuf * e->pa_warps, st>>>(
+                e->P, e->desc.p, e->sbox.p, cp0, n, e->pa_warps, e->bufA.p, e->gphimap.p);
         }
         CU(e, cudaGetLastError());
     }
@@ -398,6 +414,8 @@ int pdrt_create(const pdrt_grid *grid, const float *density, const pdrt_beam_mod
     if (grid->nx < 1 || grid->ny < 1 || grid->nz < 1 || !(grid->sx > 0) || !(grid->sy > 0) || !(grid->sz > 0))
         return fail(nullptr, PDRT_EINVAL, "grid sizes and spacings must be positive");
     if ((long long)grid->nx * grid->ny * grid->nz > (1ll << 31) - 1) return fail(nullptr, PDRT_EINVAL, "grid too large");
+    if (grid->nx > 16384 || grid->ny > 16384 || grid->nz > 16384 || m->beam_nu > 16384 || m->beam_nw > 16384)
+        return fail(nullptr, PDRT_EINVAL, "grid dimensions above 16384 are not supported");
     if (!(m->sid_mm > 0)) return fail(nullptr, PDRT_EINVAL, "sid_mm must be positive");
     if (m->n_pairs < 1 || !m->leaf_bounds_mm) return fail(nullptr, PDRT_EINVAL, "n_pairs >= 1 and leaf_bounds_mm required");
     for (int i = 0; i < m->n_pairs; ++i)
@@ -443,6 +461,7 @@ int pdrt_create(const pdrt_grid *grid, const float *density, const pdrt_beam_mod
     if (m->beam_nu > 0) { P.Nu = m->beam_nu; P.Nw = m->beam_nw; P.du = m->beam_du; P.dw = m->beam_dw; P.wmin = m->beam_wmin; }
     else { P.Nu = grid->nx; P.Nw = grid->ny; P.du = P.dw = grid->sx; P.wmin = -0.5f * (P.Nw - 1) * P.dw; }
     P.Nv = grid->nz; P.dv = grid->sz;
+    e->nzp = (grid->nz + 3) & ~3;
     P.cu = 0.5f * (P.Nu - 1); P.v0 = grid->oz - grid->iso[2];
     P.Nuf = m->flu_nu; P.Nvf = m->flu_nv; P.Du = m->flu_du; P.Dv = m->flu_dv;
     P.cuf = 0.5f * (P.Nuf - 1); P.cvf = 0.5f * (P.Nvf - 1);
@@ -505,6 +524,7 @@ void pdrt_destroy(pdrt_engine *e)
     cudaSetDevice(e->device);
     cudaDeviceSynchronize();
     e->density.release(); e->wtab.release(); e->pool.release(); e->desc.release(); e->tile_base.release();
+    e->sbox.release(); e->wbox.release();
     e->counters.release(); e->phimap.release(); e->P0.release(); e->T1.release(); e->T2.release(); e->T3.release();
     e->Abuf.release(); e->gphimap.release(); e->zrad.release(); e->rho_s.release(); e->Z_s.release();
     e->bufA.release(); e->bufB.release(); e->phimapT.release(); e->gT.release();
@@ -671,10 +691,10 @@ int pdrt_stage_beam_dose(pdrt_engine *e, const float *leaves, const float *jaws,
     CU(e, e->bufB.ensure((size_t)e->P.stride_cp));
     k_scan_items<<<1, 256, 0, st>>>(e->desc.p, 0, 1, 0, e->tile_base.p, e->counters.p);
     CU(e, cudaGetLastError());
-    k_project<<<dim3(row_blocks(e->P), 1), 256, 0, st>>>(e->P, e->desc.p, 0, 1, e->phimapT.p, e->bufB.p);
+    k_project<<<dim3(project_blocks(e->P), 1), PROJECT_THREADS, 0, st>>>(e->P, e->desc.p, e->sbox.p, 0, 1, e->phimapT.p, e->bufB.p);
     CU(e, cudaGetLastError());
     if ((rc = launch_conv<false>(e, 0, 1, e->bufB.p, e->bufA.p, st))) return rc;
-    k_expand_dense<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, 0, 0, e->bufA.p, db);
+    k_expand_dense<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, e->wbox.p, 0, 0, e->bufA.p, db);
     CU(e, cudaGetLastError());
     return PDRT_OK;
 }

@@ -87,6 +87,7 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
 __global__ void __launch_bounds__(FLU_THREADS)
 k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, const float *__restrict__ jaws,
           const float *__restrict__ gantry_deg, const float *__restrict__ mu, CpDesc *desc,
+          SliceBox16 *sbox, SliceBox16 *wbox,
           float *P0, float *T1, float *T2, float *Abuf, float *phimap, float *phimapT)
 {
     const int cp = blockIdx.x, tid = threadIdx.x;
@@ -99,11 +100,22 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
     }
     __syncthreads();
     const bool empty = d.a0 > d.a1;
-    if (!empty) {     // per-slice work counters: |S_k|, |F_k|, thread-tiles
+    if (!empty) {     // per-slice boxes for the resampling kernels, and work counters: |S_k|, |F_k|, thread-tiles
         const int C = (P.KT - 1) / 2;
         unsigned long long sup = 0, fp = 0, tf = 0, ta = 0;
         for (int k = tid; k < P.Nw; k += FLU_THREADS) {
             const SliceBox s = slice_support(P, d, k), f = dilate(P, s, C);
+            SliceBox16 sb = { 1, 0, 1, 0 }, wb = { 1, 0, 1, 0 };
+            if (!box_empty(s)) {
+                sb.u0 = (short)s.u0; sb.u1 = (short)s.u1; sb.v0 = (short)s.v0; sb.v1 = (short)s.v1;
+                // thread-tiles of the forward conv that intersect F_k (conv_load_item), clipped to the beam grid
+                wb.u0 = (short)(d.ri0 + (f.u0 - d.ri0) / RS * RS);
+                wb.u1 = (short)min(P.Nu - 1, d.ri0 + min(d.nts - 1, (f.u1 - d.ri0) / RS) * RS + RS - 1);
+                wb.v0 = (short)(d.rj0 + (f.v0 - d.rj0) / RF * RF);
+                wb.v1 = (short)(d.rj0 + (f.v1 - d.rj0) / RF * RF + RF - 1);
+            }
+            sbox[(size_t)cp * P.Nw + k] = sb;
+            wbox[(size_t)cp * P.Nw + k] = wb;
             if (box_empty(s)) continue;
             sup += (unsigned long long)(s.u1 - s.u0 + 1) * (s.v1 - s.v0 + 1);
             fp += (unsigned long long)(f.u1 - f.u0 + 1) * (f.v1 - f.v0 + 1);

@@ -1,270 +1,305 @@
 // pdrt_resample.cuh — S6 (beam -> patient resampling + MU-weighted accumulation, PAPER.md:160-168,
 // Eq. 9) and S9 (transpose of the divergent projection, Eq. 5-6, in gather form).  These are the
 // bandwidth-bound stages: each patient voxel is written once per call (accumulation over control points
-// stays in registers), the compact D_b blocks are read once as 16-byte vectors along v, and no global
+// stays in registers), the compact D_b / H_b blocks are read once as 16-byte vectors along v, and no global
 // atomics are used anywhere.  (S7, the transpose of S6, is k_resample_adjoint in pdrt_conv.cuh.)
 #pragma once
+#include <cooperative_groups.h>
+
 #include "pdrt_dev.cuh"
 
 namespace pdrt {
 
-constexpr int GATHER_TX = 16, GATHER_TY = 4;   // block = 16 x 4 patient columns (x,y): two warp patches of 8 x 4 ...
-constexpr int GATHER_Z = 32;            // ... times 32 z-slices
-constexpr int GATHER_SPLIT = 4;         // ... times 4 warps per patch that share the control-point list round-robin
-constexpr int GATHER_THREADS = 2 * GATHER_SPLIT * 32;
-constexpr int GATHER_CHUNK = 128;       // control points staged in shared memory per pass
+namespace cg = cooperative_groups;
 
-struct GatherCp {                       // the slice of CpDesc the resampler needs
-    float cg, sg, scale;
-    int ri0, pu, rj0, pv;
+constexpr int GD_PX = 8, GD_PY = 2;              // a block owns 8 x 2 patient columns (x,y): 32-byte runs of the dose rows
+constexpr int GD_COLS = GD_PX * GD_PY;           // ... one half-warp per column
+constexpr int GD_CPB = 16;                       // control points set up per round (16 columns x 16 control points = 256 threads)
+constexpr int GD_THREADS = GD_COLS * GD_CPB;
+constexpr int GD_ZSPAN = 64;                     // z covered by one pass of a half-warp (16 lanes x float4)
+constexpr int GD_MAXPASS = 4;                    // passes held in registers at once (256 z)
+constexpr int GD_LIST = 512;                     // control points listed per outer chunk
+
+struct __align__(16) GatherRec {                 // bilinear stencil of one (patient column, control point): 48 bytes
+    const float *base;                           // D_b block of the control point, shifted so that base[off + z] is voxel v = z
+    int n_valid;                                 // 0: nothing to add
     int pad_;
-    long long base;                     // slot * stride_cp
+    int off[4];                                  // rows (i0,k0), (i0+1,k0), (i0,k0+1), (i0+1,k0+1); invalid ones folded onto a valid row
+    float w[4];                                  // cal * MU * bilinear weight; 0 for invalid neighbours
+    short zlo0, zhi0, zlo1, zhi1;                // written v-range [zlo, zhi) of slice k0 and of slice k0+1 (multiples of 8)
+    int pad2_[2];
 };
 
-// S6.  Grid: (ceil(nx/16), ceil(ny/4), ceil(nz/32)); a block owns 16 x 4 patient columns (x,y) times 32
-// z-slices, a warp an 8(x) x 4(y) patch of columns (compact in the beam frame under any gantry rotation).
+// S6.  Grid: (ceil(nx/8), ceil(ny/2), 1); a block owns 8 x 2 patient columns (x,y) over all z.
 //   dose[p] (+)= sum_b scale_b * bilinear_0(D_b[.][z][.]; fu, fw)
-// The gantry rotates about z (G1), so for one control point the beam-frame position (fu, fw) and the
-// four bilinear weights of a column are the same for all its voxels.  Per control point each lane computes
-// them for ONE of the warp's 32 columns; the warp then walks the columns four at a time with 8 lanes along v
-// per column, taking offset and weights by warp shuffle: every load instruction reads four full 128-byte
-// lines of the v-fastest D_b block.  A lane accumulates 8 column groups x 4 z in registers over all control
-// points (in control-point order: deterministic) and every patient voxel is written exactly once.
-// Warp 0 first compacts the control points whose compact region can intersect this block.  The per-control-point
-// chain (setup -> shuffle -> load -> accumulate) is latency-bound, so four warps share the list of one patch
-// (entries q = s, s+4, ...) and their partial sums are added through shared memory in a fixed order.
-__global__ void __launch_bounds__(GATHER_THREADS)
-k_gather_dose(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ D,
-              float *__restrict__ dose, int accumulate)
+// The gantry rotates about z (G1), so for one control point the beam-frame position (fu, fw) and the four
+// bilinear weights of a column are the same for all its voxels.  Warp 0 first lists the control points whose compact
+// region can reach the block's columns (and the z-range they cover).  Then, 16 control points at a time: phase A, one
+// THREAD per (column, control point) builds the stencil record (offsets of the four beam rows, weights, and the v-range
+// that the forward conv wrote in the two slices — outside it D_b is zero and the block holds stale data); phase B, one
+// HALF-WARP per column streams 16-byte vectors along v for the listed control points, four loads in flight per control
+// point and several control points unrolled, accumulating in registers in control-point order (deterministic).  Every
+// patient voxel of the z-range is written exactly once; the rest of the dose grid is zeroed by the caller (memset).
+__global__ void __launch_bounds__(GD_THREADS)
+k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ wbox, int cp0, int n_cp,
+              const float *__restrict__ D, float *__restrict__ dose, int accumulate)
 {
-    __shared__ GatherCp list[GATHER_CHUNK];
-    __shared__ int n_list;
-    __shared__ float4 part[2 * (GATHER_SPLIT - 1)][8][32];
-    const int tid = threadIdx.x;
-    const int wrp = tid >> 5, lane = tid & 31;
-    const int patch = wrp & 1, split = wrp >> 1;
-    const int px0 = blockIdx.x * GATHER_TX + patch * 8, py0 = blockIdx.y * GATHER_TY;
-    const int z0 = blockIdx.z * GATHER_Z;
-    // the column this lane sets up
-    const int ix = px0 + (lane & 7), iy = py0 + (lane >> 3);
-    const float dx = P.ox + ix * P.sx - P.isox, dy = P.oy + iy * P.sy - P.isoy;
-    const bool inside = ix < P.nx && iy < P.ny;
+    __shared__ GatherRec rec[GD_CPB][GD_COLS];
+    __shared__ short list[GD_LIST];
+    __shared__ int n_list_s, zmin_s, zmax_s;
+    const int tid = threadIdx.x, lane = tid & 31, lane16 = tid & 15;
+    const int col = tid >> 4;                                    // phase B: column of this half-warp
+    const int a_col = tid & 15, a_cp = tid >> 4;                 // phase A: (column, control point of the round)
+    const int px0 = blockIdx.x * GD_PX, py0 = blockIdx.y * GD_PY;
     // tile corners (for culling), relative to the isocentre
-    const float cx0 = P.ox + (blockIdx.x * GATHER_TX) * P.sx - P.isox, cx1 = cx0 + (GATHER_TX - 1) * P.sx;
-    const float cy0 = P.oy + (blockIdx.y * GATHER_TY) * P.sy - P.isoy, cy1 = cy0 + (GATHER_TY - 1) * P.sy;
-    const int sub = lane >> 3, zl = 4 * (lane & 7);      // column within a group of four, z offset of this lane's quad
-    float4 acc[8];
-#pragma unroll
-    for (int g = 0; g < 8; ++g) acc[g] = make_float4(0.f, 0.f, 0.f, 0.f);
+    const float cx0 = P.ox + px0 * P.sx - P.isox, cx1 = cx0 + (GD_PX - 1) * P.sx;
+    const float cy0 = P.oy + py0 * P.sy - P.isoy, cy1 = cy0 + (GD_PY - 1) * P.sy;
+    // phase-A column of this thread
+    const int ax = px0 + (a_col & (GD_PX - 1)), ay = py0 + a_col / GD_PX;
+    const float adx = P.ox + ax * P.sx - P.isox, ady = P.oy + ay * P.sy - P.isoy;
+    const bool a_inside = ax < P.nx && ay < P.ny;
+    // phase-B column of this half-warp
+    const int bx = px0 + (col & (GD_PX - 1)), by = py0 + col / GD_PX;
+    const bool b_inside = bx < P.nx && by < P.ny;
 
-    for (int c0 = 0; c0 < n_cp; c0 += GATHER_CHUNK) {
+    for (int c0 = 0; c0 < n_cp; c0 += GD_LIST) {
         __syncthreads();
-        if (tid < 32) {                 // warp 0 builds the ordered list of candidate control points
-            int count = 0;
-            const int cend = min(n_cp, c0 + GATHER_CHUNK);
+        if (tid < 32) {                 // warp 0 builds the ordered list of candidate control points and their z-range
+            int count = 0, zmin = P.nz, zmax = 0;
+            const int cend = min(n_cp, c0 + GD_LIST);
             for (int cb = c0; cb < cend; cb += 32) {
                 const int c = cb + tid;
                 bool keep = false;
-                CpDesc d;
                 if (c < cend) {
-                    d = desc[cp0 + c];
-                    if (d.a0 <= d.a1 && z0 < d.rj0 + d.pv && z0 + GATHER_Z > d.rj0) {
+                    const CpDesc &d = desc[cp0 + c];
+                    if (d.a0 <= d.a1) {
                         // u-extent of the tile: extremes are at its corners
                         const float u00 = d.cg * cx0 + d.sg * cy0, u10 = d.cg * cx1 + d.sg * cy0;
                         const float u01 = d.cg * cx0 + d.sg * cy1, u11 = d.cg * cx1 + d.sg * cy1;
                         const float umin = fminf(fminf(u00, u10), fminf(u01, u11)) / P.du + P.cu;
                         const float umax = fmaxf(fmaxf(u00, u10), fmaxf(u01, u11)) / P.du + P.cu;
                         keep = umax >= (float)(d.ri0 - 1) && umin <= (float)(d.ri0 + d.pu);
+                        if (keep) { zmin = min(zmin, d.rj0); zmax = max(zmax, min(P.nz, d.rj0 + d.pv)); }
                     }
                 }
                 const unsigned m = __ballot_sync(0xffffffffu, keep);
-                if (keep) {
-                    GatherCp g;
-                    g.cg = d.cg; g.sg = d.sg; g.scale = d.scale;
-                    g.ri0 = d.ri0; g.pu = d.pu; g.rj0 = d.rj0; g.pv = d.pv; g.pad_ = 0;
-                    g.base = (long long)c * P.stride_cp;
-                    list[count + __popc(m & ((1u << tid) - 1u))] = g;
-                }
+                if (keep) list[count + __popc(m & ((1u << tid) - 1u))] = (short)(c - c0);
                 count += __popc(m);
             }
-            if (tid == 0) n_list = count;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                zmin = min(zmin, __shfl_xor_sync(0xffffffffu, zmin, o));
+                zmax = max(zmax, __shfl_xor_sync(0xffffffffu, zmax, o));
+            }
+            if (tid == 0) { n_list_s = count; zmin_s = zmin & ~7; zmax_s = zmax; }
         }
         __syncthreads();
-        const int n = n_list;
-        for (int q = split; q < n; q += GATHER_SPLIT) {
-            const GatherCp g = list[q];
-            const float fu = (g.cg * dx + g.sg * dy) / P.du + P.cu;
-            const float fw = (-g.sg * dx + g.cg * dy - P.wmin) / P.dw;
-            const float flu = floorf(fu), flw = floorf(fw);
-            const int i0 = (int)flu, k0 = (int)flw;
-            const float tu = fu - flu, tw = fw - flw;
-            // bilinear_0: neighbours outside the beam grid contribute 0; outside the compact region D_b is 0
-            const int ihi = min(P.Nu, g.ri0 + g.pu);
-            const bool iv0 = i0 >= g.ri0 && i0 < ihi, iv1 = i0 + 1 >= g.ri0 && i0 + 1 < ihi;
-            const bool kv0 = k0 >= 0 && k0 < P.Nw, kv1 = k0 + 1 >= 0 && k0 + 1 < P.Nw;
-            const bool any = inside && (iv0 || iv1) && (kv0 || kv1);
-            if (!__any_sync(0xffffffffu, any)) continue;
-            // invalid neighbours get weight 0 and are folded onto the valid one, so that every address is readable
-            const int ia = iv0 ? i0 : i0 + 1, ka = kv0 ? k0 : k0 + 1;
-            const float wu0 = iv0 ? 1.f - tu : 0.f, wu1 = iv1 ? tu : 0.f, wk0 = kv0 ? 1.f - tw : 0.f, wk1 = kv1 ? tw : 0.f;
-            int offp = 0;
-            if (any) offp = ((ka * g.pu + (ia - g.ri0)) * g.pv) | ((iv0 && iv1) ? 1 : 0) | ((kv0 && kv1) ? 2 : 0) | 4;   // pv % 8 == 0
-            const float w00 = g.scale * (wu0 * wk0), w10 = g.scale * (wu1 * wk0), w01 = g.scale * (wu0 * wk1), w11 = g.scale * (wu1 * wk1);
-            const int zq = z0 - g.rj0 + zl;                              // multiple of 4
-            const bool zok = zq >= 0 && zq + 4 <= g.pv;
-            const float *Dc = D + g.base + zq;
-            const int sk = g.pu * g.pv;
+        const int n_list = n_list_s, zmin = zmin_s, zmax = zmax_s;
+        if (n_list == 0) continue;
+        for (int zb = zmin; zb < zmax; zb += GD_ZSPAN * GD_MAXPASS) {            // one iteration unless the regions span > 256 z
+            float4 acc[GD_MAXPASS];
 #pragma unroll
-            for (int gq = 0; gq < 8; ++gq) {
-                const int src = 4 * gq + sub;
-                const int o = __shfl_sync(0xffffffffu, offp, src);
-                const float f00 = __shfl_sync(0xffffffffu, w00, src), f10 = __shfl_sync(0xffffffffu, w10, src);
-                const float f01 = __shfl_sync(0xffffffffu, w01, src), f11 = __shfl_sync(0xffffffffu, w11, src);
-                if ((o & 4) && zok) {
-                    const float *p = Dc + (o & ~7);
-                    const int di = (o & 1) ? g.pv : 0, dk = (o & 2) ? sk : 0;
-                    const float4 a = __ldg(reinterpret_cast<const float4 *>(p));
-                    const float4 b = __ldg(reinterpret_cast<const float4 *>(p + di));
-                    const float4 c = __ldg(reinterpret_cast<const float4 *>(p + dk));
-                    const float4 e = __ldg(reinterpret_cast<const float4 *>(p + dk + di));
-                    acc[gq].x += f00 * a.x + f10 * b.x + f01 * c.x + f11 * e.x;
-                    acc[gq].y += f00 * a.y + f10 * b.y + f01 * c.y + f11 * e.y;
-                    acc[gq].z += f00 * a.z + f10 * b.z + f01 * c.z + f11 * e.z;
-                    acc[gq].w += f00 * a.w + f10 * b.w + f01 * c.w + f11 * e.w;
+            for (int p = 0; p < GD_MAXPASS; ++p) acc[p] = make_float4(0.f, 0.f, 0.f, 0.f);
+            const int npass = min(GD_MAXPASS, (zmax - zb + GD_ZSPAN - 1) / GD_ZSPAN);
+            for (int q0 = 0; q0 < n_list; q0 += GD_CPB) {
+                __syncthreads();                                                 // the records of the previous round are consumed
+                {   // phase A: record of (column a_col, control point list[q0 + a_cp])
+                    GatherRec &R = rec[a_cp][a_col];
+                    int n_valid = 0;
+                    if (q0 + a_cp < n_list && a_inside) {
+                        const int c = c0 + list[q0 + a_cp];
+                        const CpDesc &d = desc[cp0 + c];
+                        const float fu = (d.cg * adx + d.sg * ady) / P.du + P.cu;
+                        const float fw = (-d.sg * adx + d.cg * ady - P.wmin) / P.dw;
+                        const float flu = floorf(fu), flw = floorf(fw);
+                        const int i0 = (int)flu, k0 = (int)flw;
+                        const float tu = fu - flu, tw = fw - flw;
+                        // bilinear_0: neighbours outside the beam grid contribute 0; outside the written box of its slice D_b is 0
+                        SliceBox16 w0 = { 1, 0, 1, 0 }, w1 = { 1, 0, 1, 0 };
+                        if (k0 >= 0 && k0 < P.Nw) w0 = load_box(wbox, (size_t)(cp0 + c) * P.Nw + k0);
+                        if (k0 + 1 >= 0 && k0 + 1 < P.Nw) w1 = load_box(wbox, (size_t)(cp0 + c) * P.Nw + k0 + 1);
+                        const bool v00 = i0 >= w0.u0 && i0 <= w0.u1, v10 = i0 + 1 >= w0.u0 && i0 + 1 <= w0.u1;
+                        const bool v01 = i0 >= w1.u0 && i0 <= w1.u1, v11 = i0 + 1 >= w1.u0 && i0 + 1 <= w1.u1;
+                        n_valid = (int)v00 + (int)v10 + (int)v01 + (int)v11;
+                        if (n_valid) {
+                            const int rs = d.pv, ks = d.pu * d.pv;
+                            const int o00 = (k0 * d.pu + (i0 - d.ri0)) * rs;
+                            const int any_off = v00 ? o00 : (v10 ? o00 + rs : (v01 ? o00 + ks : o00 + ks + rs));
+                            R.base = D + (size_t)c * (size_t)P.stride_cp - d.rj0;
+                            R.off[0] = v00 ? o00 : any_off; R.off[1] = v10 ? o00 + rs : any_off;
+                            R.off[2] = v01 ? o00 + ks : any_off; R.off[3] = v11 ? o00 + ks + rs : any_off;
+                            R.w[0] = v00 ? d.scale * ((1.f - tu) * (1.f - tw)) : 0.f; R.w[1] = v10 ? d.scale * (tu * (1.f - tw)) : 0.f;
+                            R.w[2] = v01 ? d.scale * ((1.f - tu) * tw) : 0.f; R.w[3] = v11 ? d.scale * (tu * tw) : 0.f;
+                            // a slice none of whose rows is valid gets an empty z-range: its (folded) rows are not read at all
+                            R.zlo0 = (v00 || v10) ? w0.v0 : (short)0; R.zhi0 = (v00 || v10) ? (short)(w0.v1 + 1) : (short)0;
+                            R.zlo1 = (v01 || v11) ? w1.v0 : (short)0; R.zhi1 = (v01 || v11) ? (short)(w1.v1 + 1) : (short)0;
+                        }
+                    }
+                    R.n_valid = n_valid;
+                }
+                __syncthreads();
+                // phase B: half-warp `col` adds the round's control points, in list order
+                const int nround = min(GD_CPB, n_list - q0);
+                if (b_inside) {
+#pragma unroll 4
+                    for (int e = 0; e < nround; ++e) {
+                        const GatherRec &R = rec[e][col];
+                        if (R.n_valid == 0) continue;
+                        const float *p = R.base;
+                        const int o0 = R.off[0], o1 = R.off[1], o2 = R.off[2], o3 = R.off[3];
+                        const float w0 = R.w[0], w1 = R.w[1], w2 = R.w[2], w3 = R.w[3];
+                        const int zlo0 = R.zlo0, zhi0 = R.zhi0, zlo1 = R.zlo1, zhi1 = R.zhi1;
+#pragma unroll
+                        for (int ps = 0; ps < GD_MAXPASS; ++ps) {
+                            if (ps < npass) {
+                                const int z = zb + ps * GD_ZSPAN + 4 * lane16;
+                                const bool in0 = z >= zlo0 && z < zhi0, in1 = z >= zlo1 && z < zhi1;
+                                float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, f = a;
+                                if (in0) { a = __ldg(reinterpret_cast<const float4 *>(p + o0 + z)); b = __ldg(reinterpret_cast<const float4 *>(p + o1 + z)); }
+                                if (in1) { c = __ldg(reinterpret_cast<const float4 *>(p + o2 + z)); f = __ldg(reinterpret_cast<const float4 *>(p + o3 + z)); }
+                                acc[ps].x += w0 * a.x + w1 * b.x + w2 * c.x + w3 * f.x;
+                                acc[ps].y += w0 * a.y + w1 * b.y + w2 * c.y + w3 * f.y;
+                                acc[ps].z += w0 * a.z + w1 * b.z + w2 * c.z + w3 * f.z;
+                                acc[ps].w += w0 * a.w + w1 * b.w + w2 * c.w + w3 * f.w;
+                            }
+                        }
+                    }
+                }
+            }
+            if (b_inside) {
+#pragma unroll
+                for (int ps = 0; ps < GD_MAXPASS; ++ps) {
+                    if (ps >= npass) continue;
+                    const int z = zb + ps * GD_ZSPAN + 4 * lane16;
+                    const float v[4] = { acc[ps].x, acc[ps].y, acc[ps].z, acc[ps].w };
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        if (z + e < zmax) {
+                            float *o = dose + ((size_t)(z + e) * P.ny + by) * P.nx + bx;
+                            *o = (accumulate || c0 > 0) ? *o + v[e] : v[e];
+                        }
+                    }
                 }
             }
         }
     }
-    // partial sums of the four warps of a patch, added in a fixed order
-    __syncthreads();
-    if (split > 0) {
-#pragma unroll
-        for (int gq = 0; gq < 8; ++gq) part[(split - 1) * 2 + patch][gq][lane] = acc[gq];
-    }
-    __syncthreads();
-    if (split > 0) return;
-#pragma unroll
-    for (int gq = 0; gq < 8; ++gq) {
-#pragma unroll
-        for (int sp = 0; sp < GATHER_SPLIT - 1; ++sp) {
-            const float4 v = part[sp * 2 + patch][gq][lane];
-            acc[gq].x += v.x; acc[gq].y += v.y; acc[gq].z += v.z; acc[gq].w += v.w;
-        }
-    }
-#pragma unroll
-    for (int gq = 0; gq < 8; ++gq) {
-        const int col = 4 * gq + sub;
-        const int ox = px0 + (col & 7), oy = py0 + (col >> 3);
-        if (ox >= P.nx || oy >= P.ny) continue;
-        const float v[4] = { acc[gq].x, acc[gq].y, acc[gq].z, acc[gq].w };
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const int iz = z0 + zl + e;
-            if (iz < P.nz) {
-                float *o = dose + ((size_t)iz * P.ny + oy) * P.nx + ox;
-                *o = accumulate ? *o + v[e] : v[e];
-            }
-        }
-    }
+    (void)lane;
 }
 
-// S9.  gPhimap_b[pix] = sum_k mag_k^2 sum_{voxels} weight(voxel -> pix) * H_b[voxel]  in gather form.  The bilinear
-// weight is separable, weight = wa(i; a, k) * wb(j; b, k), so a warp owns a tile of 8 (a) x 32 (b, lanes: the
-// contiguous axis of H_b) pixels of the fluence support bbox and, per slice, walks the few voxel rows i that reach
-// its 8 pixel columns: each lane contracts its (at most 4) voxels along v once per row, t = sum_j wb H[k][i][j]
-// (coalesced), and adds wa * t to the pixels a that row reaches.  Grid: (ceil(Nuf/8) * ceil(Nvf/32), n_cp); the
-// 8 warps of a block take the slices k = warp, warp + 8, ... of the same tile and are reduced through shared
-// memory in a fixed order (deterministic, no atomics).
-struct SliceGeo { float mag, su, sv, iu, iv; int u0, u1, v0, v1; };   // su = mag*du/Du, iu = Du/(mag*du)
+// S9.  gPhimap_b[pix] = sum_k mag_k^2 sum_{voxels} weight(voxel -> pix) * H_b[voxel]  in gather form.  The bilinear weight
+// is separable, weight = wa(i; a, k) * wb(j; b, k).  A warp owns 32 pixel rows b of the fluence support bbox (lanes: b, the
+// contiguous axis of H_b) and ALL pixel columns a.  Per slice it walks the voxel rows i of S_k once, in increasing i:
+// each lane contracts its (at most 4) voxels along v, t = sum_j wb H[k][i][j] (coalesced), and the row adds (1-ta) t to
+// pixel column a(i) and ta t to a(i)+1.  Since a(i) never decreases along the walk, two running sums suffice; a finished
+// column is added to the warp's private plane in shared memory.  The slices of a control point are dealt round-robin to
+// the 32 warps of a CLUSTER of four blocks; the planes are reduced in a fixed order, first inside each block, then across
+// the cluster through distributed shared memory (deterministic, no atomics).
+// Grid: (4 * ceil(Nvf/32), n_cp), cluster (4,1,1); dynamic shared memory n_act * Nuf * 32 floats.
+constexpr int PA_THREADS = 256, PA_WARPS = PA_THREADS / 32, PA_CLUSTER = 4, PA_TAPS = 4, PA_ROWS = 4;
 
-constexpr int PROJ_THREADS = 256, PROJ_KG = PROJ_THREADS / 32, PROJ_A = 8, PROJ_TAPS = 4;
-
-__global__ void __launch_bounds__(PROJ_THREADS)
-k_project_adjoint(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const float *__restrict__ H,
-                  float *__restrict__ gphimap)
+__global__ void __cluster_dims__(PA_CLUSTER, 1, 1) __launch_bounds__(PA_THREADS)
+k_project_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp, int n_act,
+                  const float *__restrict__ H, float *__restrict__ gphimap)
 {
-    extern __shared__ float4 proj_smem4[];
-    SliceGeo *geo = reinterpret_cast<SliceGeo *>(proj_smem4);
-    __shared__ float red[PROJ_KG][PROJ_A][32];
+    extern __shared__ float pa_smem[];                  // [n_act][bw][32]: n_act <= PA_WARPS warps work (very wide maps: fewer planes fit)
+    cg::cluster_group cluster = cg::this_cluster();
+    const int crank = (int)cluster.block_rank(), bchunk = blockIdx.x / PA_CLUSTER;
     const int slot = blockIdx.y;
-    if (slot >= n_cp) return;
     const int cp = cp0 + slot;
     const CpDesc d = desc[cp];
+    // every block of a cluster shares (cp, bchunk): the early exits are taken by the whole cluster
     if (d.a0 > d.a1) return;
-    const int nag = (P.Nuf + PROJ_A - 1) / PROJ_A;
-    const int ag = blockIdx.x % nag, bg = blockIdx.x / nag;
-    const int A0 = d.a0 + ag * PROJ_A, B0 = d.b0 + bg * 32;
-    if (A0 > d.a1 || B0 > d.b1) return;
-    const int A1 = min(d.a1, A0 + PROJ_A - 1);
-    const int tid = threadIdx.x, lane = tid & 31, kg = tid >> 5;
-    for (int k = tid; k < P.Nw; k += PROJ_THREADS) {
-        const SliceBox S = slice_support(P, d, k);
-        const float dist = P.sid + P.wmin + k * P.dw, mag = P.sid / dist;
-        SliceGeo q;
-        q.mag = mag; q.su = mag * P.du / P.Du; q.sv = mag * P.dv / P.Dv;
-        q.iu = P.Du / (mag * P.du); q.iv = P.Dv / (mag * P.dv);
-        q.u0 = S.u0; q.u1 = S.u1; q.v0 = S.v0; q.v1 = S.v1;
-        geo[k] = q;
-    }
-    __syncthreads();
+    const int B0 = d.b0 + 32 * bchunk;
+    if (B0 > d.b1) return;
+    const int bw = d.a1 - d.a0 + 1;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    float *plane = pa_smem + (size_t)min(warp, n_act - 1) * bw * 32;
+    if (warp < n_act)
+        for (int e = lane; e < bw * 32; e += 32) plane[e] = 0.f;
+    __syncwarp();
     const int b = B0 + lane;
     const bool live = b <= d.b1;
     const float *Hc = H + (size_t)slot * (size_t)P.stride_cp;
     const float vb = P.v0 / P.dv;                       // v_j / dv = vb + j
-    float acc[PROJ_A];
-#pragma unroll
-    for (int q = 0; q < PROJ_A; ++q) acc[q] = 0.f;
-    for (int k = kg; k < P.Nw; k += PROJ_KG) {
-        const SliceGeo q = geo[k];
-        if (q.u0 > q.u1 || q.v0 > q.v1) continue;
-        // voxels with fa(i) in (A0-1, A1+1):  i - cu in ((A0-1-cuf) iu, (A1+1-cuf) iu)
-        const int ilo = max(q.u0, (int)floorf((A0 - 1 - P.cuf) * q.iu + P.cu)), ihi = min(q.u1, (int)ceilf((A1 + 1 - P.cuf) * q.iu + P.cu));
-        int jlo = max(q.v0, (int)floorf((b - 1 - P.cvf) * q.iv - vb)), jhi = min(q.v1, (int)ceilf((b + 1 - P.cvf) * q.iv - vb));
+    for (int k = warp < n_act ? crank * n_act + warp : P.Nw; k < P.Nw; k += PA_CLUSTER * n_act) {
+        const SliceBox16 S = load_box(sbox, (size_t)cp * P.Nw + k);
+        if (S.u0 > S.u1) continue;
+        const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
+        const float su = mag * P.du / P.Du, sv = mag * P.dv / P.Dv, iv = P.Dv / (mag * P.dv);
+        int jlo = max((int)S.v0, (int)floorf((b - 1 - P.cvf) * iv - vb)), jhi = min((int)S.v1, (int)ceilf((b + 1 - P.cvf) * iv - vb));
         if (!live) jhi = jlo - 1;
-        const float m2 = q.mag * q.mag;
-        // v weights of this lane's (at most PROJ_TAPS) voxels, once per slice; wider stencils (beam voxels much finer than the
-        // map pixels) take the general loop
-        const bool few = __all_sync(0xffffffffu, jhi - jlo < PROJ_TAPS);
-        float wbq[PROJ_TAPS];
+        // v weights of this lane's (at most PA_TAPS) voxels, once per slice, times mag^2; wider stencils (beam voxels much finer
+        // than the map pixels) take the general loop
+        const bool few = __all_sync(0xffffffffu, jhi - jlo < PA_TAPS);
+        float wbq[PA_TAPS];
 #pragma unroll
-        for (int e = 0; e < PROJ_TAPS; ++e) {
-            const float wb = 1.f - fabsf((vb + jlo + e) * q.sv + P.cvf - (float)b);
-            wbq[e] = (jlo + e <= jhi && wb > 0.f) ? wb : 0.f;
+        for (int e = 0; e < PA_TAPS; ++e) {
+            const float wb = 1.f - fabsf((vb + jlo + e) * sv + P.cvf - (float)b);
+            wbq[e] = (jlo + e <= jhi && wb > 0.f) ? m2 * wb : 0.f;
         }
-        for (int i = ilo; i <= ihi; ++i) {
-            const float *hrow = Hc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
-            float t = 0.f;
-            if (few) {
-                float hv[PROJ_TAPS];
+        const float *hrow = Hc + ((size_t)k * d.pu + (S.u0 - d.ri0)) * d.pv - d.rj0;      // row S.u0; rows are d.pv apart
+        int a_cur = (int)floorf((S.u0 - P.cu) * su + P.cuf);                              // warp-uniform
+        float acc_lo = 0.f, acc_hi = 0.f;
+        for (int i = S.u0; i <= S.u1; i += PA_ROWS) {
+            float t[PA_ROWS];
 #pragma unroll
-                for (int e = 0; e < PROJ_TAPS; ++e) hv[e] = wbq[e] != 0.f ? __ldg(hrow + jlo + e) : 0.f;
+            for (int r = 0; r < PA_ROWS; ++r) {           // the loads of PA_ROWS rows are issued before any of them is used
+                t[r] = 0.f;
+                if (i + r <= S.u1) {
+                    const float *h = hrow + (size_t)r * d.pv;
+                    if (few) {
+                        float hv[PA_TAPS];
 #pragma unroll
-                for (int e = 0; e < PROJ_TAPS; ++e) t = fmaf(wbq[e], hv[e], t);
-            } else {
-                for (int j = jlo; j <= jhi; ++j) {
-                    const float wb = 1.f - fabsf((vb + j) * q.sv + P.cvf - (float)b);
-                    if (wb > 0.f) t = fmaf(wb, __ldg(hrow + j), t);
+                        for (int e = 0; e < PA_TAPS; ++e) hv[e] = wbq[e] != 0.f ? __ldg(h + jlo + e) : 0.f;
+#pragma unroll
+                        for (int e = 0; e < PA_TAPS; ++e) t[r] = fmaf(wbq[e], hv[e], t[r]);
+                    } else {
+                        for (int j = jlo; j <= jhi; ++j) {
+                            const float wb = 1.f - fabsf((vb + j) * sv + P.cvf - (float)b);
+                            if (wb > 0.f) t[r] = fmaf(m2 * wb, __ldg(h + j), t[r]);
+                        }
+                    }
                 }
             }
-            t *= m2;
-            const float fa = (i - P.cu) * q.su + P.cuf - (float)A0;      // uniform across the warp
+            hrow += (size_t)PA_ROWS * d.pv;
 #pragma unroll
-            for (int e = 0; e < PROJ_A; ++e) {
-                const float wa = 1.f - fabsf(fa - (float)e);
-                if (wa > 0.f) acc[e] = fmaf(wa, t, acc[e]);
+            for (int r = 0; r < PA_ROWS; ++r) {
+                if (i + r > S.u1) break;
+                const float fa = (i + r - P.cu) * su + P.cuf;
+                const float fla = floorf(fa);
+                const int a0 = (int)fla;
+                const float ta = fa - fla;
+                while (a_cur < a0) {                      // column a_cur is complete (a(i) never decreases): warp-uniform
+                    if (a_cur >= d.a0 && a_cur <= d.a1) plane[(a_cur - d.a0) * 32 + lane] += acc_lo;
+                    acc_lo = acc_hi; acc_hi = 0.f; ++a_cur;
+                }
+                acc_lo = fmaf(1.f - ta, t[r], acc_lo);
+                acc_hi = fmaf(ta, t[r], acc_hi);
             }
         }
+        if (a_cur >= d.a0 && a_cur <= d.a1) plane[(a_cur - d.a0) * 32 + lane] += acc_lo;
+        if (a_cur + 1 >= d.a0 && a_cur + 1 <= d.a1) plane[(a_cur + 1 - d.a0) * 32 + lane] += acc_hi;
     }
-#pragma unroll
-    for (int e = 0; e < PROJ_A; ++e) red[kg][e][lane] = acc[e];
     __syncthreads();
-    {
-        const int e = tid >> 5;                          // PROJ_A == PROJ_KG: thread (e, lane) sums one pixel
+    // the block's warps, in warp order, into plane 0
+    for (int e = tid; e < bw * 32; e += PA_THREADS) {
+        float s = 0.f;
+        for (int w = 0; w < n_act; ++w) s += pa_smem[(size_t)w * bw * 32 + e];
+        pa_smem[e] = s;
+    }
+    cluster.sync();
+    // the cluster's blocks, in rank order; block r writes the pixels e = r, r + 4, ... (a fastest in gphimap)
+    const float *remote[PA_CLUSTER];
+#pragma unroll
+    for (int q = 0; q < PA_CLUSTER; ++q) remote[q] = cluster.map_shared_rank(pa_smem, q);
+    for (int t = crank * PA_THREADS + tid; t < bw * 32; t += PA_CLUSTER * PA_THREADS) {
+        const int a = t % bw, bl = t / bw;               // consecutive threads: consecutive a
         float s = 0.f;
 #pragma unroll
-        for (int q = 0; q < PROJ_KG; ++q) s += red[q][e][lane];
-        if (live && A0 + e <= A1) gphimap[((size_t)cp * P.Nvf + b) * P.Nuf + A0 + e] = s;
+        for (int q = 0; q < PA_CLUSTER; ++q) s += remote[q][a * 32 + bl];
+        if (B0 + bl <= d.b1) gphimap[((size_t)cp * P.Nvf + B0 + bl) * P.Nuf + d.a0 + a] = s;
     }
+    cluster.sync();                                      // nobody leaves while its shared memory is still being read
 }
 
 }  // namespace pdrt

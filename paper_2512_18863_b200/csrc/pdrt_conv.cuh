@@ -58,12 +58,15 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 constexpr int PROJECT_THREADS = 128;
 
-// S3.  Phivol over S_k (Eq. 5-6) into the compact block of the control point.  Grid: (X, n_cp); a block takes the slices
-// k = blockIdx.x, blockIdx.x + X, ...; a thread owns one 16-byte quad of four consecutive v (the contiguous axis) and walks
-// the rows of S_k that fall to it: the column terms of its four voxels (pixel row b, weights, validity) are worked out
-// once per slice, the row terms once per row, and every store is one aligned float4.  The map is read with v fastest.
-// Columns [S.v0 & ~3, S.v1 | 3] are written (the conv stages its tiles in aligned pairs; the extra columns are
-// structural zeros and lie inside the region because rj0 % 8 == 0 and pv % 8 == 0).
+// S3.  Phivol over S_k (Eq. 5-6) into the compact block of the control point.  The bilinear sample is separable:
+//   Phivol(i,j) = (1-ta) T[a][j] + ta T[a+1][j],   T[a][j] = mag^2 ((1-tb) Phimap[a][b] + tb Phimap[a][b+1]),
+// with (a, ta) a function of the row i and (b, tb) of the column j.  A THREAD owns one 16-byte quad of four consecutive v
+// (the contiguous axis) of one slice and walks down the rows i of S_k: the column terms of its four voxels are worked out
+// once, the pixel row a(i) never decreases along the walk, so the thread keeps T[a] and T[a+1] of its quad in registers and
+// evaluates each pixel row once (8 map reads), and every voxel row costs 8 multiply-adds and one aligned float4 store.
+// A block works on PROJECT_THREADS / qw slices at a time (qw = quads per row of the widest slice); no shared memory,
+// no barrier.  Columns [S.v0 & ~3, S.v1 | 3] are written (the conv stages its tiles in aligned pairs; the extra
+// columns are structural zeros and lie inside the region because rj0 % 8 == 0 and pv % 8 == 0).  Grid: (X, n_cp).
 __global__ void __launch_bounds__(PROJECT_THREADS)
 k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp,
           const float *__restrict__ phimapT, float *__restrict__ vol)
@@ -75,21 +78,23 @@ k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restric
     if (d.a0 > d.a1) return;
     const float *pm = phimapT + (size_t)cp * P.Nuf * P.Nvf;
     float *vc = vol + (size_t)slot * (size_t)P.stride_cp;
-    const int tid = threadIdx.x;
-    for (int k = blockIdx.x; k < P.Nw; k += gridDim.x) {
+    // quads per row of the widest slice: S_k grows with the distance from the source, and its first column may round down
+    const SliceBox16 Sl = load_box(sbox, (size_t)cp * P.Nw + P.Nw - 1), Sf = load_box(sbox, (size_t)cp * P.Nw);
+    const int wide = max(Sl.u0 <= Sl.u1 ? Sl.v1 - Sl.v0 + 1 : 0, Sf.u0 <= Sf.u1 ? Sf.v1 - Sf.v0 + 1 : 0);
+    const int qw = min(PROJECT_THREADS, (wide + 3) / 4 + 1);
+    const int spb = PROJECT_THREADS / qw;                       // slices per block iteration
+    const int ks = threadIdx.x / qw, jq = threadIdx.x - ks * qw;
+    if (ks >= spb) return;
+    for (int k = blockIdx.x * spb + ks; k < P.Nw; k += gridDim.x * spb) {
         const SliceBox16 S = load_box(sbox, (size_t)cp * P.Nw + k);
         if (S.u0 > S.u1) continue;
         const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
         const float su = mag * P.du / P.Du, sv = mag / P.Dv;
-        const int j0 = S.v0 & ~3, nq = (((int)S.v1 | 3) - j0 + 1) >> 2;          // quads per row
-        float *slice = vc + (size_t)k * d.pu * d.pv - d.rj0;
-        for (int q0 = 0; q0 < nq; q0 += PROJECT_THREADS) {                       // one pass unless a row holds > 128 quads
-            const int nqc = min(nq - q0, PROJECT_THREADS), rows = PROJECT_THREADS / nqc;
-            const int ri = tid / nqc, jq = q0 + tid - ri * nqc;
-            if (ri >= rows) continue;
+        const int j0 = S.v0 & ~3, nq = (((int)S.v1 | 3) - j0 + 1) >> 2;
+        for (int q = jq; q < nq; q += qw) {                    // one pass (a second one only if a slice is wider than the bound)
             // column terms of this thread's four voxels: m2-scaled weights of pixel rows b and b+1; invalid rows get weight 0
             // and are folded onto a valid one, so that every address is readable
-            const int jb = j0 + 4 * jq;
+            const int jb = j0 + 4 * q;
             float wb0[4], wb1[4];
             int ib0[4], ib1[4];
 #pragma unroll
@@ -104,37 +109,80 @@ k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restric
                 wb0[e] = v0 ? m2 * (1.f - tb) : 0.f; wb1[e] = v1 ? m2 * tb : 0.f;
                 ib0[e] = v0 ? b : (v1 ? b + 1 : d.b0); ib1[e] = v1 ? b + 1 : ib0[e];
             }
-            for (int i = S.u0 + ri; i <= S.u1; i += rows) {
+            auto row_T = [&](int a, float (&T)[4]) {            // T[a][quad]; zero outside the support bbox
+                if (a >= d.a0 && a <= d.a1) {
+                    const float *pc = pm + a * P.Nvf;
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) T[e] = wb0[e] * __ldg(pc + ib0[e]) + wb1[e] * __ldg(pc + ib1[e]);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) T[e] = 0.f;
+                }
+            };
+            int a_cur = (int)floorf((S.u0 - P.cu) * su + P.cuf);
+            float T0[4], T1[4];
+            row_T(a_cur, T0);
+            row_T(a_cur + 1, T1);
+            float *op = vc + ((size_t)k * d.pu + (S.u0 - d.ri0)) * d.pv + (jb - d.rj0);
+            for (int i = S.u0; i <= S.u1; ++i, op += d.pv) {
                 const float fa = (i - P.cu) * su + P.cuf;
                 const float fla = floorf(fa);
                 const int a = (int)fla;
                 const float ta = fa - fla;
-                const bool a0 = a >= d.a0 && a <= d.a1, a1 = a + 1 >= d.a0 && a + 1 <= d.a1;
-                const float wa0 = a0 ? 1.f - ta : 0.f, wa1 = a1 ? ta : 0.f;
-                const float *pc0 = pm + (a0 ? a : (a1 ? a + 1 : d.a0)) * P.Nvf, *pc1 = pm + (a1 ? a + 1 : (a0 ? a : d.a0)) * P.Nvf;
-                float o[4];
+                while (a_cur < a) {                            // a(i) never decreases along the walk
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const float r0 = wb0[e] * __ldg(pc0 + ib0[e]) + wb1[e] * __ldg(pc0 + ib1[e]);
-                    const float r1 = wb0[e] * __ldg(pc1 + ib0[e]) + wb1[e] * __ldg(pc1 + ib1[e]);
-                    o[e] = wa0 * r0 + wa1 * r1;
+                    for (int e = 0; e < 4; ++e) T0[e] = T1[e];
+                    ++a_cur;
+                    row_T(a_cur + 1, T1);
                 }
-                *reinterpret_cast<float4 *>(slice + (size_t)(i - d.ri0) * d.pv + jb) = make_float4(o[0], o[1], o[2], o[3]);
+                *reinterpret_cast<float4 *>(op) = make_float4(T0[0] + ta * (T1[0] - T0[0]), T0[1] + ta * (T1[1] - T0[1]),
+                                                               T0[2] + ta * (T1[2] - T0[2]), T0[3] + ta * (T1[3] - T0[3]));
             }
         }
     }
 }
 
-constexpr int RA_THREADS = 256, RA_MAXC = 9;
-struct RaRow {                      // one beam row (k, i) of G_b: its patient-column candidates, compacted
+constexpr int RA_THREADS = 256, RA_MAXC = 9, RA_PADC = 12;
+struct __align__(16) RaRow {        // one beam row (k, i) of G_b: its patient-column candidates, compacted
+    int off[RA_PADC];               // offsets of gT[y][x][0]; entries past n repeat entry 0 ...
+    float w[RA_PADC];               // ... with weight 0, so that the stream loop needs no predicates
     int n;                          // candidates with a non-zero weight; -1: nothing to write; -2: stencil wider than 3 x 3
     int out;                        // offset of G_b(k, i, v = 0) in the control point's compact block
     int j0, nq;                     // first column (multiple of 4) and number of quads to write
-    int off[RA_MAXC];               // offsets of gT[y][x][0]
-    float w[RA_MAXC];
     int xa, xb, ya, yb;             // candidate box of the general path
     float eu0, ew0;
+    int pad_[2];
 };
+
+// one quad of one beam row from NC candidates (the first NC entries of the row's list), no predicates
+template <int NC>
+__device__ __forceinline__ void ra_stream(const RaRow &R, const float *__restrict__ gT, float *__restrict__ orow, int lane16)
+{
+    for (int q = lane16; q < R.nq; q += 16) {
+        const int j = R.j0 + 4 * q;
+        int off[NC];
+        float w[NC];
+#pragma unroll
+        for (int c4 = 0; c4 < NC; c4 += 4) {                  // 16-byte broadcast reads of the list
+            const int4 o = *reinterpret_cast<const int4 *>(&R.off[c4]);
+            const float4 f = *reinterpret_cast<const float4 *>(&R.w[c4]);
+            off[c4] = o.x; w[c4] = f.x;
+            if (c4 + 1 < NC) { off[c4 + 1] = o.y; w[c4 + 1] = f.y; }
+            if (c4 + 2 < NC) { off[c4 + 2] = o.z; w[c4 + 2] = f.z; }
+            if (c4 + 3 < NC) { off[c4 + 3] = o.w; w[c4 + 3] = f.w; }
+        }
+        float4 v[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) v[c] = __ldg(reinterpret_cast<const float4 *>(gT + (off[c] + j)));     // all loads first
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            acc.x = fmaf(w[c], v[c].x, acc.x); acc.y = fmaf(w[c], v[c].y, acc.y);
+            acc.z = fmaf(w[c], v[c].z, acc.z); acc.w = fmaf(w[c], v[c].w, acc.w);
+        }
+        *reinterpret_cast<float4 *>(orow + j) = acc;
+    }
+}
 
 // S7.  G_b = R_b^T g over F_k in gather form: G_b(i,j,k) = sum over the patient voxels (x,y) of slice z = j whose
 // bilinear stencil (as evaluated by k_gather_dose) reaches beam voxel (i,k), weight (1-|du|)(1-|dw|), times g.
@@ -142,8 +190,10 @@ struct RaRow {                      // one beam row (k, i) of G_b: its patient-c
 // beam rows (k, i) of the control point's region at a time.  Phase A: one THREAD per row works out the (at most 3 x 3)
 // candidate columns and keeps those with a non-zero weight (4 on average) in shared memory.  Phase B: one HALF-WARP per
 // row streams 16-byte vectors along v: coalesced reads of gT[y][x][v] (dL/dDose with z fastest, row pitch padded to a
-// multiple of 4, L2-resident) and one aligned float4 store per lane.  Grid: (X, n_cp), blocks stride over the row chunks.
-__global__ void __launch_bounds__(RA_THREADS)
+// multiple of 4, L2-resident) and one aligned float4 store per lane; the loop is specialised on the number of candidates
+// (4, 6 or 9: the list is padded with zero weights) so that it carries no predicates.
+// Grid: (X, n_cp), blocks stride over the row chunks.
+__global__ void __launch_bounds__(RA_THREADS, 3)
 k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp, int C,
                    int nzp, const float *__restrict__ gT, float *__restrict__ G)
 {
@@ -191,6 +241,8 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *
                                 const float wu = 1.f - fabsf(eu0 + cy * fu_y + cx * fu_x), ww = 1.f - fabsf(ew0 + cy * fw_y + cx * fw_x);
                                 if (wu > 0.f && ww > 0.f) { R.off[n] = ((ya + cy) * P.nx + xa + cx) * nzp; R.w[n] = wu * ww; ++n; }
                             }
+                        const int o0 = n > 0 ? R.off[0] : 0;
+                        for (int c = n; c < RA_PADC; ++c) { R.off[c] = o0; R.w[c] = 0.f; }
                     } else {
                         n = -2;
                         R.xa = xa; R.xb = xb; R.ya = ya; R.yb = yb; R.eu0 = eu0; R.ew0 = ew0;
@@ -207,22 +259,9 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *
             if (n == -1) continue;
             float *orow = Gc + R.out;
             if (n >= 0) {
-                for (int q = lane16; q < R.nq; q += 16) {
-                    const int j = R.j0 + 4 * q;
-                    float4 v[RA_MAXC];
-#pragma unroll
-                    for (int c = 0; c < RA_MAXC; ++c)          // all loads first, so that their latencies overlap
-                        if (c < n) v[c] = __ldg(reinterpret_cast<const float4 *>(gT + R.off[c] + j));
-                    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-                    for (int c = 0; c < RA_MAXC; ++c)
-                        if (c < n) {
-                            const float wc = R.w[c];
-                            acc.x = fmaf(wc, v[c].x, acc.x); acc.y = fmaf(wc, v[c].y, acc.y);
-                            acc.z = fmaf(wc, v[c].z, acc.z); acc.w = fmaf(wc, v[c].w, acc.w);
-                        }
-                    *reinterpret_cast<float4 *>(orow + j) = acc;
-                }
+                if (n <= 4) ra_stream<4>(R, gT, orow, lane16);
+                else if (n <= 6) ra_stream<6>(R, gT, orow, lane16);
+                else ra_stream<RA_MAXC>(R, gT, orow, lane16);
             } else {
                 // stencil wider than 3 x 3 (beam voxels much coarser than patient voxels): plain loop over the candidate box
                 for (int jj = lane16; jj < 4 * R.nq; jj += 16) {

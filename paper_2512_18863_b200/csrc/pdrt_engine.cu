@@ -43,7 +43,7 @@ int tile_floats_for(int kt)
     return best;
 }
 // blocks per control point of k_project (a block takes every X-th slice) and of k_resample_adjoint (256 beam rows per chunk)
-int project_blocks(const Params &P) { return std::max(1, std::min(P.Nw, 32)); }
+int project_blocks(const Params &P) { return std::max(1, std::min(P.Nw, 24)); }
 int resample_adj_blocks(const Params &P) { return std::max(1, std::min(48, (P.Nw * (P.Nu + RS) + RA_THREADS - 1) / RA_THREADS)); }
 size_t conv_smem_bytes(int kt) { return sizeof(float) * (2 * (size_t)(kt + 1) * ((kt + 3) & ~3) + tile_floats_for(kt)); }   // row-pair kernel + ring
 

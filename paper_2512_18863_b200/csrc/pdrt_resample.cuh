@@ -20,15 +20,43 @@ constexpr int GD_ZSPAN = 64;                     // z covered by one pass of a h
 constexpr int GD_MAXPASS = 4;                    // passes held in registers at once (256 z)
 constexpr int GD_LIST = 512;                     // control points listed per outer chunk
 
-struct __align__(16) GatherRec {                 // bilinear stencil of one (patient column, control point): 48 bytes
-    const float *base;                           // D_b block of the control point, shifted so that base[off + z] is voxel v = z
-    int n_valid;                                 // 0: nothing to add
-    int pad_;
-    int off[4];                                  // rows (i0,k0), (i0+1,k0), (i0,k0+1), (i0+1,k0+1); invalid ones folded onto a valid row
+struct __align__(16) GatherRec {                 // bilinear stencil of one (patient column, control point): 64 bytes
+    const float *row[4];                         // beam rows (i0,k0), (i0+1,k0), (i0,k0+1), (i0+1,k0+1), shifted so that row[q][z] is voxel
+                                                 // v = z; invalid neighbours are folded onto a valid row
     float w[4];                                  // cal * MU * bilinear weight; 0 for invalid neighbours
     short zlo0, zhi0, zlo1, zhi1;                // written v-range [zlo, zhi) of slice k0 and of slice k0+1 (multiples of 8)
-    int pad2_[2];
+    int n_valid;                                 // 0: nothing to add
+    int pad_;
 };
+
+// phase B of k_gather_dose for one round of control points, NP z-passes of 64 held in registers
+template <int NP>
+__device__ __forceinline__ void gather_round(const GatherRec (*rec)[GD_COLS], int col, int nround, int zq, float2 (&acc)[GD_MAXPASS][2])
+{
+#pragma unroll 2
+    for (int e = 0; e < nround; ++e) {
+        const GatherRec &R = rec[e][col];
+        const int4 meta = *reinterpret_cast<const int4 *>(&R.zlo0);         // z-ranges (4 shorts), n_valid
+        if (meta.z == 0) continue;
+        const float4 w = *reinterpret_cast<const float4 *>(R.w);
+        const float2 w0 = make_float2(w.x, w.x), w1 = make_float2(w.y, w.y), w2 = make_float2(w.z, w.z), w3 = make_float2(w.w, w.w);
+        const int zlo0 = (short)(meta.x & 0xffff), zhi0 = meta.x >> 16, zlo1 = (short)(meta.y & 0xffff), zhi1 = meta.y >> 16;
+        const float *r0 = R.row[0], *r1 = R.row[1], *r2 = R.row[2], *r3 = R.row[3];
+#pragma unroll
+        for (int ps = 0; ps < NP; ++ps) {
+            const int z = zq + ps * GD_ZSPAN;
+            const bool in0 = z >= zlo0 && z < zhi0, in1 = z >= zlo1 && z < zhi1;
+            float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, f = a;
+            if (in0) { a = __ldg(reinterpret_cast<const float4 *>(r0 + z)); b = __ldg(reinterpret_cast<const float4 *>(r1 + z)); }
+            if (in1) { c = __ldg(reinterpret_cast<const float4 *>(r2 + z)); f = __ldg(reinterpret_cast<const float4 *>(r3 + z)); }
+            // packed FFMA2: two z per instruction
+            acc[ps][0] = __ffma2_rn(w0, make_float2(a.x, a.y), acc[ps][0]); acc[ps][1] = __ffma2_rn(w0, make_float2(a.z, a.w), acc[ps][1]);
+            acc[ps][0] = __ffma2_rn(w1, make_float2(b.x, b.y), acc[ps][0]); acc[ps][1] = __ffma2_rn(w1, make_float2(b.z, b.w), acc[ps][1]);
+            acc[ps][0] = __ffma2_rn(w2, make_float2(c.x, c.y), acc[ps][0]); acc[ps][1] = __ffma2_rn(w2, make_float2(c.z, c.w), acc[ps][1]);
+            acc[ps][0] = __ffma2_rn(w3, make_float2(f.x, f.y), acc[ps][0]); acc[ps][1] = __ffma2_rn(w3, make_float2(f.z, f.w), acc[ps][1]);
+        }
+    }
+}
 
 // S6.  Grid: (ceil(nx/8), ceil(ny/2), 1); a block owns 8 x 2 patient columns (x,y) over all z.
 //   dose[p] (+)= sum_b scale_b * bilinear_0(D_b[.][z][.]; fu, fw)
@@ -97,9 +125,9 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
         const int n_list = n_list_s, zmin = zmin_s, zmax = zmax_s;
         if (n_list == 0) continue;
         for (int zb = zmin; zb < zmax; zb += GD_ZSPAN * GD_MAXPASS) {            // one iteration unless the regions span > 256 z
-            float4 acc[GD_MAXPASS];
+            float2 acc[GD_MAXPASS][2];                                           // [pass][z pair] of this lane's quads
 #pragma unroll
-            for (int p = 0; p < GD_MAXPASS; ++p) acc[p] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int p = 0; p < GD_MAXPASS; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
             const int npass = min(GD_MAXPASS, (zmax - zb + GD_ZSPAN - 1) / GD_ZSPAN);
             for (int q0 = 0; q0 < n_list; q0 += GD_CPB) {
                 __syncthreads();                                                 // the records of the previous round are consumed
@@ -125,9 +153,9 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
                             const int rs = d.pv, ks = d.pu * d.pv;
                             const int o00 = (k0 * d.pu + (i0 - d.ri0)) * rs;
                             const int any_off = v00 ? o00 : (v10 ? o00 + rs : (v01 ? o00 + ks : o00 + ks + rs));
-                            R.base = D + (size_t)c * (size_t)P.stride_cp - d.rj0;
-                            R.off[0] = v00 ? o00 : any_off; R.off[1] = v10 ? o00 + rs : any_off;
-                            R.off[2] = v01 ? o00 + ks : any_off; R.off[3] = v11 ? o00 + ks + rs : any_off;
+                            const float *base = D + (size_t)c * (size_t)P.stride_cp - d.rj0;
+                            R.row[0] = base + (v00 ? o00 : any_off); R.row[1] = base + (v10 ? o00 + rs : any_off);
+                            R.row[2] = base + (v01 ? o00 + ks : any_off); R.row[3] = base + (v11 ? o00 + ks + rs : any_off);
                             R.w[0] = v00 ? d.scale * ((1.f - tu) * (1.f - tw)) : 0.f; R.w[1] = v10 ? d.scale * (tu * (1.f - tw)) : 0.f;
                             R.w[2] = v01 ? d.scale * ((1.f - tu) * tw) : 0.f; R.w[3] = v11 ? d.scale * (tu * tw) : 0.f;
                             // a slice none of whose rows is valid gets an empty z-range: its (folded) rows are not read at all
@@ -141,29 +169,10 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
                 // phase B: half-warp `col` adds the round's control points, in list order
                 const int nround = min(GD_CPB, n_list - q0);
                 if (b_inside) {
-#pragma unroll 4
-                    for (int e = 0; e < nround; ++e) {
-                        const GatherRec &R = rec[e][col];
-                        if (R.n_valid == 0) continue;
-                        const float *p = R.base;
-                        const int o0 = R.off[0], o1 = R.off[1], o2 = R.off[2], o3 = R.off[3];
-                        const float w0 = R.w[0], w1 = R.w[1], w2 = R.w[2], w3 = R.w[3];
-                        const int zlo0 = R.zlo0, zhi0 = R.zhi0, zlo1 = R.zlo1, zhi1 = R.zhi1;
-#pragma unroll
-                        for (int ps = 0; ps < GD_MAXPASS; ++ps) {
-                            if (ps < npass) {
-                                const int z = zb + ps * GD_ZSPAN + 4 * lane16;
-                                const bool in0 = z >= zlo0 && z < zhi0, in1 = z >= zlo1 && z < zhi1;
-                                float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, f = a;
-                                if (in0) { a = __ldg(reinterpret_cast<const float4 *>(p + o0 + z)); b = __ldg(reinterpret_cast<const float4 *>(p + o1 + z)); }
-                                if (in1) { c = __ldg(reinterpret_cast<const float4 *>(p + o2 + z)); f = __ldg(reinterpret_cast<const float4 *>(p + o3 + z)); }
-                                acc[ps].x += w0 * a.x + w1 * b.x + w2 * c.x + w3 * f.x;
-                                acc[ps].y += w0 * a.y + w1 * b.y + w2 * c.y + w3 * f.y;
-                                acc[ps].z += w0 * a.z + w1 * b.z + w2 * c.z + w3 * f.z;
-                                acc[ps].w += w0 * a.w + w1 * b.w + w2 * c.w + w3 * f.w;
-                            }
-                        }
-                    }
+                    const int zq = zb + 4 * lane16;
+                    if (npass == 1) gather_round<1>(rec, col, nround, zq, acc);
+                    else if (npass == 2) gather_round<2>(rec, col, nround, zq, acc);
+                    else gather_round<GD_MAXPASS>(rec, col, nround, zq, acc);
                 }
             }
             if (b_inside) {
@@ -171,7 +180,7 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
                 for (int ps = 0; ps < GD_MAXPASS; ++ps) {
                     if (ps >= npass) continue;
                     const int z = zb + ps * GD_ZSPAN + 4 * lane16;
-                    const float v[4] = { acc[ps].x, acc[ps].y, acc[ps].z, acc[ps].w };
+                    const float v[4] = { acc[ps][0].x, acc[ps][0].y, acc[ps][1].x, acc[ps][1].y };
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
                         if (z + e < zmax) {
@@ -226,7 +235,8 @@ k_project_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *_
         if (S.u0 > S.u1) continue;
         const float mag = P.sid / (P.sid + P.wmin + k * P.dw), m2 = mag * mag;
         const float su = mag * P.du / P.Du, sv = mag * P.dv / P.Dv, iv = P.Dv / (mag * P.dv);
-        int jlo = max((int)S.v0, (int)floorf((b - 1 - P.cvf) * iv - vb)), jhi = min((int)S.v1, (int)ceilf((b + 1 - P.cvf) * iv - vb));
+        // voxels with a non-zero weight onto pixel row b: fb(j) in the OPEN interval (b-1, b+1), at most 2 iv + 1 of them
+        int jlo = max((int)S.v0, (int)floorf((b - 1 - P.cvf) * iv - vb) + 1), jhi = min((int)S.v1, (int)ceilf((b + 1 - P.cvf) * iv - vb) - 1);
         if (!live) jhi = jlo - 1;
         // v weights of this lane's (at most PA_TAPS) voxels, once per slice, times mag^2; wider stencils (beam voxels much finer
         // than the map pixels) take the general loop

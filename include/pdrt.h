@@ -222,6 +222,59 @@ PDRT_API int pdrt_stage_grad_fluence(pdrt_engine *engine, int32_t n_cp, const fl
                             const float *gantry_deg_dev, const float *dL_ddose_dev,
                             float *gphimap_dev, void *cuda_stream);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * Planning-loop steps: with these a whole optimisation iteration
+ *     theta^ = pdrt_validate(theta);  jaws = pdrt_track_jaws(theta^);  D = pdrt_dose(theta^);  (L, g) = pdrt_objective(D);
+ *     g^ = pdrt_dose_backward(theta^, g);  g_theta = pdrt_validate_backward(theta, g^);  theta = pdrt_plan_step(theta, g_theta)
+ * runs on the device without leaving the library (and can be captured in a CUDA graph: none of the calls synchronises).
+ * All pointers are device pointers unless named *_host; all calls are asynchronous on `cuda_stream`. */
+
+/* Limits of the hardware-constrained projection, PAPER.md:83-101 (BeamValidationLayer). */
+typedef struct {
+    float leaf_w_min;        /* minimum opening of a leaf pair, w >= w_min (Eq. 1)            */
+    float leaf_F;            /* half field width: pair centre clamped to [-F, F]              */
+    float jaw_w_min;         /* minimum opening of a jaw pair                                 */
+    float jaw_Fx, jaw_Fy;    /* centre range of the (x1,x2) and of the (y1,y2) jaw pair       */
+    float mu_eps;            /* minimum MU per control point (Eq. 3; pdrt_mu_epsilon)         */
+} pdrt_limits;
+
+/* Eq. 3: eps = D_min * delta_phi / phidot_max — minimum dose rate [MU/s] times control-point spacing
+ * [deg] over maximum gantry speed [deg/s].  Host arithmetic. */
+PDRT_API float pdrt_mu_epsilon(float dose_rate_min, float delta_phi_deg, float gantry_speed_max);
+
+/* Eq. 1-2 on every leaf pair and on the two jaw pairs, and MU >= mu_eps: c = (p_a + p_b)/2, w = p_b - p_a, w >= w_min,
+ * c clamped to [-F, F], p_a^ = c - w/2, p_b^ = c + w/2.  Shapes as in pdrt_dose; outputs may alias the inputs. */
+PDRT_API int pdrt_validate(pdrt_engine *engine, int32_t n_cp, const pdrt_limits *limits,
+                           const float *leaves_dev, const float *jaws_dev, const float *mu_dev,
+                           float *leaves_out_dev, float *jaws_out_dev, float *mu_out_dev, void *cuda_stream);
+
+/* Transposed Jacobian of pdrt_validate at the RAW parameters ("preserve gradients"): maps gradients w.r.t.
+ * the projected parameters (what pdrt_dose_backward returns) to gradients w.r.t. the raw ones.  The map is piecewise
+ * linear; a clamp passes the gradient where its input lies inside the closed interval (reading G23). */
+PDRT_API int pdrt_validate_backward(pdrt_engine *engine, int32_t n_cp, const pdrt_limits *limits,
+                                    const float *leaves_dev, const float *jaws_dev, const float *mu_dev,
+                                    const float *g_leaves_hat_dev, const float *g_jaws_hat_dev, const float *g_mu_hat_dev,
+                                    float *g_leaves_dev, float *g_jaws_dev, float *g_mu_dev, void *cuda_stream);
+
+/* Weighted-sum objective and its dose gradient (Eq. 10 for power = 1; power = 2 is the quadratic
+ * objective of BASELINE.json's c4/c5):  L = sum_s lambda_s sum_{x in s} |D(x) - p_s|^power.  structure_bits_dev
+ * [nz][ny][nx] uint32: bit s set when the voxel belongs to structure s (structures may overlap), n_struct <= 32;
+ * lambda_host / presc_host: n_struct weights and prescriptions (0 for organs at risk).  Writes dL_ddose_dev [nz][ny][nx]
+ * and the loss (float64, device).  power 1: sign(0) = 0. */
+PDRT_API int pdrt_objective(pdrt_engine *engine, const float *dose_dev, const uint32_t *structure_bits_dev, int32_t n_struct,
+                            const float *lambda_host, const float *presc_host, int32_t power,
+                            float *dL_ddose_dev, double *loss_dev, void *cuda_stream);
+
+/* Jaws tracking the aperture (BASELINE.json configs[4]): over the leaf pairs open by more than open_gap_mm (all pairs when
+ * none is) x1 = min l - margin, x2 = max r + margin, y1 / y2 = the leaf boundaries that enclose them.  jaws_dev [n_cp][4]. */
+PDRT_API int pdrt_track_jaws(pdrt_engine *engine, int32_t n_cp, const float *leaves_dev, float margin_mm, float open_gap_mm,
+                             float *jaws_dev, void *cuda_stream);
+
+/* Normalised-gradient step of the c5 planning loop: leaves -= step_leaf * g / max|g| over all leaf edges
+ * of the arc, mu -= step_mu * g / max|g|; a group with an identically zero gradient does not move.  In place. */
+PDRT_API int pdrt_plan_step(pdrt_engine *engine, int32_t n_cp, float step_leaf_mm, float step_mu,
+                            const float *g_leaves_dev, const float *g_mu_dev, float *leaves_dev, float *mu_dev, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -5,4 +5,4 @@ seeded synthetic inputs.  Importing the package does not touch CUDA; creating an
 loudly when the library is not built or no GPU is present (there is no CPU fallback).
 """
 from . import workloads  # noqa: F401
-from .binding import Engine, PdrtError, load_library, LIB_PATH, SYMBOLS, STAGES  # noqa: F401
+from .binding import Engine, PdrtError, PdrtLimits, load_library, LIB_PATH, SYMBOLS, STAGES  # noqa: F401

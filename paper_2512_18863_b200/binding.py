@@ -17,7 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libpdrt.so")
 SYMBOLS = ("pdrt_create", "pdrt_destroy", "pdrt_last_error", "pdrt_set_kernel_size", "pdrt_get_info", "pdrt_get_work",
            "pdrt_set_profiling", "pdrt_get_stage_ms",
            "pdrt_dose", "pdrt_dose_backward", "pdrt_dose_host", "pdrt_dose_backward_host",
-           "pdrt_stage_fluence", "pdrt_stage_depth", "pdrt_stage_beam_dose", "pdrt_stage_grad_fluence")
+           "pdrt_stage_fluence", "pdrt_stage_depth", "pdrt_stage_beam_dose", "pdrt_stage_grad_fluence",
+           "pdrt_mu_epsilon", "pdrt_validate", "pdrt_validate_backward", "pdrt_objective", "pdrt_track_jaws", "pdrt_plan_step")
 
 STAGES = ("fluence", "depth", "scan", "conv", "gather", "resample_adj", "conv_adj", "project_adj", "fluence_adj", "project", "transpose")
 
@@ -62,6 +63,11 @@ class PdrtWork(C.Structure):
                 ("kernel_size", C.c_int32), ("kernel_size_compiled", C.c_int32)]
 
 
+class PdrtLimits(C.Structure):
+    _fields_ = [("leaf_w_min", C.c_float), ("leaf_F", C.c_float), ("jaw_w_min", C.c_float),
+                ("jaw_Fx", C.c_float), ("jaw_Fy", C.c_float), ("mu_eps", C.c_float)]
+
+
 class PdrtError(RuntimeError):
     def __init__(self, code, message):
         super().__init__(f"pdrt error {code}: {message}")
@@ -99,8 +105,16 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.pdrt_stage_depth.argtypes = [vp, i32, vp, vp, vp]
     lib.pdrt_stage_beam_dose.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.pdrt_stage_grad_fluence.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+    f32 = C.c_float
+    lib.pdrt_mu_epsilon.argtypes = [f32, f32, f32]
+    lib.pdrt_mu_epsilon.restype = f32
+    lib.pdrt_validate.argtypes = [vp, i32, C.POINTER(PdrtLimits), vp, vp, vp, vp, vp, vp, vp]
+    lib.pdrt_validate_backward.argtypes = [vp, i32, C.POINTER(PdrtLimits), vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.pdrt_objective.argtypes = [vp, vp, vp, i32, _FP, _FP, i32, vp, vp, vp]
+    lib.pdrt_track_jaws.argtypes = [vp, i32, vp, f32, f32, vp, vp]
+    lib.pdrt_plan_step.argtypes = [vp, i32, f32, f32, vp, vp, vp, vp, vp]
     for name in SYMBOLS:
-        if name not in ("pdrt_destroy", "pdrt_last_error"):
+        if name not in ("pdrt_destroy", "pdrt_last_error", "pdrt_mu_epsilon"):
             getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -250,6 +264,68 @@ class Engine:
                                                 mu.data_ptr(), g.data_ptr(), dl.data_ptr(), dj.data_ptr(),
                                                 dm.data_ptr(), self._stream()))
         return dl, dj, dm
+
+    # ---- planning-loop steps (device tensors; asynchronous on the current stream)
+    def validate(self, limits: PdrtLimits, leaves, jaws, mu, out=None):
+        """pdrt_validate (Eq. 1-3): returns the projected (leaves, jaws, mu)."""
+        torch = self.torch
+        jw = self._dev(jaws)
+        n_cp = int(jw.shape[0])
+        lv, mu = self._dev(leaves, (n_cp, 2, self.n_pairs)), self._dev(mu, (n_cp,))
+        if out is None:
+            out = (torch.empty_like(lv), torch.empty_like(jw), torch.empty_like(mu))
+        self._check(self.lib.pdrt_validate(self.handle, n_cp, C.byref(limits), lv.data_ptr(), jw.data_ptr(), mu.data_ptr(),
+                                           out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), self._stream()))
+        return out
+
+    def validate_backward(self, limits: PdrtLimits, leaves, jaws, mu, g_leaves_hat, g_jaws_hat, g_mu_hat, out=None):
+        """pdrt_validate_backward: gradients w.r.t. the raw parameters from gradients w.r.t. the projected ones."""
+        torch = self.torch
+        jw = self._dev(jaws)
+        n_cp = int(jw.shape[0])
+        lv, mu = self._dev(leaves, (n_cp, 2, self.n_pairs)), self._dev(mu, (n_cp,))
+        gl, gj, gm = self._dev(g_leaves_hat, lv.shape), self._dev(g_jaws_hat, jw.shape), self._dev(g_mu_hat, mu.shape)
+        if out is None:
+            out = (torch.empty_like(lv), torch.empty_like(jw), torch.empty_like(mu))
+        self._check(self.lib.pdrt_validate_backward(self.handle, n_cp, C.byref(limits), lv.data_ptr(), jw.data_ptr(), mu.data_ptr(),
+                                                    gl.data_ptr(), gj.data_ptr(), gm.data_ptr(),
+                                                    out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), self._stream()))
+        return out
+
+    def mu_epsilon(self, dose_rate_min, delta_phi_deg, gantry_speed_max) -> float:
+        return float(self.lib.pdrt_mu_epsilon(dose_rate_min, delta_phi_deg, gantry_speed_max))
+
+    def objective(self, dose, structure_bits, lam, presc, power, out=None):
+        """pdrt_objective: returns (loss as a 1-element float64 device tensor, dL/dDose)."""
+        torch = self.torch
+        d = self._dev(dose, self.dose_shape)
+        assert structure_bits.dtype == torch.int32 and structure_bits.is_cuda and structure_bits.is_contiguous()   # uint32 bit patterns
+        assert tuple(structure_bits.shape) == self.dose_shape
+        lam, presc = _f32(lam), _f32(presc)
+        if out is None:
+            out = (torch.empty(1, dtype=torch.float64, device=self.device), torch.empty_like(d))
+        loss, g = out
+        self._check(self.lib.pdrt_objective(self.handle, d.data_ptr(), structure_bits.data_ptr(), len(lam), _fp(lam), _fp(presc),
+                                            int(power), g.data_ptr(), loss.data_ptr(), self._stream()))
+        return loss, g
+
+    def track_jaws(self, leaves, margin_mm, open_gap_mm, out=None):
+        lv = self._dev(leaves)
+        n_cp = int(lv.shape[0])
+        if out is None:
+            out = self.torch.empty((n_cp, 4), dtype=self.torch.float32, device=self.device)
+        self._check(self.lib.pdrt_track_jaws(self.handle, n_cp, lv.data_ptr(), margin_mm, open_gap_mm, out.data_ptr(), self._stream()))
+        return out
+
+    def plan_step(self, step_leaf_mm, step_mu, g_leaves, g_mu, leaves, mu):
+        """pdrt_plan_step: updates `leaves` and `mu` (float32 CUDA tensors) in place."""
+        torch = self.torch
+        for t in (g_leaves, g_mu, leaves, mu):
+            assert isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+        n_cp = int(mu.shape[0])
+        self._check(self.lib.pdrt_plan_step(self.handle, n_cp, step_leaf_mm, step_mu, g_leaves.data_ptr(), g_mu.data_ptr(),
+                                            leaves.data_ptr(), mu.data_ptr(), self._stream()))
+        return leaves, mu
 
     # ---- host-buffer variants (copies inside the call; synchronous)
     def dose_host(self, leaves, jaws, gantry_deg, mu, out):

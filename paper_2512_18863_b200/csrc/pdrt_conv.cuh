@@ -57,6 +57,7 @@ __device__ __forceinline__ void cp_async_8(unsigned dst, const float *src, int n
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
 constexpr int PROJECT_THREADS = 128;
+constexpr int PROJECT_MAP_FLOATS = 4096;          // support bbox of the fluence map staged in shared memory when it fits (16 KB)
 
 // S3.  Phivol over S_k (Eq. 5-6) into the compact block of the control point.  The bilinear sample is separable:
 //   Phivol(i,j) = (1-ta) T[a][j] + ta T[a+1][j],   T[a][j] = mag^2 ((1-tb) Phimap[a][b] + tb Phimap[a][b+1]),
@@ -64,8 +65,9 @@ constexpr int PROJECT_THREADS = 128;
 // (the contiguous axis) of one slice and walks down the rows i of S_k: the column terms of its four voxels are worked out
 // once, the pixel row a(i) never decreases along the walk, so the thread keeps T[a] and T[a+1] of its quad in registers and
 // evaluates each pixel row once (8 map reads), and every voxel row costs 8 multiply-adds and one aligned float4 store.
-// A block works on PROJECT_THREADS / qw slices at a time (qw = quads per row of the widest slice); no shared memory,
-// no barrier.  Columns [S.v0 & ~3, S.v1 | 3] are written (the conv stages its tiles in aligned pairs; the extra
+// A block works on PROJECT_THREADS / qw slices at a time (qw = quads per row of the widest slice).  The support bbox of
+// the map (a few KB) is staged in shared memory once per block with all its loads in flight together: the walk is a
+// chain of dependent reads, which from shared memory cost 30 cycles each instead of an L2 round trip.  Columns [S.v0 & ~3, S.v1 | 3] are written (the conv stages its tiles in aligned pairs; the extra
 // columns are structural zeros and lie inside the region because rj0 % 8 == 0 and pv % 8 == 0).  Grid: (X, n_cp).
 __global__ void __launch_bounds__(PROJECT_THREADS)
 k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp,
@@ -78,6 +80,14 @@ k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restric
     if (d.a0 > d.a1) return;
     const float *pm = phimapT + (size_t)cp * P.Nuf * P.Nvf;
     float *vc = vol + (size_t)slot * (size_t)P.stride_cp;
+    __shared__ float map_s[PROJECT_MAP_FLOATS];              // [a - a0][b - b0], b fastest
+    const int bw = d.a1 - d.a0 + 1, bh = d.b1 - d.b0 + 1;
+    const bool staged = bw * bh <= PROJECT_MAP_FLOATS;
+    if (staged) {
+        for (int a = threadIdx.x >> 5; a < bw; a += PROJECT_THREADS / 32)
+            for (int b = threadIdx.x & 31; b < bh; b += 32) map_s[a * bh + b] = __ldg(pm + (d.a0 + a) * P.Nvf + d.b0 + b);
+    }
+    __syncthreads();
     // quads per row of the widest slice: S_k grows with the distance from the source, and its first column may round down
     const SliceBox16 Sl = load_box(sbox, (size_t)cp * P.Nw + P.Nw - 1), Sf = load_box(sbox, (size_t)cp * P.Nw);
     const int wide = max(Sl.u0 <= Sl.u1 ? Sl.v1 - Sl.v0 + 1 : 0, Sf.u0 <= Sf.u1 ? Sf.v1 - Sf.v0 + 1 : 0);
@@ -111,9 +121,15 @@ k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restric
             }
             auto row_T = [&](int a, float (&T)[4]) {            // T[a][quad]; zero outside the support bbox
                 if (a >= d.a0 && a <= d.a1) {
-                    const float *pc = pm + a * P.Nvf;
+                    if (staged) {
+                        const float *pc = map_s + (a - d.a0) * bh - d.b0;
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) T[e] = wb0[e] * __ldg(pc + ib0[e]) + wb1[e] * __ldg(pc + ib1[e]);
+                        for (int e = 0; e < 4; ++e) T[e] = wb0[e] * pc[ib0[e]] + wb1[e] * pc[ib1[e]];
+                    } else {
+                        const float *pc = pm + a * P.Nvf;
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) T[e] = wb0[e] * __ldg(pc + ib0[e]) + wb1[e] * __ldg(pc + ib1[e]);
+                    }
                 } else {
 #pragma unroll
                     for (int e = 0; e < 4; ++e) T[e] = 0.f;
@@ -124,8 +140,9 @@ k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restric
             row_T(a_cur, T0);
             row_T(a_cur + 1, T1);
             float *op = vc + ((size_t)k * d.pu + (S.u0 - d.ri0)) * d.pv + (jb - d.rj0);
+            const float fa0 = (S.u0 - P.cu) * su + P.cuf;
             for (int i = S.u0; i <= S.u1; ++i, op += d.pv) {
-                const float fa = (i - P.cu) * su + P.cuf;
+                const float fa = fmaf((float)(i - S.u0), su, fa0);
                 const float fla = floorf(fa);
                 const int a = (int)fla;
                 const float ta = fa - fla;
@@ -154,33 +171,40 @@ struct __align__(16) RaRow {        // one beam row (k, i) of G_b: its patient-c
     int pad_[2];
 };
 
-// one quad of one beam row from NC candidates (the first NC entries of the row's list), no predicates
+// one quad of each of TWO beam rows from NC candidates each (the first NC entries of the rows' lists), no predicates: the
+// 2 NC loads are all in flight before the first use.  A row with nothing to write has nq = 0.
 template <int NC>
-__device__ __forceinline__ void ra_stream(const RaRow &R, const float *__restrict__ gT, float *__restrict__ orow, int lane16)
+__device__ __forceinline__ void ra_stream2(const RaRow &Ra, const RaRow &Rb, const float *__restrict__ gT, float *__restrict__ Gc, int lane16)
 {
-    for (int q = lane16; q < R.nq; q += 16) {
-        const int j = R.j0 + 4 * q;
-        int off[NC];
-        float w[NC];
+    const int nqa = Ra.n >= 0 ? Ra.nq : 0, nqb = Rb.n >= 0 ? Rb.nq : 0;
+    float *oa = Gc + Ra.out, *ob = Gc + Rb.out;
+    for (int q = lane16; q < max(nqa, nqb); q += 16) {
+        const int ja = Ra.j0 + 4 * min(q, max(nqa - 1, 0)), jb = Rb.j0 + 4 * min(q, max(nqb - 1, 0));
+        int offa[NC], offb[NC];
+        float wa[NC], wb[NC];
 #pragma unroll
-        for (int c4 = 0; c4 < NC; c4 += 4) {                  // 16-byte broadcast reads of the list
-            const int4 o = *reinterpret_cast<const int4 *>(&R.off[c4]);
-            const float4 f = *reinterpret_cast<const float4 *>(&R.w[c4]);
-            off[c4] = o.x; w[c4] = f.x;
-            if (c4 + 1 < NC) { off[c4 + 1] = o.y; w[c4 + 1] = f.y; }
-            if (c4 + 2 < NC) { off[c4 + 2] = o.z; w[c4 + 2] = f.z; }
-            if (c4 + 3 < NC) { off[c4 + 3] = o.w; w[c4 + 3] = f.w; }
+        for (int c4 = 0; c4 < NC; c4 += 4) {                  // 16-byte broadcast reads of the lists
+            const int4 o = *reinterpret_cast<const int4 *>(&Ra.off[c4]), p = *reinterpret_cast<const int4 *>(&Rb.off[c4]);
+            const float4 f = *reinterpret_cast<const float4 *>(&Ra.w[c4]), g = *reinterpret_cast<const float4 *>(&Rb.w[c4]);
+            offa[c4] = o.x; wa[c4] = f.x; offb[c4] = p.x; wb[c4] = g.x;
+            if (c4 + 1 < NC) { offa[c4 + 1] = o.y; wa[c4 + 1] = f.y; offb[c4 + 1] = p.y; wb[c4 + 1] = g.y; }
+            if (c4 + 2 < NC) { offa[c4 + 2] = o.z; wa[c4 + 2] = f.z; offb[c4 + 2] = p.z; wb[c4 + 2] = g.z; }
+            if (c4 + 3 < NC) { offa[c4 + 3] = o.w; wa[c4 + 3] = f.w; offb[c4 + 3] = p.w; wb[c4 + 3] = g.w; }
         }
-        float4 v[NC];
-#pragma unroll
-        for (int c = 0; c < NC; ++c) v[c] = __ldg(reinterpret_cast<const float4 *>(gT + (off[c] + j)));     // all loads first
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 va[NC], vb[NC];
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
-            acc.x = fmaf(w[c], v[c].x, acc.x); acc.y = fmaf(w[c], v[c].y, acc.y);
-            acc.z = fmaf(w[c], v[c].z, acc.z); acc.w = fmaf(w[c], v[c].w, acc.w);
+            va[c] = __ldg(reinterpret_cast<const float4 *>(gT + (offa[c] + ja)));
+            vb[c] = __ldg(reinterpret_cast<const float4 *>(gT + (offb[c] + jb)));
         }
-        *reinterpret_cast<float4 *>(orow + j) = acc;
+        float4 sa = make_float4(0.f, 0.f, 0.f, 0.f), sb = sa;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            sa.x = fmaf(wa[c], va[c].x, sa.x); sa.y = fmaf(wa[c], va[c].y, sa.y); sa.z = fmaf(wa[c], va[c].z, sa.z); sa.w = fmaf(wa[c], va[c].w, sa.w);
+            sb.x = fmaf(wb[c], vb[c].x, sb.x); sb.y = fmaf(wb[c], vb[c].y, sb.y); sb.z = fmaf(wb[c], vb[c].z, sb.z); sb.w = fmaf(wb[c], vb[c].w, sb.w);
+        }
+        if (q < nqa) *reinterpret_cast<float4 *>(oa + ja) = sa;
+        if (q < nqb) *reinterpret_cast<float4 *>(ob + jb) = sb;
     }
 }
 
@@ -221,6 +245,7 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *
             RaRow &R = rows[tid];
             const int r = r0 + tid;
             int n = -1;
+            R.out = 0; R.j0 = 0; R.nq = 0;
             if (r < n_rows) {
                 const int k = r / d.pu, i = d.ri0 + (r - k * d.pu);
                 const SliceBox16 S = load_box(sbox, (size_t)cp * P.Nw + k);
@@ -241,28 +266,36 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *
                                 const float wu = 1.f - fabsf(eu0 + cy * fu_y + cx * fu_x), ww = 1.f - fabsf(ew0 + cy * fw_y + cx * fw_x);
                                 if (wu > 0.f && ww > 0.f) { R.off[n] = ((ya + cy) * P.nx + xa + cx) * nzp; R.w[n] = wu * ww; ++n; }
                             }
-                        const int o0 = n > 0 ? R.off[0] : 0;
-                        for (int c = n; c < RA_PADC; ++c) { R.off[c] = o0; R.w[c] = 0.f; }
                     } else {
                         n = -2;
                         R.xa = xa; R.xb = xb; R.ya = ya; R.yb = yb; R.eu0 = eu0; R.ew0 = ew0;
                     }
                 }
             }
+            {   // entries past n repeat entry 0 with weight 0 (every address readable, no predicates in the stream loop)
+                const int o0 = n > 0 ? R.off[0] : 0;
+                for (int c = max(n, 0); c < RA_PADC; ++c) { R.off[c] = o0; R.w[c] = 0.f; }
+            }
             R.n = n;
         }
         __syncthreads();
-        // phase B: half-warp `half` streams rows half, half + 16, ...
-        for (int rr = half; rr < RA_THREADS; rr += RA_THREADS / 16) {
-            const RaRow &R = rows[rr];
-            const int n = R.n;
-            if (n == -1) continue;
-            float *orow = Gc + R.out;
-            if (n >= 0) {
-                if (n <= 4) ra_stream<4>(R, gT, orow, lane16);
-                else if (n <= 6) ra_stream<6>(R, gT, orow, lane16);
-                else ra_stream<RA_MAXC>(R, gT, orow, lane16);
-            } else {
+        // phase B: half-warp `half` streams the row pairs (half, half + 16), (half + 32, half + 48), ...
+        for (int rr = half; rr < RA_THREADS; rr += RA_THREADS / 8) {
+            const RaRow &Ra = rows[rr], &Rb = rows[rr + RA_THREADS / 16];
+            const int na = Ra.n, nb = Rb.n;
+            if (na == -1 && nb == -1) continue;
+            if (na != -2 && nb != -2) {
+                const int n = max(na, nb);
+                if (n <= 4) ra_stream2<4>(Ra, Rb, gT, Gc, lane16);
+                else if (n <= 6) ra_stream2<6>(Ra, Rb, gT, Gc, lane16);
+                else ra_stream2<RA_MAXC>(Ra, Rb, gT, Gc, lane16);
+                continue;
+            }
+            for (int side = 0; side < 2; ++side) {
+                const RaRow &R = side ? Rb : Ra;
+                if (R.n == -1) continue;
+                float *orow = Gc + R.out;
+                if (R.n >= 0) { ra_stream2<RA_MAXC>(R, R, gT, Gc, lane16); continue; }
                 // stencil wider than 3 x 3 (beam voxels much coarser than patient voxels): plain loop over the candidate box
                 for (int jj = lane16; jj < 4 * R.nq; jj += 16) {
                     const int j = R.j0 + jj;

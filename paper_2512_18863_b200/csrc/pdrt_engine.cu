@@ -16,6 +16,7 @@
 #include "pdrt_depth.cuh"
 #include "pdrt_dev.cuh"
 #include "pdrt_fluence.cuh"
+#include "pdrt_plan.cuh"
 #include "pdrt_resample.cuh"
 
 using namespace pdrt;
@@ -43,7 +44,7 @@ int tile_floats_for(int kt)
     return best;
 }
 // blocks per control point of k_project (a block takes every X-th slice) and of k_resample_adjoint (256 beam rows per chunk)
-int project_blocks(const Params &P) { return std::max(1, std::min(P.Nw, 24)); }
+int project_blocks(const Params &P) { return std::max(1, std::min(P.Nw, 8)); }
 int resample_adj_blocks(const Params &P) { return std::max(1, std::min(48, (P.Nw * (P.Nu + RS) + RA_THREADS - 1) / RA_THREADS)); }
 size_t conv_smem_bytes(int kt) { return sizeof(float) * (2 * (size_t)(kt + 1) * ((kt + 3) & ~3) + tile_floats_for(kt)); }   // row-pair kernel + ring
 
@@ -84,6 +85,7 @@ struct pdrt_engine {
     DevBuf<float> bufA, bufB;         // compact beam-frame blocks: conv output (D_b / H_b) and conv input (Phivol / G_b)
     // staging for the *_host entry points
     DevBuf<float> s_leaves, s_jaws, s_gantry, s_mu, s_vol, s_dleaves, s_djaws, s_dmu;
+    DevBuf<double> obj_partial;       // block partials of the objective
     size_t scratch_cap_bytes = (size_t)48 << 30;
     int last_n_cp = 0;
     bool last_backward = false;
@@ -263,14 +265,14 @@ int batch_size(const pdrt_engine *e, int n_cp, int nbuf)
     return (int)(b < (size_t)n_cp ? b : (size_t)n_cp);
 }
 
-int check_call(pdrt_engine *e, int n_cp, std::initializer_list<const void *> ptrs)
+int check_call(pdrt_engine *e, int n_cp, std::initializer_list<const void *> ptrs, bool dose_call = true)
 {
     if (!e) return fail(nullptr, PDRT_EINVAL, "null engine");
     if (n_cp < 1) return fail(e, PDRT_EINVAL, "n_cp must be >= 1");
     for (const void *p : ptrs)
         if (!p) return fail(e, PDRT_EINVAL, "null pointer argument");
     CU(e, cudaSetDevice(e->device));
-    reset_stage_records(e);
+    if (dose_call) reset_stage_records(e);          // the planning-loop calls keep the stage records of the last dose call
     return PDRT_OK;
 }
 
@@ -529,7 +531,7 @@ void pdrt_destroy(pdrt_engine *e)
     e->Abuf.release(); e->gphimap.release(); e->zrad.release(); e->rho_s.release(); e->Z_s.release();
     e->bufA.release(); e->bufB.release(); e->phimapT.release(); e->gT.release();
     e->s_leaves.release(); e->s_jaws.release(); e->s_gantry.release(); e->s_mu.release(); e->s_vol.release();
-    e->s_dleaves.release(); e->s_djaws.release(); e->s_dmu.release();
+    e->s_dleaves.release(); e->s_djaws.release(); e->s_dmu.release(); e->obj_partial.release();
     for (cudaEvent_t ev : e->ev_pool) cudaEventDestroy(ev);
     delete e;
 }
@@ -710,6 +712,74 @@ int pdrt_stage_grad_fluence(pdrt_engine *e, int32_t n_cp, const float *leaves, c
     CU(e, cudaMemsetAsync(e->gphimap.p, 0, nmap * sizeof(float), st));
     if ((rc = backward_to_fluence(e, n_cp, leaves, jaws, gantry, nullptr, gdose, st))) return rc;
     CU(e, cudaMemcpyAsync(gphimap, e->gphimap.p, nmap * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    return PDRT_OK;
+}
+
+// ---- planning loop (pdrt_plan.cuh)
+float pdrt_mu_epsilon(float dose_rate_min, float delta_phi_deg, float gantry_speed_max) { return dose_rate_min * delta_phi_deg / gantry_speed_max; }
+
+static PlanLimits plan_limits(const pdrt_limits *l) { return PlanLimits{ l->leaf_w_min, l->leaf_F, l->jaw_w_min, l->jaw_Fx, l->jaw_Fy, l->mu_eps }; }
+
+int pdrt_validate(pdrt_engine *e, int32_t n_cp, const pdrt_limits *lim, const float *leaves, const float *jaws, const float *mu,
+                  float *leaves_out, float *jaws_out, float *mu_out, void *stream)
+{
+    int rc = check_call(e, n_cp, { lim, leaves, jaws, mu, leaves_out, jaws_out, mu_out }, false);
+    if (rc) return rc;
+    const long long n = (long long)n_cp * (e->P.Np + 3);
+    k_validate<false><<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(n_cp, e->P.Np, plan_limits(lim), leaves, jaws, mu, nullptr, nullptr,
+                                                                                     nullptr, leaves_out, jaws_out, mu_out);
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+
+int pdrt_validate_backward(pdrt_engine *e, int32_t n_cp, const pdrt_limits *lim, const float *leaves, const float *jaws, const float *mu,
+                           const float *gl_hat, const float *gj_hat, const float *gm_hat, float *gl, float *gj, float *gm, void *stream)
+{
+    int rc = check_call(e, n_cp, { lim, leaves, jaws, mu, gl_hat, gj_hat, gm_hat, gl, gj, gm }, false);
+    if (rc) return rc;
+    const long long n = (long long)n_cp * (e->P.Np + 3);
+    k_validate<true><<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(n_cp, e->P.Np, plan_limits(lim), leaves, jaws, mu, gl_hat, gj_hat,
+                                                                                    gm_hat, gl, gj, gm);
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+
+int pdrt_objective(pdrt_engine *e, const float *dose, const uint32_t *bits, int32_t n_struct, const float *lambda, const float *presc,
+                   int32_t power, float *g, double *loss, void *stream)
+{
+    int rc = check_call(e, 1, { dose, bits, lambda, presc, g, loss }, false);
+    if (rc) return rc;
+    if (n_struct < 1 || n_struct > OBJ_MAX_STRUCT) return fail(e, PDRT_EINVAL, "n_struct must lie in 1..32");
+    if (power != 1 && power != 2) return fail(e, PDRT_EINVAL, "power must be 1 (Eq. 10) or 2 (quadratic)");
+    ObjectiveTerms T{};
+    T.n = n_struct; T.power = power;
+    for (int s = 0; s < n_struct; ++s) { T.lambda[s] = lambda[s]; T.presc[s] = presc[s]; }
+    const int nb = e->sm_count * 8;
+    CU(e, e->obj_partial.ensure(nb));
+    const size_t n_vox = (size_t)e->P.nx * e->P.ny * e->P.nz;
+    k_objective<<<nb, OBJ_THREADS, 0, (cudaStream_t)stream>>>(n_vox, dose, bits, T, g, e->obj_partial.p);
+    CU(e, cudaGetLastError());
+    k_objective_finish<<<1, 32, 0, (cudaStream_t)stream>>>(nb, e->obj_partial.p, loss);
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+
+int pdrt_track_jaws(pdrt_engine *e, int32_t n_cp, const float *leaves, float margin, float open_gap, float *jaws, void *stream)
+{
+    int rc = check_call(e, n_cp, { leaves, jaws }, false);
+    if (rc) return rc;
+    k_track_jaws<<<(n_cp * 32 + 255) / 256, 256, 0, (cudaStream_t)stream>>>(n_cp, e->P.Np, e->T.leaf_bounds, leaves, margin, open_gap, jaws);
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+
+int pdrt_plan_step(pdrt_engine *e, int32_t n_cp, float step_leaf, float step_mu, const float *g_leaves, const float *g_mu, float *leaves,
+                   float *mu, void *stream)
+{
+    int rc = check_call(e, n_cp, { g_leaves, g_mu, leaves, mu }, false);
+    if (rc) return rc;
+    k_plan_step<<<1, STEP_THREADS, 0, (cudaStream_t)stream>>>(n_cp * 2 * e->P.Np, n_cp, step_leaf, step_mu, g_leaves, g_mu, leaves, mu);
+    CU(e, cudaGetLastError());
     return PDRT_OK;
 }
 

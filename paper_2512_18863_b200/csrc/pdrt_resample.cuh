@@ -18,42 +18,58 @@ constexpr int GD_CPB = 16;                       // control points set up per ro
 constexpr int GD_THREADS = GD_COLS * GD_CPB;
 constexpr int GD_ZSPAN = 64;                     // z covered by one pass of a half-warp (16 lanes x float4)
 constexpr int GD_MAXPASS = 4;                    // passes held in registers at once (256 z)
-constexpr int GD_LIST = 512;                     // control points listed per outer chunk
+constexpr int GD_LIST = 256;                     // control points listed per outer chunk
 
+struct __align__(16) GatherCp {                  // what the stencil set-up needs of a listed control point (32 bytes, shared memory)
+    float cg, sg, scale;
+    int ri0, pu, pv, rj0, slot;
+};
 struct __align__(16) GatherRec {                 // bilinear stencil of one (patient column, control point): 64 bytes
     const float *row[4];                         // beam rows (i0,k0), (i0+1,k0), (i0,k0+1), (i0+1,k0+1), shifted so that row[q][z] is voxel
                                                  // v = z; invalid neighbours are folded onto a valid row
     float w[4];                                  // cal * MU * bilinear weight; 0 for invalid neighbours
-    short zlo0, zhi0, zlo1, zhi1;                // written v-range [zlo, zhi) of slice k0 and of slice k0+1 (multiples of 8)
-    int n_valid;                                 // 0: nothing to add
-    int pad_;
+    short zlo0, zhi0, zlo1, zhi1;                // written v-range [zlo, zhi) of slice k0 and of slice k0+1 (multiples of 8); empty: no reads
+    int pad_[2];
 };
 
-// phase B of k_gather_dose for one round of control points, NP z-passes of 64 held in registers
-template <int NP>
+// phase B of k_gather_dose for one round of control points: NP z-passes of 64 held in registers, NB control points per
+// batch.  Straight-line code: the 4 NB NP loads of a batch are all issued before the first use.  Records of control points that
+// do not reach the column carry empty z-ranges (no reads) and zero weights.
+template <int NP, int NB>
 __device__ __forceinline__ void gather_round(const GatherRec (*rec)[GD_COLS], int col, int nround, int zq, float2 (&acc)[GD_MAXPASS][2])
 {
-#pragma unroll 2
-    for (int e = 0; e < nround; ++e) {
-        const GatherRec &R = rec[e][col];
-        const int4 meta = *reinterpret_cast<const int4 *>(&R.zlo0);         // z-ranges (4 shorts), n_valid
-        if (meta.z == 0) continue;
-        const float4 w = *reinterpret_cast<const float4 *>(R.w);
-        const float2 w0 = make_float2(w.x, w.x), w1 = make_float2(w.y, w.y), w2 = make_float2(w.z, w.z), w3 = make_float2(w.w, w.w);
-        const int zlo0 = (short)(meta.x & 0xffff), zhi0 = meta.x >> 16, zlo1 = (short)(meta.y & 0xffff), zhi1 = meta.y >> 16;
-        const float *r0 = R.row[0], *r1 = R.row[1], *r2 = R.row[2], *r3 = R.row[3];
+    for (int e0 = 0; e0 < nround; e0 += NB) {
+        float4 v[NB][NP][4];
+        float4 w[NB];
 #pragma unroll
-        for (int ps = 0; ps < NP; ++ps) {
-            const int z = zq + ps * GD_ZSPAN;
-            const bool in0 = z >= zlo0 && z < zhi0, in1 = z >= zlo1 && z < zhi1;
-            float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, f = a;
-            if (in0) { a = __ldg(reinterpret_cast<const float4 *>(r0 + z)); b = __ldg(reinterpret_cast<const float4 *>(r1 + z)); }
-            if (in1) { c = __ldg(reinterpret_cast<const float4 *>(r2 + z)); f = __ldg(reinterpret_cast<const float4 *>(r3 + z)); }
-            // packed FFMA2: two z per instruction
-            acc[ps][0] = __ffma2_rn(w0, make_float2(a.x, a.y), acc[ps][0]); acc[ps][1] = __ffma2_rn(w0, make_float2(a.z, a.w), acc[ps][1]);
-            acc[ps][0] = __ffma2_rn(w1, make_float2(b.x, b.y), acc[ps][0]); acc[ps][1] = __ffma2_rn(w1, make_float2(b.z, b.w), acc[ps][1]);
-            acc[ps][0] = __ffma2_rn(w2, make_float2(c.x, c.y), acc[ps][0]); acc[ps][1] = __ffma2_rn(w2, make_float2(c.z, c.w), acc[ps][1]);
-            acc[ps][0] = __ffma2_rn(w3, make_float2(f.x, f.y), acc[ps][0]); acc[ps][1] = __ffma2_rn(w3, make_float2(f.z, f.w), acc[ps][1]);
+        for (int q = 0; q < NB; ++q) {
+            const GatherRec &R = rec[e0 + q][col];
+            const int2 zr = *reinterpret_cast<const int2 *>(&R.zlo0);
+            w[q] = *reinterpret_cast<const float4 *>(R.w);
+            const int zlo0 = (short)(zr.x & 0xffff), zhi0 = zr.x >> 16, zlo1 = (short)(zr.y & 0xffff), zhi1 = zr.y >> 16;
+            const float *r0 = R.row[0], *r1 = R.row[1], *r2 = R.row[2], *r3 = R.row[3];
+#pragma unroll
+            for (int ps = 0; ps < NP; ++ps) {
+                const int z = zq + ps * GD_ZSPAN;
+                const bool in0 = z >= zlo0 && z < zhi0, in1 = z >= zlo1 && z < zhi1;
+                const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+                v[q][ps][0] = in0 ? __ldg(reinterpret_cast<const float4 *>(r0 + z)) : zero;
+                v[q][ps][1] = in0 ? __ldg(reinterpret_cast<const float4 *>(r1 + z)) : zero;
+                v[q][ps][2] = in1 ? __ldg(reinterpret_cast<const float4 *>(r2 + z)) : zero;
+                v[q][ps][3] = in1 ? __ldg(reinterpret_cast<const float4 *>(r3 + z)) : zero;
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {                       // control-point order (deterministic); packed FFMA2: two z per instruction
+            const float wq[4] = { w[q].x, w[q].y, w[q].z, w[q].w };
+#pragma unroll
+            for (int ps = 0; ps < NP; ++ps)
+#pragma unroll
+                for (int n = 0; n < 4; ++n) {
+                    const float2 w2 = make_float2(wq[n], wq[n]);
+                    acc[ps][0] = __ffma2_rn(w2, make_float2(v[q][ps][n].x, v[q][ps][n].y), acc[ps][0]);
+                    acc[ps][1] = __ffma2_rn(w2, make_float2(v[q][ps][n].z, v[q][ps][n].w), acc[ps][1]);
+                }
         }
     }
 }
@@ -62,20 +78,22 @@ __device__ __forceinline__ void gather_round(const GatherRec (*rec)[GD_COLS], in
 //   dose[p] (+)= sum_b scale_b * bilinear_0(D_b[.][z][.]; fu, fw)
 // The gantry rotates about z (G1), so for one control point the beam-frame position (fu, fw) and the four
 // bilinear weights of a column are the same for all its voxels.  Warp 0 first lists the control points whose compact
-// region can reach the block's columns (and the z-range they cover).  Then, 16 control points at a time: phase A, one
-// THREAD per (column, control point) builds the stencil record (offsets of the four beam rows, weights, and the v-range
-// that the forward conv wrote in the two slices — outside it D_b is zero and the block holds stale data); phase B, one
-// HALF-WARP per column streams 16-byte vectors along v for the listed control points, four loads in flight per control
-// point and several control points unrolled, accumulating in registers in control-point order (deterministic).  Every
-// patient voxel of the z-range is written exactly once; the rest of the dose grid is zeroed by the caller (memset).
-__global__ void __launch_bounds__(GD_THREADS)
+// region can reach the block's columns (with the constants the set-up needs, and the z-range they cover).  Then, 16
+// control points at a time: phase A, one THREAD per (column, control point) builds the stencil record (pointers to the four
+// beam rows, weights, and the v-range that the forward conv wrote in the two slices — outside it D_b is zero and the block
+// holds stale data); phase B, one HALF-WARP per column streams 16-byte vectors along v, several control points per batch
+// with all their loads in flight at once, accumulating in registers in control-point order (deterministic).  The records
+// are double-buffered and the global reads of phase A for round r+1 are issued before phase B of round r, so that their
+// latency is covered.  Every patient voxel of the z-range is written exactly once; the rest of the dose grid is zeroed by
+// the caller (memset).
+__global__ void __launch_bounds__(GD_THREADS, 2)
 k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ wbox, int cp0, int n_cp,
               const float *__restrict__ D, float *__restrict__ dose, int accumulate)
 {
-    __shared__ GatherRec rec[GD_CPB][GD_COLS];
-    __shared__ short list[GD_LIST];
+    __shared__ GatherRec rec[2][GD_CPB][GD_COLS];
+    __shared__ GatherCp list[GD_LIST];
     __shared__ int n_list_s, zmin_s, zmax_s;
-    const int tid = threadIdx.x, lane = tid & 31, lane16 = tid & 15;
+    const int tid = threadIdx.x, lane16 = tid & 15;
     const int col = tid >> 4;                                    // phase B: column of this half-warp
     const int a_col = tid & 15, a_cp = tid >> 4;                 // phase A: (column, control point of the round)
     const int px0 = blockIdx.x * GD_PX, py0 = blockIdx.y * GD_PY;
@@ -90,6 +108,54 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
     const int bx = px0 + (col & (GD_PX - 1)), by = py0 + col / GD_PX;
     const bool b_inside = bx < P.nx && by < P.ny;
 
+    // phase A, first half: position of the column in the beam frame of control point list[q]; issues the reads of the two slice boxes
+    struct Setup { int i0, k0; float tu, tw; SliceBox16 w0, w1; bool on; };
+    auto setup_load = [&](int q, int n_list) {
+        Setup s;
+        s.on = q < n_list && a_inside;
+        s.w0 = SliceBox16{ 1, 0, 1, 0 }; s.w1 = s.w0;
+        s.i0 = s.k0 = 0; s.tu = s.tw = 0.f;
+        if (s.on) {
+            const GatherCp g = list[q];
+            const float fu = (g.cg * adx + g.sg * ady) / P.du + P.cu;
+            const float fw = (-g.sg * adx + g.cg * ady - P.wmin) / P.dw;
+            const float flu = floorf(fu), flw = floorf(fw);
+            s.i0 = (int)flu; s.k0 = (int)flw;
+            s.tu = fu - flu; s.tw = fw - flw;
+            // bilinear_0: neighbours outside the beam grid contribute 0; outside the written box of its slice D_b is 0
+            const size_t base = (size_t)(cp0 + g.slot) * P.Nw;
+            if (s.k0 >= 0 && s.k0 < P.Nw) s.w0 = load_box(wbox, base + s.k0);
+            if (s.k0 + 1 >= 0 && s.k0 + 1 < P.Nw) s.w1 = load_box(wbox, base + s.k0 + 1);
+        }
+        return s;
+    };
+    // phase A, second half: the record
+    auto setup_store = [&](const Setup &s, int q, GatherRec &R) {
+        bool v00 = false, v10 = false, v01 = false, v11 = false;
+        if (s.on) {
+            v00 = s.i0 >= s.w0.u0 && s.i0 <= s.w0.u1; v10 = s.i0 + 1 >= s.w0.u0 && s.i0 + 1 <= s.w0.u1;
+            v01 = s.i0 >= s.w1.u0 && s.i0 <= s.w1.u1; v11 = s.i0 + 1 >= s.w1.u0 && s.i0 + 1 <= s.w1.u1;
+        }
+        if (v00 || v10 || v01 || v11) {
+            const GatherCp g = list[q];
+            const int rs = g.pv, ks = g.pu * g.pv;
+            const int o00 = (s.k0 * g.pu + (s.i0 - g.ri0)) * rs;
+            const int any_off = v00 ? o00 : (v10 ? o00 + rs : (v01 ? o00 + ks : o00 + ks + rs));
+            const float *base = D + (size_t)g.slot * (size_t)P.stride_cp - g.rj0;
+            R.row[0] = base + (v00 ? o00 : any_off); R.row[1] = base + (v10 ? o00 + rs : any_off);
+            R.row[2] = base + (v01 ? o00 + ks : any_off); R.row[3] = base + (v11 ? o00 + ks + rs : any_off);
+            R.w[0] = v00 ? g.scale * ((1.f - s.tu) * (1.f - s.tw)) : 0.f; R.w[1] = v10 ? g.scale * (s.tu * (1.f - s.tw)) : 0.f;
+            R.w[2] = v01 ? g.scale * ((1.f - s.tu) * s.tw) : 0.f; R.w[3] = v11 ? g.scale * (s.tu * s.tw) : 0.f;
+            // a slice none of whose rows is valid gets an empty z-range: its (folded) rows are not read at all
+            R.zlo0 = (v00 || v10) ? s.w0.v0 : (short)0; R.zhi0 = (v00 || v10) ? (short)(s.w0.v1 + 1) : (short)0;
+            R.zlo1 = (v01 || v11) ? s.w1.v0 : (short)0; R.zhi1 = (v01 || v11) ? (short)(s.w1.v1 + 1) : (short)0;
+        } else {
+            R.row[0] = R.row[1] = R.row[2] = R.row[3] = D;
+            R.w[0] = R.w[1] = R.w[2] = R.w[3] = 0.f;
+            R.zlo0 = R.zhi0 = R.zlo1 = R.zhi1 = 0;
+        }
+    };
+
     for (int c0 = 0; c0 < n_cp; c0 += GD_LIST) {
         __syncthreads();
         if (tid < 32) {                 // warp 0 builds the ordered list of candidate control points and their z-range
@@ -98,20 +164,22 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
             for (int cb = c0; cb < cend; cb += 32) {
                 const int c = cb + tid;
                 bool keep = false;
+                GatherCp g;
                 if (c < cend) {
                     const CpDesc &d = desc[cp0 + c];
                     if (d.a0 <= d.a1) {
+                        g.cg = d.cg; g.sg = d.sg; g.scale = d.scale; g.ri0 = d.ri0; g.pu = d.pu; g.pv = d.pv; g.rj0 = d.rj0; g.slot = c;
                         // u-extent of the tile: extremes are at its corners
-                        const float u00 = d.cg * cx0 + d.sg * cy0, u10 = d.cg * cx1 + d.sg * cy0;
-                        const float u01 = d.cg * cx0 + d.sg * cy1, u11 = d.cg * cx1 + d.sg * cy1;
+                        const float u00 = g.cg * cx0 + g.sg * cy0, u10 = g.cg * cx1 + g.sg * cy0;
+                        const float u01 = g.cg * cx0 + g.sg * cy1, u11 = g.cg * cx1 + g.sg * cy1;
                         const float umin = fminf(fminf(u00, u10), fminf(u01, u11)) / P.du + P.cu;
                         const float umax = fmaxf(fmaxf(u00, u10), fmaxf(u01, u11)) / P.du + P.cu;
-                        keep = umax >= (float)(d.ri0 - 1) && umin <= (float)(d.ri0 + d.pu);
-                        if (keep) { zmin = min(zmin, d.rj0); zmax = max(zmax, min(P.nz, d.rj0 + d.pv)); }
+                        keep = umax >= (float)(g.ri0 - 1) && umin <= (float)(g.ri0 + g.pu);
+                        if (keep) { zmin = min(zmin, g.rj0); zmax = max(zmax, min(P.nz, g.rj0 + g.pv)); }
                     }
                 }
                 const unsigned m = __ballot_sync(0xffffffffu, keep);
-                if (keep) list[count + __popc(m & ((1u << tid) - 1u))] = (short)(c - c0);
+                if (keep) list[count + __popc(m & ((1u << tid) - 1u))] = g;
                 count += __popc(m);
             }
 #pragma unroll
@@ -129,51 +197,23 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
 #pragma unroll
             for (int p = 0; p < GD_MAXPASS; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
             const int npass = min(GD_MAXPASS, (zmax - zb + GD_ZSPAN - 1) / GD_ZSPAN);
-            for (int q0 = 0; q0 < n_list; q0 += GD_CPB) {
-                __syncthreads();                                                 // the records of the previous round are consumed
-                {   // phase A: record of (column a_col, control point list[q0 + a_cp])
-                    GatherRec &R = rec[a_cp][a_col];
-                    int n_valid = 0;
-                    if (q0 + a_cp < n_list && a_inside) {
-                        const int c = c0 + list[q0 + a_cp];
-                        const CpDesc &d = desc[cp0 + c];
-                        const float fu = (d.cg * adx + d.sg * ady) / P.du + P.cu;
-                        const float fw = (-d.sg * adx + d.cg * ady - P.wmin) / P.dw;
-                        const float flu = floorf(fu), flw = floorf(fw);
-                        const int i0 = (int)flu, k0 = (int)flw;
-                        const float tu = fu - flu, tw = fw - flw;
-                        // bilinear_0: neighbours outside the beam grid contribute 0; outside the written box of its slice D_b is 0
-                        SliceBox16 w0 = { 1, 0, 1, 0 }, w1 = { 1, 0, 1, 0 };
-                        if (k0 >= 0 && k0 < P.Nw) w0 = load_box(wbox, (size_t)(cp0 + c) * P.Nw + k0);
-                        if (k0 + 1 >= 0 && k0 + 1 < P.Nw) w1 = load_box(wbox, (size_t)(cp0 + c) * P.Nw + k0 + 1);
-                        const bool v00 = i0 >= w0.u0 && i0 <= w0.u1, v10 = i0 + 1 >= w0.u0 && i0 + 1 <= w0.u1;
-                        const bool v01 = i0 >= w1.u0 && i0 <= w1.u1, v11 = i0 + 1 >= w1.u0 && i0 + 1 <= w1.u1;
-                        n_valid = (int)v00 + (int)v10 + (int)v01 + (int)v11;
-                        if (n_valid) {
-                            const int rs = d.pv, ks = d.pu * d.pv;
-                            const int o00 = (k0 * d.pu + (i0 - d.ri0)) * rs;
-                            const int any_off = v00 ? o00 : (v10 ? o00 + rs : (v01 ? o00 + ks : o00 + ks + rs));
-                            const float *base = D + (size_t)c * (size_t)P.stride_cp - d.rj0;
-                            R.row[0] = base + (v00 ? o00 : any_off); R.row[1] = base + (v10 ? o00 + rs : any_off);
-                            R.row[2] = base + (v01 ? o00 + ks : any_off); R.row[3] = base + (v11 ? o00 + ks + rs : any_off);
-                            R.w[0] = v00 ? d.scale * ((1.f - tu) * (1.f - tw)) : 0.f; R.w[1] = v10 ? d.scale * (tu * (1.f - tw)) : 0.f;
-                            R.w[2] = v01 ? d.scale * ((1.f - tu) * tw) : 0.f; R.w[3] = v11 ? d.scale * (tu * tw) : 0.f;
-                            // a slice none of whose rows is valid gets an empty z-range: its (folded) rows are not read at all
-                            R.zlo0 = (v00 || v10) ? w0.v0 : (short)0; R.zhi0 = (v00 || v10) ? (short)(w0.v1 + 1) : (short)0;
-                            R.zlo1 = (v01 || v11) ? w1.v0 : (short)0; R.zhi1 = (v01 || v11) ? (short)(w1.v1 + 1) : (short)0;
-                        }
-                    }
-                    R.n_valid = n_valid;
-                }
-                __syncthreads();
-                // phase B: half-warp `col` adds the round's control points, in list order
+            const int zq = zb + 4 * lane16;
+            {   // records of round 0
+                const Setup s = setup_load(a_cp, n_list);
+                setup_store(s, a_cp, rec[0][a_cp][a_col]);
+            }
+            __syncthreads();
+            int buf = 0;
+            for (int q0 = 0; q0 < n_list; q0 += GD_CPB, buf ^= 1) {
+                const Setup s = setup_load(q0 + GD_CPB + a_cp, n_list);          // reads for the next round are in flight during phase B
                 const int nround = min(GD_CPB, n_list - q0);
                 if (b_inside) {
-                    const int zq = zb + 4 * lane16;
-                    if (npass == 1) gather_round<1>(rec, col, nround, zq, acc);
-                    else if (npass == 2) gather_round<2>(rec, col, nround, zq, acc);
-                    else gather_round<GD_MAXPASS>(rec, col, nround, zq, acc);
+                    if (npass == 1) gather_round<1, 4>(rec[buf], col, nround, zq, acc);
+                    else if (npass == 2) gather_round<2, 2>(rec[buf], col, nround, zq, acc);
+                    else gather_round<GD_MAXPASS, 1>(rec[buf], col, nround, zq, acc);
                 }
+                setup_store(s, q0 + GD_CPB + a_cp, rec[buf ^ 1][a_cp][a_col]);
+                __syncthreads();
             }
             if (b_inside) {
 #pragma unroll
@@ -192,7 +232,6 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
             }
         }
     }
-    (void)lane;
 }
 
 // S9.  gPhimap_b[pix] = sum_k mag_k^2 sum_{voxels} weight(voxel -> pix) * H_b[voxel]  in gather form.  The bilinear weight
@@ -204,7 +243,7 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
 // the 32 warps of a CLUSTER of four blocks; the planes are reduced in a fixed order, first inside each block, then across
 // the cluster through distributed shared memory (deterministic, no atomics).
 // Grid: (4 * ceil(Nvf/32), n_cp), cluster (4,1,1); dynamic shared memory n_act * Nuf * 32 floats.
-constexpr int PA_THREADS = 256, PA_WARPS = PA_THREADS / 32, PA_CLUSTER = 4, PA_TAPS = 4, PA_ROWS = 4;
+constexpr int PA_THREADS = 256, PA_WARPS = PA_THREADS / 32, PA_CLUSTER = 4, PA_TAPS = 4, PA_ROWS = 8;
 
 __global__ void __cluster_dims__(PA_CLUSTER, 1, 1) __launch_bounds__(PA_THREADS)
 k_project_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp, int n_act,
@@ -247,23 +286,35 @@ k_project_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *_
             const float wb = 1.f - fabsf((vb + jlo + e) * sv + P.cvf - (float)b);
             wbq[e] = (jlo + e <= jhi && wb > 0.f) ? m2 * wb : 0.f;
         }
-        const float *hrow = Hc + ((size_t)k * d.pu + (S.u0 - d.ri0)) * d.pv - d.rj0;      // row S.u0; rows are d.pv apart
-        int a_cur = (int)floorf((S.u0 - P.cu) * su + P.cuf);                              // warp-uniform
+        // per-lane row pointer at its first tap (a lane without taps reads column S.v0 with weight 0: every address is readable)
+        const int jfirst = jlo <= jhi ? jlo : (int)S.v0;
+        const float *hrow = Hc + ((size_t)k * d.pu + (S.u0 - d.ri0)) * d.pv - d.rj0 + jfirst;      // row S.u0; rows are d.pv apart
+        const int ntap = few ? min(PA_TAPS, (int)S.v1 - jfirst + 1) : 0;                           // taps that stay inside the row
+        int a_cur = (int)floorf((S.u0 - P.cu) * su + P.cuf);                                       // warp-uniform
         float acc_lo = 0.f, acc_hi = 0.f;
         for (int i = S.u0; i <= S.u1; i += PA_ROWS) {
             float t[PA_ROWS];
+            if (few) {
+                // straight-line: the PA_ROWS x PA_TAPS loads are all issued before the first use (rows past S.u1 re-read row S.u1)
+                float hv[PA_ROWS][PA_TAPS];
 #pragma unroll
-            for (int r = 0; r < PA_ROWS; ++r) {           // the loads of PA_ROWS rows are issued before any of them is used
-                t[r] = 0.f;
-                if (i + r <= S.u1) {
-                    const float *h = hrow + (size_t)r * d.pv;
-                    if (few) {
-                        float hv[PA_TAPS];
+                for (int r = 0; r < PA_ROWS; ++r) {
+                    const float *h = hrow + (size_t)min(r, (int)S.u1 - i) * d.pv;
 #pragma unroll
-                        for (int e = 0; e < PA_TAPS; ++e) hv[e] = wbq[e] != 0.f ? __ldg(h + jlo + e) : 0.f;
+                    for (int e = 0; e < PA_TAPS; ++e) hv[r][e] = __ldg(h + (e < ntap ? e : 0));
+                }
 #pragma unroll
-                        for (int e = 0; e < PA_TAPS; ++e) t[r] = fmaf(wbq[e], hv[e], t[r]);
-                    } else {
+                for (int r = 0; r < PA_ROWS; ++r) {
+                    t[r] = 0.f;
+#pragma unroll
+                    for (int e = 0; e < PA_TAPS; ++e) t[r] = fmaf(wbq[e], hv[r][e], t[r]);
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < PA_ROWS; ++r) {
+                    t[r] = 0.f;
+                    if (i + r <= S.u1) {
+                        const float *h = hrow + (size_t)r * d.pv - jfirst;
                         for (int j = jlo; j <= jhi; ++j) {
                             const float wb = 1.f - fabsf((vb + j) * sv + P.cvf - (float)b);
                             if (wb > 0.f) t[r] = fmaf(m2 * wb, __ldg(h + j), t[r]);

@@ -274,4 +274,24 @@ def objective_and_gradient(dose, masks):
     return L, _f32(g)
 
 
+def structure_bits(wl: Workload):
+    """The workload's masks as the inputs of pdrt_objective: (uint32 [nz][ny][nx] with bit s = membership of structure s,
+    lambda_s = weight_s / |s|, prescription_s), structures in the order of wl.masks."""
+    shape = (wl.grid["nz"], wl.grid["ny"], wl.grid["nx"])
+    bits = np.zeros(shape, np.uint32)
+    lam, presc = [], []
+    for s, (mask, weight, p) in enumerate(wl.masks.values()):
+        bits |= mask.astype(np.uint32) << np.uint32(s)
+        lam.append(weight / max(int(mask.sum()), 1))
+        presc.append(p or 0.0)
+    return bits, _f32(lam), _f32(presc)
+
+
+def plan_limits(wl: Workload) -> dict:
+    """Limits of the Eq. 1-3 projection for the planning loop (DESIGN.md §4 c5): leaf gap >= 0.5 mm, pair centres within the
+    fluence map's half width, MU >= 0.1; jaws are tracked, their limits are wide open."""
+    half_u = 0.5 * wl.model["flu_nu"] * wl.model["flu_du"]
+    return dict(leaf_w_min=0.5, leaf_F=half_u, jaw_w_min=0.0, jaw_Fx=1e6, jaw_Fy=1e6, mu_eps=0.1)
+
+
 CONFIGS = {"c1": config1, "c2": config2, "c3": config3, "c4": config4, "c5": config5}

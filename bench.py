@@ -222,6 +222,123 @@ def cpu_baseline(wl):
     return smp.record(smp.time_once())
 
 
+def run_c5_loop(args):
+    """--workload c5: BASELINE.json configs[4] — the 20-iteration planning loop on the device (PlanLoop: pdrt_validate,
+    pdrt_track_jaws, pdrt_dose, pdrt_objective, pdrt_dose_backward, pdrt_validate_backward, pdrt_plan_step).  A step is one
+    loop of 20 iterations from the same initial plan; `value` is the mean time of one forward+backward pair inside the
+    loop (the 20 library pairs), the update steps are timed separately."""
+    import torch
+    from paper_2512_18863_b200 import Engine, PdrtLimits, workloads as W
+    from paper_2512_18863_b200.planning import PlanLoop
+    n_it = 20
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    peaks = load_peaks()
+    wl = make_workload("c5", args.kernel_size)
+    eng = Engine(wl.grid, wl.model, wl.density, device=str(dev))
+    bits, lam, presc = W.structure_bits(wl)
+    limits = PdrtLimits(**W.plan_limits(wl))
+    loop = PlanLoop(eng, wl.leaves, wl.mu, wl.gantry_deg, limits, bits, lam, presc, power=2)
+    l0, m0 = loop.leaves.clone(), loop.mu.clone()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    E = lambda: torch.cuda.Event(enable_timing=True)
+
+    def one_loop(timed):
+        """20 iterations; returns per-iteration (pair, other) event triples when timed."""
+        loop.leaves.copy_(l0); loop.mu.copy_(m0)
+        evs = []
+        for _ in range(n_it):
+            a, b, c, d = (E(), E(), E(), E()) if timed else (None,) * 4
+            if timed: a.record()
+            loop.project()
+            if timed: b.record()
+            eng.dose(loop.p_leaves, loop.jaws, loop.gantry, loop.p_mu, out=loop.dose)
+            eng.objective(loop.dose, loop.bits, loop.lam, loop.presc, loop.power, out=(loop.loss, loop.g))
+            eng.dose_backward(loop.p_leaves, loop.jaws, loop.gantry, loop.p_mu, loop.g, out=loop.gh)
+            if timed: c.record()
+            loop.update()
+            if timed: d.record()
+            evs.append((a, b, c, d))
+        return evs
+
+    clk = ClockSampler(0)
+    clk.__enter__()
+    clk.wait_first()
+    for _ in range(max(1, args.warmup // 3)):
+        one_loop(False)
+    torch.cuda.synchronize()
+    steps = max(1, args.steps // 10)                      # a step is a 20-iteration loop: the default 40 steps become 4 loops
+    pair_ms, other_ms, loop_ms = [], [], []
+    for _ in range(steps):
+        flush.zero_()
+        evs = one_loop(True)
+        torch.cuda.synchronize()
+        pair_ms.append(sum(b.elapsed_time(c) for _, b, c, _ in evs))
+        other_ms.append(sum(a.elapsed_time(b) + c.elapsed_time(d) for a, b, c, d in evs))
+        loop_ms.append(evs[0][0].elapsed_time(evs[-1][3]))
+    loss_first = float(loop.loss[0])
+    clk.__exit__(None, None, None)
+    # the same loop as ONE CUDA graph of an iteration replayed 20 times (no host work between the calls)
+    graph_ms = None
+    try:
+        loop.leaves.copy_(l0); loop.mu.copy_(m0)
+        st = torch.cuda.Stream()
+        st.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(st):
+            loop.iterate()                                # warm the side stream
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                loop.iterate()
+        torch.cuda.current_stream().wait_stream(st)
+        ts = []
+        for _ in range(steps):
+            loop.leaves.copy_(l0); loop.mu.copy_(m0)
+            flush.zero_()
+            a, b = E(), E()
+            a.record()
+            for _ in range(n_it):
+                g.replay()
+            b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        graph_ms = float(np.mean(ts))
+        assert abs(float(loop.loss[0]) - loss_first) <= 1e-6 * abs(loss_first), "graph replay diverged from the eager loop"
+    except Exception as exc:                              # noqa: BLE001 — reported, not fatal
+        graph_ms = f"capture failed: {type(exc).__name__}: {exc}"
+    # stage breakdown and work counters of one forward+backward of the loop's last plan
+    eng.set_profiling(True)
+    loop.project()
+    eng.dose(loop.p_leaves, loop.jaws, loop.gantry, loop.p_mu, out=loop.dose)
+    fw_ms, fw_n = eng.get_stage_ms(); wf = eng.get_work()
+    eng.dose_backward(loop.p_leaves, loop.jaws, loop.gantry, loop.p_mu, loop.g, out=loop.gh)
+    bw_ms, bw_n = eng.get_stage_ms(); wb = eng.get_work()
+    eng.set_profiling(False)
+    K = wf.kernel_size
+    fp32_peak = eng.info.sm_count * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    conv_flops = 2.0 * K * K * wf.footprint_voxels
+    achieved = conv_flops / (fw_ms["conv"] * 1e-3) / 1e12
+    pair = float(np.mean(pair_ms)) / n_it
+    line = dict(metric=METRIC, value=pair, unit="ms", n_gpus=1, steps=steps, warmup=max(1, args.warmup // 3), ms_per_step=float(np.mean(loop_ms)),
+                higher_is_better=False, scaling="strong", vs_baseline=None, dtype="f32", data="synthetic",
+                config=config_dict(wl, 1, dict(loop=f"{n_it} planning iterations per step on the device (PlanLoop); value = mean forward+backward pair "
+                                                    "inside the loop; ms_per_step = the whole loop")),
+                loop_ms=float(np.mean(loop_ms)), pairs_ms_per_loop=float(np.mean(pair_ms)), update_ms_per_loop=float(np.mean(other_ms)),
+                graph_loop_ms=graph_ms, objective_at_iteration_20=loss_first,
+                control_points_per_s=wl.n_cp / (pair * 1e-3), clocks=clk.summary(),
+                gpu_launches=(sum(fw_n.values()) + sum(bw_n.values()) + 7) * n_it * steps,
+                roofline=dict(bound="alu", kernel="k_conv<K,false>", achieved=achieved, peak=fp32_peak, unit="TFLOP/s", frac=achieved / fp32_peak,
+                              traffic=recorded_traffic("c5", K)),
+                stages={k: round(fw_ms[k] + bw_ms[k], 4) for k in fw_ms},
+                work=dict(support_voxels=wf.support_voxels, footprint_voxels=wf.footprint_voxels, conv_macs_issued_fwd=wf.conv_macs,
+                          conv_macs_issued_bwd=wb.conv_macs))
+    if not args.no_cpu_baseline:
+        smp = OracleSample(wl)
+        rec = smp.record(smp.time_once())
+        rec["sample"] += f"; one iteration of the loop (x{n_it} for the loop: {rec['value'] * n_it:.0f} ms)"
+        line["cpu_baseline"] = rec
+    print(json.dumps(line))
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -438,6 +555,7 @@ def main():
     ap.add_argument("--kernel-size", type=int, default=0)
     ap.add_argument("--sweep", action="store_true", help="also time the kernel-size sweep of the workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--single-pass", action="store_true", help="c5: time one forward+backward instead of the 20-iteration planning loop")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     env_world = os.environ.get("WORLD_SIZE")
@@ -447,6 +565,8 @@ def main():
         run_reference(args)
     elif args.gpus > 1 and env_world is None:
         sys.exit(spawn_ranks(args.gpus))
+    elif args.workload == "c5" and args.gpus == 1 and not args.single_pass:
+        run_c5_loop(args)
     else:
         run_ours(args)
 

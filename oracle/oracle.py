@@ -269,6 +269,47 @@ class Oracle:
                                    _p(dl), _p(dj), _p(dm))
         return dl, dj, dm
 
+    # ---- divergent radiological depth
+    @property
+    def fan_shape(self):
+        return (self.m["beam_nw"], self.m["flu_nv"], self.m["flu_nu"])
+
+    def fan_depth(self, gantry_deg):
+        """z_fan[k][b][a]: radiological depth (per unit axial distance) of the ray through map pixel (a,b) at slice k."""
+        z = np.zeros(self.fan_shape)
+        self.lib.orc_fan_depth(C.byref(self.G), self.density.ctypes.data_as(C.c_void_p), C.byref(self.M), C.c_double(float(gantry_deg)), _p(z))
+        return z
+
+    def depth_term(self, z):
+        self.lib.orc_depth_term.restype = C.c_double
+        return float(self.lib.orc_depth_term(C.byref(self.M), C.c_double(float(z))))
+
+    def fan_factor(self, z_fan, z_cax):
+        zf, zc = _d(z_fan), _d(z_cax)
+        F = np.zeros(self.fan_shape)
+        self.lib.orc_fan_factor(C.byref(self.G), C.byref(self.M), _p(zf), _p(zc), _p(F))
+        return F
+
+    def apply_fan_factor(self, F, vol):
+        F, out = _d(F), _d(vol).copy()
+        self.lib.orc_apply_fan_factor(C.byref(self.G), C.byref(self.M), _p(F), _p(out))
+        return out
+
+    def dose_fan(self, leaves, jaws, gantry_deg, mu):
+        n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)
+        out = np.zeros(self.dose_shape)
+        self.lib.orc_dose_fan(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), _p(self._w_tab()), C.c_int(n_cp),
+                              _p(lv), _p(jw), _p(ga), _p(mu), _p(out))
+        return out
+
+    def dose_backward_fan(self, leaves, jaws, gantry_deg, mu, gdose):
+        n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)
+        g = np.ascontiguousarray(gdose, dtype=np.float32)
+        dl, dj, dm = np.zeros_like(lv), np.zeros_like(jw), np.zeros_like(mu)
+        self.lib.orc_dose_backward_fan(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), _p(self._w_tab()),
+                                       C.c_int(n_cp), _p(lv), _p(jw), _p(ga), _p(mu), g.ctypes.data_as(C.c_void_p), _p(dl), _p(dj), _p(dm))
+        return dl, dj, dm
+
     def dose_at(self, leaves, jaws, gantry_deg, mu, ijk):
         """Dose at selected voxels; ijk is [n][3] = (x index, y index, z index)."""
         n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)

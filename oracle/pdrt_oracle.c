@@ -763,3 +763,154 @@ void orc_plan_step(int n_cp, int n_pairs, double step_leaf, double step_mu, cons
     if (ml > 0.0) for (size_t e = 0; e < nl; ++e) leaves[e] -= step_leaf * g_leaves[e] / ml;
     if (mm > 0.0) for (int b = 0; b < n_cp; ++b) mu[b] -= step_mu * g_mu[b] / mm;
 }
+
+/* ================================================================== divergent radiological depth */
+/* PAPER.md:137 traces ONE ray per gantry angle and names the consequence (:197, :357): reduced accuracy where the patient
+ * surface is oblique to the beam.  This optional mode (reading G24) traces one diverging ray per fluence-map
+ * pixel (a,b): from the source through (uf_a, vf_b) on the isocentre plane,
+ *     P(t) = source + t * (w^ + (uf_a/SID) u^ + (vf_b/SID) v^),     t = distance travelled ALONG THE AXIS,
+ * with the sampling rule of Eq. 7 / G8 in t (rho_m at t = (m + 1/2) ds, Z_{m+1} = Z_m + rho_m ds, linear within a step), so
+ * that z_fan[k][b][a] is the radiological depth, measured along the axis direction, at which ray (a,b) crosses slice k.
+ * Depth is counted per unit AXIAL distance: in a medium that is homogeneous across the beam every ray then reproduces the
+ * central-axis profile exactly, and the mode reduces to the paper's.                                                     */
+void orc_fan_depth(const orc_grid *g, const float *rho, const orc_model *m, double gantry_deg, double *z_fan)
+{
+    double c, s;
+    gantry_axes(gantry_deg, &c, &s);
+    const double ux = c, uy = s, wx = -s, wy = c;
+    const double srcx = g->iso[0] - m->sid * wx, srcy = g->iso[1] - m->sid * wy, srcz = g->iso[2];
+    const double ds = m->ray_step;
+    const int Nw = m->beam_nw, nu = m->flu_nu, nv = m->flu_nv;
+    double dmax = m->sid + beam_w(m, Nw - 1);
+    int M = dmax > 0 ? (int)floor(dmax / ds) + 2 : 1;
+#pragma omp parallel
+    {
+        double *Z = malloc(sizeof(double) * (M + 1)), *r = malloc(sizeof(double) * (M + 1));
+#pragma omp for schedule(static)
+        for (int b = 0; b < nv; ++b)
+            for (int a = 0; a < nu; ++a) {
+                const double tu = flu_u(m, a) / m->sid, tv = flu_v(m, b) / m->sid;
+                const double dx = wx + tu * ux, dy = wy + tu * uy, dz = tv;
+                Z[0] = 0.0;
+                for (int mm = 0; mm < M; ++mm) {
+                    double t = (mm + 0.5) * ds;
+                    r[mm] = density_at(g, rho, srcx + t * dx, srcy + t * dy, srcz + t * dz);
+                    Z[mm + 1] = Z[mm] + r[mm] * ds;
+                }
+                for (int k = 0; k < Nw; ++k) {
+                    double q = (m->sid + beam_w(m, k)) / ds, zz = 0.0;
+                    if (q > 0.0) { int m0 = (int)floor(q); zz = Z[m0] + (q - m0) * r[m0] * ds; }
+                    z_fan[((size_t)k * nv + b) * nu + a] = zz;
+                }
+            }
+        free(Z); free(r);
+    }
+}
+/* Broad-beam depth term carried by the kernel amplitudes (reading G6): the plane integral of K(r;z),
+ * T(z) = 2 pi (A(z)/a(z) + B(z)/b(z)), tabulated at the kernel table's nodes and interpolated linearly like the kernels (G5). */
+double orc_depth_term(const orc_model *m, double z)
+{
+    double t = z / m->dz;
+    int n0 = (int)floor(t);
+    if (n0 < 0) n0 = 0;
+    if (n0 > m->n_z - 2) n0 = m->n_z - 2;
+    double f = t - n0;
+    if (f < 0.0) f = 0.0;
+    if (f > 1.0) f = 1.0;
+    double T0 = 2.0 * ORC_PI * (m->kA[n0] / m->ka[n0] + m->kB[n0] / m->kb[n0]);
+    double T1 = 2.0 * ORC_PI * (m->kA[n0 + 1] / m->ka[n0 + 1] + m->kB[n0 + 1] / m->kb[n0 + 1]);
+    return (1.0 - f) * T0 + f * T1;
+}
+/* Depth factor at the ray nodes: F[k][b][a] = T(z_fan[k][b][a]) / T(z_cax[k]); 1 where T(z_cax[k]) <= 0 (the slice kernel
+ * is zero there, so is the dose).  It weights the projected fluence (input side); the lateral kernel stays per slice.   */
+void orc_fan_factor(const orc_grid *g, const orc_model *m, const double *z_fan, const double *z_cax, double *F)
+{
+    (void)g;
+    const size_t nf = (size_t)m->flu_nu * m->flu_nv;
+    for (int k = 0; k < m->beam_nw; ++k) {
+        double Tc = orc_depth_term(m, z_cax[k]);
+        for (size_t e = 0; e < nf; ++e) F[(size_t)k * nf + e] = Tc > 0.0 ? orc_depth_term(m, z_fan[(size_t)k * nf + e]) / Tc : 1.0;
+    }
+}
+/* Interpolation between node centres with the indices clamped to the array (the depth factor exists beyond the map's edge). */
+static double bilinear_clamp(const double *a, int n0, int n1, double f0, double f1)
+{
+    int i0 = (int)floor(f0), i1 = (int)floor(f1);
+    double t0 = f0 - i0, t1 = f1 - i1, acc = 0.0;
+    for (int c = 0; c < 4; ++c) {
+        int x = i0 + (c & 1), y = i1 + (c >> 1);
+        x = x < 0 ? 0 : (x > n0 - 1 ? n0 - 1 : x);
+        y = y < 0 ? 0 : (y > n1 - 1 ? n1 - 1 : y);
+        acc += ((c & 1) ? t0 : 1.0 - t0) * ((c >> 1) ? t1 : 1.0 - t1) * a[(size_t)y * n0 + x];
+    }
+    return acc;
+}
+/* Depth-weighted projection: Phivol'[k][j][i] = Phivol[k][j][i] * bilinear_clamp(F[k]; fa, fb) with (fa, fb) the sampling
+ * position of Eq. 5 — the factor of the ray through the voxel, interpolated between the ray nodes.  `transpose` applies the
+ * same diagonal weighting to H before orc_project_adjoint (the factor carries no gradient).                              */
+void orc_apply_fan_factor(const orc_grid *g, const orc_model *m, const double *F, double *vol)
+{
+    const int Nu = m->beam_nu, Nv = g->nz, Nw = m->beam_nw;
+    const size_t nf = (size_t)m->flu_nu * m->flu_nv;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < Nw; ++k) {
+        double mag = m->sid / (m->sid + beam_w(m, k));
+        for (int j = 0; j < Nv; ++j)
+            for (int i = 0; i < Nu; ++i) {
+                double *p = &vol[((size_t)k * Nv + j) * Nu + i];
+                if (*p == 0.0) continue;
+                double fa = mag * beam_u(m, i) / m->flu_du + 0.5 * (m->flu_nu - 1);
+                double fb = mag * beam_v(g, j) / m->flu_dv + 0.5 * (m->flu_nv - 1);
+                *p *= bilinear_clamp(F + (size_t)k * nf, m->flu_nu, m->flu_nv, fa, fb);
+            }
+    }
+}
+/* Whole path in the divergent-depth mode: as orc_dose / orc_dose_backward with the projected fluence (resp. H) weighted. */
+void orc_dose_fan(const orc_grid *g, const orc_model *m, const float *rho, const double *W_tab, int n_cp,
+                  const double *leaves, const double *jaws, const double *gantry_deg, const double *mu, double *dose)
+{
+    const size_t nb = (size_t)m->beam_nu * g->nz * m->beam_nw, np = (size_t)g->nx * g->ny * g->nz;
+    const size_t nf = (size_t)m->flu_nu * m->flu_nv;
+    double *Db = malloc(sizeof(double) * nb), *Phivol = malloc(sizeof(double) * nb), *Phimap = malloc(sizeof(double) * nf);
+    double *z = malloc(sizeof(double) * m->beam_nw), *zf = malloc(sizeof(double) * nf * m->beam_nw), *F = malloc(sizeof(double) * nf * m->beam_nw);
+    memset(dose, 0, sizeof(double) * np);
+    for (int b = 0; b < n_cp; ++b) {
+        orc_fluence(m, leaves + (size_t)b * 2 * m->n_pairs, jaws + (size_t)b * 4, NULL, NULL, NULL, Phimap);
+        orc_radiological_depth(g, rho, m, gantry_deg[b], z);
+        orc_fan_depth(g, rho, m, gantry_deg[b], zf);
+        orc_fan_factor(g, m, zf, z, F);
+        orc_project(g, m, Phimap, Phivol);
+        orc_apply_fan_factor(g, m, F, Phivol);
+        orc_convolve(g, m, W_tab, z, Phivol, Db);
+        orc_resample_add(g, m, gantry_deg[b], m->cal * mu[b], Db, dose);
+    }
+    free(Db); free(Phivol); free(Phimap); free(z); free(zf); free(F);
+}
+void orc_dose_backward_fan(const orc_grid *g, const orc_model *m, const float *rho, const double *W_tab, int n_cp,
+                           const double *leaves, const double *jaws, const double *gantry_deg, const double *mu,
+                           const float *gdose, double *d_leaves, double *d_jaws, double *d_mu)
+{
+    const size_t nb = (size_t)m->beam_nu * g->nz * m->beam_nw, nf = (size_t)m->flu_nu * m->flu_nv;
+    const int np = m->n_pairs;
+    double *G = malloc(sizeof(double) * nb), *H = malloc(sizeof(double) * nb), *z = malloc(sizeof(double) * m->beam_nw);
+    double *Phimap = malloc(sizeof(double) * nf), *gPhimap = malloc(sizeof(double) * nf);
+    double *zf = malloc(sizeof(double) * nf * m->beam_nw), *F = malloc(sizeof(double) * nf * m->beam_nw);
+    for (int b = 0; b < n_cp; ++b) {
+        const double *lv = leaves + (size_t)b * 2 * np, *jw = jaws + (size_t)b * 4;
+        orc_fluence(m, lv, jw, NULL, NULL, NULL, Phimap);
+        orc_radiological_depth(g, rho, m, gantry_deg[b], z);
+        orc_fan_depth(g, rho, m, gantry_deg[b], zf);
+        orc_fan_factor(g, m, zf, z, F);
+        orc_resample_adjoint(g, m, gantry_deg[b], gdose, G);
+        orc_convolve_adjoint(g, m, W_tab, z, G, H);
+        orc_apply_fan_factor(g, m, F, H);
+        orc_project_adjoint(g, m, H, gPhimap);
+        double dot = 0.0;
+        for (size_t e = 0; e < nf; ++e) dot += Phimap[e] * gPhimap[e];
+        d_mu[b] = m->cal * dot;
+        orc_fluence_adjoint(m, lv, jw, gPhimap, d_leaves + (size_t)b * 2 * np, d_jaws + (size_t)b * 4);
+        for (int e = 0; e < 2 * np; ++e) d_leaves[(size_t)b * 2 * np + e] *= m->cal * mu[b];
+        for (int e = 0; e < 4; ++e) d_jaws[(size_t)b * 4 + e] *= m->cal * mu[b];
+    }
+    free(G); free(H); free(z); free(Phimap); free(gPhimap); free(zf); free(F);
+}

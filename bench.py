@@ -135,13 +135,12 @@ class ClockSampler:
                     window="NVML every 20 ms from the first warm-up step to the end of the timed steps (same load throughout)")
 
 
-def make_workload(name, kernel_size):
+def make_workload(name, kernel_size, depth_mode="axis"):
     from paper_2512_18863_b200 import workloads as W
-    if name == "c4":
-        return W.config4(kernel_size or 21)
-    wl = W.CONFIGS[name]()
+    wl = W.config4(kernel_size or 21) if name == "c4" else W.CONFIGS[name]()
     if kernel_size:
         wl.model["kernel_size"] = kernel_size
+    wl.model["depth_mode"] = 1 if depth_mode == "fan" else 0
     return wl
 
 
@@ -152,6 +151,7 @@ def config_dict(wl, n_gpus, extra=None):
                       f"kernel {m['kernel_size']}, forward+backward",
              n_cp=wl.n_cp, kernel_size=m["kernel_size"], seed=wl.seed,
              parallelism=f"control points sharded over {n_gpus} GPU(s)" if n_gpus > 1 else "1 GPU",
+             depth_mode="fan (one diverging ray per fluence-map pixel)" if m.get("depth_mode") else "axis (central-axis ray, the paper's mode)",
              l2="256 MiB memset between timed steps (L2 flush); compact D_b/G_b blocks exceed L2")
     if extra:
         c.update(extra)
@@ -355,7 +355,7 @@ def run_ours(args):
     dev = torch.device(f"cuda:{local}")
     torch.cuda.set_device(dev)
     peaks = load_peaks()
-    wl = make_workload(args.workload, args.kernel_size)
+    wl = make_workload(args.workload, args.kernel_size, args.depth_mode)
     eng = Engine(wl.grid, wl.model, wl.density, device=str(dev))
 
     # shard control points (contiguous blocks); every rank holds the density, tables and dL/dDose
@@ -470,6 +470,12 @@ def run_ours(args):
             if s in byts and stage_ms[s] > 0:
                 gbs = byts[s] / (stage_ms[s] * 1e-3) / 1e9
                 stages[s].update(algorithmic_gb=round(byts[s] / 1e9, 4), gbs=round(gbs, 1), hbm_frac=round(gbs / peaks["hbm_gbs"], 4))
+        if wf.fan_rays:          # divergent-depth mode: the ray marcher (k_fan_depth) dominates the depth stage
+            fan_b = 4.0 * nvox + 4.0 * wf.fan_rays * eng.info.beam_nw          # density read once + depth factors written
+            ms_d = stage_ms["depth"] / 2.0                                     # forward and backward both trace the rays
+            stages["depth"].update(fan_rays=wf.fan_rays, algorithmic_gb=round(fan_b / 1e9, 4), gbs=round(fan_b / (ms_d * 1e-3) / 1e9, 1),
+                                   hbm_frac=round(fan_b / (ms_d * 1e-3) / 1e9 / peaks["hbm_gbs"], 4),
+                                   note="k_depth + k_fan_depth, per call; bytes = density once + factors written; at most fan_rays x ray_samples trilinear samples")
         stages["conv"].update(tflops=round(conv_flops / (stage_ms["conv"] * 1e-3) / 1e12, 2) if stage_ms["conv"] > 0 else None,
                               issued_tflops=round(2.0 * wf.conv_macs / (stage_ms["conv"] * 1e-3) / 1e12, 2) if stage_ms["conv"] > 0 else None)
         stages["conv_adj"].update(tflops=round(conv_adj_flops / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None,
@@ -555,6 +561,7 @@ def main():
     ap.add_argument("--kernel-size", type=int, default=0)
     ap.add_argument("--sweep", action="store_true", help="also time the kernel-size sweep of the workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--depth-mode", default="axis", choices=("axis", "fan"), help="fan: one diverging ray per fluence-map pixel (NEXT-1)")
     ap.add_argument("--single-pass", action="store_true", help="c5: time one forward+backward instead of the 20-iteration planning loop")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

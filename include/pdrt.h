@@ -105,7 +105,16 @@ typedef struct {
     int32_t beam_nu, beam_nw;            /* beam grid; beam_nu == 0 selects the default grid as a whole:  */
     float   beam_du, beam_dw, beam_wmin; /*   Nu = nx, Nw = ny, du = dw = sx, wmin = -(Nw-1)/2 * dw       */
     float   ray_step_mm;                 /* ray-march step; 0 => 0.5 * min(sx, sy, sz)                    */
+    int32_t depth_mode;                  /* PDRT_DEPTH_AXIS (0, the paper's mode) or PDRT_DEPTH_FAN       */
 } pdrt_beam_model;
+
+/* Radiological-depth modes.  PDRT_DEPTH_AXIS: one ray per gantry angle through the isocentre (the paper's
+ * mode and the default).  PDRT_DEPTH_FAN (reading G24): additionally one diverging ray
+ * per fluence-map pixel, depth counted per unit axial distance; the projected fluence is weighted by
+ * T(z_ray)/T(z_axis), T(z) = 2 pi (A/a + B/b)(z) the plane integral of the kernel, interpolated between the rays; the
+ * lateral kernel stays per slice.  Identical to the paper's mode where the medium is homogeneous across the beam. */
+#define PDRT_DEPTH_AXIS 0
+#define PDRT_DEPTH_FAN  1
 
 /* Resolved sizes of an engine (after defaults). */
 typedef struct {
@@ -131,6 +140,8 @@ typedef struct {
     int64_t  region_voxels;     /* voxels of the compact per-CP beam-frame regions (materialised) */
     int64_t  conv_macs;         /* multiply-adds the conv kernel issues (k_compiled^2 per output) */
     int32_t  kernel_size, kernel_size_compiled;
+    int64_t  fan_rays;          /* PDRT_DEPTH_FAN: diverging rays traced (sum over control points), else 0  */
+    int32_t  ray_samples;       /* samples per ray (upper bound: samples outside the grid are skipped)     */
 } pdrt_work;
 
 /* pdrt_create: grid geometry, density volume [nz][ny][nx] (host OR device pointer; copied) and
@@ -147,6 +158,9 @@ PDRT_API const char *pdrt_last_error(const pdrt_engine *engine);
 /* Rebuilds W_tab for another lateral kernel size (odd, 3..63); used by the kernel-size sweep
  * (Table 4).  Synchronises the device. */
 PDRT_API int pdrt_set_kernel_size(pdrt_engine *engine, int32_t kernel_size);
+
+/* Switches the radiological-depth mode (PDRT_DEPTH_AXIS / PDRT_DEPTH_FAN) for subsequent calls. */
+PDRT_API int pdrt_set_depth_mode(pdrt_engine *engine, int32_t depth_mode);
 
 PDRT_API int pdrt_get_info(const pdrt_engine *engine, pdrt_info *info);
 PDRT_API int pdrt_get_work(pdrt_engine *engine, pdrt_work *work);
@@ -211,9 +225,14 @@ PDRT_API int pdrt_dose_backward_host(pdrt_engine *engine, int32_t n_cp,
  *   pdrt_stage_beam_dose S3-S5: beam-frame dose D_b of ONE control point, dense
  *                                                    db_dev     [beam_nw][beam_nv][beam_nu]
  *   pdrt_stage_grad_fluence S7-S9: dL/dPhimap per control point (zero outside the fluence
- *                        support of that control point) gphimap_dev [n_cp][flu_nv][flu_nu]      */
+ *                        support of that control point) gphimap_dev [n_cp][flu_nv][flu_nu]
+ *   pdrt_stage_fan_factor (PDRT_DEPTH_FAN) depth factor at the ray nodes, dense
+ *                                                    factor_dev [n_cp][beam_nw][flu_nv][flu_nu], 0 outside the rays traced
+ *                                                    (the fluence support bbox grown by one pixel)                          */
 PDRT_API int pdrt_stage_fluence(pdrt_engine *engine, int32_t n_cp, const float *leaves_dev, const float *jaws_dev,
                        float *phimap_dev, void *cuda_stream);
+PDRT_API int pdrt_stage_fan_factor(pdrt_engine *engine, int32_t n_cp, const float *leaves_dev, const float *jaws_dev,
+                          const float *gantry_deg_dev, float *factor_dev, void *cuda_stream);
 PDRT_API int pdrt_stage_depth(pdrt_engine *engine, int32_t n_cp, const float *gantry_deg_dev,
                      float *zrad_dev, void *cuda_stream);
 PDRT_API int pdrt_stage_beam_dose(pdrt_engine *engine, const float *leaves_dev, const float *jaws_dev,

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpdrt.so")
 
 SYMBOLS = ("pdrt_create", "pdrt_destroy", "pdrt_last_error", "pdrt_set_kernel_size", "pdrt_get_info", "pdrt_get_work",
-           "pdrt_set_profiling", "pdrt_get_stage_ms",
+           "pdrt_set_profiling", "pdrt_get_stage_ms", "pdrt_set_depth_mode", "pdrt_stage_fan_factor",
            "pdrt_dose", "pdrt_dose_backward", "pdrt_dose_host", "pdrt_dose_backward_host",
            "pdrt_stage_fluence", "pdrt_stage_depth", "pdrt_stage_beam_dose", "pdrt_stage_grad_fluence",
            "pdrt_mu_epsilon", "pdrt_validate", "pdrt_validate_backward", "pdrt_objective", "pdrt_track_jaws", "pdrt_plan_step")
@@ -44,7 +44,7 @@ class PdrtBeamModel(C.Structure):
                 ("kernel_size", C.c_int32), ("cal", C.c_float),
                 ("beam_nu", C.c_int32), ("beam_nw", C.c_int32),
                 ("beam_du", C.c_float), ("beam_dw", C.c_float), ("beam_wmin", C.c_float),
-                ("ray_step_mm", C.c_float)]
+                ("ray_step_mm", C.c_float), ("depth_mode", C.c_int32)]
 
 
 class PdrtInfo(C.Structure):
@@ -60,7 +60,8 @@ class PdrtInfo(C.Structure):
 class PdrtWork(C.Structure):
     _fields_ = [("n_cp", C.c_int32), ("conv_items", C.c_int64), ("support_voxels", C.c_int64),
                 ("footprint_voxels", C.c_int64), ("region_voxels", C.c_int64), ("conv_macs", C.c_int64),
-                ("kernel_size", C.c_int32), ("kernel_size_compiled", C.c_int32)]
+                ("kernel_size", C.c_int32), ("kernel_size_compiled", C.c_int32),
+                ("fan_rays", C.c_int64), ("ray_samples", C.c_int32)]
 
 
 class PdrtLimits(C.Structure):
@@ -93,6 +94,8 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.pdrt_last_error.argtypes = [vp]
     lib.pdrt_last_error.restype = C.c_char_p
     lib.pdrt_set_kernel_size.argtypes = [vp, i32]
+    lib.pdrt_set_depth_mode.argtypes = [vp, i32]
+    lib.pdrt_stage_fan_factor.argtypes = [vp, i32, vp, vp, vp, vp, vp]
     lib.pdrt_get_info.argtypes = [vp, C.POINTER(PdrtInfo)]
     lib.pdrt_get_work.argtypes = [vp, C.POINTER(PdrtWork)]
     lib.pdrt_set_profiling.argtypes = [vp, i32]
@@ -156,7 +159,7 @@ class Engine:
                           model["kernel_size"], model["cal"],
                           int(model.get("beam_nu", 0)), int(model.get("beam_nw", 0)),
                           float(model.get("beam_du", 0.0)), float(model.get("beam_dw", 0.0)),
-                          float(model.get("beam_wmin", 0.0)), float(model.get("ray_step_mm", 0.0)))
+                          float(model.get("beam_wmin", 0.0)), float(model.get("ray_step_mm", 0.0)), int(model.get("depth_mode", 0)))
         if isinstance(density, torch.Tensor):
             dens = density.to(dtype=torch.float32).contiguous()
             dptr = dens.data_ptr()
@@ -223,6 +226,18 @@ class Engine:
     def set_kernel_size(self, k: int):
         self._check(self.lib.pdrt_set_kernel_size(self.handle, int(k)))
         self.info = self.get_info()
+
+    def set_depth_mode(self, mode: int):
+        """0 = central-axis ray (the paper's mode), 1 = one diverging ray per fluence-map pixel (PDRT_DEPTH_FAN)."""
+        self._check(self.lib.pdrt_set_depth_mode(self.handle, int(mode)))
+
+    def stage_fan_factor(self, leaves, jaws, gantry_deg):
+        ga = self._dev(gantry_deg)
+        n_cp = int(ga.shape[0])
+        lv, jw = self._dev(leaves, (n_cp, 2, self.n_pairs)), self._dev(jaws, (n_cp, 4))
+        out = self.torch.empty((n_cp, self.info.beam_nw, *self.flu_shape), dtype=self.torch.float32, device=self.device)
+        self._check(self.lib.pdrt_stage_fan_factor(self.handle, n_cp, lv.data_ptr(), jw.data_ptr(), ga.data_ptr(), out.data_ptr(), self._stream()))
+        return out
 
     @property
     def dose_shape(self):

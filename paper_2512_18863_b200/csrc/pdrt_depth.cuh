@@ -84,4 +84,155 @@ k_depth(Params P, int n_cp, const float *__restrict__ rho, const float *__restri
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Divergent radiological depth (optional mode; reading G24 of DESIGN.md).  One diverging ray per
+// fluence-map pixel (a,b) of the support bbox (grown by one pixel, for the interpolation): from the source through
+// (uf_a, vf_b) on the isocentre plane, P(t) = source + t (w^ + uf/SID u^ + vf/SID v^), t = distance along the axis; Eq. 7
+// with the sampling rule of the central-axis ray in t, so depth counts per unit axial distance and a medium that is
+// homogeneous across the beam gives every ray the central-axis profile.  At every slice the depth factor
+//   F[k][b][a] = T(z_fan) / T(z_cax[k])   (1 where T(z_cax[k]) <= 0),   T(z) = 2 pi (A/a + B/b)(z)  (plane integral of K)
+// is stored; k_apply_fan multiplies the projected fluence (forward) resp. H_b (adjoint) by its bilinear interpolant.
+struct FanBox { int a0, b0, bw, bh; };     // pixels [a0, a0+bw) x [b0, b0+bh) of the control point's rays
+__device__ __forceinline__ FanBox fan_box(const Params &P, const CpDesc &d)
+{
+    FanBox f;
+    f.a0 = max(0, d.a0 - 1); f.b0 = max(0, d.b0 - 1);
+    f.bw = min(P.Nuf - 1, d.a1 + 1) - f.a0 + 1; f.bh = min(P.Nvf - 1, d.b1 + 1) - f.b0 + 1;
+    return f;
+}
+__device__ __forceinline__ float depth_term(const float *__restrict__ Ttab, int n_z, float dz, float z)
+{
+    const float t = z / dz;
+    int n0 = (int)floorf(t);
+    n0 = min(max(n0, 0), n_z - 2);
+    const float f = fminf(fmaxf(t - n0, 0.f), 1.f);
+    return (1.f - f) * __ldg(Ttab + n0) + f * __ldg(Ttab + n0 + 1);
+}
+
+constexpr int FAN_THREADS = 128;
+// Grid: (ceil(Nuf*Nvf / 128), n_cp); one thread per ray, lanes along a (= along u^ in the patient x-y plane).
+// fan [n_cp][Nw][bh][bw] with stride fan_stride per control point.  Positions and the running sum are float64 (R1).
+__global__ void __launch_bounds__(FAN_THREADS)
+k_fan_depth(Params P, const CpDesc *__restrict__ desc, int n_cp, const float *__restrict__ rho, const float *__restrict__ gantry_deg,
+            const float *__restrict__ zrad, const float *__restrict__ Ttab, size_t fan_stride, float *__restrict__ fan)
+{
+    const int cp = blockIdx.y;
+    if (cp >= n_cp) return;
+    const CpDesc d = desc[cp];
+    if (d.a0 > d.a1) return;
+    const FanBox fb = fan_box(P, d);
+    const int r = blockIdx.x * FAN_THREADS + threadIdx.x;
+    if (r >= fb.bw * fb.bh) return;
+    const int rb = r / fb.bw, ra = r - rb * fb.bw;
+    const double phi = (double)gantry_deg[cp] * 3.14159265358979323846 / 180.0;
+    const double cs = cos(phi), sn = sin(phi);
+    const double tu = (double)((fb.a0 + ra - P.cuf) * P.Du) / (double)P.sid, tv = (double)((fb.b0 + rb - P.cvf) * P.Dv) / (double)P.sid;
+    const double dx = -sn + tu * cs, dy = cs + tu * sn, dz = tv;
+    const double srcx = (double)P.isox + (double)P.sid * sn, srcy = (double)P.isoy - (double)P.sid * cs, srcz = (double)P.isoz;
+    const double ds = P.ray_step;
+    const int M = P.M_ray;
+    // samples before the ray enters the grid's box contribute exact zeros: start at the first sample that can be inside
+    double t_in = 0.0;
+    {
+        const double o[3] = { (double)P.ox, (double)P.oy, (double)P.oz }, sp[3] = { (double)P.sx, (double)P.sy, (double)P.sz };
+        const double s0[3] = { srcx, srcy, srcz }, dd[3] = { dx, dy, dz };
+        const int N[3] = { P.nx, P.ny, P.nz };
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (dd[a] != 0.0) {
+                const double t0 = (o[a] - 0.5 * sp[a] - s0[a]) / dd[a], t1 = (o[a] + (N[a] - 0.5) * sp[a] - s0[a]) / dd[a];
+                t_in = fmax(t_in, fmin(t0, t1));
+            }
+        }
+    }
+    int m = max(0, (int)floor(t_in / ds - 0.5) - 1);          // one sample of slack: the per-sample box test decides
+    float *out = fan + (size_t)cp * fan_stride + (size_t)rb * fb.bw + ra;
+    const size_t kstride = (size_t)fb.bw * fb.bh;
+    const float *zc = zrad + (size_t)cp * P.Nw;
+    double Z = 0.0;
+    int k = 0;
+    auto emit = [&](int kk, double z) {
+        const float Tc = depth_term(Ttab, P.n_z, P.dz, zc[kk]);
+        out[(size_t)kk * kstride] = Tc > 0.f ? depth_term(Ttab, P.n_z, P.dz, (float)z) / Tc : 1.f;
+    };
+    // slices in front of the first sample taken: depth 0
+    for (; k < P.Nw; ++k) {
+        const double q = ((double)P.sid + (double)P.wmin + k * (double)P.dw) / ds;
+        if (q > 0.0 && (int)floor(q) >= m) break;
+        emit(k, 0.0);
+    }
+    for (; m < M && k < P.Nw; ++m) {
+        const double t = (m + 0.5) * ds;
+        const double v = density_at(P, rho, srcx + t * dx, srcy + t * dy, srcz + t * dz);
+        for (; k < P.Nw; ++k) {                                // slices whose depth falls into this step
+            const double q = ((double)P.sid + (double)P.wmin + k * (double)P.dw) / ds;
+            const int m0 = min((int)floor(q), M - 1);
+            if (m0 != m) break;
+            emit(k, Z + (q - m0) * v * ds);
+        }
+        Z += v * ds;
+    }
+    for (; k < P.Nw; ++k) emit(k, Z);
+}
+
+// Multiplies vol (Phivol over S_k, forward; H_b over S_k, adjoint) by the bilinear interpolant (indices clamped to the ray
+// box) of the depth factor at the voxel's sampling position (fa, fb) of Eq. 5.  Grid: (X, n_cp); a warp per (slice, row).
+__global__ void __launch_bounds__(256)
+k_apply_fan(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp, size_t fan_stride,
+            const float *__restrict__ fan, float *__restrict__ vol)
+{
+    const int slot = blockIdx.y;
+    if (slot >= n_cp) return;
+    const int cp = cp0 + slot;
+    const CpDesc d = desc[cp];
+    if (d.a0 > d.a1) return;
+    const FanBox fb = fan_box(P, d);
+    const int lane = threadIdx.x & 31;
+    const int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+    float *vc = vol + (size_t)slot * (size_t)P.stride_cp;
+    for (int k = 0; k < P.Nw; ++k) {
+        const SliceBox16 S = load_box(sbox, (size_t)cp * P.Nw + k);
+        if (S.u0 > S.u1) continue;
+        const float mag = P.sid / (P.sid + P.wmin + k * P.dw);
+        const float su = mag * P.du / P.Du, sv = mag / P.Dv;
+        const float *Fk = fan + (size_t)cp * fan_stride + (size_t)k * fb.bw * fb.bh;
+        for (int i = S.u0 + warp0; i <= S.u1; i += n_warps) {
+            const float fa = (i - P.cu) * su + P.cuf - (float)fb.a0;
+            const float fla = floorf(fa);
+            const float ta = fa - fla;
+            const int a0 = min(max((int)fla, 0), fb.bw - 1), a1 = min(max((int)fla + 1, 0), fb.bw - 1);
+            float *row = vc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
+            for (int j = S.v0 + lane; j <= S.v1; j += 32) {
+                const float fbv = (P.v0 + j * P.dv) * sv + P.cvf - (float)fb.b0;
+                const float flb = floorf(fbv);
+                const float tb = fbv - flb;
+                const int b0 = min(max((int)flb, 0), fb.bh - 1), b1 = min(max((int)flb + 1, 0), fb.bh - 1);
+                const float f = (1.f - tb) * ((1.f - ta) * __ldg(Fk + b0 * fb.bw + a0) + ta * __ldg(Fk + b0 * fb.bw + a1)) +
+                                tb * ((1.f - ta) * __ldg(Fk + b1 * fb.bw + a0) + ta * __ldg(Fk + b1 * fb.bw + a1));
+                row[j] *= f;
+            }
+        }
+    }
+}
+
+// Expands the compact depth factors to dense [n_cp][Nw][Nvf][Nuf] maps, 0 outside the rays traced (stage tap for tests).
+__global__ void k_expand_fan(Params P, const CpDesc *__restrict__ desc, int n_cp, size_t fan_stride, const float *__restrict__ fan,
+                             float *__restrict__ dense)
+{
+    const size_t per = (size_t)P.Nw * P.Nvf * P.Nuf, n = per * n_cp;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        const int cp = (int)(e / per);
+        const size_t r = e - (size_t)cp * per;
+        const int a = (int)(r % P.Nuf), b = (int)((r / P.Nuf) % P.Nvf), k = (int)(r / ((size_t)P.Nuf * P.Nvf));
+        const CpDesc &d = desc[cp];
+        float v = 0.f;
+        if (d.a0 <= d.a1) {
+            const FanBox fb = fan_box(P, d);
+            if (a >= fb.a0 && a < fb.a0 + fb.bw && b >= fb.b0 && b < fb.b0 + fb.bh)
+                v = fan[(size_t)cp * fan_stride + ((size_t)k * fb.bh + (b - fb.b0)) * fb.bw + (a - fb.a0)];
+        }
+        dense[e] = v;
+    }
+}
+
 }  // namespace pdrt

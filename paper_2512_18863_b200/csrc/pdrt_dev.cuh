@@ -84,7 +84,7 @@ struct CpDesc {
 };
 
 struct WorkCounters {
-    long long items, support_vox, footprint_vox, region_vox, macs_fwd, macs_adj;
+    long long items, support_vox, footprint_vox, region_vox, macs_fwd, macs_adj, fan_rays;
 };
 
 // Row pitch [floats] of the conv input tile for `naf` thread-tiles along v: the (K+7)-wide register window of

@@ -74,7 +74,10 @@ struct pdrt_engine {
     std::vector<double> kA, ka, kB, kb;
     std::string err;
     // persistent device data
-    DevBuf<float> density, wtab, pool;
+    DevBuf<float> density, wtab, pool, ttab;
+    int depth_mode = PDRT_DEPTH_AXIS;
+    DevBuf<float> fan;                // PDRT_DEPTH_FAN: depth factor at the ray nodes, [n_cp][Nw][bh][bw] with stride fan_stride()
+    size_t fan_stride() const { return (size_t)P.Nw * P.Nuf * P.Nvf; }
     // per-call scratch (sized by control-point capacity)
     DevBuf<CpDesc> desc;
     DevBuf<SliceBox16> sbox, wbox;     // [n_cp][Nw] per-slice boxes: fluence support S_k, written part of D_b
@@ -289,8 +292,13 @@ int run_setup(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, 
     }
     CU(e, cudaGetLastError());
     if (need_depth) {
-        StageTimer t(e, PDRT_STAGE_DEPTH, st);
+        const bool fan = e->depth_mode == PDRT_DEPTH_FAN;
+        if (fan) CU(e, e->fan.ensure((size_t)n_cp * e->fan_stride()));
+        StageTimer t(e, PDRT_STAGE_DEPTH, st, fan ? 2 : 1);
         k_depth<<<n_cp, DEPTH_THREADS, 0, st>>>(e->P, n_cp, e->density.p, gantry, e->rho_s.p, e->Z_s.p, e->zrad.p);
+        if (fan)
+            k_fan_depth<<<dim3((e->P.Nuf * e->P.Nvf + FAN_THREADS - 1) / FAN_THREADS, n_cp), FAN_THREADS, 0, st>>>(
+                e->P, e->desc.p, n_cp, e->density.p, gantry, e->zrad.p, e->ttab.p, e->fan_stride(), e->fan.p);
     }
     CU(e, cudaGetLastError());
     return PDRT_OK;
@@ -311,12 +319,14 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
         const int n = std::min(nb, n_cp - cp0);
         {
             StageTimer t(e, PDRT_STAGE_SCAN, st);
-            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, 0, e->tile_base.p, e->counters.p);
+            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, 0, e->P.Nuf, e->P.Nvf, e->tile_base.p, e->counters.p);
         }
         CU(e, cudaGetLastError());
         {
             StageTimer t(e, PDRT_STAGE_PROJECT, st);
             k_project<<<dim3(project_blocks(e->P), n), PROJECT_THREADS, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->phimapT.p, e->bufB.p);
+            if (e->depth_mode == PDRT_DEPTH_FAN)
+                k_apply_fan<<<dim3(4, n), 256, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->fan_stride(), e->fan.p, e->bufB.p);
         }
         CU(e, cudaGetLastError());
         {
@@ -364,7 +374,7 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
         const int n = std::min(nb, n_cp - cp0);
         {
             StageTimer t(e, PDRT_STAGE_SCAN, st);
-            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, 1, e->tile_base.p, e->counters.p);
+            k_scan_items<<<1, 256, 0, st>>>(e->desc.p, cp0, n, 1, e->P.Nuf, e->P.Nvf, e->tile_base.p, e->counters.p);
         }
         CU(e, cudaGetLastError());
         {
@@ -380,6 +390,8 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
         if (rc) return rc;
         {
             StageTimer t(e, PDRT_STAGE_PROJECT_ADJ, st);
+            if (e->depth_mode == PDRT_DEPTH_FAN)      // the factor is a fixed diagonal weighting: the transpose applies it to H_b
+                k_apply_fan<<<dim3(4, n), 256, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->fan_stride(), e->fan.p, e->bufA.p);
             k_project_adjoint<<<dim3(PA_CLUSTER * ((e->P.Nvf + 31) / 32), n), PA_THREADS, sizeof(float) * 32 * (size_t)e->P.Nuf * e->pa_warps, st>>>(
                 e->P, e->desc.p, e->sbox.p, cp0, n, e->pa_warps, e->bufA.p, e->gphimap.p);
         }
@@ -514,6 +526,15 @@ int pdrt_create(const pdrt_grid *grid, const float *density, const pdrt_beam_mod
     const size_t nvox = (size_t)P.nx * P.ny * P.nz;
     if ((s = e->density.ensure(nvox)) != cudaSuccess) return cuda_bail(s, "cudaMalloc(density)");
     if ((s = cudaMemcpy(e->density.p, density, nvox * sizeof(float), cudaMemcpyDefault)) != cudaSuccess) return cuda_bail(s, "cudaMemcpy(density)");
+    {   // broad-beam depth term T(z) = 2 pi (A/a + B/b) at the table nodes (PDRT_DEPTH_FAN)
+        std::vector<float> tt(m->n_z);
+        for (int n = 0; n < m->n_z; ++n)
+            tt[n] = (float)(2.0 * 3.14159265358979323846 * ((double)m->kA[n] / (double)m->ka[n] + (double)m->kB[n] / (double)m->kb[n]));
+        if ((s = e->ttab.ensure(tt.size())) != cudaSuccess) return cuda_bail(s, "cudaMalloc(depth term)");
+        if ((s = cudaMemcpy(e->ttab.p, tt.data(), tt.size() * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_bail(s, "cudaMemcpy(depth term)");
+    }
+    if (m->depth_mode != PDRT_DEPTH_AXIS && m->depth_mode != PDRT_DEPTH_FAN) { fail(e, PDRT_EINVAL, "unknown depth_mode"); return bail(PDRT_EINVAL); }
+    e->depth_mode = m->depth_mode;
     int rc = build_kernel_table(e, m->kernel_size);
     if (rc) return bail(rc);
     *out = e;
@@ -526,6 +547,7 @@ void pdrt_destroy(pdrt_engine *e)
     cudaSetDevice(e->device);
     cudaDeviceSynchronize();
     e->density.release(); e->wtab.release(); e->pool.release(); e->desc.release(); e->tile_base.release();
+    e->ttab.release(); e->fan.release();
     e->sbox.release(); e->wbox.release();
     e->counters.release(); e->phimap.release(); e->P0.release(); e->T1.release(); e->T2.release(); e->T3.release();
     e->Abuf.release(); e->gphimap.release(); e->zrad.release(); e->rho_s.release(); e->Z_s.release();
@@ -543,6 +565,14 @@ int pdrt_set_kernel_size(pdrt_engine *e, int32_t k)
     CU(e, cudaSetDevice(e->device));
     CU(e, cudaDeviceSynchronize());
     return build_kernel_table(e, k);
+}
+
+int pdrt_set_depth_mode(pdrt_engine *e, int32_t mode)
+{
+    if (!e) return fail(nullptr, PDRT_EINVAL, "null engine");
+    if (mode != PDRT_DEPTH_AXIS && mode != PDRT_DEPTH_FAN) return fail(e, PDRT_EINVAL, "unknown depth_mode");
+    e->depth_mode = mode;
+    return PDRT_OK;
 }
 
 int pdrt_get_info(const pdrt_engine *e, pdrt_info *info)
@@ -572,6 +602,8 @@ int pdrt_get_work(pdrt_engine *e, pdrt_work *w)
     w->conv_items = wc.items; w->support_voxels = wc.support_vox; w->footprint_voxels = wc.footprint_vox;
     w->region_voxels = wc.region_vox; w->conv_macs = e->last_backward ? wc.macs_adj : wc.macs_fwd;
     w->kernel_size = e->P.K; w->kernel_size_compiled = e->P.KT;
+    w->fan_rays = e->depth_mode == PDRT_DEPTH_FAN ? wc.fan_rays : 0;
+    w->ray_samples = e->P.M_ray;
     return PDRT_OK;
 }
 
@@ -671,6 +703,18 @@ int pdrt_stage_fluence(pdrt_engine *e, int32_t n_cp, const float *leaves, const 
     return PDRT_OK;
 }
 
+int pdrt_stage_fan_factor(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry, float *factor, void *stream)
+{
+    int rc = check_call(e, n_cp, { leaves, jaws, gantry, factor });
+    if (rc) return rc;
+    if (e->depth_mode != PDRT_DEPTH_FAN) return fail(e, PDRT_EINVAL, "pdrt_stage_fan_factor needs PDRT_DEPTH_FAN");
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = run_setup(e, n_cp, leaves, jaws, gantry, nullptr, true, st))) return rc;
+    k_expand_fan<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, n_cp, e->fan_stride(), e->fan.p, factor);
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+
 int pdrt_stage_depth(pdrt_engine *e, int32_t n_cp, const float *gantry, float *zrad, void *stream)
 {
     int rc = check_call(e, n_cp, { gantry, zrad });
@@ -691,9 +735,11 @@ int pdrt_stage_beam_dose(pdrt_engine *e, const float *leaves, const float *jaws,
     if ((rc = run_setup(e, 1, leaves, jaws, gantry, nullptr, true, st))) return rc;
     CU(e, e->bufA.ensure((size_t)e->P.stride_cp));
     CU(e, e->bufB.ensure((size_t)e->P.stride_cp));
-    k_scan_items<<<1, 256, 0, st>>>(e->desc.p, 0, 1, 0, e->tile_base.p, e->counters.p);
+    k_scan_items<<<1, 256, 0, st>>>(e->desc.p, 0, 1, 0, e->P.Nuf, e->P.Nvf, e->tile_base.p, e->counters.p);
     CU(e, cudaGetLastError());
     k_project<<<dim3(project_blocks(e->P), 1), PROJECT_THREADS, 0, st>>>(e->P, e->desc.p, e->sbox.p, 0, 1, e->phimapT.p, e->bufB.p);
+    if (e->depth_mode == PDRT_DEPTH_FAN)
+        k_apply_fan<<<dim3(4, 1), 256, 0, st>>>(e->P, e->desc.p, e->sbox.p, 0, 1, e->fan_stride(), e->fan.p, e->bufB.p);
     CU(e, cudaGetLastError());
     if ((rc = launch_conv<false>(e, 0, 1, e->bufB.p, e->bufA.p, st))) return rc;
     k_expand_dense<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, e->wbox.p, 0, 0, e->bufA.p, db);

@@ -209,16 +209,16 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
 
 // Exclusive prefix of the conv work items over the control points [cp0, cp0+n) and the totals.
 // One block of 256 threads: warp-shuffle scan per 256-entry chunk with a running carry.
-__global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0, int n, int adjoint, int *tile_base, WorkCounters *wc)
+__global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0, int n, int adjoint, int nuf, int nvf, int *tile_base, WorkCounters *wc)
 {
     __shared__ int wsum[8];
-    __shared__ unsigned long long tot[5];
+    __shared__ unsigned long long tot[6];
     __shared__ int carry_s;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid < 5) tot[tid] = 0ull;
+    if (tid < 6) tot[tid] = 0ull;
     if (tid == 0) carry_s = 0;
     __syncthreads();
-    unsigned long long acc[5] = { 0ull, 0ull, 0ull, 0ull, 0ull };
+    unsigned long long acc[6] = { 0ull, 0ull, 0ull, 0ull, 0ull, 0ull };
     for (int c0 = 0; c0 < n; c0 += 256) {
         const int c = c0 + tid;
         int v = 0;
@@ -226,6 +226,8 @@ __global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0,
             const CpDesc &d = desc[cp0 + c];
             v = adjoint ? d.n_items_adj : d.n_items;
             acc[0] += d.support_vox; acc[1] += d.footprint_vox; acc[2] += d.region_vox; acc[3] += d.macs_fwd; acc[4] += d.macs_adj;
+            if (d.a0 <= d.a1)       // rays of the divergent-depth mode: the support bbox grown by one pixel, clipped to the map
+                acc[5] += (unsigned long long)(min(nuf - 1, d.a1 + 1) - max(0, d.a0 - 1) + 1) * (min(nvf - 1, d.b1 + 1) - max(0, d.b0 - 1) + 1);
         }
         int incl = v;
 #pragma unroll
@@ -244,7 +246,7 @@ __global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0,
         __syncthreads();
     }
 #pragma unroll
-    for (int q = 0; q < 5; ++q) {
+    for (int q = 0; q < 6; ++q) {
         unsigned long long v = acc[q];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -254,9 +256,9 @@ __global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0,
     if (tid == 0) {
         tile_base[n] = carry_s;
         tile_base[n + 1] = 0;           // unit counter of the conv launch that follows
-        if (cp0 == 0) { wc->items = 0; wc->support_vox = 0; wc->footprint_vox = 0; wc->region_vox = 0; wc->macs_fwd = 0; wc->macs_adj = 0; }
+        if (cp0 == 0) { wc->items = 0; wc->support_vox = 0; wc->footprint_vox = 0; wc->region_vox = 0; wc->macs_fwd = 0; wc->macs_adj = 0; wc->fan_rays = 0; }
         wc->items += carry_s; wc->support_vox += tot[0]; wc->footprint_vox += tot[1];
-        wc->region_vox += tot[2]; wc->macs_fwd += tot[3]; wc->macs_adj += tot[4];
+        wc->region_vox += tot[2]; wc->macs_fwd += tot[3]; wc->macs_adj += tot[4]; wc->fan_rays += tot[5];
     }
 }
 

@@ -36,6 +36,34 @@ __device__ __forceinline__ double density_at(const Params &P, const float *__res
     return acc;
 }
 
+// The same lookup for the ray bundle of the divergent-depth mode: position, in-box decision and cell index in float64 (the
+// decision a float64 reference takes), interpolation weights and arithmetic in float32.
+__device__ __forceinline__ float density_at_f(const Params &P, const float *__restrict__ rho, double px, double py, double pz)
+{
+    const double p[3] = { px, py, pz };
+    const double o[3] = { (double)P.ox, (double)P.oy, (double)P.oz }, s[3] = { (double)P.sx, (double)P.sy, (double)P.sz };
+    const int N[3] = { P.nx, P.ny, P.nz };
+    int i0[3], i1[3];
+    float t[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (p[a] < o[a] - 0.5 * s[a] || p[a] > o[a] + (N[a] - 0.5) * s[a]) return 0.f;
+        const double f = (p[a] - o[a]) / s[a];
+        const double fl = floor(f);
+        t[a] = (float)(f - fl);
+        i0[a] = min(max((int)fl, 0), N[a] - 1);
+        i1[a] = min(max((int)fl + 1, 0), N[a] - 1);
+    }
+    const float *r00 = rho + ((size_t)i0[2] * P.ny + i0[1]) * P.nx, *r01 = rho + ((size_t)i0[2] * P.ny + i1[1]) * P.nx;
+    const float *r10 = rho + ((size_t)i1[2] * P.ny + i0[1]) * P.nx, *r11 = rho + ((size_t)i1[2] * P.ny + i1[1]) * P.nx;
+    const float a00 = __ldg(r00 + i0[0]) + t[0] * (__ldg(r00 + i1[0]) - __ldg(r00 + i0[0]));
+    const float a01 = __ldg(r01 + i0[0]) + t[0] * (__ldg(r01 + i1[0]) - __ldg(r01 + i0[0]));
+    const float a10 = __ldg(r10 + i0[0]) + t[0] * (__ldg(r10 + i1[0]) - __ldg(r10 + i0[0]));
+    const float a11 = __ldg(r11 + i0[0]) + t[0] * (__ldg(r11 + i1[0]) - __ldg(r11 + i0[0]));
+    const float b0 = a00 + t[1] * (a01 - a00), b1 = a10 + t[1] * (a11 - a10);
+    return b0 + t[2] * (b1 - b0);
+}
+
 // Grid: n_cp blocks.  rho_s [n_cp][M], Z_s [n_cp][M+1] are float64 scratch; zrad [n_cp][Nw] float32.
 __global__ void __launch_bounds__(DEPTH_THREADS)
 k_depth(Params P, int n_cp, const float *__restrict__ rho, const float *__restrict__ gantry_deg,
@@ -131,8 +159,9 @@ k_fan_depth(Params P, const CpDesc *__restrict__ desc, int n_cp, const float *__
     const double srcx = (double)P.isox + (double)P.sid * sn, srcy = (double)P.isoy - (double)P.sid * cs, srcz = (double)P.isoz;
     const double ds = P.ray_step;
     const int M = P.M_ray;
-    // samples before the ray enters the grid's box contribute exact zeros: start at the first sample that can be inside
-    double t_in = 0.0;
+    // samples before the ray enters the grid's box and after it leaves contribute exact zeros: march only the samples
+    // that can be inside (one sample of slack at either end: the per-sample box test decides)
+    double t_in = 0.0, t_out = (double)M * ds;
     {
         const double o[3] = { (double)P.ox, (double)P.oy, (double)P.oz }, sp[3] = { (double)P.sx, (double)P.sy, (double)P.sz };
         const double s0[3] = { srcx, srcy, srcz }, dd[3] = { dx, dy, dz };
@@ -142,10 +171,12 @@ k_fan_depth(Params P, const CpDesc *__restrict__ desc, int n_cp, const float *__
             if (dd[a] != 0.0) {
                 const double t0 = (o[a] - 0.5 * sp[a] - s0[a]) / dd[a], t1 = (o[a] + (N[a] - 0.5) * sp[a] - s0[a]) / dd[a];
                 t_in = fmax(t_in, fmin(t0, t1));
+                t_out = fmin(t_out, fmax(t0, t1));
             }
         }
     }
-    int m = max(0, (int)floor(t_in / ds - 0.5) - 1);          // one sample of slack: the per-sample box test decides
+    int m = max(0, (int)floor(t_in / ds - 0.5) - 1);
+    const int m_end = min(M, (int)ceil(t_out / ds - 0.5) + 2);
     float *out = fan + (size_t)cp * fan_stride + (size_t)rb * fb.bw + ra;
     const size_t kstride = (size_t)fb.bw * fb.bh;
     const float *zc = zrad + (size_t)cp * P.Nw;
@@ -161,9 +192,9 @@ k_fan_depth(Params P, const CpDesc *__restrict__ desc, int n_cp, const float *__
         if (q > 0.0 && (int)floor(q) >= m) break;
         emit(k, 0.0);
     }
-    for (; m < M && k < P.Nw; ++m) {
+    for (; m < m_end && k < P.Nw; ++m) {
         const double t = (m + 0.5) * ds;
-        const double v = density_at(P, rho, srcx + t * dx, srcy + t * dy, srcz + t * dz);
+        const double v = (double)density_at_f(P, rho, srcx + t * dx, srcy + t * dy, srcz + t * dz);
         for (; k < P.Nw; ++k) {                                // slices whose depth falls into this step
             const double q = ((double)P.sid + (double)P.wmin + k * (double)P.dw) / ds;
             const int m0 = min((int)floor(q), M - 1);
@@ -176,7 +207,7 @@ k_fan_depth(Params P, const CpDesc *__restrict__ desc, int n_cp, const float *__
 }
 
 // Multiplies vol (Phivol over S_k, forward; H_b over S_k, adjoint) by the bilinear interpolant (indices clamped to the ray
-// box) of the depth factor at the voxel's sampling position (fa, fb) of Eq. 5.  Grid: (X, n_cp); a warp per (slice, row).
+// box) of the depth factor at the voxel's sampling position (fa, fb) of Eq. 5.  Grid: (X, n_cp); a warp per (slice, row) unit.
 __global__ void __launch_bounds__(256)
 k_apply_fan(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp, size_t fan_stride,
             const float *__restrict__ fan, float *__restrict__ vol)
@@ -190,27 +221,26 @@ k_apply_fan(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restr
     const int lane = threadIdx.x & 31;
     const int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
     float *vc = vol + (size_t)slot * (size_t)P.stride_cp;
-    for (int k = 0; k < P.Nw; ++k) {
+    for (int q = warp0; q < P.Nw * d.pu; q += n_warps) {           // (slice, row) units of the control point's region
+        const int k = q / d.pu, i = d.ri0 + (q - k * d.pu);
         const SliceBox16 S = load_box(sbox, (size_t)cp * P.Nw + k);
-        if (S.u0 > S.u1) continue;
+        if (S.u0 > S.u1 || i < S.u0 || i > S.u1) continue;
         const float mag = P.sid / (P.sid + P.wmin + k * P.dw);
         const float su = mag * P.du / P.Du, sv = mag / P.Dv;
         const float *Fk = fan + (size_t)cp * fan_stride + (size_t)k * fb.bw * fb.bh;
-        for (int i = S.u0 + warp0; i <= S.u1; i += n_warps) {
-            const float fa = (i - P.cu) * su + P.cuf - (float)fb.a0;
-            const float fla = floorf(fa);
-            const float ta = fa - fla;
-            const int a0 = min(max((int)fla, 0), fb.bw - 1), a1 = min(max((int)fla + 1, 0), fb.bw - 1);
-            float *row = vc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
-            for (int j = S.v0 + lane; j <= S.v1; j += 32) {
-                const float fbv = (P.v0 + j * P.dv) * sv + P.cvf - (float)fb.b0;
-                const float flb = floorf(fbv);
-                const float tb = fbv - flb;
-                const int b0 = min(max((int)flb, 0), fb.bh - 1), b1 = min(max((int)flb + 1, 0), fb.bh - 1);
-                const float f = (1.f - tb) * ((1.f - ta) * __ldg(Fk + b0 * fb.bw + a0) + ta * __ldg(Fk + b0 * fb.bw + a1)) +
-                                tb * ((1.f - ta) * __ldg(Fk + b1 * fb.bw + a0) + ta * __ldg(Fk + b1 * fb.bw + a1));
-                row[j] *= f;
-            }
+        const float fa = (i - P.cu) * su + P.cuf - (float)fb.a0;
+        const float fla = floorf(fa);
+        const float ta = fa - fla;
+        const int a0 = min(max((int)fla, 0), fb.bw - 1), a1 = min(max((int)fla + 1, 0), fb.bw - 1);
+        float *row = vc + ((size_t)k * d.pu + (i - d.ri0)) * d.pv - d.rj0;
+        for (int j = S.v0 + lane; j <= S.v1; j += 32) {
+            const float fbv = (P.v0 + j * P.dv) * sv + P.cvf - (float)fb.b0;
+            const float flb = floorf(fbv);
+            const float tb = fbv - flb;
+            const int b0 = min(max((int)flb, 0), fb.bh - 1), b1 = min(max((int)flb + 1, 0), fb.bh - 1);
+            const float f = (1.f - tb) * ((1.f - ta) * __ldg(Fk + b0 * fb.bw + a0) + ta * __ldg(Fk + b0 * fb.bw + a1)) +
+                            tb * ((1.f - ta) * __ldg(Fk + b1 * fb.bw + a0) + ta * __ldg(Fk + b1 * fb.bw + a1));
+            row[j] *= f;
         }
     }
 }

@@ -326,7 +326,7 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
             StageTimer t(e, PDRT_STAGE_PROJECT, st);
             k_project<<<dim3(project_blocks(e->P), n), PROJECT_THREADS, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->phimapT.p, e->bufB.p);
             if (e->depth_mode == PDRT_DEPTH_FAN)
-                k_apply_fan<<<dim3(4, n), 256, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->fan_stride(), e->fan.p, e->bufB.p);
+                k_apply_fan<<<dim3(32, n), 256, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->fan_stride(), e->fan.p, e->bufB.p);
         }
         CU(e, cudaGetLastError());
         {
@@ -391,7 +391,7 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
         {
             StageTimer t(e, PDRT_STAGE_PROJECT_ADJ, st);
             if (e->depth_mode == PDRT_DEPTH_FAN)      // the factor is a fixed diagonal weighting: the transpose applies it to H_b
-                k_apply_fan<<<dim3(4, n), 256, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->fan_stride(), e->fan.p, e->bufA.p);
+                k_apply_fan<<<dim3(32, n), 256, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->fan_stride(), e->fan.p, e->bufA.p);
             k_project_adjoint<<<dim3(PA_CLUSTER * ((e->P.Nvf + 31) / 32), n), PA_THREADS, sizeof(float) * 32 * (size_t)e->P.Nuf * e->pa_warps, st>>>(
                 e->P, e->desc.p, e->sbox.p, cp0, n, e->pa_warps, e->bufA.p, e->gphimap.p);
         }
@@ -739,7 +739,7 @@ int pdrt_stage_beam_dose(pdrt_engine *e, const float *leaves, const float *jaws,
     CU(e, cudaGetLastError());
     k_project<<<dim3(project_blocks(e->P), 1), PROJECT_THREADS, 0, st>>>(e->P, e->desc.p, e->sbox.p, 0, 1, e->phimapT.p, e->bufB.p);
     if (e->depth_mode == PDRT_DEPTH_FAN)
-        k_apply_fan<<<dim3(4, 1), 256, 0, st>>>(e->P, e->desc.p, e->sbox.p, 0, 1, e->fan_stride(), e->fan.p, e->bufB.p);
+        k_apply_fan<<<dim3(32, 1), 256, 0, st>>>(e->P, e->desc.p, e->sbox.p, 0, 1, e->fan_stride(), e->fan.p, e->bufB.p);
     CU(e, cudaGetLastError());
     if ((rc = launch_conv<false>(e, 0, 1, e->bufB.p, e->bufA.p, st))) return rc;
     k_expand_dense<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, e->wbox.p, 0, 0, e->bufA.p, db);

@@ -310,6 +310,31 @@ class Oracle:
                                        C.c_int(n_cp), _p(lv), _p(jw), _p(ga), _p(mu), g.ctypes.data_as(C.c_void_p), _p(dl), _p(dj), _p(dm))
         return dl, dj, dm
 
+    # ---- collimator rotation
+    def rotate_map(self, coll_deg, Phimap, transpose=False):
+        P = _d(Phimap)
+        out = np.zeros(self.flu_shape)
+        fn = self.lib.orc_rotate_map_adjoint if transpose else self.lib.orc_rotate_map
+        fn(C.byref(self.M), C.c_double(float(coll_deg)), _p(P), _p(out))
+        return out
+
+    def dose_coll(self, leaves, jaws, gantry_deg, coll_deg, mu):
+        n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)
+        co = _d(coll_deg)
+        out = np.zeros(self.dose_shape)
+        self.lib.orc_dose_coll(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), _p(self._w_tab()), C.c_int(n_cp),
+                               _p(lv), _p(jw), _p(ga), _p(co), _p(mu), _p(out))
+        return out
+
+    def dose_backward_coll(self, leaves, jaws, gantry_deg, coll_deg, mu, gdose):
+        n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)
+        co = _d(coll_deg)
+        g = np.ascontiguousarray(gdose, dtype=np.float32)
+        dl, dj, dm = np.zeros_like(lv), np.zeros_like(jw), np.zeros_like(mu)
+        self.lib.orc_dose_backward_coll(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), _p(self._w_tab()),
+                                        C.c_int(n_cp), _p(lv), _p(jw), _p(ga), _p(co), _p(mu), g.ctypes.data_as(C.c_void_p), _p(dl), _p(dj), _p(dm))
+        return dl, dj, dm
+
     def dose_at(self, leaves, jaws, gantry_deg, mu, ijk):
         """Dose at selected voxels; ijk is [n][3] = (x index, y index, z index)."""
         n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)

@@ -914,3 +914,86 @@ void orc_dose_backward_fan(const orc_grid *g, const orc_model *m, const float *r
     }
     free(G); free(H); free(z); free(Phimap); free(gPhimap); free(zf); free(F);
 }
+
+/* ================================================================== collimator rotation */
+/* "For non-zero collimator angles, the fluence map is rotated in the beam's eye view about the beam central
+ * axis ... applied prior to ray-based projection."  Reading G25: the aperture point (uf, vf) of the collimator
+ * frame appears at R(phi_c) (uf, vf) in the beam frame, R the counter-clockwise rotation in the (u, v) plane; the rotated
+ * map is the bilinear_0 resampling of the collimator-frame map on the same pixel grid:
+ *     Phirot[b][a] = bilinear_0(Phimap; R(-phi_c) (uf_a, vf_b) / (Du, Dv) + centre).                                   */
+void orc_rotate_map(const orc_model *m, double coll_deg, const double *Phimap, double *Phirot)
+{
+    const int nu = m->flu_nu, nv = m->flu_nv;
+    const double phi = coll_deg * ORC_PI / 180.0, c = cos(phi), s = sin(phi);
+    for (int b = 0; b < nv; ++b)
+        for (int a = 0; a < nu; ++a) {
+            double u = flu_u(m, a), v = flu_v(m, b);
+            double uc = c * u + s * v, vc = -s * u + c * v;                 /* R(-phi_c) (u, v) */
+            Phirot[(size_t)b * nu + a] = bilinear0(Phimap, nu, nv, uc / m->flu_du + 0.5 * (nu - 1), vc / m->flu_dv + 0.5 * (nv - 1));
+        }
+}
+/* Transpose of orc_rotate_map, written as the scatter that mirrors it. */
+void orc_rotate_map_adjoint(const orc_model *m, double coll_deg, const double *gPhirot, double *gPhimap)
+{
+    const int nu = m->flu_nu, nv = m->flu_nv;
+    const double phi = coll_deg * ORC_PI / 180.0, c = cos(phi), s = sin(phi);
+    memset(gPhimap, 0, sizeof(double) * (size_t)nu * nv);
+    for (int b = 0; b < nv; ++b)
+        for (int a = 0; a < nu; ++a) {
+            double u = flu_u(m, a), v = flu_v(m, b);
+            double f0 = (c * u + s * v) / m->flu_du + 0.5 * (nu - 1), f1 = (-s * u + c * v) / m->flu_dv + 0.5 * (nv - 1);
+            int i0 = (int)floor(f0), i1 = (int)floor(f1);
+            double t0 = f0 - i0, t1 = f1 - i1;
+            for (int q = 0; q < 4; ++q) {
+                int x = i0 + (q & 1), y = i1 + (q >> 1);
+                if (x < 0 || x >= nu || y < 0 || y >= nv) continue;
+                gPhimap[(size_t)y * nu + x] += ((q & 1) ? t0 : 1.0 - t0) * ((q >> 1) ? t1 : 1.0 - t1) * gPhirot[(size_t)b * nu + a];
+            }
+        }
+}
+/* Whole path with per-control-point collimator angles (coll_deg[n_cp]): as orc_dose / orc_dose_backward with the map
+ * rotated between the fluence layer and the projection. */
+void orc_dose_coll(const orc_grid *g, const orc_model *m, const float *rho, const double *W_tab, int n_cp,
+                   const double *leaves, const double *jaws, const double *gantry_deg, const double *coll_deg, const double *mu, double *dose)
+{
+    const size_t nb = (size_t)m->beam_nu * g->nz * m->beam_nw, np = (size_t)g->nx * g->ny * g->nz, nf = (size_t)m->flu_nu * m->flu_nv;
+    double *Db = malloc(sizeof(double) * nb), *Phivol = malloc(sizeof(double) * nb);
+    double *Phimap = malloc(sizeof(double) * nf), *Phirot = malloc(sizeof(double) * nf), *z = malloc(sizeof(double) * m->beam_nw);
+    memset(dose, 0, sizeof(double) * np);
+    for (int b = 0; b < n_cp; ++b) {
+        orc_fluence(m, leaves + (size_t)b * 2 * m->n_pairs, jaws + (size_t)b * 4, NULL, NULL, NULL, Phimap);
+        orc_rotate_map(m, coll_deg[b], Phimap, Phirot);
+        orc_radiological_depth(g, rho, m, gantry_deg[b], z);
+        orc_project(g, m, Phirot, Phivol);
+        orc_convolve(g, m, W_tab, z, Phivol, Db);
+        orc_resample_add(g, m, gantry_deg[b], m->cal * mu[b], Db, dose);
+    }
+    free(Db); free(Phivol); free(Phimap); free(Phirot); free(z);
+}
+void orc_dose_backward_coll(const orc_grid *g, const orc_model *m, const float *rho, const double *W_tab, int n_cp,
+                            const double *leaves, const double *jaws, const double *gantry_deg, const double *coll_deg, const double *mu,
+                            const float *gdose, double *d_leaves, double *d_jaws, double *d_mu)
+{
+    const size_t nb = (size_t)m->beam_nu * g->nz * m->beam_nw, nf = (size_t)m->flu_nu * m->flu_nv;
+    const int np = m->n_pairs;
+    double *G = malloc(sizeof(double) * nb), *H = malloc(sizeof(double) * nb), *z = malloc(sizeof(double) * m->beam_nw);
+    double *Phimap = malloc(sizeof(double) * nf), *Phirot = malloc(sizeof(double) * nf);
+    double *gPhirot = malloc(sizeof(double) * nf), *gPhimap = malloc(sizeof(double) * nf);
+    for (int b = 0; b < n_cp; ++b) {
+        const double *lv = leaves + (size_t)b * 2 * np, *jw = jaws + (size_t)b * 4;
+        orc_fluence(m, lv, jw, NULL, NULL, NULL, Phimap);
+        orc_rotate_map(m, coll_deg[b], Phimap, Phirot);
+        orc_radiological_depth(g, rho, m, gantry_deg[b], z);
+        orc_resample_adjoint(g, m, gantry_deg[b], gdose, G);
+        orc_convolve_adjoint(g, m, W_tab, z, G, H);
+        orc_project_adjoint(g, m, H, gPhirot);
+        double dot = 0.0;
+        for (size_t e = 0; e < nf; ++e) dot += Phirot[e] * gPhirot[e];
+        d_mu[b] = m->cal * dot;
+        orc_rotate_map_adjoint(m, coll_deg[b], gPhirot, gPhimap);
+        orc_fluence_adjoint(m, lv, jw, gPhimap, d_leaves + (size_t)b * 2 * np, d_jaws + (size_t)b * 4);
+        for (int e = 0; e < 2 * np; ++e) d_leaves[(size_t)b * 2 * np + e] *= m->cal * mu[b];
+        for (int e = 0; e < 4; ++e) d_jaws[(size_t)b * 4 + e] *= m->cal * mu[b];
+    }
+    free(G); free(H); free(z); free(Phimap); free(Phirot); free(gPhirot); free(gPhimap);
+}

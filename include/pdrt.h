@@ -162,6 +162,13 @@ PDRT_API int pdrt_set_kernel_size(pdrt_engine *engine, int32_t kernel_size);
 /* Switches the radiological-depth mode (PDRT_DEPTH_AXIS / PDRT_DEPTH_FAN) for subsequent calls. */
 PDRT_API int pdrt_set_depth_mode(pdrt_engine *engine, int32_t depth_mode);
 
+/* Collimator rotation (reading G25).  coll_deg [n_cp] (host or device
+ * pointer; copied on `cuda_stream`) are per-control-point collimator angles for subsequent pdrt_dose / pdrt_dose_backward
+ * calls with the same n_cp: the aperture point (uf, vf) appears at R(phi_c)(uf, vf) in the beam frame (counter-clockwise in
+ * the (u, v) plane); the fluence map is resampled (bilinear, zero outside) on its own grid after the rotation and before
+ * the projection.  n_cp = 0 removes the angles (the default: no rotation).  No gradient w.r.t. the angle is returned. */
+PDRT_API int pdrt_set_collimator(pdrt_engine *engine, int32_t n_cp, const float *coll_deg, void *cuda_stream);
+
 PDRT_API int pdrt_get_info(const pdrt_engine *engine, pdrt_info *info);
 PDRT_API int pdrt_get_work(pdrt_engine *engine, pdrt_work *work);
 
@@ -220,7 +227,8 @@ PDRT_API int pdrt_dose_backward_host(pdrt_engine *engine, int32_t n_cp,
 
 /* Stage taps for parity tests (device pointers, outputs overwritten; they run the same kernels
  * as pdrt_dose / pdrt_dose_backward and copy an intermediate out):
- *   pdrt_stage_fluence   S1: fluence maps            phimap_dev [n_cp][flu_nv][flu_nu]
+ *   pdrt_stage_fluence   S1: fluence maps (as they enter the projection: after the collimator rotation, if any)
+ *                                                    phimap_dev [n_cp][flu_nv][flu_nu]
  *   pdrt_stage_depth     S2: radiological depths     zrad_dev   [n_cp][beam_nw]
  *   pdrt_stage_beam_dose S3-S5: beam-frame dose D_b of ONE control point, dense
  *                                                    db_dev     [beam_nw][beam_nv][beam_nu]

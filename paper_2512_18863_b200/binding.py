@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpdrt.so")
 
 SYMBOLS = ("pdrt_create", "pdrt_destroy", "pdrt_last_error", "pdrt_set_kernel_size", "pdrt_get_info", "pdrt_get_work",
-           "pdrt_set_profiling", "pdrt_get_stage_ms", "pdrt_set_depth_mode", "pdrt_stage_fan_factor",
+           "pdrt_set_profiling", "pdrt_get_stage_ms", "pdrt_set_depth_mode", "pdrt_stage_fan_factor", "pdrt_set_collimator",
            "pdrt_dose", "pdrt_dose_backward", "pdrt_dose_host", "pdrt_dose_backward_host",
            "pdrt_stage_fluence", "pdrt_stage_depth", "pdrt_stage_beam_dose", "pdrt_stage_grad_fluence",
            "pdrt_mu_epsilon", "pdrt_validate", "pdrt_validate_backward", "pdrt_objective", "pdrt_track_jaws", "pdrt_plan_step")
@@ -95,6 +95,7 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.pdrt_last_error.restype = C.c_char_p
     lib.pdrt_set_kernel_size.argtypes = [vp, i32]
     lib.pdrt_set_depth_mode.argtypes = [vp, i32]
+    lib.pdrt_set_collimator.argtypes = [vp, i32, vp, vp]
     lib.pdrt_stage_fan_factor.argtypes = [vp, i32, vp, vp, vp, vp, vp]
     lib.pdrt_get_info.argtypes = [vp, C.POINTER(PdrtInfo)]
     lib.pdrt_get_work.argtypes = [vp, C.POINTER(PdrtWork)]
@@ -230,6 +231,14 @@ class Engine:
     def set_depth_mode(self, mode: int):
         """0 = central-axis ray (the paper's mode), 1 = one diverging ray per fluence-map pixel (PDRT_DEPTH_FAN)."""
         self._check(self.lib.pdrt_set_depth_mode(self.handle, int(mode)))
+
+    def set_collimator(self, coll_deg):
+        """Per-control-point collimator angles [n_cp] for subsequent calls (None removes them)."""
+        if coll_deg is None:
+            self._check(self.lib.pdrt_set_collimator(self.handle, 0, None, self._stream()))
+            return
+        co = self._dev(coll_deg)
+        self._check(self.lib.pdrt_set_collimator(self.handle, int(co.shape[0]), co.data_ptr(), self._stream()))
 
     def stage_fan_factor(self, leaves, jaws, gantry_deg):
         ga = self._dev(gantry_deg)

@@ -81,11 +81,11 @@ k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restric
     const float *pm = phimapT + (size_t)cp * P.Nuf * P.Nvf;
     float *vc = vol + (size_t)slot * (size_t)P.stride_cp;
     __shared__ float map_s[PROJECT_MAP_FLOATS];              // [a - a0][b - b0], b fastest
-    const int bw = d.a1 - d.a0 + 1, bh = d.b1 - d.b0 + 1;
+    const int bw = d.pa1 - d.pa0 + 1, bh = d.pb1 - d.pb0 + 1;
     const bool staged = bw * bh <= PROJECT_MAP_FLOATS;
     if (staged) {
         for (int a = threadIdx.x >> 5; a < bw; a += PROJECT_THREADS / 32)
-            for (int b = threadIdx.x & 31; b < bh; b += 32) map_s[a * bh + b] = __ldg(pm + (d.a0 + a) * P.Nvf + d.b0 + b);
+            for (int b = threadIdx.x & 31; b < bh; b += 32) map_s[a * bh + b] = __ldg(pm + (d.pa0 + a) * P.Nvf + d.pb0 + b);
     }
     __syncthreads();
     // quads per row of the widest slice: S_k grows with the distance from the source, and its first column may round down
@@ -115,14 +115,14 @@ k_project(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restric
                 const int b = (int)flb;
                 const float tb = fb - flb;
                 const bool jgrid = j < P.Nv;
-                const bool v0 = jgrid && b >= d.b0 && b <= d.b1, v1 = jgrid && b + 1 >= d.b0 && b + 1 <= d.b1;
+                const bool v0 = jgrid && b >= d.pb0 && b <= d.pb1, v1 = jgrid && b + 1 >= d.pb0 && b + 1 <= d.pb1;
                 wb0[e] = v0 ? m2 * (1.f - tb) : 0.f; wb1[e] = v1 ? m2 * tb : 0.f;
-                ib0[e] = v0 ? b : (v1 ? b + 1 : d.b0); ib1[e] = v1 ? b + 1 : ib0[e];
+                ib0[e] = v0 ? b : (v1 ? b + 1 : d.pb0); ib1[e] = v1 ? b + 1 : ib0[e];
             }
             auto row_T = [&](int a, float (&T)[4]) {            // T[a][quad]; zero outside the support bbox
-                if (a >= d.a0 && a <= d.a1) {
+                if (a >= d.pa0 && a <= d.pa1) {
                     if (staged) {
-                        const float *pc = map_s + (a - d.a0) * bh - d.b0;
+                        const float *pc = map_s + (a - d.pa0) * bh - d.pb0;
 #pragma unroll
                         for (int e = 0; e < 4; ++e) T[e] = wb0[e] * pc[ib0[e]] + wb1[e] * pc[ib1[e]];
                     } else {

@@ -124,8 +124,8 @@ struct FanBox { int a0, b0, bw, bh; };     // pixels [a0, a0+bw) x [b0, b0+bh) o
 __device__ __forceinline__ FanBox fan_box(const Params &P, const CpDesc &d)
 {
     FanBox f;
-    f.a0 = max(0, d.a0 - 1); f.b0 = max(0, d.b0 - 1);
-    f.bw = min(P.Nuf - 1, d.a1 + 1) - f.a0 + 1; f.bh = min(P.Nvf - 1, d.b1 + 1) - f.b0 + 1;
+    f.a0 = max(0, d.pa0 - 1); f.b0 = max(0, d.pb0 - 1);
+    f.bw = min(P.Nuf - 1, d.pa1 + 1) - f.a0 + 1; f.bh = min(P.Nvf - 1, d.pb1 + 1) - f.b0 + 1;
     return f;
 }
 __device__ __forceinline__ float depth_term(const float *__restrict__ Ttab, int n_z, float dz, float z)

@@ -73,12 +73,14 @@ struct FluTables {
 struct CpDesc {
     float cg, sg;                // cos / sin of the gantry angle
     float scale;                 // cal * MU
-    int a0, a1, b0, b1;          // fluence support bbox (inclusive); empty when a0 > a1
+    int a0, a1, b0, b1;          // fluence support bbox in the COLLIMATOR frame (inclusive); empty when a0 > a1
+    int pa0, pa1, pb0, pb1;      // the same in the PROJECTION frame (after the collimator rotation; equal to a0.. when the angle is 0):
+                                 // what S3 / S9 and every slice box are derived from
+    float cc, sc;                // cos / sin of the collimator angle
     int ja0, ja1, jb0, jb1;      // jaw bbox (pixels where Phi0 or its jaw derivative can be non-zero)
     int ri0, rj0, pu, pv;        // compact region origin and extents (rj0 % 8 == 0, pv % 8 == 0, pu % RS == 0)
     int ntf, nts;                // region size in thread-tiles: RF along v (fast), RS along u (slow)
     int ncf, ntfc;               // conv chunks along v and their width [thread-tiles]
-    int nuc_fwd, nuc_adj;        // (reserved)
     int n_items, n_items_adj;    // Nw * ncf conv work items, forward / adjoint (0 when empty)
     unsigned long long support_vox, footprint_vox, region_vox, macs_fwd, macs_adj;
 };
@@ -113,13 +115,13 @@ __device__ __forceinline__ SliceBox16 load_box(const SliceBox16 *__restrict__ t,
 __device__ __forceinline__ bool box_empty(const SliceBox &b) { return b.u0 > b.u1 || b.v0 > b.v1; }
 
 // S_k: beam voxels of slice k whose bilinear stencil (Eq. 5) can touch a pixel of the fluence
-// support bbox, i.e. fa in (a0-1, a1+1), fb in (b0-1, b1+1); rounded outward, clipped to the grid.
+// support bbox (projection frame), i.e. fa in (pa0-1, pa1+1), fb in (pb0-1, pb1+1); rounded outward, clipped to the grid.
 // Every kernel derives its per-slice extents from this one function.
 __device__ __forceinline__ SliceBox slice_support(const Params &P, const CpDesc &d, int k)
 {
     const float inv_mag = (P.sid + P.wmin + k * P.dw) / P.sid;
-    const float ulo = (d.a0 - 1 - P.cuf) * P.Du * inv_mag, uhi = (d.a1 + 1 - P.cuf) * P.Du * inv_mag;
-    const float vlo = (d.b0 - 1 - P.cvf) * P.Dv * inv_mag, vhi = (d.b1 + 1 - P.cvf) * P.Dv * inv_mag;
+    const float ulo = (d.pa0 - 1 - P.cuf) * P.Du * inv_mag, uhi = (d.pa1 + 1 - P.cuf) * P.Du * inv_mag;
+    const float vlo = (d.pb0 - 1 - P.cvf) * P.Dv * inv_mag, vhi = (d.pb1 + 1 - P.cvf) * P.Dv * inv_mag;
     SliceBox s;
     s.u0 = max(0, (int)floorf(ulo / P.du + P.cu));
     s.u1 = min(P.Nu - 1, (int)ceilf(uhi / P.du + P.cu));

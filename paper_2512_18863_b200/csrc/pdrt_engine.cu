@@ -95,6 +95,8 @@ struct pdrt_engine {
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
     int conv_per_sm[2][64] = {};      // resident conv blocks per SM on THIS engine's device, by [adjoint][KT]; 0 = not queried yet
+    DevBuf<float> coll;               // collimator angles [coll_n] set by pdrt_set_collimator (coll_n = 0: none)
+    int coll_n = 0;
     int nzp = 0;                      // row pitch of gT: nz rounded up to 4
     int pa_warps = 0;                 // warps of k_project_adjoint that hold a shared-memory plane (0: attribute not set yet)
     // per-stage device timing of the most recent call (CUDA events on the call's stream)
@@ -285,9 +287,10 @@ int run_setup(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, 
 {
     int rc = ensure_cp_scratch(e, n_cp);
     if (rc) return rc;
+    if (e->coll_n != 0 && e->coll_n != n_cp) return fail(e, PDRT_EINVAL, "collimator angles were set for a different number of control points");
     {
         StageTimer t(e, PDRT_STAGE_FLUENCE, st);
-        k_fluence<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, gantry, mu, e->desc.p, e->sbox.p, e->wbox.p,
+        k_fluence<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, gantry, e->coll_n ? e->coll.p : nullptr, mu, e->desc.p, e->sbox.p, e->wbox.p,
                                                e->P0.p, e->T1.p, e->T2.p, e->Abuf.p, e->phimap.p, e->phimapT.p);
     }
     CU(e, cudaGetLastError());
@@ -547,7 +550,7 @@ void pdrt_destroy(pdrt_engine *e)
     cudaSetDevice(e->device);
     cudaDeviceSynchronize();
     e->density.release(); e->wtab.release(); e->pool.release(); e->desc.release(); e->tile_base.release();
-    e->ttab.release(); e->fan.release();
+    e->ttab.release(); e->fan.release(); e->coll.release();
     e->sbox.release(); e->wbox.release();
     e->counters.release(); e->phimap.release(); e->P0.release(); e->T1.release(); e->T2.release(); e->T3.release();
     e->Abuf.release(); e->gphimap.release(); e->zrad.release(); e->rho_s.release(); e->Z_s.release();
@@ -572,6 +575,19 @@ int pdrt_set_depth_mode(pdrt_engine *e, int32_t mode)
     if (!e) return fail(nullptr, PDRT_EINVAL, "null engine");
     if (mode != PDRT_DEPTH_AXIS && mode != PDRT_DEPTH_FAN) return fail(e, PDRT_EINVAL, "unknown depth_mode");
     e->depth_mode = mode;
+    return PDRT_OK;
+}
+
+int pdrt_set_collimator(pdrt_engine *e, int32_t n_cp, const float *coll_deg, void *stream)
+{
+    if (!e) return fail(nullptr, PDRT_EINVAL, "null engine");
+    if (n_cp < 0 || (n_cp > 0 && !coll_deg)) return fail(e, PDRT_EINVAL, "n_cp >= 0 and a pointer when n_cp > 0");
+    CU(e, cudaSetDevice(e->device));
+    if (n_cp > 0) {
+        CU(e, e->coll.ensure(n_cp));
+        CU(e, cudaMemcpyAsync(e->coll.p, coll_deg, sizeof(float) * n_cp, cudaMemcpyDefault, (cudaStream_t)stream));
+    }
+    e->coll_n = n_cp;
     return PDRT_OK;
 }
 

@@ -44,11 +44,14 @@ __device__ __forceinline__ float blur_at(const float *m, const Params &P, const 
 }
 
 // Builds CpDesc: gantry axes, jaw and support bboxes, compact region, conv chunking, work counters.
-__device__ void build_desc(const Params &P, const float *jaws, float gantry_deg, float mu, CpDesc &d)
+__device__ void build_desc(const Params &P, const float *jaws, float gantry_deg, float coll_deg, float mu, CpDesc &d)
 {
     const double phi = (double)gantry_deg * 3.14159265358979323846 / 180.0;
     d.cg = (float)cos(phi);
     d.sg = (float)sin(phi);
+    const double phc = (double)coll_deg * 3.14159265358979323846 / 180.0;
+    d.cc = coll_deg == 0.f ? 1.f : (float)cos(phc);
+    d.sc = coll_deg == 0.f ? 0.f : (float)sin(phc);
     d.scale = P.cal * mu;
     const float x1 = jaws[0], x2 = jaws[1], y1 = jaws[2], y2 = jaws[3];
     const float eu = -0.5f * P.Nuf * P.Du, ev = -0.5f * P.Nvf * P.Dv;     // left edge of pixel 0
@@ -61,14 +64,29 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     d.a0 = max(0, d.ja0 - P.Tu_max); d.a1 = min(P.Nuf - 1, d.ja1 + P.Tu_max);
     d.b0 = max(0, d.jb0 - P.Tv_max); d.b1 = min(P.Nvf - 1, d.jb1 + P.Tv_max);
     d.ri0 = d.rj0 = d.pu = d.pv = d.ntf = d.nts = 0;
-    d.ncf = d.ntfc = d.nuc_fwd = d.nuc_adj = d.n_items = d.n_items_adj = 0;
+    d.ncf = d.ntfc = d.n_items = d.n_items_adj = 0;
     d.support_vox = d.footprint_vox = d.region_vox = d.macs_fwd = d.macs_adj = 0ull;
+    d.pa0 = d.pb0 = 1; d.pa1 = d.pb1 = 0;
     if (empty) { d.a0 = d.ja0 = 1; d.a1 = d.ja1 = 0; d.b0 = d.jb0 = 1; d.b1 = d.jb1 = 0; return; }
+    // support bbox in the projection frame: the collimator-frame box, grown by the one-pixel reach of the bilinear resampling,
+    // rotated by R(phi_c) about the axis; identical when the angle is 0
+    d.pa0 = d.a0; d.pa1 = d.a1; d.pb0 = d.b0; d.pb1 = d.b1;
+    if (d.sc != 0.f || d.cc != 1.f) {
+        float ulo = 1e30f, uhi = -1e30f, vlo = 1e30f, vhi = -1e30f;
+        for (int q = 0; q < 4; ++q) {
+            const float uc = ((q & 1 ? d.a1 + 1 : d.a0 - 1) - P.cuf) * P.Du, vc = ((q & 2 ? d.b1 + 1 : d.b0 - 1) - P.cvf) * P.Dv;
+            const float ur = d.cc * uc - d.sc * vc, vr = d.sc * uc + d.cc * vc;
+            ulo = fminf(ulo, ur); uhi = fmaxf(uhi, ur); vlo = fminf(vlo, vr); vhi = fmaxf(vhi, vr);
+        }
+        d.pa0 = max(0, (int)floorf(ulo / P.Du + P.cuf)); d.pa1 = min(P.Nuf - 1, (int)ceilf(uhi / P.Du + P.cuf));
+        d.pb0 = max(0, (int)floorf(vlo / P.Dv + P.cvf)); d.pb1 = min(P.Nvf - 1, (int)ceilf(vhi / P.Dv + P.cvf));
+        if (d.pa0 > d.pa1 || d.pb0 > d.pb1) { d.a0 = d.ja0 = d.pa0 = 1; d.a1 = d.ja1 = d.pa1 = 0; d.b0 = d.jb0 = d.pb0 = 1; d.b1 = d.jb1 = d.pb1 = 0; return; }
+    }
     const int C = (P.KT - 1) / 2;
     const SliceBox s0 = slice_support(P, d, 0), s1 = slice_support(P, d, P.Nw - 1);
     const int u0 = max(0, min(s0.u0, s1.u0) - C), u1 = min(P.Nu - 1, max(s0.u1, s1.u1) + C);
     const int v0 = max(0, min(s0.v0, s1.v0) - C), v1 = min(P.Nv - 1, max(s0.v1, s1.v1) + C);
-    if (u0 > u1 || v0 > v1) { d.a0 = d.ja0 = 1; d.a1 = d.ja1 = 0; d.b0 = d.jb0 = 1; d.b1 = d.jb1 = 0; return; }
+    if (u0 > u1 || v0 > v1) { d.a0 = d.ja0 = d.pa0 = 1; d.a1 = d.ja1 = d.pa1 = 0; d.b0 = d.jb0 = d.pb0 = 1; d.b1 = d.jb1 = d.pb1 = 0; return; }
     d.ri0 = u0;
     d.pu = ((u1 - u0 + 1) + RS - 1) / RS * RS;
     d.rj0 = v0 & ~7;
@@ -78,7 +96,6 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     d.ncf = (d.ntf + NTFC_MAX - 1) / NTFC_MAX;
     d.ntfc = (d.ntf + d.ncf - 1) / d.ncf;
     // conv work items: one per slice and chunk along v (the warp that takes an item walks its active thread-tiles)
-    d.nuc_fwd = d.nuc_adj = 1;
     d.n_items = d.n_items_adj = P.Nw * d.ncf;
     d.region_vox = (unsigned long long)d.pu * d.pv * P.Nw;
 }
@@ -86,7 +103,7 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
 // S1.  Grid: n_cp blocks.  Scratch maps P0, T1, T2, A are [n_cp][Nvf][Nuf]; phimapT is [n_cp][Nuf][Nvf].
 __global__ void __launch_bounds__(FLU_THREADS)
 k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, const float *__restrict__ jaws,
-          const float *__restrict__ gantry_deg, const float *__restrict__ mu, CpDesc *desc,
+          const float *__restrict__ gantry_deg, const float *__restrict__ coll_deg, const float *__restrict__ mu, CpDesc *desc,
           SliceBox16 *sbox, SliceBox16 *wbox,
           float *P0, float *T1, float *T2, float *Abuf, float *phimap, float *phimapT)
 {
@@ -95,7 +112,7 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
     __shared__ CpDesc d;
     __shared__ unsigned long long cnt[4];
     if (tid == 0) {
-        build_desc(P, jaws + 4 * cp, gantry_deg ? gantry_deg[cp] : 0.f, mu ? mu[cp] : 0.f, d);
+        build_desc(P, jaws + 4 * cp, gantry_deg ? gantry_deg[cp] : 0.f, coll_deg ? coll_deg[cp] : 0.f, mu ? mu[cp] : 0.f, d);
         cnt[0] = cnt[1] = cnt[2] = cnt[3] = 0ull;
     }
     __syncthreads();
@@ -200,9 +217,32 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
         pm[b * P.Nuf + a] *= oar_factor(T, sqrtf(uf * uf + vf * vf));
     }
     __syncthreads();
+    // collimator rotation (G25): the map is resampled (bilinear_0) on its own grid at R(-phi_c) of
+    // each pixel centre; from here on the map lives in the projection frame (bbox pa0..pb1)
+    const int pw = d.pa1 - d.pa0 + 1, ph = d.pb1 - d.pb0 + 1, npp = pw * ph;
+    if (d.sc != 0.f || d.cc != 1.f) {
+        for (int p = tid; p < npp; p += FLU_THREADS) {
+            const int a = d.pa0 + p % pw, b = d.pb0 + p / pw;
+            const float u = flu_u(P, a), v = flu_v(P, b);
+            const float fa = (d.cc * u + d.sc * v) / P.Du + P.cuf, fb = (-d.sc * u + d.cc * v) / P.Dv + P.cvf;
+            const float fla = floorf(fa), flb = floorf(fb);
+            const int ia = (int)fla, ib = (int)flb;
+            const float ta = fa - fla, tb = fb - flb;
+            t1[b * P.Nuf + a] = (1.f - tb) * ((1.f - ta) * at_bbox(pm, P, d, ia, ib) + ta * at_bbox(pm, P, d, ia + 1, ib)) +
+                                tb * ((1.f - ta) * at_bbox(pm, P, d, ia, ib + 1) + ta * at_bbox(pm, P, d, ia + 1, ib + 1));
+        }
+        __syncthreads();
+        for (int p = tid; p < npx; p += FLU_THREADS) pm[(d.b0 + p / bw) * P.Nuf + d.a0 + p % bw] = 0.f;
+        __syncthreads();
+        for (int p = tid; p < npp; p += FLU_THREADS) {
+            const int a = d.pa0 + p % pw, b = d.pb0 + p / pw;
+            pm[b * P.Nuf + a] = t1[b * P.Nuf + a];
+        }
+        __syncthreads();
+    }
     // the same map with v fastest, for the conv tile fill (lanes run along v there)
-    for (int p = tid; p < npx; p += FLU_THREADS) {
-        const int a = d.a0 + p / bh, b = d.b0 + p % bh;
+    for (int p = tid; p < npp; p += FLU_THREADS) {
+        const int a = d.pa0 + p / ph, b = d.pb0 + p % ph;
         pmT[a * P.Nvf + b] = pm[b * P.Nuf + a];
     }
 }
@@ -227,7 +267,7 @@ __global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0,
             v = adjoint ? d.n_items_adj : d.n_items;
             acc[0] += d.support_vox; acc[1] += d.footprint_vox; acc[2] += d.region_vox; acc[3] += d.macs_fwd; acc[4] += d.macs_adj;
             if (d.a0 <= d.a1)       // rays of the divergent-depth mode: the support bbox grown by one pixel, clipped to the map
-                acc[5] += (unsigned long long)(min(nuf - 1, d.a1 + 1) - max(0, d.a0 - 1) + 1) * (min(nvf - 1, d.b1 + 1) - max(0, d.b0 - 1) + 1);
+                acc[5] += (unsigned long long)(min(nuf - 1, d.pa1 + 1) - max(0, d.pa0 - 1) + 1) * (min(nvf - 1, d.pb1 + 1) - max(0, d.pb0 - 1) + 1);
         }
         int incl = v;
 #pragma unroll
@@ -266,7 +306,7 @@ __global__ void __launch_bounds__(256) k_scan_items(const CpDesc *desc, int cp0,
 // zero-padded) Gaussians, the product Phi0 = J (tau + (1-tau) A) and Eq. 4's subgradients.
 // One block per control point; leaf gradients need no reduction (one thread per leaf edge),
 // jaw and MU gradients use warp-shuffle + shared-memory block reductions (no global atomics).
-__global__ void __launch_bounds__(FLU_THREADS)
+__global__ void __launch_bounds__(FLU_THREADS, 2)
 k_fluence_adjoint(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, const float *__restrict__ jaws,
                   const CpDesc *__restrict__ desc, const float *__restrict__ phimap, const float *__restrict__ Abuf,
                   const float *__restrict__ gphimap, float *T1, float *T2, float *T3,
@@ -293,11 +333,38 @@ k_fluence_adjoint(Params P, FluTables T, int n_cp, const float *__restrict__ lea
     const float x1 = jw[0], x2 = jw[1], y1 = jw[2], y2 = jw[3];
     float acc[5] = { 0.f, 0.f, 0.f, 0.f, 0.f };     // d_x1, d_x2, d_y1, d_y2, <Phimap, gPhimap>
 
-    for (int p = tid; p < npx; p += FLU_THREADS) {          // O5 transposed, scaled by cal*MU
+    const bool rotated = d.sc != 0.f || d.cc != 1.f;
+    if (rotated) {      // <Phimap, gPhimap> over the projection-frame bbox (both live in the projection frame)
+        const int pw = d.pa1 - d.pa0 + 1, npp = pw * (d.pb1 - d.pb0 + 1);
+        for (int p = tid; p < npp; p += FLU_THREADS) {
+            const int a = d.pa0 + p % pw, b = d.pb0 + p / pw;
+            acc[4] += pm[b * P.Nuf + a] * gp[b * P.Nuf + a];
+        }
+    }
+    // half-extent, in pixels of the projection frame, of a collimator-frame pixel's hat after the rotation
+    const float hra = (fabsf(d.cc) * P.Du + fabsf(d.sc) * P.Dv) / P.Du, hrb = (fabsf(d.sc) * P.Du + fabsf(d.cc) * P.Dv) / P.Dv;
+    for (int p = tid; p < npx; p += FLU_THREADS) {          // (rotation transposed,) O5 transposed, scaled by cal*MU
         const int a = d.a0 + p % bw, b = d.b0 + p / bw;
         const float uf = flu_u(P, a), vf = flu_v(P, b);
-        const float gv = gp[b * P.Nuf + a];
-        acc[4] += pm[b * P.Nuf + a] * gv;
+        float gv;
+        if (!rotated) {
+            gv = gp[b * P.Nuf + a];
+            acc[4] += pm[b * P.Nuf + a] * gv;
+        } else {
+            // gather form of the transpose: the projection-frame pixels (a', b') whose sample point R(-phi_c)(uf_a', vf_b')
+            // lies within one pixel of (a, b) sit around R(phi_c)(uf_a, vf_b)
+            const float far = (d.cc * uf - d.sc * vf) / P.Du + P.cuf, fbr = (d.sc * uf + d.cc * vf) / P.Dv + P.cvf;
+            const int a_lo = max(d.pa0, (int)ceilf(far - hra)), a_hi = min(d.pa1, (int)floorf(far + hra));
+            const int b_lo = max(d.pb0, (int)ceilf(fbr - hrb)), b_hi = min(d.pb1, (int)floorf(fbr + hrb));
+            gv = 0.f;
+            for (int bb = b_lo; bb <= b_hi; ++bb)
+                for (int aa = a_lo; aa <= a_hi; ++aa) {
+                    const float u = flu_u(P, aa), v = flu_v(P, bb);
+                    const float wa = 1.f - fabsf((d.cc * u + d.sc * v) / P.Du + P.cuf - (float)a);
+                    const float wb = 1.f - fabsf((-d.sc * u + d.cc * v) / P.Dv + P.cvf - (float)b);
+                    if (wa > 0.f && wb > 0.f) gv = fmaf(wa * wb, gp[bb * P.Nuf + aa], gv);
+                }
+        }
         g2[b * P.Nuf + a] = d.scale * gv * oar_factor(T, sqrtf(uf * uf + vf * vf));
     }
     __syncthreads();

@@ -257,16 +257,16 @@ k_project_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *_
     const CpDesc d = desc[cp];
     // every block of a cluster shares (cp, bchunk): the early exits are taken by the whole cluster
     if (d.a0 > d.a1) return;
-    const int B0 = d.b0 + 32 * bchunk;
-    if (B0 > d.b1) return;
-    const int bw = d.a1 - d.a0 + 1;
+    const int B0 = d.pb0 + 32 * bchunk;
+    if (B0 > d.pb1) return;
+    const int bw = d.pa1 - d.pa0 + 1;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     float *plane = pa_smem + (size_t)min(warp, n_act - 1) * bw * 32;
     if (warp < n_act)
         for (int e = lane; e < bw * 32; e += 32) plane[e] = 0.f;
     __syncwarp();
     const int b = B0 + lane;
-    const bool live = b <= d.b1;
+    const bool live = b <= d.pb1;
     const float *Hc = H + (size_t)slot * (size_t)P.stride_cp;
     const float vb = P.v0 / P.dv;                       // v_j / dv = vb + j
     for (int k = warp < n_act ? crank * n_act + warp : P.Nw; k < P.Nw; k += PA_CLUSTER * n_act) {
@@ -331,15 +331,15 @@ k_project_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *_
                 const int a0 = (int)fla;
                 const float ta = fa - fla;
                 while (a_cur < a0) {                      // column a_cur is complete (a(i) never decreases): warp-uniform
-                    if (a_cur >= d.a0 && a_cur <= d.a1) plane[(a_cur - d.a0) * 32 + lane] += acc_lo;
+                    if (a_cur >= d.pa0 && a_cur <= d.pa1) plane[(a_cur - d.pa0) * 32 + lane] += acc_lo;
                     acc_lo = acc_hi; acc_hi = 0.f; ++a_cur;
                 }
                 acc_lo = fmaf(1.f - ta, t[r], acc_lo);
                 acc_hi = fmaf(ta, t[r], acc_hi);
             }
         }
-        if (a_cur >= d.a0 && a_cur <= d.a1) plane[(a_cur - d.a0) * 32 + lane] += acc_lo;
-        if (a_cur + 1 >= d.a0 && a_cur + 1 <= d.a1) plane[(a_cur + 1 - d.a0) * 32 + lane] += acc_hi;
+        if (a_cur >= d.pa0 && a_cur <= d.pa1) plane[(a_cur - d.pa0) * 32 + lane] += acc_lo;
+        if (a_cur + 1 >= d.pa0 && a_cur + 1 <= d.pa1) plane[(a_cur + 1 - d.pa0) * 32 + lane] += acc_hi;
     }
     __syncthreads();
     // the block's warps, in warp order, into plane 0
@@ -358,7 +358,7 @@ k_project_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *_
         float s = 0.f;
 #pragma unroll
         for (int q = 0; q < PA_CLUSTER; ++q) s += remote[q][a * 32 + bl];
-        if (B0 + bl <= d.b1) gphimap[((size_t)cp * P.Nvf + B0 + bl) * P.Nuf + d.a0 + a] = s;
+        if (B0 + bl <= d.pb1) gphimap[((size_t)cp * P.Nvf + B0 + bl) * P.Nuf + d.pa0 + a] = s;
     }
     cluster.sync();                                      // nobody leaves while its shared memory is still being read
 }

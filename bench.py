@@ -514,7 +514,7 @@ def run_ours(args):
     sweep = None
     if args.sweep and world == 1:
         sweep = {}
-        for k in wl.kernel_sizes:
+        for k in ([int(x) for x in args.sweep_sizes.split(",")] if args.sweep_sizes else wl.kernel_sizes):
             eng.set_kernel_size(k)
             for _ in range(2):
                 step()
@@ -526,7 +526,8 @@ def run_ours(args):
                 a.record(); forward(); b.record(); backward(); c.record()
                 torch.cuda.synchronize()
                 ts.append((a.elapsed_time(b), b.elapsed_time(c)))
-            sweep[str(k)] = dict(forward_ms=round(float(np.median([x[0] for x in ts])), 4), backward_ms=round(float(np.median([x[1] for x in ts])), 4))
+            sweep[str(k)] = dict(forward_ms=round(float(np.median([x[0] for x in ts])), 4), backward_ms=round(float(np.median([x[1] for x in ts])), 4),
+                                 passes=eng.info.kernel_passes, pass_size=eng.info.kernel_size_compiled)
         eng.set_kernel_size(wl.model["kernel_size"])
 
     if rank == 0:
@@ -560,6 +561,7 @@ def main():
     ap.add_argument("--workload", default="c4", choices=("c3", "c4", "c5"))
     ap.add_argument("--kernel-size", type=int, default=0)
     ap.add_argument("--sweep", action="store_true", help="also time the kernel-size sweep of the workload")
+    ap.add_argument("--sweep-sizes", default="", help="comma-separated kernel sizes for --sweep (default: the workload's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--depth-mode", default="axis", choices=("axis", "fan"), help="fan: one diverging ray per fluence-map pixel (NEXT-1)")
     ap.add_argument("--single-pass", action="store_true", help="c5: time one forward+backward instead of the 20-iteration planning loop")

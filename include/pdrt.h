@@ -100,7 +100,7 @@ typedef struct {
     const float *oar;                    /* n_oar factors at r = n * oar_dr_mm, clamped at the last entry */
     int32_t n_z; float dz_mm;            /* kernel parameters tabulated at radiological depth z = n * dz  */
     const float *kA, *ka, *kB, *kb;      /* n_z each: K(r;z) = (A e^{-a r} + B e^{-b r}) / r */
-    int32_t kernel_size;                 /* lateral kernel size in beam-grid pixels: odd, 3..63           */
+    int32_t kernel_size;                 /* lateral kernel size in beam-grid pixels: odd, 3..255          */
     float   cal;                         /* global dose scale (PAPER.md:178 energy scaling factor)        */
     int32_t beam_nu, beam_nw;            /* beam grid; beam_nu == 0 selects the default grid as a whole:  */
     float   beam_du, beam_dw, beam_wmin; /*   Nu = nx, Nw = ny, du = dw = sx, wmin = -(Nw-1)/2 * dw       */
@@ -123,11 +123,12 @@ typedef struct {
     float   beam_du, beam_dv, beam_dw, beam_wmin;
     int32_t flu_nu, flu_nv, n_pairs;
     int32_t kernel_size;                 /* as requested                                      */
-    int32_t kernel_size_compiled;        /* smallest compiled conv variant >= kernel_size     */
+    int32_t kernel_size_compiled;        /* compiled conv variant of one pass (single pass: >= kernel_size) */
     float   ray_step_mm;
     int32_t ray_samples;                 /* samples per central-axis ray                      */
     int32_t sm_count;
     uint64_t scratch_bytes;              /* device scratch currently held                     */
+    int32_t kernel_passes;               /* conv passes per slice: 1, or NB^2 sub-kernels for kernel sizes above 55 */
 } pdrt_info;
 
 /* Work counters of the most recent pdrt_dose / pdrt_dose_backward (device-counted from the actual
@@ -155,7 +156,8 @@ PDRT_API void pdrt_destroy(pdrt_engine *engine);
 /* Message of the last failure; valid until the next call on that engine. */
 PDRT_API const char *pdrt_last_error(const pdrt_engine *engine);
 
-/* Rebuilds W_tab for another lateral kernel size (odd, 3..63); used by the kernel-size sweep
+/* Rebuilds W_tab for another lateral kernel size (odd, 3..255; the paper's operating point is 55, and its
+ * sensitivity study goes to 225, Table 4); used by the kernel-size sweep
  * (Table 4).  Synchronises the device. */
 PDRT_API int pdrt_set_kernel_size(pdrt_engine *engine, int32_t kernel_size);
 

@@ -54,7 +54,7 @@ class PdrtInfo(C.Structure):
                 ("flu_nu", C.c_int32), ("flu_nv", C.c_int32), ("n_pairs", C.c_int32),
                 ("kernel_size", C.c_int32), ("kernel_size_compiled", C.c_int32),
                 ("ray_step_mm", C.c_float), ("ray_samples", C.c_int32), ("sm_count", C.c_int32),
-                ("scratch_bytes", C.c_uint64)]
+                ("scratch_bytes", C.c_uint64), ("kernel_passes", C.c_int32)]
 
 
 class PdrtWork(C.Structure):

@@ -314,13 +314,18 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *
     }
 }
 
+// One pass of the convolution: sub-kernel (bi, bj) of the (NB KT)^2 window reads its inputs shifted by (su, sv) = ((bi, bj) - (NB-1)/2) KT:
+//   out(i, j) (+)= sum_{di', dj' < KT} W_blk[di'][dj'] in(i + di' - c' + su, j + dj' - c' + sv),   c' = (KT-1)/2.
+// The first pass (the centre block) writes every thread-tile of the output box, the others add to the tiles they reach.
+struct ConvPass { int su, sv, first; };
+
 // Geometry of one conv work item (control point, slice, chunk along v); identical in every lane of the warp.
 struct ConvItem {
     int slot, cp, k;
     int pv, nts;
     long long slice_off;             // slot * stride_cp + k * pu * pv  (start of the [pu][pv] slice in the compact blocks)
     int ri0, rj0;
-    SliceBox S, B;                   // fluence support of the slice; source box of the input rows (S forward, F adjoint)
+    SliceBox S, B, R;                // fluence support of the slice; source box of the input rows (S forward, F adjoint); outputs this pass reaches
     int ctf0, ctf1;                  // thread-tile range of the chunk along v
     int atf0, ats0, naf, nas;        // active thread-tiles of the slice and chunk (outputs to compute)
     int av0;                         // v index of the first active output column (forward: tile-aligned; adjoint: S.v0 & ~1)
@@ -330,10 +335,10 @@ struct ConvItem {
     float f;
 };
 
-template <int KT, bool ADJ>
+template <int KT, bool ADJ, int CPL>
 __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__restrict__ desc, int cp0, int n_cp,
                                                const int *__restrict__ tile_base, const float *__restrict__ zrad,
-                                               int item, int &slot_hint, ConvItem &it)
+                                               const ConvPass &pass, int item, int &slot_hint, ConvItem &it)
 {
     constexpr int C = (KT - 1) / 2;
     while (slot_hint + 1 < n_cp && item >= tile_base[slot_hint + 1]) ++slot_hint;   // items arrive in increasing order
@@ -347,10 +352,17 @@ __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__
     it.slice_off = (long long)it.slot * P.stride_cp + (long long)it.k * d.pu * d.pv;
     it.ctf0 = cf * d.ntfc; it.ctf1 = min(d.ntf, it.ctf0 + d.ntfc);
     it.S = slice_support(P, d, it.k);
-    const SliceBox F = dilate(P, it.S, C);
+    const SliceBox F = dilate(P, it.S, P.CH);
     it.B = ADJ ? F : it.S;
-    if (C % 2 == 0) { it.B.v0 &= ~1; it.B.v1 |= 1; }              // row copies move aligned pairs (k_project / k_resample_adjoint write them)
-    const SliceBox A = ADJ ? it.S : F;                            // outputs to compute
+    if (CPL == 2) { it.B.v0 &= ~1; it.B.v1 |= 1; }                // row copies move aligned pairs (k_project / k_resample_adjoint write them)
+    // outputs this pass can reach: forward, the footprint of the shifted sub-kernel; adjoint, all of S_k (every input in F_k counts)
+    it.R = ADJ ? it.S : F;
+    if (!ADJ) {
+        it.R.u0 = max(F.u0, it.S.u0 - pass.su - C); it.R.u1 = min(F.u1, it.S.u1 - pass.su + C);
+        it.R.v0 = max(F.v0, it.S.v0 - pass.sv - C); it.R.v1 = min(F.v1, it.S.v1 - pass.sv + C);
+        if (box_empty(it.S)) { it.R.u0 = 1; it.R.u1 = 0; }
+    }
+    const SliceBox A = ADJ ? it.S : (pass.first ? F : it.R);      // outputs to compute (the first pass also zero-fills what it does not reach)
     int atf0 = 0, atf1 = -1, ats0 = 0, ats1 = -1;
     if (!box_empty(A)) {
         atf0 = max(it.ctf0, (A.v0 - d.rj0) / RF); atf1 = min(it.ctf1 - 1, (A.v1 - d.rj0) / RF);
@@ -368,7 +380,7 @@ __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__
     it.n_tiles = it.naf * it.nas;
     it.pitch = conv_pitch(KT, max(it.naf, 1));
     it.ring = P.tile_floats / it.pitch;
-    it.tv0 = it.av0 - C; it.tu0 = d.ri0 + ats0 * RS - C;
+    it.tv0 = it.av0 - C + pass.sv; it.tu0 = d.ri0 + ats0 * RS - C + pass.su;
     it.n0 = 0; it.f = 0.f;
     if (!any) return;
     // S4: slice kernel = lerp of the table in radiological depth
@@ -389,17 +401,15 @@ __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__
 // hundred thread-tiles): a block-wide tile shared through __syncthreads left the warps waiting on each other for
 // almost half of their time (profiles/); independent warps balance by construction, and the other warps resident
 // on the SM keep the FFMA pipe busy while one waits for its copies.
-template <int KT, bool ADJ>
+template <int KT, bool ADJ, int CPL>                  // CPL: floats per asynchronous copy, 2 when source and tile columns share parity ((C - sv) even)
 __global__ void __launch_bounds__(CONV_THREADS)
 k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
        const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
-       int *item_counter)
+       int *item_counter, ConvPass pass)
 {
-    constexpr int C = (KT - 1) / 2;
     constexpr int KP = (KT + 3) & ~3;                 // weight row pitch [floats]
     constexpr int XW = (KT + RF - 1 + 3) & ~3;        // register window along v [floats]
     constexpr int NXQ = XW / 4;
-    constexpr int CPL = (C % 2 == 0) ? 2 : 1;         // floats per asynchronous copy (source and tile columns share parity when C is even)
     constexpr int PMAX = (NTFC_MAX * RF + XW - RF + 7) & ~7;   // widest row
     constexpr int MC = (PMAX / CPL + 31) / 32;        // copies per lane and row
     extern __shared__ float4 smem4[];
@@ -418,7 +428,7 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
         item = __shfl_sync(0xffffffffu, item, 0);
         if (item >= total) break;
         ConvItem I;
-        conv_load_item<KT, ADJ>(P, desc, cp0, n_cp, tile_base, zrad, item, slot_hint, I);
+        conv_load_item<KT, ADJ, CPL>(P, desc, cp0, n_cp, tile_base, zrad, pass, item, slot_hint, I);
         float *oslice = out + I.slice_off;             // [pu][pv] of slice k
         if (I.n_tiles == 0) continue;                  // uniform across the warp
         const int pitch = I.pitch, ring = I.ring, naf = I.naf;
@@ -491,13 +501,16 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                 for (int r = 0; r < RF; ++r) acc2[r] = make_float2(0.f, 0.f);
                 // forward: input rows outside S_k hold zeros (structurally zero fluence) and are skipped
                 const int ylo = ADJ ? 0 : max(0, I.S.u0 - I.tu0 - tsa * RS), yhi = ADJ ? KT + RS - 2 : min(KT + RS - 2, I.S.u1 - I.tu0 - tsa * RS);
+                // forward: a thread-tile that this pass's sub-kernel does not reach keeps its zeros (only the first pass has such tiles)
+                const int ou = (I.ats0 + tsa) * RS + I.ri0, ov = I.av0 + tf * RF;
+                const bool live = ADJ || (ou + RS - 1 >= I.R.u0 && ou <= I.R.u1 && ov + RF - 1 >= I.R.v0 && ov <= I.R.v1);
                 const float *xrow = tile + ((tsa * RS + ylo) % ring) * pitch;
                 int xoff[NXQ];
 #pragma unroll
                 for (int q = 0; q < NXQ; ++q) xoff[q] = swz_col(tf * RF + 4 * q);
                 const float4 *w4 = reinterpret_cast<const float4 *>(Ws2 + ylo * KP);
 #pragma unroll 1
-                for (int y = ylo; y <= yhi; ++y) {
+                for (int y = live ? ylo : yhi + 1; y <= yhi; ++y) {
                     float2 xx[XW];                 // window element duplicated: it multiplies the weights of both output rows
 #pragma unroll
                     for (int q = 0; q < NXQ; ++q) {
@@ -534,11 +547,20 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                         const int room = I.pv - ((I.av0 - I.rj0) + tf * RF);
 #pragma unroll
                         for (int r = 0; r < RF; r += 2)
-                            if (r + 2 <= room) *reinterpret_cast<float2 *>(op + r) = make_float2(acc[ii][r], acc[ii][r + 1]);
+                            if (r + 2 <= room) {
+                                float2 *o = reinterpret_cast<float2 *>(op + r);
+                                float2 v = make_float2(acc[ii][r], acc[ii][r + 1]);
+                                if (!pass.first) { const float2 p = *o; v.x += p.x; v.y += p.y; }
+                                *o = v;
+                            }
                     } else {
                         float4 *o = reinterpret_cast<float4 *>(op);
-                        o[0] = make_float4(acc[ii][0], acc[ii][1], acc[ii][2], acc[ii][3]);
-                        o[1] = make_float4(acc[ii][4], acc[ii][5], acc[ii][6], acc[ii][7]);
+                        float4 v0 = make_float4(acc[ii][0], acc[ii][1], acc[ii][2], acc[ii][3]), v1 = make_float4(acc[ii][4], acc[ii][5], acc[ii][6], acc[ii][7]);
+                        if (!pass.first) {
+                            const float4 p0 = o[0], p1 = o[1];
+                            v0.x += p0.x; v0.y += p0.y; v0.z += p0.z; v0.w += p0.w; v1.x += p1.x; v1.y += p1.y; v1.z += p1.z; v1.w += p1.w;
+                        }
+                        o[0] = v0; o[1] = v1;
                     }
                 }
             }

@@ -42,7 +42,9 @@ struct Params {
     float sid, tau, cal;
     int Np;                              // leaf pairs
     // lateral kernel
-    int K, KT;                           // requested size, compiled variant (KT >= K)
+    int K, KT;                           // requested size; compiled variant of ONE pass (single pass: KT >= K)
+    int NB, CH;                          // passes per axis (odd): the K x K kernel, centred in an (NB KT)^2 window, is applied as NB^2
+                                         // KT x KT sub-kernels with shifted inputs;  CH = (K-1)/2, the halo of the footprint F_k
     int n_z;
     float dz;
     int tile_floats;                     // conv input-tile budget in shared memory [floats]

@@ -26,7 +26,16 @@ namespace {
 std::string g_create_error;
 
 // compiled conv variants; a requested size k runs on the smallest KT >= k with the table embedded in zeros
-const int kCompiled[] = { 5, 11, 15, 21, 25, 31, 41, 51, 63 };
+const int kCompiled[] = { 5, 11, 15, 21, 25, 31, 41, 51, 55, 63 };
+const int kMaxKernel = 255;            // NB = 9 passes per axis of KT = 31 at most
+// Kernels up to `single_max` run as one pass on the smallest compiled variant; larger ones are split into NB x NB sub-kernels of
+// at most 31 taps (NB odd, so that the window stays centred): fewer multiply-adds with structural zeros than one wide pass
+// (halo overhead ((s + KT - 1)/s)^2 per pass instead of ((s + K - 1)/s)^2), and no limit on K from registers or shared memory.
+int conv_single_max()
+{
+    if (const char *v = std::getenv("PDRT_CONV_SINGLE_MAX")) { const int m = std::atoi(v); if (m >= 3 && m <= 63) return m; }
+    return 55;       // measured on c4: one pass wins up to 55 taps, 3 x 3 passes of 21 from 63 on
+}
 int compiled_size(int k)
 {
     for (int kt : kCompiled)
@@ -94,7 +103,7 @@ struct pdrt_engine {
     bool last_backward = false;
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
-    int conv_per_sm[2][64] = {};      // resident conv blocks per SM on THIS engine's device, by [adjoint][KT]; 0 = not queried yet
+    int conv_per_sm[2][2][64] = {};   // resident conv blocks per SM on THIS engine's device, by [adjoint][copy width - 1][KT]; 0 = not queried yet
     DevBuf<float> coll;               // collimator angles [coll_n] set by pdrt_set_collimator (coll_n = 0: none)
     int coll_n = 0;
     int nzp = 0;                      // row pitch of gT: nz rounded up to 4
@@ -178,11 +187,18 @@ int gaussian_taps(double sigma, double D, std::vector<float> &g)
 // flipped kernel of the adjoint is the same table (R3).
 int build_kernel_table(pdrt_engine *e, int k)
 {
-    const int kt = compiled_size(k);
-    const int c = (k - 1) / 2, ct = (kt - 1) / 2, nz = e->P.n_z;
+    int nb = 1, kt = compiled_size(k);
+    if (k > conv_single_max()) {
+        nb = 3;
+        while ((k + nb - 1) / nb > 31) nb += 2;
+        kt = compiled_size(((k + nb - 1) / nb) | 1);
+    }
+    const int T = nb * kt;                              // odd: the K x K kernel sits centred in the T x T window
+    const int c = (k - 1) / 2, cT = (T - 1) / 2, nz = e->P.n_z;
     const double du = e->P.du, dv = e->P.dv;
     const int kp = (kt + 3) & ~3;
-    std::vector<float> tab((size_t)nz * kt * kp, 0.f);
+    const size_t blk = (size_t)nz * kt * kp;
+    std::vector<float> tab(blk * nb * nb, 0.f);
     std::vector<double> rad((size_t)(c + 1) * (c + 1) * 64);
     for (int qj = 0; qj <= c; ++qj)
         for (int qi = 0; qi <= c; ++qi)
@@ -191,6 +207,10 @@ int build_kernel_table(pdrt_engine *e, int k)
                     const double x = (qi + (si + 0.5) / 8.0 - 0.5) * du, y = (qj + (sj + 0.5) / 8.0 - 0.5) * dv;
                     rad[(((size_t)qj * (c + 1) + qi) * 8 + sj) * 8 + si] = std::sqrt(x * x + y * y);
                 }
+    // window position (wi along u, wj along v) -> block (wi / kt, wj / kt), image [du][dv padded to kp] of that block
+    auto at = [&](int n, int wi, int wj) -> float & {
+        return tab[(size_t)((wi / kt) * nb + (wj / kt)) * blk + (size_t)n * kt * kp + (size_t)(wi % kt) * kp + (wj % kt)];
+    };
     for (int n = 0; n < nz; ++n) {
         const double A = e->kA[n], a = e->ka[n], B = e->kB[n], b = e->kb[n];
         for (int qj = 0; qj <= c; ++qj)
@@ -199,9 +219,8 @@ int build_kernel_table(pdrt_engine *e, int k)
                 const double *r = &rad[((size_t)qj * (c + 1) + qi) * 64];
                 for (int q = 0; q < 64; ++q) s += (A * std::exp(-a * r[q]) + B * std::exp(-b * r[q])) / r[q];
                 const float w = (float)(s * du * dv / 64.0);
-                float *slice = &tab[(size_t)n * kt * kp];        // [di][dj]: qi runs along u, qj along v
-                slice[(ct + qi) * kp + (ct + qj)] = w; slice[(ct + qi) * kp + (ct - qj)] = w;
-                slice[(ct - qi) * kp + (ct + qj)] = w; slice[(ct - qi) * kp + (ct - qj)] = w;
+                at(n, cT + qi, cT + qj) = w; at(n, cT + qi, cT - qj) = w;
+                at(n, cT - qi, cT + qj) = w; at(n, cT - qi, cT - qj) = w;
             }
     }
     CU(e, e->wtab.ensure(tab.size()));
@@ -209,26 +228,50 @@ int build_kernel_table(pdrt_engine *e, int k)
     e->K = k;
     e->P.K = k;
     e->P.KT = kt;
+    e->P.NB = nb;
+    e->P.CH = c;
     e->P.tile_floats = tile_floats_for(kt);
     return PDRT_OK;
 }
 
-template <int KT, bool ADJ>
-int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
+template <int KT, bool ADJ, int CPL>
+int launch_conv_pass(pdrt_engine *e, int cp0, int n, const float *wtab, const float *in, float *out, const ConvPass &pass, cudaStream_t st)
 {
     static_assert(KT < 64, "conv_per_sm is indexed by KT");
-    int &per_sm = e->conv_per_sm[ADJ ? 1 : 0][KT];    // per engine (= per device): the opt-in attribute is a per-device setting
+    int &per_sm = e->conv_per_sm[ADJ ? 1 : 0][CPL - 1][KT];   // per engine (= per device): the opt-in attribute is a per-device setting
     const size_t smem = conv_smem_bytes(KT);
     if (per_sm == 0) {
-        CU(e, cudaFuncSetAttribute(k_conv<KT, ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(e, cudaFuncSetAttribute(k_conv<KT, ADJ, CPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int n_res = 0;
-        CU(e, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n_res, k_conv<KT, ADJ>, CONV_THREADS, smem));
+        CU(e, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n_res, k_conv<KT, ADJ, CPL>, CONV_THREADS, smem));
         per_sm = n_res < 1 ? 1 : n_res;
     }
     e->conv_grid = e->sm_count * per_sm;              // persistent grid: a multiple of the SM count
-    k_conv<KT, ADJ><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->zrad.p, e->wtab.p, in, out,
-                                                             e->tile_base.p + n + 1);
+    k_conv<KT, ADJ, CPL><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->zrad.p, wtab, in, out,
+                                                                  e->tile_base.p + n + 1, pass);
     CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+// All NB x NB passes of one convolution, the centre block first (it writes; the others accumulate).  Returns the launches made.
+template <int KT, bool ADJ>
+int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
+{
+    const int nb = e->P.NB, nbh = (nb - 1) / 2, C = (KT - 1) / 2;
+    const size_t blk = (size_t)e->P.n_z * KT * ((KT + 3) & ~3);
+    bool first = true;
+    for (int pi = 0; pi < nb * nb; ++pi) {
+        // visit order: centre block, then the rest
+        const int centre = nbh * nb + nbh;
+        const int q = pi == 0 ? centre : (pi <= centre ? pi - 1 : pi);
+        const int bi = q / nb, bj = q % nb;
+        const ConvPass pass{ (bi - nbh) * KT, (bj - nbh) * KT, first ? 1 : 0 };
+        if (!first) CU(e, cudaMemsetAsync(e->tile_base.p + n + 1, 0, sizeof(int), st));      // the unit counter of the next pass
+        const float *wt = e->wtab.p + (size_t)q * blk;
+        const int rc = ((C - pass.sv) % 2 == 0) ? launch_conv_pass<KT, ADJ, 2>(e, cp0, n, wt, in, out, pass, st)
+                                                : launch_conv_pass<KT, ADJ, 1>(e, cp0, n, wt, in, out, pass, st);
+        if (rc) return rc;
+        first = false;
+    }
     return PDRT_OK;
 }
 template <bool ADJ> int launch_conv(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
@@ -242,6 +285,7 @@ template <bool ADJ> int launch_conv(pdrt_engine *e, int cp0, int n, const float 
     case 31: return launch_conv_t<31, ADJ>(e, cp0, n, in, out, st);
     case 41: return launch_conv_t<41, ADJ>(e, cp0, n, in, out, st);
     case 51: return launch_conv_t<51, ADJ>(e, cp0, n, in, out, st);
+    case 55: return launch_conv_t<55, ADJ>(e, cp0, n, in, out, st);
     case 63: return launch_conv_t<63, ADJ>(e, cp0, n, in, out, st);
     }
     return fail(e, PDRT_EINVAL, "no compiled convolution variant for this kernel size");
@@ -333,7 +377,7 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
         }
         CU(e, cudaGetLastError());
         {
-            StageTimer t(e, PDRT_STAGE_CONV, st);
+            StageTimer t(e, PDRT_STAGE_CONV, st, e->P.NB * e->P.NB);
             rc = launch_conv<false>(e, cp0, n, e->bufB.p, e->bufA.p, st);
         }
         if (rc) return rc;
@@ -382,12 +426,12 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
         CU(e, cudaGetLastError());
         {
             StageTimer t(e, PDRT_STAGE_RESAMPLE_ADJ, st);
-            k_resample_adjoint<<<dim3(resample_adj_blocks(e->P), n), RA_THREADS, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, (e->P.KT - 1) / 2, e->nzp,
+            k_resample_adjoint<<<dim3(resample_adj_blocks(e->P), n), RA_THREADS, 0, st>>>(e->P, e->desc.p, e->sbox.p, cp0, n, e->P.CH, e->nzp,
                                                                                           e->gT.p, e->bufB.p);
         }
         CU(e, cudaGetLastError());
         {
-            StageTimer t(e, PDRT_STAGE_CONV_ADJ, st);
+            StageTimer t(e, PDRT_STAGE_CONV_ADJ, st, e->P.NB * e->P.NB);
             rc = launch_conv<true>(e, cp0, n, e->bufB.p, e->bufA.p, st);
         }
         if (rc) return rc;
@@ -447,7 +491,7 @@ int pdrt_create(const pdrt_grid *grid, const float *density, const pdrt_beam_mod
     for (int n = 0; n < m->n_z; ++n)
         if (!std::isfinite(m->kA[n]) || !std::isfinite(m->ka[n]) || !std::isfinite(m->kB[n]) || !std::isfinite(m->kb[n]))
             return fail(nullptr, PDRT_EINVAL, "non-finite kernel table entry");
-    if (m->kernel_size < 3 || m->kernel_size > 63 || m->kernel_size % 2 == 0) return fail(nullptr, PDRT_EINVAL, "kernel_size must be odd, 3..63");
+    if (m->kernel_size < 3 || m->kernel_size > kMaxKernel || m->kernel_size % 2 == 0) return fail(nullptr, PDRT_EINVAL, "kernel_size must be odd, 3..255");
     if (m->beam_nu < 0 || (m->beam_nu > 0 && (m->beam_nw < 1 || !(m->beam_du > 0) || !(m->beam_dw > 0))))
         return fail(nullptr, PDRT_EINVAL, "bad beam grid");
     if (!(m->ray_step_mm >= 0)) return fail(nullptr, PDRT_EINVAL, "ray_step_mm must be >= 0");
@@ -564,7 +608,7 @@ void pdrt_destroy(pdrt_engine *e)
 int pdrt_set_kernel_size(pdrt_engine *e, int32_t k)
 {
     if (!e) return fail(nullptr, PDRT_EINVAL, "null engine");
-    if (k < 3 || k > 63 || k % 2 == 0) return fail(e, PDRT_EINVAL, "kernel_size must be odd, 3..63");
+    if (k < 3 || k > kMaxKernel || k % 2 == 0) return fail(e, PDRT_EINVAL, "kernel_size must be odd, 3..255");
     CU(e, cudaSetDevice(e->device));
     CU(e, cudaDeviceSynchronize());
     return build_kernel_table(e, k);
@@ -599,7 +643,7 @@ int pdrt_get_info(const pdrt_engine *e, pdrt_info *info)
     info->beam_nu = P.Nu; info->beam_nv = P.Nv; info->beam_nw = P.Nw;
     info->beam_du = P.du; info->beam_dv = P.dv; info->beam_dw = P.dw; info->beam_wmin = P.wmin;
     info->flu_nu = P.Nuf; info->flu_nv = P.Nvf; info->n_pairs = P.Np;
-    info->kernel_size = P.K; info->kernel_size_compiled = P.KT;
+    info->kernel_size = P.K; info->kernel_size_compiled = P.KT; info->kernel_passes = P.NB * P.NB;
     info->ray_step_mm = (float)P.ray_step; info->ray_samples = P.M_ray;
     info->sm_count = e->sm_count;
     info->scratch_bytes = e->scratch_bytes();

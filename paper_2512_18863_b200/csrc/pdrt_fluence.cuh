@@ -82,7 +82,7 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
         d.pb0 = max(0, (int)floorf(vlo / P.Dv + P.cvf)); d.pb1 = min(P.Nvf - 1, (int)ceilf(vhi / P.Dv + P.cvf));
         if (d.pa0 > d.pa1 || d.pb0 > d.pb1) { d.a0 = d.ja0 = d.pa0 = 1; d.a1 = d.ja1 = d.pa1 = 0; d.b0 = d.jb0 = d.pb0 = 1; d.b1 = d.jb1 = d.pb1 = 0; return; }
     }
-    const int C = (P.KT - 1) / 2;
+    const int C = P.CH;
     const SliceBox s0 = slice_support(P, d, 0), s1 = slice_support(P, d, P.Nw - 1);
     const int u0 = max(0, min(s0.u0, s1.u0) - C), u1 = min(P.Nu - 1, max(s0.u1, s1.u1) + C);
     const int v0 = max(0, min(s0.v0, s1.v0) - C), v1 = min(P.Nv - 1, max(s0.v1, s1.v1) + C);
@@ -118,7 +118,7 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
     __syncthreads();
     const bool empty = d.a0 > d.a1;
     if (!empty) {     // per-slice boxes for the resampling kernels, and work counters: |S_k|, |F_k|, thread-tiles
-        const int C = (P.KT - 1) / 2;
+        const int C = P.CH, CB = (P.KT - 1) / 2, nbh = (P.NB - 1) / 2;
         unsigned long long sup = 0, fp = 0, tf = 0, ta = 0;
         for (int k = tid; k < P.Nw; k += FLU_THREADS) {
             const SliceBox s = slice_support(P, d, k), f = dilate(P, s, C);
@@ -136,8 +136,15 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
             if (box_empty(s)) continue;
             sup += (unsigned long long)(s.u1 - s.u0 + 1) * (s.v1 - s.v0 + 1);
             fp += (unsigned long long)(f.u1 - f.u0 + 1) * (f.v1 - f.v0 + 1);
-            tf += (unsigned long long)((f.u1 - d.ri0) / RS - (f.u0 - d.ri0) / RS + 1) * ((f.v1 - d.rj0) / RF - (f.v0 - d.rj0) / RF + 1);
-            ta += (unsigned long long)((s.u1 - d.ri0) / RS - (s.u0 - d.ri0) / RS + 1) * ((s.v1 - d.rj0) / RF - (s.v0 - d.rj0) / RF + 1);
+            // thread-tiles that do multiply-adds: forward, per pass the tiles the shifted sub-kernel reaches inside F_k; adjoint, S_k in every pass
+            for (int bi = -nbh; bi <= nbh; ++bi)
+                for (int bj = -nbh; bj <= nbh; ++bj) {
+                    const int u0 = max(f.u0, s.u0 - bi * P.KT - CB), u1 = min(f.u1, s.u1 - bi * P.KT + CB);
+                    const int v0 = max(f.v0, s.v0 - bj * P.KT - CB), v1 = min(f.v1, s.v1 - bj * P.KT + CB);
+                    if (u0 <= u1 && v0 <= v1)
+                        tf += (unsigned long long)((u1 - d.ri0) / RS - (u0 - d.ri0) / RS + 1) * ((v1 - d.rj0) / RF - (v0 - d.rj0) / RF + 1);
+                }
+            ta += (unsigned long long)P.NB * P.NB * ((s.u1 - d.ri0) / RS - (s.u0 - d.ri0) / RS + 1) * ((s.v1 - d.rj0) / RF - (s.v0 - d.rj0) / RF + 1);
         }
         atomicAdd(&cnt[0], sup); atomicAdd(&cnt[1], fp); atomicAdd(&cnt[2], tf); atomicAdd(&cnt[3], ta);
     }

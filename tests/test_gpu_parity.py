@@ -173,16 +173,17 @@ def test_edge_cases(torch):
             assert float(one.abs().max()) == 0.0
 
 
-@pytest.mark.parametrize("k", [3, 5, 9, 17, 23, 33, 43, 51, 55, 63])
+@pytest.mark.parametrize("k", [3, 5, 9, 17, 23, 33, 41, 43, 51, 55, 63, 75, 93, 125])
 def test_kernel_size_sweep_small(torch, k):
-    """pdrt_set_kernel_size, including sizes that have no compiled variant of their own and the variants whose
-    shared memory exceeds the 48 KB default (KT = 51, 63)."""
+    """pdrt_set_kernel_size, including sizes that have no compiled variant of their own, and sizes above 55, which run as
+    NB x NB passes of shifted sub-kernels (63..93: 3 x 3; 125: 5 x 5)."""
     big = k > 33                       # a grid that holds the halo of the large kernels
     wl = W.tiny(seed=13, n_cp=2, kernel_size=5, nx=80 if big else 48, ny=44, nz=76 if big else 36, spacing=3.0, flu=(30, 30))
     eng, orc = pair(wl)
     eng.set_kernel_size(k)
     orc.set_kernel_size(k)
-    assert eng.info.kernel_size == k and eng.info.kernel_size_compiled >= k
+    passes = int(round(eng.info.kernel_passes ** 0.5))
+    assert eng.info.kernel_size == k and passes * eng.info.kernel_size_compiled >= k and (passes == 1) == (k <= 55)
     assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), f"k={k}")
     g = W.seeded_dose_gradient(wl, seed=k)
     dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
@@ -210,7 +211,7 @@ def test_host_entry_points_and_errors(torch):
     with pytest.raises(PdrtError):
         Engine(wl.grid, bad, wl.density)
     with pytest.raises(PdrtError):
-        eng.set_kernel_size(65)
+        eng.set_kernel_size(257)
     with pytest.raises(PdrtError):
         Engine(wl.grid, dict(wl.model, leaf_bounds_mm=np.zeros(wl.model["n_pairs"] + 1, np.float32)), wl.density)
 
@@ -285,9 +286,37 @@ def test_config4_full_arc_whole_grid_and_all_gradient_rows(torch):
         assert_grad(dl[b], rl[b], f"c4 d_leaves row {b}"); assert_grad(dj[b], rj[b], f"c4 d_jaws row {b}")
 
 
-@pytest.mark.parametrize("k", [11, 31, 41])
+def test_wide_single_pass_variants(torch, monkeypatch):
+    """The widest compiled variants (more than 48 KB of shared memory per warp) as ONE pass, including 63, which the default
+    splits into 3 x 3 sub-kernels; and the split forced on small kernels."""
+    monkeypatch.setenv("PDRT_CONV_SINGLE_MAX", "63")
+    wl = W.tiny(seed=13, n_cp=2, kernel_size=5, nx=80, ny=44, nz=76, spacing=3.0, flu=(30, 30))
+    eng, orc = pair(wl)
+    for k in (47, 55, 63):
+        eng.set_kernel_size(k)
+        orc.set_kernel_size(k)
+        assert eng.info.kernel_passes == 1 and eng.info.kernel_size_compiled >= k
+        assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), f"single pass k={k}")
+        g = W.seeded_dose_gradient(wl, seed=k)
+        dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+        rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+        assert_grad(dm, rm, f"single pass k={k} d_mu"); assert_grad(dl, rl, f"single pass k={k} d_leaves")
+    monkeypatch.setenv("PDRT_CONV_SINGLE_MAX", "5")
+    for k in (7, 13, 33):                           # 3 x 3 passes of 5 / 5 / 11 taps
+        eng.set_kernel_size(k)
+        orc.set_kernel_size(k)
+        assert eng.info.kernel_passes == 9
+        assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), f"split k={k}")
+        g = W.seeded_dose_gradient(wl, seed=k)
+        dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+        rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+        assert_grad(dm, rm, f"split k={k} d_mu"); assert_grad(dl, rl, f"split k={k} d_leaves")
+
+
+@pytest.mark.parametrize("k", [11, 31, 41, 55])
 def test_config4_kernel_size_sweep_sampled(torch, k):
-    """The other kernel sizes of the c4 sweep at full size: sampled voxels and sampled control points."""
+    """The other kernel sizes of the c4 sweep at full size, and the paper's operating point k = 55: sampled
+    voxels and sampled control points."""
     wl = W.config4(k)
     eng, orc = pair(wl)
     check_sampled_dose(eng, orc, wl, 90, 40 + k, f"c4 k={k}")

@@ -215,11 +215,21 @@ PDRT_API int pdrt_dose_backward(pdrt_engine *engine, int32_t n_cp,
                        void *cuda_stream);
 
 /* The same two calls with HOST buffers: host->device copies of the parameters (and dL/dDose),
- * the kernels, the device->host copy of the result, and a stream synchronise. */
+ * the kernels, the device->host copy of the result, and a stream synchronise.  The two volumes move on copy streams of
+ * the engine: dL/dDose is uploaded while the backward pass uploads its parameters and runs S1 / S2. */
 PDRT_API int pdrt_dose_host(pdrt_engine *engine, int32_t n_cp,
                    const float *leaves_host, const float *jaws_host,
                    const float *gantry_deg_host, const float *mu_host,
                    float *dose_host, void *cuda_stream);
+/* pdrt_dose_host without the final wait: the parameters are uploaded, the kernels run and the dose travels to dose_host
+ * (pinned memory) on a copy stream of the engine; pdrt_host_wait blocks until it has arrived.  Between the two the caller may
+ * issue further calls (e.g. pdrt_dose_backward_host for a dL/dDose it already has): the download overlaps with them.
+ * All host buffers of the call must stay valid until pdrt_host_wait (or the next synchronising call on the stream) returns. */
+PDRT_API int pdrt_dose_host_async(pdrt_engine *engine, int32_t n_cp,
+                   const float *leaves_host, const float *jaws_host,
+                   const float *gantry_deg_host, const float *mu_host,
+                   float *dose_host, void *cuda_stream);
+PDRT_API int pdrt_host_wait(pdrt_engine *engine);
 PDRT_API int pdrt_dose_backward_host(pdrt_engine *engine, int32_t n_cp,
                             const float *leaves_host, const float *jaws_host,
                             const float *gantry_deg_host, const float *mu_host,

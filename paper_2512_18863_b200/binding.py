@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libpdrt.so")
 
 SYMBOLS = ("pdrt_create", "pdrt_destroy", "pdrt_last_error", "pdrt_set_kernel_size", "pdrt_get_info", "pdrt_get_work",
            "pdrt_set_profiling", "pdrt_get_stage_ms", "pdrt_set_depth_mode", "pdrt_stage_fan_factor", "pdrt_set_collimator",
-           "pdrt_dose", "pdrt_dose_backward", "pdrt_dose_host", "pdrt_dose_backward_host",
+           "pdrt_dose", "pdrt_dose_backward", "pdrt_dose_host", "pdrt_dose_backward_host", "pdrt_dose_host_async", "pdrt_host_wait",
            "pdrt_stage_fluence", "pdrt_stage_depth", "pdrt_stage_beam_dose", "pdrt_stage_grad_fluence",
            "pdrt_mu_epsilon", "pdrt_validate", "pdrt_validate_backward", "pdrt_objective", "pdrt_track_jaws", "pdrt_plan_step")
 
@@ -104,6 +104,8 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.pdrt_dose.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
     lib.pdrt_dose_backward.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.pdrt_dose_host.argtypes = lib.pdrt_dose.argtypes
+    lib.pdrt_dose_host_async.argtypes = lib.pdrt_dose.argtypes
+    lib.pdrt_host_wait.argtypes = [vp]
     lib.pdrt_dose_backward_host.argtypes = lib.pdrt_dose_backward.argtypes
     lib.pdrt_stage_fluence.argtypes = [vp, i32, vp, vp, vp, vp]
     lib.pdrt_stage_depth.argtypes = [vp, i32, vp, vp, vp]
@@ -358,6 +360,16 @@ class Engine:
         self._check(self.lib.pdrt_dose_host(self.handle, n_cp, _hptr(leaves), _hptr(jaws), _hptr(gantry_deg), _hptr(mu),
                                             _hptr(out), self._stream()))
         return out
+
+    def dose_host_async(self, leaves, jaws, gantry_deg, mu, out):
+        """pdrt_dose_host_async: as dose_host, but returns while the dose is still on its way to `out` (pinned); see host_wait."""
+        n_cp = int(gantry_deg.shape[0])
+        self._check(self.lib.pdrt_dose_host_async(self.handle, n_cp, _hptr(leaves), _hptr(jaws), _hptr(gantry_deg), _hptr(mu),
+                                                  _hptr(out), self._stream()))
+        return out
+
+    def host_wait(self):
+        self._check(self.lib.pdrt_host_wait(self.handle))
 
     def dose_backward_host(self, leaves, jaws, gantry_deg, mu, dL_ddose, d_leaves, d_jaws, d_mu):
         n_cp = int(gantry_deg.shape[0])

@@ -96,7 +96,12 @@ struct pdrt_engine {
     DevBuf<double> rho_s, Z_s;
     DevBuf<float> bufA, bufB;         // compact beam-frame blocks: conv output (D_b / H_b) and conv input (Phivol / G_b)
     // staging for the *_host entry points
-    DevBuf<float> s_leaves, s_jaws, s_gantry, s_mu, s_vol, s_dleaves, s_djaws, s_dmu;
+    DevBuf<float> s_leaves, s_jaws, s_gantry, s_mu, s_dose, s_g, s_dleaves, s_djaws, s_dmu;
+    // the host variants move the two volumes on copy streams of their own, so that the dose can travel to the host while the
+    // next call computes and dL/dDose can travel to the device while the backward pass sets up (PCIe is full duplex)
+    cudaStream_t cs_in = nullptr, cs_out = nullptr;
+    cudaEvent_t ev_fwd = nullptr, ev_out = nullptr, ev_g = nullptr, ev_bwd = nullptr;
+    bool out_pending = false, bwd_recorded = false;
     DevBuf<double> obj_partial;       // block partials of the objective
     size_t scratch_cap_bytes = (size_t)48 << 30;
     int last_n_cp = 0;
@@ -393,10 +398,11 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
 
 // S7-S9 for all control points: leaves dL/dPhimap (per control point, inside its support bbox) in e->gphimap
 int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry,
-                        const float *mu, const float *gdose, cudaStream_t st)
+                        const float *mu, const float *gdose, cudaStream_t st, cudaEvent_t gdose_ready = nullptr)
 {
     int rc = run_setup(e, n_cp, leaves, jaws, gantry, mu, true, st);
     if (rc) return rc;
+    if (gdose_ready) CU(e, cudaStreamWaitEvent(st, gdose_ready, 0));      // S1 / S2 above do not read dL/dDose
     const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
     CU(e, e->gphimap.ensure(nmap));
     CU(e, e->T3.ensure(nmap));
@@ -448,9 +454,9 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
 }
 
 int backward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry, const float *mu,
-                  const float *gdose, float *d_leaves, float *d_jaws, float *d_mu, cudaStream_t st)
+                  const float *gdose, float *d_leaves, float *d_jaws, float *d_mu, cudaStream_t st, cudaEvent_t gdose_ready = nullptr)
 {
-    int rc = backward_to_fluence(e, n_cp, leaves, jaws, gantry, mu, gdose, st);
+    int rc = backward_to_fluence(e, n_cp, leaves, jaws, gantry, mu, gdose, st, gdose_ready);
     if (rc) return rc;
     {
         StageTimer t(e, PDRT_STAGE_FLUENCE_ADJ, st);
@@ -599,7 +605,10 @@ void pdrt_destroy(pdrt_engine *e)
     e->counters.release(); e->phimap.release(); e->P0.release(); e->T1.release(); e->T2.release(); e->T3.release();
     e->Abuf.release(); e->gphimap.release(); e->zrad.release(); e->rho_s.release(); e->Z_s.release();
     e->bufA.release(); e->bufB.release(); e->phimapT.release(); e->gT.release();
-    e->s_leaves.release(); e->s_jaws.release(); e->s_gantry.release(); e->s_mu.release(); e->s_vol.release();
+    e->s_leaves.release(); e->s_jaws.release(); e->s_gantry.release(); e->s_mu.release(); e->s_dose.release(); e->s_g.release();
+    if (e->cs_in) cudaStreamDestroy(e->cs_in);
+    if (e->cs_out) cudaStreamDestroy(e->cs_out);
+    for (cudaEvent_t ev : { e->ev_fwd, e->ev_out, e->ev_g, e->ev_bwd }) if (ev) cudaEventDestroy(ev);
     e->s_dleaves.release(); e->s_djaws.release(); e->s_dmu.release(); e->obj_partial.release();
     for (cudaEvent_t ev : e->ev_pool) cudaEventDestroy(ev);
     delete e;
@@ -716,19 +725,48 @@ static int stage_params_in(pdrt_engine *e, int n_cp, const float *leaves, const 
     return PDRT_OK;
 }
 
-int pdrt_dose_host(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry,
-                   const float *mu, float *dose, void *stream)
+static int host_streams(pdrt_engine *e)
+{
+    if (e->cs_in) return PDRT_OK;
+    CU(e, cudaStreamCreateWithFlags(&e->cs_in, cudaStreamNonBlocking));
+    CU(e, cudaStreamCreateWithFlags(&e->cs_out, cudaStreamNonBlocking));
+    for (cudaEvent_t *ev : { &e->ev_fwd, &e->ev_out, &e->ev_g, &e->ev_bwd }) CU(e, cudaEventCreateWithFlags(ev, cudaEventDisableTiming));
+    return PDRT_OK;
+}
+
+int pdrt_dose_host_async(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry,
+                         const float *mu, float *dose, void *stream)
 {
     int rc = check_call(e, n_cp, { leaves, jaws, gantry, mu, dose });
     if (rc) return rc;
+    if ((rc = host_streams(e))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t nvox = (size_t)e->P.nx * e->P.ny * e->P.nz;
     if ((rc = stage_params_in(e, n_cp, leaves, jaws, gantry, mu, st))) return rc;
-    CU(e, e->s_vol.ensure(nvox));
-    if ((rc = forward_impl(e, n_cp, e->s_leaves.p, e->s_jaws.p, e->s_gantry.p, e->s_mu.p, e->s_vol.p, st))) return rc;
-    CU(e, cudaMemcpyAsync(dose, e->s_vol.p, nvox * sizeof(float), cudaMemcpyDeviceToHost, st));
-    CU(e, cudaStreamSynchronize(st));
+    CU(e, e->s_dose.ensure(nvox));
+    if (e->out_pending) CU(e, cudaStreamWaitEvent(st, e->ev_out, 0));        // the previous dose has left the staging buffer
+    if ((rc = forward_impl(e, n_cp, e->s_leaves.p, e->s_jaws.p, e->s_gantry.p, e->s_mu.p, e->s_dose.p, st))) return rc;
+    CU(e, cudaEventRecord(e->ev_fwd, st));
+    CU(e, cudaStreamWaitEvent(e->cs_out, e->ev_fwd, 0));
+    CU(e, cudaMemcpyAsync(dose, e->s_dose.p, nvox * sizeof(float), cudaMemcpyDeviceToHost, e->cs_out));
+    CU(e, cudaEventRecord(e->ev_out, e->cs_out));
+    e->out_pending = true;
     return PDRT_OK;
+}
+
+int pdrt_host_wait(pdrt_engine *e)
+{
+    if (!e) return fail(nullptr, PDRT_EINVAL, "null engine");
+    CU(e, cudaSetDevice(e->device));
+    if (e->out_pending) CU(e, cudaEventSynchronize(e->ev_out));
+    return PDRT_OK;
+}
+
+int pdrt_dose_host(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry,
+                   const float *mu, float *dose, void *stream)
+{
+    const int rc = pdrt_dose_host_async(e, n_cp, leaves, jaws, gantry, mu, dose, stream);
+    return rc ? rc : pdrt_host_wait(e);
 }
 
 int pdrt_dose_backward_host(pdrt_engine *e, int32_t n_cp, const float *leaves, const float *jaws, const float *gantry,
@@ -736,13 +774,19 @@ int pdrt_dose_backward_host(pdrt_engine *e, int32_t n_cp, const float *leaves, c
 {
     int rc = check_call(e, n_cp, { leaves, jaws, gantry, mu, gdose, d_leaves, d_jaws, d_mu });
     if (rc) return rc;
+    if ((rc = host_streams(e))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t nvox = (size_t)e->P.nx * e->P.ny * e->P.nz, nl = (size_t)n_cp * 2 * e->P.Np;
+    CU(e, e->s_g.ensure(nvox)); CU(e, e->s_dleaves.ensure(nl)); CU(e, e->s_djaws.ensure((size_t)n_cp * 4)); CU(e, e->s_dmu.ensure(n_cp));
+    // dL/dDose travels on the input copy stream while this stream uploads the parameters and runs S1 / S2
+    if (e->bwd_recorded) CU(e, cudaStreamWaitEvent(e->cs_in, e->ev_bwd, 0));  // the previous backward pass has read the staging buffer
+    CU(e, cudaMemcpyAsync(e->s_g.p, gdose, nvox * sizeof(float), cudaMemcpyHostToDevice, e->cs_in));
+    CU(e, cudaEventRecord(e->ev_g, e->cs_in));
     if ((rc = stage_params_in(e, n_cp, leaves, jaws, gantry, mu, st))) return rc;
-    CU(e, e->s_vol.ensure(nvox)); CU(e, e->s_dleaves.ensure(nl)); CU(e, e->s_djaws.ensure((size_t)n_cp * 4)); CU(e, e->s_dmu.ensure(n_cp));
-    CU(e, cudaMemcpyAsync(e->s_vol.p, gdose, nvox * sizeof(float), cudaMemcpyHostToDevice, st));
-    if ((rc = backward_impl(e, n_cp, e->s_leaves.p, e->s_jaws.p, e->s_gantry.p, e->s_mu.p, e->s_vol.p, e->s_dleaves.p,
-                            e->s_djaws.p, e->s_dmu.p, st))) return rc;
+    if ((rc = backward_impl(e, n_cp, e->s_leaves.p, e->s_jaws.p, e->s_gantry.p, e->s_mu.p, e->s_g.p, e->s_dleaves.p,
+                            e->s_djaws.p, e->s_dmu.p, st, e->ev_g))) return rc;
+    CU(e, cudaEventRecord(e->ev_bwd, st));
+    e->bwd_recorded = true;
     CU(e, cudaMemcpyAsync(d_leaves, e->s_dleaves.p, nl * sizeof(float), cudaMemcpyDeviceToHost, st));
     CU(e, cudaMemcpyAsync(d_jaws, e->s_djaws.p, sizeof(float) * n_cp * 4, cudaMemcpyDeviceToHost, st));
     CU(e, cudaMemcpyAsync(d_mu, e->s_dmu.p, sizeof(float) * n_cp, cudaMemcpyDeviceToHost, st));

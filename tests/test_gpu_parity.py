@@ -202,6 +202,15 @@ def test_host_entry_points_and_errors(torch):
     assert_dose(out, orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), "dose_host")
     g = W.seeded_dose_gradient(wl, seed=14)
     dl, dj, dm = (torch.empty(wl.leaves.shape).pin_memory(), torch.empty(wl.jaws.shape).pin_memory(), torch.empty(wl.mu.shape).pin_memory())
+    # asynchronous download of the dose overlapping the backward call, twice in a row (the staging buffers are reused)
+    hl, hj, hg, hm, hgd = t(wl.leaves), t(wl.jaws), t(wl.gantry_deg), t(wl.mu), t(g)      # stay alive until host_wait
+    for rep in range(2):
+        out.zero_()
+        hm2 = t(wl.mu * (1 + rep))
+        eng.dose_host_async(hl, hj, hg, hm2, out)
+        eng.dose_backward_host(hl, hj, hg, hm, hgd, dl, dj, dm)
+        eng.host_wait()
+        assert_dose(out, (1 + rep) * orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), f"dose_host_async {rep}")
     eng.dose_backward_host(t(wl.leaves), t(wl.jaws), t(wl.gantry_deg), t(wl.mu), t(g), dl, dj, dm)
     rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
     assert_grad(dl, rl, "host d_leaves"); assert_grad(dj, rj, "host d_jaws"); assert_grad(dm, rm, "host d_mu")

@@ -401,7 +401,9 @@ __device__ __forceinline__ void conv_load_item(const Params &P, const CpDesc *__
 // hundred thread-tiles): a block-wide tile shared through __syncthreads left the warps waiting on each other for
 // almost half of their time (profiles/); independent warps balance by construction, and the other warps resident
 // on the SM keep the FFMA pipe busy while one waits for its copies.
-template <int KT, bool ADJ, int CPL>                  // CPL: floats per asynchronous copy, 2 when source and tile columns share parity ((C - sv) even)
+// CPL: floats per asynchronous copy, 2 when source and tile columns share parity ((C - sv) even).  MULTI: one of several passes
+// (shifted sub-kernel: unreached tiles, accumulation into the output); the single-pass instance carries none of that code.
+template <int KT, bool ADJ, int CPL, bool MULTI>
 __global__ void __launch_bounds__(CONV_THREADS)
 k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
        const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
@@ -503,7 +505,7 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                 const int ylo = ADJ ? 0 : max(0, I.S.u0 - I.tu0 - tsa * RS), yhi = ADJ ? KT + RS - 2 : min(KT + RS - 2, I.S.u1 - I.tu0 - tsa * RS);
                 // forward: a thread-tile that this pass's sub-kernel does not reach keeps its zeros (only the first pass has such tiles)
                 const int ou = (I.ats0 + tsa) * RS + I.ri0, ov = I.av0 + tf * RF;
-                const bool live = ADJ || (ou + RS - 1 >= I.R.u0 && ou <= I.R.u1 && ov + RF - 1 >= I.R.v0 && ov <= I.R.v1);
+                const bool live = ADJ || !MULTI || (ou + RS - 1 >= I.R.u0 && ou <= I.R.u1 && ov + RF - 1 >= I.R.v0 && ov <= I.R.v1);
                 const float *xrow = tile + ((tsa * RS + ylo) % ring) * pitch;
                 int xoff[NXQ];
 #pragma unroll
@@ -550,13 +552,13 @@ k_conv(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *
                             if (r + 2 <= room) {
                                 float2 *o = reinterpret_cast<float2 *>(op + r);
                                 float2 v = make_float2(acc[ii][r], acc[ii][r + 1]);
-                                if (!pass.first) { const float2 p = *o; v.x += p.x; v.y += p.y; }
+                                if (MULTI && !pass.first) { const float2 p = *o; v.x += p.x; v.y += p.y; }
                                 *o = v;
                             }
                     } else {
                         float4 *o = reinterpret_cast<float4 *>(op);
                         float4 v0 = make_float4(acc[ii][0], acc[ii][1], acc[ii][2], acc[ii][3]), v1 = make_float4(acc[ii][4], acc[ii][5], acc[ii][6], acc[ii][7]);
-                        if (!pass.first) {
+                        if (MULTI && !pass.first) {
                             const float4 p0 = o[0], p1 = o[1];
                             v0.x += p0.x; v0.y += p0.y; v0.z += p0.z; v0.w += p0.w; v1.x += p1.x; v1.y += p1.y; v1.z += p1.z; v1.w += p1.w;
                         }

@@ -108,7 +108,7 @@ struct pdrt_engine {
     bool last_backward = false;
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
-    int conv_per_sm[2][2][64] = {};   // resident conv blocks per SM on THIS engine's device, by [adjoint][copy width - 1][KT]; 0 = not queried yet
+    int conv_per_sm[2][2][2][64] = {};   // resident conv blocks per SM on THIS engine's device, by [adjoint][copy width - 1][multi-pass][KT]; 0 = not queried yet
     DevBuf<float> coll;               // collimator angles [coll_n] set by pdrt_set_collimator (coll_n = 0: none)
     int coll_n = 0;
     int nzp = 0;                      // row pitch of gT: nz rounded up to 4
@@ -239,21 +239,21 @@ int build_kernel_table(pdrt_engine *e, int k)
     return PDRT_OK;
 }
 
-template <int KT, bool ADJ, int CPL>
+template <int KT, bool ADJ, int CPL, bool MULTI>
 int launch_conv_pass(pdrt_engine *e, int cp0, int n, const float *wtab, const float *in, float *out, const ConvPass &pass, cudaStream_t st)
 {
     static_assert(KT < 64, "conv_per_sm is indexed by KT");
-    int &per_sm = e->conv_per_sm[ADJ ? 1 : 0][CPL - 1][KT];   // per engine (= per device): the opt-in attribute is a per-device setting
+    int &per_sm = e->conv_per_sm[ADJ ? 1 : 0][CPL - 1][MULTI ? 1 : 0][KT];   // per engine (= per device): the opt-in attribute is a per-device setting
     const size_t smem = conv_smem_bytes(KT);
     if (per_sm == 0) {
-        CU(e, cudaFuncSetAttribute(k_conv<KT, ADJ, CPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(e, cudaFuncSetAttribute(k_conv<KT, ADJ, CPL, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int n_res = 0;
-        CU(e, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n_res, k_conv<KT, ADJ, CPL>, CONV_THREADS, smem));
+        CU(e, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n_res, k_conv<KT, ADJ, CPL, MULTI>, CONV_THREADS, smem));
         per_sm = n_res < 1 ? 1 : n_res;
     }
     e->conv_grid = e->sm_count * per_sm;              // persistent grid: a multiple of the SM count
-    k_conv<KT, ADJ, CPL><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->zrad.p, wtab, in, out,
-                                                                  e->tile_base.p + n + 1, pass);
+    k_conv<KT, ADJ, CPL, MULTI><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->zrad.p, wtab, in, out,
+                                                                         e->tile_base.p + n + 1, pass);
     CU(e, cudaGetLastError());
     return PDRT_OK;
 }
@@ -272,8 +272,17 @@ int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *in, float *out, c
         const ConvPass pass{ (bi - nbh) * KT, (bj - nbh) * KT, first ? 1 : 0 };
         if (!first) CU(e, cudaMemsetAsync(e->tile_base.p + n + 1, 0, sizeof(int), st));      // the unit counter of the next pass
         const float *wt = e->wtab.p + (size_t)q * blk;
-        const int rc = ((C - pass.sv) % 2 == 0) ? launch_conv_pass<KT, ADJ, 2>(e, cp0, n, wt, in, out, pass, st)
-                                                : launch_conv_pass<KT, ADJ, 1>(e, cp0, n, wt, in, out, pass, st);
+        int rc;
+        if constexpr (KT <= 31) {                     // sub-kernels of a split have at most 31 taps
+            if (nb > 1)
+                rc = ((C - pass.sv) % 2 == 0) ? launch_conv_pass<KT, ADJ, 2, true>(e, cp0, n, wt, in, out, pass, st)
+                                              : launch_conv_pass<KT, ADJ, 1, true>(e, cp0, n, wt, in, out, pass, st);
+            else
+                rc = launch_conv_pass<KT, ADJ, (C % 2 == 0) ? 2 : 1, false>(e, cp0, n, wt, in, out, pass, st);
+        } else {
+            if (nb > 1) return fail(e, PDRT_EINVAL, "sub-kernels of a split convolution have at most 31 taps");
+            rc = launch_conv_pass<KT, ADJ, (C % 2 == 0) ? 2 : 1, false>(e, cp0, n, wt, in, out, pass, st);
+        }
         if (rc) return rc;
         first = false;
     }

@@ -481,10 +481,13 @@ def run_ours(args):
         stages["conv_adj"].update(tflops=round(conv_adj_flops / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None,
                                   issued_tflops=round(2.0 * wb.conv_macs / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None)
     achieved = conv_flops / (stage_ms["conv"] * 1e-3) / 1e12 if stage_ms["conv"] > 0 else None
+    useful = 2.0 * K * K * wf.support_voxels / (stage_ms["conv"] * 1e-3) / 1e12 if stage_ms["conv"] > 0 else None
     roofline = dict(bound="alu", kernel="k_conv<K,false> (S4+S5: depth-indexed kernel lookup + lateral convolution)",
                     achieved=achieved, peak=fp32_peak, unit="TFLOP/s", frac=(achieved / fp32_peak) if achieved else None,
+                    achieved_on_nonzero_inputs=useful, frac_on_nonzero_inputs=(useful / fp32_peak) if useful else None,
                     traffic=recorded_traffic(wl.name, K),
-                    note=f"algorithmic flops = 2*k^2*|footprint| per launch; peak = {eng.info.sm_count} SMs x 128 FP32 lanes x 2 x "
+                    note=f"algorithmic flops = 2*k^2*|footprint| per launch (SURVEY.md 8(d): the output-tiled count); *_on_nonzero_inputs uses 2*k^2*|support| "
+                         f"(products with structurally zero fluence not counted); peak = {eng.info.sm_count} SMs x 128 FP32 lanes x 2 x "
                          f"{peaks['sm_max_mhz']:.0f} MHz (plain FP32 FMA pipe; FFMA microbenchmark on this pool: 72.5 TFLOP/s); "
                          f"HBM fractions of the bandwidth-bound stages are under 'stages' against {peaks['hbm_gbs']} GB/s {peaks['source']}")
 

@@ -243,9 +243,9 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
 // the 32 warps of a CLUSTER of four blocks; the planes are reduced in a fixed order, first inside each block, then across
 // the cluster through distributed shared memory (deterministic, no atomics).
 // Grid: (4 * ceil(Nvf/32), n_cp), cluster (4,1,1); dynamic shared memory n_act * Nuf * 32 floats.
-constexpr int PA_THREADS = 256, PA_WARPS = PA_THREADS / 32, PA_CLUSTER = 4, PA_TAPS = 4, PA_ROWS = 8;
+constexpr int PA_THREADS = 256, PA_WARPS = PA_THREADS / 32, PA_CLUSTER = 4, PA_TAPS = 4, PA_ROWS = 4;
 
-__global__ void __cluster_dims__(PA_CLUSTER, 1, 1) __launch_bounds__(PA_THREADS)
+__global__ void __cluster_dims__(PA_CLUSTER, 1, 1) __launch_bounds__(PA_THREADS, 3)
 k_project_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp, int n_act,
                   const float *__restrict__ H, float *__restrict__ gphimap)
 {

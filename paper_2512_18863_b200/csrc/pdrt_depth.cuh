@@ -38,7 +38,7 @@ __device__ __forceinline__ double density_at(const Params &P, const float *__res
 
 // The same lookup for the ray bundle of the divergent-depth mode: position, in-box decision and cell index in float64 (the
 // decision a float64 reference takes), interpolation weights and arithmetic in float32.
-__device__ __forceinline__ float density_at_f(const Params &P, const float *__restrict__ rho, double px, double py, double pz)
+__device__ __forceinline__ float density_at_f(const Params &P, const float *__restrict__ rho, const double (&inv_s)[3], double px, double py, double pz)
 {
     const double p[3] = { px, py, pz };
     const double o[3] = { (double)P.ox, (double)P.oy, (double)P.oz }, s[3] = { (double)P.sx, (double)P.sy, (double)P.sz };
@@ -47,9 +47,9 @@ __device__ __forceinline__ float density_at_f(const Params &P, const float *__re
     float t[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        if (p[a] < o[a] - 0.5 * s[a] || p[a] > o[a] + (N[a] - 0.5) * s[a]) return 0.f;
-        const double f = (p[a] - o[a]) / s[a];
-        const double fl = floor(f);
+        if (p[a] < o[a] - 0.5 * s[a] || p[a] > o[a] + (N[a] - 0.5) * s[a]) return 0.f;     // the box decision: in float64, as a reference takes it
+        const double f = (p[a] - o[a]) * inv_s[a];                                          // the cell index may differ by rounding only on a cell
+        const double fl = floor(f);                                                         // boundary, where the interpolant is continuous
         t[a] = (float)(f - fl);
         i0[a] = min(max((int)fl, 0), N[a] - 1);
         i1[a] = min(max((int)fl + 1, 0), N[a] - 1);
@@ -180,30 +180,35 @@ k_fan_depth(Params P, const CpDesc *__restrict__ desc, int n_cp, const float *__
     float *out = fan + (size_t)cp * fan_stride + (size_t)rb * fb.bw + ra;
     const size_t kstride = (size_t)fb.bw * fb.bh;
     const float *zc = zrad + (size_t)cp * P.Nw;
+    const double inv_s[3] = { 1.0 / (double)P.sx, 1.0 / (double)P.sy, 1.0 / (double)P.sz };
+    const double inv_ds = 1.0 / ds, q0 = ((double)P.sid + (double)P.wmin) * inv_ds, dq = (double)P.dw * inv_ds;   // slice k sits at q0 + k dq steps
+    const float inv_dz = 1.f / P.dz;
+    auto term = [&](float z) {                                  // T(z): linear between the table nodes, clamped
+        const float t = z * inv_dz;
+        int n0 = (int)floorf(t);
+        n0 = min(max(n0, 0), P.n_z - 2);
+        const float f = fminf(fmaxf(t - n0, 0.f), 1.f);
+        return (1.f - f) * __ldg(Ttab + n0) + f * __ldg(Ttab + n0 + 1);
+    };
+    auto emit = [&](int kk, double z) {
+        const float Tc = term(zc[kk]);
+        out[(size_t)kk * kstride] = Tc > 0.f ? term((float)z) / Tc : 1.f;
+    };
     double Z = 0.0;
     int k = 0;
-    auto emit = [&](int kk, double z) {
-        const float Tc = depth_term(Ttab, P.n_z, P.dz, zc[kk]);
-        out[(size_t)kk * kstride] = Tc > 0.f ? depth_term(Ttab, P.n_z, P.dz, (float)z) / Tc : 1.f;
-    };
+    // step index m_k = min(floor(q_k), M - 1) of the next slice to emit (slices with q_k <= 0 have depth 0)
+    double qk = q0;
+    int mk = qk > 0.0 ? min((int)floor(qk), M - 1) : -1;
+    auto next_slice = [&]() { ++k; qk = q0 + k * dq; mk = qk > 0.0 ? min((int)floor(qk), M - 1) : -1; };
     // slices in front of the first sample taken: depth 0
-    for (; k < P.Nw; ++k) {
-        const double q = ((double)P.sid + (double)P.wmin + k * (double)P.dw) / ds;
-        if (q > 0.0 && (int)floor(q) >= m) break;
-        emit(k, 0.0);
-    }
+    while (k < P.Nw && mk < m) { emit(k, 0.0); next_slice(); }
     for (; m < m_end && k < P.Nw; ++m) {
         const double t = (m + 0.5) * ds;
-        const double v = (double)density_at_f(P, rho, srcx + t * dx, srcy + t * dy, srcz + t * dz);
-        for (; k < P.Nw; ++k) {                                // slices whose depth falls into this step
-            const double q = ((double)P.sid + (double)P.wmin + k * (double)P.dw) / ds;
-            const int m0 = min((int)floor(q), M - 1);
-            if (m0 != m) break;
-            emit(k, Z + (q - m0) * v * ds);
-        }
+        const double v = (double)density_at_f(P, rho, inv_s, srcx + t * dx, srcy + t * dy, srcz + t * dz);
+        while (k < P.Nw && mk == m) { emit(k, Z + (qk - mk) * v * ds); next_slice(); }     // slices whose depth falls into this step
         Z += v * ds;
     }
-    for (; k < P.Nw; ++k) emit(k, Z);
+    while (k < P.Nw) { emit(k, Z); next_slice(); }
 }
 
 // Multiplies vol (Phivol over S_k, forward; H_b over S_k, adjoint) by the bilinear interpolant (indices clamped to the ray

@@ -1,0 +1,285 @@
+// pdrt_conv_sym.cuh — S4+S5 (forward) and S8 (adjoint): the per-slice lateral convolution (Eq. 8) in
+// ROW-SYMMETRIC form, the single-pass kernel of the path.
+//
+// The pencil kernel is radially symmetric and its pixel-integrated table is built mirrored (R3), so
+// W[C+d][.] = W[C-d][.].  With the row correlation
+//     T_d[r][j] = sum_dj W[C+d][dj] x[r][j + dj - C],        d = 0 .. C,
+// every output row is  out[i] = T_0[i] + sum_{d=1..C} (T_d[i+d] + T_d[i-d]):  a row correlation of INPUT row r is computed
+// once and added to the TWO output rows r-d and r+d.  That is (C+1) KT multiply-adds per input value instead of KT^2, and
+// the loop runs over the rows that hold input (S_k forward: no multiply-adds on the structurally zero rows of the halo;
+// F_k adjoint), not over output rows.
+//
+// One WARP per block, persistent over the work items (control point, slice, chunk along v) like k_conv.  A lane owns a UNIT =
+// (pair of input rows r, r+1) x (8 output columns): the (KT+7)-wide window of both rows sits in registers as float2 (row r,
+// row r+1), the weights come as warp-broadcast LDS.128 of duplicated taps, and one packed FFMA2 per tap and column yields
+// (a_d, b_d) = (T_d[r], T_d[r+1]).  Output rows are accumulated in a shared-memory RING of rows private to the warp; since
+// out[r-d] takes a_d + b_{d+1} and out[r+1+d] takes b_d + a_{d+1}, walking d downwards with the previous (a, b) kept in
+// registers costs ONE read-modify-write of 8 columns per side and step.  In one step the "minus" rows r-d (parity of d) and
+// the "plus" rows r+1+d (other parity) cannot coincide, and the lanes of a group hold distinct (row pair, tile), so a step
+// has no write conflicts; one __syncwarp per step orders the steps.  Rows that no later unit can reach are written to HBM
+// and their ring slots zeroed.  The input rows of the 32 units in flight are staged with cp.async (zero-filled outside the
+// source box), interleaved by row pair so that a window load is LDS.128.
+#pragma once
+#include "pdrt_conv.cuh"
+
+namespace pdrt {
+
+constexpr int SYM_NTFC_MAX = 12;       // widest work item [thread-tiles of 8 columns along v]
+
+// Ring row [floats]: columns 0-3 of every tile first, then columns 4-7 (second plane at 4 nt), so that the two LDS.128 of a
+// read-modify-write hit consecutive 16-byte chunks across the lanes of a row; the pitch is chosen so that the chunks of
+// the next row pair (two rows on) continue where this one ends (modulo the 8 chunks of a wavefront).
+__host__ __device__ __forceinline__ int sym_out_pitch(int nt)
+{
+    int p = 8 * nt;
+    const int want = (nt + (nt & 1)) & 7;
+    while (((p >> 1) & 7) != want) p += 4;
+    return p;
+}
+// most row pairs that 32 consecutive units of `nt` tiles per pair can touch
+__host__ __device__ __forceinline__ int sym_pairs_per_group(int nt) { return (30 + nt) / nt + 1; }
+// 16-byte chunks (2 columns x 2 rows) per staged row pair: the windows of nt tiles, rounded to the 8-chunk swizzle period
+__host__ __device__ __forceinline__ int sym_in_chunks(int nt, int c) { return (4 * nt + c + 7) & ~7; }
+inline int sym_out_floats(int kt)
+{
+    const int c = (kt - 1) / 2;
+    int best = 0;
+    for (int nt = 1; nt <= SYM_NTFC_MAX; ++nt) best = best > (2 * sym_pairs_per_group(nt) + 2 * c) * sym_out_pitch(nt) ? best : (2 * sym_pairs_per_group(nt) + 2 * c) * sym_out_pitch(nt);
+    return best;
+}
+inline int sym_in_floats(int kt)
+{
+    const int c = (kt - 1) / 2;
+    int best = 0;
+    for (int nt = 1; nt <= SYM_NTFC_MAX; ++nt) best = best > sym_pairs_per_group(nt) * sym_in_chunks(nt, c) * 4 ? best : sym_pairs_per_group(nt) * sym_in_chunks(nt, c) * 4;
+    return best;
+}
+inline size_t sym_smem_bytes(int kt)
+{
+    const int c = (kt - 1) / 2, kq = (kt + 1) / 2;
+    return sizeof(float) * ((size_t)4 * (c + 1) * kq + sym_in_floats(kt) + sym_out_floats(kt));
+}
+
+__device__ __forceinline__ int pmod(int a, int m) { const int r = a % m; return r < 0 ? r + m : r; }
+
+template <int KT, bool ADJ>
+__global__ void __launch_bounds__(CONV_THREADS)
+k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
+           const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
+           int *item_counter, WorkCounters *wc, int in_floats, int out_floats)
+{
+    constexpr int C = (KT - 1) / 2;
+    constexpr int KP = (KT + 3) & ~3;                 // row pitch of the table image [floats]
+    constexpr int KQ = (KT + 1) / 2;                  // float4 (two duplicated taps) per weight row
+    constexpr int XW = KT + 7;                        // register window along v [columns], even
+    constexpr int NXQ = XW / 2;                       // LDS.128 per window (2 columns x 2 rows each)
+    constexpr int MCX = (8 * SYM_NTFC_MAX + 2 * C + 31) / 32;    // staged columns per lane and row
+    extern __shared__ float4 smem4[];
+    float4 *Wd = smem4;                               // [C+1 (d)][KQ]: (w[2q], w[2q], w[2q+1], w[2q+1]) of kernel row C+d
+    float4 *xin4 = smem4 + (C + 1) * KQ;              // [pair][chunk]: (x[r][c], x[r+1][c], x[r][c+1], x[r+1][c+1]), chunks swizzled
+    float *oring = reinterpret_cast<float *>(xin4) + in_floats;   // [slot][pitch]: ring of output rows, all zero between uses
+    const unsigned xin_s = (unsigned)__cvta_generic_to_shared(xin4);
+    const int lane = threadIdx.x;
+    const int total = tile_base[n_cp];
+    const int CHk = min(P.CH, C);                     // rows C+d with d > CH of an embedded smaller kernel are zero
+    int slot_hint = 0;
+    unsigned long long macs = 0ull;                   // multiply-adds of this lane (work counter)
+
+    for (int e = lane; e < out_floats / 4; e += 32) reinterpret_cast<float4 *>(oring)[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncwarp();
+
+    for (;;) {
+        int item = 0;
+        if (lane == 0) item = atomicAdd(item_counter, 1);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= total) break;
+        while (slot_hint + 1 < n_cp && item >= tile_base[slot_hint + 1]) ++slot_hint;   // items arrive in increasing order
+        const int slot = slot_hint, cp = cp0 + slot;
+        const CpDesc d = desc[cp];
+        const int local = item - tile_base[slot];
+        const int k = local / d.ncf, cf = local - k * d.ncf;
+        const SliceBox S = slice_support(P, d, k);
+        if (box_empty(S)) continue;
+        const SliceBox F = dilate(P, S, P.CH);
+        const SliceBox A = ADJ ? S : F;               // outputs to compute
+        const SliceBox B = ADJ ? F : S;               // source box of the input (zero outside)
+        // tiles of the chunk along v
+        const int ctf0 = cf * d.ntfc, ctf1 = min(d.ntf, ctf0 + d.ntfc);
+        int atf0 = max(ctf0, (A.v0 - d.rj0) / RF), atf1 = min(ctf1 - 1, (A.v1 - d.rj0) / RF);
+        if (atf0 > atf1) continue;
+        int nt = atf1 - atf0 + 1, av0 = d.rj0 + atf0 * RF;
+        if (ADJ && d.ncf == 1) { av0 = A.v0 & ~1; nt = (A.v1 - av0) / RF + 1; }      // adjoint outputs are read back on S_k only
+        // rows: input row pairs, output rows held in the ring (T), output rows written to HBM (wu)
+        const int in_u0 = B.u0, in_u1 = B.u1, npair = (in_u1 - in_u0 + 2) >> 1;
+        int wu0, wu1, Tu0, Tu1;
+        if (ADJ) { wu0 = Tu0 = S.u0; wu1 = Tu1 = S.u1; }
+        else {      // the thread-tile rows that intersect F_k (wbox of k_fluence), clipped to the beam grid
+            wu0 = d.ri0 + (F.u0 - d.ri0) / RS * RS;
+            wu1 = min(P.Nu - 1, d.ri0 + min(d.nts - 1, (F.u1 - d.ri0) / RS) * RS + RS - 1);
+            Tu0 = min(wu0, in_u0 - CHk); Tu1 = max(wu1, in_u0 + 2 * npair - 1 + CHk);
+        }
+        const int pitch = sym_out_pitch(nt), hp = 4 * nt, R = out_floats / pitch;
+        const int PPc = sym_in_chunks(nt, C);
+        const int ncols = 8 * nt + 2 * C;
+        const long long slice_off = (long long)slot * P.stride_cp + (long long)k * d.pu * d.pv;
+        const float *sbase = in + slice_off;
+        float *oslice = out + slice_off;
+
+        {   // S4: rows C .. C+CHk of the slice kernel = lerp of the table in radiological depth, taps duplicated for FFMA2
+            const float tz = zrad[(size_t)cp * P.Nw + k] / P.dz;
+            int n0 = (int)floorf(tz);
+            n0 = min(max(n0, 0), P.n_z - 2);
+            const float f = fminf(fmaxf(tz - n0, 0.f), 1.f);
+            const float *w0 = wtab + (size_t)n0 * KT * KP + C * KP, *w1 = w0 + KT * KP;
+            for (int e = lane; e < (CHk + 1) * KQ; e += 32) {
+                const int dd = e / KQ, q = e - dd * KQ;
+                const int o = dd * KP + 2 * q;
+                const float wa = (1.f - f) * __ldg(w0 + o) + f * __ldg(w1 + o);
+                const float wb = 2 * q + 1 < KT ? (1.f - f) * __ldg(w0 + o + 1) + f * __ldg(w1 + o + 1) : 0.f;
+                Wd[dd * KQ + q] = make_float4(wa, wa, wb, wb);
+            }
+        }
+        // column terms of the staged rows: source offset, swizzled destination, validity (once per item)
+        int joff[MCX];
+        unsigned doff[MCX];
+        bool cex[MCX], cin[MCX];
+#pragma unroll
+        for (int m = 0; m < MCX; ++m) {
+            const int c = lane + 32 * m, j = av0 - C + c, q = c >> 1;
+            cex[m] = c < ncols;
+            cin[m] = cex[m] && j >= B.v0 && j <= B.v1;
+            joff[m] = cin[m] ? j - d.rj0 : 0;
+            doff[m] = 16u * (unsigned)(q ^ ((q >> 3) & 7)) + 8u * (unsigned)(c & 1);
+        }
+        // flush geometry: lanes over the 16-byte (forward) / 8-byte (adjoint) chunks of a row
+        const int nchunk = ADJ ? 4 * nt : 2 * nt;
+        const int rpi = nchunk >= 32 ? 1 : 32 / nchunk;
+        const int lrow = nchunk >= 32 ? 0 : lane / nchunk, lch = nchunk >= 32 ? lane : lane - lrow * nchunk;
+        const int room = d.pv - (av0 - d.rj0);            // columns of the region from av0 on
+        auto flush = [&](int a, int b) {                   // rows [a, b): ring -> HBM (inside the written box), slots back to zero
+            for (int i0 = a; i0 < b; i0 += rpi) {
+                const int i = i0 + lrow;
+                if (lrow < rpi && i < b) {
+                    float *rowp = oring + pmod(i - Tu0, R) * pitch;
+                    const bool wr = i >= wu0 && i <= wu1;
+                    float *orow = oslice + (long long)(i - d.ri0) * d.pv + (av0 - d.rj0);
+                    for (int ch = lch; ch < nchunk; ch += 32) {
+                        if (ADJ) {
+                            const int c = 2 * ch;
+                            float2 *p = reinterpret_cast<float2 *>(rowp + ((c >> 2) & 1) * hp + 4 * (c >> 3) + (c & 3));
+                            const float2 v = *p;
+                            *p = make_float2(0.f, 0.f);
+                            if (wr && c + 2 <= room) *reinterpret_cast<float2 *>(orow + c) = v;
+                        } else {
+                            float4 *p = reinterpret_cast<float4 *>(rowp + (ch & 1) * hp + 4 * (ch >> 1));
+                            const float4 v = *p;
+                            *p = make_float4(0.f, 0.f, 0.f, 0.f);
+                            if (wr) *reinterpret_cast<float4 *>(orow + 4 * ch) = v;
+                        }
+                    }
+                }
+            }
+        };
+
+        const int n_units = npair * nt;
+        int flushed = Tu0;                                 // rows below are final and written
+        __syncwarp();                                      // Wd is complete; the previous item has left the ring zeroed
+        for (int u0 = 0; u0 < n_units; u0 += 32) {
+            const int p_lo = u0 / nt, p_hi = (min(n_units, u0 + 32) - 1) / nt;
+            const int r_lo = in_u0 + 2 * p_lo, r_hi = in_u0 + 2 * p_hi;
+            {   // rows that no unit from here on reaches
+                const int lo = min(max(r_lo - CHk, Tu0), Tu1 + 1);
+                if (lo > flushed) { flush(flushed, lo); flushed = lo; }
+            }
+            // stage the input rows of the group's pairs
+            for (int rl = 0; rl < 2 * (p_hi - p_lo + 1); ++rl) {
+                const int i = r_lo + rl;
+                const bool rin = i <= in_u1;
+                const float *srow = sbase + (long long)(i - d.ri0) * d.pv;
+                const unsigned drow = xin_s + 16u * (unsigned)((rl >> 1) * PPc) + 4u * (unsigned)(rl & 1);
+#pragma unroll
+                for (int m = 0; m < MCX; ++m)
+                    if (cex[m]) {
+                        const bool ok = rin && cin[m];
+                        cp_async_4(drow + doff[m], ok ? srow + joff[m] : sbase, ok ? 4 : 0);
+                    }
+            }
+            cp_async_wait_all();
+            __syncwarp();
+
+            const int u = u0 + lane;
+            const bool active = u < n_units;
+            const int p = active ? u / nt : p_lo, t = active ? u - p * nt : 0;
+            const int r = in_u0 + 2 * p;
+            float2 xx[XW];                                 // (x[r][c], x[r+1][c]) of window column c
+            {
+                const float4 *xw = xin4 + (p - p_lo) * PPc;
+#pragma unroll
+                for (int mm = 0; mm < NXQ; ++mm) {
+                    const int q = 4 * t + mm;
+                    const float4 v = xw[q ^ ((q >> 3) & 7)];
+                    xx[2 * mm] = make_float2(v.x, v.y); xx[2 * mm + 1] = make_float2(v.z, v.w);
+                }
+            }
+            // steps whose two target rows lie outside the held rows for every unit of the group are skipped (adjoint halo)
+            int d_lo = 0;
+            if (ADJ) {
+                if (r_hi + 1 < Tu0) d_lo = Tu0 - r_hi - 1;
+                else if (r_lo > Tu1) d_lo = r_lo - Tu1;
+            }
+            float pa[RF], pb[RF];                          // (a, b) of the previous step (d + 1)
+#pragma unroll
+            for (int c = 0; c < RF; ++c) { pa[c] = 0.f; pb[c] = 0.f; }
+            int rowm = r - CHk, rowp = r + 1 + CHk;
+            int sm = pmod(rowm - Tu0, R), sp = pmod(rowp - Tu0, R);
+            const float4 *wrow = Wd + CHk * KQ;
+            if (active && CHk >= d_lo) macs += (unsigned long long)(CHk - d_lo + 1) * (KT * RF * 2);
+#pragma unroll 1
+            for (int dd = CHk; dd >= d_lo; --dd) {
+                if (active) {
+                    float2 acc2[RF];
+#pragma unroll
+                    for (int c = 0; c < RF; ++c) acc2[c] = make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int q = 0; q < KQ; ++q) {
+                        const float4 w = wrow[q];
+                        const float2 wa = make_float2(w.x, w.y), wb = make_float2(w.z, w.w);
+#pragma unroll
+                        for (int c = 0; c < RF; ++c) acc2[c] = __ffma2_rn(xx[c + 2 * q], wa, acc2[c]);
+                        if (2 * q + 1 < KT) {
+#pragma unroll
+                            for (int c = 0; c < RF; ++c) acc2[c] = __ffma2_rn(xx[c + 2 * q + 1], wb, acc2[c]);
+                        }
+                    }
+                    if (!ADJ || (rowm >= Tu0 && rowm <= Tu1)) {       // out[r - d] += a_d + b_{d+1}
+                        float4 *o = reinterpret_cast<float4 *>(oring + sm * pitch + 4 * t), *o2 = reinterpret_cast<float4 *>(oring + sm * pitch + hp + 4 * t);
+                        float4 v0 = *o, v1 = *o2;
+                        v0.x += acc2[0].x + pb[0]; v0.y += acc2[1].x + pb[1]; v0.z += acc2[2].x + pb[2]; v0.w += acc2[3].x + pb[3];
+                        v1.x += acc2[4].x + pb[4]; v1.y += acc2[5].x + pb[5]; v1.z += acc2[6].x + pb[6]; v1.w += acc2[7].x + pb[7];
+                        *o = v0; *o2 = v1;
+                    }
+                    if (!ADJ || (rowp >= Tu0 && rowp <= Tu1)) {       // out[r + 1 + d] += b_d + a_{d+1}
+                        float4 *o = reinterpret_cast<float4 *>(oring + sp * pitch + 4 * t), *o2 = reinterpret_cast<float4 *>(oring + sp * pitch + hp + 4 * t);
+                        float4 v0 = *o, v1 = *o2;
+                        v0.x += acc2[0].y + pa[0]; v0.y += acc2[1].y + pa[1]; v0.z += acc2[2].y + pa[2]; v0.w += acc2[3].y + pa[3];
+                        v1.x += acc2[4].y + pa[4]; v1.y += acc2[5].y + pa[5]; v1.z += acc2[6].y + pa[6]; v1.w += acc2[7].y + pa[7];
+                        *o = v0; *o2 = v1;
+                    }
+#pragma unroll
+                    for (int c = 0; c < RF; ++c) { pa[c] = acc2[c].x; pb[c] = acc2[c].y; }
+                }
+                wrow -= KQ;
+                ++rowm; --rowp;
+                sm = sm + 1 == R ? 0 : sm + 1;
+                sp = sp == 0 ? R - 1 : sp - 1;
+                __syncwarp();                              // the rows of this step are visible to the next one
+            }
+        }
+        __syncwarp();
+        flush(flushed, Tu1 + 1);
+        __syncwarp();                                      // the next item overwrites Wd and the staged rows
+    }
+    if (macs) atomicAdd(reinterpret_cast<unsigned long long *>(ADJ ? &wc->macs_adj : &wc->macs_fwd), macs);
+}
+
+}  // namespace pdrt

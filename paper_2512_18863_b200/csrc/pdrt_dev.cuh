@@ -48,6 +48,8 @@ struct Params {
     int n_z;
     float dz;
     int tile_floats;                     // conv input-tile budget in shared memory [floats]
+    int ntfc_max;                        // widest conv work item [thread-tiles along v]: NTFC_MAX (k_conv) or SYM_NTFC_MAX (k_conv_sym)
+    int conv_sym;                        // 1: the row-symmetric single-pass kernel runs (it counts its own multiply-adds)
     // fluence corrections
     int Tu_max, Tv_max;                  // largest Gaussian half-widths along u / v
     // ray marcher

@@ -13,6 +13,7 @@
 
 #include "../../include/pdrt.h"
 #include "pdrt_conv.cuh"
+#include "pdrt_conv_sym.cuh"
 #include "pdrt_depth.cuh"
 #include "pdrt_dev.cuh"
 #include "pdrt_fluence.cuh"
@@ -35,6 +36,13 @@ int conv_single_max()
 {
     if (const char *v = std::getenv("PDRT_CONV_SINGLE_MAX")) { const int m = std::atoi(v); if (m >= 3 && m <= 63) return m; }
     return 55;       // measured on c4: one pass wins up to 55 taps, 3 x 3 passes of 21 from 63 on
+}
+// The single-pass convolution runs in row-symmetric form (k_conv_sym) unless PDRT_CONV_LEGACY=1 asks for the output-stationary
+// kernel (k_conv), which also serves the sub-kernel passes of a split (their off-centre blocks are not symmetric by themselves).
+bool conv_legacy()
+{
+    const char *v = std::getenv("PDRT_CONV_LEGACY");
+    return v && std::atoi(v) != 0;
 }
 int compiled_size(int k)
 {
@@ -108,6 +116,7 @@ struct pdrt_engine {
     bool last_backward = false;
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
+    int conv_sym_per_sm[2][64] = {};     // the same for k_conv_sym, by [adjoint][KT]
     int conv_per_sm[2][2][2][64] = {};   // resident conv blocks per SM on THIS engine's device, by [adjoint][copy width - 1][multi-pass][KT]; 0 = not queried yet
     DevBuf<float> coll;               // collimator angles [coll_n] set by pdrt_set_collimator (coll_n = 0: none)
     int coll_n = 0;
@@ -236,6 +245,8 @@ int build_kernel_table(pdrt_engine *e, int k)
     e->P.NB = nb;
     e->P.CH = c;
     e->P.tile_floats = tile_floats_for(kt);
+    e->P.conv_sym = (nb == 1 && !conv_legacy()) ? 1 : 0;
+    e->P.ntfc_max = e->P.conv_sym ? SYM_NTFC_MAX : NTFC_MAX;
     return PDRT_OK;
 }
 
@@ -257,10 +268,28 @@ int launch_conv_pass(pdrt_engine *e, int cp0, int n, const float *wtab, const fl
     CU(e, cudaGetLastError());
     return PDRT_OK;
 }
+template <int KT, bool ADJ>
+int launch_conv_sym(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
+{
+    int &per_sm = e->conv_sym_per_sm[ADJ ? 1 : 0][KT];
+    const size_t smem = sym_smem_bytes(KT);
+    if (per_sm == 0) {
+        CU(e, cudaFuncSetAttribute(k_conv_sym<KT, ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int n_res = 0;
+        CU(e, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n_res, k_conv_sym<KT, ADJ>, CONV_THREADS, smem));
+        per_sm = n_res < 1 ? 1 : n_res;
+    }
+    e->conv_grid = e->sm_count * per_sm;              // persistent grid: a multiple of the SM count
+    k_conv_sym<KT, ADJ><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->zrad.p, e->wtab.p, in, out,
+                                                                  e->tile_base.p + n + 1, e->counters.p, sym_in_floats(KT), sym_out_floats(KT));
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
 // All NB x NB passes of one convolution, the centre block first (it writes; the others accumulate).  Returns the launches made.
 template <int KT, bool ADJ>
 int launch_conv_t(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
 {
+    if (e->P.conv_sym) return launch_conv_sym<KT, ADJ>(e, cp0, n, in, out, st);
     const int nb = e->P.NB, nbh = (nb - 1) / 2, C = (KT - 1) / 2;
     const size_t blk = (size_t)e->P.n_z * KT * ((KT + 3) & ~3);
     bool first = true;

@@ -93,7 +93,7 @@ __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg,
     d.pv = ((v1 - d.rj0 + 1) + RF - 1) / RF * RF;
     d.ntf = d.pv / RF;
     d.nts = d.pu / RS;
-    d.ncf = (d.ntf + NTFC_MAX - 1) / NTFC_MAX;
+    d.ncf = (d.ntf + P.ntfc_max - 1) / P.ntfc_max;
     d.ntfc = (d.ntf + d.ncf - 1) / d.ncf;
     // conv work items: one per slice and chunk along v (the warp that takes an item walks its active thread-tiles)
     d.n_items = d.n_items_adj = P.Nw * d.ncf;
@@ -151,8 +151,9 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
     __syncthreads();
     if (tid == 0) {
         d.support_vox = cnt[0]; d.footprint_vox = cnt[1];
-        d.macs_fwd = cnt[2] * (unsigned long long)(RF * RS * P.KT * P.KT);
-        d.macs_adj = cnt[3] * (unsigned long long)(RF * RS * P.KT * P.KT);
+        // k_conv: KT^2 multiply-adds per output of an active thread-tile; k_conv_sym counts what it executes itself
+        d.macs_fwd = P.conv_sym ? 0ull : cnt[2] * (unsigned long long)(RF * RS * P.KT * P.KT);
+        d.macs_adj = P.conv_sym ? 0ull : cnt[3] * (unsigned long long)(RF * RS * P.KT * P.KT);
         desc[cp] = d;
     }
     if (empty) return;

@@ -24,34 +24,27 @@
 
 namespace pdrt {
 
-constexpr int SYM_NTFC_MAX = 12;       // widest work item [thread-tiles of 8 columns along v]
+constexpr int SYM_NTFC_MAX = 10;       // widest work item [thread-tiles of 8 columns along v]
 
 // Ring row [floats]: columns 0-3 of every tile first, then columns 4-7 (second plane at 4 nt), so that the two LDS.128 of a
-// read-modify-write hit consecutive 16-byte chunks across the lanes of a row; the pitch is chosen so that the chunks of
-// the next row pair (two rows on) continue where this one ends (modulo the 8 chunks of a wavefront).
-__host__ __device__ __forceinline__ int sym_out_pitch(int nt)
-{
-    int p = 8 * nt;
-    const int want = (nt + (nt & 1)) & 7;
-    while (((p >> 1) & 7) != want) p += 4;
-    return p;
-}
-// most row pairs that 32 consecutive units of `nt` tiles per pair can touch
-__host__ __device__ __forceinline__ int sym_pairs_per_group(int nt) { return (30 + nt) / nt + 1; }
+// read-modify-write hit consecutive 16-byte chunks across the lanes of a row.
+__host__ __device__ __forceinline__ int sym_out_pitch(int nt) { return 8 * nt; }
+// row pairs per group of units: as many whole-or-part pairs as 32 units span, at most 8
+__host__ __device__ __forceinline__ int sym_max_pairs(int nt) { return (32 + nt - 1) / nt < 8 ? (32 + nt - 1) / nt : 8; }
 // 16-byte chunks (2 columns x 2 rows) per staged row pair: the windows of nt tiles, rounded to the 8-chunk swizzle period
 __host__ __device__ __forceinline__ int sym_in_chunks(int nt, int c) { return (4 * nt + c + 7) & ~7; }
 inline int sym_out_floats(int kt)
 {
     const int c = (kt - 1) / 2;
     int best = 0;
-    for (int nt = 1; nt <= SYM_NTFC_MAX; ++nt) best = best > (2 * sym_pairs_per_group(nt) + 2 * c) * sym_out_pitch(nt) ? best : (2 * sym_pairs_per_group(nt) + 2 * c) * sym_out_pitch(nt);
+    for (int nt = 1; nt <= SYM_NTFC_MAX; ++nt) best = std::max(best, (2 * sym_max_pairs(nt) + 2 * c) * sym_out_pitch(nt));
     return best;
 }
 inline int sym_in_floats(int kt)
 {
     const int c = (kt - 1) / 2;
     int best = 0;
-    for (int nt = 1; nt <= SYM_NTFC_MAX; ++nt) best = best > sym_pairs_per_group(nt) * sym_in_chunks(nt, c) * 4 ? best : sym_pairs_per_group(nt) * sym_in_chunks(nt, c) * 4;
+    for (int nt = 1; nt <= SYM_NTFC_MAX; ++nt) best = std::max(best, sym_max_pairs(nt) * sym_in_chunks(nt, c) * 4);
     return best;
 }
 inline size_t sym_smem_bytes(int kt)
@@ -62,8 +55,53 @@ inline size_t sym_smem_bytes(int kt)
 
 __device__ __forceinline__ int pmod(int a, int m) { const int r = a % m; return r < 0 ? r + m : r; }
 
+// One step d of a unit: acc = (a_d, b_d) from the window and weight row d; out[r-d] += a_d + b_{d+1}, out[r+1+d] += b_d + a_{d+1},
+// with (a_{d+1}, b_{d+1}) = prev.  `om` / `op` point at the unit's 8 columns (first plane) of the two ring rows; null: row not held.
+template <int KT>
+__device__ __forceinline__ void sym_step(const float2 (&xx)[KT + 7], const float4 *__restrict__ wrow, float2 (&acc)[RF], const float2 (&prev)[RF],
+                                         float *om, float *op, int hp)
+{
+    constexpr int KQ = (KT + 1) / 2;
+    {
+        const float4 w = wrow[0];
+        const float2 wa = make_float2(w.x, w.y), wb = make_float2(w.z, w.w);
+#pragma unroll
+        for (int c = 0; c < RF; ++c) acc[c] = __fmul2_rn(xx[c], wa);
+#pragma unroll
+        for (int c = 0; c < RF; ++c) acc[c] = __ffma2_rn(xx[c + 1], wb, acc[c]);
+    }
+#pragma unroll
+    for (int q = 1; q < KQ; ++q) {
+        const float4 w = wrow[q];
+        const float2 wa = make_float2(w.x, w.y), wb = make_float2(w.z, w.w);
+#pragma unroll
+        for (int c = 0; c < RF; ++c) acc[c] = __ffma2_rn(xx[c + 2 * q], wa, acc[c]);
+        if (2 * q + 1 < KT) {
+#pragma unroll
+            for (int c = 0; c < RF; ++c) acc[c] = __ffma2_rn(xx[c + 2 * q + 1], wb, acc[c]);
+        }
+    }
+    if (om) {
+        float4 *o = reinterpret_cast<float4 *>(om), *o2 = reinterpret_cast<float4 *>(om + hp);
+        float4 v0 = *o, v1 = *o2;
+        v0.x += acc[0].x + prev[0].y; v0.y += acc[1].x + prev[1].y; v0.z += acc[2].x + prev[2].y; v0.w += acc[3].x + prev[3].y;
+        v1.x += acc[4].x + prev[4].y; v1.y += acc[5].x + prev[5].y; v1.z += acc[6].x + prev[6].y; v1.w += acc[7].x + prev[7].y;
+        *o = v0; *o2 = v1;
+    }
+    if (op) {
+        float4 *o = reinterpret_cast<float4 *>(op), *o2 = reinterpret_cast<float4 *>(op + hp);
+        float4 v0 = *o, v1 = *o2;
+        v0.x += acc[0].y + prev[0].x; v0.y += acc[1].y + prev[1].x; v0.z += acc[2].y + prev[2].x; v0.w += acc[3].y + prev[3].x;
+        v1.x += acc[4].y + prev[4].x; v1.y += acc[5].y + prev[5].x; v1.z += acc[6].y + prev[6].x; v1.w += acc[7].y + prev[7].x;
+        *o = v0; *o2 = v1;
+    }
+}
+
+// resident warps per SM the register allocation aims at (the window takes 2 (KT + 7) registers)
+constexpr int sym_min_blocks(int kt) { return kt <= 25 ? 14 : kt <= 31 ? 11 : 8; }
+
 template <int KT, bool ADJ>
-__global__ void __launch_bounds__(CONV_THREADS)
+__global__ void __launch_bounds__(CONV_THREADS, sym_min_blocks(KT))
 k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
            const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
            int *item_counter, WorkCounters *wc, int in_floats, int out_floats)
@@ -95,35 +133,36 @@ k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const i
         if (item >= total) break;
         while (slot_hint + 1 < n_cp && item >= tile_base[slot_hint + 1]) ++slot_hint;   // items arrive in increasing order
         const int slot = slot_hint, cp = cp0 + slot;
-        const CpDesc d = desc[cp];
+        const CpDesc &d = desc[cp];
+        const int ncf = d.ncf, ntfc = d.ntfc, ntf = d.ntf, nts = d.nts, ri0 = d.ri0, rj0 = d.rj0, pu = d.pu, pv = d.pv;
         const int local = item - tile_base[slot];
-        const int k = local / d.ncf, cf = local - k * d.ncf;
+        const int k = local / ncf, cf = local - k * ncf;
         const SliceBox S = slice_support(P, d, k);
         if (box_empty(S)) continue;
         const SliceBox F = dilate(P, S, P.CH);
         const SliceBox A = ADJ ? S : F;               // outputs to compute
         const SliceBox B = ADJ ? F : S;               // source box of the input (zero outside)
         // tiles of the chunk along v
-        const int ctf0 = cf * d.ntfc, ctf1 = min(d.ntf, ctf0 + d.ntfc);
-        int atf0 = max(ctf0, (A.v0 - d.rj0) / RF), atf1 = min(ctf1 - 1, (A.v1 - d.rj0) / RF);
+        const int ctf0 = cf * ntfc, ctf1 = min(ntf, ctf0 + ntfc);
+        const int atf0 = max(ctf0, (A.v0 - rj0) / RF), atf1 = min(ctf1 - 1, (A.v1 - rj0) / RF);
         if (atf0 > atf1) continue;
-        int nt = atf1 - atf0 + 1, av0 = d.rj0 + atf0 * RF;
-        if (ADJ && d.ncf == 1) { av0 = A.v0 & ~1; nt = (A.v1 - av0) / RF + 1; }      // adjoint outputs are read back on S_k only
+        int nt = atf1 - atf0 + 1, av0 = rj0 + atf0 * RF;
+        if (ADJ && ncf == 1) { av0 = A.v0 & ~1; nt = (A.v1 - av0) / RF + 1; }      // adjoint outputs are read back on S_k only
         // rows: input row pairs, output rows held in the ring (T), output rows written to HBM (wu)
         const int in_u0 = B.u0, in_u1 = B.u1, npair = (in_u1 - in_u0 + 2) >> 1;
         int wu0, wu1, Tu0, Tu1;
         if (ADJ) { wu0 = Tu0 = S.u0; wu1 = Tu1 = S.u1; }
         else {      // the thread-tile rows that intersect F_k (wbox of k_fluence), clipped to the beam grid
-            wu0 = d.ri0 + (F.u0 - d.ri0) / RS * RS;
-            wu1 = min(P.Nu - 1, d.ri0 + min(d.nts - 1, (F.u1 - d.ri0) / RS) * RS + RS - 1);
+            wu0 = ri0 + (F.u0 - ri0) / RS * RS;
+            wu1 = min(P.Nu - 1, ri0 + min(nts - 1, (F.u1 - ri0) / RS) * RS + RS - 1);
             Tu0 = min(wu0, in_u0 - CHk); Tu1 = max(wu1, in_u0 + 2 * npair - 1 + CHk);
         }
         const int pitch = sym_out_pitch(nt), hp = 4 * nt, R = out_floats / pitch;
-        const int PPc = sym_in_chunks(nt, C);
+        const int PPc = sym_in_chunks(nt, C), maxp = sym_max_pairs(nt);
         const int ncols = 8 * nt + 2 * C;
-        const long long slice_off = (long long)slot * P.stride_cp + (long long)k * d.pu * d.pv;
+        const long long slice_off = (long long)slot * P.stride_cp + (long long)k * pu * pv;
         const float *sbase = in + slice_off;
-        float *oslice = out + slice_off;
+        float *oslice = out + slice_off + (av0 - rj0) - (long long)ri0 * pv;       // row i, column av0 + c at oslice + i pv + c
 
         {   // S4: rows C .. C+CHk of the slice kernel = lerp of the table in radiological depth, taps duplicated for FFMA2
             const float tz = zrad[(size_t)cp * P.Nw + k] / P.dz;
@@ -139,30 +178,21 @@ k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const i
                 Wd[dd * KQ + q] = make_float4(wa, wa, wb, wb);
             }
         }
-        // column terms of the staged rows: source offset, swizzled destination, validity (once per item)
-        int joff[MCX];
-        unsigned doff[MCX];
-        bool cex[MCX], cin[MCX];
-#pragma unroll
-        for (int m = 0; m < MCX; ++m) {
-            const int c = lane + 32 * m, j = av0 - C + c, q = c >> 1;
-            cex[m] = c < ncols;
-            cin[m] = cex[m] && j >= B.v0 && j <= B.v1;
-            joff[m] = cin[m] ? j - d.rj0 : 0;
-            doff[m] = 16u * (unsigned)(q ^ ((q >> 3) & 7)) + 8u * (unsigned)(c & 1);
-        }
         // flush geometry: lanes over the 16-byte (forward) / 8-byte (adjoint) chunks of a row
         const int nchunk = ADJ ? 4 * nt : 2 * nt;
         const int rpi = nchunk >= 32 ? 1 : 32 / nchunk;
         const int lrow = nchunk >= 32 ? 0 : lane / nchunk, lch = nchunk >= 32 ? lane : lane - lrow * nchunk;
-        const int room = d.pv - (av0 - d.rj0);            // columns of the region from av0 on
-        auto flush = [&](int a, int b) {                   // rows [a, b): ring -> HBM (inside the written box), slots back to zero
-            for (int i0 = a; i0 < b; i0 += rpi) {
+        const int room = pv - (av0 - rj0);                 // columns of the region from av0 on
+        int flushed = Tu0, fslot = 0;                      // rows below `flushed` are final and written; ring slot of row `flushed`
+        auto flush = [&](int b) {                          // rows [flushed, b): ring -> HBM (inside the written box), slots back to zero
+            for (int i0 = flushed; i0 < b; i0 += rpi) {
                 const int i = i0 + lrow;
                 if (lrow < rpi && i < b) {
-                    float *rowp = oring + pmod(i - Tu0, R) * pitch;
+                    int sl = fslot + (i - flushed);
+                    while (sl >= R) sl -= R;
+                    float *rowp = oring + sl * pitch;
                     const bool wr = i >= wu0 && i <= wu1;
-                    float *orow = oslice + (long long)(i - d.ri0) * d.pv + (av0 - d.rj0);
+                    float *orow = oslice + (long long)i * pv;
                     for (int ch = lch; ch < nchunk; ch += 32) {
                         if (ADJ) {
                             const int c = 2 * ch;
@@ -179,36 +209,50 @@ k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const i
                     }
                 }
             }
+            fslot += b - flushed;
+            while (fslot >= R) fslot -= R;
+            flushed = b;
         };
 
         const int n_units = npair * nt;
-        int flushed = Tu0;                                 // rows below are final and written
         __syncwarp();                                      // Wd is complete; the previous item has left the ring zeroed
-        for (int u0 = 0; u0 < n_units; u0 += 32) {
-            const int p_lo = u0 / nt, p_hi = (min(n_units, u0 + 32) - 1) / nt;
+        for (int u0 = 0; u0 < n_units;) {
+            const int p_lo = u0 / nt;
+            const int u1 = min(min(n_units, u0 + 32), (p_lo + maxp) * nt);       // units [u0, u1) of at most `maxp` row pairs
+            const int p_hi = (u1 - 1) / nt;
             const int r_lo = in_u0 + 2 * p_lo, r_hi = in_u0 + 2 * p_hi;
             {   // rows that no unit from here on reaches
                 const int lo = min(max(r_lo - CHk, Tu0), Tu1 + 1);
-                if (lo > flushed) { flush(flushed, lo); flushed = lo; }
+                if (lo > flushed) flush(lo);
             }
-            // stage the input rows of the group's pairs
-            for (int rl = 0; rl < 2 * (p_hi - p_lo + 1); ++rl) {
-                const int i = r_lo + rl;
-                const bool rin = i <= in_u1;
-                const float *srow = sbase + (long long)(i - d.ri0) * d.pv;
-                const unsigned drow = xin_s + 16u * (unsigned)((rl >> 1) * PPc) + 4u * (unsigned)(rl & 1);
+            {   // stage the input rows of the group's pairs: per-lane column terms, then one pass over the rows
+                const float *sp[MCX];
+                unsigned dp[MCX];
+                int csz[MCX];
 #pragma unroll
-                for (int m = 0; m < MCX; ++m)
-                    if (cex[m]) {
-                        const bool ok = rin && cin[m];
-                        cp_async_4(drow + doff[m], ok ? srow + joff[m] : sbase, ok ? 4 : 0);
+                for (int m = 0; m < MCX; ++m) {
+                    const int c = lane + 32 * m, j = av0 - C + c, q = c >> 1;
+                    const bool cin = j >= B.v0 && j <= B.v1;
+                    csz[m] = c < ncols ? (cin ? 4 : 0) : -1;
+                    sp[m] = sbase + (long long)(r_lo - ri0) * pv + (cin ? j - rj0 : 0);
+                    dp[m] = xin_s + 16u * (unsigned)(q ^ ((q >> 3) & 7)) + 8u * (unsigned)(c & 1);
+                }
+                const int nrow = 2 * (p_hi - p_lo + 1);
+                for (int rl = 0; rl < nrow; ++rl) {
+                    const bool rin = r_lo + rl <= in_u1;   // only the second row of the last pair can lie outside
+                    const unsigned ro = 16u * (unsigned)((rl >> 1) * PPc) + 4u * (unsigned)(rl & 1);
+#pragma unroll
+                    for (int m = 0; m < MCX; ++m) {
+                        if (csz[m] >= 0) cp_async_4(dp[m] + ro, rin ? sp[m] : sbase, rin ? csz[m] : 0);
+                        sp[m] += pv;
                     }
+                }
             }
             cp_async_wait_all();
             __syncwarp();
 
             const int u = u0 + lane;
-            const bool active = u < n_units;
+            const bool active = u < u1;
             const int p = active ? u / nt : p_lo, t = active ? u - p * nt : 0;
             const int r = in_u0 + 2 * p;
             float2 xx[XW];                                 // (x[r][c], x[r+1][c]) of window column c
@@ -227,56 +271,38 @@ k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const i
                 if (r_hi + 1 < Tu0) d_lo = Tu0 - r_hi - 1;
                 else if (r_lo > Tu1) d_lo = r_lo - Tu1;
             }
-            float pa[RF], pb[RF];                          // (a, b) of the previous step (d + 1)
-#pragma unroll
-            for (int c = 0; c < RF; ++c) { pa[c] = 0.f; pb[c] = 0.f; }
-            int rowm = r - CHk, rowp = r + 1 + CHk;
-            int sm = pmod(rowm - Tu0, R), sp = pmod(rowp - Tu0, R);
-            const float4 *wrow = Wd + CHk * KQ;
             if (active && CHk >= d_lo) macs += (unsigned long long)(CHk - d_lo + 1) * (KT * RF * 2);
+            // ring rows of the two sides: r - d walks up the ring as d falls, r + 1 + d walks down; an inactive lane or a row
+            // that is not held gets no address
+            int rowm = r - CHk, rowp = r + 1 + CHk;
+            int sm = pmod(rowm - flushed + fslot, R), sp_ = pmod(rowp - flushed + fslot, R);
+            const float *wrow = reinterpret_cast<const float *>(Wd + CHk * KQ);
+            float *const obase = oring + 4 * t;
+            float2 accA[RF], accB[RF];
+#pragma unroll
+            for (int c = 0; c < RF; ++c) accB[c] = make_float2(0.f, 0.f);
+            auto held = [&](int row) { return active && (!ADJ || (row >= Tu0 && row <= Tu1)); };
+            int dd = CHk;
 #pragma unroll 1
-            for (int dd = CHk; dd >= d_lo; --dd) {
-                if (active) {
-                    float2 acc2[RF];
-#pragma unroll
-                    for (int c = 0; c < RF; ++c) acc2[c] = make_float2(0.f, 0.f);
-#pragma unroll
-                    for (int q = 0; q < KQ; ++q) {
-                        const float4 w = wrow[q];
-                        const float2 wa = make_float2(w.x, w.y), wb = make_float2(w.z, w.w);
-#pragma unroll
-                        for (int c = 0; c < RF; ++c) acc2[c] = __ffma2_rn(xx[c + 2 * q], wa, acc2[c]);
-                        if (2 * q + 1 < KT) {
-#pragma unroll
-                            for (int c = 0; c < RF; ++c) acc2[c] = __ffma2_rn(xx[c + 2 * q + 1], wb, acc2[c]);
-                        }
-                    }
-                    if (!ADJ || (rowm >= Tu0 && rowm <= Tu1)) {       // out[r - d] += a_d + b_{d+1}
-                        float4 *o = reinterpret_cast<float4 *>(oring + sm * pitch + 4 * t), *o2 = reinterpret_cast<float4 *>(oring + sm * pitch + hp + 4 * t);
-                        float4 v0 = *o, v1 = *o2;
-                        v0.x += acc2[0].x + pb[0]; v0.y += acc2[1].x + pb[1]; v0.z += acc2[2].x + pb[2]; v0.w += acc2[3].x + pb[3];
-                        v1.x += acc2[4].x + pb[4]; v1.y += acc2[5].x + pb[5]; v1.z += acc2[6].x + pb[6]; v1.w += acc2[7].x + pb[7];
-                        *o = v0; *o2 = v1;
-                    }
-                    if (!ADJ || (rowp >= Tu0 && rowp <= Tu1)) {       // out[r + 1 + d] += b_d + a_{d+1}
-                        float4 *o = reinterpret_cast<float4 *>(oring + sp * pitch + 4 * t), *o2 = reinterpret_cast<float4 *>(oring + sp * pitch + hp + 4 * t);
-                        float4 v0 = *o, v1 = *o2;
-                        v0.x += acc2[0].y + pa[0]; v0.y += acc2[1].y + pa[1]; v0.z += acc2[2].y + pa[2]; v0.w += acc2[3].y + pa[3];
-                        v1.x += acc2[4].y + pa[4]; v1.y += acc2[5].y + pa[5]; v1.z += acc2[6].y + pa[6]; v1.w += acc2[7].y + pa[7];
-                        *o = v0; *o2 = v1;
-                    }
-#pragma unroll
-                    for (int c = 0; c < RF; ++c) { pa[c] = acc2[c].x; pb[c] = acc2[c].y; }
-                }
-                wrow -= KQ;
-                ++rowm; --rowp;
-                sm = sm + 1 == R ? 0 : sm + 1;
-                sp = sp == 0 ? R - 1 : sp - 1;
+            for (; dd > d_lo; dd -= 2) {                   // two steps per trip: the accumulators swap roles, no register copies
+                sym_step<KT>(xx, reinterpret_cast<const float4 *>(wrow), accA, accB, held(rowm) ? obase + sm * pitch : nullptr,
+                             held(rowp) ? obase + sp_ * pitch : nullptr, hp);
+                ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
                 __syncwarp();                              // the rows of this step are visible to the next one
+                sym_step<KT>(xx, reinterpret_cast<const float4 *>(wrow - 4 * KQ), accB, accA, held(rowm) ? obase + sm * pitch : nullptr,
+                             held(rowp) ? obase + sp_ * pitch : nullptr, hp);
+                ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
+                wrow -= 8 * KQ;
+                __syncwarp();
             }
+            if (dd == d_lo) {                              // odd number of steps: the last one
+                sym_step<KT>(xx, reinterpret_cast<const float4 *>(wrow), accA, accB, held(rowm) ? obase + sm * pitch : nullptr,
+                             held(rowp) ? obase + sp_ * pitch : nullptr, hp);
+                __syncwarp();
+            }
+            u0 = u1;
         }
-        __syncwarp();
-        flush(flushed, Tu1 + 1);
+        flush(Tu1 + 1);
         __syncwarp();                                      // the next item overwrites Wd and the staged rows
     }
     if (macs) atomicAdd(reinterpret_cast<unsigned long long *>(ADJ ? &wc->macs_adj : &wc->macs_fwd), macs);

@@ -11,8 +11,8 @@
 //
 // One WARP per block, persistent over the work items (control point, slice, chunk along v) like k_conv.  A lane owns a UNIT =
 // (pair of input rows r, r+1) x (8 output columns): the (KT+7)-wide window of both rows sits in registers as float2 (row r,
-// row r+1), the weights come as warp-broadcast LDS.128 of duplicated taps, and one packed FFMA2 per tap and column yields
-// (a_d, b_d) = (T_d[r], T_d[r+1]).  Output rows are accumulated in a shared-memory RING of rows private to the warp; since
+// row r+1), the weights come as warp-broadcast LDS.128 (four taps each; FFMA2 takes a tap as a scalar operand for both halves),
+// and one packed FFMA2 per tap and column yields (a_d, b_d) = (T_d[r], T_d[r+1]).  Output rows are accumulated in a shared-memory RING of rows private to the warp; since
 // out[r-d] takes a_d + b_{d+1} and out[r+1+d] takes b_d + a_{d+1}, walking d downwards with the previous (a, b) kept in
 // registers costs ONE read-modify-write of 8 columns per side and step.  In one step the "minus" rows r-d (parity of d) and
 // the "plus" rows r+1+d (other parity) cannot coincide, and the lanes of a group hold distinct (row pair, tile), so a step
@@ -27,8 +27,17 @@ namespace pdrt {
 constexpr int SYM_NTFC_MAX = 10;       // widest work item [thread-tiles of 8 columns along v]
 
 // Ring row [floats]: columns 0-3 of every tile first, then columns 4-7 (second plane at 4 nt), so that the two LDS.128 of a
-// read-modify-write hit consecutive 16-byte chunks across the lanes of a row.
-__host__ __device__ __forceinline__ int sym_out_pitch(int nt) { return 8 * nt; }
+// read-modify-write hit consecutive 16-byte chunks across the lanes of a row.  The lanes of a quarter-warp that fall on the
+// next row pair are two rows on: the pitch is padded until that offset (pitch/2 chunks, modulo the 8 chunks of a wavefront)
+// continues where the row ends, give or take one chunk.
+__host__ __device__ __forceinline__ int sym_out_pitch(int nt)
+{
+    int p = 8 * nt;
+    for (;; p += 4) {
+        const int dl = (p >> 1) & 7;
+        if (dl == (nt & 7) || dl == ((nt + 1) & 7) || dl == ((nt - 1) & 7)) return p;
+    }
+}
 // row pairs per group of units: as many whole-or-part pairs as 32 units span, at most 8
 __host__ __device__ __forceinline__ int sym_max_pairs(int nt) { return (32 + nt - 1) / nt < 8 ? (32 + nt - 1) / nt : 8; }
 // 16-byte chunks (2 columns x 2 rows) per staged row pair: the windows of nt tiles, rounded to the 8-chunk swizzle period
@@ -49,38 +58,35 @@ inline int sym_in_floats(int kt)
 }
 inline size_t sym_smem_bytes(int kt)
 {
-    const int c = (kt - 1) / 2, kq = (kt + 1) / 2;
-    return sizeof(float) * ((size_t)4 * (c + 1) * kq + sym_in_floats(kt) + sym_out_floats(kt));
+    const int c = (kt - 1) / 2, kp = (kt + 3) & ~3;
+    return sizeof(float) * ((size_t)(c + 1) * kp + sym_in_floats(kt) + sym_out_floats(kt));
 }
 
 __device__ __forceinline__ int pmod(int a, int m) { const int r = a % m; return r < 0 ? r + m : r; }
 
-// One step d of a unit: acc = (a_d, b_d) from the window and weight row d; out[r-d] += a_d + b_{d+1}, out[r+1+d] += b_d + a_{d+1},
+// One step d of a unit: acc = (a_d, b_d) from the window and the weight row `w` (registers); then the weight row of the NEXT step is
+// fetched into `w` (its latency hides behind the read-modify-writes) and out[r-d] += a_d + b_{d+1}, out[r+1+d] += b_d + a_{d+1},
 // with (a_{d+1}, b_{d+1}) = prev.  `om` / `op` point at the unit's 8 columns (first plane) of the two ring rows; null: row not held.
 template <int KT>
-__device__ __forceinline__ void sym_step(const float2 (&xx)[KT + 7], const float4 *__restrict__ wrow, float2 (&acc)[RF], const float2 (&prev)[RF],
-                                         float *om, float *op, int hp)
+__device__ __forceinline__ void sym_step(const float2 (&xx)[KT + 7], float4 (&w)[(KT + 3) / 4], const float4 *__restrict__ wnext,
+                                         float2 (&acc)[RF], const float2 (&prev)[RF], float *om, float *op, int hp)
 {
-    constexpr int KQ = (KT + 1) / 2;
-    {
-        const float4 w = wrow[0];
-        const float2 wa = make_float2(w.x, w.y), wb = make_float2(w.z, w.w);
+    constexpr int KQ4 = (KT + 3) / 4;
 #pragma unroll
-        for (int c = 0; c < RF; ++c) acc[c] = __fmul2_rn(xx[c], wa);
+    for (int q = 0; q < KQ4; ++q) {
+        const float ws[4] = { w[q].x, w[q].y, w[q].z, w[q].w };
 #pragma unroll
-        for (int c = 0; c < RF; ++c) acc[c] = __ffma2_rn(xx[c + 1], wb, acc[c]);
-    }
+        for (int e = 0; e < 4; ++e) {
+            const int dj = 4 * q + e;
+            if (dj < KT) {
+                const float2 wd = make_float2(ws[e], ws[e]);          // one register: FFMA2 takes it as a scalar operand
 #pragma unroll
-    for (int q = 1; q < KQ; ++q) {
-        const float4 w = wrow[q];
-        const float2 wa = make_float2(w.x, w.y), wb = make_float2(w.z, w.w);
-#pragma unroll
-        for (int c = 0; c < RF; ++c) acc[c] = __ffma2_rn(xx[c + 2 * q], wa, acc[c]);
-        if (2 * q + 1 < KT) {
-#pragma unroll
-            for (int c = 0; c < RF; ++c) acc[c] = __ffma2_rn(xx[c + 2 * q + 1], wb, acc[c]);
+                for (int c = 0; c < RF; ++c) acc[c] = dj == 0 ? __fmul2_rn(xx[c], wd) : __ffma2_rn(xx[c + dj], wd, acc[c]);
+            }
         }
     }
+#pragma unroll
+    for (int q = 0; q < KQ4; ++q) w[q] = wnext[q];
     if (om) {
         float4 *o = reinterpret_cast<float4 *>(om), *o2 = reinterpret_cast<float4 *>(om + hp);
         float4 v0 = *o, v1 = *o2;
@@ -107,14 +113,14 @@ k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const i
            int *item_counter, WorkCounters *wc, int in_floats, int out_floats)
 {
     constexpr int C = (KT - 1) / 2;
-    constexpr int KP = (KT + 3) & ~3;                 // row pitch of the table image [floats]
-    constexpr int KQ = (KT + 1) / 2;                  // float4 (two duplicated taps) per weight row
+    constexpr int KP = (KT + 3) & ~3;                 // row pitch of the table image and of Wd [floats]
+    constexpr int KQ4 = KP / 4;                       // LDS.128 per weight row
     constexpr int XW = KT + 7;                        // register window along v [columns], even
     constexpr int NXQ = XW / 2;                       // LDS.128 per window (2 columns x 2 rows each)
     constexpr int MCX = (8 * SYM_NTFC_MAX + 2 * C + 31) / 32;    // staged columns per lane and row
     extern __shared__ float4 smem4[];
-    float4 *Wd = smem4;                               // [C+1 (d)][KQ]: (w[2q], w[2q], w[2q+1], w[2q+1]) of kernel row C+d
-    float4 *xin4 = smem4 + (C + 1) * KQ;              // [pair][chunk]: (x[r][c], x[r+1][c], x[r][c+1], x[r+1][c+1]), chunks swizzled
+    float4 *Wd = smem4;                               // [C+1 (d)][KQ4]: kernel row C+d, zero past KT
+    float4 *xin4 = smem4 + (C + 1) * KQ4;             // [pair][chunk]: (x[r][c], x[r+1][c], x[r][c+1], x[r+1][c+1]), chunks swizzled
     float *oring = reinterpret_cast<float *>(xin4) + in_floats;   // [slot][pitch]: ring of output rows, all zero between uses
     const unsigned xin_s = (unsigned)__cvta_generic_to_shared(xin4);
     const int lane = threadIdx.x;
@@ -147,7 +153,11 @@ k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const i
         const int atf0 = max(ctf0, (A.v0 - rj0) / RF), atf1 = min(ctf1 - 1, (A.v1 - rj0) / RF);
         if (atf0 > atf1) continue;
         int nt = atf1 - atf0 + 1, av0 = rj0 + atf0 * RF;
-        if (ADJ && ncf == 1) { av0 = A.v0 & ~1; nt = (A.v1 - av0) / RF + 1; }      // adjoint outputs are read back on S_k only
+        if (ncf == 1) {     // one chunk: the tiles start at the box instead of the region's tile grid (fewer tiles; k_fluence tabulates the same
+                            // columns as the written box); forward stores are 16-byte, adjoint stores 8-byte aligned
+            av0 = ADJ ? A.v0 & ~1 : A.v0 & ~3;
+            nt = (A.v1 - av0) / RF + 1;
+        }
         // rows: input row pairs, output rows held in the ring (T), output rows written to HBM (wu)
         const int in_u0 = B.u0, in_u1 = B.u1, npair = (in_u1 - in_u0 + 2) >> 1;
         int wu0, wu1, Tu0, Tu1;
@@ -164,50 +174,46 @@ k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const i
         const float *sbase = in + slice_off;
         float *oslice = out + slice_off + (av0 - rj0) - (long long)ri0 * pv;       // row i, column av0 + c at oslice + i pv + c
 
-        {   // S4: rows C .. C+CHk of the slice kernel = lerp of the table in radiological depth, taps duplicated for FFMA2
+        {   // S4: rows C .. C+CHk of the slice kernel = lerp of the table in radiological depth
             const float tz = zrad[(size_t)cp * P.Nw + k] / P.dz;
             int n0 = (int)floorf(tz);
             n0 = min(max(n0, 0), P.n_z - 2);
             const float f = fminf(fmaxf(tz - n0, 0.f), 1.f);
-            const float *w0 = wtab + (size_t)n0 * KT * KP + C * KP, *w1 = w0 + KT * KP;
-            for (int e = lane; e < (CHk + 1) * KQ; e += 32) {
-                const int dd = e / KQ, q = e - dd * KQ;
-                const int o = dd * KP + 2 * q;
-                const float wa = (1.f - f) * __ldg(w0 + o) + f * __ldg(w1 + o);
-                const float wb = 2 * q + 1 < KT ? (1.f - f) * __ldg(w0 + o + 1) + f * __ldg(w1 + o + 1) : 0.f;
-                Wd[dd * KQ + q] = make_float4(wa, wa, wb, wb);
+            const float4 *w0 = reinterpret_cast<const float4 *>(wtab + (size_t)n0 * KT * KP + C * KP), *w1 = w0 + KT * KQ4;
+            for (int e = lane; e < (CHk + 1) * KQ4; e += 32) {
+                const float4 a = __ldg(w0 + e), b = __ldg(w1 + e);
+                Wd[e] = make_float4((1.f - f) * a.x + f * b.x, (1.f - f) * a.y + f * b.y, (1.f - f) * a.z + f * b.z, (1.f - f) * a.w + f * b.w);
             }
         }
-        // flush geometry: lanes over the 16-byte (forward) / 8-byte (adjoint) chunks of a row
+        // flush geometry: the lanes walk the 16-byte (forward) / 8-byte (adjoint) chunks of consecutive rows, 32 chunks per trip
         const int nchunk = ADJ ? 4 * nt : 2 * nt;
-        const int rpi = nchunk >= 32 ? 1 : 32 / nchunk;
-        const int lrow = nchunk >= 32 ? 0 : lane / nchunk, lch = nchunk >= 32 ? lane : lane - lrow * nchunk;
+        const int lrow0 = lane / nchunk, lch0 = lane - lrow0 * nchunk, srow = 32 / nchunk, sch = 32 - srow * nchunk;
         const int room = pv - (av0 - rj0);                 // columns of the region from av0 on
         int flushed = Tu0, fslot = 0;                      // rows below `flushed` are final and written; ring slot of row `flushed`
         auto flush = [&](int b) {                          // rows [flushed, b): ring -> HBM (inside the written box), slots back to zero
-            for (int i0 = flushed; i0 < b; i0 += rpi) {
-                const int i = i0 + lrow;
-                if (lrow < rpi && i < b) {
-                    int sl = fslot + (i - flushed);
-                    while (sl >= R) sl -= R;
+            int i = flushed + lrow0, ch = lch0, sl = fslot + lrow0;
+            while (sl >= R) sl -= R;
+            while (__any_sync(0xffffffffu, i < b)) {
+                if (i < b) {
                     float *rowp = oring + sl * pitch;
                     const bool wr = i >= wu0 && i <= wu1;
                     float *orow = oslice + (long long)i * pv;
-                    for (int ch = lch; ch < nchunk; ch += 32) {
-                        if (ADJ) {
-                            const int c = 2 * ch;
-                            float2 *p = reinterpret_cast<float2 *>(rowp + ((c >> 2) & 1) * hp + 4 * (c >> 3) + (c & 3));
-                            const float2 v = *p;
-                            *p = make_float2(0.f, 0.f);
-                            if (wr && c + 2 <= room) *reinterpret_cast<float2 *>(orow + c) = v;
-                        } else {
-                            float4 *p = reinterpret_cast<float4 *>(rowp + (ch & 1) * hp + 4 * (ch >> 1));
-                            const float4 v = *p;
-                            *p = make_float4(0.f, 0.f, 0.f, 0.f);
-                            if (wr) *reinterpret_cast<float4 *>(orow + 4 * ch) = v;
-                        }
+                    if (ADJ) {
+                        const int c = 2 * ch;
+                        float2 *p = reinterpret_cast<float2 *>(rowp + ((c >> 2) & 1) * hp + 4 * (c >> 3) + (c & 3));
+                        const float2 v = *p;
+                        *p = make_float2(0.f, 0.f);
+                        if (wr && c + 2 <= room) *reinterpret_cast<float2 *>(orow + c) = v;
+                    } else {
+                        float4 *p = reinterpret_cast<float4 *>(rowp + (ch & 1) * hp + 4 * (ch >> 1));
+                        const float4 v = *p;
+                        *p = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (wr && 4 * ch + 4 <= room) *reinterpret_cast<float4 *>(orow + 4 * ch) = v;
                     }
                 }
+                ch += sch; i += srow; sl += srow;
+                if (ch >= nchunk) { ch -= nchunk; ++i; ++sl; }
+                while (sl >= R) sl -= R;
             }
             fslot += b - flushed;
             while (fslot >= R) fslot -= R;
@@ -229,23 +235,31 @@ k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const i
                 const float *sp[MCX];
                 unsigned dp[MCX];
                 int csz[MCX];
+                bool cex[MCX];
 #pragma unroll
                 for (int m = 0; m < MCX; ++m) {
                     const int c = lane + 32 * m, j = av0 - C + c, q = c >> 1;
                     const bool cin = j >= B.v0 && j <= B.v1;
-                    csz[m] = c < ncols ? (cin ? 4 : 0) : -1;
+                    cex[m] = c < ncols;
+                    csz[m] = cin ? 4 : 0;
                     sp[m] = sbase + (long long)(r_lo - ri0) * pv + (cin ? j - rj0 : 0);
                     dp[m] = xin_s + 16u * (unsigned)(q ^ ((q >> 3) & 7)) + 8u * (unsigned)(c & 1);
                 }
                 const int nrow = 2 * (p_hi - p_lo + 1);
-                for (int rl = 0; rl < nrow; ++rl) {
-                    const bool rin = r_lo + rl <= in_u1;   // only the second row of the last pair can lie outside
-                    const unsigned ro = 16u * (unsigned)((rl >> 1) * PPc) + 4u * (unsigned)(rl & 1);
+                const int nin = min(nrow, in_u1 - r_lo + 1);      // only the second row of the last pair can lie outside the input rows
+                unsigned ro = 0;
+                for (int rl = 0; rl < nin; ++rl) {
 #pragma unroll
                     for (int m = 0; m < MCX; ++m) {
-                        if (csz[m] >= 0) cp_async_4(dp[m] + ro, rin ? sp[m] : sbase, rin ? csz[m] : 0);
+                        if (cex[m]) cp_async_4(dp[m] + ro, sp[m], csz[m]);
                         sp[m] += pv;
                     }
+                    ro += (rl & 1) ? 16u * (unsigned)PPc - 4u : 4u;
+                }
+                if (nin < nrow) {
+#pragma unroll
+                    for (int m = 0; m < MCX; ++m)
+                        if (cex[m]) cp_async_4(dp[m] + ro, sbase, 0);
                 }
             }
             cp_async_wait_all();
@@ -276,28 +290,28 @@ k_conv_sym(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const i
             // that is not held gets no address
             int rowm = r - CHk, rowp = r + 1 + CHk;
             int sm = pmod(rowm - flushed + fslot, R), sp_ = pmod(rowp - flushed + fslot, R);
-            const float *wrow = reinterpret_cast<const float *>(Wd + CHk * KQ);
+            const float4 *wrow = Wd + CHk * KQ4;
             float *const obase = oring + 4 * t;
             float2 accA[RF], accB[RF];
 #pragma unroll
             for (int c = 0; c < RF; ++c) accB[c] = make_float2(0.f, 0.f);
+            float4 w[KQ4];
+#pragma unroll
+            for (int q = 0; q < KQ4; ++q) w[q] = wrow[q];
             auto held = [&](int row) { return active && (!ADJ || (row >= Tu0 && row <= Tu1)); };
             int dd = CHk;
 #pragma unroll 1
             for (; dd > d_lo; dd -= 2) {                   // two steps per trip: the accumulators swap roles, no register copies
-                sym_step<KT>(xx, reinterpret_cast<const float4 *>(wrow), accA, accB, held(rowm) ? obase + sm * pitch : nullptr,
-                             held(rowp) ? obase + sp_ * pitch : nullptr, hp);
+                sym_step<KT>(xx, w, wrow - KQ4, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr, hp);
                 ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
                 __syncwarp();                              // the rows of this step are visible to the next one
-                sym_step<KT>(xx, reinterpret_cast<const float4 *>(wrow - 4 * KQ), accB, accA, held(rowm) ? obase + sm * pitch : nullptr,
-                             held(rowp) ? obase + sp_ * pitch : nullptr, hp);
+                wrow -= dd >= 2 ? 2 * KQ4 : KQ4;           // row dd - 2 of the next trip (row 0 again after the last step: never used)
+                sym_step<KT>(xx, w, wrow, accB, accA, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr, hp);
                 ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
-                wrow -= 8 * KQ;
                 __syncwarp();
             }
             if (dd == d_lo) {                              // odd number of steps: the last one
-                sym_step<KT>(xx, reinterpret_cast<const float4 *>(wrow), accA, accB, held(rowm) ? obase + sm * pitch : nullptr,
-                             held(rowp) ? obase + sp_ * pitch : nullptr, hp);
+                sym_step<KT>(xx, w, wrow, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr, hp);
                 __syncwarp();
             }
             u0 = u1;

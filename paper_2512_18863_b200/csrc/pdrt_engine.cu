@@ -44,6 +44,20 @@ bool conv_legacy()
     const char *v = std::getenv("PDRT_CONV_LEGACY");
     return v && std::atoi(v) != 0;
 }
+// Largest compiled size for which the ADJOINT also runs in row-symmetric form.  The forward shares every row correlation between two
+// output rows; the adjoint only where both rows r-d and r+d lie in S_k, i.e. for supports taller than the kernel, and its wide-window
+// variants hold fewer warps per SM.  Measured: at 31 taps it loses 10 % on c4 (supports 34 rows tall) and wins 37 % on c5
+// (taller supports); from 41 taps on the output-stationary kernel wins on both.
+int conv_sym_adj_max()
+{
+    if (const char *v = std::getenv("PDRT_CONV_SYM_ADJ_MAX")) return std::atoi(v);
+    return 31;
+}
+int conv_sym_fwd_min()
+{
+    if (const char *v = std::getenv("PDRT_CONV_SYM_FWD_MIN")) return std::atoi(v);
+    return 11;
+}
 int compiled_size(int k)
 {
     for (int kt : kCompiled)
@@ -116,6 +130,7 @@ struct pdrt_engine {
     bool last_backward = false;
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
+    bool sym_fwd = false, sym_adj = false;   // which directions run k_conv_sym (single pass; forward from 11 taps, adjoint from 11 to 31)
     int conv_sym_per_sm[2][64] = {};     // the same for k_conv_sym, by [adjoint][KT]
     int conv_per_sm[2][2][2][64] = {};   // resident conv blocks per SM on THIS engine's device, by [adjoint][copy width - 1][multi-pass][KT]; 0 = not queried yet
     DevBuf<float> coll;               // collimator angles [coll_n] set by pdrt_set_collimator (coll_n = 0: none)
@@ -199,6 +214,13 @@ int gaussian_taps(double sigma, double D, std::vector<float> &g)
 // embedded centred in the compiled KT x KT window.  Device layout: [n_z][KT (du)][KP (dv)], KP = KT rounded up to 4,
 // i.e. exactly the shared-memory image the conv kernel wants.  The table is point-symmetric (mirrored quadrant), so the
 // flipped kernel of the adjoint is the same table (R3).
+// The work-item layout (chunk width, written box of D_b) follows the kernel that runs in this direction; k_fluence tabulates it per call.
+void set_conv_direction(pdrt_engine *e, bool adjoint)
+{
+    e->P.conv_sym = (adjoint ? e->sym_adj : e->sym_fwd) ? 1 : 0;
+    e->P.ntfc_max = e->P.conv_sym ? SYM_NTFC_MAX : NTFC_MAX;
+}
+
 int build_kernel_table(pdrt_engine *e, int k)
 {
     int nb = 1, kt = compiled_size(k);
@@ -245,8 +267,9 @@ int build_kernel_table(pdrt_engine *e, int k)
     e->P.NB = nb;
     e->P.CH = c;
     e->P.tile_floats = tile_floats_for(kt);
-    e->P.conv_sym = (nb == 1 && !conv_legacy()) ? 1 : 0;
-    e->P.ntfc_max = e->P.conv_sym ? SYM_NTFC_MAX : NTFC_MAX;
+    e->sym_fwd = nb == 1 && !conv_legacy() && kt >= conv_sym_fwd_min();
+    e->sym_adj = nb == 1 && !conv_legacy() && kt >= conv_sym_fwd_min() && kt <= conv_sym_adj_max();
+    set_conv_direction(e, false);
     return PDRT_OK;
 }
 
@@ -397,6 +420,7 @@ int run_setup(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, 
 int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry, const float *mu,
                  float *dose, cudaStream_t st)
 {
+    set_conv_direction(e, false);
     int rc = run_setup(e, n_cp, leaves, jaws, gantry, mu, true, st);
     if (rc) return rc;
     const int nb = batch_size(e, n_cp, 2);
@@ -438,6 +462,7 @@ int forward_impl(pdrt_engine *e, int n_cp, const float *leaves, const float *jaw
 int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry,
                         const float *mu, const float *gdose, cudaStream_t st, cudaEvent_t gdose_ready = nullptr)
 {
+    set_conv_direction(e, true);
     int rc = run_setup(e, n_cp, leaves, jaws, gantry, mu, true, st);
     if (rc) return rc;
     if (gdose_ready) CU(e, cudaStreamWaitEvent(st, gdose_ready, 0));      // S1 / S2 above do not read dL/dDose
@@ -840,6 +865,7 @@ int pdrt_stage_fluence(pdrt_engine *e, int32_t n_cp, const float *leaves, const 
     if ((rc = ensure_cp_scratch(e, n_cp))) return rc;
     const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
     CU(e, cudaMemsetAsync(e->phimap.p, 0, nmap * sizeof(float), st));     // outside the support bbox the map is zero
+    set_conv_direction(e, false);
     if ((rc = run_setup(e, n_cp, leaves, jaws, nullptr, nullptr, false, st))) return rc;
     CU(e, cudaMemcpyAsync(phimap, e->phimap.p, nmap * sizeof(float), cudaMemcpyDeviceToDevice, st));
     return PDRT_OK;
@@ -851,6 +877,7 @@ int pdrt_stage_fan_factor(pdrt_engine *e, int32_t n_cp, const float *leaves, con
     if (rc) return rc;
     if (e->depth_mode != PDRT_DEPTH_FAN) return fail(e, PDRT_EINVAL, "pdrt_stage_fan_factor needs PDRT_DEPTH_FAN");
     cudaStream_t st = (cudaStream_t)stream;
+    set_conv_direction(e, false);
     if ((rc = run_setup(e, n_cp, leaves, jaws, gantry, nullptr, true, st))) return rc;
     k_expand_fan<<<e->sm_count * 4, 256, 0, st>>>(e->P, e->desc.p, n_cp, e->fan_stride(), e->fan.p, factor);
     CU(e, cudaGetLastError());
@@ -874,6 +901,7 @@ int pdrt_stage_beam_dose(pdrt_engine *e, const float *leaves, const float *jaws,
     int rc = check_call(e, 1, { leaves, jaws, gantry, db });
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    set_conv_direction(e, false);
     if ((rc = run_setup(e, 1, leaves, jaws, gantry, nullptr, true, st))) return rc;
     CU(e, e->bufA.ensure((size_t)e->P.stride_cp));
     CU(e, e->bufB.ensure((size_t)e->P.stride_cp));

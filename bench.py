@@ -315,8 +315,9 @@ def run_c5_loop(args):
     eng.set_profiling(False)
     K = wf.kernel_size
     fp32_peak = eng.info.sm_count * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    conv_flops = 2.0 * K * K * wf.footprint_voxels
-    achieved = conv_flops / (fw_ms["conv"] * 1e-3) / 1e12
+    achieved = 2.0 * K * K * wf.support_voxels / (fw_ms["conv"] * 1e-3) / 1e12          # on inputs that can be non-zero (see run_ours)
+    on_tiles = 2.0 * K * K * wf.footprint_voxels / (fw_ms["conv"] * 1e-3) / 1e12
+    executed = 2.0 * wf.conv_macs / (fw_ms["conv"] * 1e-3) / 1e12
     pair = float(np.mean(pair_ms)) / n_it
     line = dict(metric=METRIC, value=pair, unit="ms", n_gpus=1, steps=steps, warmup=max(1, args.warmup // 3), ms_per_step=float(np.mean(loop_ms)),
                 higher_is_better=False, scaling="strong", vs_baseline=None, dtype="f32", data="synthetic",
@@ -326,8 +327,10 @@ def run_c5_loop(args):
                 graph_loop_ms=graph_ms, objective_at_iteration_20=loss_first,
                 control_points_per_s=wl.n_cp / (pair * 1e-3), clocks=clk.summary(),
                 gpu_launches=(sum(fw_n.values()) + sum(bw_n.values()) + 7) * n_it * steps,
-                roofline=dict(bound="alu", kernel="k_conv<K,false>", achieved=achieved, peak=fp32_peak, unit="TFLOP/s", frac=achieved / fp32_peak,
-                              traffic=recorded_traffic("c5", K)),
+                roofline=dict(bound="alu", kernel="k_conv_sym<K,false>" if wf.conv_symmetric else "k_conv<K,false,...>", achieved=achieved, peak=fp32_peak,
+                              unit="TFLOP/s", frac=achieved / fp32_peak, achieved_on_footprint_tiles=on_tiles, frac_on_footprint_tiles=on_tiles / fp32_peak,
+                              executed=executed, executed_frac=executed / fp32_peak, traffic=recorded_traffic("c5", K),
+                              note="algorithmic flops = 2*k^2*|support|; see the c4 line for the other two counts"),
                 stages={k: round(fw_ms[k] + bw_ms[k], 4) for k in fw_ms},
                 work=dict(support_voxels=wf.support_voxels, footprint_voxels=wf.footprint_voxels, conv_macs_issued_fwd=wf.conv_macs,
                           conv_macs_issued_bwd=wb.conv_macs))
@@ -480,14 +483,24 @@ def run_ours(args):
                               issued_tflops=round(2.0 * wf.conv_macs / (stage_ms["conv"] * 1e-3) / 1e12, 2) if stage_ms["conv"] > 0 else None)
         stages["conv_adj"].update(tflops=round(conv_adj_flops / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None,
                                   issued_tflops=round(2.0 * wb.conv_macs / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None)
-    achieved = conv_flops / (stage_ms["conv"] * 1e-3) / 1e12 if stage_ms["conv"] > 0 else None
-    useful = 2.0 * K * K * wf.support_voxels / (stage_ms["conv"] * 1e-3) / 1e12 if stage_ms["conv"] > 0 else None
-    roofline = dict(bound="alu", kernel="k_conv<K,false> (S4+S5: depth-indexed kernel lookup + lateral convolution)",
+    # The dominant kernel is the forward convolution.  Algorithmic flops = 2 k^2 |S|: the multiply-adds of Eq. 8 on inputs that can
+    # be non-zero (SURVEY.md 8(d) "algorithmic MAC"; products with structurally zero fluence earn nothing).  The row-symmetric kernel
+    # executes about (k+1)/2k of them (each row correlation serves two output rows), the output-stationary one more (zeros in the
+    # halo): `executed` is what the kernel counted, and executed / peak is the FMA-pipe share of the launch.
+    t_conv = stage_ms["conv"] * 1e-3
+    achieved = 2.0 * K * K * wf.support_voxels / t_conv / 1e12 if t_conv > 0 else None
+    on_tiles = conv_flops / t_conv / 1e12 if t_conv > 0 else None
+    executed = 2.0 * wf.conv_macs / t_conv / 1e12 if t_conv > 0 else None
+    kname = "k_conv_sym<K,false>" if wf.conv_symmetric else "k_conv<K,false,...>"
+    roofline = dict(bound="alu", kernel=f"{kname} (S4+S5: depth-indexed kernel lookup + lateral convolution)",
                     achieved=achieved, peak=fp32_peak, unit="TFLOP/s", frac=(achieved / fp32_peak) if achieved else None,
-                    achieved_on_nonzero_inputs=useful, frac_on_nonzero_inputs=(useful / fp32_peak) if useful else None,
+                    achieved_on_footprint_tiles=on_tiles, frac_on_footprint_tiles=(on_tiles / fp32_peak) if on_tiles else None,
+                    executed=executed, executed_frac=(executed / fp32_peak) if executed else None,
                     traffic=recorded_traffic(wl.name, K),
-                    note=f"algorithmic flops = 2*k^2*|footprint| per launch (SURVEY.md 8(d): the output-tiled count); *_on_nonzero_inputs uses 2*k^2*|support| "
-                         f"(products with structurally zero fluence not counted); peak = {eng.info.sm_count} SMs x 128 FP32 lanes x 2 x "
+                    note=f"algorithmic flops = 2*k^2*|support| per launch (products with structurally zero fluence not counted); "
+                         f"*_on_footprint_tiles uses 2*k^2*|footprint| (SURVEY.md 8(d): the output-tiled count; a kernel that uses the kernel's "
+                         f"row symmetry executes about half of it, so this can exceed the peak); executed = 2 x the multiply-adds the kernel counted; "
+                         f"peak = {eng.info.sm_count} SMs x 128 FP32 lanes x 2 x "
                          f"{peaks['sm_max_mhz']:.0f} MHz (plain FP32 FMA pipe; FFMA microbenchmark on this pool: 72.5 TFLOP/s); "
                          f"HBM fractions of the bandwidth-bound stages are under 'stages' against {peaks['hbm_gbs']} GB/s {peaks['source']}")
 

@@ -139,10 +139,12 @@ typedef struct {
     int64_t  support_voxels;    /* sum over CPs and slices of |S_k| (possibly non-zero Phi_vol)   */
     int64_t  footprint_voxels;  /* sum over CPs and slices of |F_k| = |S_k (+) k x k|             */
     int64_t  region_voxels;     /* voxels of the compact per-CP beam-frame regions (materialised) */
-    int64_t  conv_macs;         /* multiply-adds the conv kernel issues (k_compiled^2 per output) */
+    int64_t  conv_macs;         /* multiply-adds the conv kernel executed (counted by the kernel; the row-symmetric kernel shares
+                                   each row correlation between two output rows, so this can be below k^2 per output)          */
     int32_t  kernel_size, kernel_size_compiled;
     int64_t  fan_rays;          /* PDRT_DEPTH_FAN: diverging rays traced (sum over control points), else 0  */
     int32_t  ray_samples;       /* samples per ray (upper bound: samples outside the grid are skipped)     */
+    int32_t  conv_symmetric;    /* 1: that call's convolution ran in row-symmetric form (k_conv_sym), 0: output-stationary (k_conv) */
 } pdrt_work;
 
 /* pdrt_create: grid geometry, density volume [nz][ny][nx] (host OR device pointer; copied) and

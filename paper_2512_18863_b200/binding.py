@@ -61,7 +61,7 @@ class PdrtWork(C.Structure):
     _fields_ = [("n_cp", C.c_int32), ("conv_items", C.c_int64), ("support_voxels", C.c_int64),
                 ("footprint_voxels", C.c_int64), ("region_voxels", C.c_int64), ("conv_macs", C.c_int64),
                 ("kernel_size", C.c_int32), ("kernel_size_compiled", C.c_int32),
-                ("fan_rays", C.c_int64), ("ray_samples", C.c_int32)]
+                ("fan_rays", C.c_int64), ("ray_samples", C.c_int32), ("conv_symmetric", C.c_int32)]
 
 
 class PdrtLimits(C.Structure):

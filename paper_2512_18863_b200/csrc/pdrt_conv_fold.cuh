@@ -1,0 +1,309 @@
+// pdrt_conv_fold.cuh — the row-symmetric convolution of pdrt_conv_sym.cuh with the kernel's COLUMN symmetry folded in as well
+// (the pencil kernel is radially symmetric; R3: the table is built mirrored in both axes).
+//
+// A row correlation is  T_d[r][j] = W_d[C] x[r][j] + sum_{m=1..C} W_d[C+m] (x[r][j-m] + x[r][j+m]),  W_d = row C+d of the slice
+// kernel.  The folded window  z[j][m] = x[r][j-m] + x[r][j+m]  does not depend on d: a unit = (row pair r, r+1) x 4 output columns
+// builds its 4 x (C+1) folded values once (packed adds on the (row r, row r+1) pairs) and then runs the C+1 steps d = C .. 0 with
+// C+1 packed FFMA2 per column instead of 2C+1.  Together with the row symmetry that is (C+1)^2 multiply-adds per input value
+// instead of (2C+1)^2.  Everything else is pdrt_conv_sym.cuh: one warp per block, units of 32 lanes, output rows accumulated in a
+// warp-private shared-memory ring (one 16-byte read-modify-write per side and step), staged input rows, rows written to HBM
+// when no later unit reaches them.  The folded window takes 8 (C+2) registers, so this form serves kernels up to 25 taps.
+#pragma once
+#include "pdrt_conv_sym.cuh"
+
+namespace pdrt {
+
+constexpr int FRF = 4;                 // output columns per unit
+constexpr int FOLD_NT4_MAX = 2 * SYM_NTFC_MAX;      // widest work item [tiles of 4 columns]
+
+// ring row pitch [floats]: one 16-byte chunk per tile; padded until the chunks of the next row pair (two rows on) continue where
+// this row ends, give or take one chunk (modulo the 8 chunks of a wavefront)
+__host__ __device__ __forceinline__ int fold_out_pitch(int nt4)
+{
+    for (int p = 4 * nt4;; p += 4) {
+        const int dl = (p >> 1) & 7;
+        if (dl == (nt4 & 7) || dl == ((nt4 + 1) & 7) || dl == ((nt4 - 1) & 7)) return p;
+    }
+}
+__host__ __device__ __forceinline__ int fold_max_pairs(int nt4) { return (30 + nt4) / nt4 + 1 < 8 ? (30 + nt4) / nt4 + 1 : 8; }
+// 16-byte chunks (2 columns x 2 rows) per staged row pair (even: the swizzle swaps neighbours)
+__host__ __device__ __forceinline__ int fold_in_chunks(int nt4, int c) { return (2 * nt4 + c + 1) & ~1; }
+inline int fold_out_floats(int kt)
+{
+    const int c = (kt - 1) / 2;
+    int best = 0;
+    for (int n = 1; n <= FOLD_NT4_MAX; ++n) best = std::max(best, (2 * fold_max_pairs(n) + 2 * c) * fold_out_pitch(n));
+    return best;
+}
+inline int fold_in_floats(int kt)
+{
+    const int c = (kt - 1) / 2;
+    int best = 0;
+    for (int n = 1; n <= FOLD_NT4_MAX; ++n) best = std::max(best, fold_max_pairs(n) * fold_in_chunks(n, c) * 4);
+    return best;
+}
+__host__ __device__ constexpr int fold_wpitch(int kt) { return ((kt - 1) / 2 + 1 + 3) & ~3; }         // floats per weight row: W_d[C .. 2C], padded to 4
+inline size_t fold_smem_bytes(int kt)
+{
+    const int c = (kt - 1) / 2;
+    return sizeof(float) * ((size_t)(c + 1) * fold_wpitch(kt) + fold_in_floats(kt) + fold_out_floats(kt));
+}
+
+// One step d of a unit: acc = (a_d, b_d) from the folded window and the weight row in `w`; then the next step's weights are fetched
+// and out[r-d] += a_d + b_{d+1}, out[r+1+d] += b_d + a_{d+1} with (a_{d+1}, b_{d+1}) = prev.  om / op: the unit's 4 columns of the two
+// ring rows, null when the row is not held.
+template <int C>
+__device__ __forceinline__ void fold_step(const float2 (&zc)[FRF], const float2 (&z)[C][FRF], float4 (&w)[(C + 4) / 4], const float4 *__restrict__ wnext,
+                                          float2 (&acc)[FRF], const float2 (&prev)[FRF], float *om, float *op)
+{
+    constexpr int WQ = (C + 4) / 4;
+#pragma unroll
+    for (int q = 0; q < WQ; ++q) {
+        const float ws[4] = { w[q].x, w[q].y, w[q].z, w[q].w };
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int m = 4 * q + e;
+            if (m <= C) {
+                const float2 wd = make_float2(ws[e], ws[e]);          // one register: FFMA2 takes it as a scalar operand
+#pragma unroll
+                for (int c = 0; c < FRF; ++c) acc[c] = m == 0 ? __fmul2_rn(zc[c], wd) : __ffma2_rn(z[m - 1][c], wd, acc[c]);
+            }
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < WQ; ++q) w[q] = wnext[q];
+    if (om) {
+        float4 *o = reinterpret_cast<float4 *>(om);
+        float4 v = *o;
+        v.x += acc[0].x + prev[0].y; v.y += acc[1].x + prev[1].y; v.z += acc[2].x + prev[2].y; v.w += acc[3].x + prev[3].y;
+        *o = v;
+    }
+    if (op) {
+        float4 *o = reinterpret_cast<float4 *>(op);
+        float4 v = *o;
+        v.x += acc[0].y + prev[0].x; v.y += acc[1].y + prev[1].x; v.z += acc[2].y + prev[2].x; v.w += acc[3].y + prev[3].x;
+        *o = v;
+    }
+}
+
+template <int KT, bool ADJ>
+__global__ void __maxnreg__(168)
+k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
+            const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
+            int *item_counter, WorkCounters *wc, int in_floats, int out_floats)
+{
+    constexpr int C = (KT - 1) / 2;
+    constexpr int KP = (KT + 3) & ~3;                 // row pitch of the table image [floats]
+    constexpr int WP = fold_wpitch(KT), WQ = WP / 4;  // weight row W_d[C .. 2C] in shared memory [floats], LDS.128 per row
+    constexpr int XW = KT + FRF - 1;                  // window along v [columns]: 2C + 4, even
+    constexpr int NXQ = XW / 2;                       // LDS.128 per window (2 columns x 2 rows each)
+    constexpr int MCX = (4 * FOLD_NT4_MAX + 2 * C + 31) / 32;    // staged columns per lane and row
+    extern __shared__ float4 smem4[];
+    float4 *Wd = smem4;                               // [C+1 (d)][WQ]: kernel row C+d, columns C .. 2C, zero past them
+    float4 *xin4 = smem4 + (C + 1) * WQ;              // [pair][chunk]: (x[r][c], x[r+1][c], x[r][c+1], x[r+1][c+1]), chunks swizzled
+    float *oring = reinterpret_cast<float *>(xin4) + in_floats;   // [slot][pitch]: ring of output rows, all zero between uses
+    const unsigned xin_s = (unsigned)__cvta_generic_to_shared(xin4);
+    const int lane = threadIdx.x;
+    const int total = tile_base[n_cp];
+    const int CHk = min(P.CH, C);                     // rows C+d with d > CH of an embedded smaller kernel are zero
+    int slot_hint = 0;
+    unsigned long long macs = 0ull;                   // multiply-adds of this lane (work counter)
+
+    for (int e = lane; e < out_floats / 4; e += 32) reinterpret_cast<float4 *>(oring)[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncwarp();
+
+    for (;;) {
+        int item = 0;
+        if (lane == 0) item = atomicAdd(item_counter, 1);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= total) break;
+        while (slot_hint + 1 < n_cp && item >= tile_base[slot_hint + 1]) ++slot_hint;   // items arrive in increasing order
+        const int slot = slot_hint, cp = cp0 + slot;
+        const CpDesc &d = desc[cp];
+        const int ncf = d.ncf, ntfc = d.ntfc, ntf = d.ntf, nts = d.nts, ri0 = d.ri0, rj0 = d.rj0, pu = d.pu, pv = d.pv;
+        const int local = item - tile_base[slot];
+        const int k = local / ncf, cf = local - k * ncf;
+        const SliceBox S = slice_support(P, d, k);
+        if (box_empty(S)) continue;
+        const SliceBox F = dilate(P, S, P.CH);
+        const SliceBox A = ADJ ? S : F;               // outputs to compute
+        const SliceBox B = ADJ ? F : S;               // source box of the input (zero outside)
+        // tiles of the chunk along v: the region's 8-column tile grid, or (one chunk) 4-column tiles from the box on
+        const int ctf0 = cf * ntfc, ctf1 = min(ntf, ctf0 + ntfc);
+        const int atf0 = max(ctf0, (A.v0 - rj0) / RF), atf1 = min(ctf1 - 1, (A.v1 - rj0) / RF);
+        if (atf0 > atf1) continue;
+        int nt = 2 * (atf1 - atf0 + 1), av0 = rj0 + atf0 * RF;
+        if (ncf == 1) {     // k_fluence tabulates the same columns as the written box; forward stores are 16-byte, adjoint stores 8-byte aligned
+            av0 = ADJ ? A.v0 & ~1 : A.v0 & ~3;
+            nt = (A.v1 - av0) / FRF + 1;
+        }
+        // rows: input row pairs, output rows held in the ring (T), output rows written to HBM (wu)
+        const int in_u0 = B.u0, in_u1 = B.u1, npair = (in_u1 - in_u0 + 2) >> 1;
+        int wu0, wu1, Tu0, Tu1;
+        if (ADJ) { wu0 = Tu0 = S.u0; wu1 = Tu1 = S.u1; }
+        else {      // the thread-tile rows that intersect F_k (wbox of k_fluence), clipped to the beam grid
+            wu0 = ri0 + (F.u0 - ri0) / RS * RS;
+            wu1 = min(P.Nu - 1, ri0 + min(nts - 1, (F.u1 - ri0) / RS) * RS + RS - 1);
+            Tu0 = min(wu0, in_u0 - CHk); Tu1 = max(wu1, in_u0 + 2 * npair - 1 + CHk);
+        }
+        const int pitch = fold_out_pitch(nt), R = out_floats / pitch;
+        const int PPc = fold_in_chunks(nt, C), maxp = fold_max_pairs(nt);
+        const int ncols = FRF * nt + 2 * C;
+        const long long slice_off = (long long)slot * P.stride_cp + (long long)k * pu * pv;
+        const float *sbase = in + slice_off;
+        float *oslice = out + slice_off + (av0 - rj0) - (long long)ri0 * pv;       // row i, column av0 + c at oslice + i pv + c
+
+        {   // S4: columns C .. 2C of rows C .. C+CHk of the slice kernel = lerp of the table in radiological depth
+            const float tz = zrad[(size_t)cp * P.Nw + k] / P.dz;
+            int n0 = (int)floorf(tz);
+            n0 = min(max(n0, 0), P.n_z - 2);
+            const float f = fminf(fmaxf(tz - n0, 0.f), 1.f);
+            const float *w0 = wtab + (size_t)n0 * KT * KP + C * KP + C, *w1 = w0 + KT * KP;
+            float *Wf = reinterpret_cast<float *>(Wd);
+            for (int e = lane; e < (CHk + 1) * WP; e += 32) {
+                const int dd = e / WP, m = e - dd * WP;
+                Wf[e] = m <= C ? (1.f - f) * __ldg(w0 + dd * KP + m) + f * __ldg(w1 + dd * KP + m) : 0.f;
+            }
+        }
+        // flush geometry: the lanes walk the 16-byte (forward) / 8-byte (adjoint) chunks of consecutive rows, 32 chunks per trip
+        const int nchunk = ADJ ? 2 * nt : nt;
+        const int lrow0 = lane / nchunk, lch0 = lane - lrow0 * nchunk, srow = 32 / nchunk, sch = 32 - srow * nchunk;
+        const int room = pv - (av0 - rj0);                 // columns of the region from av0 on
+        int flushed = Tu0, fslot = 0;                      // rows below `flushed` are final and written; ring slot of row `flushed`
+        auto flush = [&](int b) {                          // rows [flushed, b): ring -> HBM (inside the written box), slots back to zero
+            int i = flushed + lrow0, ch = lch0, sl = fslot + lrow0;
+            while (sl >= R) sl -= R;
+            while (__any_sync(0xffffffffu, i < b)) {
+                if (i < b) {
+                    float *rowp = oring + sl * pitch;
+                    const bool wr = i >= wu0 && i <= wu1;
+                    float *orow = oslice + (long long)i * pv;
+                    if (ADJ) {
+                        float2 *p = reinterpret_cast<float2 *>(rowp + 2 * ch);
+                        const float2 v = *p;
+                        *p = make_float2(0.f, 0.f);
+                        if (wr && 2 * ch + 2 <= room) *reinterpret_cast<float2 *>(orow + 2 * ch) = v;
+                    } else {
+                        float4 *p = reinterpret_cast<float4 *>(rowp + 4 * ch);
+                        const float4 v = *p;
+                        *p = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (wr && 4 * ch + 4 <= room) *reinterpret_cast<float4 *>(orow + 4 * ch) = v;
+                    }
+                }
+                ch += sch; i += srow; sl += srow;
+                if (ch >= nchunk) { ch -= nchunk; ++i; ++sl; }
+                while (sl >= R) sl -= R;
+            }
+            fslot += b - flushed;
+            while (fslot >= R) fslot -= R;
+            flushed = b;
+        };
+
+        const int n_units = npair * nt;
+        __syncwarp();                                      // Wd is complete; the previous item has left the ring zeroed
+        for (int u0 = 0; u0 < n_units;) {
+            const int p_lo = u0 / nt;
+            const int u1 = min(min(n_units, u0 + 32), (p_lo + maxp) * nt);       // units [u0, u1) of at most `maxp` row pairs
+            const int p_hi = (u1 - 1) / nt;
+            const int r_lo = in_u0 + 2 * p_lo, r_hi = in_u0 + 2 * p_hi;
+            {   // rows that no unit from here on reaches
+                const int lo = min(max(r_lo - CHk, Tu0), Tu1 + 1);
+                if (lo > flushed) flush(lo);
+            }
+            {   // stage the input rows of the group's pairs: per-lane column terms, then one pass over the rows
+                const float *sp[MCX];
+                unsigned dp[MCX];
+                int csz[MCX];
+                bool cex[MCX];
+#pragma unroll
+                for (int m = 0; m < MCX; ++m) {
+                    const int c = lane + 32 * m, j = av0 - C + c, q = c >> 1;
+                    const bool cin = j >= B.v0 && j <= B.v1;
+                    cex[m] = c < ncols;
+                    csz[m] = cin ? 4 : 0;
+                    sp[m] = sbase + (long long)(r_lo - ri0) * pv + (cin ? j - rj0 : 0);
+                    dp[m] = xin_s + 16u * (unsigned)(q ^ ((q >> 3) & 1)) + 8u * (unsigned)(c & 1);
+                }
+                const int nrow = 2 * (p_hi - p_lo + 1);
+                const int nin = min(nrow, in_u1 - r_lo + 1);      // only the second row of the last pair can lie outside the input rows
+                unsigned ro = 0;
+                for (int rl = 0; rl < nin; ++rl) {
+#pragma unroll
+                    for (int m = 0; m < MCX; ++m) {
+                        if (cex[m]) cp_async_4(dp[m] + ro, sp[m], csz[m]);
+                        sp[m] += pv;
+                    }
+                    ro += (rl & 1) ? 16u * (unsigned)PPc - 4u : 4u;
+                }
+                if (nin < nrow) {
+#pragma unroll
+                    for (int m = 0; m < MCX; ++m)
+                        if (cex[m]) cp_async_4(dp[m] + ro, sbase, 0);
+                }
+            }
+            cp_async_wait_all();
+            __syncwarp();
+
+            const int u = u0 + lane;
+            const bool active = u < u1;
+            const int p = active ? u / nt : p_lo, t = active ? u - p * nt : 0;
+            const int r = in_u0 + 2 * p;
+            float2 zc[FRF], z[C][FRF];                     // folded window: zc[c] = x[j_c], z[m-1][c] = x[j_c - m] + x[j_c + m], as (row r, row r+1)
+            {
+                float2 xx[XW];                             // (x[r][c], x[r+1][c]) of window column c
+                const float4 *xw = xin4 + (p - p_lo) * PPc;
+#pragma unroll
+                for (int mm = 0; mm < NXQ; ++mm) {
+                    const int q = 2 * t + mm;
+                    const float4 v = xw[q ^ ((q >> 3) & 1)];
+                    xx[2 * mm] = make_float2(v.x, v.y); xx[2 * mm + 1] = make_float2(v.z, v.w);
+                }
+#pragma unroll
+                for (int c = 0; c < FRF; ++c) {
+                    zc[c] = xx[c + C];
+#pragma unroll
+                    for (int m = 1; m <= C; ++m) z[m - 1][c] = __fadd2_rn(xx[c + C - m], xx[c + C + m]);
+                }
+            }
+            // steps whose two target rows lie outside the held rows for every unit of the group are skipped (adjoint halo)
+            int d_lo = 0;
+            if (ADJ) {
+                if (r_hi + 1 < Tu0) d_lo = Tu0 - r_hi - 1;
+                else if (r_lo > Tu1) d_lo = r_lo - Tu1;
+            }
+            if (active && CHk >= d_lo) macs += (unsigned long long)(CHk - d_lo + 1) * ((C + 1) * FRF * 2);
+            int rowm = r - CHk, rowp = r + 1 + CHk;
+            int sm = pmod(rowm - flushed + fslot, R), sp_ = pmod(rowp - flushed + fslot, R);
+            const float4 *wrow = Wd + CHk * WQ;
+            float *const obase = oring + FRF * t;
+            float2 accA[FRF], accB[FRF];
+#pragma unroll
+            for (int c = 0; c < FRF; ++c) accB[c] = make_float2(0.f, 0.f);
+            float4 w[WQ];
+#pragma unroll
+            for (int q = 0; q < WQ; ++q) w[q] = wrow[q];
+            auto held = [&](int row) { return active && (!ADJ || (row >= Tu0 && row <= Tu1)); };
+            int dd = CHk;
+#pragma unroll 1
+            for (; dd > d_lo; dd -= 2) {                   // two steps per trip: the accumulators swap roles, no register copies
+                fold_step<C>(zc, z, w, wrow - WQ, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
+                ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
+                __syncwarp();                              // the rows of this step are visible to the next one
+                wrow -= dd >= 2 ? 2 * WQ : WQ;             // row dd - 2 of the next trip (row 0 again after the last step: never used)
+                fold_step<C>(zc, z, w, wrow, accB, accA, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
+                ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
+                __syncwarp();
+            }
+            if (dd == d_lo) {                              // odd number of steps: the last one
+                fold_step<C>(zc, z, w, wrow, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
+                __syncwarp();
+            }
+            u0 = u1;
+        }
+        flush(Tu1 + 1);
+        __syncwarp();                                      // the next item overwrites Wd and the staged rows
+    }
+    if (macs) atomicAdd(reinterpret_cast<unsigned long long *>(ADJ ? &wc->macs_adj : &wc->macs_fwd), macs);
+}
+
+}  // namespace pdrt

@@ -49,7 +49,7 @@ struct Params {
     float dz;
     int tile_floats;                     // conv input-tile budget in shared memory [floats]
     int ntfc_max;                        // widest conv work item [thread-tiles along v]: NTFC_MAX (k_conv) or SYM_NTFC_MAX (k_conv_sym)
-    int conv_sym;                        // 1: the row-symmetric single-pass kernel runs (it counts its own multiply-adds)
+    int conv_sym;                        // 0: k_conv; 1: k_conv_sym (row-symmetric); 2: k_conv_fold (row- and column-symmetric); the last two count their own multiply-adds
     // fluence corrections
     int Tu_max, Tv_max;                  // largest Gaussian half-widths along u / v
     // ray marcher

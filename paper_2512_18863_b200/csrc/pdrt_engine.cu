@@ -14,6 +14,7 @@
 #include "../../include/pdrt.h"
 #include "pdrt_conv.cuh"
 #include "pdrt_conv_sym.cuh"
+#include "pdrt_conv_fold.cuh"
 #include "pdrt_depth.cuh"
 #include "pdrt_dev.cuh"
 #include "pdrt_fluence.cuh"
@@ -52,6 +53,12 @@ int conv_sym_adj_max()
 {
     if (const char *v = std::getenv("PDRT_CONV_SYM_ADJ_MAX")) return std::atoi(v);
     return 31;
+}
+// Largest compiled size that also folds the column symmetry (k_conv_fold): its folded window takes 8 (C + 2) registers.
+int conv_fold_max()
+{
+    if (const char *v = std::getenv("PDRT_CONV_FOLD_MAX")) return std::atoi(v);
+    return 25;
 }
 int conv_sym_fwd_min()
 {
@@ -131,7 +138,8 @@ struct pdrt_engine {
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
     bool sym_fwd = false, sym_adj = false;   // which directions run k_conv_sym (single pass; forward from 11 taps, adjoint from 11 to 31)
-    int conv_sym_per_sm[2][64] = {};     // the same for k_conv_sym, by [adjoint][KT]
+    int conv_sym_per_sm[2][64] = {};
+    int conv_fold_per_sm[2][32] = {};     // the same for k_conv_sym, by [adjoint][KT]
     int conv_per_sm[2][2][2][64] = {};   // resident conv blocks per SM on THIS engine's device, by [adjoint][copy width - 1][multi-pass][KT]; 0 = not queried yet
     DevBuf<float> coll;               // collimator angles [coll_n] set by pdrt_set_collimator (coll_n = 0: none)
     int coll_n = 0;
@@ -217,7 +225,7 @@ int gaussian_taps(double sigma, double D, std::vector<float> &g)
 // The work-item layout (chunk width, written box of D_b) follows the kernel that runs in this direction; k_fluence tabulates it per call.
 void set_conv_direction(pdrt_engine *e, bool adjoint)
 {
-    e->P.conv_sym = (adjoint ? e->sym_adj : e->sym_fwd) ? 1 : 0;
+    e->P.conv_sym = (adjoint ? e->sym_adj : e->sym_fwd) ? (e->P.KT <= conv_fold_max() ? 2 : 1) : 0;
     e->P.ntfc_max = e->P.conv_sym ? SYM_NTFC_MAX : NTFC_MAX;
 }
 
@@ -292,8 +300,28 @@ int launch_conv_pass(pdrt_engine *e, int cp0, int n, const float *wtab, const fl
     return PDRT_OK;
 }
 template <int KT, bool ADJ>
+int launch_conv_fold(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
+{
+    int &per_sm = e->conv_fold_per_sm[ADJ ? 1 : 0][KT];
+    const size_t smem = fold_smem_bytes(KT);
+    if (per_sm == 0) {
+        CU(e, cudaFuncSetAttribute(k_conv_fold<KT, ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int n_res = 0;
+        CU(e, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n_res, k_conv_fold<KT, ADJ>, CONV_THREADS, smem));
+        per_sm = n_res < 1 ? 1 : n_res;
+    }
+    e->conv_grid = e->sm_count * per_sm;              // persistent grid: a multiple of the SM count
+    k_conv_fold<KT, ADJ><<<e->conv_grid, CONV_THREADS, smem, st>>>(e->P, e->desc.p, cp0, n, e->tile_base.p, e->zrad.p, e->wtab.p, in, out,
+                                                                   e->tile_base.p + n + 1, e->counters.p, fold_in_floats(KT), fold_out_floats(KT));
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+template <int KT, bool ADJ>
 int launch_conv_sym(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
 {
+    if constexpr (KT <= 25) {
+        if (e->P.conv_sym == 2) return launch_conv_fold<KT, ADJ>(e, cp0, n, in, out, st);
+    }
     int &per_sm = e->conv_sym_per_sm[ADJ ? 1 : 0][KT];
     const size_t smem = sym_smem_bytes(KT);
     if (per_sm == 0) {
@@ -736,6 +764,7 @@ int pdrt_get_work(pdrt_engine *e, pdrt_work *w)
     w->kernel_size = e->P.K; w->kernel_size_compiled = e->P.KT;
     w->fan_rays = e->depth_mode == PDRT_DEPTH_FAN ? wc.fan_rays : 0;
     w->ray_samples = e->P.M_ray;
+    w->conv_symmetric = (e->last_backward ? e->sym_adj : e->sym_fwd) ? 1 : 0;
     return PDRT_OK;
 }
 

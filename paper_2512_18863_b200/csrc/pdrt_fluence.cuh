@@ -130,9 +130,10 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
                 wb.u1 = (short)min(P.Nu - 1, d.ri0 + min(d.nts - 1, (f.u1 - d.ri0) / RS) * RS + RS - 1);
                 wb.v0 = (short)(d.rj0 + (f.v0 - d.rj0) / RF * RF);
                 wb.v1 = (short)(d.rj0 + (f.v1 - d.rj0) / RF * RF + RF - 1);
-                if (P.conv_sym && d.ncf == 1) {     // k_conv_sym starts its tiles at the box (16-byte aligned), clipped to the region
+                if (P.conv_sym && d.ncf == 1) {     // k_conv_sym / k_conv_fold start their 8- / 4-column tiles at the box (16-byte aligned), clipped to the region
+                    const int tw = P.conv_sym == 2 ? 4 : RF;
                     wb.v0 = (short)(f.v0 & ~3);
-                    wb.v1 = (short)min(wb.v0 + ((f.v1 - wb.v0) / RF + 1) * RF - 1, d.rj0 + d.pv - 1);
+                    wb.v1 = (short)min(wb.v0 + ((f.v1 - wb.v0) / tw + 1) * tw - 1, d.rj0 + d.pv - 1);
                 }
             }
             sbox[(size_t)cp * P.Nw + k] = sb;

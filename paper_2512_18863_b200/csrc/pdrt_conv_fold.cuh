@@ -200,46 +200,51 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
         };
 
         const int n_units = npair * nt;
-        __syncwarp();                                      // Wd is complete; the previous item has left the ring zeroed
+        // units [u0, u1) of one group: at most 32, of at most `maxp` row pairs
+        auto group_end = [&](int u0) { return min(min(n_units, u0 + 32), (u0 / nt + maxp) * nt); };
+        // stage the input rows of a group's pairs (asynchronous copies, zero outside the source box): per-lane column terms, then one
+        // pass over the rows
+        auto stage = [&](int u0, int u1) {
+            const int p_lo = u0 / nt, p_hi = (u1 - 1) / nt, r_lo = in_u0 + 2 * p_lo;
+            const float *sp[MCX];
+            unsigned dp[MCX];
+            int csz[MCX];
+            bool cex[MCX];
+#pragma unroll
+            for (int m = 0; m < MCX; ++m) {
+                const int c = lane + 32 * m, j = av0 - C + c, q = c >> 1;
+                const bool cin = j >= B.v0 && j <= B.v1;
+                cex[m] = c < ncols;
+                csz[m] = cin ? 4 : 0;
+                sp[m] = sbase + (long long)(r_lo - ri0) * pv + (cin ? j - rj0 : 0);
+                dp[m] = xin_s + 16u * (unsigned)(q ^ ((q >> 3) & 1)) + 8u * (unsigned)(c & 1);
+            }
+            const int nrow = 2 * (p_hi - p_lo + 1);
+            const int nin = min(nrow, in_u1 - r_lo + 1);          // only the second row of the last pair can lie outside the input rows
+            unsigned ro = 0;
+            for (int rl = 0; rl < nin; ++rl) {
+#pragma unroll
+                for (int m = 0; m < MCX; ++m) {
+                    if (cex[m]) cp_async_4(dp[m] + ro, sp[m], csz[m]);
+                    sp[m] += pv;
+                }
+                ro += (rl & 1) ? 16u * (unsigned)PPc - 4u : 4u;
+            }
+            if (nin < nrow) {
+#pragma unroll
+                for (int m = 0; m < MCX; ++m)
+                    if (cex[m]) cp_async_4(dp[m] + ro, sbase, 0);
+            }
+        };
+        __syncwarp();                                      // Wd is complete; the previous item has left the ring zeroed and the staged rows free
+        stage(0, group_end(0));
         for (int u0 = 0; u0 < n_units;) {
-            const int p_lo = u0 / nt;
-            const int u1 = min(min(n_units, u0 + 32), (p_lo + maxp) * nt);       // units [u0, u1) of at most `maxp` row pairs
-            const int p_hi = (u1 - 1) / nt;
+            const int u1 = group_end(u0);
+            const int p_lo = u0 / nt, p_hi = (u1 - 1) / nt;
             const int r_lo = in_u0 + 2 * p_lo, r_hi = in_u0 + 2 * p_hi;
             {   // rows that no unit from here on reaches
                 const int lo = min(max(r_lo - CHk, Tu0), Tu1 + 1);
                 if (lo > flushed) flush(lo);
-            }
-            {   // stage the input rows of the group's pairs: per-lane column terms, then one pass over the rows
-                const float *sp[MCX];
-                unsigned dp[MCX];
-                int csz[MCX];
-                bool cex[MCX];
-#pragma unroll
-                for (int m = 0; m < MCX; ++m) {
-                    const int c = lane + 32 * m, j = av0 - C + c, q = c >> 1;
-                    const bool cin = j >= B.v0 && j <= B.v1;
-                    cex[m] = c < ncols;
-                    csz[m] = cin ? 4 : 0;
-                    sp[m] = sbase + (long long)(r_lo - ri0) * pv + (cin ? j - rj0 : 0);
-                    dp[m] = xin_s + 16u * (unsigned)(q ^ ((q >> 3) & 1)) + 8u * (unsigned)(c & 1);
-                }
-                const int nrow = 2 * (p_hi - p_lo + 1);
-                const int nin = min(nrow, in_u1 - r_lo + 1);      // only the second row of the last pair can lie outside the input rows
-                unsigned ro = 0;
-                for (int rl = 0; rl < nin; ++rl) {
-#pragma unroll
-                    for (int m = 0; m < MCX; ++m) {
-                        if (cex[m]) cp_async_4(dp[m] + ro, sp[m], csz[m]);
-                        sp[m] += pv;
-                    }
-                    ro += (rl & 1) ? 16u * (unsigned)PPc - 4u : 4u;
-                }
-                if (nin < nrow) {
-#pragma unroll
-                    for (int m = 0; m < MCX; ++m)
-                        if (cex[m]) cp_async_4(dp[m] + ro, sbase, 0);
-                }
             }
             cp_async_wait_all();
             __syncwarp();
@@ -258,6 +263,8 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
                     const float4 v = xw[q ^ ((q >> 3) & 1)];
                     xx[2 * mm] = make_float2(v.x, v.y); xx[2 * mm + 1] = make_float2(v.z, v.w);
                 }
+                __syncwarp();                              // every lane holds its window: the staged rows are free again ...
+                if (u1 < n_units) stage(u1, group_end(u1));    // ... for the next group's rows, which arrive behind this group's arithmetic
 #pragma unroll
                 for (int c = 0; c < FRF; ++c) {
                     zc[c] = xx[c + C];

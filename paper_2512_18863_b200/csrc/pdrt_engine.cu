@@ -225,7 +225,7 @@ int gaussian_taps(double sigma, double D, std::vector<float> &g)
 // The work-item layout (chunk width, written box of D_b) follows the kernel that runs in this direction; k_fluence tabulates it per call.
 void set_conv_direction(pdrt_engine *e, bool adjoint)
 {
-    e->P.conv_sym = (adjoint ? e->sym_adj : e->sym_fwd) ? (e->P.KT <= conv_fold_max() ? 2 : 1) : 0;
+    e->P.conv_sym = (adjoint ? e->sym_adj : e->sym_fwd) ? (e->P.KT >= 15 && e->P.KT <= conv_fold_max() ? 2 : 1) : 0;   // measured: the fold pays from 15 taps
     e->P.ntfc_max = e->P.conv_sym ? SYM_NTFC_MAX : NTFC_MAX;
 }
 

@@ -43,6 +43,24 @@ __device__ __forceinline__ float blur_at(const float *m, const Params &P, const 
     return s;
 }
 
+// A bbox-confined map either in shared memory (pitch = bbox width, origin = bbox corner) or in its global scratch plane (pitch Nuf).
+struct MapView {
+    float *p; int pitch, oa, ob;
+    __device__ __forceinline__ float &at(int a, int b) const { return p[(b - ob) * pitch + (a - oa)]; }
+};
+// value at (a,b); zero outside the box [a0,a1] x [b0,b1] (zero padding of the blurs)
+__device__ __forceinline__ float view_at(const MapView &m, int a0, int a1, int b0, int b1, int a, int b)
+{
+    return (a >= a0 && a <= a1 && b >= b0 && b <= b1) ? m.at(a, b) : 0.f;
+}
+__device__ __forceinline__ float view_blur(const MapView &m, const CpDesc &d, int a, int b, int axis, int T, const float *g)
+{
+    float s = 0.f;
+    for (int t = -T; t <= T; ++t) s += g[t + T] * view_at(m, d.a0, d.a1, d.b0, d.b1, axis == 0 ? a + t : a, axis == 1 ? b + t : b);
+    return s;
+}
+constexpr int FLU_TILE = 3072;       // pixels of a support bbox that k_fluence keeps in shared memory (three planes)
+
 // Builds CpDesc: gantry axes, jaw and support bboxes, compact region, conv chunking, work counters.
 __device__ void build_desc(const Params &P, const float *jaws, float gantry_deg, float coll_deg, float mu, CpDesc &d)
 {
@@ -151,7 +169,12 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
                 }
             ta += (unsigned long long)P.NB * P.NB * ((s.u1 - d.ri0) / RS - (s.u0 - d.ri0) / RS + 1) * ((s.v1 - d.rj0) / RF - (s.v0 - d.rj0) / RF + 1);
         }
-        atomicAdd(&cnt[0], sup); atomicAdd(&cnt[1], fp); atomicAdd(&cnt[2], tf); atomicAdd(&cnt[3], ta);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            sup += __shfl_xor_sync(0xffffffffu, sup, o); fp += __shfl_xor_sync(0xffffffffu, fp, o);
+            tf += __shfl_xor_sync(0xffffffffu, tf, o); ta += __shfl_xor_sync(0xffffffffu, ta, o);
+        }
+        if ((tid & 31) == 0) { atomicAdd(&cnt[0], sup); atomicAdd(&cnt[1], fp); atomicAdd(&cnt[2], tf); atomicAdd(&cnt[3], ta); }
     }
     __syncthreads();
     if (tid == 0) {
@@ -164,10 +187,19 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
     if (empty) return;
 
     const size_t mo = (size_t)cp * P.Nuf * P.Nvf;
-    float *p0 = P0 + mo, *t1 = T1 + mo, *t2 = T2 + mo, *Am = Abuf + mo, *pm = phimap + mo, *pmT = phimapT + mo;
+    float *Am = Abuf + mo, *pm = phimap + mo, *pmT = phimapT + mo;
     const float *lv = leaves + (size_t)cp * 2 * P.Np, *jw = jaws + 4 * cp;
     const int bw = d.a1 - d.a0 + 1, bh = d.b1 - d.b0 + 1, npx = bw * bh;
+    const int pw = d.pa1 - d.pa0 + 1, ph = d.pb1 - d.pb0 + 1, npp = pw * ph;
     const float x1 = jw[0], x2 = jw[1], y1 = jw[2], y2 = jw[3];
+    const bool rotated = d.sc != 0.f || d.cc != 1.f;
+    // The intermediate maps (Phi0, the blur temporaries, the map itself) live in shared memory when the support bbox fits: every
+    // pass is then a chain of shared-memory round trips instead of L2 ones.  Larger fields work in the global scratch planes.
+    __shared__ float tile[3][FLU_TILE];
+    const bool in_smem = npx <= FLU_TILE && npp <= FLU_TILE;
+    const MapView vP0 = in_smem ? MapView{ tile[0], bw, d.a0, d.b0 } : MapView{ P0 + mo, P.Nuf, 0, 0 };
+    const MapView vT = in_smem ? MapView{ tile[1], bw, d.a0, d.b0 } : MapView{ T1 + mo, P.Nuf, 0, 0 };
+    const MapView vM = in_smem ? MapView{ tile[2], bw, d.a0, d.b0 } : MapView{ pm, P.Nuf, 0, 0 };
 
     // leaf pairs that can overlap each pixel row of the jaw opening (the bounds are ascending): once per row
     __shared__ short leaf_lo[FLU_MAX_ROWS], leaf_hi[FLU_MAX_ROWS];
@@ -195,31 +227,31 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
             }
             J = ov(uf, P.Du, x1, x2) * ov(vf, P.Dv, y1, y2);
         }
-        Am[b * P.Nuf + a] = A;
-        p0[b * P.Nuf + a] = J * (P.tau + (1.f - P.tau) * A);
+        Am[b * P.Nuf + a] = A;                               // read again by k_fluence_adjoint
+        vP0.at(a, b) = J * (P.tau + (1.f - P.tau) * A);
     }
     __syncthreads();
     // O3: penumbra, u with the MLC width then v with the jaw width
     for (int p = tid; p < npx; p += FLU_THREADS) {
         const int a = d.a0 + p % bw, b = d.b0 + p / bw;
-        t1[b * P.Nuf + a] = blur_at(p0, P, d, a, b, 0, T.Tu, T.gu);
+        vT.at(a, b) = view_blur(vP0, d, a, b, 0, T.Tu, T.gu);
     }
     __syncthreads();
     for (int p = tid; p < npx; p += FLU_THREADS) {
         const int a = d.a0 + p % bw, b = d.b0 + p / bw;
-        pm[b * P.Nuf + a] = blur_at(t1, P, d, a, b, 1, T.Tv, T.gv);
+        vM.at(a, b) = view_blur(vT, d, a, b, 1, T.Tv, T.gv);
     }
     // O4: head scatter
     for (int q = 0; q < T.n_hs; ++q) {
         __syncthreads();
         for (int p = tid; p < npx; p += FLU_THREADS) {
             const int a = d.a0 + p % bw, b = d.b0 + p / bw;
-            t2[b * P.Nuf + a] = blur_at(p0, P, d, a, b, 1, T.hs_Tv[q], T.hs_gv[q]);
+            vT.at(a, b) = view_blur(vP0, d, a, b, 1, T.hs_Tv[q], T.hs_gv[q]);
         }
         __syncthreads();
         for (int p = tid; p < npx; p += FLU_THREADS) {
             const int a = d.a0 + p % bw, b = d.b0 + p / bw;
-            pm[b * P.Nuf + a] += T.hs_amp[q] * blur_at(t2, P, d, a, b, 0, T.hs_Tu[q], T.hs_gu[q]);
+            vM.at(a, b) += T.hs_amp[q] * view_blur(vT, d, a, b, 0, T.hs_Tu[q], T.hs_gu[q]);
         }
     }
     __syncthreads();
@@ -227,13 +259,14 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
     for (int p = tid; p < npx; p += FLU_THREADS) {
         const int a = d.a0 + p % bw, b = d.b0 + p / bw;
         const float uf = flu_u(P, a), vf = flu_v(P, b);
-        pm[b * P.Nuf + a] *= oar_factor(T, sqrtf(uf * uf + vf * vf));
+        vM.at(a, b) *= oar_factor(T, sqrtf(uf * uf + vf * vf));
     }
     __syncthreads();
     // collimator rotation (G25): the map is resampled (bilinear_0) on its own grid at R(-phi_c) of
     // each pixel centre; from here on the map lives in the projection frame (bbox pa0..pb1)
-    const int pw = d.pa1 - d.pa0 + 1, ph = d.pb1 - d.pb0 + 1, npp = pw * ph;
-    if (d.sc != 0.f || d.cc != 1.f) {
+    MapView vF = vM;                                         // the final map
+    if (rotated) {
+        const MapView vR = in_smem ? MapView{ tile[1], pw, d.pa0, d.pb0 } : MapView{ T1 + mo, P.Nuf, 0, 0 };
         for (int p = tid; p < npp; p += FLU_THREADS) {
             const int a = d.pa0 + p % pw, b = d.pb0 + p / pw;
             const float u = flu_u(P, a), v = flu_v(P, b);
@@ -241,22 +274,26 @@ k_fluence(Params P, FluTables T, int n_cp, const float *__restrict__ leaves, con
             const float fla = floorf(fa), flb = floorf(fb);
             const int ia = (int)fla, ib = (int)flb;
             const float ta = fa - fla, tb = fb - flb;
-            t1[b * P.Nuf + a] = (1.f - tb) * ((1.f - ta) * at_bbox(pm, P, d, ia, ib) + ta * at_bbox(pm, P, d, ia + 1, ib)) +
-                                tb * ((1.f - ta) * at_bbox(pm, P, d, ia, ib + 1) + ta * at_bbox(pm, P, d, ia + 1, ib + 1));
+            vR.at(a, b) = (1.f - tb) * ((1.f - ta) * view_at(vM, d.a0, d.a1, d.b0, d.b1, ia, ib) + ta * view_at(vM, d.a0, d.a1, d.b0, d.b1, ia + 1, ib)) +
+                          tb * ((1.f - ta) * view_at(vM, d.a0, d.a1, d.b0, d.b1, ia, ib + 1) + ta * view_at(vM, d.a0, d.a1, d.b0, d.b1, ia + 1, ib + 1));
         }
         __syncthreads();
-        for (int p = tid; p < npx; p += FLU_THREADS) pm[(d.b0 + p / bw) * P.Nuf + d.a0 + p % bw] = 0.f;
-        __syncthreads();
+        vF = vR;
+        if (!in_smem) {     // the global plane of the map held the collimator-frame values: clear them, the projection-frame box follows
+            for (int p = tid; p < npx; p += FLU_THREADS) pm[(d.b0 + p / bw) * P.Nuf + d.a0 + p % bw] = 0.f;
+            __syncthreads();
+        }
+    }
+    // the map [b][a] (k_fluence_adjoint, stage tap) and the same with v fastest (k_project stages that one)
+    if (in_smem || rotated) {
         for (int p = tid; p < npp; p += FLU_THREADS) {
             const int a = d.pa0 + p % pw, b = d.pb0 + p / pw;
-            pm[b * P.Nuf + a] = t1[b * P.Nuf + a];
+            pm[b * P.Nuf + a] = vF.at(a, b);
         }
-        __syncthreads();
     }
-    // the same map with v fastest, for the conv tile fill (lanes run along v there)
     for (int p = tid; p < npp; p += FLU_THREADS) {
         const int a = d.pa0 + p / ph, b = d.pb0 + p % ph;
-        pmT[a * P.Nvf + b] = pm[b * P.Nuf + a];
+        pmT[a * P.Nvf + b] = vF.at(a, b);
     }
 }
 

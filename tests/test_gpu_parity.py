@@ -322,6 +322,29 @@ def test_wide_single_pass_variants(torch, monkeypatch):
         assert_grad(dm, rm, f"split k={k} d_mu"); assert_grad(dl, rl, f"split k={k} d_leaves")
 
 
+@pytest.mark.parametrize("mode", ["default", "row_symmetric", "output_stationary"])
+def test_convolution_kernel_families_on_a_field_wider_than_one_work_item(torch, monkeypatch, mode):
+    """The three convolution kernels (k_conv_fold: row + column symmetry, 15..25 taps; k_conv_sym: row symmetry; k_conv:
+    output-stationary) on a field so long in v that a slice is split into two work items (chunks along v), forward and adjoint,
+    and pdrt_work.conv_symmetric."""
+    if mode == "row_symmetric":
+        monkeypatch.setenv("PDRT_CONV_FOLD_MAX", "0")
+    elif mode == "output_stationary":
+        monkeypatch.setenv("PDRT_CONV_LEGACY", "1")
+    wl = W.tiny(seed=21, nx=44, ny=40, nz=110, spacing=2.5, n_cp=2, n_pairs=20, kernel_size=21, flu=(24, 110), flu_d=2.5, head_scatter=False)
+    eng, orc = pair(wl)
+    for k in (21, 11):
+        eng.set_kernel_size(k)
+        orc.set_kernel_size(k)
+        assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), f"{mode} k={k}")
+        wf = eng.get_work()
+        assert wf.conv_items > 2 * wl.n_cp * eng.info.beam_nw * 0.5 and wf.conv_symmetric == (0 if mode == "output_stationary" else 1)
+        g = W.seeded_dose_gradient(wl, seed=k)
+        dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+        rl, rj, rm = orc.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+        assert_grad(dm, rm, f"{mode} k={k} d_mu"); assert_grad(dl, rl, f"{mode} k={k} d_leaves"); assert_grad(dj, rj, f"{mode} k={k} d_jaws")
+
+
 @pytest.mark.parametrize("k", [11, 31, 41, 55])
 def test_config4_kernel_size_sweep_sampled(torch, k):
     """The other kernel sizes of the c4 sweep at full size, and the paper's operating point k = 55: sampled

@@ -2,44 +2,46 @@
 // (the pencil kernel is radially symmetric; R3: the table is built mirrored in both axes).
 //
 // A row correlation is  T_d[r][j] = W_d[C] x[r][j] + sum_{m=1..C} W_d[C+m] (x[r][j-m] + x[r][j+m]),  W_d = row C+d of the slice
-// kernel.  The folded window  z[j][m] = x[r][j-m] + x[r][j+m]  does not depend on d: a unit = (row pair r, r+1) x 4 output columns
-// builds its 4 x (C+1) folded values once (packed adds on the (row r, row r+1) pairs) and then runs the C+1 steps d = C .. 0 with
+// kernel.  The folded window  z[j][m] = x[r][j-m] + x[r][j+m]  does not depend on d: a unit = (row pair r, r+1) x W output columns
+// (W = 4 up to 31 taps, 2 above) builds its W x (C+1) folded values once (packed adds on the (row r, row r+1) pairs) and then runs the C+1 steps d = C .. 0 with
 // C+1 packed FFMA2 per column instead of 2C+1.  Together with the row symmetry that is (C+1)^2 multiply-adds per input value
 // instead of (2C+1)^2.  Everything else is pdrt_conv_sym.cuh: one warp per block, units of 32 lanes, output rows accumulated in a
-// warp-private shared-memory ring (one 16-byte read-modify-write per side and step), staged input rows, rows written to HBM
-// when no later unit reaches them.  The folded window takes 8 (C+2) registers, so this form serves kernels up to 25 taps.
+// warp-private shared-memory ring (one 16- or 8-byte read-modify-write per side and step), staged input rows, rows written to HBM
+// when no later unit reaches them.  The folded window takes 2 W (C+2) registers.
 #pragma once
 #include "pdrt_conv_sym.cuh"
 
 namespace pdrt {
 
-constexpr int FRF = 4;                 // output columns per unit
-constexpr int FOLD_NT4_MAX = 2 * SYM_NTFC_MAX;      // widest work item [tiles of 4 columns]
+constexpr int FOLD_COLS_MAX = 8 * SYM_NTFC_MAX;     // widest work item [columns]
+// output columns per unit: 4 up to 31 taps, 2 above (the folded window takes 2 W (C + 2) registers)
+__host__ __device__ constexpr int fold_unit_cols(int kt) { return kt <= 31 ? 4 : 2; }
 
-// ring row pitch [floats]: one 16-byte chunk per tile; padded until the chunks of the next row pair (two rows on) continue where
-// this row ends, give or take one chunk (modulo the 8 chunks of a wavefront)
-__host__ __device__ __forceinline__ int fold_out_pitch(int nt4)
+// ring row pitch [floats] for nt units of w columns.  Units of 4 columns: one 16-byte chunk per unit, padded until the chunks of
+// the next row pair (two rows on) continue where this row ends, give or take one chunk (modulo the 8 chunks of a wavefront).
+__host__ __device__ __forceinline__ int fold_out_pitch(int nt, int w)
 {
-    for (int p = 4 * nt4;; p += 4) {
+    if (w != 4) return (w * nt + 3) & ~3;
+    for (int p = 4 * nt;; p += 4) {
         const int dl = (p >> 1) & 7;
-        if (dl == (nt4 & 7) || dl == ((nt4 + 1) & 7) || dl == ((nt4 - 1) & 7)) return p;
+        if (dl == (nt & 7) || dl == ((nt + 1) & 7) || dl == ((nt - 1) & 7)) return p;
     }
 }
-__host__ __device__ __forceinline__ int fold_max_pairs(int nt4) { return (30 + nt4) / nt4 + 1 < 8 ? (30 + nt4) / nt4 + 1 : 8; }
+__host__ __device__ __forceinline__ int fold_max_pairs(int nt) { return (30 + nt) / nt + 1 < 8 ? (30 + nt) / nt + 1 : 8; }
 // 16-byte chunks (2 columns x 2 rows) per staged row pair (even: the swizzle swaps neighbours)
-__host__ __device__ __forceinline__ int fold_in_chunks(int nt4, int c) { return (2 * nt4 + c + 1) & ~1; }
+__host__ __device__ __forceinline__ int fold_in_chunks(int nt, int w, int c) { return ((w * nt + 2 * c) / 2 + 1) & ~1; }
 inline int fold_out_floats(int kt)
 {
-    const int c = (kt - 1) / 2;
+    const int c = (kt - 1) / 2, w = fold_unit_cols(kt);
     int best = 0;
-    for (int n = 1; n <= FOLD_NT4_MAX; ++n) best = std::max(best, (2 * fold_max_pairs(n) + 2 * c) * fold_out_pitch(n));
+    for (int n = 1; n <= FOLD_COLS_MAX / w; ++n) best = std::max(best, (2 * fold_max_pairs(n) + 2 * c) * fold_out_pitch(n, w));
     return best;
 }
 inline int fold_in_floats(int kt)
 {
-    const int c = (kt - 1) / 2;
+    const int c = (kt - 1) / 2, w = fold_unit_cols(kt);
     int best = 0;
-    for (int n = 1; n <= FOLD_NT4_MAX; ++n) best = std::max(best, fold_max_pairs(n) * fold_in_chunks(n, c) * 4);
+    for (int n = 1; n <= FOLD_COLS_MAX / w; ++n) best = std::max(best, fold_max_pairs(n) * fold_in_chunks(n, w, c) * 4);
     return best;
 }
 __host__ __device__ constexpr int fold_wpitch(int kt) { return ((kt - 1) / 2 + 1 + 3) & ~3; }         // floats per weight row: W_d[C .. 2C], padded to 4
@@ -52,7 +54,7 @@ inline size_t fold_smem_bytes(int kt)
 // One step d of a unit: acc = (a_d, b_d) from the folded window and the weight row in `w`; then the next step's weights are fetched
 // and out[r-d] += a_d + b_{d+1}, out[r+1+d] += b_d + a_{d+1} with (a_{d+1}, b_{d+1}) = prev.  om / op: the unit's 4 columns of the two
 // ring rows, null when the row is not held.
-template <int C>
+template <int C, int FRF>
 __device__ __forceinline__ void fold_step(const float2 (&zc)[FRF], const float2 (&z)[C][FRF], float4 (&w)[(C + 4) / 4], const float4 *__restrict__ wnext,
                                           float2 (&acc)[FRF], const float2 (&prev)[FRF], float *om, float *op)
 {
@@ -72,32 +74,49 @@ __device__ __forceinline__ void fold_step(const float2 (&zc)[FRF], const float2 
     }
 #pragma unroll
     for (int q = 0; q < WQ; ++q) w[q] = wnext[q];
-    if (om) {
-        float4 *o = reinterpret_cast<float4 *>(om);
-        float4 v = *o;
-        v.x += acc[0].x + prev[0].y; v.y += acc[1].x + prev[1].y; v.z += acc[2].x + prev[2].y; v.w += acc[3].x + prev[3].y;
-        *o = v;
-    }
-    if (op) {
-        float4 *o = reinterpret_cast<float4 *>(op);
-        float4 v = *o;
-        v.x += acc[0].y + prev[0].x; v.y += acc[1].y + prev[1].x; v.z += acc[2].y + prev[2].x; v.w += acc[3].y + prev[3].x;
-        *o = v;
+    if constexpr (FRF == 4) {
+        if (om) {
+            float4 *o = reinterpret_cast<float4 *>(om);
+            float4 v = *o;
+            v.x += acc[0].x + prev[0].y; v.y += acc[1].x + prev[1].y; v.z += acc[2].x + prev[2].y; v.w += acc[3].x + prev[3].y;
+            *o = v;
+        }
+        if (op) {
+            float4 *o = reinterpret_cast<float4 *>(op);
+            float4 v = *o;
+            v.x += acc[0].y + prev[0].x; v.y += acc[1].y + prev[1].x; v.z += acc[2].y + prev[2].x; v.w += acc[3].y + prev[3].x;
+            *o = v;
+        }
+    } else {
+        static_assert(FRF == 2 || FRF == 4, "units are 2 or 4 columns wide");
+        if (om) {
+            float2 *o = reinterpret_cast<float2 *>(om);
+            float2 v = *o;
+            v.x += acc[0].x + prev[0].y; v.y += acc[1].x + prev[1].y;
+            *o = v;
+        }
+        if (op) {
+            float2 *o = reinterpret_cast<float2 *>(op);
+            float2 v = *o;
+            v.x += acc[0].y + prev[0].x; v.y += acc[1].y + prev[1].x;
+            *o = v;
+        }
     }
 }
 
 template <int KT, bool ADJ>
-__global__ void __maxnreg__(168)
+__global__ void __maxnreg__(KT <= 25 ? 168 : 255)
 k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
             const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
             int *item_counter, WorkCounters *wc, int in_floats, int out_floats)
 {
     constexpr int C = (KT - 1) / 2;
+    constexpr int FRF = fold_unit_cols(KT);           // output columns per unit
     constexpr int KP = (KT + 3) & ~3;                 // row pitch of the table image [floats]
     constexpr int WP = fold_wpitch(KT), WQ = WP / 4;  // weight row W_d[C .. 2C] in shared memory [floats], LDS.128 per row
-    constexpr int XW = KT + FRF - 1;                  // window along v [columns]: 2C + 4, even
+    constexpr int XW = KT + FRF - 1;                  // window along v [columns]: 2C + FRF, even
     constexpr int NXQ = XW / 2;                       // LDS.128 per window (2 columns x 2 rows each)
-    constexpr int MCX = (4 * FOLD_NT4_MAX + 2 * C + 31) / 32;    // staged columns per lane and row
+    constexpr int MCX = (FOLD_COLS_MAX + 2 * C + 31) / 32;       // staged columns per lane and row
     extern __shared__ float4 smem4[];
     float4 *Wd = smem4;                               // [C+1 (d)][WQ]: kernel row C+d, columns C .. 2C, zero past them
     float4 *xin4 = smem4 + (C + 1) * WQ;              // [pair][chunk]: (x[r][c], x[r+1][c], x[r][c+1], x[r+1][c+1]), chunks swizzled
@@ -132,10 +151,11 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
         const int ctf0 = cf * ntfc, ctf1 = min(ntf, ctf0 + ntfc);
         const int atf0 = max(ctf0, (A.v0 - rj0) / RF), atf1 = min(ctf1 - 1, (A.v1 - rj0) / RF);
         if (atf0 > atf1) continue;
-        int nt = 2 * (atf1 - atf0 + 1), av0 = rj0 + atf0 * RF;
-        if (ncf == 1) {     // k_fluence tabulates the same columns as the written box; forward stores are 16-byte, adjoint stores 8-byte aligned
+        int nt = (RF / FRF) * (atf1 - atf0 + 1), av0 = rj0 + atf0 * RF;
+        if (ncf == 1) {     // forward: whole 4-column (16-byte) groups from the box on, the columns k_fluence tabulates as the written box;
+                            // adjoint: 8-byte aligned stores
             av0 = ADJ ? A.v0 & ~1 : A.v0 & ~3;
-            nt = (A.v1 - av0) / FRF + 1;
+            nt = ADJ ? (A.v1 - av0) / FRF + 1 : (4 / FRF) * ((A.v1 - av0) / 4 + 1);
         }
         // rows: input row pairs, output rows held in the ring (T), output rows written to HBM (wu)
         const int in_u0 = B.u0, in_u1 = B.u1, npair = (in_u1 - in_u0 + 2) >> 1;
@@ -146,8 +166,8 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
             wu1 = min(P.Nu - 1, ri0 + min(nts - 1, (F.u1 - ri0) / RS) * RS + RS - 1);
             Tu0 = min(wu0, in_u0 - CHk); Tu1 = max(wu1, in_u0 + 2 * npair - 1 + CHk);
         }
-        const int pitch = fold_out_pitch(nt), R = out_floats / pitch;
-        const int PPc = fold_in_chunks(nt, C), maxp = fold_max_pairs(nt);
+        const int pitch = fold_out_pitch(nt, FRF), R = out_floats / pitch;
+        const int PPc = fold_in_chunks(nt, FRF, C), maxp = fold_max_pairs(nt);
         const int ncols = FRF * nt + 2 * C;
         const long long slice_off = (long long)slot * P.stride_cp + (long long)k * pu * pv;
         const float *sbase = in + slice_off;
@@ -166,7 +186,7 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
             }
         }
         // flush geometry: the lanes walk the 16-byte (forward) / 8-byte (adjoint) chunks of consecutive rows, 32 chunks per trip
-        const int nchunk = ADJ ? 2 * nt : nt;
+        const int nchunk = ADJ ? FRF * nt / 2 : FRF * nt / 4;
         const int lrow0 = lane / nchunk, lch0 = lane - lrow0 * nchunk, srow = 32 / nchunk, sch = 32 - srow * nchunk;
         const int room = pv - (av0 - rj0);                 // columns of the region from av0 on
         int flushed = Tu0, fslot = 0;                      // rows below `flushed` are final and written; ring slot of row `flushed`
@@ -259,7 +279,7 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
                 const float4 *xw = xin4 + (p - p_lo) * PPc;
 #pragma unroll
                 for (int mm = 0; mm < NXQ; ++mm) {
-                    const int q = 2 * t + mm;
+                    const int q = (FRF / 2) * t + mm;
                     const float4 v = xw[q ^ ((q >> 3) & 1)];
                     xx[2 * mm] = make_float2(v.x, v.y); xx[2 * mm + 1] = make_float2(v.z, v.w);
                 }
@@ -293,16 +313,16 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
             int dd = CHk;
 #pragma unroll 1
             for (; dd > d_lo; dd -= 2) {                   // two steps per trip: the accumulators swap roles, no register copies
-                fold_step<C>(zc, z, w, wrow - WQ, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
+                fold_step<C, FRF>(zc, z, w, wrow - WQ, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
                 ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
                 __syncwarp();                              // the rows of this step are visible to the next one
                 wrow -= dd >= 2 ? 2 * WQ : WQ;             // row dd - 2 of the next trip (row 0 again after the last step: never used)
-                fold_step<C>(zc, z, w, wrow, accB, accA, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
+                fold_step<C, FRF>(zc, z, w, wrow, accB, accA, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
                 ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
                 __syncwarp();
             }
             if (dd == d_lo) {                              // odd number of steps: the last one
-                fold_step<C>(zc, z, w, wrow, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
+                fold_step<C, FRF>(zc, z, w, wrow, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
                 __syncwarp();
             }
             u0 = u1;

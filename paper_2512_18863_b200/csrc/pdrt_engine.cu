@@ -45,20 +45,19 @@ bool conv_legacy()
     const char *v = std::getenv("PDRT_CONV_LEGACY");
     return v && std::atoi(v) != 0;
 }
-// Largest compiled size for which the ADJOINT also runs in row-symmetric form.  The forward shares every row correlation between two
-// output rows; the adjoint only where both rows r-d and r+d lie in S_k, i.e. for supports taller than the kernel, and its wide-window
-// variants hold fewer warps per SM.  Measured: at 31 taps it loses 10 % on c4 (supports 34 rows tall) and wins 37 % on c5
-// (taller supports); from 41 taps on the output-stationary kernel wins on both.
+// Largest compiled size for which the ADJOINT also runs in symmetric form.  The forward shares every row correlation between two output
+// rows; the adjoint only where both rows r-d and r+d lie in S_k, so it gains less on supports shorter than the kernel.  With the column
+// symmetry folded in as well (k_conv_fold) it wins at every single-pass size measured; the knob stays for experiments.
 int conv_sym_adj_max()
 {
     if (const char *v = std::getenv("PDRT_CONV_SYM_ADJ_MAX")) return std::atoi(v);
-    return 31;
+    return 55;
 }
-// Largest compiled size that also folds the column symmetry (k_conv_fold): its folded window takes 8 (C + 2) registers.
+// Largest compiled size that also folds the column symmetry (k_conv_fold; units of 4 columns up to 31 taps, of 2 above).
 int conv_fold_max()
 {
-    if (const char *v = std::getenv("PDRT_CONV_FOLD_MAX")) return std::atoi(v);
-    return 25;
+    if (const char *v = std::getenv("PDRT_CONV_FOLD_MAX")) return std::min(55, std::atoi(v));
+    return 55;
 }
 int conv_sym_fwd_min()
 {
@@ -137,9 +136,9 @@ struct pdrt_engine {
     bool last_backward = false;
     cudaStream_t last_stream = nullptr;
     int conv_grid = 0;
-    bool sym_fwd = false, sym_adj = false;   // which directions run k_conv_sym (single pass; forward from 11 taps, adjoint from 11 to 31)
+    bool sym_fwd = false, sym_adj = false;   // which directions run k_conv_sym / k_conv_fold (single pass, from 11 taps)
     int conv_sym_per_sm[2][64] = {};
-    int conv_fold_per_sm[2][32] = {};     // the same for k_conv_sym, by [adjoint][KT]
+    int conv_fold_per_sm[2][64] = {};     // the same for k_conv_sym, by [adjoint][KT]
     int conv_per_sm[2][2][2][64] = {};   // resident conv blocks per SM on THIS engine's device, by [adjoint][copy width - 1][multi-pass][KT]; 0 = not queried yet
     DevBuf<float> coll;               // collimator angles [coll_n] set by pdrt_set_collimator (coll_n = 0: none)
     int coll_n = 0;
@@ -319,7 +318,7 @@ int launch_conv_fold(pdrt_engine *e, int cp0, int n, const float *in, float *out
 template <int KT, bool ADJ>
 int launch_conv_sym(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
 {
-    if constexpr (KT <= 25) {
+    if constexpr (KT >= 15 && KT <= 55) {
         if (e->P.conv_sym == 2) return launch_conv_fold<KT, ADJ>(e, cp0, n, in, out, st);
     }
     int &per_sm = e->conv_sym_per_sm[ADJ ? 1 : 0][KT];

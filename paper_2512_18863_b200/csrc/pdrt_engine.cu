@@ -36,7 +36,7 @@ const int kMaxKernel = 255;            // NB = 9 passes per axis of KT = 31 at m
 int conv_single_max()
 {
     if (const char *v = std::getenv("PDRT_CONV_SINGLE_MAX")) { const int m = std::atoi(v); if (m >= 3 && m <= 63) return m; }
-    return 55;       // measured on c4: one pass wins up to 55 taps, 3 x 3 passes of 21 from 63 on
+    return 63;       // measured on c4: one pass (k_conv_fold) wins up to the widest compiled variant, 63 taps
 }
 // The single-pass convolution runs in row-symmetric form (k_conv_sym) unless PDRT_CONV_LEGACY=1 asks for the output-stationary
 // kernel (k_conv), which also serves the sub-kernel passes of a split (their off-centre blocks are not symmetric by themselves).
@@ -51,13 +51,13 @@ bool conv_legacy()
 int conv_sym_adj_max()
 {
     if (const char *v = std::getenv("PDRT_CONV_SYM_ADJ_MAX")) return std::atoi(v);
-    return 55;
+    return 63;
 }
 // Largest compiled size that also folds the column symmetry (k_conv_fold; units of 4 columns up to 31 taps, of 2 above).
 int conv_fold_max()
 {
-    if (const char *v = std::getenv("PDRT_CONV_FOLD_MAX")) return std::min(55, std::atoi(v));
-    return 55;
+    if (const char *v = std::getenv("PDRT_CONV_FOLD_MAX")) return std::atoi(v);
+    return 63;
 }
 int conv_sym_fwd_min()
 {
@@ -318,7 +318,7 @@ int launch_conv_fold(pdrt_engine *e, int cp0, int n, const float *in, float *out
 template <int KT, bool ADJ>
 int launch_conv_sym(pdrt_engine *e, int cp0, int n, const float *in, float *out, cudaStream_t st)
 {
-    if constexpr (KT >= 15 && KT <= 55) {
+    if constexpr (KT >= 15) {
         if (e->P.conv_sym == 2) return launch_conv_fold<KT, ADJ>(e, cp0, n, in, out, st);
     }
     int &per_sm = e->conv_sym_per_sm[ADJ ? 1 : 0][KT];

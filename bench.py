@@ -327,7 +327,7 @@ def run_c5_loop(args):
                 graph_loop_ms=graph_ms, objective_at_iteration_20=loss_first,
                 control_points_per_s=wl.n_cp / (pair * 1e-3), clocks=clk.summary(),
                 gpu_launches=(sum(fw_n.values()) + sum(bw_n.values()) + 7) * n_it * steps,
-                roofline=dict(bound="alu", kernel="k_conv_sym<K,false>" if wf.conv_symmetric else "k_conv<K,false,...>", achieved=achieved, peak=fp32_peak,
+                roofline=dict(bound="alu", kernel=("k_conv<K,false,...>", "k_conv_sym<K,false>", "k_conv_fold<K,false>")[wf.conv_symmetric], achieved=achieved, peak=fp32_peak,
                               unit="TFLOP/s", frac=achieved / fp32_peak, achieved_on_footprint_tiles=on_tiles, frac_on_footprint_tiles=on_tiles / fp32_peak,
                               executed=executed, executed_frac=executed / fp32_peak, traffic=recorded_traffic("c5", K),
                               note="algorithmic flops = 2*k^2*|support|; see the c4 line for the other two counts"),
@@ -484,22 +484,22 @@ def run_ours(args):
         stages["conv_adj"].update(tflops=round(conv_adj_flops / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None,
                                   issued_tflops=round(2.0 * wb.conv_macs / (stage_ms["conv_adj"] * 1e-3) / 1e12, 2) if stage_ms["conv_adj"] > 0 else None)
     # The dominant kernel is the forward convolution.  Algorithmic flops = 2 k^2 |S|: the multiply-adds of Eq. 8 on inputs that can
-    # be non-zero (SURVEY.md 8(d) "algorithmic MAC"; products with structurally zero fluence earn nothing).  The row-symmetric kernel
-    # executes about (k+1)/2k of them (each row correlation serves two output rows), the output-stationary one more (zeros in the
-    # halo): `executed` is what the kernel counted, and executed / peak is the FMA-pipe share of the launch.
+    # be non-zero (SURVEY.md 8(d) "algorithmic MAC"; products with structurally zero fluence earn nothing).  The symmetric kernels
+    # execute about (k+1)/2k of them (k_conv_sym: each row correlation serves two output rows) or ((k+1)/2k)^2 (k_conv_fold: folded
+    # columns as well), the output-stationary one more (zeros in the halo): `executed` is what the kernel counted, and executed / peak is the FMA-pipe share of the launch.
     t_conv = stage_ms["conv"] * 1e-3
     achieved = 2.0 * K * K * wf.support_voxels / t_conv / 1e12 if t_conv > 0 else None
     on_tiles = conv_flops / t_conv / 1e12 if t_conv > 0 else None
     executed = 2.0 * wf.conv_macs / t_conv / 1e12 if t_conv > 0 else None
-    kname = "k_conv_sym<K,false>" if wf.conv_symmetric else "k_conv<K,false,...>"
+    kname = ("k_conv<K,false,...>", "k_conv_sym<K,false>", "k_conv_fold<K,false>")[wf.conv_symmetric]
     roofline = dict(bound="alu", kernel=f"{kname} (S4+S5: depth-indexed kernel lookup + lateral convolution)",
                     achieved=achieved, peak=fp32_peak, unit="TFLOP/s", frac=(achieved / fp32_peak) if achieved else None,
                     achieved_on_footprint_tiles=on_tiles, frac_on_footprint_tiles=(on_tiles / fp32_peak) if on_tiles else None,
                     executed=executed, executed_frac=(executed / fp32_peak) if executed else None,
                     traffic=recorded_traffic(wl.name, K),
                     note=f"algorithmic flops = 2*k^2*|support| per launch (products with structurally zero fluence not counted); "
-                         f"*_on_footprint_tiles uses 2*k^2*|footprint| (SURVEY.md 8(d): the output-tiled count; a kernel that uses the kernel's "
-                         f"row symmetry executes about half of it, so this can exceed the peak); executed = 2 x the multiply-adds the kernel counted; "
+                         f"*_on_footprint_tiles uses 2*k^2*|footprint| (SURVEY.md 8(d): the output-tiled count; a kernel that uses the pencil kernel's "
+                         f"symmetry executes a half or a quarter of it, so this can exceed the peak); executed = 2 x the multiply-adds the kernel counted; "
                          f"peak = {eng.info.sm_count} SMs x 128 FP32 lanes x 2 x "
                          f"{peaks['sm_max_mhz']:.0f} MHz (plain FP32 FMA pipe; FFMA microbenchmark on this pool: 72.5 TFLOP/s); "
                          f"HBM fractions of the bandwidth-bound stages are under 'stages' against {peaks['hbm_gbs']} GB/s {peaks['source']}")

@@ -144,7 +144,8 @@ typedef struct {
     int32_t  kernel_size, kernel_size_compiled;
     int64_t  fan_rays;          /* PDRT_DEPTH_FAN: diverging rays traced (sum over control points), else 0  */
     int32_t  ray_samples;       /* samples per ray (upper bound: samples outside the grid are skipped)     */
-    int32_t  conv_symmetric;    /* 1: that call's convolution ran in row-symmetric form (k_conv_sym), 0: output-stationary (k_conv) */
+    int32_t  conv_symmetric;    /* that call's convolution kernel: 0 output-stationary (k_conv), 1 row-symmetric (k_conv_sym),
+                                   2 row- and column-symmetric (k_conv_fold)                                                   */
 } pdrt_work;
 
 /* pdrt_create: grid geometry, density volume [nz][ny][nx] (host OR device pointer; copied) and

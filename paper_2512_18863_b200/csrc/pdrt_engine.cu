@@ -763,7 +763,7 @@ int pdrt_get_work(pdrt_engine *e, pdrt_work *w)
     w->kernel_size = e->P.K; w->kernel_size_compiled = e->P.KT;
     w->fan_rays = e->depth_mode == PDRT_DEPTH_FAN ? wc.fan_rays : 0;
     w->ray_samples = e->P.M_ray;
-    w->conv_symmetric = (e->last_backward ? e->sym_adj : e->sym_fwd) ? 1 : 0;
+    w->conv_symmetric = (e->last_backward ? e->sym_adj : e->sym_fwd) ? (e->P.KT >= 15 && e->P.KT <= conv_fold_max() ? 2 : 1) : 0;
     return PDRT_OK;
 }
 

@@ -218,8 +218,11 @@ PDRT_API int pdrt_dose_backward(pdrt_engine *engine, int32_t n_cp,
                        void *cuda_stream);
 
 /* The same two calls with HOST buffers: host->device copies of the parameters (and dL/dDose),
- * the kernels, the device->host copy of the result, and a stream synchronise.  The two volumes move on copy streams of
- * the engine: dL/dDose is uploaded while the backward pass uploads its parameters and runs S1 / S2. */
+ * the kernels, the device->host copy of the result, and a stream synchronise.  The four parameter arrays are packed into a
+ * pinned block of the engine when the call is made (the caller's arrays may be reused at once) and travel as ONE copy; the
+ * three gradient arrays come back as one copy and are unpacked on the host before the call returns.  The two volumes move on
+ * copy streams of the engine: the backward call's parameters and dL/dDose are uploaded there, so they do not wait for
+ * work still queued on `cuda_stream` (e.g. the forward pass of the same step). */
 PDRT_API int pdrt_dose_host(pdrt_engine *engine, int32_t n_cp,
                    const float *leaves_host, const float *jaws_host,
                    const float *gantry_deg_host, const float *mu_host,

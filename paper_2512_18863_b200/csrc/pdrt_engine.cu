@@ -124,7 +124,14 @@ struct pdrt_engine {
     DevBuf<double> rho_s, Z_s;
     DevBuf<float> bufA, bufB;         // compact beam-frame blocks: conv output (D_b / H_b) and conv input (Phivol / G_b)
     // staging for the *_host entry points
-    DevBuf<float> s_leaves, s_jaws, s_gantry, s_mu, s_dose, s_g, s_dleaves, s_djaws, s_dmu;
+    DevBuf<float> s_dose, s_g;
+    // parameters and gradients of the host calls travel packed: one pinned host block, one copy per direction and call
+    // ([0]: forward call, [1]: backward call; leaves | jaws | gantry | mu, each padded to 4 floats)
+    DevBuf<float> s_par[2], s_grad;
+    float *h_par[2] = { nullptr, nullptr }, *h_grad = nullptr;
+    size_t h_par_n[2] = { 0, 0 }, h_grad_n = 0;
+    cudaEvent_t ev_par[2] = { nullptr, nullptr };     // the packed block has left the pinned host buffer
+    bool par_recorded[2] = { false, false };
     // the host variants move the two volumes on copy streams of their own, so that the dose can travel to the host while the
     // next call computes and dL/dDose can travel to the device while the backward pass sets up (PCIe is full duplex)
     cudaStream_t cs_in = nullptr, cs_out = nullptr;
@@ -695,11 +702,13 @@ void pdrt_destroy(pdrt_engine *e)
     e->counters.release(); e->phimap.release(); e->P0.release(); e->T1.release(); e->T2.release(); e->T3.release();
     e->Abuf.release(); e->gphimap.release(); e->zrad.release(); e->rho_s.release(); e->Z_s.release();
     e->bufA.release(); e->bufB.release(); e->phimapT.release(); e->gT.release();
-    e->s_leaves.release(); e->s_jaws.release(); e->s_gantry.release(); e->s_mu.release(); e->s_dose.release(); e->s_g.release();
+    e->s_dose.release(); e->s_g.release(); e->s_grad.release();
+    for (int q = 0; q < 2; ++q) { e->s_par[q].release(); if (e->h_par[q]) cudaFreeHost(e->h_par[q]); if (e->ev_par[q]) cudaEventDestroy(e->ev_par[q]); }
+    if (e->h_grad) cudaFreeHost(e->h_grad);
     if (e->cs_in) cudaStreamDestroy(e->cs_in);
     if (e->cs_out) cudaStreamDestroy(e->cs_out);
     for (cudaEvent_t ev : { e->ev_fwd, e->ev_out, e->ev_g, e->ev_bwd }) if (ev) cudaEventDestroy(ev);
-    e->s_dleaves.release(); e->s_djaws.release(); e->s_dmu.release(); e->obj_partial.release();
+    e->obj_partial.release();
     for (cudaEvent_t ev : e->ev_pool) cudaEventDestroy(ev);
     delete e;
 }
@@ -804,15 +813,48 @@ int pdrt_dose_backward(pdrt_engine *e, int32_t n_cp, const float *leaves, const 
     return backward_impl(e, n_cp, leaves, jaws, gantry, mu, gdose, d_leaves, d_jaws, d_mu, (cudaStream_t)stream);
 }
 
-static int stage_params_in(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry,
-                           const float *mu, cudaStream_t st)
+// Offsets [floats] of the packed parameter / gradient blocks: leaves | jaws | gantry (parameters only) | mu, each padded to 4 floats.
+struct PackOff { size_t leaves, jaws, gantry, mu, total; };
+static PackOff pack_offsets(const pdrt_engine *e, int n_cp, bool with_gantry)
 {
-    CU(e, e->s_leaves.ensure((size_t)n_cp * 2 * e->P.Np)); CU(e, e->s_jaws.ensure((size_t)n_cp * 4));
-    CU(e, e->s_gantry.ensure(n_cp)); CU(e, e->s_mu.ensure(n_cp));
-    CU(e, cudaMemcpyAsync(e->s_leaves.p, leaves, sizeof(float) * n_cp * 2 * e->P.Np, cudaMemcpyHostToDevice, st));
-    CU(e, cudaMemcpyAsync(e->s_jaws.p, jaws, sizeof(float) * n_cp * 4, cudaMemcpyHostToDevice, st));
-    CU(e, cudaMemcpyAsync(e->s_gantry.p, gantry, sizeof(float) * n_cp, cudaMemcpyHostToDevice, st));
-    CU(e, cudaMemcpyAsync(e->s_mu.p, mu, sizeof(float) * n_cp, cudaMemcpyHostToDevice, st));
+    auto pad4 = [](size_t n) { return (n + 3) & ~(size_t)3; };
+    PackOff o;
+    o.leaves = 0;
+    o.jaws = pad4((size_t)n_cp * 2 * e->P.Np);
+    o.gantry = o.jaws + pad4((size_t)n_cp * 4);
+    o.mu = with_gantry ? o.gantry + pad4(n_cp) : o.gantry;
+    o.total = o.mu + pad4(n_cp);
+    return o;
+}
+static int ensure_pinned(pdrt_engine *e, float **p, size_t *have, size_t want)
+{
+    if (want <= *have) return PDRT_OK;
+    if (*p) cudaFreeHost(*p);
+    *p = nullptr; *have = 0;
+    CU(e, cudaHostAlloc((void **)p, want * sizeof(float), cudaHostAllocDefault));
+    *have = want;
+    return PDRT_OK;
+}
+// Packs the four host arrays into the pinned block `which` and sends it with ONE copy on `cs`; the device pointers come back in `dev`.
+static int stage_params_in(pdrt_engine *e, int which, int n_cp, const float *leaves, const float *jaws, const float *gantry,
+                           const float *mu, cudaStream_t cs, const float *(&dev)[4])
+{
+    const PackOff o = pack_offsets(e, n_cp, true);
+    int rc = ensure_pinned(e, &e->h_par[which], &e->h_par_n[which], o.total);
+    if (rc) return rc;
+    CU(e, e->s_par[which].ensure(o.total));
+    if (!e->ev_par[which]) CU(e, cudaEventCreateWithFlags(&e->ev_par[which], cudaEventDisableTiming));
+    if (e->par_recorded[which]) CU(e, cudaEventSynchronize(e->ev_par[which]));       // the previous call's copy has read the pinned block
+    float *h = e->h_par[which];
+    std::memcpy(h + o.leaves, leaves, sizeof(float) * n_cp * 2 * e->P.Np);
+    std::memcpy(h + o.jaws, jaws, sizeof(float) * n_cp * 4);
+    std::memcpy(h + o.gantry, gantry, sizeof(float) * n_cp);
+    std::memcpy(h + o.mu, mu, sizeof(float) * n_cp);
+    CU(e, cudaMemcpyAsync(e->s_par[which].p, h, o.total * sizeof(float), cudaMemcpyHostToDevice, cs));
+    CU(e, cudaEventRecord(e->ev_par[which], cs));
+    e->par_recorded[which] = true;
+    const float *d = e->s_par[which].p;
+    dev[0] = d + o.leaves; dev[1] = d + o.jaws; dev[2] = d + o.gantry; dev[3] = d + o.mu;
     return PDRT_OK;
 }
 
@@ -833,10 +875,11 @@ int pdrt_dose_host_async(pdrt_engine *e, int32_t n_cp, const float *leaves, cons
     if ((rc = host_streams(e))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t nvox = (size_t)e->P.nx * e->P.ny * e->P.nz;
-    if ((rc = stage_params_in(e, n_cp, leaves, jaws, gantry, mu, st))) return rc;
+    const float *par[4];
+    if ((rc = stage_params_in(e, 0, n_cp, leaves, jaws, gantry, mu, st, par))) return rc;
     CU(e, e->s_dose.ensure(nvox));
     if (e->out_pending) CU(e, cudaStreamWaitEvent(st, e->ev_out, 0));        // the previous dose has left the staging buffer
-    if ((rc = forward_impl(e, n_cp, e->s_leaves.p, e->s_jaws.p, e->s_gantry.p, e->s_mu.p, e->s_dose.p, st))) return rc;
+    if ((rc = forward_impl(e, n_cp, par[0], par[1], par[2], par[3], e->s_dose.p, st))) return rc;
     CU(e, cudaEventRecord(e->ev_fwd, st));
     CU(e, cudaStreamWaitEvent(e->cs_out, e->ev_fwd, 0));
     CU(e, cudaMemcpyAsync(dose, e->s_dose.p, nvox * sizeof(float), cudaMemcpyDeviceToHost, e->cs_out));
@@ -868,20 +911,26 @@ int pdrt_dose_backward_host(pdrt_engine *e, int32_t n_cp, const float *leaves, c
     if ((rc = host_streams(e))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t nvox = (size_t)e->P.nx * e->P.ny * e->P.nz, nl = (size_t)n_cp * 2 * e->P.Np;
-    CU(e, e->s_g.ensure(nvox)); CU(e, e->s_dleaves.ensure(nl)); CU(e, e->s_djaws.ensure((size_t)n_cp * 4)); CU(e, e->s_dmu.ensure(n_cp));
-    // dL/dDose travels on the input copy stream while this stream uploads the parameters and runs S1 / S2
+    const PackOff go = pack_offsets(e, n_cp, false);
+    CU(e, e->s_g.ensure(nvox)); CU(e, e->s_grad.ensure(go.total));
+    if ((rc = ensure_pinned(e, &e->h_grad, &e->h_grad_n, go.total))) return rc;
+    // The parameters and dL/dDose travel on the input copy stream (they need not wait for whatever still runs on this stream, e.g. the
+    // forward pass of the same step); S1 / S2 wait for the parameters, the transposition of dL/dDose for the volume.
+    const float *par[4];
+    if ((rc = stage_params_in(e, 1, n_cp, leaves, jaws, gantry, mu, e->cs_in, par))) return rc;
+    CU(e, cudaStreamWaitEvent(st, e->ev_par[1], 0));
     if (e->bwd_recorded) CU(e, cudaStreamWaitEvent(e->cs_in, e->ev_bwd, 0));  // the previous backward pass has read the staging buffer
     CU(e, cudaMemcpyAsync(e->s_g.p, gdose, nvox * sizeof(float), cudaMemcpyHostToDevice, e->cs_in));
     CU(e, cudaEventRecord(e->ev_g, e->cs_in));
-    if ((rc = stage_params_in(e, n_cp, leaves, jaws, gantry, mu, st))) return rc;
-    if ((rc = backward_impl(e, n_cp, e->s_leaves.p, e->s_jaws.p, e->s_gantry.p, e->s_mu.p, e->s_g.p, e->s_dleaves.p,
-                            e->s_djaws.p, e->s_dmu.p, st, e->ev_g))) return rc;
+    float *dg = e->s_grad.p;
+    if ((rc = backward_impl(e, n_cp, par[0], par[1], par[2], par[3], e->s_g.p, dg + go.leaves, dg + go.jaws, dg + go.mu, st, e->ev_g))) return rc;
     CU(e, cudaEventRecord(e->ev_bwd, st));
     e->bwd_recorded = true;
-    CU(e, cudaMemcpyAsync(d_leaves, e->s_dleaves.p, nl * sizeof(float), cudaMemcpyDeviceToHost, st));
-    CU(e, cudaMemcpyAsync(d_jaws, e->s_djaws.p, sizeof(float) * n_cp * 4, cudaMemcpyDeviceToHost, st));
-    CU(e, cudaMemcpyAsync(d_mu, e->s_dmu.p, sizeof(float) * n_cp, cudaMemcpyDeviceToHost, st));
+    CU(e, cudaMemcpyAsync(e->h_grad, dg, go.total * sizeof(float), cudaMemcpyDeviceToHost, st));      // one copy; unpacked on the host
     CU(e, cudaStreamSynchronize(st));
+    std::memcpy(d_leaves, e->h_grad + go.leaves, nl * sizeof(float));
+    std::memcpy(d_jaws, e->h_grad + go.jaws, sizeof(float) * n_cp * 4);
+    std::memcpy(d_mu, e->h_grad + go.mu, sizeof(float) * n_cp);
     return PDRT_OK;
 }
 

@@ -18,7 +18,7 @@ constexpr int GD_CPB = 16;                       // control points set up per ro
 constexpr int GD_THREADS = GD_COLS * GD_CPB;
 constexpr int GD_ZSPAN = 64;                     // z covered by one pass of a half-warp (16 lanes x float4)
 constexpr int GD_MAXPASS = 4;                    // passes held in registers at once (256 z)
-constexpr int GD_LIST = 256;                     // control points listed per outer chunk
+constexpr int GD_LIST = GD_THREADS;              // control points listed per outer chunk: one thread each
 
 struct __align__(16) GatherCp {                  // what the stencil set-up needs of a listed control point (32 bytes, shared memory)
     float cg, sg, scale;
@@ -92,7 +92,7 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
 {
     __shared__ GatherRec rec[2][GD_CPB][GD_COLS];
     __shared__ GatherCp list[GD_LIST];
-    __shared__ int n_list_s, zmin_s, zmax_s;
+    __shared__ int n_list_s, zmin_s, zmax_s, wcount_s[GD_THREADS / 32], wzlo_s[GD_THREADS / 32], wzhi_s[GD_THREADS / 32];
     const int tid = threadIdx.x, lane16 = tid & 15;
     const int col = tid >> 4;                                    // phase B: column of this half-warp
     const int a_col = tid & 15, a_cp = tid >> 4;                 // phase A: (column, control point of the round)
@@ -158,36 +158,42 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
 
     for (int c0 = 0; c0 < n_cp; c0 += GD_LIST) {
         __syncthreads();
-        if (tid < 32) {                 // warp 0 builds the ordered list of candidate control points and their z-range
-            int count = 0, zmin = P.nz, zmax = 0;
-            const int cend = min(n_cp, c0 + GD_LIST);
-            for (int cb = c0; cb < cend; cb += 32) {
-                const int c = cb + tid;
-                bool keep = false;
-                GatherCp g;
-                if (c < cend) {
-                    const CpDesc &d = desc[cp0 + c];
-                    if (d.a0 <= d.a1) {
-                        g.cg = d.cg; g.sg = d.sg; g.scale = d.scale; g.ri0 = d.ri0; g.pu = d.pu; g.pv = d.pv; g.rj0 = d.rj0; g.slot = c;
-                        // u-extent of the tile: extremes are at its corners
-                        const float u00 = g.cg * cx0 + g.sg * cy0, u10 = g.cg * cx1 + g.sg * cy0;
-                        const float u01 = g.cg * cx0 + g.sg * cy1, u11 = g.cg * cx1 + g.sg * cy1;
-                        const float umin = fminf(fminf(u00, u10), fminf(u01, u11)) / P.du + P.cu;
-                        const float umax = fmaxf(fmaxf(u00, u10), fmaxf(u01, u11)) / P.du + P.cu;
-                        keep = umax >= (float)(g.ri0 - 1) && umin <= (float)(g.ri0 + g.pu);
-                        if (keep) { zmin = min(zmin, g.rj0); zmax = max(zmax, min(P.nz, g.rj0 + g.pv)); }
-                    }
+        {   // the ordered list of candidate control points and their z-range: one thread per control point of the chunk (GD_LIST = the
+            // block size), kept entries compacted in control-point order by a ballot per warp and a prefix over the warps
+            const int c = c0 + tid;
+            bool keep = false;
+            GatherCp g;
+            int zlo = P.nz, zhi = 0;
+            if (c < n_cp) {
+                const CpDesc &d = desc[cp0 + c];
+                if (d.a0 <= d.a1) {
+                    g.cg = d.cg; g.sg = d.sg; g.scale = d.scale; g.ri0 = d.ri0; g.pu = d.pu; g.pv = d.pv; g.rj0 = d.rj0; g.slot = c;
+                    // u-extent of the tile: extremes are at its corners
+                    const float u00 = g.cg * cx0 + g.sg * cy0, u10 = g.cg * cx1 + g.sg * cy0;
+                    const float u01 = g.cg * cx0 + g.sg * cy1, u11 = g.cg * cx1 + g.sg * cy1;
+                    const float umin = fminf(fminf(u00, u10), fminf(u01, u11)) / P.du + P.cu;
+                    const float umax = fmaxf(fmaxf(u00, u10), fmaxf(u01, u11)) / P.du + P.cu;
+                    keep = umax >= (float)(g.ri0 - 1) && umin <= (float)(g.ri0 + g.pu);
+                    if (keep) { zlo = g.rj0; zhi = min(P.nz, g.rj0 + g.pv); }
                 }
-                const unsigned m = __ballot_sync(0xffffffffu, keep);
-                if (keep) list[count + __popc(m & ((1u << tid) - 1u))] = g;
-                count += __popc(m);
             }
+            const int lane = tid & 31, warp = tid >> 5;
+            const unsigned m = __ballot_sync(0xffffffffu, keep);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
-                zmin = min(zmin, __shfl_xor_sync(0xffffffffu, zmin, o));
-                zmax = max(zmax, __shfl_xor_sync(0xffffffffu, zmax, o));
+                zlo = min(zlo, __shfl_xor_sync(0xffffffffu, zlo, o));
+                zhi = max(zhi, __shfl_xor_sync(0xffffffffu, zhi, o));
             }
-            if (tid == 0) { n_list_s = count; zmin_s = zmin & ~7; zmax_s = zmax; }
+            if (lane == 0) { wcount_s[warp] = __popc(m); wzlo_s[warp] = zlo; wzhi_s[warp] = zhi; }
+            __syncthreads();
+            int base = 0, total = 0, zmin = P.nz, zmax = 0;
+#pragma unroll
+            for (int w = 0; w < GD_THREADS / 32; ++w) {
+                if (w < warp) base += wcount_s[w];
+                total += wcount_s[w]; zmin = min(zmin, wzlo_s[w]); zmax = max(zmax, wzhi_s[w]);
+            }
+            if (keep) list[base + __popc(m & ((1u << lane) - 1u))] = g;
+            if (tid == 0) { n_list_s = total; zmin_s = zmin & ~7; zmax_s = zmax; }
         }
         __syncthreads();
         const int n_list = n_list_s, zmin = zmin_s, zmax = zmax_s;

@@ -416,12 +416,29 @@ def test_results_are_bit_reproducible(torch):
     wl = W.tiny(seed=33, n_cp=6, nx=40, ny=36, nz=20, kernel_size=9, flu=(28, 24))
     eng, _ = pair(wl)
     g = W.seeded_dose_gradient(wl, seed=33)
+    for k in (9, 21, 5):            # row-symmetric, folded (shared-memory ring of output rows) and output-stationary convolution
+        eng.set_kernel_size(k)
+        d1 = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu).clone()
+        b1 = [t.clone() for t in eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)]
+        for _ in range(3):
+            d2 = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
+            b2 = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+            assert torch.equal(d1, d2), f"k={k}"
+            assert all(torch.equal(a, b) for a, b in zip(b1, b2)), f"k={k}"
+
+
+def test_config2_is_bit_reproducible(torch):
+    """The same on c2 (k = 21: k_conv_fold, many work items in flight on every SM)."""
+    wl = W.config2()
+    eng, _ = pair(wl)
+    g = W.seeded_dose_gradient(wl, seed=2)
     d1 = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu).clone()
     b1 = [t.clone() for t in eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)]
-    d2 = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
-    b2 = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
-    assert torch.equal(d1, d2)
-    assert all(torch.equal(a, b) for a, b in zip(b1, b2))
+    for _ in range(3):
+        d2 = eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
+        b2 = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+        assert torch.equal(d1, d2)
+        assert all(torch.equal(a, b) for a, b in zip(b1, b2))
 
 
 def test_sharded_driver_around_the_cuda_engine_world_size_1(torch):

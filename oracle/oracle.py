@@ -335,6 +335,24 @@ class Oracle:
                                         C.c_int(n_cp), _p(lv), _p(jw), _p(ga), _p(co), _p(mu), g.ctypes.data_as(C.c_void_p), _p(dl), _p(dj), _p(dm))
         return dl, dj, dm
 
+    def dose_fan_coll(self, leaves, jaws, gantry_deg, coll_deg, mu):
+        """Divergent-depth mode and collimator rotation together (composition of the pinned steps, in the paper's order)."""
+        n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)
+        co = _d(coll_deg)
+        out = np.zeros(self.dose_shape)
+        self.lib.orc_dose_fan_coll(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), _p(self._w_tab()), C.c_int(n_cp),
+                                   _p(lv), _p(jw), _p(ga), _p(co), _p(mu), _p(out))
+        return out
+
+    def dose_backward_fan_coll(self, leaves, jaws, gantry_deg, coll_deg, mu, gdose):
+        n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)
+        co = _d(coll_deg)
+        g = np.ascontiguousarray(gdose, dtype=np.float32)
+        dl, dj, dm = np.zeros_like(lv), np.zeros_like(jw), np.zeros_like(mu)
+        self.lib.orc_dose_backward_fan_coll(C.byref(self.G), C.byref(self.M), self.density.ctypes.data_as(C.c_void_p), _p(self._w_tab()),
+                                            C.c_int(n_cp), _p(lv), _p(jw), _p(ga), _p(co), _p(mu), g.ctypes.data_as(C.c_void_p), _p(dl), _p(dj), _p(dm))
+        return dl, dj, dm
+
     def dose_at(self, leaves, jaws, gantry_deg, mu, ijk):
         """Dose at selected voxels; ijk is [n][3] = (x index, y index, z index)."""
         n_cp, lv, jw, ga, mu = self._cp_args(leaves, jaws, gantry_deg, mu)

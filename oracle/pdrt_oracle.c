@@ -997,3 +997,60 @@ void orc_dose_backward_coll(const orc_grid *g, const orc_model *m, const float *
     }
     free(G); free(H); free(z); free(Phimap); free(Phirot); free(gPhirot); free(gPhimap);
 }
+
+/* ================================================================== divergent depth AND collimator rotation together */
+/* The two optional steps compose in the paper's order ("rotated ... prior to ray-based projection"; reading G24: the
+ * depth factor lives at the ray nodes of the beam frame and weights the PROJECTED fluence): fluence -> rotation (G25) -> projection
+ * (Eq. 5-6) -> depth factor (G24) -> convolution -> resampling.  No new arithmetic: every step is one of the functions above. */
+void orc_dose_fan_coll(const orc_grid *g, const orc_model *m, const float *rho, const double *W_tab, int n_cp,
+                       const double *leaves, const double *jaws, const double *gantry_deg, const double *coll_deg, const double *mu, double *dose)
+{
+    const size_t nb = (size_t)m->beam_nu * g->nz * m->beam_nw, np = (size_t)g->nx * g->ny * g->nz, nf = (size_t)m->flu_nu * m->flu_nv;
+    double *Db = malloc(sizeof(double) * nb), *Phivol = malloc(sizeof(double) * nb);
+    double *Phimap = malloc(sizeof(double) * nf), *Phirot = malloc(sizeof(double) * nf), *z = malloc(sizeof(double) * m->beam_nw);
+    double *zf = malloc(sizeof(double) * nf * m->beam_nw), *F = malloc(sizeof(double) * nf * m->beam_nw);
+    memset(dose, 0, sizeof(double) * np);
+    for (int b = 0; b < n_cp; ++b) {
+        orc_fluence(m, leaves + (size_t)b * 2 * m->n_pairs, jaws + (size_t)b * 4, NULL, NULL, NULL, Phimap);
+        orc_rotate_map(m, coll_deg[b], Phimap, Phirot);
+        orc_radiological_depth(g, rho, m, gantry_deg[b], z);
+        orc_fan_depth(g, rho, m, gantry_deg[b], zf);
+        orc_fan_factor(g, m, zf, z, F);
+        orc_project(g, m, Phirot, Phivol);
+        orc_apply_fan_factor(g, m, F, Phivol);
+        orc_convolve(g, m, W_tab, z, Phivol, Db);
+        orc_resample_add(g, m, gantry_deg[b], m->cal * mu[b], Db, dose);
+    }
+    free(Db); free(Phivol); free(Phimap); free(Phirot); free(z); free(zf); free(F);
+}
+void orc_dose_backward_fan_coll(const orc_grid *g, const orc_model *m, const float *rho, const double *W_tab, int n_cp,
+                                const double *leaves, const double *jaws, const double *gantry_deg, const double *coll_deg, const double *mu,
+                                const float *gdose, double *d_leaves, double *d_jaws, double *d_mu)
+{
+    const size_t nb = (size_t)m->beam_nu * g->nz * m->beam_nw, nf = (size_t)m->flu_nu * m->flu_nv;
+    const int np = m->n_pairs;
+    double *G = malloc(sizeof(double) * nb), *H = malloc(sizeof(double) * nb), *z = malloc(sizeof(double) * m->beam_nw);
+    double *Phimap = malloc(sizeof(double) * nf), *Phirot = malloc(sizeof(double) * nf);
+    double *gPhirot = malloc(sizeof(double) * nf), *gPhimap = malloc(sizeof(double) * nf);
+    double *zf = malloc(sizeof(double) * nf * m->beam_nw), *F = malloc(sizeof(double) * nf * m->beam_nw);
+    for (int b = 0; b < n_cp; ++b) {
+        const double *lv = leaves + (size_t)b * 2 * np, *jw = jaws + (size_t)b * 4;
+        orc_fluence(m, lv, jw, NULL, NULL, NULL, Phimap);
+        orc_rotate_map(m, coll_deg[b], Phimap, Phirot);
+        orc_radiological_depth(g, rho, m, gantry_deg[b], z);
+        orc_fan_depth(g, rho, m, gantry_deg[b], zf);
+        orc_fan_factor(g, m, zf, z, F);
+        orc_resample_adjoint(g, m, gantry_deg[b], gdose, G);
+        orc_convolve_adjoint(g, m, W_tab, z, G, H);
+        orc_apply_fan_factor(g, m, F, H);
+        orc_project_adjoint(g, m, H, gPhirot);
+        double dot = 0.0;
+        for (size_t e = 0; e < nf; ++e) dot += Phirot[e] * gPhirot[e];
+        d_mu[b] = m->cal * dot;
+        orc_rotate_map_adjoint(m, coll_deg[b], gPhirot, gPhimap);
+        orc_fluence_adjoint(m, lv, jw, gPhimap, d_leaves + (size_t)b * 2 * np, d_jaws + (size_t)b * 4);
+        for (int e = 0; e < 2 * np; ++e) d_leaves[(size_t)b * 2 * np + e] *= m->cal * mu[b];
+        for (int e = 0; e < 4; ++e) d_jaws[(size_t)b * 4 + e] *= m->cal * mu[b];
+    }
+    free(G); free(H); free(z); free(Phimap); free(Phirot); free(gPhirot); free(gPhimap); free(zf); free(F);
+}

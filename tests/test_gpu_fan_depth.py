@@ -76,3 +76,18 @@ def test_fan_mode_on_the_pelvis_phantom_sampled(torch):
     ref = orc.dose_fan(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)
     assert_dose(d, ref, "pelvis fan dose")
     assert np.abs(ref - orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)).max() > 1e-3 * ref.max()
+
+
+def test_fan_mode_with_collimator_rotation(torch):
+    """Both optional steps at once (pdrt_set_collimator on a PDRT_DEPTH_FAN engine) against the oracle's composition."""
+    wl = W.tiny(seed=73, nx=40, ny=36, nz=16, kernel_size=7, n_cp=3, flu=(26, 22))
+    eng, orc = pair(wl)
+    coll = np.asarray([25.0, -70.0, 130.0], np.float32)
+    eng.set_collimator(coll)
+    d_ref = orc.dose_fan_coll(wl.leaves, wl.jaws, wl.gantry_deg, coll, wl.mu)
+    assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), d_ref, "fan + collimator dose")
+    assert np.abs(d_ref - orc.dose_fan(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu)).max() > 1e-3 * d_ref.max()
+    g = W.seeded_dose_gradient(wl, seed=73)
+    dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)
+    rl, rj, rm = orc.dose_backward_fan_coll(wl.leaves, wl.jaws, wl.gantry_deg, coll, wl.mu, g)
+    assert_grad(dm, rm, "fan + collimator d_mu"); assert_grad(dj, rj, "fan + collimator d_jaws"); assert_grad(dl, rl, "fan + collimator d_leaves")

@@ -147,3 +147,40 @@ def test_gradients_of_the_fan_mode_vs_finite_differences():
     assert dm[1] == pytest.approx((L(lv, jw, p) - L(lv, jw, q)) / (2 * h), rel=1e-8)
     # and the mode differs from the paper's on this laterally inhomogeneous phantom
     assert np.abs(orc.dose_fan(lv, jw, wl.gantry_deg, mu) - orc.dose(lv, jw, wl.gantry_deg, mu)).max() > 1e-3 * orc.dose(lv, jw, wl.gantry_deg, mu).max()
+
+
+def test_fan_mode_with_collimator_rotation_reduces_to_each_mode_and_matches_finite_differences():
+    """orc_dose_fan_coll composes the two optional steps (rotation, then projection, then the depth factor).  Pins: collimator 0
+    gives the fan-mode dose bit for bit; in slabs normal to the axis (factor 1 on the rays that stay inside) it gives the
+    collimator-mode dose; it differs from both where both steps act; its gradients match central differences of its own dose."""
+    wl = W.tiny(seed=68, n_cp=2, nx=22, ny=20, nz=10, kernel_size=5, flu=(16, 12), head_scatter=False)
+    orc = Oracle(wl.grid, wl.model, wl.density)
+    lv, jw, mu = wl.leaves.astype(np.float64), wl.jaws.astype(np.float64), wl.mu.astype(np.float64)
+    zero, coll = np.zeros(2), np.asarray([27.0, -64.0])
+    assert np.array_equal(orc.dose_fan_coll(lv, jw, wl.gantry_deg, zero, mu), orc.dose_fan(lv, jw, wl.gantry_deg, mu))
+    d_fc = orc.dose_fan_coll(lv, jw, wl.gantry_deg, coll, mu)
+    d_f, d_c = orc.dose_fan(lv, jw, wl.gantry_deg, mu), orc.dose_coll(lv, jw, wl.gantry_deg, coll, mu)
+    assert np.abs(d_fc - d_f).max() > 1e-3 * d_f.max() and np.abs(d_fc - d_c).max() > 1e-3 * d_c.max()
+    # slabs normal to the axis, field well inside the rays that stay in the grid: the factor is 1, only the rotation acts
+    ws = slab_case()
+    os_ = Oracle(ws.grid, ws.model, ws.density)
+    jaws = np.tile([-9.0, 9.0, -7.0, 7.0], (2, 1))
+    c2 = np.asarray([15.0, -40.0])
+    a, b = os_.dose_fan_coll(ws.leaves, jaws, ws.gantry_deg, c2, ws.mu), os_.dose_coll(ws.leaves, jaws, ws.gantry_deg, c2, ws.mu)
+    assert b.max() > 0 and np.abs(a - b).max() <= 1e-9 * b.max()
+    # gradients vs central differences
+    rng = np.random.Generator(np.random.PCG64(68))
+    g = rng.standard_normal(orc.dose_shape).astype(np.float32)
+    dl, dj, dm = orc.dose_backward_fan_coll(lv, jw, wl.gantry_deg, coll, mu, g)
+    L = lambda l, j, m: float((orc.dose_fan_coll(l, j, wl.gantry_deg, coll, m) * g).sum())
+    h = 1e-4
+    for (bb, bank, i) in ((0, 0, 2), (1, 1, 3)):
+        p, q = lv.copy(), lv.copy()
+        p[bb, bank, i] += h; q[bb, bank, i] -= h
+        assert dl[bb, bank, i] == pytest.approx((L(p, jw, mu) - L(q, jw, mu)) / (2 * h), rel=1e-6, abs=1e-10)
+    p, q = jw.copy(), jw.copy()
+    p[1, 2] += h; q[1, 2] -= h
+    assert dj[1, 2] == pytest.approx((L(lv, p, mu) - L(lv, q, mu)) / (2 * h), rel=1e-6, abs=1e-10)
+    p, q = mu.copy(), mu.copy()
+    p[0] += h; q[0] -= h
+    assert dm[0] == pytest.approx((L(lv, jw, p) - L(lv, jw, q)) / (2 * h), rel=1e-8)

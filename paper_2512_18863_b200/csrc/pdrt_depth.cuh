@@ -87,16 +87,18 @@ k_depth(Params P, int n_cp, const float *__restrict__ rho, const float *__restri
         r[m] = v;
         run += v * ds;
     }
-    // exclusive scan of the per-thread sums
-    __shared__ double part[DEPTH_THREADS];
-    part[tid] = run;
-    __syncthreads();
-    if (tid == 0) {
-        double s = 0.0;
-        for (int q = 0; q < DEPTH_THREADS; ++q) { const double v = part[q]; part[q] = s; s += v; }
+    // exclusive scan of the per-thread sums: shuffle scan inside each warp, then the warp totals in warp order (fixed order of additions)
+    __shared__ double wtot[DEPTH_THREADS / 32];
+    double incl = run;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double up = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((tid & 31) >= o) incl += up;
     }
+    if ((tid & 31) == 31) wtot[tid >> 5] = incl;
     __syncthreads();
-    double z = part[tid];
+    double z = incl - run;
+    for (int w = 0; w < (tid >> 5); ++w) z += wtot[w];
     for (int m = m_lo; m < m_hi; ++m) { Z[m] = z; z += r[m] * ds; }
     if (m_hi == M && m_lo < M) Z[M] = z;
     if (M == 0 && tid == 0) Z[0] = 0.0;

@@ -128,7 +128,7 @@ typedef struct {
     int32_t ray_samples;                 /* samples per central-axis ray                      */
     int32_t sm_count;
     uint64_t scratch_bytes;              /* device scratch currently held                     */
-    int32_t kernel_passes;               /* conv passes per slice: 1, or NB^2 sub-kernels for kernel sizes above 63 */
+    int32_t kernel_passes;               /* conv passes per slice: 1, or NB^2 sub-kernels for kernel sizes above 75 */
 } pdrt_info;
 
 /* Work counters of the most recent pdrt_dose / pdrt_dose_backward (device-counted from the actual

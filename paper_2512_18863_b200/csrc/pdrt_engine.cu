@@ -28,16 +28,8 @@ namespace {
 std::string g_create_error;
 
 // compiled conv variants; a requested size k runs on the smallest KT >= k with the table embedded in zeros
-const int kCompiled[] = { 5, 11, 15, 21, 25, 31, 41, 51, 55, 63 };
+const int kCompiled[] = { 5, 11, 15, 21, 25, 31, 41, 51, 55, 63, 75 };     // 75: k_conv_fold only
 const int kMaxKernel = 255;            // NB = 9 passes per axis of KT = 31 at most
-// Kernels up to `single_max` run as one pass on the smallest compiled variant; larger ones are split into NB x NB sub-kernels of
-// at most 31 taps (NB odd, so that the window stays centred): fewer multiply-adds with structural zeros than one wide pass
-// (halo overhead ((s + KT - 1)/s)^2 per pass instead of ((s + K - 1)/s)^2), and no limit on K from registers or shared memory.
-int conv_single_max()
-{
-    if (const char *v = std::getenv("PDRT_CONV_SINGLE_MAX")) { const int m = std::atoi(v); if (m >= 3 && m <= 63) return m; }
-    return 63;       // measured on c4: one pass (k_conv_fold) wins up to the widest compiled variant, 63 taps
-}
 // The single-pass convolution runs in row-symmetric form (k_conv_sym) unless PDRT_CONV_LEGACY=1 asks for the output-stationary
 // kernel (k_conv), which also serves the sub-kernel passes of a split (their off-centre blocks are not symmetric by themselves).
 bool conv_legacy()
@@ -45,19 +37,28 @@ bool conv_legacy()
     const char *v = std::getenv("PDRT_CONV_LEGACY");
     return v && std::atoi(v) != 0;
 }
+// Kernels up to `single_max` run as one pass on the smallest compiled variant; larger ones are split into NB x NB sub-kernels of
+// at most 31 taps (NB odd, so that the window stays centred): fewer multiply-adds with structural zeros than one wide pass
+// (halo overhead ((s + KT - 1)/s)^2 per pass instead of ((s + K - 1)/s)^2), and no limit on K from registers or shared memory.
+int conv_single_max()
+{
+    const int widest = conv_legacy() ? 63 : 75;      // the 75-tap variant exists as k_conv_fold only
+    if (const char *v = std::getenv("PDRT_CONV_SINGLE_MAX")) { const int m = std::atoi(v); if (m >= 3 && m <= widest) return m; }
+    return widest;   // measured on c4: one pass (k_conv_fold) wins up to the widest compiled variant
+}
 // Largest compiled size for which the ADJOINT also runs in symmetric form.  The forward shares every row correlation between two output
 // rows; the adjoint only where both rows r-d and r+d lie in S_k, so it gains less on supports shorter than the kernel.  With the column
 // symmetry folded in as well (k_conv_fold) it wins at every single-pass size measured; the knob stays for experiments.
 int conv_sym_adj_max()
 {
     if (const char *v = std::getenv("PDRT_CONV_SYM_ADJ_MAX")) return std::atoi(v);
-    return 63;
+    return 75;
 }
 // Largest compiled size that also folds the column symmetry (k_conv_fold; units of 4 columns up to 31 taps, of 2 above).
 int conv_fold_max()
 {
     if (const char *v = std::getenv("PDRT_CONV_FOLD_MAX")) return std::atoi(v);
-    return 63;
+    return 75;
 }
 int conv_sym_fwd_min()
 {
@@ -145,7 +146,7 @@ struct pdrt_engine {
     int conv_grid = 0;
     bool sym_fwd = false, sym_adj = false;   // which directions run k_conv_sym / k_conv_fold (single pass, from 11 taps)
     int conv_sym_per_sm[2][64] = {};
-    int conv_fold_per_sm[2][64] = {};     // the same for k_conv_sym, by [adjoint][KT]
+    int conv_fold_per_sm[2][80] = {};     // the same for k_conv_sym, by [adjoint][KT]
     int conv_per_sm[2][2][2][64] = {};   // resident conv blocks per SM on THIS engine's device, by [adjoint][copy width - 1][multi-pass][KT]; 0 = not queried yet
     DevBuf<float> coll;               // collimator angles [coll_n] set by pdrt_set_collimator (coll_n = 0: none)
     int coll_n = 0;
@@ -387,6 +388,7 @@ template <bool ADJ> int launch_conv(pdrt_engine *e, int cp0, int n, const float 
     case 51: return launch_conv_t<51, ADJ>(e, cp0, n, in, out, st);
     case 55: return launch_conv_t<55, ADJ>(e, cp0, n, in, out, st);
     case 63: return launch_conv_t<63, ADJ>(e, cp0, n, in, out, st);
+    case 75: if (e->P.conv_sym == 2) return launch_conv_fold<75, ADJ>(e, cp0, n, in, out, st); break;
     }
     return fail(e, PDRT_EINVAL, "no compiled convolution variant for this kernel size");
 }

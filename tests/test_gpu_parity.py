@@ -175,15 +175,15 @@ def test_edge_cases(torch):
 
 @pytest.mark.parametrize("k", [3, 5, 9, 17, 23, 33, 41, 43, 51, 55, 63, 75, 93, 125])
 def test_kernel_size_sweep_small(torch, k):
-    """pdrt_set_kernel_size, including sizes that have no compiled variant of their own, and sizes above 63, which run as
-    NB x NB passes of shifted sub-kernels (75, 93: 3 x 3; 125: 5 x 5)."""
+    """pdrt_set_kernel_size, including sizes that have no compiled variant of their own, and sizes above 75, which run as
+    NB x NB passes of shifted sub-kernels (93: 3 x 3; 125: 5 x 5)."""
     big = k > 33                       # a grid that holds the halo of the large kernels
     wl = W.tiny(seed=13, n_cp=2, kernel_size=5, nx=80 if big else 48, ny=44, nz=76 if big else 36, spacing=3.0, flu=(30, 30))
     eng, orc = pair(wl)
     eng.set_kernel_size(k)
     orc.set_kernel_size(k)
     passes = int(round(eng.info.kernel_passes ** 0.5))
-    assert eng.info.kernel_size == k and passes * eng.info.kernel_size_compiled >= k and (passes == 1) == (k <= 63)
+    assert eng.info.kernel_size == k and passes * eng.info.kernel_size_compiled >= k and (passes == 1) == (k <= 75)
     assert_dose(eng.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), orc.dose(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu), f"k={k}")
     g = W.seeded_dose_gradient(wl, seed=k)
     dl, dj, dm = eng.dose_backward(wl.leaves, wl.jaws, wl.gantry_deg, wl.mu, g)

@@ -1,5 +1,5 @@
 // pdrt_conv_sym.cuh — S4+S5 (forward) and S8 (adjoint): the per-slice lateral convolution (Eq. 8) in
-// ROW-SYMMETRIC form, the single-pass kernel of the path.
+// ROW-SYMMETRIC form (runs at 11 taps; pdrt_conv_fold.cuh adds the column symmetry and serves 15-75 taps).
 //
 // The pencil kernel is radially symmetric and its pixel-integrated table is built mirrored (R3), so
 // W[C+d][.] = W[C-d][.].  With the row correlation
@@ -12,9 +12,9 @@
 // One WARP per block, persistent over the work items (control point, slice, chunk along v) like k_conv.  A lane owns a UNIT =
 // (pair of input rows r, r+1) x (8 output columns): the (KT+7)-wide window of both rows sits in registers as float2 (row r,
 // row r+1), the weights come as warp-broadcast LDS.128 (four taps each; FFMA2 takes a tap as a scalar operand for both halves),
-// and one packed FFMA2 per tap and column yields (a_d, b_d) = (T_d[r], T_d[r+1]).  Output rows are accumulated in a shared-memory RING of rows private to the warp; since
-// out[r-d] takes a_d + b_{d+1} and out[r+1+d] takes b_d + a_{d+1}, walking d downwards with the previous (a, b) kept in
-// registers costs ONE read-modify-write of 8 columns per side and step.  In one step the "minus" rows r-d (parity of d) and
+// and one packed FFMA2 per tap and column yields (a_d, b_d) = (T_d[r], T_d[r+1]).  Output rows are accumulated in a
+// shared-memory RING of rows private to the warp; since out[r-d] takes a_d + b_{d+1} and out[r+1+d] takes b_d + a_{d+1},
+// walking d downwards with the previous (a, b) kept in registers costs ONE read-modify-write of 8 columns per side and step.  In one step the "minus" rows r-d (parity of d) and
 // the "plus" rows r+1+d (other parity) cannot coincide, and the lanes of a group hold distinct (row pair, tile), so a step
 // has no write conflicts; one __syncwarp per step orders the steps.  Rows that no later unit can reach are written to HBM
 // and their ring slots zeroed.  The input rows of the 32 units in flight are staged with cp.async (zero-filled outside the

@@ -105,7 +105,7 @@ __device__ __forceinline__ void fold_step(const float2 (&zc)[FRF], const float2 
 }
 
 template <int KT, bool ADJ>
-__global__ void __maxnreg__(KT <= 25 ? 168 : 255)
+__global__ void __maxnreg__(KT <= 25 ? 144 : 255)      // measured: 144 beats 128 .. 168 at 21 taps (the register file leaves 3 warps per scheduler from 129 to 168)
 k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
             const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
             int *item_counter, WorkCounters *wc, int in_floats, int out_floats)

@@ -217,7 +217,7 @@ __device__ __forceinline__ void ra_stream2(const RaRow &Ra, const RaRow &Rb, con
 // multiple of 4, L2-resident) and one aligned float4 store per lane; the loop is specialised on the number of candidates
 // (4, 6 or 9: the list is padded with zero weights) so that it carries no predicates.
 // Grid: (X, n_cp), blocks stride over the row chunks.
-__global__ void __launch_bounds__(RA_THREADS, 3)
+__global__ void __launch_bounds__(RA_THREADS, 4)
 k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__restrict__ sbox, int cp0, int n_cp, int C,
                    int nzp, const float *__restrict__ gT, float *__restrict__ G)
 {

@@ -138,6 +138,11 @@ struct pdrt_engine {
     cudaStream_t cs_in = nullptr, cs_out = nullptr;
     cudaEvent_t ev_fwd = nullptr, ev_out = nullptr, ev_g = nullptr, ev_bwd = nullptr;
     bool out_pending = false, bwd_recorded = false;
+    // S2 (and, in the backward call, the transposition of dL/dDose) do not depend on S1: they run on a side stream beside k_fluence
+    // (fork after what is queued on the call's stream, join before the first kernel that needs them); not while stage timing is on
+    cudaStream_t cs_side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    bool side_open = false;
     DevBuf<double> obj_partial;       // block partials of the objective
     size_t scratch_cap_bytes = (size_t)48 << 30;
     int last_n_cp = 0;
@@ -428,20 +433,49 @@ int check_call(pdrt_engine *e, int n_cp, std::initializer_list<const void *> ptr
 }
 
 // S1 + descriptors for all control points, S2 depths
+// Side stream: opened after everything queued on `st` so far, closed (joined) before the first kernel that needs its results.
+int side_fork(pdrt_engine *e, cudaStream_t st)
+{
+    if (!e->cs_side) {
+        CU(e, cudaStreamCreateWithFlags(&e->cs_side, cudaStreamNonBlocking));
+        CU(e, cudaEventCreateWithFlags(&e->ev_fork, cudaEventDisableTiming));
+        CU(e, cudaEventCreateWithFlags(&e->ev_join, cudaEventDisableTiming));
+    }
+    CU(e, cudaEventRecord(e->ev_fork, st));
+    CU(e, cudaStreamWaitEvent(e->cs_side, e->ev_fork, 0));
+    e->side_open = true;
+    return PDRT_OK;
+}
+int side_join(pdrt_engine *e, cudaStream_t st)
+{
+    if (!e->side_open) return PDRT_OK;
+    CU(e, cudaEventRecord(e->ev_join, e->cs_side));
+    CU(e, cudaStreamWaitEvent(st, e->ev_join, 0));
+    e->side_open = false;
+    return PDRT_OK;
+}
+
 int run_setup(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, const float *gantry, const float *mu,
-              bool need_depth, cudaStream_t st)
+              bool need_depth, cudaStream_t st, bool defer_join = false)
 {
     int rc = ensure_cp_scratch(e, n_cp);
     if (rc) return rc;
     if (e->coll_n != 0 && e->coll_n != n_cp) return fail(e, PDRT_EINVAL, "collimator angles were set for a different number of control points");
+    const bool fan = e->depth_mode == PDRT_DEPTH_FAN;
+    const bool beside = need_depth && !fan && !e->profiling;       // k_depth beside k_fluence (the fan marcher needs both their results)
+    if (beside) {
+        if ((rc = side_fork(e, st))) return rc;
+        ++e->launches[PDRT_STAGE_DEPTH];
+        k_depth<<<n_cp, DEPTH_THREADS, 0, e->cs_side>>>(e->P, n_cp, e->density.p, gantry, e->rho_s.p, e->Z_s.p, e->zrad.p);
+        CU(e, cudaGetLastError());
+    }
     {
         StageTimer t(e, PDRT_STAGE_FLUENCE, st);
         k_fluence<<<n_cp, FLU_THREADS, 0, st>>>(e->P, e->T, n_cp, leaves, jaws, gantry, e->coll_n ? e->coll.p : nullptr, mu, e->desc.p, e->sbox.p, e->wbox.p,
                                                e->P0.p, e->T1.p, e->T2.p, e->Abuf.p, e->phimap.p, e->phimapT.p);
     }
     CU(e, cudaGetLastError());
-    if (need_depth) {
-        const bool fan = e->depth_mode == PDRT_DEPTH_FAN;
+    if (need_depth && !beside) {
         if (fan) CU(e, e->fan.ensure((size_t)n_cp * e->fan_stride()));
         StageTimer t(e, PDRT_STAGE_DEPTH, st, fan ? 2 : 1);
         k_depth<<<n_cp, DEPTH_THREADS, 0, st>>>(e->P, n_cp, e->density.p, gantry, e->rho_s.p, e->Z_s.p, e->zrad.p);
@@ -450,6 +484,7 @@ int run_setup(pdrt_engine *e, int n_cp, const float *leaves, const float *jaws, 
                 e->P, e->desc.p, n_cp, e->density.p, gantry, e->zrad.p, e->ttab.p, e->fan_stride(), e->fan.p);
     }
     CU(e, cudaGetLastError());
+    if (!defer_join && (rc = side_join(e, st))) return rc;
     return PDRT_OK;
 }
 
@@ -499,9 +534,11 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
                         const float *mu, const float *gdose, cudaStream_t st, cudaEvent_t gdose_ready = nullptr)
 {
     set_conv_direction(e, true);
-    int rc = run_setup(e, n_cp, leaves, jaws, gantry, mu, true, st);
+    int rc = run_setup(e, n_cp, leaves, jaws, gantry, mu, true, st, true);
     if (rc) return rc;
-    if (gdose_ready) CU(e, cudaStreamWaitEvent(st, gdose_ready, 0));      // S1 / S2 above do not read dL/dDose
+    // S1 / S2 above do not read dL/dDose; its transposition runs on the side stream too when one is open
+    cudaStream_t ts = e->side_open ? e->cs_side : st;
+    if (gdose_ready) CU(e, cudaStreamWaitEvent(ts, gdose_ready, 0));
     const size_t nmap = (size_t)n_cp * e->P.Nuf * e->P.Nvf;
     CU(e, e->gphimap.ensure(nmap));
     CU(e, e->T3.ensure(nmap));
@@ -509,8 +546,10 @@ int backward_to_fluence(pdrt_engine *e, int n_cp, const float *leaves, const flo
     CU(e, e->gT.ensure(nxy * e->nzp));
     {   // S7 prologue: dL/dDose with z fastest, so that the resampling adjoint streams along v
         StageTimer t(e, PDRT_STAGE_TRANSPOSE, st);
-        k_transpose_g<<<dim3((unsigned)((nxy + 31) / 32), (e->nzp + 31) / 32), 256, 0, st>>>((int)nxy, e->P.nz, e->nzp, gdose, e->gT.p);
+        k_transpose_g<<<dim3((unsigned)((nxy + 31) / 32), (e->nzp + 31) / 32), 256, 0, ts>>>((int)nxy, e->P.nz, e->nzp, gdose, e->gT.p);
     }
+    CU(e, cudaGetLastError());
+    if ((rc = side_join(e, st))) return rc;
     if (e->pa_warps == 0) {   // planes of k_project_adjoint: as many of its 8 warps as fit into shared memory (opt-in above 48 KB, per device)
         const size_t per_warp = sizeof(float) * 32 * (size_t)e->P.Nuf;
         const int fit = (int)std::min<size_t>(PA_WARPS, (size_t)(200 << 10) / per_warp);
@@ -707,6 +746,8 @@ void pdrt_destroy(pdrt_engine *e)
     e->s_dose.release(); e->s_g.release(); e->s_grad.release();
     for (int q = 0; q < 2; ++q) { e->s_par[q].release(); if (e->h_par[q]) cudaFreeHost(e->h_par[q]); if (e->ev_par[q]) cudaEventDestroy(e->ev_par[q]); }
     if (e->h_grad) cudaFreeHost(e->h_grad);
+    if (e->cs_side) cudaStreamDestroy(e->cs_side);
+    for (cudaEvent_t ev : { e->ev_fork, e->ev_join }) if (ev) cudaEventDestroy(ev);
     if (e->cs_in) cudaStreamDestroy(e->cs_in);
     if (e->cs_out) cudaStreamDestroy(e->cs_out);
     for (cudaEvent_t ev : { e->ev_fwd, e->ev_out, e->ev_g, e->ev_bwd }) if (ev) cudaEventDestroy(ev);

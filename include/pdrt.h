@@ -310,6 +310,23 @@ PDRT_API int pdrt_objective(pdrt_engine *engine, const float *dose_dev, const ui
                             const float *lambda_host, const float *presc_host, int32_t power,
                             float *dL_ddose_dev, double *loss_dev, void *cuda_stream);
 
+/* pdrt_objective for callers that cannot allocate device memory (code under CUDA stream capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments, same result (dL/dDose bit-identical; the loss differs by float64
+ * rounding order only and does not depend on the GPU's SM count), but the call makes no cudaMalloc / cudaFree and uses no
+ * engine scratch.  Its scratch (8192 float64 block partials and a ticket, 64.25 KiB) is a static __device__ array of the
+ * library: every GPU that loads libpdrt.so holds it until the process exits.  Limits and rules:
+ *   - the dose grid may have at most PDRT_NOALLOC_MAX_VOXELS voxels; a larger grid is rejected with PDRT_EINVAL and a
+ *     message naming both numbers (use pdrt_objective there);
+ *   - all calls on one GPU — of every engine and every stream — share the array: calls that overlap on the GPU race
+ *     (wrong loss).  Order them on one stream or with events.  What must start at zero (the ticket) is cleared by
+ *     the call itself on `cuda_stream`, so a call does not depend on what the previous one left;
+ *   - the first call on a device resolves the array's device address (cudaGetSymbolAddress; no allocation): make one call
+ *     before stream capture begins.  One kernel launch and one 256-byte memset node per call, no synchronisation. */
+#define PDRT_NOALLOC_MAX_VOXELS (1 << 25)   /* 33 554 432 voxels, e.g. 512 x 512 x 128 */
+PDRT_API int pdrt_objective_noalloc(pdrt_engine *engine, const float *dose_dev, const uint32_t *structure_bits_dev, int32_t n_struct,
+                                    const float *lambda_host, const float *presc_host, int32_t power,
+                                    float *dL_ddose_dev, double *loss_dev, void *cuda_stream);
+
 /* Jaws tracking the aperture (BASELINE.json configs[4]): over the leaf pairs open by more than open_gap_mm (all pairs when
  * none is) x1 = min l - margin, x2 = max r + margin, y1 / y2 = the leaf boundaries that enclose them.  jaws_dev [n_cp][4]. */
 PDRT_API int pdrt_track_jaws(pdrt_engine *engine, int32_t n_cp, const float *leaves_dev, float margin_mm, float open_gap_mm,

@@ -18,7 +18,8 @@ SYMBOLS = ("pdrt_create", "pdrt_destroy", "pdrt_last_error", "pdrt_set_kernel_si
            "pdrt_set_profiling", "pdrt_get_stage_ms", "pdrt_set_depth_mode", "pdrt_stage_fan_factor", "pdrt_set_collimator",
            "pdrt_dose", "pdrt_dose_backward", "pdrt_dose_host", "pdrt_dose_backward_host", "pdrt_dose_host_async", "pdrt_host_wait",
            "pdrt_stage_fluence", "pdrt_stage_depth", "pdrt_stage_beam_dose", "pdrt_stage_grad_fluence",
-           "pdrt_mu_epsilon", "pdrt_validate", "pdrt_validate_backward", "pdrt_objective", "pdrt_track_jaws", "pdrt_plan_step")
+           "pdrt_mu_epsilon", "pdrt_validate", "pdrt_validate_backward", "pdrt_objective", "pdrt_objective_noalloc", "pdrt_track_jaws",
+           "pdrt_plan_step")
 
 STAGES = ("fluence", "depth", "scan", "conv", "gather", "resample_adj", "conv_adj", "project_adj", "fluence_adj", "project", "transpose")
 
@@ -117,6 +118,7 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.pdrt_validate.argtypes = [vp, i32, C.POINTER(PdrtLimits), vp, vp, vp, vp, vp, vp, vp]
     lib.pdrt_validate_backward.argtypes = [vp, i32, C.POINTER(PdrtLimits), vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.pdrt_objective.argtypes = [vp, vp, vp, i32, _FP, _FP, i32, vp, vp, vp]
+    lib.pdrt_objective_noalloc.argtypes = lib.pdrt_objective.argtypes
     lib.pdrt_track_jaws.argtypes = [vp, i32, vp, f32, f32, vp, vp]
     lib.pdrt_plan_step.argtypes = [vp, i32, f32, f32, vp, vp, vp, vp, vp]
     for name in SYMBOLS:
@@ -333,6 +335,20 @@ class Engine:
         loss, g = out
         self._check(self.lib.pdrt_objective(self.handle, d.data_ptr(), structure_bits.data_ptr(), len(lam), _fp(lam), _fp(presc),
                                             int(power), g.data_ptr(), loss.data_ptr(), self._stream()))
+        return loss, g
+
+    def objective_noalloc(self, dose, structure_bits, lam, presc, power, out):
+        """pdrt_objective_noalloc: pdrt_objective on the library's static device scratch — no device allocation in the call, so
+        `out` = (loss: 1-element float64 device tensor, dL/dDose: float32 device tensor of the dose shape) and a device-resident
+        float32 `dose` are the caller's.  Calls on one GPU share the scratch and must not overlap."""
+        torch = self.torch
+        loss, g = out
+        for t, dt in ((dose, torch.float32), (g, torch.float32), (structure_bits, torch.int32)):
+            assert t.is_cuda and t.is_contiguous() and t.dtype == dt and tuple(t.shape) == self.dose_shape
+        assert loss.is_cuda and loss.dtype == torch.float64 and loss.numel() == 1
+        lam, presc = _f32(lam), _f32(presc)
+        self._check(self.lib.pdrt_objective_noalloc(self.handle, dose.data_ptr(), structure_bits.data_ptr(), len(lam), _fp(lam), _fp(presc),
+                                                    int(power), g.data_ptr(), loss.data_ptr(), self._stream()))
         return loss, g
 
     def track_jaws(self, leaves, margin_mm, open_gap_mm, out=None):

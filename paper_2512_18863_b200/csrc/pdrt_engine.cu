@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <initializer_list>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1115,6 +1116,139 @@ int pdrt_plan_step(pdrt_engine *e, int32_t n_cp, float step_leaf, float step_mu,
     int rc = check_call(e, n_cp, { g_leaves, g_mu, leaves, mu }, false);
     if (rc) return rc;
     k_plan_step<<<1, STEP_THREADS, 0, (cudaStream_t)stream>>>(n_cp * 2 * e->P.Np, n_cp, step_leaf, step_mu, g_leaves, g_mu, leaves, mu);
+    CU(e, cudaGetLastError());
+    return PDRT_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// pdrt_objective_noalloc — pdrt_objective (Eq. 10 / quadratic) for callers that cannot allocate device
+// memory (stream capture, serving loops, harnesses that forbid it).  Its scratch — the block partials of the loss and the
+// ticket that elects the block which adds them up — lives in a file-scope __device__ array of fixed size; the call makes
+// no cudaMalloc / cudaFree and uses no engine scratch.
+//
+// In host code `g_noalloc_scratch` is a host-side stand-in for the symbol, NOT a device address: the address is resolved
+// with cudaGetSymbolAddress once per device (that device current) and handed to the kernel as a plain pointer.
+namespace {
+
+constexpr int NOALLOC_TILE = OBJ_THREADS * 16;                                  // voxels per block: fixed, so that the
+                                                                                // summation order does not depend on the GPU
+constexpr int NOALLOC_MAX_PARTIALS = PDRT_NOALLOC_MAX_VOXELS / NOALLOC_TILE;    // 8192 block partials
+constexpr int NOALLOC_HEADER = 32;                                              // doubles in front of the partials (256 bytes):
+                                                                                // the ticket (unsigned) sits in the first 4 bytes
+static_assert((long long)NOALLOC_MAX_PARTIALS * NOALLOC_TILE == PDRT_NOALLOC_MAX_VOXELS, "the maximum is a whole number of tiles");
+
+}  // namespace
+
+// 64.25 KiB per GPU that loads the library, held until the process exits.  Shared by every call on that GPU.
+static __device__ __align__(256) double g_noalloc_scratch[NOALLOC_HEADER + NOALLOC_MAX_PARTIALS];
+
+namespace {
+
+// k_objective with a fixed tile of voxels per block and the final sum folded in: every block writes its float64 partial to
+// scratch[NOALLOC_HEADER + block]; the block that draws the last ticket adds the partials in index order (thread t takes
+// t, t + 256, ...; then a fixed tree) and writes the loss.  The per-voxel arithmetic and the order of the structures are
+// those of k_objective, so dL/dDose is bit-identical; the loss differs from k_objective's by float64 rounding order only.
+// The ticket must be zero at launch (the entry point clears it on the stream); the partials need no clearing.
+__global__ void __launch_bounds__(OBJ_THREADS)
+k_objective_noalloc(size_t n_vox, const float *__restrict__ dose, const unsigned *__restrict__ bits, ObjectiveTerms T, float *__restrict__ g,
+                    double *scratch, double *__restrict__ loss)
+{
+    __shared__ double red[OBJ_THREADS];
+    __shared__ bool last;
+    unsigned *ticket = reinterpret_cast<unsigned *>(scratch);
+    double *partial = scratch + NOALLOC_HEADER;
+    const size_t base = (size_t)blockIdx.x * NOALLOC_TILE;
+    double L = 0.0;
+#pragma unroll 4
+    for (int q = 0; q < NOALLOC_TILE / OBJ_THREADS; ++q) {
+        const size_t x = base + (size_t)q * OBJ_THREADS + threadIdx.x;
+        if (x >= n_vox) break;
+        unsigned m = __ldg(bits + x);
+        float gx = 0.f;
+        if (m) {
+            const float D = __ldg(dose + x);
+            while (m) {
+                const int s = __ffs(m) - 1;
+                m &= m - 1;
+                if (s < T.n) {
+                    const float dlt = D - T.presc[s];
+                    if (T.power == 1) { L += (double)T.lambda[s] * fabs((double)dlt); gx += dlt > 0.f ? T.lambda[s] : (dlt < 0.f ? -T.lambda[s] : 0.f); }
+                    else { L += (double)T.lambda[s] * (double)dlt * (double)dlt; gx += 2.f * T.lambda[s] * dlt; }
+                }
+            }
+        }
+        g[x] = gx;
+    }
+    red[threadIdx.x] = L;
+    __syncthreads();
+    for (int o = OBJ_THREADS / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        partial[blockIdx.x] = red[0];
+        __threadfence();                                     // the partial is visible before the ticket is drawn
+        last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    const volatile double *pv = partial;                     // written by other blocks during this launch: no cached reads
+    double s = 0.0;
+    for (unsigned b = threadIdx.x; b < gridDim.x; b += OBJ_THREADS) s += pv[b];
+    red[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = OBJ_THREADS / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { *loss = red[0]; *ticket = 0u; }
+}
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+double *g_noalloc_addr[NOALLOC_MAX_DEVICES] = {};            // device address of g_noalloc_scratch, per device ordinal
+std::mutex g_noalloc_mutex;
+
+// Device address of the scratch array on the engine's device (current: check_call has set it).  Resolved once per device.
+int noalloc_scratch(pdrt_engine *e, double **out)
+{
+    if (e->device < 0 || e->device >= NOALLOC_MAX_DEVICES) return fail(e, PDRT_EINVAL, "pdrt_objective_noalloc: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_addr[e->device]) {
+        void *p = nullptr;
+        CU(e, cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        if (!p) return fail(e, PDRT_ECUDA, "pdrt_objective_noalloc: cudaGetSymbolAddress returned a null address");
+        g_noalloc_addr[e->device] = static_cast<double *>(p);
+    }
+    *out = g_noalloc_addr[e->device];
+    return PDRT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pdrt_objective_noalloc(pdrt_engine *e, const float *dose, const uint32_t *bits, int32_t n_struct, const float *lambda, const float *presc,
+                           int32_t power, float *g, double *loss, void *stream)
+{
+    int rc = check_call(e, 1, { dose, bits, lambda, presc, g, loss }, false);
+    if (rc) return rc;
+    if (n_struct < 1 || n_struct > OBJ_MAX_STRUCT) return fail(e, PDRT_EINVAL, "n_struct must lie in 1..32");
+    if (power != 1 && power != 2) return fail(e, PDRT_EINVAL, "power must be 1 (Eq. 10) or 2 (quadratic)");
+    const size_t n_vox = (size_t)e->P.nx * e->P.ny * e->P.nz;
+    if (n_vox > (size_t)PDRT_NOALLOC_MAX_VOXELS)
+        return fail(e, PDRT_EINVAL, "pdrt_objective_noalloc: the dose grid has " + std::to_string(n_vox) + " voxels, the static scratch serves at most " +
+                                        std::to_string((long long)PDRT_NOALLOC_MAX_VOXELS) + " (PDRT_NOALLOC_MAX_VOXELS); use pdrt_objective");
+    ObjectiveTerms T{};
+    T.n = n_struct; T.power = power;
+    for (int s = 0; s < n_struct; ++s) { T.lambda[s] = lambda[s]; T.presc[s] = presc[s]; }
+    double *scratch = nullptr;
+    if ((rc = noalloc_scratch(e, &scratch))) return rc;
+    const unsigned nb = (unsigned)((n_vox + NOALLOC_TILE - 1) / NOALLOC_TILE);
+    CU(e, cudaMemsetAsync(scratch, 0, NOALLOC_HEADER * sizeof(double), (cudaStream_t)stream));      // the ticket starts at zero whatever the last call left
+    k_objective_noalloc<<<nb, OBJ_THREADS, 0, (cudaStream_t)stream>>>(n_vox, dose, bits, T, g, scratch, loss);
     CU(e, cudaGetLastError());
     return PDRT_OK;
 }

@@ -185,34 +185,34 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
                 Wf[e] = m <= C ? (1.f - f) * __ldg(w0 + dd * KP + m) + f * __ldg(w1 + dd * KP + m) : 0.f;
             }
         }
-        // flush geometry: the lanes walk the 16-byte (forward) / 8-byte (adjoint) chunks of consecutive rows, 32 chunks per trip
-        const int nchunk = ADJ ? FRF * nt / 2 : FRF * nt / 4;
-        const int lrow0 = lane / nchunk, lch0 = lane - lrow0 * nchunk, srow = 32 / nchunk, sch = 32 - srow * nchunk;
+        // flush geometry: a lane owns one 16-byte chunk column (chunks 32 apart when a row has more) and every srow-th row of a trip
+        const int nchunk = (FRF * nt + 3) >> 2;
+        const int srow = nchunk >= 32 ? 1 : 32 / nchunk;
+        const int lrow0 = nchunk >= 32 ? 0 : lane / nchunk, lch0 = lane - lrow0 * nchunk;
+        const bool lane_on = lrow0 < srow;
         const int room = pv - (av0 - rj0);                 // columns of the region from av0 on
         int flushed = Tu0, fslot = 0;                      // rows below `flushed` are final and written; ring slot of row `flushed`
         auto flush = [&](int b) {                          // rows [flushed, b): ring -> HBM (inside the written box), slots back to zero
-            int i = flushed + lrow0, ch = lch0, sl = fslot + lrow0;
+            int sl = fslot + lrow0;
             while (sl >= R) sl -= R;
-            while (__any_sync(0xffffffffu, i < b)) {
-                if (i < b) {
-                    float *rowp = oring + sl * pitch;
+            float *rowp = oring + sl * pitch + 4 * lch0;
+            float *orow = oslice + (long long)(flushed + lrow0) * pv + 4 * lch0;
+            for (int i = flushed + lrow0, i0 = flushed; i0 < b; i0 += srow, i += srow) {
+                if (lane_on && i < b) {
                     const bool wr = i >= wu0 && i <= wu1;
-                    float *orow = oslice + (long long)i * pv;
-                    if (ADJ) {
-                        float2 *p = reinterpret_cast<float2 *>(rowp + 2 * ch);
-                        const float2 v = *p;
-                        *p = make_float2(0.f, 0.f);
-                        if (wr && 2 * ch + 2 <= room) *reinterpret_cast<float2 *>(orow + 2 * ch) = v;
-                    } else {
-                        float4 *p = reinterpret_cast<float4 *>(rowp + 4 * ch);
+                    for (int ch = lch0, o = 0; ch < nchunk; ch += 32, o += 128) {
+                        float4 *p = reinterpret_cast<float4 *>(rowp + o);
                         const float4 v = *p;
                         *p = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (wr && 4 * ch + 4 <= room) *reinterpret_cast<float4 *>(orow + 4 * ch) = v;
+                        if (ADJ) {                         // the adjoint's columns start on an 8-byte boundary
+                            if (wr && 4 * ch + 2 <= room) *reinterpret_cast<float2 *>(orow + o) = make_float2(v.x, v.y);
+                            if (wr && 4 * ch + 4 <= room) *reinterpret_cast<float2 *>(orow + o + 2) = make_float2(v.z, v.w);
+                        } else if (wr && 4 * ch + 4 <= room) *reinterpret_cast<float4 *>(orow + o) = v;
                     }
                 }
-                ch += sch; i += srow; sl += srow;
-                if (ch >= nchunk) { ch -= nchunk; ++i; ++sl; }
-                while (sl >= R) sl -= R;
+                sl += srow; rowp += srow * pitch;
+                if (sl >= R) { sl -= R; rowp -= R * pitch; }
+                orow += (long long)srow * pv;
             }
             fslot += b - flushed;
             while (fslot >= R) fslot -= R;
@@ -220,12 +220,15 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
         };
 
         const int n_units = npair * nt;
+        // u / nt for unit indices (u < 2^16, nt < 2^8: the multiply-high by ceil(2^32 / nt) is exact)
+        const unsigned nt_magic = nt > 1 ? 0xffffffffu / (unsigned)nt + 1u : 0u;
+        auto div_nt = [&](int u) { return nt > 1 ? (int)__umulhi((unsigned)u, nt_magic) : u; };
         // units [u0, u1) of one group: at most 32, of at most `maxp` row pairs
-        auto group_end = [&](int u0) { return min(min(n_units, u0 + 32), (u0 / nt + maxp) * nt); };
+        auto group_end = [&](int u0) { return min(min(n_units, u0 + 32), (div_nt(u0) + maxp) * nt); };
         // stage the input rows of a group's pairs (asynchronous copies, zero outside the source box): per-lane column terms, then one
         // pass over the rows
         auto stage = [&](int u0, int u1) {
-            const int p_lo = u0 / nt, p_hi = (u1 - 1) / nt, r_lo = in_u0 + 2 * p_lo;
+            const int p_lo = div_nt(u0), p_hi = div_nt(u1 - 1), r_lo = in_u0 + 2 * p_lo;
             const float *sp[MCX];
             unsigned dp[MCX];
             int csz[MCX];
@@ -241,26 +244,37 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
             }
             const int nrow = 2 * (p_hi - p_lo + 1);
             const int nin = min(nrow, in_u1 - r_lo + 1);          // only the second row of the last pair can lie outside the input rows
-            unsigned ro = 0;
-            for (int rl = 0; rl < nin; ++rl) {
+            auto rows = [&](auto ns_) {                           // ns = the column slots in use (warp-uniform)
+                constexpr int ns = decltype(ns_)::value;
+                unsigned ro = 0;
+                for (int rl = 0; rl < nin; ++rl) {
 #pragma unroll
-                for (int m = 0; m < MCX; ++m) {
-                    if (cex[m]) cp_async_4(dp[m] + ro, sp[m], csz[m]);
-                    sp[m] += pv;
+                    for (int m = 0; m < ns; ++m) {
+                        if (cex[m]) cp_async_4(dp[m] + ro, sp[m], csz[m]);
+                        sp[m] += pv;
+                    }
+                    ro += (rl & 1) ? 16u * (unsigned)PPc - 4u : 4u;
                 }
-                ro += (rl & 1) ? 16u * (unsigned)PPc - 4u : 4u;
-            }
-            if (nin < nrow) {
+                if (nin < nrow) {
 #pragma unroll
-                for (int m = 0; m < MCX; ++m)
-                    if (cex[m]) cp_async_4(dp[m] + ro, sbase, 0);
+                    for (int m = 0; m < ns; ++m)
+                        if (cex[m]) cp_async_4(dp[m] + ro, sbase, 0);
+                }
+            };
+            static_assert(MCX <= 5, "column slots per lane");
+            switch ((ncols + 31) >> 5) {
+            case 1: rows(std::integral_constant<int, 1>{}); break;
+            case 2: rows(std::integral_constant<int, MCX < 2 ? MCX : 2>{}); break;
+            case 3: rows(std::integral_constant<int, MCX < 3 ? MCX : 3>{}); break;
+            case 4: rows(std::integral_constant<int, MCX < 4 ? MCX : 4>{}); break;
+            default: rows(std::integral_constant<int, MCX>{}); break;
             }
         };
         __syncwarp();                                      // Wd is complete; the previous item has left the ring zeroed and the staged rows free
         stage(0, group_end(0));
         for (int u0 = 0; u0 < n_units;) {
             const int u1 = group_end(u0);
-            const int p_lo = u0 / nt, p_hi = (u1 - 1) / nt;
+            const int p_lo = div_nt(u0), p_hi = div_nt(u1 - 1);
             const int r_lo = in_u0 + 2 * p_lo, r_hi = in_u0 + 2 * p_hi;
             {   // rows that no unit from here on reaches
                 const int lo = min(max(r_lo - CHk, Tu0), Tu1 + 1);
@@ -271,7 +285,7 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
 
             const int u = u0 + lane;
             const bool active = u < u1;
-            const int p = active ? u / nt : p_lo, t = active ? u - p * nt : 0;
+            const int p = active ? div_nt(u) : p_lo, t = active ? u - p * nt : 0;
             const int r = in_u0 + 2 * p;
             float2 zc[FRF], z[C][FRF];                     // folded window: zc[c] = x[j_c], z[m-1][c] = x[j_c - m] + x[j_c + m], as (row r, row r+1)
             {
@@ -300,7 +314,10 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
             }
             if (active && CHk >= d_lo) macs += (unsigned long long)(CHk - d_lo + 1) * ((C + 1) * FRF * 2);
             int rowm = r - CHk, rowp = r + 1 + CHk;
-            int sm = pmod(rowm - flushed + fslot, R), sp_ = pmod(rowp - flushed + fslot, R);
+            int sm = rowm - flushed + fslot, sp_ = rowp - flushed + fslot;     // ring slots: a few rings off at most
+            while (sm < 0) sm += R;
+            while (sm >= R) sm -= R;
+            while (sp_ >= R) sp_ -= R;
             const float4 *wrow = Wd + CHk * WQ;
             float *const obase = oring + FRF * t;
             float2 accA[FRF], accB[FRF];

@@ -51,12 +51,35 @@ inline size_t fold_smem_bytes(int kt)
     return sizeof(float) * ((size_t)(c + 1) * fold_wpitch(kt) + fold_in_floats(kt) + fold_out_floats(kt));
 }
 
+// 16- / 8-byte accesses of the ring by shared-window address (an address register per row instead of a generic pointer whose
+// window base the compiler would re-derive from the special registers in every step)
+__device__ __forceinline__ float4 ring_ld4(unsigned a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void ring_st4(unsigned a, const float4 &v)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ float2 ring_ld2(unsigned a)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void ring_st2(unsigned a, const float2 &v)
+{
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.x), "f"(v.y) : "memory");
+}
+
 // One step d of a unit: acc = (a_d, b_d) from the folded window and the weight row in `w`; then the next step's weights are fetched
-// and out[r-d] += a_d + b_{d+1}, out[r+1+d] += b_d + a_{d+1} with (a_{d+1}, b_{d+1}) = prev.  om / op: the unit's 4 columns of the two
-// ring rows, null when the row is not held.
+// and out[r-d] += a_d + b_{d+1}, out[r+1+d] += b_d + a_{d+1} with (a_{d+1}, b_{d+1}) = prev.  om / op: shared-window addresses of the
+// unit's columns in the two ring rows; hm / hp: whether the row is held.
 template <int C, int FRF>
 __device__ __forceinline__ void fold_step(const float2 (&zc)[FRF], const float2 (&z)[C][FRF], float4 (&w)[(C + 4) / 4], const float4 *__restrict__ wnext,
-                                          float2 (&acc)[FRF], const float2 (&prev)[FRF], float *om, float *op)
+                                          float2 (&acc)[FRF], const float2 (&prev)[FRF], unsigned om, bool hm, unsigned op, bool hp)
 {
     constexpr int WQ = (C + 4) / 4;
 #pragma unroll
@@ -75,31 +98,27 @@ __device__ __forceinline__ void fold_step(const float2 (&zc)[FRF], const float2 
 #pragma unroll
     for (int q = 0; q < WQ; ++q) w[q] = wnext[q];
     if constexpr (FRF == 4) {
-        if (om) {
-            float4 *o = reinterpret_cast<float4 *>(om);
-            float4 v = *o;
+        if (hm) {
+            float4 v = ring_ld4(om);
             v.x += acc[0].x + prev[0].y; v.y += acc[1].x + prev[1].y; v.z += acc[2].x + prev[2].y; v.w += acc[3].x + prev[3].y;
-            *o = v;
+            ring_st4(om, v);
         }
-        if (op) {
-            float4 *o = reinterpret_cast<float4 *>(op);
-            float4 v = *o;
+        if (hp) {
+            float4 v = ring_ld4(op);
             v.x += acc[0].y + prev[0].x; v.y += acc[1].y + prev[1].x; v.z += acc[2].y + prev[2].x; v.w += acc[3].y + prev[3].x;
-            *o = v;
+            ring_st4(op, v);
         }
     } else {
         static_assert(FRF == 2 || FRF == 4, "units are 2 or 4 columns wide");
-        if (om) {
-            float2 *o = reinterpret_cast<float2 *>(om);
-            float2 v = *o;
+        if (hm) {
+            float2 v = ring_ld2(om);
             v.x += acc[0].x + prev[0].y; v.y += acc[1].x + prev[1].y;
-            *o = v;
+            ring_st2(om, v);
         }
-        if (op) {
-            float2 *o = reinterpret_cast<float2 *>(op);
-            float2 v = *o;
+        if (hp) {
+            float2 v = ring_ld2(op);
             v.x += acc[0].y + prev[0].x; v.y += acc[1].y + prev[1].x;
-            *o = v;
+            ring_st2(op, v);
         }
     }
 }
@@ -122,6 +141,8 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
     float4 *xin4 = smem4 + (C + 1) * WQ;              // [pair][chunk]: (x[r][c], x[r+1][c], x[r][c+1], x[r+1][c+1]), chunks swizzled
     float *oring = reinterpret_cast<float *>(xin4) + in_floats;   // [slot][pitch]: ring of output rows, all zero between uses
     const unsigned xin_s = (unsigned)__cvta_generic_to_shared(xin4);
+    unsigned oring_s = (unsigned)__cvta_generic_to_shared(oring);
+    asm volatile("" : "+r"(oring_s));                 // an ordinary register value from here on
     const int lane = threadIdx.x;
     const int total = tile_base[n_cp];
     const int CHk = min(P.CH, C);                     // rows C+d with d > CH of an embedded smaller kernel are zero
@@ -167,6 +188,7 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
             Tu0 = min(wu0, in_u0 - CHk); Tu1 = max(wu1, in_u0 + 2 * npair - 1 + CHk);
         }
         const int pitch = fold_out_pitch(nt, FRF), R = out_floats / pitch;
+        const unsigned pitch_b = 4u * (unsigned)pitch, ring_bytes = pitch_b * (unsigned)R;
         const int PPc = fold_in_chunks(nt, FRF, C), maxp = fold_max_pairs(nt);
         const int ncols = FRF * nt + 2 * C;
         const long long slice_off = (long long)slot * P.stride_cp + (long long)k * pu * pv;
@@ -319,7 +341,9 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
             while (sm >= R) sm -= R;
             while (sp_ >= R) sp_ -= R;
             const float4 *wrow = Wd + CHk * WQ;
-            float *const obase = oring + FRF * t;
+            // byte addresses of the unit's columns in its two ring rows; the "minus" row walks up the ring, the "plus" row down
+            unsigned am = oring_s + 4u * (unsigned)(FRF * t + sm * pitch), ap = oring_s + 4u * (unsigned)(FRF * t + sp_ * pitch);
+            const unsigned a_lo = oring_s + 4u * (unsigned)(FRF * t), a_hi = a_lo + ring_bytes;   // row 0 and one past row R - 1
             float2 accA[FRF], accB[FRF];
 #pragma unroll
             for (int c = 0; c < FRF; ++c) accB[c] = make_float2(0.f, 0.f);
@@ -327,19 +351,25 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
 #pragma unroll
             for (int q = 0; q < WQ; ++q) w[q] = wrow[q];
             auto held = [&](int row) { return active && (!ADJ || (row >= Tu0 && row <= Tu1)); };
+            auto advance = [&]() {
+                ++rowm; --rowp;
+                am += pitch_b; if (am == a_hi) am = a_lo;
+                if (ap == a_lo) ap = a_hi;
+                ap -= pitch_b;
+            };
             int dd = CHk;
 #pragma unroll 1
             for (; dd > d_lo; dd -= 2) {                   // two steps per trip: the accumulators swap roles, no register copies
-                fold_step<C, FRF>(zc, z, w, wrow - WQ, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
-                ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
+                fold_step<C, FRF>(zc, z, w, wrow - WQ, accA, accB, am, held(rowm), ap, held(rowp));
+                advance();
                 __syncwarp();                              // the rows of this step are visible to the next one
                 wrow -= dd >= 2 ? 2 * WQ : WQ;             // row dd - 2 of the next trip (row 0 again after the last step: never used)
-                fold_step<C, FRF>(zc, z, w, wrow, accB, accA, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
-                ++rowm; --rowp; sm = sm + 1 == R ? 0 : sm + 1; sp_ = sp_ == 0 ? R - 1 : sp_ - 1;
+                fold_step<C, FRF>(zc, z, w, wrow, accB, accA, am, held(rowm), ap, held(rowp));
+                advance();
                 __syncwarp();
             }
             if (dd == d_lo) {                              // odd number of steps: the last one
-                fold_step<C, FRF>(zc, z, w, wrow, accA, accB, held(rowm) ? obase + sm * pitch : nullptr, held(rowp) ? obase + sp_ * pitch : nullptr);
+                fold_step<C, FRF>(zc, z, w, wrow, accA, accB, am, held(rowm), ap, held(rowp));
                 __syncwarp();
             }
             u0 = u1;

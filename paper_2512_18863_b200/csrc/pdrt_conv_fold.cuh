@@ -207,33 +207,31 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
                 Wf[e] = m <= C ? (1.f - f) * __ldg(w0 + dd * KP + m) + f * __ldg(w1 + dd * KP + m) : 0.f;
             }
         }
-        // flush geometry: a lane owns one 16-byte chunk column (chunks 32 apart when a row has more) and every srow-th row of a trip
+        // flush geometry: a row has at most FOLD_COLS_MAX / 4 = 20 chunks of 16 bytes; a lane owns one chunk column and every srow-th row
         const int nchunk = (FRF * nt + 3) >> 2;
-        const int srow = nchunk >= 32 ? 1 : 32 / nchunk;
-        const int lrow0 = nchunk >= 32 ? 0 : lane / nchunk, lch0 = lane - lrow0 * nchunk;
-        const bool lane_on = lrow0 < srow;
+        const int srow = 32 / nchunk;
+        const int lrow0 = lane / nchunk, lch0 = lane - lrow0 * nchunk;
         const int room = pv - (av0 - rj0);                 // columns of the region from av0 on
+        const int fl_step = lrow0 < srow ? srow : 0x10000; // rows per trip of this lane; lanes past the last whole row sit out
+        const bool col_ok = 4 * lch0 + 4 <= room, col_ok2 = 4 * lch0 + 2 <= room;
+        const unsigned fl_a0 = oring_s + 16u * (unsigned)lch0, fl_a1 = fl_a0 + ring_bytes;     // the lane's chunk in ring row 0, and one ring on
         int flushed = Tu0, fslot = 0;                      // rows below `flushed` are final and written; ring slot of row `flushed`
         auto flush = [&](int b) {                          // rows [flushed, b): ring -> HBM (inside the written box), slots back to zero
             int sl = fslot + lrow0;
             while (sl >= R) sl -= R;
-            float *rowp = oring + sl * pitch + 4 * lch0;
+            unsigned ra = fl_a0 + pitch_b * (unsigned)sl;
             float *orow = oslice + (long long)(flushed + lrow0) * pv + 4 * lch0;
-            for (int i = flushed + lrow0, i0 = flushed; i0 < b; i0 += srow, i += srow) {
-                if (lane_on && i < b) {
-                    const bool wr = i >= wu0 && i <= wu1;
-                    for (int ch = lch0, o = 0; ch < nchunk; ch += 32, o += 128) {
-                        float4 *p = reinterpret_cast<float4 *>(rowp + o);
-                        const float4 v = *p;
-                        *p = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (ADJ) {                         // the adjoint's columns start on an 8-byte boundary
-                            if (wr && 4 * ch + 2 <= room) *reinterpret_cast<float2 *>(orow + o) = make_float2(v.x, v.y);
-                            if (wr && 4 * ch + 4 <= room) *reinterpret_cast<float2 *>(orow + o + 2) = make_float2(v.z, v.w);
-                        } else if (wr && 4 * ch + 4 <= room) *reinterpret_cast<float4 *>(orow + o) = v;
-                    }
+            for (int i = flushed + lrow0; i < b && fl_step <= 32; i += fl_step) {
+                const float4 v = ring_ld4(ra);
+                ring_st4(ra, make_float4(0.f, 0.f, 0.f, 0.f));
+                if (i >= wu0 && i <= wu1) {
+                    if (ADJ) {                             // the adjoint's columns start on an 8-byte boundary
+                        if (col_ok2) *reinterpret_cast<float2 *>(orow) = make_float2(v.x, v.y);
+                        if (col_ok) *reinterpret_cast<float2 *>(orow + 2) = make_float2(v.z, v.w);
+                    } else if (col_ok) *reinterpret_cast<float4 *>(orow) = v;
                 }
-                sl += srow; rowp += srow * pitch;
-                if (sl >= R) { sl -= R; rowp -= R * pitch; }
+                ra += pitch_b * (unsigned)srow;
+                if (ra >= fl_a1) ra -= ring_bytes;
                 orow += (long long)srow * pv;
             }
             fslot += b - flushed;

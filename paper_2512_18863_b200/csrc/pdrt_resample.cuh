@@ -12,12 +12,17 @@ namespace pdrt {
 
 namespace cg = cooperative_groups;
 
-constexpr int GD_PX = 8, GD_PY = 2;              // a block owns 8 x 2 patient columns (x,y): 32-byte runs of the dose rows
-constexpr int GD_COLS = GD_PX * GD_PY;           // ... one half-warp per column
-constexpr int GD_CPB = 16;                       // control points set up per round (16 columns x 16 control points = 256 threads)
+constexpr int GD_PX = 8, GD_PY = 4;              // a block owns 8 x 4 patient columns (x,y): 32-byte runs of the dose rows
+constexpr int GD_COLS = GD_PX * GD_PY;
+constexpr int GD_LANES = 8;                      // lanes per column: a quarter-warp reads 128 contiguous bytes of a beam row.  Every lane
+                                                 // of a column fetches the column's stencil record from shared memory, and a warp-wide
+                                                 // LDS.128 takes four data-pipe cycles however many lanes share an address: with 8 lanes
+                                                 // instead of 16 the records cost half as many cycles per byte of D_b
+constexpr int GD_CPB = 8;                        // control points set up per round (32 columns x 8 control points = 256 threads)
 constexpr int GD_THREADS = GD_COLS * GD_CPB;
-constexpr int GD_ZSPAN = 64;                     // z covered by one pass of a half-warp (16 lanes x float4)
-constexpr int GD_MAXPASS = 4;                    // passes held in registers at once (256 z)
+static_assert(GD_THREADS == GD_COLS * GD_LANES, "phase A (column, control point) and phase B (column, lane) use the same threads");
+constexpr int GD_ZSPAN = 4 * GD_LANES;           // z covered by one pass of a column's lanes (8 lanes x float4)
+constexpr int GD_MAXPASS = 4;                    // passes held in registers at once (128 z)
 constexpr int GD_LIST = GD_THREADS;              // control points listed per outer chunk: one thread each
 
 struct __align__(16) GatherCp {                  // what the stencil set-up needs of a listed control point (32 bytes, shared memory)
@@ -32,7 +37,7 @@ struct __align__(16) GatherRec {                 // bilinear stencil of one (pat
     int pad_[2];
 };
 
-// phase B of k_gather_dose for one round of control points: NP z-passes of 64 held in registers, NB control points per
+// phase B of k_gather_dose for one round of control points: NP z-passes of 32 held in registers, NB control points per
 // batch.  Straight-line code: the 4 NB NP loads of a batch are all issued before the first use.  Records of control points that
 // do not reach the column carry empty z-ranges (no reads) and zero weights.
 template <int NP, int NB>
@@ -74,14 +79,14 @@ __device__ __forceinline__ void gather_round(const GatherRec (*rec)[GD_COLS], in
     }
 }
 
-// S6.  Grid: (ceil(nx/8), ceil(ny/2), 1); a block owns 8 x 2 patient columns (x,y) over all z.
+// S6.  Grid: (ceil(nx/8), ceil(ny/4), 1); a block owns 8 x 4 patient columns (x,y) over all z.
 //   dose[p] (+)= sum_b scale_b * bilinear_0(D_b[.][z][.]; fu, fw)
 // The gantry rotates about z (G1), so for one control point the beam-frame position (fu, fw) and the four
 // bilinear weights of a column are the same for all its voxels.  Warp 0 first lists the control points whose compact
-// region can reach the block's columns (with the constants the set-up needs, and the z-range they cover).  Then, 16
+// region can reach the block's columns (with the constants the set-up needs, and the z-range they cover).  Then, 8
 // control points at a time: phase A, one THREAD per (column, control point) builds the stencil record (pointers to the four
 // beam rows, weights, and the v-range that the forward conv wrote in the two slices — outside it D_b is zero and the block
-// holds stale data); phase B, one HALF-WARP per column streams 16-byte vectors along v, several control points per batch
+// holds stale data); phase B, one QUARTER-WARP per column streams 16-byte vectors along v, several control points per batch
 // with all their loads in flight at once, accumulating in registers in control-point order (deterministic).  The records
 // are double-buffered and the global reads of phase A for round r+1 are issued before phase B of round r, so that their
 // latency is covered.  Every patient voxel of the z-range is written exactly once; the rest of the dose grid is zeroed by
@@ -93,9 +98,9 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
     __shared__ GatherRec rec[2][GD_CPB][GD_COLS];
     __shared__ GatherCp list[GD_LIST];
     __shared__ int n_list_s, zmin_s, zmax_s, wcount_s[GD_THREADS / 32], wzlo_s[GD_THREADS / 32], wzhi_s[GD_THREADS / 32];
-    const int tid = threadIdx.x, lane16 = tid & 15;
-    const int col = tid >> 4;                                    // phase B: column of this half-warp
-    const int a_col = tid & 15, a_cp = tid >> 4;                 // phase A: (column, control point of the round)
+    const int tid = threadIdx.x, lz = tid & (GD_LANES - 1);
+    const int col = tid / GD_LANES;                              // phase B: column of this quarter-warp
+    const int a_col = tid & (GD_COLS - 1), a_cp = tid / GD_COLS; // phase A: (column, control point of the round)
     const int px0 = blockIdx.x * GD_PX, py0 = blockIdx.y * GD_PY;
     // tile corners (for culling), relative to the isocentre
     const float cx0 = P.ox + px0 * P.sx - P.isox, cx1 = cx0 + (GD_PX - 1) * P.sx;
@@ -104,7 +109,7 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
     const int ax = px0 + (a_col & (GD_PX - 1)), ay = py0 + a_col / GD_PX;
     const float adx = P.ox + ax * P.sx - P.isox, ady = P.oy + ay * P.sy - P.isoy;
     const bool a_inside = ax < P.nx && ay < P.ny;
-    // phase-B column of this half-warp
+    // phase-B column of this quarter-warp
     const int bx = px0 + (col & (GD_PX - 1)), by = py0 + col / GD_PX;
     const bool b_inside = bx < P.nx && by < P.ny;
 
@@ -198,12 +203,12 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
         __syncthreads();
         const int n_list = n_list_s, zmin = zmin_s, zmax = zmax_s;
         if (n_list == 0) continue;
-        for (int zb = zmin; zb < zmax; zb += GD_ZSPAN * GD_MAXPASS) {            // one iteration unless the regions span > 256 z
+        for (int zb = zmin; zb < zmax; zb += GD_ZSPAN * GD_MAXPASS) {            // one iteration unless the regions span > 128 z
             float2 acc[GD_MAXPASS][2];                                           // [pass][z pair] of this lane's quads
 #pragma unroll
             for (int p = 0; p < GD_MAXPASS; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
             const int npass = min(GD_MAXPASS, (zmax - zb + GD_ZSPAN - 1) / GD_ZSPAN);
-            const int zq = zb + 4 * lane16;
+            const int zq = zb + 4 * lz;
             {   // records of round 0
                 const Setup s = setup_load(a_cp, n_list);
                 setup_store(s, a_cp, rec[0][a_cp][a_col]);
@@ -225,7 +230,7 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
 #pragma unroll
                 for (int ps = 0; ps < GD_MAXPASS; ++ps) {
                     if (ps >= npass) continue;
-                    const int z = zb + ps * GD_ZSPAN + 4 * lane16;
+                    const int z = zb + ps * GD_ZSPAN + 4 * lz;
                     const float v[4] = { acc[ps][0].x, acc[ps][0].y, acc[ps][1].x, acc[ps][1].y };
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {

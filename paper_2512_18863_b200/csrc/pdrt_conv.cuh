@@ -168,8 +168,10 @@ struct __align__(16) RaRow {        // one beam row (k, i) of G_b: its patient-c
     int j0, nq;                     // first column (multiple of 4) and number of quads to write
     int xa, xb, ya, yb;             // candidate box of the general path
     float eu0, ew0;
-    int pad_[2];
+    int pad_[2];                    // 144 bytes: an odd number of 16-byte chunks, so that the set-up's stores (one row per thread) spread
+                                    // over the banks
 };
+static_assert(sizeof(RaRow) == 144, "row records are 9 chunks of 16 bytes");
 
 // one quad of each of TWO beam rows from NC candidates each (the first NC entries of the rows' lists), no predicates: the
 // 2 NC loads are all in flight before the first use.  A row with nothing to write has nq = 0.
@@ -274,7 +276,7 @@ k_resample_adjoint(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *
             }
             {   // entries past n repeat entry 0 with weight 0 (every address readable, no predicates in the stream loop)
                 const int o0 = n > 0 ? R.off[0] : 0;
-                for (int c = max(n, 0); c < RA_PADC; ++c) { R.off[c] = o0; R.w[c] = 0.f; }
+                for (int c = max(n, 0); c < RA_MAXC; ++c) { R.off[c] = o0; R.w[c] = 0.f; }
             }
             R.n = n;
         }

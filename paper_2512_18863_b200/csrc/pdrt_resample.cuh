@@ -29,13 +29,17 @@ struct __align__(16) GatherCp {                  // what the stencil set-up need
     float cg, sg, scale;
     int ri0, pu, pv, rj0, slot;
 };
-struct __align__(16) GatherRec {                 // bilinear stencil of one (patient column, control point): 64 bytes
-    const float *row[4];                         // beam rows (i0,k0), (i0+1,k0), (i0,k0+1), (i0+1,k0+1), shifted so that row[q][z] is voxel
-                                                 // v = z; invalid neighbours are folded onto a valid row
-    float w[4];                                  // cal * MU * bilinear weight; 0 for invalid neighbours
-    short zlo0, zhi0, zlo1, zhi1;                // written v-range [zlo, zhi) of slice k0 and of slice k0+1 (multiples of 8); empty: no reads
-    int pad_[2];
+struct __align__(16) GatherRec {                 // bilinear stencil of one (patient column, control point): 64 bytes in four 16-byte chunks
+    ulonglong2 q[4];                             // chunk c sits at q[c ^ gather_swz(column)]: the records of consecutive columns are 64 bytes
+                                                 // apart, and unswizzled their chunks would fall on two bank groups (4-way conflicts
+                                                 // of the set-up's stores)
+    // chunk 0: beam rows (i0,k0), (i0+1,k0); chunk 1: rows (i0,k0+1), (i0+1,k0+1) — pointers shifted so that row[z] is voxel v = z,
+    //          invalid neighbours folded onto a valid row
+    // chunk 2: four floats cal * MU * bilinear weight, 0 for invalid neighbours
+    // chunk 3: .x = four shorts zlo0, zhi0, zlo1, zhi1: written v-range [zlo, zhi) of slice k0 and of slice k0+1 (multiples of 8);
+    //          empty: no reads
 };
+__device__ __forceinline__ int gather_swz(int column) { return (column >> 1) & 3; }
 
 // phase B of k_gather_dose for one round of control points: NP z-passes of 32 held in registers, NB control points per
 // batch.  Straight-line code: the 4 NB NP loads of a batch are all issued before the first use.  Records of control points that
@@ -43,16 +47,19 @@ struct __align__(16) GatherRec {                 // bilinear stencil of one (pat
 template <int NP, int NB>
 __device__ __forceinline__ void gather_round(const GatherRec (*rec)[GD_COLS], int col, int nround, int zq, float2 (&acc)[GD_MAXPASS][2])
 {
+    const int sw = gather_swz(col);
     for (int e0 = 0; e0 < nround; e0 += NB) {
         float4 v[NB][NP][4];
         float4 w[NB];
 #pragma unroll
         for (int q = 0; q < NB; ++q) {
             const GatherRec &R = rec[e0 + q][col];
-            const int2 zr = *reinterpret_cast<const int2 *>(&R.zlo0);
-            w[q] = *reinterpret_cast<const float4 *>(R.w);
+            const int2 zr = *reinterpret_cast<const int2 *>(&R.q[3 ^ sw]);
+            w[q] = *reinterpret_cast<const float4 *>(&R.q[2 ^ sw]);
             const int zlo0 = (short)(zr.x & 0xffff), zhi0 = zr.x >> 16, zlo1 = (short)(zr.y & 0xffff), zhi1 = zr.y >> 16;
-            const float *r0 = R.row[0], *r1 = R.row[1], *r2 = R.row[2], *r3 = R.row[3];
+            const ulonglong2 ra = R.q[sw], rb = R.q[1 ^ sw];
+            const float *r0 = reinterpret_cast<const float *>(ra.x), *r1 = reinterpret_cast<const float *>(ra.y);
+            const float *r2 = reinterpret_cast<const float *>(rb.x), *r3 = reinterpret_cast<const float *>(rb.y);
 #pragma unroll
             for (int ps = 0; ps < NP; ++ps) {
                 const int z = zq + ps * GD_ZSPAN;
@@ -141,24 +148,28 @@ k_gather_dose(Params P, const CpDesc *__restrict__ desc, const SliceBox16 *__res
             v00 = s.i0 >= s.w0.u0 && s.i0 <= s.w0.u1; v10 = s.i0 + 1 >= s.w0.u0 && s.i0 + 1 <= s.w0.u1;
             v01 = s.i0 >= s.w1.u0 && s.i0 <= s.w1.u1; v11 = s.i0 + 1 >= s.w1.u0 && s.i0 + 1 <= s.w1.u1;
         }
+        const float *row[4] = { D, D, D, D };
+        float4 wv = make_float4(0.f, 0.f, 0.f, 0.f);
+        short zlo0 = 0, zhi0 = 0, zlo1 = 0, zhi1 = 0;
         if (v00 || v10 || v01 || v11) {
             const GatherCp g = list[q];
             const int rs = g.pv, ks = g.pu * g.pv;
             const int o00 = (s.k0 * g.pu + (s.i0 - g.ri0)) * rs;
             const int any_off = v00 ? o00 : (v10 ? o00 + rs : (v01 ? o00 + ks : o00 + ks + rs));
             const float *base = D + (size_t)g.slot * (size_t)P.stride_cp - g.rj0;
-            R.row[0] = base + (v00 ? o00 : any_off); R.row[1] = base + (v10 ? o00 + rs : any_off);
-            R.row[2] = base + (v01 ? o00 + ks : any_off); R.row[3] = base + (v11 ? o00 + ks + rs : any_off);
-            R.w[0] = v00 ? g.scale * ((1.f - s.tu) * (1.f - s.tw)) : 0.f; R.w[1] = v10 ? g.scale * (s.tu * (1.f - s.tw)) : 0.f;
-            R.w[2] = v01 ? g.scale * ((1.f - s.tu) * s.tw) : 0.f; R.w[3] = v11 ? g.scale * (s.tu * s.tw) : 0.f;
+            row[0] = base + (v00 ? o00 : any_off); row[1] = base + (v10 ? o00 + rs : any_off);
+            row[2] = base + (v01 ? o00 + ks : any_off); row[3] = base + (v11 ? o00 + ks + rs : any_off);
+            wv.x = v00 ? g.scale * ((1.f - s.tu) * (1.f - s.tw)) : 0.f; wv.y = v10 ? g.scale * (s.tu * (1.f - s.tw)) : 0.f;
+            wv.z = v01 ? g.scale * ((1.f - s.tu) * s.tw) : 0.f; wv.w = v11 ? g.scale * (s.tu * s.tw) : 0.f;
             // a slice none of whose rows is valid gets an empty z-range: its (folded) rows are not read at all
-            R.zlo0 = (v00 || v10) ? s.w0.v0 : (short)0; R.zhi0 = (v00 || v10) ? (short)(s.w0.v1 + 1) : (short)0;
-            R.zlo1 = (v01 || v11) ? s.w1.v0 : (short)0; R.zhi1 = (v01 || v11) ? (short)(s.w1.v1 + 1) : (short)0;
-        } else {
-            R.row[0] = R.row[1] = R.row[2] = R.row[3] = D;
-            R.w[0] = R.w[1] = R.w[2] = R.w[3] = 0.f;
-            R.zlo0 = R.zhi0 = R.zlo1 = R.zhi1 = 0;
+            if (v00 || v10) { zlo0 = s.w0.v0; zhi0 = (short)(s.w0.v1 + 1); }
+            if (v01 || v11) { zlo1 = s.w1.v0; zhi1 = (short)(s.w1.v1 + 1); }
         }
+        const int sw = gather_swz(a_col);
+        R.q[sw] = make_ulonglong2((unsigned long long)row[0], (unsigned long long)row[1]);
+        R.q[1 ^ sw] = make_ulonglong2((unsigned long long)row[2], (unsigned long long)row[3]);
+        *reinterpret_cast<float4 *>(&R.q[2 ^ sw]) = wv;
+        *reinterpret_cast<int4 *>(&R.q[3 ^ sw]) = make_int4((int)(unsigned short)zlo0 | ((int)zhi0 << 16), (int)(unsigned short)zlo1 | ((int)zhi1 << 16), 0, 0);
     };
 
     for (int c0 = 0; c0 < n_cp; c0 += GD_LIST) {

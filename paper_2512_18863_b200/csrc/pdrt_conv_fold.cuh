@@ -124,9 +124,11 @@ __device__ __forceinline__ void fold_step(const float2 (&zc)[FRF], const float2 
 }
 
 template <int KT, bool ADJ>
-__global__ void __maxnreg__(KT <= 21 ? 160 : KT <= 25 ? 168 : 255)      // 129 .. 168 registers leave 3 warps per scheduler; measured at 21 taps (cap 128 / 136 /
-                                                                        // 144 / 152 / 160 / 168: forward 0.847 / 0.767 / 0.724 / 0.712 / 0.696 / 0.720 ms) and at 25
-                                                                        // (144 / 152 / 160 / 168: 1.035 / 0.951 / 0.928 / 0.915 ms): below 152 the step loop spills
+__global__ void __maxnreg__(KT <= 21 ? 160 : KT <= 25 ? 168 : (KT >= 41 && KT <= 51 && !ADJ) ? 168 : 255)
+// 129 .. 168 registers leave 3 warps per scheduler.  Measured at 21 taps (cap 128 / 136 / 144 / 152 / 160 / 168: forward 0.847 / 0.767 / 0.724 /
+// 0.712 / 0.696 / 0.720 ms) and at 25 (144 / 152 / 160 / 168: 1.035 / 0.951 / 0.928 / 0.915 ms): below 152 the step loop spills.  2-column units
+// (41 taps and up) with 168 instead of 255: forward 41 / 51 taps 4.19 -> 3.90 / 6.09 -> 5.83 ms per c4 arc, adjoint slower; from 55 taps shared
+// memory allows 8 blocks per SM either way.
 k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
             const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
             int *item_counter, WorkCounters *wc, int in_floats, int out_floats)

@@ -14,6 +14,9 @@
 namespace pdrt {
 
 constexpr int FOLD_COLS_MAX = 8 * SYM_NTFC_MAX;     // widest work item [columns]
+// from 55 taps the work items are at most 48 columns wide: the ring of 2 C + 2 maxp output rows is what fills the shared memory there
+// (measured on c4, forward / backward of the whole call: 63 taps 9.58 / 7.91 -> 9.00 / 7.18 ms, 75 taps 14.5 / 11.4 -> 12.9 / 9.8 ms)
+__host__ __device__ constexpr int fold_cols_max(int kt) { return kt >= 55 ? 48 : FOLD_COLS_MAX; }
 // output columns per unit: 4 up to 31 taps, 2 above (the folded window takes 2 W (C + 2) registers)
 __host__ __device__ constexpr int fold_unit_cols(int kt) { return kt <= 31 ? 4 : 2; }
 
@@ -34,14 +37,14 @@ inline int fold_out_floats(int kt)
 {
     const int c = (kt - 1) / 2, w = fold_unit_cols(kt);
     int best = 0;
-    for (int n = 1; n <= FOLD_COLS_MAX / w; ++n) best = std::max(best, (2 * fold_max_pairs(n) + 2 * c) * fold_out_pitch(n, w));
+    for (int n = 1; n <= fold_cols_max(kt) / w; ++n) best = std::max(best, (2 * fold_max_pairs(n) + 2 * c) * fold_out_pitch(n, w));
     return best;
 }
 inline int fold_in_floats(int kt)
 {
     const int c = (kt - 1) / 2, w = fold_unit_cols(kt);
     int best = 0;
-    for (int n = 1; n <= FOLD_COLS_MAX / w; ++n) best = std::max(best, fold_max_pairs(n) * fold_in_chunks(n, w, c) * 4);
+    for (int n = 1; n <= fold_cols_max(kt) / w; ++n) best = std::max(best, fold_max_pairs(n) * fold_in_chunks(n, w, c) * 4);
     return best;
 }
 __host__ __device__ constexpr int fold_wpitch(int kt) { return ((kt - 1) / 2 + 1 + 3) & ~3; }         // floats per weight row: W_d[C .. 2C], padded to 4
@@ -124,11 +127,11 @@ __device__ __forceinline__ void fold_step(const float2 (&zc)[FRF], const float2 
 }
 
 template <int KT, bool ADJ>
-__global__ void __maxnreg__(KT <= 21 ? 160 : KT <= 25 ? 168 : (KT >= 41 && KT <= 51 && !ADJ) ? 168 : 255)
+__global__ void __maxnreg__(KT <= 21 ? 160 : KT <= 25 ? 168 : (KT >= 41 && KT <= 55 && !ADJ) ? 168 : 255)
 // 129 .. 168 registers leave 3 warps per scheduler.  Measured at 21 taps (cap 128 / 136 / 144 / 152 / 160 / 168: forward 0.847 / 0.767 / 0.724 /
 // 0.712 / 0.696 / 0.720 ms) and at 25 (144 / 152 / 160 / 168: 1.035 / 0.951 / 0.928 / 0.915 ms): below 152 the step loop spills.  2-column units
-// (41 taps and up) with 168 instead of 255: forward 41 / 51 taps 4.19 -> 3.90 / 6.09 -> 5.83 ms per c4 arc, adjoint slower; from 55 taps shared
-// memory allows 8 blocks per SM either way.
+// (41 taps and up) with 168 instead of 255: forward 41 / 51 / 55 taps 4.19 -> 3.90 / 6.09 -> 5.83 / 7.00 -> 6.56 ms per c4 arc (55 with the
+// 48-column work items), adjoint slower; 63 and 75 taps spill heavily under 168.
 k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const int *__restrict__ tile_base,
             const float *__restrict__ zrad, const float *__restrict__ wtab, const float *__restrict__ in, float *__restrict__ out,
             int *item_counter, WorkCounters *wc, int in_floats, int out_floats)
@@ -139,7 +142,7 @@ k_conv_fold(Params P, const CpDesc *__restrict__ desc, int cp0, int n_cp, const 
     constexpr int WP = fold_wpitch(KT), WQ = WP / 4;  // weight row W_d[C .. 2C] in shared memory [floats], LDS.128 per row
     constexpr int XW = KT + FRF - 1;                  // window along v [columns]: 2C + FRF, even
     constexpr int NXQ = XW / 2;                       // LDS.128 per window (2 columns x 2 rows each)
-    constexpr int MCX = (FOLD_COLS_MAX + 2 * C + 31) / 32;       // staged columns per lane and row
+    constexpr int MCX = (fold_cols_max(KT) + 2 * C + 31) / 32;       // staged columns per lane and row
     extern __shared__ float4 smem4[];
     float4 *Wd = smem4;                               // [C+1 (d)][WQ]: kernel row C+d, columns C .. 2C, zero past them
     float4 *xin4 = smem4 + (C + 1) * WQ;              // [pair][chunk]: (x[r][c], x[r+1][c], x[r][c+1], x[r+1][c+1]), chunks swizzled

@@ -239,7 +239,7 @@ int gaussian_taps(double sigma, double D, std::vector<float> &g)
 void set_conv_direction(pdrt_engine *e, bool adjoint)
 {
     e->P.conv_sym = (adjoint ? e->sym_adj : e->sym_fwd) ? (e->P.KT >= 15 && e->P.KT <= conv_fold_max() ? 2 : 1) : 0;   // measured: the fold pays from 15 taps
-    e->P.ntfc_max = e->P.conv_sym ? SYM_NTFC_MAX : NTFC_MAX;
+    e->P.ntfc_max = e->P.conv_sym == 2 ? fold_cols_max(e->P.KT) / 8 : e->P.conv_sym ? SYM_NTFC_MAX : NTFC_MAX;
 }
 
 int build_kernel_table(pdrt_engine *e, int k)
